@@ -1,0 +1,752 @@
+/*
+ * dtn_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU restatement (C99, double precision, brute
+ * force geometry) of the hot path of "Monte Carlo Steklov Operators for
+ * Large-Scale Geometry Processing in the Wild" (arxiv 2606.05581, PAPER.md):
+ * the walk-on-spheres estimator of the discrete Dirichlet-to-Neumann matrix,
+ * interior (Alg. 2, Eq. 26) and exterior (Eq. 32,
+ * PAPER.md:348-353, App. C.3-C.7).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load this.  It shares no code, header, table or
+ * helper with paper_2606_05581_b200/csrc.  Every function cites the passage of
+ * PAPER.md it follows; where the paper is silent the reading is the one listed
+ * in DESIGN.md ("Readings") and named here as [Rn].
+ *
+ * Pins (tests/test_oracle_*.py, all run without a GPU):
+ *   philox4x32_10        cuRAND host generator + Random123 known answers
+ *   closest point        second formulation + invariants + brute force
+ *   tangent ball         closed forms (sphere, cube face)
+ *   WoS                  martingale E[t] = z, Poisson kernel of the ball (Eq. 22)
+ *   interior weights     analytic unit ball: S -> diag(l) minus the cap term
+ *   exterior weights     analytic sphere, centred and off-centre: l, l+1, capacity
+ *   mesh estimators      symmetry, PSD, zero row sums, multiplicities 1,3,5,7
+ * Parity unpinned: nothing in this file.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_PI 3.14159265358979323846
+
+/* ------------------------------------------------------------------------- */
+/* Counter-based RNG: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).      */
+/* The paper does not describe its RNG; BASELINE.json north_star fixes        */
+/* "Philox keyed by (seed, sample, walk, step)"  [R18].                        */
+/* key = (seed_lo, seed_hi); counter = (sample, walk, step, purpose).         */
+/* ------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;          /* golden-ratio Weyl increments */
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* uint32 -> uniform in (0,1): ((x >> 9) + 1/2) * 2^-23, exact in fp32 and fp64 [R18]. */
+double orc_u01(uint32_t x)
+{
+    return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0);
+}
+
+enum { ORC_PURPOSE_INIT = 1, ORC_PURPOSE_STEP = 2 };
+#define ORC_KILLING_SAMPLE 0xFFFFFFFFu
+
+static void orc_uniform2(uint64_t seed, uint32_t sample, uint32_t walk, uint32_t step,
+                         uint32_t purpose, double *u1, double *u2)
+{
+    uint32_t ctr[4] = { sample, walk, step, purpose };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t w[4];
+    orc_philox4x32_10(ctr, key, w);
+    *u1 = orc_u01(w[0]);
+    *u2 = orc_u01(w[1]);
+}
+
+/* ------------------------------------------------------------------------- */
+/* small vector helpers                                                       */
+/* ------------------------------------------------------------------------- */
+static double dot3(const double a[3], const double b[3]) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+static void sub3(const double a[3], const double b[3], double o[3]) { o[0]=a[0]-b[0]; o[1]=a[1]-b[1]; o[2]=a[2]-b[2]; }
+static void cross3(const double a[3], const double b[3], double o[3])
+{
+    o[0] = a[1]*b[2] - a[2]*b[1];
+    o[1] = a[2]*b[0] - a[0]*b[2];
+    o[2] = a[0]*b[1] - a[1]*b[0];
+}
+static double norm3(const double a[3]) { return sqrt(dot3(a, a)); }
+
+/* ------------------------------------------------------------------------- */
+/* Closest point on a segment / triangle (the geometric query under WoS,      */
+/* PAPER.md:155 "the nearest boundary point").                  */
+/* ------------------------------------------------------------------------- */
+static double closest_on_segment(const double p[3], const double a[3], const double b[3],
+                                 double cp[3], double *t_out)
+{
+    double ab[3], ap[3];
+    sub3(b, a, ab); sub3(p, a, ap);
+    double den = dot3(ab, ab);
+    double t = den > 0.0 ? dot3(ap, ab) / den : 0.0;
+    if (t < 0.0) t = 0.0;
+    if (t > 1.0) t = 1.0;
+    for (int k = 0; k < 3; ++k) cp[k] = a[k] + t * ab[k];
+    double d[3]; sub3(p, cp, d);
+    *t_out = t;
+    return dot3(d, d);
+}
+
+/* Closest point over the three edges; used for degenerate triangles [R16]. */
+static double closest_on_edges(const double p[3], const double a[3], const double b[3],
+                               const double c[3], double cp[3], double bary[3])
+{
+    double best = INFINITY, q[3], t;
+    double d2 = closest_on_segment(p, a, b, q, &t);
+    if (d2 < best) { best = d2; memcpy(cp, q, sizeof q); bary[0] = 1.0 - t; bary[1] = t; bary[2] = 0.0; }
+    d2 = closest_on_segment(p, b, c, q, &t);
+    if (d2 < best) { best = d2; memcpy(cp, q, sizeof q); bary[0] = 0.0; bary[1] = 1.0 - t; bary[2] = t; }
+    d2 = closest_on_segment(p, c, a, q, &t);
+    if (d2 < best) { best = d2; memcpy(cp, q, sizeof q); bary[0] = t; bary[1] = 0.0; bary[2] = 1.0 - t; }
+    return best;
+}
+
+/*
+ * Voronoi-region method (Ericson, Real-Time Collision Detection, sec. 5.1.5,
+ * restated): classify p against the vertex, edge and face regions of triangle
+ * abc; returns the squared distance, the closest point and its barycentric
+ * coordinates (weights of a, b, c).
+ */
+double orc_closest_point_triangle(const double p[3], const double a[3], const double b[3],
+                                  const double c[3], double cp[3], double bary[3])
+{
+    double ab[3], ac[3], ap[3], bp[3], cpv[3], nrm[3];
+    sub3(b, a, ab); sub3(c, a, ac);
+    cross3(ab, ac, nrm);
+    double e2 = fmax(dot3(ab, ab), dot3(ac, ac));
+    if (dot3(nrm, nrm) <= 1e-24 * e2 * e2)                /* zero-area face [R16] */
+        return closest_on_edges(p, a, b, c, cp, bary);
+
+    sub3(p, a, ap);
+    double d1 = dot3(ab, ap), d2 = dot3(ac, ap);
+    double v, w;
+    if (d1 <= 0.0 && d2 <= 0.0) { v = 0.0; w = 0.0; goto done; }            /* vertex a */
+    sub3(p, b, bp);
+    double d3 = dot3(ab, bp), d4 = dot3(ac, bp);
+    if (d3 >= 0.0 && d4 <= d3) { v = 1.0; w = 0.0; goto done; }              /* vertex b */
+    double vc = d1 * d4 - d3 * d2;
+    if (vc <= 0.0 && d1 >= 0.0 && d3 <= 0.0) { v = d1 / (d1 - d3); w = 0.0; goto done; }   /* edge ab */
+    sub3(p, c, cpv);
+    double d5 = dot3(ab, cpv), d6 = dot3(ac, cpv);
+    if (d6 >= 0.0 && d5 <= d6) { v = 0.0; w = 1.0; goto done; }              /* vertex c */
+    double vb = d5 * d2 - d1 * d6;
+    if (vb <= 0.0 && d2 >= 0.0 && d6 <= 0.0) { v = 0.0; w = d2 / (d2 - d6); goto done; }   /* edge ac */
+    double va = d3 * d6 - d5 * d4;
+    if (va <= 0.0 && (d4 - d3) >= 0.0 && (d5 - d6) >= 0.0) {                               /* edge bc */
+        w = (d4 - d3) / ((d4 - d3) + (d5 - d6)); v = 1.0 - w; goto done;
+    }
+    {                                                                                      /* face */
+        double denom = 1.0 / (va + vb + vc);
+        v = vb * denom; w = vc * denom;
+    }
+done:
+    bary[0] = 1.0 - v - w; bary[1] = v; bary[2] = w;
+    for (int k = 0; k < 3; ++k) cp[k] = a[k] + v * ab[k] + w * ac[k];
+    double d[3]; sub3(p, cp, d);
+    return dot3(d, d);
+}
+
+/*
+ * Second, independent formulation used only to pin the first one
+ * (tests/test_oracle_geometry.py): project p on the plane; if the projection
+ * is inside the triangle that is the answer, otherwise the nearest point of
+ * the three edges.
+ */
+double orc_closest_point_triangle_alt(const double p[3], const double a[3], const double b[3],
+                                      const double c[3], double cp[3])
+{
+    double ab[3], ac[3], ap[3], n[3], bary[3];
+    sub3(b, a, ab); sub3(c, a, ac); sub3(p, a, ap);
+    cross3(ab, ac, n);
+    double nn = dot3(n, n);
+    if (nn > 0.0) {
+        double h = dot3(ap, n) / nn;
+        double q[3] = { p[0] - h * n[0], p[1] - h * n[1], p[2] - h * n[2] };
+        /* inside test by signed sub-areas */
+        double qa[3], qb[3], qc[3], c0[3], c1[3], c2[3];
+        sub3(a, q, qa); sub3(b, q, qb); sub3(c, q, qc);
+        cross3(qb, qc, c0); cross3(qc, qa, c1); cross3(qa, qb, c2);
+        if (dot3(c0, n) >= 0.0 && dot3(c1, n) >= 0.0 && dot3(c2, n) >= 0.0) {
+            memcpy(cp, q, sizeof q);
+            double d[3]; sub3(p, q, d);
+            return dot3(d, d);
+        }
+    }
+    return closest_on_edges(p, a, b, c, cp, bary);
+}
+
+/* ------------------------------------------------------------------------- */
+/* Geometry: a triangle soup (brute force over all faces) or, for the         */
+/* closed-form pins only, an analytic sphere.                                 */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    int32_t kind;               /* 0 = triangle mesh, 1 = analytic sphere (pins) */
+    int32_t pad_;
+    const float *verts;         /* [V][3] fp32, as given to the CUDA path        */
+    int64_t V;
+    const int32_t *faces;       /* [F][3]                                         */
+    int64_t F;
+    double centre[3];           /* kind 1                                         */
+    double radius;
+} orc_geom;
+
+typedef struct {
+    double dist;                /* unsigned distance to the surface */
+    double cp[3];               /* closest point                    */
+    double bary[3];             /* barycentrics of cp in face `tri` */
+    int64_t tri;                /* closest face, -1 for the sphere  */
+} orc_hit;
+
+static void load_vertex(const orc_geom *g, int64_t vi, double o[3])
+{
+    o[0] = (double)g->verts[3*vi]; o[1] = (double)g->verts[3*vi+1]; o[2] = (double)g->verts[3*vi+2];
+}
+
+/* Brute force over ALL faces: the definition of the query.  Ties: the smaller
+ * squared distance wins, on equality the smaller face index [R15] (strict <
+ * while scanning in increasing index order). */
+void orc_closest_point(const orc_geom *g, const double x[3], orc_hit *h)
+{
+    if (g->kind == 1) {
+        double d[3]; sub3(x, g->centre, d);
+        double rho = norm3(d);
+        h->dist = fabs(g->radius - rho);
+        if (rho > 0.0) for (int k = 0; k < 3; ++k) h->cp[k] = g->centre[k] + g->radius * d[k] / rho;
+        else { h->cp[0] = g->centre[0] + g->radius; h->cp[1] = g->centre[1]; h->cp[2] = g->centre[2]; }
+        h->bary[0] = 1.0; h->bary[1] = 0.0; h->bary[2] = 0.0;
+        h->tri = -1;
+        return;
+    }
+    double best = INFINITY;
+    h->tri = -1;
+    for (int64_t f = 0; f < g->F; ++f) {
+        double a[3], b[3], c[3], cp[3], bary[3];
+        load_vertex(g, g->faces[3*f], a); load_vertex(g, g->faces[3*f+1], b); load_vertex(g, g->faces[3*f+2], c);
+        double d2 = orc_closest_point_triangle(x, a, b, c, cp, bary);
+        if (d2 < best) {
+            best = d2; h->tri = f;
+            memcpy(h->cp, cp, sizeof cp); memcpy(h->bary, bary, sizeof bary);
+        }
+    }
+    h->dist = sqrt(best);
+}
+
+/* Batch form for the parity tests: queries in fp32 (same numbers the GPU gets).
+ * second[q] = smallest distance over faces that share no vertex with the winner
+ * (for the tie filter of SURVEY.md 8(c)); may be NULL. */
+void orc_closest_points(const orc_geom *g, const float *q, int64_t Q,
+                        double *dist, int64_t *tri, double *cp, double *bary, double *second)
+{
+    #pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < Q; ++i) {
+        double x[3] = { q[3*i], q[3*i+1], q[3*i+2] };
+        orc_hit h;
+        orc_closest_point(g, x, &h);
+        dist[i] = h.dist; tri[i] = h.tri;
+        if (cp)   memcpy(cp + 3*i, h.cp, sizeof h.cp);
+        if (bary) memcpy(bary + 3*i, h.bary, sizeof h.bary);
+        if (second && g->kind == 0) {
+            const int32_t *wf = g->faces + 3*h.tri;
+            double best = INFINITY;
+            for (int64_t f = 0; f < g->F; ++f) {
+                const int32_t *ff = g->faces + 3*f;
+                int share = 0;
+                for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) share |= (ff[a] == wf[b]);
+                if (share) continue;
+                double a3[3], b3[3], c3[3], p3[3], bb[3];
+                load_vertex(g, ff[0], a3); load_vertex(g, ff[1], b3); load_vertex(g, ff[2], c3);
+                double d2 = orc_closest_point_triangle(x, a3, b3, c3, p3, bb);
+                if (d2 < best) best = d2;
+            }
+            second[i] = sqrt(best);
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------- */
+/* Mesh quantities: face normal, area, AABB, r_max.            */
+/* ------------------------------------------------------------------------- */
+static void face_normal_area(const orc_geom *g, int64_t f, double n[3], double *area)
+{
+    double a[3], b[3], c[3], ab[3], ac[3];
+    load_vertex(g, g->faces[3*f], a); load_vertex(g, g->faces[3*f+1], b); load_vertex(g, g->faces[3*f+2], c);
+    sub3(b, a, ab); sub3(c, a, ac);
+    cross3(ab, ac, n);
+    double l = norm3(n);
+    *area = 0.5 * l;
+    if (l > 0.0) { n[0] /= l; n[1] /= l; n[2] /= l; }
+}
+
+/* r_max = half of the shortest AABB side ("maximum diameter ... shortest side
+ * length of the mesh's axis-aligned bounding box").  For the
+ * exterior the box is that of the Kelvin-inverted vertices kappa(v - origin). */
+double orc_rmax(const orc_geom *g, int exterior, const double origin[3])
+{
+    double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    for (int64_t i = 0; i < g->V; ++i) {
+        double v[3]; load_vertex(g, i, v);
+        if (exterior) {
+            double w[3]; sub3(v, origin, w);
+            double s = dot3(w, w);
+            for (int k = 0; k < 3; ++k) v[k] = w[k] / s;          /* kappa(x) = x/|x|^2 */
+        }
+        for (int k = 0; k < 3; ++k) { lo[k] = fmin(lo[k], v[k]); hi[k] = fmax(hi[k], v[k]); }
+    }
+    double side = fmin(hi[0] - lo[0], fmin(hi[1] - lo[1], hi[2] - lo[2]));
+    return (double)(float)(0.5 * side);       /* rounded to fp32: the value both sides bisect on [R4] */
+}
+
+/* R_max = largest vertex distance from the Kelvin origin (used by E3). */
+double orc_max_vertex_norm(const orc_geom *g, const double origin[3])
+{
+    double m = 0.0;
+    for (int64_t i = 0; i < g->V; ++i) {
+        double v[3], w[3]; load_vertex(g, i, v); sub3(v, origin, w);
+        m = fmax(m, norm3(w));
+    }
+    return (double)(float)m;
+}
+
+double orc_total_area(const orc_geom *g)
+{
+    double tot = 0.0, n[3], a;
+    for (int64_t f = 0; f < g->F; ++f) { face_normal_area(g, f, n, &a); tot += a; }
+    return tot;
+}
+
+/* Consistent P1 mass matrix M_pq = sum_T area_T (1 + delta_pq) / 12  [R14]. */
+void orc_mass_matrix_p1(const orc_geom *g, double *M /* [V][V], zeroed by caller */)
+{
+    for (int64_t f = 0; f < g->F; ++f) {
+        double n[3], a; face_normal_area(g, f, n, &a);
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j)
+            M[(int64_t)g->faces[3*f+i] * g->V + g->faces[3*f+j]] += a * (i == j ? 2.0 : 1.0) / 12.0;
+    }
+}
+
+/* ------------------------------------------------------------------------- */
+/* Parameters and per-sample state                                            */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    uint64_t seed;
+    int32_t walks_per_sample;       /* W                                               */
+    int32_t max_steps;              /* [R10] truncated walks contribute nothing         */
+    double eps;                     /* WoS shell, absolute [R8]     */
+    double cap_half_angle_deg;      /* theta_0 ("~2.5 deg") [R5]           */
+    double rmax;                    /* from orc_rmax() times the caller's scale         */
+    int32_t bisection_iters;        /* 10                                */
+    int32_t importance_sample;      /* 1: z ~ J^B; 0: z uniform          */
+    int32_t antithetic;             /* [R7]                                             */
+    int32_t include_killing;        /* exterior: second expectation of Eq. 32           */
+    int64_t n_kill_walks;
+    double origin[3];               /* Kelvin origin [R12]               */
+    double Rmax_norm;               /* orc_max_vertex_norm(), exterior only             */
+} orc_params;
+
+typedef struct {                    /* one boundary sample            */
+    double s[3];                    /* surface point                                    */
+    double n[3];                    /* unit normal pointing out of the solid            */
+    double a;                       /* quadrature weight, sum = |dOmega|                */
+    int64_t tri;                    /* its face (-1 for the analytic sphere)            */
+    double bary[3];
+} orc_sample;
+
+typedef struct {                    /* tangent ball in the walk domain                  */
+    double c[3];                    /* centre (interior: primal; exterior: Kelvin coords about origin) */
+    double pole[3];                 /* unit vector from c to the tangent point          */
+    double r;                       /* 0 => sample discarded             */
+    double sstar_norm;              /* |s*| (exterior), 1 otherwise                     */
+} orc_ball;
+
+/* ------------------------------------------------------------------------- */
+/* LargestTangentBall ("bisection algorithm of Yu et al. with   */
+/* 10 iterations"; clamp PAPER.md:642)  [R4].                   */
+/* The ball of radius r about c = s - r n is accepted when no surface point is */
+/* closer to c than r - eps/2.                                                */
+/* ------------------------------------------------------------------------- */
+void orc_tangent_ball_interior(const orc_geom *g, const orc_params *P, const orc_sample *S, orc_ball *B)
+{
+    double lo = 0.0, hi = P->rmax;
+    for (int it = 0; it < P->bisection_iters; ++it) {
+        double r = 0.5 * (lo + hi);
+        double c[3] = { S->s[0] - r * S->n[0], S->s[1] - r * S->n[1], S->s[2] - r * S->n[2] };
+        orc_hit h;
+        orc_closest_point(g, c, &h);
+        if (h.dist >= r - 0.5 * P->eps) lo = r; else hi = r;
+    }
+    B->r = lo;
+    for (int k = 0; k < 3; ++k) { B->c[k] = S->s[k] - lo * S->n[k]; B->pole[k] = S->n[k]; }
+    B->sstar_norm = 1.0;
+}
+
+/*
+ * Exterior: the tangent ball lives in the inverted domain Omega*_ext
+ * (PAPER.md:348-353).  s* = kappa(s - o); the unit normal at s* pointing out of
+ * Omega*_ext is n* = -H_shat n (Eq. 54).  The ball B_r(c*),
+ * c* = s* - r n*, is tested through its primal image, which is again a ball as
+ * long as 0 is outside it: centre c* / (|c*|^2 - r^2), radius r / (|c*|^2 - r^2)
+ * [DESIGN.md reading E2].  r is limited so that 0 stays outside
+ * (r < |s*|^2 / (2 s*.n*)) and by r_max of the inverted box.
+ */
+void orc_tangent_ball_exterior(const orc_geom *g, const orc_params *P, const orc_sample *S, orc_ball *B)
+{
+    double st[3]; sub3(S->s, P->origin, st);
+    double sig = dot3(st, st);
+    B->r = 0.0; B->sstar_norm = 0.0;
+    memset(B->c, 0, sizeof B->c); memset(B->pole, 0, sizeof B->pole);
+    if (!(sig > 0.0)) return;
+    double sstar[3] = { st[0] / sig, st[1] / sig, st[2] / sig };
+    double sn = dot3(st, S->n) / sig;                       /* shat (shat . n) = st * sn */
+    double nstar[3];
+    for (int k = 0; k < 3; ++k) nstar[k] = -(S->n[k] - 2.0 * st[k] * sn);   /* -(n - 2 shat (shat.n)), Eq. 54 */
+    double ss2 = dot3(sstar, sstar);
+    double sdn = dot3(sstar, nstar);
+    double hi = P->rmax;
+    if (sdn > 0.0) hi = fmin(hi, 0.45 * ss2 / sdn);
+    double lo = 0.0;
+    for (int it = 0; it < P->bisection_iters; ++it) {
+        double r = 0.5 * (lo + hi);
+        double cs[3] = { sstar[0] - r * nstar[0], sstar[1] - r * nstar[1], sstar[2] - r * nstar[2] };
+        double den = dot3(cs, cs) - r * r;
+        double cprime[3] = { P->origin[0] + cs[0] / den, P->origin[1] + cs[1] / den, P->origin[2] + cs[2] / den };
+        double rprime = r / den;
+        orc_hit h;
+        orc_closest_point(g, cprime, &h);
+        if (h.dist >= rprime * (1.0 - 0.5 * P->eps / r)) lo = r; else hi = r;
+    }
+    B->r = lo;
+    for (int k = 0; k < 3; ++k) { B->c[k] = sstar[k] - lo * nstar[k]; B->pole[k] = nstar[k]; }
+    B->sstar_norm = sqrt(ss2);
+}
+
+/* Orthonormal frame (e1, e2, n) from a unit vector n: the branchless
+ * construction of Duff et al., "Building an Orthonormal Basis, Revisited"
+ * (JCGT 2017), restated.  Both sides use the same rule so that a walk's start
+ * point is the same point  [DESIGN.md reading R6b]. */
+static void frame_from_normal(const double n[3], double e1[3], double e2[3])
+{
+    double sign = copysign(1.0, n[2]);
+    double a = -1.0 / (sign + n[2]);
+    double b = n[0] * n[1] * a;
+    e1[0] = 1.0 + sign * n[0] * n[0] * a; e1[1] = sign * b; e1[2] = -sign * n[0];
+    e2[0] = b; e2[1] = sign + n[1] * n[1] * a; e2[2] = -n[1];
+}
+
+/*
+ * SampleBallSurface + BallJumpKernel (Eq. 23).
+ * Polar angle theta from the pole (the tangent point), q = sin(theta/2), so
+ * |s - z| = 2 r q.  The cap theta < theta_0 is excluded [R5].
+ *   importance: density on the sphere proportional to J^B = 1/(2 pi |s-z|^3)
+ *     => pdf(q) ~ q^-2 on [q0, 1], q = 1 / (1/q0 - u1 (1/q0 - 1)); the
+ *     per-walk factor  (|dB|/2) J / pdf  is the constant (1/(4r)) (1/q0 - 1) [R6]
+ *   uniform: cos(theta) = 1 - 2 u1; factor (4 pi r^2 / 2) J = 1 / (8 r q^3),
+ *     zero inside the cap.
+ * Returns the factor; z is written in the coordinates of the ball.
+ */
+static double sample_ball_surface(const orc_params *P, const orc_ball *B, uint32_t sample, uint32_t walk, double z[3])
+{
+    double q0 = sin(0.5 * P->cap_half_angle_deg * ORC_PI / 180.0);
+    uint32_t wq = P->antithetic ? (walk >> 1) : walk;
+    double u1, u2;
+    orc_uniform2(P->seed, sample, wq, 0u, ORC_PURPOSE_INIT, &u1, &u2);
+    double q, factor;
+    if (P->importance_sample) {
+        q = 1.0 / (1.0 / q0 - u1 * (1.0 / q0 - 1.0));
+        factor = (1.0 / (4.0 * B->r)) * (1.0 / q0 - 1.0);
+    } else {
+        q = sqrt(u1);
+        factor = (q < q0) ? 0.0 : 1.0 / (8.0 * B->r * q * q * q);
+    }
+    double ct = 1.0 - 2.0 * q * q;
+    double st = 2.0 * q * sqrt(fmax(0.0, 1.0 - q * q));
+    double phi = 2.0 * ORC_PI * u2;
+    if (P->antithetic && (walk & 1u)) phi += ORC_PI;          /* antithetic partner [R7] */
+    double e1[3], e2[3];
+    frame_from_normal(B->pole, e1, e2);
+    double cphi = cos(phi), sphi = sin(phi);
+    for (int k = 0; k < 3; ++k)
+        z[k] = B->c[k] + B->r * (ct * B->pole[k] + st * (cphi * e1[k] + sphi * e2[k]));
+    return factor;
+}
+
+/* Uniform direction on S^2 from two uniforms [R19]. */
+static void step_direction(uint64_t seed, uint32_t sample, uint32_t walk, uint32_t step, double w[3])
+{
+    double u1, u2;
+    orc_uniform2(seed, sample, walk, step, ORC_PURPOSE_STEP, &u1, &u2);
+    double ct = 1.0 - 2.0 * u1;
+    double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+    double phi = 2.0 * ORC_PI * u2;
+    w[0] = st * cos(phi); w[1] = st * sin(phi); w[2] = ct;
+}
+
+/*
+ * WalkOnSpheres in the primal domain  [R9]:
+ * repeat { closest point; stop if D < eps; jump to a uniform point of the
+ * sphere of radius D }.  Returns the number of jumps, or -1 if max_steps
+ * jumps did not reach the shell [R10].
+ */
+static int walk_on_spheres(const orc_geom *g, const orc_params *P, uint32_t sample, uint32_t walk,
+                           const double z[3], orc_hit *h)
+{
+    double x[3] = { z[0], z[1], z[2] };
+    for (int k = 0; ; ++k) {
+        orc_closest_point(g, x, h);
+        if (h->dist < P->eps) return k;
+        if (k == P->max_steps) return -1;
+        double w[3];
+        step_direction(P->seed, sample, walk, (uint32_t)(k + 1), w);
+        for (int j = 0; j < 3; ++j) x[j] += h->dist * w[j];
+    }
+}
+
+/*
+ * WalkOnSpheres in the inverted domain Omega*_ext, carried in Kelvin
+ * coordinates y about the origin  [DESIGN.md reading E3].
+ * A ball about y inside Omega*_ext is found from flat-triangle queries on the
+ * PRIMAL mesh:  x = kappa(y), rho = |x|, D = dist(x), and every point p of the
+ * surface satisfies |kappa(x) - kappa(p)| = |x - p| / (|x||p|) with |x-p| >= D,
+ * |p| <= min(R_max, rho + |x-p|), so
+ *     R* = D / (rho * min(R_max, rho + D))
+ * is a valid radius.  Far field (|y| R_max <= 1/2): the ball about 0 of radius
+ * 1/R_max is the image of the outside of the bounding sphere, so
+ * R* = 1/R_max - |y| needs no query.  Stop when R* < eps; the exit point is
+ * the primal closest point.
+ */
+static int walk_on_spheres_kelvin(const orc_geom *g, const orc_params *P, uint32_t sample, uint32_t walk,
+                                  const double z[3], orc_hit *h)
+{
+    double y[3] = { z[0], z[1], z[2] };
+    for (int k = 0; ; ++k) {
+        double yn = norm3(y), Rstar;
+        if (yn * P->Rmax_norm <= 0.5) {
+            Rstar = 1.0 / P->Rmax_norm - yn;
+        } else {
+            double x[3] = { P->origin[0] + y[0] / (yn * yn), P->origin[1] + y[1] / (yn * yn), P->origin[2] + y[2] / (yn * yn) };
+            double rho = 1.0 / yn;
+            orc_closest_point(g, x, h);
+            Rstar = h->dist / (rho * fmin(P->Rmax_norm, rho + h->dist));
+            if (Rstar < P->eps) return k;
+        }
+        if (k == P->max_steps) return -1;
+        double w[3];
+        step_direction(P->seed, sample, walk, (uint32_t)(k + 1), w);
+        for (int j = 0; j < 3; ++j) y[j] += Rstar * w[j];
+    }
+}
+
+/* ------------------------------------------------------------------------- */
+/* Per-walk record: what one Monte Carlo sample contributes (Alg. 2 lines     */
+/* 273-285; Eq. 32).                                                          */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    int64_t sample;             /* boundary sample index, -1 for a killing walk             */
+    int64_t tri_t;              /* exit face (-1: analytic sphere)                          */
+    double bary_t[3];
+    double t[3];                /* exit point on the primal surface                         */
+    double z[3];                /* start point of the walk (walk-domain coordinates)        */
+    double weight;              /* full scalar multiplying d d^T (0 if truncated/discarded) */
+    int32_t steps;              /* jumps taken; -1 truncated; -2 sample discarded           */
+    int32_t pad_;
+} orc_record;
+
+static void fill_sample(const orc_geom *g, const int32_t *tri, const float *bary, const float *weight,
+                        const float *normal, const double *pos, int64_t i, orc_sample *S)
+{
+    S->a = weight[i];
+    if (g->kind == 0) {
+        int64_t f = tri[i];
+        double a[3], b[3], c[3], area;
+        load_vertex(g, g->faces[3*f], a); load_vertex(g, g->faces[3*f+1], b); load_vertex(g, g->faces[3*f+2], c);
+        for (int k = 0; k < 3; ++k) S->bary[k] = bary[3*i+k];
+        for (int k = 0; k < 3; ++k) S->s[k] = S->bary[0] * a[k] + S->bary[1] * b[k] + S->bary[2] * c[k];
+        face_normal_area(g, f, S->n, &area);
+        S->tri = f;
+    } else {                       /* analytic sphere: position given, normal radial */
+        for (int k = 0; k < 3; ++k) S->s[k] = pos[3*i+k];
+        double d[3]; sub3(S->s, g->centre, d);
+        double l = norm3(d);
+        for (int k = 0; k < 3; ++k) S->n[k] = d[k] / l;
+        S->tri = -1; S->bary[0] = 1.0; S->bary[1] = S->bary[2] = 0.0;
+    }
+    if (normal) for (int k = 0; k < 3; ++k) S->n[k] = normal[3*i+k];
+}
+
+/*
+ * Run every walk of every sample and write one record per walk at slot
+ * sample*W + walk (then the killing walks).  exterior = 0: Alg. 2; 1: Eq. 32.
+ * balls_out (optional) receives r, c, |s*| per sample for the A2 parity test.
+ * Returns the number of records.
+ */
+int64_t orc_run_walks(const orc_geom *g, const orc_params *P, int exterior,
+                      const int32_t *tri, const float *bary, const float *weight,
+                      const float *normal, const double *pos, int64_t n_s,
+                      orc_record *rec, double *balls_out /* [n_s][5] or NULL */)
+{
+    const int W = P->walks_per_sample;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < n_s; ++i) {
+        orc_sample S;
+        orc_ball B;
+        fill_sample(g, tri, bary, weight, normal, pos, i, &S);
+        if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
+        else          orc_tangent_ball_interior(g, P, &S, &B);
+        if (balls_out) { balls_out[5*i] = B.r; balls_out[5*i+1] = B.c[0]; balls_out[5*i+2] = B.c[1]; balls_out[5*i+3] = B.c[2]; balls_out[5*i+4] = B.sstar_norm; }
+        for (int w = 0; w < W; ++w) {
+            orc_record *R = rec + i * W + w;
+            memset(R, 0, sizeof *R);
+            R->sample = i; R->tri_t = -1;
+            if (!(B.r > 0.0)) { R->steps = -2; continue; }      /* discarded sample */
+            double factor = sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, R->z);
+            orc_hit h;
+            int steps = exterior ? walk_on_spheres_kelvin(g, P, (uint32_t)i, (uint32_t)w, R->z, &h)
+                                 : walk_on_spheres(g, P, (uint32_t)i, (uint32_t)w, R->z, &h);
+            R->steps = steps;
+            if (steps < 0) continue;                              /* truncated: contributes nothing */
+            R->tri_t = h.tri;
+            memcpy(R->bary_t, h.bary, sizeof h.bary);
+            memcpy(R->t, h.cp, sizeof h.cp);
+            double wgt = (S.a / W) * factor;                      /* |dOmega| |dB| J / (2N), Alg. 2 */
+            if (exterior) {
+                double tt[3]; sub3(h.cp, P->origin, tt);
+                /* |s*|^3 / |t*|, Eq. 32;  1/|t*| = |t - o| */
+                wgt *= B.sstar_norm * B.sstar_norm * B.sstar_norm * norm3(tt);
+            }
+            R->weight = wgt;
+        }
+    }
+    int64_t n_rec = n_s * W;
+    if (exterior && P->include_killing) {
+        /* second expectation of Eq. 32: walks from 0 = kappa(infinity), Eq. 74 */
+        #pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t j = 0; j < P->n_kill_walks; ++j) {
+            orc_record *R = rec + n_rec + j;
+            memset(R, 0, sizeof *R);
+            R->sample = -1; R->tri_t = -1;
+            orc_hit h;
+            int steps = walk_on_spheres_kelvin(g, P, ORC_KILLING_SAMPLE, (uint32_t)j, R->z, &h);
+            R->steps = steps;
+            if (steps < 0) continue;
+            R->tri_t = h.tri;
+            memcpy(R->bary_t, h.bary, sizeof h.bary);
+            memcpy(R->t, h.cp, sizeof h.cp);
+            double tt[3]; sub3(h.cp, P->origin, tt);
+            R->weight = 4.0 * ORC_PI * norm3(tt) / (double)P->n_kill_walks;    /* 4 pi / |t0*| */
+        }
+        n_rec += P->n_kill_walks;
+    }
+    return n_rec;
+}
+
+/*
+ * Accumulate S = sum_w weight_w d d^T in the hat basis (PAPER.md:177-190,
+ * 277-285): d = b(s) - b(t) has the barycentric coordinates of s on the
+ * vertices of tri_s and minus those of t on the vertices of tri_t; a killing
+ * record contributes weight * b(t0) b(t0)^T.  Records are visited in slot
+ * order.  S2 (optional) receives an estimate of the variance of every entry:
+ * for each sample, W/(W-1) * (sum x^2 - (sum x)^2 / W) over its walks' entry
+ * contributions x (killing walks form one group).
+ */
+typedef struct { int64_t key; double val; } orc_entry;
+static int entry_cmp(const void *a, const void *b)
+{
+    int64_t ka = ((const orc_entry *)a)->key, kb = ((const orc_entry *)b)->key;
+    return (ka > kb) - (ka < kb);
+}
+
+static int build_d(const orc_geom *g, const orc_record *R, const int32_t *tri, const float *bary,
+                   int64_t idx[6], double val[6])
+{
+    int n = 0;
+    if (R->sample >= 0) {
+        const int32_t *fs = g->faces + 3 * (int64_t)tri[R->sample];
+        for (int k = 0; k < 3; ++k) { idx[n] = fs[k]; val[n] = (double)bary[3*R->sample + k]; ++n; }
+    }
+    const int32_t *ft = g->faces + 3 * R->tri_t;
+    double sign = (R->sample >= 0) ? -1.0 : 1.0;
+    for (int k = 0; k < 3; ++k) {
+        int found = -1;
+        for (int m = 0; m < n; ++m) if (idx[m] == ft[k]) found = m;
+        if (found >= 0) val[found] += sign * R->bary_t[k];
+        else { idx[n] = ft[k]; val[n] = sign * R->bary_t[k]; ++n; }
+    }
+    return n;
+}
+
+void orc_accumulate_hat(const orc_geom *g, const orc_record *rec, int64_t n_rec,
+                        const int32_t *tri, const float *bary, int64_t K,
+                        double *S /* [K][K] zeroed by caller */, double *S2 /* [K][K] or NULL */)
+{
+    orc_entry *buf = NULL;
+    int64_t cap = 0;
+    for (int64_t g0 = 0; g0 < n_rec; ) {
+        /* one group = the walks of one sample (or all killing walks) */
+        int64_t g1 = g0;
+        int64_t sample = rec[g0].sample;
+        while (g1 < n_rec && rec[g1].sample == sample) ++g1;
+        int64_t n_e = 0;
+        if (S2 && 36 * (g1 - g0) > cap) { cap = 36 * (g1 - g0); buf = (orc_entry *)realloc(buf, cap * sizeof *buf); }
+        for (int64_t r = g0; r < g1; ++r) {
+            const orc_record *R = rec + r;
+            if (R->steps < 0 || R->weight == 0.0) continue;
+            int64_t idx[6]; double val[6];
+            int n = build_d(g, R, tri, bary, idx, val);
+            for (int p = 0; p < n; ++p) for (int q = 0; q < n; ++q) {
+                double x = R->weight * val[p] * val[q];
+                S[idx[p] * K + idx[q]] += x;
+                if (S2) { buf[n_e].key = idx[p] * K + idx[q]; buf[n_e].val = x; ++n_e; }
+            }
+        }
+        if (S2 && n_e > 0) {
+            double Wg = (double)(g1 - g0);
+            qsort(buf, (size_t)n_e, sizeof *buf, entry_cmp);
+            for (int64_t e0 = 0; e0 < n_e; ) {
+                int64_t e1 = e0; double s1 = 0.0, s2 = 0.0;
+                while (e1 < n_e && buf[e1].key == buf[e0].key) { s1 += buf[e1].val; s2 += buf[e1].val * buf[e1].val; ++e1; }
+                double var = (Wg > 1.0) ? Wg / (Wg - 1.0) * (s2 - s1 * s1 / Wg) : s2;
+                S2[buf[e0].key] += var > 0.0 ? var : 0.0;
+                e0 = e1;
+            }
+        }
+        g0 = g1;
+    }
+    free(buf);
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+size_t orc_sizeof_record(void) { return sizeof(orc_record); }
+size_t orc_sizeof_params(void) { return sizeof(orc_params); }
+size_t orc_sizeof_geom(void)   { return sizeof(orc_geom); }

@@ -1,0 +1,355 @@
+"""Pins for the oracle's estimator pieces against what the paper and the
+mathematics fix (no GPU): tangent balls, walk-on-spheres harmonic-measure
+identities, the analytic-ball spectra l (interior) and l+1 (exterior, centred
+and off-centre), capacity, and the structural invariants on meshes."""
+import numpy as np
+import pytest
+from scipy.integrate import quad
+from scipy.special import eval_legendre
+
+from oracle import Oracle, OracleParams, mesh_geom, sphere_geom, steklov_eigs
+from synth import box, icosphere, merge_meshes, uniform_samples, vertex_cell_samples
+
+from sph import DEGREES, fibonacci_sphere, real_sph_harm
+
+
+# --------------------------------------------------------------------------
+# tangent balls
+# --------------------------------------------------------------------------
+def test_tangent_ball_interior_sphere_closed_form():
+    orc = Oracle(sphere_geom((0.1, -0.2, 0.3), 2.0))
+    pos = fibonacci_sphere(32) * 2.0 + np.array([0.1, -0.2, 0.3])
+    w = np.full(32, 1.0, np.float32)
+    for rmax, want in ((1.4, 1.4 * 1023 / 1024), (4.0, 2.0)):
+        P = OracleParams(walks_per_sample=1, eps=1e-4, rmax=rmax)
+        _, balls = orc.run_walks(P, False, weight=w, pos=pos)
+        assert np.abs(balls[:, 0] - want).max() <= rmax / 1024 + 1e-4
+        c = balls[:, 1:4]
+        n = (pos - np.array([0.1, -0.2, 0.3])) / 2.0
+        assert np.abs(c - (pos - balls[:, :1] * n)).max() < 1e-12
+
+
+def test_tangent_ball_cube_face_closed_form():
+    """Unit cube: r_max = 1/2.  At distance a from a (90 degree) edge, well away from
+    the other edges, the largest tangent ball has radius min(a, r_max)."""
+    v, f = box((1, 1, 1), (1, 1, 1))
+    orc = Oracle(mesh_geom(v, f))
+    assert orc.rmax() == 0.5
+    # face +x is made of two triangles; pick points by brute force through bary of face 0
+    fx = [k for k in range(len(f)) if np.allclose(v[f[k]][:, 0], 0.5)]
+    k = fx[0]
+    tv = v[f[k]].astype(np.float64)
+    rng = np.random.default_rng(0)
+    bary = rng.dirichlet(np.ones(3), 200)
+    p = bary @ tv
+    a = 0.5 - np.abs(p[:, 1:]).max(1)                      # distance to the nearest edge of the face
+    P = OracleParams(walks_per_sample=1, eps=1e-6)
+    _, balls = orc.run_walks(P, False, tri=np.full(200, k), bary=bary, weight=np.ones(200))
+    assert np.abs(balls[:, 0] - np.minimum(a, 0.5)).max() <= 0.5 / 1024 + 1e-6
+
+
+def test_tangent_ball_exterior_offcentre_sphere():
+    """Kelvin image of a sphere (centre c0, radius R, origin inside) is a sphere; the
+    normal n* of Eq. 54 must be its outward normal at s*, and every admissible
+    tangent ball fits, so r = hi * 1023/1024 with hi = min(r_max, 0.45 |s*|^2 / (s*.n*))."""
+    c0, R = np.array([0.3, 0.0, 0.0]), 1.0
+    orc = Oracle(sphere_geom(c0, R))
+    pos = fibonacci_sphere(64) * R + c0
+    P = OracleParams(walks_per_sample=1, eps=1e-6, rmax=10.0, Rmax_norm=1.3)
+    _, balls = orc.run_walks(P, True, weight=np.ones(64, np.float32), pos=pos)
+    sstar = pos / (pos ** 2).sum(1, keepdims=True)
+    den = R * R - c0 @ c0
+    cstar_img, r_img = -c0 / den, R / den                  # inverted sphere
+    n_true = (sstar - cstar_img) / r_img
+    r, c = balls[:, 0], balls[:, 1:4]
+    nstar = (sstar - c) / r[:, None]
+    assert np.abs(nstar - n_true).max() < 1e-9
+    assert np.abs(balls[:, 4] - np.linalg.norm(sstar, axis=1)).max() < 1e-12
+    hi = 0.45 * (sstar ** 2).sum(1) / np.einsum("ij,ij->i", sstar, n_true)
+    assert np.allclose(r, hi * 1023 / 1024, rtol=1e-12)
+    assert (np.linalg.norm(c, axis=1) > r).all()           # the ball does not contain 0
+
+
+# --------------------------------------------------------------------------
+# walk on spheres: exit points follow harmonic measure (Eq. 5)
+# --------------------------------------------------------------------------
+def _assert_mean_zero(x, nsig=4.5):
+    x = np.asarray(x, np.float64)
+    se = x.std(ddof=1) / np.sqrt(len(x))
+    assert abs(x.mean()) <= nsig * se + 1e-4, (x.mean(), se)
+
+
+def test_wos_interior_harmonic_functions_sphere_and_mesh():
+    # analytic sphere: E[h(t)] = h(z) for harmonic h
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    pos = fibonacci_sphere(200)
+    P = OracleParams(seed=5, walks_per_sample=64, eps=1e-5, rmax=0.5, importance_sample=False)
+    rec, _ = orc.run_walks(P, False, weight=np.ones(200, np.float32), pos=pos)
+    ok = rec["steps"] >= 0
+    t, z = rec["t"][ok], rec["z"][ok]
+    assert (np.abs(np.linalg.norm(t, axis=1) - 1) < 1e-12).all()
+    assert rec["steps"][ok].mean() > 3
+    pole = np.array([0.4, -1.1, 0.9])                      # outside the ball
+    for h in (lambda x: x[:, 0], lambda x: x[:, 2], lambda x: x[:, 0] ** 2 - x[:, 1] ** 2,
+              lambda x: x[:, 0] * x[:, 1] * x[:, 2], lambda x: 1 / np.linalg.norm(x - pole, axis=1)):
+        _assert_mean_zero(h(t) - h(z))
+    # mesh (cube): coordinates are harmonic, E[t] = z
+    v, f = box((1, 1, 1), (2, 2, 2))
+    orc = Oracle(mesh_geom(v, f))
+    smp = uniform_samples(v, f, 300, seed=1)
+    P = OracleParams(seed=6, walks_per_sample=32, eps=1e-4, importance_sample=False)
+    rec, _ = orc.run_walks(P, False, smp["tri"], smp["bary"], smp["weight"])
+    ok = rec["steps"] >= 0
+    for k in range(3):
+        _assert_mean_zero(rec["t"][ok][:, k] - rec["z"][ok][:, k])
+    # exit points are on the surface, on the reported face
+    tri = f[rec["tri_t"][ok]]
+    cp = np.einsum("qk,qkd->qd", rec["bary_t"][ok], v[tri].astype(np.float64))
+    assert np.abs(cp - rec["t"][ok]).max() < 1e-12
+
+
+@pytest.mark.parametrize("origin", [(0.0, 0.0, 0.0), (0.3, 0.1, -0.2)])
+def test_wos_kelvin_harmonic_measure(origin):
+    """u(x) = 1/|x - p| (p inside the solid) is harmonic outside and decays, so
+    kappa[u](y) = |x| u(x) is harmonic in the inverted domain (Eq. 55): its mean
+    over the exit points of walks from z* equals its value at z*; from y = 0
+    (killing walks) it equals lim |x| u(x) = 1, and E|t0 - o| is the capacity R."""
+    o = np.array(origin)
+    R = 1.2
+    orc = Oracle(sphere_geom((0, 0, 0), R))
+    pos = fibonacci_sphere(150) * R
+    P = OracleParams(seed=9, walks_per_sample=64, eps=1e-6, rmax=10.0, importance_sample=False,
+                     origin=origin, Rmax_norm=R + np.linalg.norm(o),
+                     include_killing=True, n_kill_walks=20000)
+    rec, _ = orc.run_walks(P, True, weight=np.ones(150, np.float32), pos=pos)
+    ok = rec["steps"] >= 0
+    assert ok.all()
+    jump, kill = rec[rec["sample"] >= 0], rec[rec["sample"] < 0]
+    p = o + np.array([0.2, -0.3, 0.1])
+
+    def kelvin_u(y_or_t, is_kelvin):
+        if is_kelvin:
+            xt = y_or_t / (y_or_t ** 2).sum(1, keepdims=True)          # x - o
+        else:
+            xt = y_or_t - o
+        return np.linalg.norm(xt, axis=1) / np.linalg.norm(xt + o - p, axis=1)
+
+    _assert_mean_zero(kelvin_u(jump["t"], False) - kelvin_u(jump["z"], True))
+    _assert_mean_zero(kelvin_u(kill["t"], False) - 1.0)
+    _assert_mean_zero(np.linalg.norm(kill["t"] - o, axis=1) - R)
+    assert np.abs(np.linalg.norm(rec["t"], axis=1) - R).max() < 1e-9
+
+
+# --------------------------------------------------------------------------
+# analytic ball: Steklov spectra l (interior) and l + 1 (exterior)
+# --------------------------------------------------------------------------
+def _cap_spectrum(l, theta0_deg):
+    """Expectation of the estimator on the unit ball when the tangent ball is the
+    whole ball (Funk-Hecke applied to Eq. 20 with J of Eq. 23 outside the cap)."""
+    t0 = np.deg2rad(theta0_deg)
+    f = lambda th: (1 - eval_legendre(l, np.cos(th))) * np.cos(th / 2) / (4 * np.sin(th / 2) ** 2)
+    return quad(f, t0, np.pi, limit=200)[0]
+
+
+def _galerkin_from_records(rec, pos_s, centre):
+    """S = sum_w weight (Y(s) - Y(t)) (Y(s) - Y(t))^T, killing: weight Y(t) Y(t)^T."""
+    jump, kill = rec[rec["sample"] >= 0], rec[rec["sample"] < 0]
+    jump = jump[jump["steps"] >= 0]
+    Ys = real_sph_harm(pos_s - centre)[jump["sample"]]
+    Yt = real_sph_harm(jump["t"] - centre)
+    d = Ys - Yt
+    S = (d * jump["weight"][:, None]).T @ d
+    Sk = np.zeros_like(S)
+    if len(kill):
+        Yk = real_sph_harm(kill["t"] - centre)
+        Sk = (Yk * kill["weight"][:, None]).T @ Yk
+    return S, Sk
+
+
+def test_interior_unit_ball_whole_ball_matches_cap_quadrature():
+    n_s, W = 4000, 64
+    pos = fibonacci_sphere(n_s)
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    for imp in (True, False):
+        P = OracleParams(seed=1, walks_per_sample=W, eps=1e-2, rmax=1.0 * 1024 / 1023,
+                         importance_sample=imp, cap_half_angle_deg=2.5)
+        rec, balls = orc.run_walks(P, False, weight=np.full(n_s, 4 * np.pi / n_s, np.float32), pos=pos)
+        assert np.allclose(balls[:, 0], 1.0, atol=1e-12)
+        assert (rec["steps"] == 0).all()
+        S, _ = _galerkin_from_records(rec, pos, np.zeros(3))
+        want = np.array([_cap_spectrum(l, 2.5) for l in DEGREES])
+        tol = 0.03 if imp else 0.15
+        assert np.abs(np.diag(S) - want).max() < tol, (np.diag(S), want)
+        off = S - np.diag(np.diag(S))
+        assert np.abs(off).max() < tol
+
+
+def test_cap_quadrature_tends_to_l():
+    for l in range(0, 5):
+        assert abs(_cap_spectrum(l, 1e-3) - l) < 1e-3
+    assert abs(_cap_spectrum(1, 2.5) - (1 - np.sin(np.deg2rad(1.25)))) < 1e-9
+
+
+def test_interior_unit_ball_half_radius_walks_give_l():
+    """Tangent balls of radius 1/2: now the walks matter.  Small cap, so the
+    spectrum is l minus about (l+1) sin(theta0/2)."""
+    n_s, W = 6000, 64
+    pos = fibonacci_sphere(n_s)
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    P = OracleParams(seed=2, walks_per_sample=W, eps=1e-5, rmax=0.5 * 1024 / 1023, cap_half_angle_deg=0.5)
+    rec, balls = orc.run_walks(P, False, weight=np.full(n_s, 4 * np.pi / n_s, np.float32), pos=pos)
+    assert np.allclose(balls[:, 0], 0.5, atol=1e-9)
+    S, _ = _galerkin_from_records(rec, pos, np.zeros(3))
+    lam = np.diag(S)
+    assert abs(lam[0]) < 1e-12                                        # constants are annihilated
+    for k in range(1, len(DEGREES)):
+        l = DEGREES[k]
+        assert abs(lam[k] - l) < 0.06 * l + 0.02, (l, lam[k])
+    off = S - np.diag(lam)
+    assert np.abs(off).max() < 0.12
+
+
+@pytest.mark.parametrize("origin,R", [((0.0, 0.0, 0.0), 1.0), ((0.3, 0.0, 0.0), 1.0), ((0.0, 0.2, 0.1), 2.0)])
+def test_exterior_sphere_jump_l_killing_one(origin, R):
+    """Exterior Steklov eigenvalues of a sphere are (l+1)/R: jump part l/R
+    (Eq. 30 weights |s*|^3/|t*|), killing part K = 1/R (Eq. 31), also when the
+    Kelvin origin is off-centre so that both factors are non-trivial."""
+    n_s, W = 6000, 64
+    o = np.array(origin)
+    pos = fibonacci_sphere(n_s) * R
+    orc = Oracle(sphere_geom((0, 0, 0), R))
+    P = OracleParams(seed=3, walks_per_sample=W, eps=1e-5 / R, rmax=10.0, cap_half_angle_deg=0.5,
+                     origin=origin, Rmax_norm=R + np.linalg.norm(o),
+                     include_killing=True, n_kill_walks=n_s * W)
+    rec, _ = orc.run_walks(P, True, weight=np.full(n_s, 4 * np.pi * R * R / n_s, np.float32), pos=pos)
+    assert (rec["steps"] >= 0).all()
+    S, Sk = _galerkin_from_records(rec, pos, np.zeros(3))
+    # Y is orthonormal on the UNIT sphere: int_{|x|=R} Y_i Y_j = R^2 delta_ij
+    lam_jump, lam_kill = np.diag(S) / R ** 2, np.diag(Sk) / R ** 2
+    for k, l in enumerate(DEGREES):
+        assert abs(lam_jump[k] - l / R) < (0.07 * l + 0.03) / R, ("jump", l, lam_jump[k])
+        assert abs(lam_kill[k] - 1 / R) < 0.06 / R, ("kill", l, lam_kill[k])
+    assert np.abs(S - np.diag(np.diag(S))).max() / R ** 2 < 0.2 / R
+    assert np.abs(Sk - np.diag(np.diag(Sk))).max() / R ** 2 < 0.06 / R
+    # capacity: 1^T S_kill 1 = 4 pi E|t0| = 4 pi R
+    kill = rec[rec["sample"] < 0]
+    assert abs(kill["weight"].sum() - 4 * np.pi * R) < 0.02 * 4 * np.pi * R
+
+
+# --------------------------------------------------------------------------
+# meshes: structural invariants of Alg. 2 / Eq. 32 and sphere multiplicities
+# --------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def ico2_interior():
+    v, f = icosphere(2)
+    orc = Oracle(mesh_geom(v, f))
+    smp = vertex_cell_samples(v, f, 8, seed=0)
+    P = OracleParams(seed=0, walks_per_sample=128, eps=1e-3)
+    out = orc.estimate_dtn(P, False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    return v, f, orc, smp, out
+
+
+def test_config0_interior_invariants_and_multiplicities(ico2_interior):
+    v, f, orc, smp, out = ico2_interior
+    S = out["S"]
+    assert np.abs(S - S.T).max() <= 1e-15 * np.abs(S).max()            # symmetric by construction
+    assert np.linalg.eigvalsh(S).min() >= -1e-12 * np.abs(S).max()     # PSD for any N
+    assert np.abs(S.sum(1)).max() <= 1e-6 * np.abs(S).max()            # constants annihilated (385)
+    lam = steklov_eigs(S, orc.mass_matrix(), 16)
+    assert abs(lam[0]) < 1e-6
+    groups = [lam[1:4], lam[4:9], lam[9:16]]
+    for l, g in zip((1, 2, 3), groups):
+        assert abs(g.mean() - l) < 0.12 * l                            # biased low by cap and eps
+        assert g.max() - g.min() < 0.25
+    assert groups[1].min() - groups[0].max() > 0.5 and groups[2].min() - groups[1].max() > 0.4
+    rec = out["records"]
+    assert (rec["steps"] >= 0).all() and 3.0 < rec["steps"].mean() < 5.0
+    assert 0.45 < (rec["steps"] == 0).mean() < 0.6
+
+
+def test_interior_scales_inversely_with_size(ico2_interior):
+    v, f, orc, smp, out = ico2_interior
+    v2 = (v.astype(np.float64) * 2.0).astype(np.float32)               # exact in fp32
+    orc2 = Oracle(mesh_geom(v2, f))
+    P2 = OracleParams(seed=0, walks_per_sample=128, eps=2e-3)
+    out2 = orc2.estimate_dtn(P2, False, smp["tri"], smp["bary"], smp["weight"] * 4.0)
+    assert np.allclose(out2["S"], 2.0 * out["S"], rtol=1e-9, atol=1e-12)
+    lam = steklov_eigs(out["S"], orc.mass_matrix(), 9)
+    lam2 = steklov_eigs(out2["S"], orc2.mass_matrix(), 9)
+    assert np.allclose(lam2[1:], lam[1:] / 2.0, rtol=1e-6)
+
+
+def test_variance_is_order_one_over_n():
+    v, f = icosphere(1)
+    orc = Oracle(mesh_geom(v, f))
+    tot = []
+    for W in (32, 128):
+        smp = vertex_cell_samples(v, f, 16, seed=1)
+        P = OracleParams(seed=4, walks_per_sample=W, eps=1e-3)
+        out = orc.estimate_dtn(P, False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+        tot.append(out["var"].sum())
+    assert 3.0 < tot[0] / tot[1] < 5.3                                 # 4x the walks, 1/4 the variance
+    # the variance estimate is honest: two seeds differ by about sqrt(2) sigma
+    smp = vertex_cell_samples(v, f, 16, seed=1)
+    outs = [orc.estimate_dtn(OracleParams(seed=s, walks_per_sample=128, eps=1e-3), False,
+                             smp["tri"], smp["bary"], smp["weight"], want_var=True) for s in (11, 12)]
+    sig = np.sqrt(outs[0]["var"] + outs[1]["var"])
+    m = sig > 0
+    zscore = (outs[0]["S"] - outs[1]["S"])[m] / sig[m]
+    assert 0.8 < zscore.std() < 1.25
+    assert (np.abs(zscore) > 4).mean() < 2e-3
+
+
+def test_exterior_mesh_sphere_l_plus_one_and_killing_flag():
+    v, f = icosphere(2)
+    orc = Oracle(mesh_geom(v, f))
+    smp = vertex_cell_samples(v, f, 8, seed=0)
+    M = orc.mass_matrix()
+    base = dict(seed=0, walks_per_sample=128, eps=1e-3, origin=(0.1, 0.0, 0.05))
+    off = orc.estimate_dtn(OracleParams(**base), True, smp["tri"], smp["bary"], smp["weight"])
+    on = orc.estimate_dtn(OracleParams(**base, include_killing=True, n_kill_walks=len(smp["tri"]) * 128),
+                          True, smp["tri"], smp["bary"], smp["weight"])
+    for out in (off, on):
+        S = out["S"]
+        assert np.abs(S - S.T).max() <= 1e-15 * np.abs(S).max()
+        assert np.linalg.eigvalsh(S).min() >= -1e-12 * np.abs(S).max()
+    assert np.abs(off["S"].sum(1)).max() <= 1e-6 * np.abs(off["S"]).max()      # footnote at PAPER.md:385
+    lam_off = steklov_eigs(off["S"], M, 9)
+    lam_on = steklov_eigs(on["S"], M, 9)
+    assert abs(lam_off[0]) < 1e-6
+    assert abs(lam_off[1:4].mean() - 1) < 0.12 and abs(lam_off[4:9].mean() - 2) < 0.25
+    assert abs(lam_on[0] - 1) < 0.06                                            # l + 1 with l = 0
+    assert abs(lam_on[1:4].mean() - 2) < 0.15 and abs(lam_on[4:9].mean() - 3) < 0.3
+    kill = on["records"][on["records"]["sample"] < 0]
+    cap = kill["weight"].sum() / (4 * np.pi)
+    assert 0.95 < cap < 1.0                                                     # polyhedron inside the unit ball
+
+
+def test_interior_blocks_vanish_and_exterior_couples_with_decay():
+    """the interior operator does not couple disjoint solids, the
+    exterior one does, less so as they move apart.  Also the capacity of two unit
+    spheres at centre distance 2.5 from the classical image series."""
+    norms = []
+    for dist in (2.5, 4.0):
+        parts = [icosphere(1, 1.0, (-dist / 2, 0, 0)), icosphere(1, 1.0, (dist / 2, 0, 0))]
+        v, f, vid, fid = merge_meshes(parts)
+        orc = Oracle(mesh_geom(v, f))
+        smp = vertex_cell_samples(v, f, 4, seed=2)
+        A, B = vid == 0, vid == 1
+        if dist == 2.5:
+            Si = orc.estimate_dtn(OracleParams(seed=1, walks_per_sample=32, eps=1e-3), False,
+                                  smp["tri"], smp["bary"], smp["weight"])["S"]
+            assert np.abs(Si[np.ix_(A, B)]).max() == 0.0
+        P = OracleParams(seed=1, walks_per_sample=256, eps=1e-3, origin=(-dist / 2, 0, 0),
+                         include_killing=(dist == 2.5), n_kill_walks=40000)
+        out = orc.estimate_dtn(P, True, smp["tri"], smp["bary"], smp["weight"])
+        Se = out["S"]
+        norms.append(np.linalg.norm(Se[np.ix_(A, B)]))
+        if dist == 2.5:
+            kill = out["records"][out["records"]["sample"] < 0]
+            cap = kill["weight"].sum() / (4 * np.pi)
+            beta = np.arccosh(dist / 2.0)
+            series = 2 * np.sinh(beta) * sum((-1) ** (n + 1) / np.sinh(n * beta) for n in range(1, 200))
+            assert abs(series - 1.4553) < 1e-3
+            assert 0.90 * series < cap < 1.01 * series          # level-1 polyhedra are a bit smaller
+    assert norms[0] > 0 and norms[1] > 0 and norms[1] < 0.7 * norms[0]
