@@ -260,7 +260,7 @@ def test_config0_interior_invariants_and_multiplicities(ico2_interior):
     groups = [lam[1:4], lam[4:9], lam[9:16]]
     for l, g in zip((1, 2, 3), groups):
         assert abs(g.mean() - l) < 0.12 * l                            # biased low by cap and eps
-        assert g.max() - g.min() < 0.25
+        assert g.max() - g.min() < 0.12 * l + 0.05      # MC spread inside a multiplet
     assert groups[1].min() - groups[0].max() > 0.5 and groups[2].min() - groups[1].max() > 0.4
     rec = out["records"]
     assert (rec["steps"] >= 0).all() and 3.0 < rec["steps"].mean() < 5.0
