@@ -1,0 +1,233 @@
+/*
+ * mcdtn.h -- C ABI of the B200-native Monte Carlo Dirichlet-to-Neumann estimator.
+ *
+ * Hot path of "Monte Carlo Steklov Operators for Large-Scale Geometry Processing
+ * in the Wild" (arxiv 2606.05581; citations are PAPER.md:<line>): the
+ * walk-on-spheres estimator that fills the discrete DtN matrix of a triangle
+ * mesh, interior (Alg. 2 / Eq. 26) and exterior (Eq. 32,
+ * PAPER.md:348-353, App. C.3-C.7).
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its comment says "host".
+ *   - The caller owns every buffer it passes in; the library owns only the
+ *     opaque mcs_bvh handle (packed triangles + nodes in device memory).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *     Work is enqueued on it; a call blocks the host only where stated.
+ *   - Return value: MCS_OK (0) or a negative MCS_E* code.  No exceptions, no
+ *     aborts.  mcs_error_string() names a code.
+ *   - All floating point on this path is fp32 (the paper states no precision);
+ *     statistics counters are 64-bit integers.
+ *   - There is no CPU fallback: every entry point needs a CUDA device.
+ */
+#ifndef MCDTN_H
+#define MCDTN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MCS_OK            0
+#define MCS_EINVAL      (-1)   /* null / negative size / index out of range / eps <= 0 / K mismatch */
+#define MCS_EDEGENERATE (-2)   /* zero total area, non-finite vertex, Kelvin origin on a vertex      */
+#define MCS_ENOMEM      (-3)   /* workspace too small or device allocation failed                     */
+#define MCS_ECUDA       (-4)   /* CUDA runtime error (code in mcs_stats.cuda_error when available)    */
+
+typedef struct mcs_bvh mcs_bvh;
+
+/* ------------------------------------------------------------------------ */
+/* (1) LBVH over the triangle soup -- subsystem "A0 mesh pack" + "A1 LBVH     */
+/* build" of SURVEY.md 8(a).  The paper uses a BVH for its distance queries   */
+/* and treats every triangle as absorbing, so   */
+/* the build assumes nothing about manifoldness, orientation, area or the     */
+/* number of components.                                                       */
+/* ------------------------------------------------------------------------ */
+typedef struct {
+    int32_t reserved;            /* must be 0 */
+} mcs_build_opts;
+
+typedef struct {
+    int64_t V, F;                /* vertices, faces                                  */
+    int64_t n_nodes;             /* internal nodes of the packed tree                */
+    int32_t max_depth;           /* deepest leaf (root = 0)                          */
+    int32_t n_degenerate;        /* zero-area faces (kept: they absorb as segments)  */
+    float   aabb_lo[3], aabb_hi[3];   /* box of the vertices referenced by faces     */
+    double  area;                /* total surface area |dOmega|                      */
+    size_t  device_bytes;        /* device memory owned by the handle                */
+} mcs_bvh_info_t;
+
+/*
+ * Build.  verts [V][3] fp32 and faces [F][3] int32 are read on `stream`; the
+ * handle keeps its own copies, so the caller may free them after the call.
+ * Blocks the host until the build has finished (it reads back error flags).
+ * Errors: MCS_EINVAL (null pointer, V < 1, F < 1, face index outside [0,V)),
+ * MCS_EDEGENERATE (non-finite vertex, zero total area), MCS_ENOMEM, MCS_ECUDA.
+ */
+int  mcs_build_bvh(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                   const mcs_build_opts* opts /* host, may be NULL */,
+                   void* stream, mcs_bvh** out /* host */);
+void mcs_free_bvh(mcs_bvh* bvh);
+int  mcs_bvh_info(const mcs_bvh* bvh, mcs_bvh_info_t* out /* host */);
+
+/*
+ * Structure dump for the invariant tests (SURVEY.md 8(c) "LBVH (GPU)").
+ * Each output may be NULL.  nodes: [n_nodes][16] 32-bit words, the packed node
+ * (see DESIGN.md "BVH node"); leaf_tri: [F] original face index of the k-th
+ * leaf in Morton order; morton: [F] sorted 63-bit keys.  Blocks the host.
+ */
+int  mcs_bvh_dump(const mcs_bvh* bvh, uint32_t* nodes, int32_t* leaf_tri, uint64_t* morton,
+                  void* stream);
+
+/* ------------------------------------------------------------------------ */
+/* (2) Closest point on the triangle soup -- the geometric query under WoS    */
+/* ("nearest boundary point").                      */
+/* q [Q][3] -> dist [Q] (unsigned distance), tri [Q] (original face index;    */
+/* ties: smaller fp32 squared distance, then smaller index), bary [Q][3]       */
+/* (barycentrics of the closest point in that face).  Outputs may be NULL.    */
+/* Asynchronous on `stream`.                                                   */
+/* ------------------------------------------------------------------------ */
+int  mcs_closest_point(const mcs_bvh* bvh, const float* q, int64_t Q,
+                       float* dist, int32_t* tri, float* bary, void* stream);
+
+/* Same query by exhaustive scan over all faces on the device (cross-check of
+ * the tree; thread per query, faces tiled through shared memory).            */
+int  mcs_closest_point_bruteforce(const mcs_bvh* bvh, const float* q, int64_t Q,
+                                  float* dist, int32_t* tri, float* bary, void* stream);
+
+/* ------------------------------------------------------------------------ */
+/* (3)-(4) Estimators.                                                         */
+/* ------------------------------------------------------------------------ */
+typedef struct {                 /* boundary samples: point s with its face */
+    const int32_t* tri;          /* [n_s] face of each sample                              */
+    const float*   bary;         /* [n_s][3] barycentrics of s in that face                */
+    const float*   weight;       /* [n_s] quadrature weight a_i, sum = |dOmega| (Eq. 26)   */
+    const float*   normal;       /* [n_s][3] unit normal pointing out of the solid, or NULL
+                                    (then the face normal (v1-v0)x(v2-v0) is used)         */
+    int64_t n_s;
+} mcs_samples;
+
+typedef struct {                 /* boundary basis functions b(.) of Alg. 2 */
+    int32_t kind;                /* 0 = hat functions on the mesh vertices (K = V)            */
+    int32_t pad_;
+    int64_t K;
+} mcs_basis;
+
+typedef struct {
+    uint64_t seed;               /* Philox4x32-10 key; counter = (sample, walk, step, purpose) */
+    int32_t  walks_per_sample;   /* W >= 1                                                     */
+    int32_t  max_steps;          /* walks longer than this contribute nothing (counted)        */
+    float    eps;                /* WoS shell, absolute                    */
+    float    cap_half_angle_deg; /* excluded cap about s, PAPER.md:395 ("~2.5 deg")            */
+    float    rmax_scale;         /* r_max = rmax_scale * (shortest AABB side)/2  */
+    float    rmax_override;      /* > 0: use this r_max instead of the AABB rule               */
+    int32_t  bisection_iters;    /* LargestTangentBall iterations, PAPER.md:383 (10)           */
+    int32_t  importance_sample;  /* 1: z ~ J^B; 0: z uniform on the ball        */
+    int32_t  antithetic;         /* 1: walks 2j, 2j+1 are antipodal in azimuth  */
+    int32_t  include_killing;    /* exterior only: second expectation of Eq. 32                */
+    int64_t  n_kill_walks;       /* exterior only                                              */
+    float    kelvin_origin[3];   /* exterior only: a point strictly inside the solid */
+    int32_t  output_kind;        /* 0: dense row-major fp32 [K][K]                             */
+} mcs_params;
+
+typedef struct {
+    int32_t kind;                /* must equal params.output_kind                    */
+    int32_t pad_;
+    int64_t K;
+    float*  dense;               /* [K][K] row-major, overwritten                    */
+} mcs_matrix;
+
+typedef struct {                 /* host; filled when passed non-NULL (forces a stream sync) */
+    int64_t n_samples, n_discarded;       /* samples whose tangent ball degenerated */
+    int64_t n_walks, n_truncated;         /* walks started / cut at max_steps       */
+    int64_t n_steps;                      /* position updates x += d*omega                         */
+    int64_t n_queries;                    /* closest-point queries (bisection + every WoS iteration) */
+    int64_t n_nodes_visited, n_tris_tested;   /* traversal work actually done (flop/byte model)    */
+    int64_t n_entries, n_unique;          /* (row,col,value) records expanded / after reduction    */
+    int64_t workspace_needed;             /* bytes; set on MCS_ENOMEM too                           */
+    int32_t cuda_error;                   /* cudaError_t on MCS_ECUDA                               */
+    int32_t pad_;
+} mcs_stats;
+
+/*
+ * Workspace (bytes) the estimators need for these arguments; `exterior` selects
+ * the operator.  Pointers inside samples are not dereferenced.
+ */
+size_t mcs_workspace_bytes(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                           const mcs_params* params, int exterior);
+
+/*
+ * Interior DtN estimate (Alg. 2):
+ *   S = sum over samples i, walks w of  (a_i / W) * (|dB_r(c)| / 2) J / pdf * d d^T,
+ *   d = b(s_i) - b(t_iw), t_iw the WoS exit point of a walk started on the
+ *   largest tangent ball at s_i.  S is symmetric PSD by construction.
+ * samples/basis/params/out are host structs holding device pointers.  The
+ * library never allocates here: all scratch lives in `workspace`.
+ * Asynchronous on `stream` unless host_stats != NULL.
+ * Errors: MCS_EINVAL, MCS_ENOMEM (workspace_bytes too small), MCS_ECUDA.
+ */
+int mcs_estimate_dtn_interior(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                              const mcs_params* params, void* workspace, size_t workspace_bytes,
+                              const mcs_matrix* out, mcs_stats* host_stats, void* stream);
+
+/*
+ * Exterior DtN estimate (Eq. 32): the same estimator in the
+ * Kelvin-inverted domain about params.kelvin_origin with the factor
+ * |s*|^3 / |t*|, plus (include_killing) n_kill_walks walks from kappa(infinity)
+ * adding (4 pi / |t0*|) b(t0) b(t0)^T / n_kill_walks.
+ */
+int mcs_estimate_dtn_exterior(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                              const mcs_params* params, void* workspace, size_t workspace_bytes,
+                              const mcs_matrix* out, mcs_stats* host_stats, void* stream);
+
+/* ------------------------------------------------------------------------ */
+/* Test / benchmark hooks for the individual steps of SURVEY.md 8(a).         */
+/* ------------------------------------------------------------------------ */
+typedef struct {                 /* one termination record per walk, slot = sample*W + walk, */
+    int32_t tri_t;               /* then the killing walks.  tri_t < 0: no contribution      */
+    float   b1, b2;              /* barycentrics of t on vertices 1, 2 of tri_t (b0 = 1-b1-b2) */
+    float   weight;              /* full scalar multiplying d d^T                             */
+} mcs_record;
+
+/* A2: tangent balls.  balls [n_s][8] = (c.x, c.y, c.z, r, pole.x, pole.y, pole.z, |s*|) in
+ * the walk domain's coordinates (exterior: Kelvin coordinates about the origin). */
+int mcs_tangent_balls(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_params* params,
+                      int exterior, float* balls, void* stream);
+
+/* Workspace (bytes) of mcs_run_walks and of mcs_accumulate. */
+size_t mcs_walk_workspace_bytes(const mcs_samples* samples);
+size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_basis* basis, int64_t n_records);
+
+/* A2-A6: run every walk and write records [n_s*W (+ n_kill_walks)] and, if non-NULL,
+ * steps [same length] (jumps taken; -1 truncated; -2 sample discarded). */
+int mcs_run_walks(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_params* params,
+                  int exterior, void* workspace, size_t workspace_bytes,
+                  mcs_record* records, int32_t* steps, mcs_stats* host_stats, void* stream);
+
+/* A7: deterministic accumulation of records into the matrix (sort by key +
+ * segmented sum; no float atomics). */
+int mcs_accumulate(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                   const mcs_params* params, const mcs_record* records, int64_t n_records,
+                   void* workspace, size_t workspace_bytes, const mcs_matrix* out,
+                   mcs_stats* host_stats, void* stream);
+
+/* Philox4x32-10 words for counters [n][4] and one key [2] (host): out [n][4].
+ * Lets the tests pin the device generator against the known answers. */
+int mcs_philox4x32_10(const uint32_t* counters, int64_t n, const uint32_t* key /* host */,
+                      uint32_t* out, void* stream);
+
+/* Stable LSD radix sort of (key, value) pairs, test hook for the sort used by
+ * the LBVH build and by the accumulation.  keys/vals are sorted in place;
+ * workspace must hold mcs_sort_workspace_bytes(n) bytes. */
+size_t mcs_sort_workspace_bytes(int64_t n);
+int mcs_sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int32_t key_bits,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
+const char* mcs_error_string(int code);
+const char* mcs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCDTN_H */

@@ -1,0 +1,12 @@
+"""B200-native (sm_100a, hand-written CUDA) Monte Carlo Dirichlet-to-Neumann
+estimator: the walk-on-spheres hot path of arxiv 2606.05581, behind
+the C ABI of include/mcdtn.h.  This package is only the thin binding; it never
+imports `oracle/` and has no CPU fallback."""
+from .api import (Bvh, BvhInfo, McsError, Params, Samples, Stats, accumulate, build_bvh, closest_point,
+                  closest_point_bruteforce, estimate_dtn_exterior, estimate_dtn_interior, lib, num_records,
+                  philox4x32_10, run_walks, sort_pairs_u64, tangent_balls, version, workspace_bytes)
+
+__all__ = ["Bvh", "BvhInfo", "McsError", "Params", "Samples", "Stats", "accumulate", "build_bvh",
+           "closest_point", "closest_point_bruteforce", "estimate_dtn_exterior", "estimate_dtn_interior", "lib",
+           "num_records", "philox4x32_10", "run_walks", "sort_pairs_u64", "tangent_balls", "version",
+           "workspace_bytes"]

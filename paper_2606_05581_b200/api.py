@@ -1,0 +1,352 @@
+"""Thin ctypes binding of include/mcdtn.h: argument marshalling only.
+
+Every step of the path runs in the CUDA library (libmcdtn.so, built in-tree by
+paper_2606_05581_b200/build.py).  PyTorch supplies device memory and streams,
+nothing else.  There is no CPU fallback: loading fails loudly if the library is
+missing, and every call raises McsError on a non-zero return code.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmcdtn.so")
+
+MCS_OK, MCS_EINVAL, MCS_EDEGENERATE, MCS_ENOMEM, MCS_ECUDA = 0, -1, -2, -3, -4
+
+
+class McsError(RuntimeError):
+    def __init__(self, code: int, where: str, msg: str):
+        super().__init__(f"{where}: {msg} (code {code})")
+        self.code = code
+
+
+class _BuildOpts(C.Structure):
+    _fields_ = [("reserved", C.c_int32)]
+
+
+class BvhInfo(C.Structure):
+    _fields_ = [("V", C.c_int64), ("F", C.c_int64), ("n_nodes", C.c_int64), ("max_depth", C.c_int32),
+                ("n_degenerate", C.c_int32), ("aabb_lo", C.c_float * 3), ("aabb_hi", C.c_float * 3),
+                ("area", C.c_double), ("device_bytes", C.c_size_t)]
+
+
+class _Samples(C.Structure):
+    _fields_ = [("tri", C.c_void_p), ("bary", C.c_void_p), ("weight", C.c_void_p), ("normal", C.c_void_p),
+                ("n_s", C.c_int64)]
+
+
+class _Basis(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("walks_per_sample", C.c_int32), ("max_steps", C.c_int32),
+                ("eps", C.c_float), ("cap_half_angle_deg", C.c_float), ("rmax_scale", C.c_float),
+                ("rmax_override", C.c_float), ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
+                ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
+                ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32)]
+
+
+class _Matrix(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64), ("dense", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_samples", C.c_int64), ("n_discarded", C.c_int64), ("n_walks", C.c_int64),
+                ("n_truncated", C.c_int64), ("n_steps", C.c_int64), ("n_queries", C.c_int64),
+                ("n_nodes_visited", C.c_int64), ("n_tris_tested", C.c_int64), ("n_entries", C.c_int64),
+                ("n_unique", C.c_int64), ("workspace_needed", C.c_int64), ("cuda_error", C.c_int32),
+                ("pad_", C.c_int32)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad_"}
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_05581_b200.build` "
+                              "(there is no CPU or PyTorch fallback for this path)")
+        L = C.CDLL(LIB_PATH)
+        L.mcs_error_string.restype = C.c_char_p
+        L.mcs_version.restype = C.c_char_p
+        for name in ("mcs_workspace_bytes", "mcs_walk_workspace_bytes", "mcs_accumulate_workspace_bytes",
+                     "mcs_sort_workspace_bytes"):
+            getattr(L, name).restype = C.c_size_t
+        L.mcs_free_bvh.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, where: str):
+    if rc != MCS_OK:
+        raise McsError(rc, where, lib().mcs_error_string(rc).decode())
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _stream(device):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _dev(t, dtype, name):
+    if not isinstance(t, torch.Tensor):
+        t = torch.as_tensor(t)
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (this path has no CPU implementation)")
+    return t.to(dtype).contiguous()
+
+
+@dataclass
+class Params:
+    seed: int = 0
+    walks_per_sample: int = 1
+    max_steps: int = 4096
+    eps: float = 1e-3
+    cap_half_angle_deg: float = 2.5
+    rmax_scale: float = 1.0
+    rmax_override: float = 0.0
+    bisection_iters: int = 10
+    importance_sample: bool = True
+    antithetic: bool = False
+    include_killing: bool = False
+    n_kill_walks: int = 0
+    kelvin_origin: tuple = (0.0, 0.0, 0.0)
+
+    def c(self) -> _Params:
+        p = _Params(seed=self.seed, walks_per_sample=self.walks_per_sample, max_steps=self.max_steps,
+                    eps=self.eps, cap_half_angle_deg=self.cap_half_angle_deg, rmax_scale=self.rmax_scale,
+                    rmax_override=self.rmax_override, bisection_iters=self.bisection_iters,
+                    importance_sample=int(self.importance_sample), antithetic=int(self.antithetic),
+                    include_killing=int(self.include_killing), n_kill_walks=int(self.n_kill_walks),
+                    output_kind=0)
+        p.kelvin_origin[:] = [float(x) for x in self.kelvin_origin]
+        return p
+
+
+@dataclass
+class Samples:
+    """Boundary samples on the device."""
+    tri: torch.Tensor
+    bary: torch.Tensor
+    weight: torch.Tensor
+    normal: torch.Tensor | None = None
+    _keep: list = field(default_factory=list, repr=False)
+
+    @classmethod
+    def from_arrays(cls, tri, bary, weight, normal=None, device="cuda"):
+        tri = torch.as_tensor(tri).to(device=device, dtype=torch.int32).contiguous()
+        bary = torch.as_tensor(bary).to(device=device, dtype=torch.float32).contiguous()
+        weight = torch.as_tensor(weight).to(device=device, dtype=torch.float32).contiguous()
+        if normal is not None:
+            normal = torch.as_tensor(normal).to(device=device, dtype=torch.float32).contiguous()
+        return cls(tri, bary, weight, normal)
+
+    @property
+    def n_s(self):
+        return int(self.tri.shape[0])
+
+    def c(self) -> _Samples:
+        assert self.bary.shape == (self.n_s, 3) and self.weight.shape == (self.n_s,)
+        return _Samples(tri=self.tri.data_ptr(), bary=self.bary.data_ptr(), weight=self.weight.data_ptr(),
+                        normal=self.normal.data_ptr() if self.normal is not None else None, n_s=self.n_s)
+
+
+class Bvh:
+    """Opaque LBVH handle (mcs_build_bvh / mcs_free_bvh)."""
+
+    def __init__(self, verts, faces):
+        self.verts = _dev(verts, torch.float32, "verts")
+        self.faces = _dev(faces, torch.int32, "faces")
+        if self.verts.ndim != 2 or self.verts.shape[1] != 3 or self.faces.ndim != 2 or self.faces.shape[1] != 3:
+            raise ValueError("verts must be [V,3], faces [F,3]")
+        self.device = self.verts.device
+        self._h = C.c_void_p(0)
+        with torch.cuda.device(self.device):
+            rc = lib().mcs_build_bvh(_ptr(self.verts), C.c_int64(self.verts.shape[0]), _ptr(self.faces),
+                                     C.c_int64(self.faces.shape[0]), None, _stream(self.device), C.byref(self._h))
+        _check(rc, "mcs_build_bvh")
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            lib().mcs_free_bvh(h)
+            self._h = C.c_void_p(0)
+
+    @property
+    def handle(self):
+        return self._h
+
+    @property
+    def V(self):
+        return int(self.verts.shape[0])
+
+    @property
+    def F(self):
+        return int(self.faces.shape[0])
+
+    def info(self) -> BvhInfo:
+        o = BvhInfo()
+        _check(lib().mcs_bvh_info(self._h, C.byref(o)), "mcs_bvh_info")
+        return o
+
+    def dump(self):
+        info = self.info()
+        nodes = torch.empty((info.n_nodes, 16), dtype=torch.int32, device=self.device)
+        leaf_tri = torch.empty(info.F, dtype=torch.int32, device=self.device)
+        morton = torch.empty(info.F, dtype=torch.int64, device=self.device)
+        with torch.cuda.device(self.device):
+            _check(lib().mcs_bvh_dump(self._h, _ptr(nodes), _ptr(leaf_tri), _ptr(morton), _stream(self.device)),
+                   "mcs_bvh_dump")
+        return nodes, leaf_tri, morton
+
+
+def build_bvh(verts, faces) -> Bvh:
+    return Bvh(verts, faces)
+
+
+def _closest(fn, name, bvh: Bvh, q):
+    q = _dev(q, torch.float32, "q")
+    n = q.shape[0]
+    dist = torch.empty(n, dtype=torch.float32, device=bvh.device)
+    tri = torch.empty(n, dtype=torch.int32, device=bvh.device)
+    bary = torch.empty((n, 3), dtype=torch.float32, device=bvh.device)
+    with torch.cuda.device(bvh.device):
+        _check(fn(bvh.handle, _ptr(q), C.c_int64(n), _ptr(dist), _ptr(tri), _ptr(bary), _stream(bvh.device)), name)
+    return dist, tri, bary
+
+
+def closest_point(bvh: Bvh, q):
+    return _closest(lib().mcs_closest_point, "mcs_closest_point", bvh, q)
+
+
+def closest_point_bruteforce(bvh: Bvh, q):
+    return _closest(lib().mcs_closest_point_bruteforce, "mcs_closest_point_bruteforce", bvh, q)
+
+
+def _basis(bvh: Bvh) -> _Basis:
+    return _Basis(kind=0, K=bvh.V)
+
+
+def workspace_bytes(bvh: Bvh, samples: Samples, params: Params, exterior: bool) -> int:
+    cs, cb, cp = samples.c(), _basis(bvh), params.c()
+    return int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
+
+
+def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace):
+    cs, cb, cp = samples.c(), _basis(bvh), params.c()
+    K = bvh.V
+    if out is None:
+        out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
+    need = workspace_bytes(bvh, samples, params, exterior)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+    m = _Matrix(kind=0, K=K, dense=out.data_ptr())
+    st = Stats() if want_stats else None
+    with torch.cuda.device(bvh.device):
+        rc = fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(workspace), C.c_size_t(workspace.numel()),
+                C.byref(m), C.byref(st) if st is not None else None, _stream(bvh.device))
+    _check(rc, name)
+    return (out, st) if want_stats else out
+
+
+def estimate_dtn_interior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None):
+    """Interior DtN matrix, Alg. 2: dense [K,K] fp32 on the device."""
+    return _estimate(lib().mcs_estimate_dtn_interior, "mcs_estimate_dtn_interior", bvh, samples, params, False,
+                     want_stats, out, workspace)
+
+
+def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None):
+    """Exterior DtN matrix, Eq. 32."""
+    return _estimate(lib().mcs_estimate_dtn_exterior, "mcs_estimate_dtn_exterior", bvh, samples, params, True,
+                     want_stats, out, workspace)
+
+
+def tangent_balls(bvh: Bvh, samples: Samples, params: Params, exterior: bool):
+    cs, cp = samples.c(), params.c()
+    balls = torch.empty((samples.n_s, 8), dtype=torch.float32, device=bvh.device)
+    with torch.cuda.device(bvh.device):
+        _check(lib().mcs_tangent_balls(bvh.handle, C.byref(cs), C.byref(cp), C.c_int(int(exterior)), _ptr(balls),
+                                       _stream(bvh.device)), "mcs_tangent_balls")
+    return balls
+
+
+def num_records(samples: Samples, params: Params, exterior: bool) -> int:
+    n = samples.n_s * params.walks_per_sample
+    if exterior and params.include_killing:
+        n += params.n_kill_walks
+    return n
+
+
+def run_walks(bvh: Bvh, samples: Samples, params: Params, exterior: bool, want_stats=False):
+    """Records [n,4] fp32 (column 0 holds tri_t as int32 bits) and steps [n] int32."""
+    cs, cp = samples.c(), params.c()
+    n = num_records(samples, params, exterior)
+    rec = torch.empty((n, 4), dtype=torch.float32, device=bvh.device)
+    steps = torch.empty(n, dtype=torch.int32, device=bvh.device)
+    need = int(lib().mcs_walk_workspace_bytes(C.byref(cs)))
+    ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+    st = Stats() if want_stats else None
+    with torch.cuda.device(bvh.device):
+        rc = lib().mcs_run_walks(bvh.handle, C.byref(cs), C.byref(cp), C.c_int(int(exterior)), _ptr(ws),
+                                 C.c_size_t(need), _ptr(rec), _ptr(steps),
+                                 C.byref(st) if st is not None else None, _stream(bvh.device))
+    _check(rc, "mcs_run_walks")
+    return (rec, steps, st) if want_stats else (rec, steps)
+
+
+def accumulate(bvh: Bvh, samples: Samples, params: Params, records, want_stats=False):
+    cs, cb, cp = samples.c(), _basis(bvh), params.c()
+    records = _dev(records, torch.float32, "records")
+    n = records.shape[0]
+    K = bvh.V
+    out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
+    need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cb), C.c_int64(n)))
+    ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+    m = _Matrix(kind=0, K=K, dense=out.data_ptr())
+    st = Stats() if want_stats else None
+    with torch.cuda.device(bvh.device):
+        rc = lib().mcs_accumulate(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(records), C.c_int64(n),
+                                  _ptr(ws), C.c_size_t(need), C.byref(m),
+                                  C.byref(st) if st is not None else None, _stream(bvh.device))
+    _check(rc, "mcs_accumulate")
+    return (out, st) if want_stats else out
+
+
+def philox4x32_10(counters, key):
+    counters = _dev(counters, torch.int32, "counters")
+    n = counters.shape[0]
+    out = torch.empty((n, 4), dtype=torch.int32, device=counters.device)
+    k = (C.c_uint32 * 2)(int(key[0]) & 0xFFFFFFFF, int(key[1]) & 0xFFFFFFFF)
+    with torch.cuda.device(counters.device):
+        _check(lib().mcs_philox4x32_10(_ptr(counters), C.c_int64(n), k, _ptr(out), _stream(counters.device)),
+               "mcs_philox4x32_10")
+    return out
+
+
+def sort_pairs_u64(keys, vals, key_bits=64):
+    """In-place stable radix sort of int64 keys (as unsigned) with int32 payloads."""
+    assert keys.is_cuda and vals.is_cuda and keys.dtype == torch.int64 and vals.dtype == torch.int32
+    n = keys.numel()
+    need = int(lib().mcs_sort_workspace_bytes(C.c_int64(n)))
+    ws = torch.empty(need, dtype=torch.uint8, device=keys.device)
+    with torch.cuda.device(keys.device):
+        _check(lib().mcs_sort_pairs_u64(_ptr(keys), _ptr(vals), C.c_int64(n), C.c_int32(key_bits), _ptr(ws),
+                                        C.c_size_t(need), _stream(keys.device)), "mcs_sort_pairs_u64")
+    return keys, vals
+
+
+def version() -> str:
+    return lib().mcs_version().decode()

@@ -1,0 +1,346 @@
+// bvh.cu -- GPU LBVH build over the triangle soup (SURVEY.md 8(a) A0 + A1).
+//
+// The paper's implementation takes its BVH from a library; here
+// it is built on the device: vertex AABB -> 63-bit Morton keys of the face
+// centroids -> stable radix sort -> binary radix tree (Karras 2012, restated;
+// equal keys are split by their sorted position) -> bottom-up refit with one
+// arrival counter per internal node -> 64-byte two-child-box nodes.
+// Nothing here assumes a manifold, consistently oriented, non-degenerate or
+// connected mesh: every face is a leaf (all triangles absorb).
+#include "common.cuh"
+
+#include <new>
+#include <string.h>
+
+namespace {
+
+constexpr int BT = 256;
+
+__device__ __forceinline__ int float_to_ordered(float f)
+{
+    int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7FFFFFFF;
+}
+__device__ __forceinline__ float ordered_to_float(int i)
+{
+    return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF);
+}
+
+struct BuildScratch {
+    int      flags;          // bit 0: face index out of range; bit 1: non-finite vertex
+    int      n_degenerate;
+    int      max_depth;
+    int      pad;
+    int      lo[3], hi[3];   // ordered-int AABB
+    double   area;
+};
+
+// Pass 1: validate faces, AABB of the referenced vertices, per-block area partials.
+__global__ void __launch_bounds__(BT)
+face_bounds_kernel(const float* __restrict__ verts, int64_t V, const int32_t* __restrict__ faces, int64_t F,
+                   BuildScratch* __restrict__ sc, double* __restrict__ area_partials)
+{
+    __shared__ double s_area[BT];
+    __shared__ int s_lo[3], s_hi[3];
+    if (threadIdx.x < 3) { s_lo[threadIdx.x] = 0x7FFFFFFF; s_hi[threadIdx.x] = (int)0x80000000; }
+    __syncthreads();
+    const int64_t f = (int64_t)blockIdx.x * BT + threadIdx.x;
+    double area = 0.0;
+    if (f < F) {
+        const int i0 = faces[3 * f], i1 = faces[3 * f + 1], i2 = faces[3 * f + 2];
+        if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= V || i1 >= V || i2 >= V) {
+            atomicOr(&sc->flags, 1);
+        } else {
+            float p[3][3];
+            const int idx[3] = { i0, i1, i2 };
+            bool finite = true;
+            for (int k = 0; k < 3; ++k)
+                for (int d = 0; d < 3; ++d) { p[k][d] = verts[3 * (int64_t)idx[k] + d]; finite = finite && isfinite(p[k][d]); }
+            if (!finite) {
+                atomicOr(&sc->flags, 2);
+            } else {
+                for (int d = 0; d < 3; ++d) {
+                    float lo = fminf(p[0][d], fminf(p[1][d], p[2][d]));
+                    float hi = fmaxf(p[0][d], fmaxf(p[1][d], p[2][d]));
+                    atomicMin(&s_lo[d], float_to_ordered(lo));
+                    atomicMax(&s_hi[d], float_to_ordered(hi));
+                }
+                const double ax = (double)p[1][0] - p[0][0], ay = (double)p[1][1] - p[0][1], az = (double)p[1][2] - p[0][2];
+                const double bx = (double)p[2][0] - p[0][0], by = (double)p[2][1] - p[0][1], bz = (double)p[2][2] - p[0][2];
+                const double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;
+                area = 0.5 * sqrt(cx * cx + cy * cy + cz * cz);
+                if (!(area > 0.0)) atomicAdd(&sc->n_degenerate, 1);
+            }
+        }
+    }
+    s_area[threadIdx.x] = area;
+    __syncthreads();
+    for (int s = BT / 2; s > 0; s >>= 1) {          // fixed-shape tree: deterministic
+        if (threadIdx.x < s) s_area[threadIdx.x] += s_area[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) area_partials[blockIdx.x] = s_area[0];
+    if (threadIdx.x < 3) {
+        atomicMin(&sc->lo[threadIdx.x], s_lo[threadIdx.x]);
+        atomicMax(&sc->hi[threadIdx.x], s_hi[threadIdx.x]);
+    }
+}
+
+__global__ void area_total_kernel(const double* __restrict__ partials, int n, BuildScratch* sc)
+{
+    double t = 0.0;
+    for (int i = 0; i < n; ++i) t += partials[i];   // one thread, fixed order
+    sc->area = t;
+}
+
+__device__ __forceinline__ uint64_t spread21(uint64_t x)
+{
+    x &= 0x1FFFFFull;
+    x = (x | x << 32) & 0x1F00000000FFFFull;
+    x = (x | x << 16) & 0x1F0000FF0000FFull;
+    x = (x | x << 8)  & 0x100F00F00F00F00Full;
+    x = (x | x << 4)  & 0x10C30C30C30C30C3ull;
+    x = (x | x << 2)  & 0x1249249249249249ull;
+    return x;
+}
+
+__global__ void __launch_bounds__(BT)
+morton_kernel(const float* __restrict__ verts, const int32_t* __restrict__ faces, int64_t F,
+              const BuildScratch* __restrict__ sc, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    const int64_t f = (int64_t)blockIdx.x * BT + threadIdx.x;
+    if (f >= F) return;
+    uint64_t key = 0;
+    for (int d = 0; d < 3; ++d) {
+        const float lo = ordered_to_float(sc->lo[d]), hi = ordered_to_float(sc->hi[d]);
+        const float c = (verts[3 * (int64_t)faces[3 * f] + d] + verts[3 * (int64_t)faces[3 * f + 1] + d] +
+                         verts[3 * (int64_t)faces[3 * f + 2] + d]) * (1.0f / 3.0f);
+        const float ext = hi - lo;
+        float t = ext > 0.0f ? (c - lo) / ext : 0.0f;
+        t = fminf(fmaxf(t, 0.0f), 1.0f);
+        uint64_t q = (uint64_t)fminf(t * 2097152.0f, 2097151.0f);
+        key |= spread21(q) << (2 - d);              // x is the most significant axis
+    }
+    keys[f] = key;
+    vals[f] = (uint32_t)f;
+}
+
+// Length of the common prefix of the (key, position) pairs at sorted positions i, j.
+__device__ __forceinline__ int delta(const uint64_t* __restrict__ keys, int64_t F, int64_t i, int64_t j)
+{
+    if (j < 0 || j >= F) return -1;
+    const uint64_t ki = keys[i], kj = keys[j];
+    if (ki == kj) return 64 + __clz((unsigned)(i ^ j));
+    return __clzll((long long)(ki ^ kj));
+}
+
+// Binary radix tree: internal node i covers a range of sorted leaves that has i at one end.
+// node words: [0..5] box of child 0, [6..11] box of child 1, [12] child0, [13] child1, [14] parent.
+__global__ void __launch_bounds__(BT)
+radix_tree_kernel(const uint64_t* __restrict__ keys, int64_t F, int32_t* __restrict__ node_words,
+                  int32_t* __restrict__ leaf_parent)
+{
+    const int64_t i = (int64_t)blockIdx.x * BT + threadIdx.x;
+    if (i >= F - 1) return;
+    const int d = (delta(keys, F, i, i + 1) - delta(keys, F, i, i - 1)) >= 0 ? 1 : -1;
+    const int dmin = delta(keys, F, i, i - d);
+    int64_t lmax = 2;
+    while (delta(keys, F, i, i + lmax * d) > dmin) lmax *= 2;
+    int64_t l = 0;
+    for (int64_t t = lmax / 2; t >= 1; t /= 2)
+        if (delta(keys, F, i, i + (l + t) * d) > dmin) l += t;
+    const int64_t j = i + l * d;
+    const int dnode = delta(keys, F, i, j);
+    int64_t s = 0, t = l;
+    do {
+        t = (t + 1) / 2;
+        if (delta(keys, F, i, i + (s + t) * d) > dnode) s += t;
+    } while (t > 1);
+    const int64_t gamma = i + s * d + (d < 0 ? -1 : 0);
+    const int64_t lo = i < j ? i : j, hi = i < j ? j : i;
+    int32_t* w = node_words + 16 * i;
+    if (lo == gamma) { w[12] = ~(int32_t)gamma; leaf_parent[gamma] = (int32_t)i; }
+    else             { w[12] = (int32_t)gamma;  node_words[16 * gamma + 14] = (int32_t)i; }
+    if (hi == gamma + 1) { w[13] = ~(int32_t)(gamma + 1); leaf_parent[gamma + 1] = (int32_t)i; }
+    else                 { w[13] = (int32_t)(gamma + 1);  node_words[16 * (gamma + 1) + 14] = (int32_t)i; }
+    if (i == 0) w[14] = -1;
+    w[15] = 0;
+}
+
+// Pack sorted triangles and refit boxes bottom-up.  The second thread to reach
+// a node owns it (arrival counter), reads both child boxes and carries their
+// union to the parent.
+__global__ void __launch_bounds__(BT)
+pack_refit_kernel(const float* __restrict__ verts, const int32_t* __restrict__ faces, int64_t F,
+                  const uint32_t* __restrict__ sorted_face, const int32_t* __restrict__ leaf_parent,
+                  int32_t* node_words, int* __restrict__ arrivals, PackedTri* __restrict__ tris,
+                  int32_t* __restrict__ leaf_tri, int32_t* __restrict__ face_slot, BuildScratch* sc)
+{
+    const int64_t k = (int64_t)blockIdx.x * BT + threadIdx.x;
+    if (k >= F) return;
+    const int32_t f = (int32_t)sorted_face[k];
+    leaf_tri[k] = f;
+    face_slot[f] = (int32_t)k;
+    float p[3][3];
+    for (int v = 0; v < 3; ++v)
+        for (int d = 0; d < 3; ++d) p[v][d] = verts[3 * (int64_t)faces[3 * (int64_t)f + v] + d];
+    PackedTri t;
+    t.t0 = make_float4(p[0][0], p[0][1], p[0][2], __int_as_float(f));
+    t.t1 = make_float4(p[1][0], p[1][1], p[1][2], 0.0f);
+    t.t2 = make_float4(p[2][0], p[2][1], p[2][2], 0.0f);
+    tris[k] = t;
+    float box[6];
+    for (int d = 0; d < 3; ++d) {
+        box[d] = fminf(p[0][d], fminf(p[1][d], p[2][d]));
+        box[3 + d] = fmaxf(p[0][d], fmaxf(p[1][d], p[2][d]));
+    }
+    if (F == 1) {                                   // single face: node 0 holds the leaf twice
+        float* w = reinterpret_cast<float*>(node_words);
+        for (int c = 0; c < 2; ++c) for (int q = 0; q < 6; ++q) w[6 * c + q] = box[q];
+        node_words[12] = ~0; node_words[13] = ~0; node_words[14] = -1; node_words[15] = 0;
+        sc->max_depth = 1;
+        return;
+    }
+    int32_t child = ~(int32_t)k;
+    int32_t node = leaf_parent[k];
+    int depth = 1;
+    for (;;) {
+        volatile float* w = reinterpret_cast<volatile float*>(node_words + 16 * (int64_t)node);
+        volatile int32_t* wi = reinterpret_cast<volatile int32_t*>(node_words + 16 * (int64_t)node);
+        const int side = (wi[12] == child) ? 0 : 1;
+        for (int q = 0; q < 6; ++q) w[6 * side + q] = box[q];
+        __threadfence();
+        const int old = atomicAdd(&arrivals[node], 1);
+        if (old == 0) return;                       // first arrival: the sibling will carry on
+        __threadfence();
+        const int other = 1 - side;
+        for (int d = 0; d < 3; ++d) {
+            box[d] = fminf(box[d], w[6 * other + d]);
+            box[3 + d] = fmaxf(box[3 + d], w[6 * other + 3 + d]);
+        }
+        const int32_t parent = wi[14];
+        if (parent < 0) return;                     // root done
+        child = node;
+        node = parent;
+        ++depth;
+    }
+}
+
+__global__ void __launch_bounds__(BT)
+depth_kernel(const int32_t* __restrict__ node_words, const int32_t* __restrict__ leaf_parent, int64_t F, BuildScratch* sc)
+{
+    const int64_t k = (int64_t)blockIdx.x * BT + threadIdx.x;
+    int depth = 0;
+    if (k < F && F > 1) {
+        depth = 1;
+        int32_t node = leaf_parent[k];
+        while (node_words[16 * (int64_t)node + 14] >= 0) { node = node_words[16 * (int64_t)node + 14]; ++depth; }
+    }
+    for (int o = 16; o > 0; o >>= 1) depth = max(depth, __shfl_xor_sync(0xFFFFFFFFu, depth, o));
+    if ((threadIdx.x & 31) == 0 && depth > 0) atomicMax(&sc->max_depth, depth);
+}
+
+}  // namespace
+
+extern "C" void mcs_free_bvh(mcs_bvh* b)
+{
+    if (!b) return;
+    cudaFree(b->verts); cudaFree(b->faces); cudaFree(b->nodes); cudaFree(b->tris);
+    cudaFree(b->leaf_tri); cudaFree(b->face_slot); cudaFree(b->morton);
+    delete b;
+}
+
+extern "C" int mcs_build_bvh(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                             const mcs_build_opts* opts, void* stream, mcs_bvh** out)
+{
+    if (!out) return MCS_EINVAL;
+    *out = nullptr;
+    if (!verts || !faces || V < 1 || F < 1 || V >= (int64_t)1 << 31 || F >= (int64_t)1 << 30) return MCS_EINVAL;
+    if (opts && opts->reserved != 0) return MCS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    mcs_bvh* b = new (std::nothrow) mcs_bvh();
+    if (!b) return MCS_ENOMEM;
+    b->V = V; b->F = F; b->n_nodes = F > 1 ? F - 1 : 1; b->root = 0;
+    cudaGetDevice(&b->device);
+
+    const size_t nb_verts = (size_t)V * 3 * sizeof(float), nb_faces = (size_t)F * 3 * sizeof(int32_t);
+    const size_t nb_nodes = (size_t)b->n_nodes * sizeof(BvhNode), nb_tris = (size_t)F * sizeof(PackedTri);
+    BuildScratch* sc = nullptr; double* partials = nullptr; uint32_t* vals = nullptr;
+    int32_t* leaf_parent = nullptr; int* arrivals = nullptr; void* sort_ws = nullptr;
+    const int nblk = (int)ceil_div64(F, BT);
+    const size_t sort_bytes = sort_workspace_bytes(F, 8);
+    int rc = MCS_OK;
+    cudaError_t e = cudaSuccess;
+#define ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
+    ALLOC(b->verts, nb_verts); ALLOC(b->faces, nb_faces); ALLOC(b->nodes, nb_nodes); ALLOC(b->tris, nb_tris);
+    ALLOC(b->leaf_tri, (size_t)F * 4); ALLOC(b->face_slot, (size_t)F * 4); ALLOC(b->morton, (size_t)F * 8);
+    ALLOC(sc, sizeof(BuildScratch)); ALLOC(partials, (size_t)nblk * 8); ALLOC(vals, (size_t)F * 4);
+    ALLOC(leaf_parent, (size_t)F * 4); ALLOC(arrivals, (size_t)b->n_nodes * 4); ALLOC(sort_ws, sort_bytes);
+#undef ALLOC
+    BuildScratch h;
+    if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MCS_ENOMEM : MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+    b->device_bytes = nb_verts + nb_faces + nb_nodes + nb_tris + (size_t)F * 16;
+
+    cudaMemcpyAsync(b->verts, verts, nb_verts, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(b->faces, faces, nb_faces, cudaMemcpyDeviceToDevice, st);
+    memset(&h, 0, sizeof h);
+    for (int d = 0; d < 3; ++d) { h.lo[d] = 0x7FFFFFFF; h.hi[d] = (int)0x80000000; }
+    cudaMemcpyAsync(sc, &h, sizeof h, cudaMemcpyHostToDevice, st);
+    cudaMemsetAsync(arrivals, 0, (size_t)b->n_nodes * 4, st);
+    cudaMemsetAsync(b->nodes, 0, nb_nodes, st);
+
+    face_bounds_kernel<<<nblk, BT, 0, st>>>(b->verts, V, b->faces, F, sc, partials);
+    area_total_kernel<<<1, 1, 0, st>>>(partials, nblk, sc);
+    e = cudaMemcpyAsync(&h, sc, sizeof h, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { rc = MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+    if (h.flags & 1) { rc = MCS_EINVAL; goto done; }
+    if ((h.flags & 2) || !(h.area > 0.0)) { rc = MCS_EDEGENERATE; goto done; }
+
+    morton_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, sc, b->morton, vals);
+    rc = sort_pairs_u64(b->morton, vals, F, 63, sort_ws, sort_bytes, st);
+    if (rc != MCS_OK) goto done;
+    if (F > 1)
+        radix_tree_kernel<<<(int)ceil_div64(F - 1, BT), BT, 0, st>>>(b->morton, F, (int32_t*)b->nodes, leaf_parent);
+    pack_refit_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, vals, leaf_parent, (int32_t*)b->nodes,
+                                           arrivals, b->tris, b->leaf_tri, b->face_slot, sc);
+    depth_kernel<<<nblk, BT, 0, st>>>((const int32_t*)b->nodes, leaf_parent, F, sc);
+    e = cudaMemcpyAsync(&h, sc, sizeof h, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { rc = MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+    b->max_depth = h.max_depth;
+    b->n_degenerate = h.n_degenerate;
+    b->area = h.area;
+    for (int d = 0; d < 3; ++d) {
+        int lo = h.lo[d], hi = h.hi[d];
+        lo = lo >= 0 ? lo : lo ^ 0x7FFFFFFF; hi = hi >= 0 ? hi : hi ^ 0x7FFFFFFF;
+        memcpy(&b->aabb_lo[d], &lo, 4); memcpy(&b->aabb_hi[d], &hi, 4);
+    }
+done:
+    cudaFree(sc); cudaFree(partials); cudaFree(vals); cudaFree(leaf_parent); cudaFree(arrivals); cudaFree(sort_ws);
+    if (rc != MCS_OK) { mcs_free_bvh(b); return rc; }
+    *out = b;
+    return MCS_OK;
+}
+
+extern "C" int mcs_bvh_info(const mcs_bvh* b, mcs_bvh_info_t* o)
+{
+    if (!b || !o) return MCS_EINVAL;
+    o->V = b->V; o->F = b->F; o->n_nodes = b->n_nodes; o->max_depth = b->max_depth;
+    o->n_degenerate = b->n_degenerate;
+    for (int d = 0; d < 3; ++d) { o->aabb_lo[d] = b->aabb_lo[d]; o->aabb_hi[d] = b->aabb_hi[d]; }
+    o->area = b->area; o->device_bytes = b->device_bytes;
+    return MCS_OK;
+}
+
+extern "C" int mcs_bvh_dump(const mcs_bvh* b, uint32_t* nodes, int32_t* leaf_tri, uint64_t* morton, void* stream)
+{
+    if (!b) return MCS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (nodes) MCS_CUDA_TRY(cudaMemcpyAsync(nodes, b->nodes, (size_t)b->n_nodes * sizeof(BvhNode), cudaMemcpyDeviceToDevice, st));
+    if (leaf_tri) MCS_CUDA_TRY(cudaMemcpyAsync(leaf_tri, b->leaf_tri, (size_t)b->F * 4, cudaMemcpyDeviceToDevice, st));
+    if (morton) MCS_CUDA_TRY(cudaMemcpyAsync(morton, b->morton, (size_t)b->F * 8, cudaMemcpyDeviceToDevice, st));
+    MCS_CUDA_TRY(cudaStreamSynchronize(st));
+    return MCS_OK;
+}

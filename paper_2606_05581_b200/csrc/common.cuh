@@ -1,0 +1,77 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a only).
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/mcdtn.h"
+
+#define MCS_CUDA_TRY(expr)                                     \
+    do {                                                       \
+        cudaError_t e__ = (expr);                              \
+        if (e__ != cudaSuccess) { mcs_set_last_cuda_error((int)e__); return MCS_ECUDA; } \
+    } while (0)
+
+void mcs_set_last_cuda_error(int e);
+int  mcs_get_last_cuda_error();
+
+static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------
+// Packed geometry owned by the handle.
+// ---------------------------------------------------------------------------
+// One internal node = 64 bytes = 4 x 16-byte loads:
+//   w0 = (lo0.x, lo0.y, lo0.z, hi0.x)
+//   w1 = (hi0.y, hi0.z, lo1.x, lo1.y)
+//   w2 = (lo1.z, hi1.x, hi1.y, hi1.z)
+//   w3 = (child0, child1, parent, unused) as int32
+// child >= 0: internal node index; child < 0: leaf, sorted triangle k = ~child.
+struct __align__(16) BvhNode {
+    float4 w0, w1, w2;
+    int4   w3;
+};
+
+// One packed triangle = 48 bytes = 3 x 16-byte loads, in Morton order:
+//   t0 = (v0.x, v0.y, v0.z, original face index as int bits)
+//   t1 = (v1.x, v1.y, v1.z, 0)   t2 = (v2.x, v2.y, v2.z, 0)
+struct __align__(16) PackedTri {
+    float4 t0, t1, t2;
+};
+
+struct mcs_bvh {
+    int64_t V, F, n_nodes;
+    float*     verts;      // [V][3] copy of the input
+    int32_t*   faces;      // [F][3] copy of the input
+    BvhNode*   nodes;      // [max(F-1,1)]
+    PackedTri* tris;       // [F] Morton order
+    int32_t*   leaf_tri;   // [F] original face index of sorted leaf k
+    int32_t*   face_slot;  // [F] sorted slot of original face f (inverse of leaf_tri)
+    uint64_t*  morton;     // [F] sorted keys
+    int32_t    root;       // index of the root node (0)
+    int32_t    max_depth;
+    int32_t    n_degenerate;
+    float      aabb_lo[3], aabb_hi[3];
+    double     area;
+    size_t     device_bytes;
+    int        device;
+};
+
+// ---------------------------------------------------------------------------
+// radix sort / scan (sort.cu)
+// ---------------------------------------------------------------------------
+size_t sort_workspace_bytes(int64_t n, int key_bytes);
+// Stable LSD radix sort, 8 bits per pass over bits [0, key_bits).  keys/vals are
+// sorted in place (the workspace holds the ping-pong copies).
+int sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int key_bits,
+                   void* ws, size_t ws_bytes, cudaStream_t st);
+int sort_pairs_u32(uint32_t* keys, uint32_t* vals, int64_t n, int key_bits,
+                   void* ws, size_t ws_bytes, cudaStream_t st);
+size_t scan_workspace_bytes(int64_t n);
+// Exclusive prefix sum of uint32 counts into uint64-safe? No: totals fit in
+// int64 on the host side; device array is uint32 (n_entries per chunk < 2^32).
+int exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, uint32_t* total_out /* device, may be NULL */,
+                       void* ws, size_t ws_bytes, cudaStream_t st);

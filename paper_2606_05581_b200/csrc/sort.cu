@@ -1,0 +1,235 @@
+// sort.cu -- stable LSD radix sort (8 bits per pass) and exclusive scan.
+//
+// Used by the LBVH build (Morton keys), the Z-order sort of
+// the boundary samples and the deterministic accumulation
+// (sort (row,col) keys, then segmented sum).  Hand-written:
+// no CUB/Thrust on the product path.
+//
+// One pass = histogram per tile -> exclusive scan of counts[digit][tile] ->
+// stable scatter.  Inside a tile a key's position is (warp, round, lane): warp w
+// owns 32*ITEMS consecutive keys and reads them 32 at a time, so loads are
+// coalesced and the stable rank of a key is
+//   (#same digit in earlier warps) + (#same digit in this warp, earlier rounds)
+//   + (#same digit in this round at lower lanes),
+// the last two from __match_any_sync and one shared counter per (warp, digit).
+#include "common.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 512;
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 8192 keys per block
+
+constexpr int SCAN_THREADS = 512;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;   // 4096 counts per block
+
+__device__ __forceinline__ unsigned lanemask_lt()
+{
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+template <typename K>
+__global__ void __launch_bounds__(SORT_THREADS)
+radix_hist_kernel(const K* __restrict__ keys, int64_t n, int shift, uint32_t* __restrict__ counts, int nblocks)
+{
+    __shared__ uint32_t hist[256];
+    if (threadIdx.x < 256) hist[threadIdx.x] = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t warp_base = (int64_t)blockIdx.x * SORT_TILE + (int64_t)warp * 32 * SORT_ITEMS;
+#pragma unroll 4
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        int64_t pos = warp_base + r * 32 + lane;
+        bool valid = pos < n;
+        unsigned d = valid ? (unsigned)((keys[pos] >> shift) & 0xFF) : 0x100u + lane;
+        unsigned m = __match_any_sync(0xFFFFFFFFu, d);
+        if (valid && (m & lanemask_lt()) == 0) atomicAdd(&hist[d], __popc(m));
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) counts[(size_t)threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
+}
+
+template <typename K>
+__global__ void __launch_bounds__(SORT_THREADS)
+radix_scatter_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin,
+                     K* __restrict__ kout, uint32_t* __restrict__ vout,
+                     int64_t n, int shift, const uint32_t* __restrict__ offsets, int nblocks)
+{
+    __shared__ uint32_t cnt[SORT_WARPS][256];
+    for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t warp_base = (int64_t)blockIdx.x * SORT_TILE + (int64_t)warp * 32 * SORT_ITEMS;
+    K key[SORT_ITEMS];
+    uint32_t rank[SORT_ITEMS];
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        int64_t pos = warp_base + r * 32 + lane;
+        bool valid = pos < n;
+        key[r] = valid ? kin[pos] : (K)0;
+        unsigned d = valid ? (unsigned)((key[r] >> shift) & 0xFF) : 0x100u + lane;
+        unsigned m = __match_any_sync(0xFFFFFFFFu, d);
+        int leader = __ffs(m) - 1;
+        uint32_t old = 0;
+        if (valid && lane == leader) { old = cnt[warp][d]; cnt[warp][d] = old + __popc(m); }
+        old = __shfl_sync(0xFFFFFFFFu, old, leader);
+        rank[r] = old + __popc(m & lanemask_lt());
+        __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) {
+        uint32_t run = offsets[(size_t)threadIdx.x * nblocks + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) { uint32_t c = cnt[w][threadIdx.x]; cnt[w][threadIdx.x] = run; run += c; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        int64_t pos = warp_base + r * 32 + lane;
+        if (pos < n) {
+            unsigned d = (unsigned)((key[r] >> shift) & 0xFF);
+            uint32_t dst = cnt[warp][d] + rank[r];
+            kout[dst] = key[r];
+            vout[dst] = vin[pos];
+        }
+    }
+}
+
+// ------------------------------ scan ---------------------------------------
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
+{
+    __shared__ uint32_t warp_sums[SCAN_THREADS / 32];
+    __shared__ uint32_t block_total;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) warp_sums[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t s = lane < SCAN_THREADS / 32 ? warp_sums[lane] : 0, si = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, si, o); if (lane >= o) si += t; }
+        if (lane < SCAN_THREADS / 32) warp_sums[lane] = si - s;
+        if (lane == 31) block_total = si;
+    }
+    __syncthreads();
+    *total = block_total;
+    uint32_t r = warp_sums[warp] + inc - v;
+    __syncthreads();
+    return r;
+}
+
+// mode 0: write the tile total to sums[blockIdx]; mode 1: write the scanned tile,
+// offset by sums[blockIdx] (already exclusive-scanned) when sums != NULL.
+__global__ void __launch_bounds__(SCAN_THREADS)
+scan_tile_kernel(const uint32_t* in, uint32_t* out, int64_t n,   // in may alias out
+                 uint32_t* sums, int mode, uint32_t* total_out)
+{
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { v[i] = (base + i < n) ? in[base + i] : 0u; s += v[i]; }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(s, &total);
+    if (mode == 0) {
+        if (threadIdx.x == 0) sums[blockIdx.x] = total;
+        return;
+    }
+    uint32_t off = sums ? sums[blockIdx.x] : 0u;
+    uint32_t run = ex + off;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { if (base + i < n) out[base + i] = run; run += v[i]; }
+    if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_THREADS - 1) *total_out = run;
+}
+
+template <typename K>
+int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (n < 0 || key_bits < 0 || key_bits > (int)sizeof(K) * 8) return MCS_EINVAL;
+    if (n <= 1 || key_bits == 0) return MCS_OK;
+    if (n >= ((int64_t)1 << 32)) return MCS_EINVAL;
+    if (ws_bytes < sort_workspace_bytes(n, sizeof(K))) return MCS_ENOMEM;
+    const int nblocks = (int)ceil_div64(n, SORT_TILE);
+    char* p = (char*)ws;
+    K* kalt = (K*)p;                 p += align_up((size_t)n * sizeof(K));
+    uint32_t* valt = (uint32_t*)p;   p += align_up((size_t)n * sizeof(uint32_t));
+    uint32_t* counts = (uint32_t*)p; p += align_up((size_t)256 * nblocks * sizeof(uint32_t));
+    void* scan_ws = p;
+    size_t scan_ws_bytes = ws_bytes - (size_t)(p - (char*)ws);
+    K* kin = keys; uint32_t* vin = vals; K* kout = kalt; uint32_t* vout = valt;
+    const int passes = (key_bits + 7) / 8;
+    for (int pass = 0; pass < passes; ++pass) {
+        int shift = pass * 8;
+        radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks);
+        int rc = exclusive_scan_u32(counts, counts, (int64_t)256 * nblocks, nullptr, scan_ws, scan_ws_bytes, st);
+        if (rc != MCS_OK) return rc;
+        radix_scatter_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
+        K* tk = kin; kin = kout; kout = tk;
+        uint32_t* tv = vin; vin = vout; vout = tv;
+    }
+    if (kin != keys) {
+        MCS_CUDA_TRY(cudaMemcpyAsync(keys, kin, (size_t)n * sizeof(K), cudaMemcpyDeviceToDevice, st));
+        MCS_CUDA_TRY(cudaMemcpyAsync(vals, vin, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+}  // namespace
+
+size_t scan_workspace_bytes(int64_t n)
+{
+    size_t total = 0;
+    while (n > SCAN_TILE) {
+        n = ceil_div64(n, SCAN_TILE);
+        total += align_up((size_t)n * sizeof(uint32_t));
+    }
+    return total + 256;
+}
+
+int exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, uint32_t* total_out,
+                       void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (n <= 0) {
+        if (total_out) MCS_CUDA_TRY(cudaMemsetAsync(total_out, 0, sizeof(uint32_t), st));
+        return MCS_OK;
+    }
+    if (ws_bytes < scan_workspace_bytes(n)) return MCS_ENOMEM;
+    const int64_t nb = ceil_div64(n, SCAN_TILE);
+    if (nb == 1) {
+        scan_tile_kernel<<<1, SCAN_THREADS, 0, st>>>(in, out, n, nullptr, 1, total_out);
+    } else {
+        uint32_t* sums = (uint32_t*)ws;
+        char* rest = (char*)ws + align_up((size_t)nb * sizeof(uint32_t));
+        size_t rest_bytes = ws_bytes - align_up((size_t)nb * sizeof(uint32_t));
+        scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, nullptr, n, sums, 0, nullptr);
+        int rc = exclusive_scan_u32(sums, sums, nb, nullptr, rest, rest_bytes, st);
+        if (rc != MCS_OK) return rc;
+        scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, out, n, sums, 1, total_out);
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+size_t sort_workspace_bytes(int64_t n, int key_bytes)
+{
+    if (n < 1) n = 1;
+    const int64_t nblocks = ceil_div64(n, SORT_TILE);
+    return align_up((size_t)n * key_bytes) + align_up((size_t)n * sizeof(uint32_t)) +
+           align_up((size_t)256 * nblocks * sizeof(uint32_t)) + scan_workspace_bytes(256 * nblocks) + 256;
+}
+
+int sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    return radix_sort_impl<uint64_t>(keys, vals, n, key_bits, ws, ws_bytes, st);
+}
+
+int sort_pairs_u32(uint32_t* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    return radix_sort_impl<uint32_t>(keys, vals, n, key_bits, ws, ws_bytes, st);
+}

@@ -1,0 +1,542 @@
+// walk.cu -- sample preparation (A2), walk initialisation (A3), the
+// walk-on-spheres loop (A4), termination records (A5) and killing walks (A6) of
+// SURVEY.md 8(a).  Follows Alg. 2 for the interior operator
+// and Eq. 32 for the exterior one, in fp32.
+//
+// Scheduling: a persistent grid (a multiple of the SM count).  A warp takes a
+// chunk of consecutive walk indices from one global counter; every lane runs
+// one walk and, when it terminates, takes the next index of the warp's chunk
+// (wavefront compaction at lane granularity), so a warp never idles behind its
+// longest walk.  Results do not depend on the schedule: the RNG is
+// Philox4x32-10 keyed by (seed; sample, walk, step, purpose) and each walk
+// writes its record to the fixed slot sample*W + walk.
+#include "traverse.cuh"
+#include "walk.cuh"
+
+#include <limits.h>
+
+namespace {
+
+constexpr int WT = 128;                 // threads per block of the walk kernel
+constexpr int PT = 128;                 // threads per block of the per-sample kernels
+
+__device__ __forceinline__ int float_to_ordered(float f)
+{
+    int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7FFFFFFF;
+}
+
+// ---------------------------------------------------------------------------
+// Exterior prerequisites: AABB of the Kelvin-inverted vertices (r_max rule,
+// PAPER.md:642) and R_max = max |v - o| (reading E3).
+// out: int[7] = ordered lo[3], hi[3], ordered max norm.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(PT)
+kelvin_bounds_kernel(const float* __restrict__ verts, int64_t V, float3 o, int* __restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * PT + threadIdx.x;
+    float lo[3] = { CUDART_INF_F, CUDART_INF_F, CUDART_INF_F }, hi[3] = { -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F };
+    float nrm = 0.0f;
+    if (i < V) {
+        const float3 w = f3(verts[3 * i] - o.x, verts[3 * i + 1] - o.y, verts[3 * i + 2] - o.z);
+        const float s = dot3(w, w);
+        nrm = sqrtf(s);
+        if (s > 0.0f) {
+            lo[0] = hi[0] = w.x / s; lo[1] = hi[1] = w.y / s; lo[2] = hi[2] = w.z / s;
+        } else {
+            out[7] = 1;                 // a vertex at the Kelvin origin
+        }
+    }
+    for (int off = 16; off > 0; off >>= 1) {
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fminf(lo[d], __shfl_xor_sync(0xFFFFFFFFu, lo[d], off));
+            hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xFFFFFFFFu, hi[d], off));
+        }
+        nrm = fmaxf(nrm, __shfl_xor_sync(0xFFFFFFFFu, nrm, off));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        for (int d = 0; d < 3; ++d) {
+            if (lo[d] <= hi[d]) { atomicMin(&out[d], float_to_ordered(lo[d])); atomicMax(&out[3 + d], float_to_ordered(hi[d])); }
+        }
+        atomicMax(&out[6], float_to_ordered(nrm));
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Z-order keys of the sample points ("sort sample points s via
+// Z-order curves, which greatly reduces warp divergence").
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned spread10(unsigned x)
+{
+    x &= 0x3FFu;
+    x = (x | (x << 16)) & 0x030000FFu;
+    x = (x | (x << 8))  & 0x0300F00Fu;
+    x = (x | (x << 4))  & 0x030C30C3u;
+    x = (x | (x << 2))  & 0x09249249u;
+    return x;
+}
+
+__device__ __forceinline__ void sample_point(const float* __restrict__ verts, const int32_t* __restrict__ faces,
+                                             const int32_t* __restrict__ tri, const float* __restrict__ bary, int64_t i,
+                                             float3& s, float3& n)
+{
+    const int64_t f = tri[i];
+    const int i0 = faces[3 * f], i1 = faces[3 * f + 1], i2 = faces[3 * f + 2];
+    const float3 a = f3(verts[3 * (int64_t)i0], verts[3 * (int64_t)i0 + 1], verts[3 * (int64_t)i0 + 2]);
+    const float3 b = f3(verts[3 * (int64_t)i1], verts[3 * (int64_t)i1 + 1], verts[3 * (int64_t)i1 + 2]);
+    const float3 c = f3(verts[3 * (int64_t)i2], verts[3 * (int64_t)i2 + 1], verts[3 * (int64_t)i2 + 2]);
+    const float b0 = bary[3 * i], b1 = bary[3 * i + 1], b2 = bary[3 * i + 2];
+    s = f3(fmaf(b0, a.x, fmaf(b1, b.x, b2 * c.x)), fmaf(b0, a.y, fmaf(b1, b.y, b2 * c.y)), fmaf(b0, a.z, fmaf(b1, b.z, b2 * c.z)));
+    n = cross3(b - a, c - a);
+    const float l = sqrtf(dot3(n, n));
+    if (l > 0.0f) n = (1.0f / l) * n;
+}
+
+__global__ void __launch_bounds__(PT)
+sample_keys_kernel(const float* __restrict__ verts, const int32_t* __restrict__ faces, int64_t F,
+                   const int32_t* __restrict__ tri, const float* __restrict__ bary, int64_t n_s,
+                   float3 lo, float3 hi, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, int* __restrict__ err)
+{
+    const int64_t i = (int64_t)blockIdx.x * PT + threadIdx.x;
+    if (i >= n_s) return;
+    vals[i] = (uint32_t)i;
+    if (tri[i] < 0 || tri[i] >= F) { *err = 1; keys[i] = 0; return; }
+    float3 s, n;
+    sample_point(verts, faces, tri, bary, i, s, n);
+    const float ex = hi.x - lo.x, ey = hi.y - lo.y, ez = hi.z - lo.z;
+    const float tx = ex > 0.f ? fminf(fmaxf((s.x - lo.x) / ex, 0.f), 1.f) : 0.f;
+    const float ty = ey > 0.f ? fminf(fmaxf((s.y - lo.y) / ey, 0.f), 1.f) : 0.f;
+    const float tz = ez > 0.f ? fminf(fmaxf((s.z - lo.z) / ez, 0.f), 1.f) : 0.f;
+    keys[i] = (spread10((unsigned)fminf(tx * 1024.f, 1023.f)) << 2) | (spread10((unsigned)fminf(ty * 1024.f, 1023.f)) << 1) |
+              spread10((unsigned)fminf(tz * 1024.f, 1023.f));
+}
+
+// ---------------------------------------------------------------------------
+// LargestTangentBall: bisection with `iters` iterations
+// (PAPER.md:383), radius clamped to r_max.  Each probe is a
+// bounded "is any face closer than r - eps/2" traversal (R4).
+// Exterior: the ball lives in the inverted domain and is probed through its
+// primal image (E2).
+// ---------------------------------------------------------------------------
+template <bool EXT>
+__global__ void __launch_bounds__(PT)
+tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
+                    const float* __restrict__ normal, const uint32_t* __restrict__ order, int64_t n_s,
+                    float rmax, float eps, int iters, float3 o,
+                    float4* __restrict__ balls, unsigned long long* __restrict__ stats)
+{
+    const int64_t j = (int64_t)blockIdx.x * PT + threadIdx.x;
+    TraversalCounters cnt; cnt.nodes = 0; cnt.tris = 0;
+    unsigned queries = 0, discarded = 0;
+    if (j < n_s) {
+        const int64_t i = order[j];
+        float3 s, n;
+        sample_point(g.verts, g.faces, tri, bary, i, s, n);
+        if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
+        float3 base = s, pole = n;       // ball centre = base - r * pole
+        float hi = rmax, ss2 = 1.0f, sdn = 0.0f, sstar_norm = 1.0f;
+        bool ok = true;
+        if (EXT) {
+            const float3 st = s - o;
+            const float sig = dot3(st, st);
+            ok = sig > 0.0f;
+            if (ok) {
+                base = (1.0f / sig) * st;                                  // s* = kappa(s - o)
+                const float sn = dot3(st, n) / sig;
+                pole = f3(-(n.x - 2.0f * st.x * sn), -(n.y - 2.0f * st.y * sn), -(n.z - 2.0f * st.z * sn));   // Eq. 54
+                ss2 = dot3(base, base);
+                sdn = dot3(base, pole);
+                if (sdn > 0.0f) hi = fminf(hi, 0.45f * ss2 / sdn);       // keep 0 = kappa(inf) outside the ball
+                sstar_norm = sqrtf(ss2);
+            }
+        }
+        float lo = 0.0f;
+        if (ok) {
+            for (int it = 0; it < iters; ++it) {
+                const float r = 0.5f * (lo + hi);
+                float3 c = f3(fmaf(-r, pole.x, base.x), fmaf(-r, pole.y, base.y), fmaf(-r, pole.z, base.z));
+                float thr;
+                if (EXT) {
+                    const float den = ss2 - 2.0f * r * sdn;               // |c*|^2 - r^2
+                    c = f3(o.x + c.x / den, o.y + c.y / den, o.z + c.z / den);
+                    thr = (r / den) * (1.0f - 0.5f * eps / r);
+                } else {
+                    thr = r - 0.5f * eps;
+                }
+                bool closer = false;
+                if (thr > 0.0f) {
+                    ClosestHit h; h.d2 = thr * thr; h.tri = -1; h.k = -1; h.v = h.w = 0.0f;
+                    const float bound = h.d2;
+                    bvh_closest_point<true, true>(g.nodes, g.tris, c, h, cnt);
+                    closer = h.d2 < bound;
+                    ++queries;
+                }
+                if (closer) hi = r; else lo = r;
+            }
+        }
+        const float r = lo;
+        if (!(r > 0.0f)) discarded = 1;
+        balls[2 * i] = make_float4(fmaf(-r, pole.x, base.x), fmaf(-r, pole.y, base.y), fmaf(-r, pole.z, base.z), r);
+        balls[2 * i + 1] = make_float4(pole.x, pole.y, pole.z, ok ? sstar_norm : 0.0f);
+    }
+    // statistics (integer atomics: order-independent)
+    unsigned vals[4] = { queries, discarded, cnt.nodes, cnt.tris };
+    for (int q = 0; q < 4; ++q) {
+        unsigned v = vals[q];
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+        vals[q] = v;
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (vals[0]) atomicAdd(&stats[ST_QUERIES], (unsigned long long)vals[0]);
+        if (vals[1]) atomicAdd(&stats[ST_DISCARDED], (unsigned long long)vals[1]);
+        if (vals[2]) atomicAdd(&stats[ST_NODES], (unsigned long long)vals[2]);
+        if (vals[3]) atomicAdd(&stats[ST_TRIS], (unsigned long long)vals[3]);
+    }
+}
+
+// Orthonormal frame (e1, e2, n) of a unit vector n: branchless construction of
+// Duff et al. (JCGT 2017), restated (R6b: the frame rule is part of
+// the definition of a walk's start point).
+__device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& e2)
+{
+    const float sign = copysignf(1.0f, n.z);
+    const float a = -1.0f / (sign + n.z);
+    const float b = n.x * n.y * a;
+    e1 = f3(1.0f + sign * n.x * n.x * a, sign * b, -sign * n.x);
+    e2 = f3(b, sign + n.y * n.y * a, -n.y);
+}
+
+struct LaneWalk {
+    float3 x;          // interior: position; exterior: Kelvin coordinates y about the origin
+    float  wfac;       // weight without the exit-point factor
+    unsigned sample, walk;
+    int    k;          // jumps taken so far
+    int    slot_hi, slot_lo;   // record slot (64-bit split)
+    int    prev;       // sorted slot of the last closest triangle (-1: none)
+};
+
+// ---------------------------------------------------------------------------
+// The walk kernel.
+// ---------------------------------------------------------------------------
+template <bool EXT, bool COUNT>
+__global__ void __launch_bounds__(WT)
+walk_kernel(WalkGeom g, WalkArgs a)
+{
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const long long total = a.n_s * a.W + a.n_kill;
+    const long long n_main = a.n_s * a.W;
+    const uint2 key = make_uint2(a.key0, a.key1);
+    const float3 o = f3(a.ox, a.oy, a.oz);
+
+    long long chunk_cur = 0, chunk_end = 0;      // warp-uniform
+    bool exhausted = false;
+    bool active = false;
+    float3 x = f3(0.f, 0.f, 0.f);
+    float wfac = 0.f;
+    unsigned sample = 0, walk = 0;
+    int k = 0, prev = -1;
+    long long slot = 0;
+    TraversalCounters cnt; cnt.nodes = 0; cnt.tris = 0;
+    unsigned n_steps = 0, n_queries = 0, n_trunc = 0;
+
+    for (;;) {
+        // ---- refill idle lanes from the warp's chunk ------------------------
+        unsigned idle = __ballot_sync(FULL, !active);
+        while (idle != 0 && !exhausted) {
+            if (chunk_cur >= chunk_end) {
+                long long base = 0;
+                if (lane == 0) base = (long long)atomicAdd(a.work_counter, (unsigned long long)a.chunk);
+                base = __shfl_sync(FULL, base, 0);
+                if (base >= total) { exhausted = true; break; }
+                chunk_cur = base;
+                chunk_end = base + a.chunk < total ? base + a.chunk : total;
+            }
+            const int avail = (int)(chunk_end - chunk_cur);
+            const int n_idle = __popc(idle);
+            const int rank = __popc(idle & lt);
+            if (!active && rank < avail) {
+                const long long j = chunk_cur + rank;
+                active = true; k = 0; prev = -1;
+                if (j < n_main) {
+                    const long long pos = j / a.W;
+                    walk = (unsigned)(j - pos * a.W);
+                    sample = a.order[pos];
+                    slot = (long long)sample * a.W + walk;
+                    const float4 b0 = __ldg(&a.balls[2 * (long long)sample]);
+                    const float4 b1 = __ldg(&a.balls[2 * (long long)sample + 1]);
+                    const float r = b0.w;
+                    if (!(r > 0.0f)) {                               // discarded sample
+                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                        if (a.steps) a.steps[slot] = -2;
+                        active = false;
+                    } else {
+                        // SampleBallSurface + BallJumpKernel (Eq. 23; R5-R7)
+                        const unsigned wq = a.antithetic ? (walk >> 1) : walk;
+                        const uint4 rn = philox4x32_10(make_uint4(sample, wq, 0u, MCS_PURPOSE_INIT), key);
+                        const float u1 = u01(rn.x), u2 = u01(rn.y);
+                        float q, factor;
+                        if (a.importance) {
+                            q = 1.0f / (a.inv_q0 - u1 * (a.inv_q0 - 1.0f));
+                            factor = (1.0f / (4.0f * r)) * (a.inv_q0 - 1.0f);
+                        } else {
+                            q = sqrtf(u1);
+                            factor = (q < a.q0) ? 0.0f : 1.0f / (8.0f * r * q * q * q);
+                        }
+                        const float ct = 1.0f - 2.0f * q * q;
+                        const float st = 2.0f * q * sqrtf(fmaxf(0.0f, 1.0f - q * q));
+                        float sphi, cphi;
+                        sincospif(2.0f * u2 + ((a.antithetic && (walk & 1u)) ? 1.0f : 0.0f), &sphi, &cphi);
+                        const float3 pole = f3(b1.x, b1.y, b1.z);
+                        float3 e1, e2;
+                        frame_from_normal(pole, e1, e2);
+                        x = f3(b0.x + r * (ct * pole.x + st * (cphi * e1.x + sphi * e2.x)),
+                               b0.y + r * (ct * pole.y + st * (cphi * e1.y + sphi * e2.y)),
+                               b0.z + r * (ct * pole.z + st * (cphi * e1.z + sphi * e2.z)));
+                        wfac = (__ldg(&a.weight[sample]) / (float)a.W) * factor;
+                        if (EXT) wfac *= b1.w * b1.w * b1.w;          // |s*|^3, Eq. 32
+                        prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
+                    }
+                } else {                                             // killing walk from kappa(inf) = 0
+                    sample = MCS_KILLING_SAMPLE;
+                    walk = (unsigned)(j - n_main);
+                    slot = j;
+                    x = f3(0.f, 0.f, 0.f);
+                    wfac = 4.0f * CUDART_PI_F / (float)a.n_kill;
+                }
+            }
+            chunk_cur += n_idle < avail ? n_idle : avail;
+            idle = __ballot_sync(FULL, !active);
+        }
+        if (!__any_sync(FULL, active)) break;
+
+        // ---- one walk-on-spheres iteration (R9) ---
+        if (active) {
+            float3 xq = x;
+            float radius = 0.0f, rho = 0.0f;
+            bool need_query = true;
+            if (EXT) {
+                const float yn = sqrtf(dot3(x, x));
+                if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
+                    radius = 1.0f / a.Rmax - yn;
+                    need_query = false;
+                } else {
+                    const float inv = 1.0f / (yn * yn);
+                    xq = f3(fmaf(inv, x.x, o.x), fmaf(inv, x.y, o.y), fmaf(inv, x.z, o.z));
+                    rho = 1.0f / yn;
+                }
+            }
+            bool done = false;
+            if (need_query) {
+                ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
+                if (prev >= 0) { test_triangle(g.tris, prev, xq, h); if (COUNT) cnt.tris++; }
+                bvh_closest_point<COUNT, false>(g.nodes, g.tris, xq, h, cnt);
+                ++n_queries;
+                prev = h.k;
+                const float D = sqrtf(h.d2);
+                radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
+                if (radius < a.eps) {
+                    float wgt = wfac;
+                    if (EXT) {
+                        const float3 t = hit_point(g.tris, h) - o;
+                        wgt *= sqrtf(dot3(t, t));                    // 1/|t*| = |t - o|, Eq. 32
+                    }
+                    a.records[slot] = make_float4(__int_as_float(h.tri), h.v, h.w, wgt);
+                    if (a.steps) a.steps[slot] = k;
+                    done = true;
+                }
+            }
+            if (!done) {
+                if (k == a.max_steps) {                              // DESIGN.md R10
+                    a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                    if (a.steps) a.steps[slot] = -1;
+                    ++n_trunc;
+                    done = true;
+                } else {
+                    ++k; ++n_steps;
+                    const uint4 rn = philox4x32_10(make_uint4(sample, walk, (unsigned)k, MCS_PURPOSE_STEP), key);
+                    const float ct = 1.0f - 2.0f * u01(rn.x);
+                    const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+                    float sphi, cphi;
+                    sincospif(2.0f * u01(rn.y), &sphi, &cphi);
+                    x = f3(fmaf(radius, st * cphi, x.x), fmaf(radius, st * sphi, x.y), fmaf(radius, ct, x.z));
+                }
+            }
+            if (done) active = false;
+        }
+    }
+
+    // ---- statistics ----------------------------------------------------------
+    unsigned vals[5] = { n_steps, n_queries, n_trunc, cnt.nodes, cnt.tris };
+    for (int q = 0; q < 5; ++q) {
+        unsigned long long v = vals[q];
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+        if (lane == 0 && v) {
+            const int idx = q == 0 ? ST_STEPS : q == 1 ? ST_QUERIES : q == 2 ? ST_TRUNCATED : q == 3 ? ST_NODES : ST_TRIS;
+            atomicAdd(&a.stats[idx], v);
+        }
+    }
+}
+
+__global__ void face_slot_lookup_kernel(const int32_t* __restrict__ face_slot, const int32_t* __restrict__ tri,
+                                        int64_t n_s, int32_t* __restrict__ sample_slot)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_s) sample_slot[i] = face_slot[tri[i]];
+}
+
+__global__ void balls_export_kernel(const float4* __restrict__ balls, int64_t n_s, float* __restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_s) return;
+    const float4 b0 = balls[2 * i], b1 = balls[2 * i + 1];
+    float* o = out + 8 * i;
+    o[0] = b0.x; o[1] = b0.y; o[2] = b0.z; o[3] = b0.w; o[4] = b1.x; o[5] = b1.y; o[6] = b1.z; o[7] = b1.w;
+}
+
+int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior)
+{
+    if (!b || !s || !p) return MCS_EINVAL;
+    if (s->n_s < 1 || !s->tri || !s->bary || !s->weight) return MCS_EINVAL;
+    if (p->walks_per_sample < 1 || p->max_steps < 0 || !(p->eps > 0.0f)) return MCS_EINVAL;
+    if (!(p->cap_half_angle_deg > 0.0f) || p->cap_half_angle_deg >= 180.0f) return MCS_EINVAL;
+    if (p->bisection_iters < 1 || p->bisection_iters > 64) return MCS_EINVAL;
+    if (!(p->rmax_scale > 0.0f) && !(p->rmax_override > 0.0f)) return MCS_EINVAL;
+    if (s->n_s >= ((int64_t)1 << 32) - 1) return MCS_EINVAL;
+    if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
+    if (s->n_s * (int64_t)p->walks_per_sample >= ((int64_t)1 << 40)) return MCS_EINVAL;
+    return MCS_OK;
+}
+
+}  // namespace
+
+int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior)
+{
+    int64_t n = s->n_s * (int64_t)p->walks_per_sample;
+    if (exterior && p->include_killing) n += p->n_kill_walks;
+    return n;
+}
+
+size_t walk_workspace_bytes(const mcs_samples* s)
+{
+    const int64_t n = s->n_s;
+    return align_up((size_t)n * 32)                 // balls
+         + align_up((size_t)n * 4) * 3              // keys, order, sample_slot
+         + align_up(ST_COUNT * 8 + 64)              // counters
+         + sort_workspace_bytes(n, 4) + 256;
+}
+
+// Runs A2-A6.  Layout of `ws`: see walk_workspace_bytes.
+int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
+             void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st)
+{
+    int rc = check_params(b, s, p, exterior);
+    if (rc != MCS_OK) return rc;
+    if (!ws || ws_bytes < walk_workspace_bytes(s)) return MCS_ENOMEM;
+    const int64_t n_s = s->n_s;
+    char* ptr = (char*)ws;
+    float4* balls = (float4*)ptr;                 ptr += align_up((size_t)n_s * 32);
+    uint32_t* keys = (uint32_t*)ptr;              ptr += align_up((size_t)n_s * 4);
+    uint32_t* order = (uint32_t*)ptr;             ptr += align_up((size_t)n_s * 4);
+    int32_t* sample_slot = (int32_t*)ptr;         ptr += align_up((size_t)n_s * 4);
+    unsigned long long* stats = (unsigned long long*)ptr;  ptr += align_up(ST_COUNT * 8 + 64);
+    void* sort_ws = ptr;
+    const size_t sort_bytes = ws_bytes - (size_t)(ptr - (char*)ws);
+    int* ibuf = (int*)(stats + ST_COUNT);         // 8 ints of scratch after the counters
+    if (stats_dev_out) *stats_dev_out = stats;
+
+    WalkGeom g;
+    g.nodes = b->nodes; g.tris = b->tris; g.verts = b->verts; g.faces = b->faces;
+
+    MCS_CUDA_TRY(cudaMemsetAsync(stats, 0, ST_COUNT * 8 + 64, st));
+    const float3 lo = f3(b->aabb_lo[0], b->aabb_lo[1], b->aabb_lo[2]);
+    const float3 hi = f3(b->aabb_hi[0], b->aabb_hi[1], b->aabb_hi[2]);
+    const float3 o = exterior ? f3(p->kelvin_origin[0], p->kelvin_origin[1], p->kelvin_origin[2]) : f3(0.f, 0.f, 0.f);
+    const unsigned nblk_s = (unsigned)ceil_div64(n_s, PT);
+
+    // r_max and, for the exterior, R_max
+    float side = fminf(hi.x - lo.x, fminf(hi.y - lo.y, hi.z - lo.z));
+    float Rmax = 0.0f;
+    if (exterior) {
+        int h[8];
+        for (int d = 0; d < 3; ++d) { h[d] = 0x7FFFFFFF; h[3 + d] = (int)0x80000000; }
+        h[6] = (int)0x80000000; h[7] = 0;
+        MCS_CUDA_TRY(cudaMemcpyAsync(ibuf, h, sizeof h, cudaMemcpyHostToDevice, st));
+        kelvin_bounds_kernel<<<(unsigned)ceil_div64(b->V, PT), PT, 0, st>>>(b->verts, b->V, o, ibuf);
+        MCS_CUDA_TRY(cudaMemcpyAsync(h, ibuf, sizeof h, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (h[7]) return MCS_EDEGENERATE;
+        float f[7];
+        for (int d = 0; d < 7; ++d) { int v = h[d] >= 0 ? h[d] : h[d] ^ 0x7FFFFFFF; memcpy(&f[d], &v, 4); }
+        side = fminf(f[3] - f[0], fminf(f[4] - f[1], f[5] - f[2]));
+        Rmax = f[6];
+        if (!(Rmax > 0.0f)) return MCS_EDEGENERATE;
+    }
+    const float rmax = p->rmax_override > 0.0f ? p->rmax_override : p->rmax_scale * (0.5f * side);
+
+    // Z-order of the samples
+    int* err = ibuf + 7;
+    sample_keys_kernel<<<nblk_s, PT, 0, st>>>(b->verts, b->faces, b->F, s->tri, s->bary, n_s, lo, hi, keys, order, err);
+    rc = sort_pairs_u32(keys, order, n_s, 30, sort_ws, sort_bytes, st);
+    if (rc != MCS_OK) return rc;
+    {
+        int h_err = 0;
+        MCS_CUDA_TRY(cudaMemcpyAsync(&h_err, err, 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (h_err) return MCS_EINVAL;                 // sample face index out of range
+    }
+    face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
+
+    if (exterior)
+        tangent_ball_kernel<true><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
+                                                         p->bisection_iters, o, balls, stats);
+    else
+        tangent_ball_kernel<false><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
+                                                          p->bisection_iters, o, balls, stats);
+    if (balls_out) balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
+    MCS_CUDA_TRY(cudaGetLastError());
+    if (balls_only) return MCS_OK;
+
+    WalkArgs a;
+    a.balls = balls; a.order = order; a.weight = s->weight; a.sample_slot = sample_slot;
+    a.n_s = n_s; a.W = p->walks_per_sample;
+    a.n_kill = (exterior && p->include_killing) ? p->n_kill_walks : 0;
+    a.eps = p->eps; a.max_steps = p->max_steps;
+    a.q0 = (float)sin(0.5 * (double)p->cap_half_angle_deg * 3.14159265358979323846 / 180.0);
+    a.inv_q0 = 1.0f / a.q0;
+    a.importance = p->importance_sample; a.antithetic = p->antithetic;
+    a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
+    a.key0 = (uint32_t)(p->seed & 0xFFFFFFFFu); a.key1 = (uint32_t)(p->seed >> 32);
+    a.records = records; a.steps = steps;
+    a.work_counter = stats + ST_WORK; a.stats = stats;
+
+    // persistent grid: resident blocks per SM x number of SMs
+    int dev = 0, n_sm = 0, per_sm = 0;
+    MCS_CUDA_TRY(cudaGetDevice(&dev));
+    MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    const void* fn = exterior ? (count ? (const void*)walk_kernel<true, true> : (const void*)walk_kernel<true, false>)
+                              : (count ? (const void*)walk_kernel<false, true> : (const void*)walk_kernel<false, false>);
+    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, WT, 0));
+    if (per_sm < 1) per_sm = 1;
+    const long long total = a.n_s * a.W + a.n_kill;
+    long long grid = (long long)n_sm * per_sm;
+    const long long warps = grid * (WT / 32);
+    long long chunk = total / (warps * 8);
+    chunk = chunk < 32 ? 32 : (chunk > 256 ? 256 : chunk);
+    chunk = (chunk / 32) * 32;
+    a.chunk = (int)chunk;
+    const long long need_blocks = ceil_div64(ceil_div64(total, chunk), WT / 32);
+    if (grid > need_blocks) grid = need_blocks;
+    if (grid < 1) grid = 1;
+    if (exterior) {
+        if (count) walk_kernel<true, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        else       walk_kernel<true, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
+    } else {
+        if (count) walk_kernel<false, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        else       walk_kernel<false, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}

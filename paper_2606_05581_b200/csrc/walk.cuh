@@ -1,0 +1,45 @@
+// walk.cuh -- internal interface between walk.cu, accumulate.cu and capi.cu.
+#pragma once
+#include "common.cuh"
+
+enum {
+    ST_WORK = 0,        // work-queue head of the persistent walk kernel
+    ST_STEPS, ST_QUERIES, ST_TRUNCATED, ST_DISCARDED, ST_NODES, ST_TRIS,
+    ST_ENTRIES, ST_UNIQUE,
+    ST_COUNT = 16
+};
+
+struct WalkGeom {
+    const BvhNode*   nodes;
+    const PackedTri* tris;
+    const float*     verts;
+    const int32_t*   faces;
+};
+
+struct WalkArgs {
+    const float4*   balls;         // [n_s][2]: (c.xyz, r), (pole.xyz, |s*|)
+    const uint32_t* order;         // Z-order permutation of the samples
+    const float*    weight;        // [n_s] quadrature weights a_i
+    const int32_t*  sample_slot;   // [n_s] sorted triangle slot of each sample's face
+    long long n_s, n_kill;
+    int   W, max_steps, chunk;
+    int   importance, antithetic;
+    float eps, q0, inv_q0;
+    float ox, oy, oz, Rmax;
+    uint32_t key0, key1;
+    float4* records;               // mcs_record viewed as float4
+    int32_t* steps;
+    unsigned long long* work_counter;
+    unsigned long long* stats;
+};
+
+int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior);
+size_t  walk_workspace_bytes(const mcs_samples* s);
+int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
+             void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st);
+
+size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records);
+int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+                   const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
+                   const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);
