@@ -224,8 +224,27 @@ size_t mcs_sort_workspace_bytes(int64_t n);
 int mcs_sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int32_t key_bits,
                        void* workspace, size_t workspace_bytes, void* stream);
 
+/* Measurement hooks (bench.py).  mcs_launch_count: kernels this library has launched in
+ * this process.  mcs_profile_enable(1): estimate_* calls record CUDA events on their stream
+ * around their phases; mcs_profile_last blocks on the last call's events and returns the
+ * elapsed device time of each phase in milliseconds (MCS_EINVAL if nothing was recorded).
+ * Not thread safe: one profiled call at a time. */
+typedef struct {
+    float prep_ms;               /* A2: Z-order sort + tangent balls            */
+    float walk_ms;               /* A3-A6: the persistent walk kernel           */
+    float accumulate_ms;         /* A7                                          */
+    float total_ms;
+} mcs_phase_times;
+unsigned long long mcs_launch_count(void);
+int mcs_profile_enable(int on);
+int mcs_profile_last(mcs_phase_times* out /* host */);
+
 const char* mcs_error_string(int code);
 const char* mcs_version(void);
+/* sizeof of the ABI structs, for bindings to check their mirrors against:
+ * 0 mcs_samples, 1 mcs_basis, 2 mcs_params, 3 mcs_matrix, 4 mcs_stats, 5 mcs_bvh_info_t,
+ * 6 mcs_record; anything else: 0. */
+size_t mcs_abi_sizeof(int which);
 
 #ifdef __cplusplus
 }

@@ -288,6 +288,31 @@ void orc_closest_points(const orc_geom *g, const float *q, int64_t Q,
     }
 }
 
+/* Tie filter helper for the parity tests (no method arithmetic of its own):
+ * runner_up[q] = smallest distance over all faces other than the winner tri[q]
+ * that are not copies of it (same three vertex indices in any order). */
+void orc_runner_up(const orc_geom *g, const float *q, int64_t Q, const int64_t *tri, double *runner_up)
+{
+    #pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < Q; ++i) {
+        double x[3] = { q[3*i], q[3*i+1], q[3*i+2] };
+        const int32_t *wf = g->faces + 3*tri[i];
+        double best = INFINITY;
+        for (int64_t f = 0; f < g->F; ++f) {
+            const int32_t *ff = g->faces + 3*f;
+            if (f == tri[i]) continue;
+            int same = 0;
+            for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) same += (ff[a] == wf[b]);
+            if (same >= 3) continue;
+            double a3[3], b3[3], c3[3], p3[3], bb[3];
+            load_vertex(g, ff[0], a3); load_vertex(g, ff[1], b3); load_vertex(g, ff[2], c3);
+            double d2 = orc_closest_point_triangle(x, a3, b3, c3, p3, bb);
+            if (d2 < best) best = d2;
+        }
+        runner_up[i] = sqrt(best);
+    }
+}
+
 /* ------------------------------------------------------------------------- */
 /* Mesh quantities: face normal, area, AABB, r_max.            */
 /* ------------------------------------------------------------------------- */

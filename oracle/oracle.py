@@ -150,6 +150,15 @@ class Oracle:
             out["second"] = second
         return out
 
+    def runner_up(self, queries, tri):
+        """Distance to the nearest face other than `tri` (and its exact copies): tie filter."""
+        q = np.ascontiguousarray(queries, np.float32)
+        t = np.ascontiguousarray(tri, np.int64)
+        out = np.empty(len(q))
+        self.lib.orc_runner_up(C.byref(self.geom.c), q.ctypes.data_as(C.c_void_p), C.c_int64(len(q)),
+                               t.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
+        return out
+
     def rmax(self, exterior=False, origin=(0, 0, 0)):
         return self.lib.orc_rmax(C.byref(self.geom.c), C.c_int(int(exterior)), _d3(origin))
 

@@ -245,13 +245,13 @@ def workspace_bytes(bvh: Bvh, samples: Samples, params: Params, exterior: bool) 
     return int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
 
 
-def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace):
+def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace, _exact_workspace=False):
     cs, cb, cp = samples.c(), _basis(bvh), params.c()
     K = bvh.V
     if out is None:
         out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
     need = workspace_bytes(bvh, samples, params, exterior)
-    if workspace is None or workspace.numel() < need:
+    if workspace is None or (workspace.numel() < need and not _exact_workspace):
         workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
     m = _Matrix(kind=0, K=K, dense=out.data_ptr())
     st = Stats() if want_stats else None
@@ -262,16 +262,18 @@ def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspa
     return (out, st) if want_stats else out
 
 
-def estimate_dtn_interior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None):
+def estimate_dtn_interior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
+                          _exact_workspace=False):
     """Interior DtN matrix, Alg. 2: dense [K,K] fp32 on the device."""
     return _estimate(lib().mcs_estimate_dtn_interior, "mcs_estimate_dtn_interior", bvh, samples, params, False,
-                     want_stats, out, workspace)
+                     want_stats, out, workspace, _exact_workspace)
 
 
-def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None):
+def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
+                          _exact_workspace=False):
     """Exterior DtN matrix, Eq. 32."""
     return _estimate(lib().mcs_estimate_dtn_exterior, "mcs_estimate_dtn_exterior", bvh, samples, params, True,
-                     want_stats, out, workspace)
+                     want_stats, out, workspace, _exact_workspace)
 
 
 def tangent_balls(bvh: Bvh, samples: Samples, params: Params, exterior: bool):
@@ -346,6 +348,27 @@ def sort_pairs_u64(keys, vals, key_bits=64):
         _check(lib().mcs_sort_pairs_u64(_ptr(keys), _ptr(vals), C.c_int64(n), C.c_int32(key_bits), _ptr(ws),
                                         C.c_size_t(need), _stream(keys.device)), "mcs_sort_pairs_u64")
     return keys, vals
+
+
+class PhaseTimes(C.Structure):
+    _fields_ = [("prep_ms", C.c_float), ("walk_ms", C.c_float), ("accumulate_ms", C.c_float),
+                ("total_ms", C.c_float)]
+
+
+def launch_count() -> int:
+    f = lib().mcs_launch_count
+    f.restype = C.c_ulonglong
+    return int(f())
+
+
+def profile_enable(on: bool):
+    _check(lib().mcs_profile_enable(C.c_int(int(on))), "mcs_profile_enable")
+
+
+def profile_last() -> PhaseTimes:
+    o = PhaseTimes()
+    _check(lib().mcs_profile_last(C.byref(o)), "mcs_profile_last")
+    return o
 
 
 def version() -> str:

@@ -166,7 +166,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     for (int64_t j0 = 0; j0 < n_records; j0 += C) {
         const long long n = (n_records - j0) < C ? (n_records - j0) : C;
         const unsigned nblk = (unsigned)ceil_div64(n, AT);
-        count_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts);
+        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts);
         int rc = exclusive_scan_u32(counts, counts, n, counts + n, scan_ws, scan_workspace_bytes(C) + 256, st);
         if (rc != MCS_OK) return rc;
         uint32_t n_entries = 0;
@@ -174,13 +174,13 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (n_entries == 0) continue;
         entries_total += n_entries;
-        expand_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts, keys, vals);
+        mcs_note_launch(), expand_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts, keys, vals);
         rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
-        reduce_runs_dense_kernel<<<(unsigned)ceil_div64(n_entries, AT), AT, 0, st>>>(
+        mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)ceil_div64(n_entries, AT), AT, 0, st>>>(
             keys, vals, n_entries, out->dense, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
     }
-    mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);
+    mcs_note_launch(), mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);
     if (stats_dev)
         MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_ENTRIES, &entries_total, 8, cudaMemcpyHostToDevice, st));
     MCS_CUDA_TRY(cudaGetLastError());

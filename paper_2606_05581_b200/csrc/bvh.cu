@@ -289,22 +289,22 @@ extern "C" int mcs_build_bvh(const float* verts, int64_t V, const int32_t* faces
     cudaMemsetAsync(arrivals, 0, (size_t)b->n_nodes * 4, st);
     cudaMemsetAsync(b->nodes, 0, nb_nodes, st);
 
-    face_bounds_kernel<<<nblk, BT, 0, st>>>(b->verts, V, b->faces, F, sc, partials);
-    area_total_kernel<<<1, 1, 0, st>>>(partials, nblk, sc);
+    mcs_note_launch(), face_bounds_kernel<<<nblk, BT, 0, st>>>(b->verts, V, b->faces, F, sc, partials);
+    mcs_note_launch(), area_total_kernel<<<1, 1, 0, st>>>(partials, nblk, sc);
     e = cudaMemcpyAsync(&h, sc, sizeof h, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { rc = MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
     if (h.flags & 1) { rc = MCS_EINVAL; goto done; }
     if ((h.flags & 2) || !(h.area > 0.0)) { rc = MCS_EDEGENERATE; goto done; }
 
-    morton_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, sc, b->morton, vals);
+    mcs_note_launch(), morton_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, sc, b->morton, vals);
     rc = sort_pairs_u64(b->morton, vals, F, 63, sort_ws, sort_bytes, st);
     if (rc != MCS_OK) goto done;
     if (F > 1)
-        radix_tree_kernel<<<(int)ceil_div64(F - 1, BT), BT, 0, st>>>(b->morton, F, (int32_t*)b->nodes, leaf_parent);
-    pack_refit_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, vals, leaf_parent, (int32_t*)b->nodes,
+        mcs_note_launch(), radix_tree_kernel<<<(int)ceil_div64(F - 1, BT), BT, 0, st>>>(b->morton, F, (int32_t*)b->nodes, leaf_parent);
+    mcs_note_launch(), pack_refit_kernel<<<nblk, BT, 0, st>>>(b->verts, b->faces, F, vals, leaf_parent, (int32_t*)b->nodes,
                                            arrivals, b->tris, b->leaf_tri, b->face_slot, sc);
-    depth_kernel<<<nblk, BT, 0, st>>>((const int32_t*)b->nodes, leaf_parent, F, sc);
+    mcs_note_launch(), depth_kernel<<<nblk, BT, 0, st>>>((const int32_t*)b->nodes, leaf_parent, F, sc);
     e = cudaMemcpyAsync(&h, sc, sizeof h, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e == cudaSuccess) e = cudaGetLastError();

@@ -7,6 +7,25 @@ static thread_local int g_last_cuda_error = 0;
 void mcs_set_last_cuda_error(int e) { g_last_cuda_error = e; }
 int  mcs_get_last_cuda_error() { return g_last_cuda_error; }
 
+#include <atomic>
+static std::atomic<unsigned long long> g_launches{0};
+void mcs_note_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static int g_prof_on = 0;
+static cudaEvent_t g_prof_ev[MCS_MARK_COUNT];
+static bool g_prof_have = false, g_prof_marked[MCS_MARK_COUNT];
+void mcs_prof_mark(int which, cudaStream_t st)
+{
+    if (!g_prof_on || which < 0 || which >= MCS_MARK_COUNT) return;
+    if (!g_prof_have) {
+        for (int i = 0; i < MCS_MARK_COUNT; ++i) cudaEventCreate(&g_prof_ev[i]);
+        g_prof_have = true;
+    }
+    if (which == MCS_MARK_BEGIN) for (int i = 0; i < MCS_MARK_COUNT; ++i) g_prof_marked[i] = false;
+    cudaEventRecord(g_prof_ev[which], st);
+    g_prof_marked[which] = true;
+}
+
 namespace {
 
 struct Layout {
@@ -61,12 +80,14 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
     char* base = (char*)ws;
     float4* records = (float4*)(base + L.records_off);
     unsigned long long* stats_dev = nullptr;
+    mcs_prof_mark(MCS_MARK_BEGIN, st);
     int rc = walk_run(b, s, p, exterior, base + L.walk_off, align_up(walk_workspace_bytes(s)), records, nullptr,
                       false, nullptr, hs != nullptr, &stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
     rc = accumulate_run(b, s, basis, p->walks_per_sample, records, L.n_records, base + L.acc_off,
                         align_up(accumulate_workspace_bytes(b, basis, L.n_records)), out, stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
+    mcs_prof_mark(MCS_MARK_END, st);
     if (hs) {
         unsigned long long h[ST_COUNT];
         cudaError_t e = cudaMemcpyAsync(h, stats_dev, sizeof h, cudaMemcpyDeviceToHost, st);
@@ -78,6 +99,24 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
 }
 
 }  // namespace
+
+extern "C" unsigned long long mcs_launch_count(void) { return g_launches.load(); }
+
+extern "C" int mcs_profile_enable(int on) { g_prof_on = on ? 1 : 0; return MCS_OK; }
+
+extern "C" int mcs_profile_last(mcs_phase_times* out)
+{
+    if (!out) return MCS_EINVAL;
+    memset(out, 0, sizeof *out);
+    if (!g_prof_have) return MCS_EINVAL;
+    for (int i = 0; i < MCS_MARK_COUNT; ++i) if (!g_prof_marked[i]) return MCS_EINVAL;
+    MCS_CUDA_TRY(cudaEventSynchronize(g_prof_ev[MCS_MARK_END]));
+    MCS_CUDA_TRY(cudaEventElapsedTime(&out->prep_ms, g_prof_ev[MCS_MARK_BEGIN], g_prof_ev[MCS_MARK_WALK_BEGIN]));
+    MCS_CUDA_TRY(cudaEventElapsedTime(&out->walk_ms, g_prof_ev[MCS_MARK_WALK_BEGIN], g_prof_ev[MCS_MARK_WALK_END]));
+    MCS_CUDA_TRY(cudaEventElapsedTime(&out->accumulate_ms, g_prof_ev[MCS_MARK_WALK_END], g_prof_ev[MCS_MARK_END]));
+    MCS_CUDA_TRY(cudaEventElapsedTime(&out->total_ms, g_prof_ev[MCS_MARK_BEGIN], g_prof_ev[MCS_MARK_END]));
+    return MCS_OK;
+}
 
 extern "C" size_t mcs_workspace_bytes(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
                                       const mcs_params* p, int exterior)
@@ -194,6 +233,20 @@ extern "C" const char* mcs_error_string(int code)
         case MCS_ENOMEM: return "workspace too small or device allocation failed";
         case MCS_ECUDA: return "CUDA runtime error";
         default: return "unknown error";
+    }
+}
+
+extern "C" size_t mcs_abi_sizeof(int which)
+{
+    switch (which) {
+        case 0: return sizeof(mcs_samples);
+        case 1: return sizeof(mcs_basis);
+        case 2: return sizeof(mcs_params);
+        case 3: return sizeof(mcs_matrix);
+        case 4: return sizeof(mcs_stats);
+        case 5: return sizeof(mcs_bvh_info_t);
+        case 6: return sizeof(mcs_record);
+        default: return 0;
     }
 }
 

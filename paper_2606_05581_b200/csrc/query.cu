@@ -21,7 +21,7 @@ closest_point_kernel(const BvhNode* __restrict__ nodes, const PackedTri* __restr
     bvh_closest_point<false, false>(nodes, tris, p, h, cnt);
     if (dist) dist[i] = sqrtf(h.d2);
     if (tri) tri[i] = h.k >= 0 ? h.tri : -1;
-    if (bary) { bary[3 * i] = 1.0f - h.v - h.w; bary[3 * i + 1] = h.v; bary[3 * i + 2] = h.w; }
+    if (bary) { bary[3 * i] = fmaxf(1.0f - h.v - h.w, 0.0f); bary[3 * i + 1] = h.v; bary[3 * i + 2] = h.w; }
 }
 
 // Exhaustive scan: every thread tests every face; faces staged through shared memory.
@@ -55,7 +55,7 @@ closest_point_bruteforce_kernel(const PackedTri* __restrict__ tris, int64_t F,
     if (!active) return;
     if (dist) dist[i] = sqrtf(h.d2);
     if (tri) tri[i] = h.tri;
-    if (bary) { bary[3 * i] = 1.0f - h.v - h.w; bary[3 * i + 1] = h.v; bary[3 * i + 2] = h.w; }
+    if (bary) { bary[3 * i] = fmaxf(1.0f - h.v - h.w, 0.0f); bary[3 * i + 1] = h.v; bary[3 * i + 2] = h.w; }
 }
 
 __global__ void philox_kernel(const uint32_t* __restrict__ ctr, int64_t n, uint2 key, uint32_t* __restrict__ out)
@@ -74,7 +74,7 @@ extern "C" int mcs_closest_point(const mcs_bvh* b, const float* q, int64_t Q,
 {
     if (!b || Q < 0 || (Q > 0 && !q)) return MCS_EINVAL;
     if (Q == 0) return MCS_OK;
-    closest_point_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->nodes, b->tris, q, Q, dist, tri, bary);
+    mcs_note_launch(), closest_point_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->nodes, b->tris, q, Q, dist, tri, bary);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }
@@ -84,7 +84,7 @@ extern "C" int mcs_closest_point_bruteforce(const mcs_bvh* b, const float* q, in
 {
     if (!b || Q < 0 || (Q > 0 && !q)) return MCS_EINVAL;
     if (Q == 0) return MCS_OK;
-    closest_point_bruteforce_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->tris, b->F, q, Q, dist, tri, bary);
+    mcs_note_launch(), closest_point_bruteforce_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->tris, b->F, q, Q, dist, tri, bary);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }
@@ -93,7 +93,7 @@ extern "C" int mcs_philox4x32_10(const uint32_t* counters, int64_t n, const uint
 {
     if (n < 0 || !key || (n > 0 && (!counters || !out))) return MCS_EINVAL;
     if (n == 0) return MCS_OK;
-    philox_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, (cudaStream_t)stream>>>(counters, n, make_uint2(key[0], key[1]), out);
+    mcs_note_launch(), philox_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, (cudaStream_t)stream>>>(counters, n, make_uint2(key[0], key[1]), out);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

@@ -165,10 +165,10 @@ int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, 
     const int passes = (key_bits + 7) / 8;
     for (int pass = 0; pass < passes; ++pass) {
         int shift = pass * 8;
-        radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks);
+        mcs_note_launch(), radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks);
         int rc = exclusive_scan_u32(counts, counts, (int64_t)256 * nblocks, nullptr, scan_ws, scan_ws_bytes, st);
         if (rc != MCS_OK) return rc;
-        radix_scatter_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
+        mcs_note_launch(), radix_scatter_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
         K* tk = kin; kin = kout; kout = tk;
         uint32_t* tv = vin; vin = vout; vout = tv;
     }
@@ -202,15 +202,15 @@ int exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, uint32_t* t
     if (ws_bytes < scan_workspace_bytes(n)) return MCS_ENOMEM;
     const int64_t nb = ceil_div64(n, SCAN_TILE);
     if (nb == 1) {
-        scan_tile_kernel<<<1, SCAN_THREADS, 0, st>>>(in, out, n, nullptr, 1, total_out);
+        mcs_note_launch(), scan_tile_kernel<<<1, SCAN_THREADS, 0, st>>>(in, out, n, nullptr, 1, total_out);
     } else {
         uint32_t* sums = (uint32_t*)ws;
         char* rest = (char*)ws + align_up((size_t)nb * sizeof(uint32_t));
         size_t rest_bytes = ws_bytes - align_up((size_t)nb * sizeof(uint32_t));
-        scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, nullptr, n, sums, 0, nullptr);
+        mcs_note_launch(), scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, nullptr, n, sums, 0, nullptr);
         int rc = exclusive_scan_u32(sums, sums, nb, nullptr, rest, rest_bytes, st);
         if (rc != MCS_OK) return rc;
-        scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, out, n, sums, 1, total_out);
+        mcs_note_launch(), scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, out, n, sums, 1, total_out);
     }
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;

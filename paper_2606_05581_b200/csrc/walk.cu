@@ -464,7 +464,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         for (int d = 0; d < 3; ++d) { h[d] = 0x7FFFFFFF; h[3 + d] = (int)0x80000000; }
         h[6] = (int)0x80000000; h[7] = 0;
         MCS_CUDA_TRY(cudaMemcpyAsync(ibuf, h, sizeof h, cudaMemcpyHostToDevice, st));
-        kelvin_bounds_kernel<<<(unsigned)ceil_div64(b->V, PT), PT, 0, st>>>(b->verts, b->V, o, ibuf);
+        mcs_note_launch(), kelvin_bounds_kernel<<<(unsigned)ceil_div64(b->V, PT), PT, 0, st>>>(b->verts, b->V, o, ibuf);
         MCS_CUDA_TRY(cudaMemcpyAsync(h, ibuf, sizeof h, cudaMemcpyDeviceToHost, st));
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (h[7]) return MCS_EDEGENERATE;
@@ -478,7 +478,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
 
     // Z-order of the samples
     int* err = ibuf + 7;
-    sample_keys_kernel<<<nblk_s, PT, 0, st>>>(b->verts, b->faces, b->F, s->tri, s->bary, n_s, lo, hi, keys, order, err);
+    mcs_note_launch(), sample_keys_kernel<<<nblk_s, PT, 0, st>>>(b->verts, b->faces, b->F, s->tri, s->bary, n_s, lo, hi, keys, order, err);
     rc = sort_pairs_u32(keys, order, n_s, 30, sort_ws, sort_bytes, st);
     if (rc != MCS_OK) return rc;
     {
@@ -487,15 +487,15 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (h_err) return MCS_EINVAL;                 // sample face index out of range
     }
-    face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
+    mcs_note_launch(), face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
 
     if (exterior)
-        tangent_ball_kernel<true><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
+        mcs_note_launch(), tangent_ball_kernel<true><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
                                                          p->bisection_iters, o, balls, stats);
     else
-        tangent_ball_kernel<false><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
+        mcs_note_launch(), tangent_ball_kernel<false><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
                                                           p->bisection_iters, o, balls, stats);
-    if (balls_out) balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
+    if (balls_out) mcs_note_launch(), balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
     MCS_CUDA_TRY(cudaGetLastError());
     if (balls_only) return MCS_OK;
 
@@ -530,13 +530,15 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     const long long need_blocks = ceil_div64(ceil_div64(total, chunk), WT / 32);
     if (grid > need_blocks) grid = need_blocks;
     if (grid < 1) grid = 1;
+    mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
     if (exterior) {
-        if (count) walk_kernel<true, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
-        else       walk_kernel<true, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        if (count) mcs_note_launch(), walk_kernel<true, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        else       mcs_note_launch(), walk_kernel<true, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
     } else {
-        if (count) walk_kernel<false, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
-        else       walk_kernel<false, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        if (count) mcs_note_launch(), walk_kernel<false, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
+        else       mcs_note_launch(), walk_kernel<false, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
     }
+    mcs_prof_mark(MCS_MARK_WALK_END, st);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

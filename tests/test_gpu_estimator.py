@@ -1,0 +1,323 @@
+"""GPU parity, estimator half: tangent balls, per-walk records, the deterministic
+accumulation, and the assembled interior / exterior DtN matrices against the CPU
+oracle (same Philox streams, brute-force fp64 geometry).  Bars (BASELINE.json
+north_star): matrix entries within 4 Monte Carlo standard errors of the oracle,
+identical seeds bit-identical run to run, exact symmetry, zero row sums for the
+interior operator.  Everything goes through the C ABI."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import Oracle, OracleParams, mesh_geom, steklov_eigs              # noqa: E402
+from synth import (box, icosphere, merge_meshes, stress_mesh, torus,            # noqa: E402
+                   uniform_samples, vertex_cell_samples)
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    from paper_2606_05581_b200 import api as _api
+    _api.lib()
+    return _api
+
+
+def _cuda(a, dtype):
+    return torch.as_tensor(np.ascontiguousarray(a)).to(device="cuda", dtype=dtype)
+
+
+def _setup(api, v, f, smp):
+    bvh = api.build_bvh(_cuda(v, torch.float32), _cuda(f, torch.int32))
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    return bvh, S
+
+
+def _params(api, **kw):
+    g = dict(kw)
+    o = dict(kw)
+    if "kelvin_origin" in g:
+        o["origin"] = o.pop("kelvin_origin")
+    return api.Params(**g), OracleParams(**o)
+
+
+def _unpack_records(rec):
+    r = rec.cpu().numpy()
+    return r[:, 0].copy().view(np.int32), r[:, 1], r[:, 2], r[:, 3]
+
+
+# ------------------------------------------------------------------------------
+# A2: tangent balls
+# ------------------------------------------------------------------------------
+@pytest.mark.parametrize("exterior", [False, True])
+def test_tangent_balls_match_oracle(api, exterior):
+    v, f = merge_meshes([icosphere(3), box((0.6, 0.8, 1.0), (3, 3, 3), center=(1.4, 0.2, 0.0))])[:2]
+    smp = uniform_samples(v, f, 3000, seed=4)
+    bvh, S = _setup(api, v, f, smp)
+    P, OP = _params(api, eps=1e-4, walks_per_sample=1, max_steps=0, kelvin_origin=(0.1, 0.05, -0.1))
+    balls = api.tangent_balls(bvh, S, P, exterior).cpu().numpy()
+    _, ob = Oracle(mesh_geom(v, f)).run_walks(OP, exterior, smp["tri"], smp["bary"], smp["weight"])
+    r_gpu, r_orc = balls[:, 3], ob[:, 0]
+    # the bisection takes the same branch unless a probe distance is within fp32 rounding of
+    # its threshold; then the two radii differ by one bisection cell at some level
+    same = np.abs(r_gpu - r_orc) <= 2e-6 * np.maximum(r_orc, 1e-3)
+    assert same.mean() > 0.995, same.mean()
+    assert np.abs(balls[same][:, :3] - ob[same][:, 1:4]).max() < 5e-6
+    if exterior:
+        assert np.abs(balls[:, 7] - ob[:, 4]).max() < 1e-5 * ob[:, 4].max()
+    assert ((r_gpu > 0) == (r_orc > 0)).mean() > 0.995
+
+
+# ------------------------------------------------------------------------------
+# A3-A6: per-walk records.  fp32 vs fp64 walks follow the same Philox stream, so
+# nearly every walk takes the same number of jumps and lands at the same point.
+# ------------------------------------------------------------------------------
+def _compare_records(api, v, f, smp, exterior, gp, op, min_same=0.97):
+    bvh, S = _setup(api, v, f, smp)
+    rec, steps, st = api.run_walks(bvh, S, gp, exterior, want_stats=True)
+    tri_t, b1, b2, wgt = _unpack_records(rec)
+    steps = steps.cpu().numpy()
+    orc = Oracle(mesh_geom(v, f))
+    orec, _ = orc.run_walks(op, exterior, smp["tri"], smp["bary"], smp["weight"])
+    assert len(orec) == len(steps)
+    # statistics kept by the kernel agree with what it wrote
+    assert st.n_walks == len(steps)
+    assert st.n_truncated == int((steps == -1).sum())
+    assert st.n_steps == int(steps[steps > 0].sum()) + int((steps == -1).sum()) * gp.max_steps
+    same = steps == orec["steps"]
+    assert same.mean() >= min_same, same.mean()
+    ok = same & (steps >= 0)
+    # exit point: same place on the surface
+    bt = np.stack([1 - b1 - b2, b1, b2], 1).astype(np.float64)
+    t_gpu = np.einsum("qk,qkd->qd", bt[ok], v[f[tri_t[ok]]].astype(np.float64))
+    err = np.linalg.norm(t_gpu - orec["t"][ok], axis=1)
+    scale = float(np.abs(v).max())
+    assert np.quantile(err, 0.99) < 2e-4 * scale, np.quantile(err, [0.5, 0.99, 1.0])
+    same_tri = tri_t[ok] == orec["tri_t"][ok]
+    assert same_tri.mean() > 0.98
+    rel = np.abs(wgt[ok] - orec["weight"][ok]) / np.abs(orec["weight"][ok]).max()
+    assert np.quantile(rel, 0.99) < 1e-4
+    # distribution of walk lengths (all walks, diverged ones included)
+    g, o = steps[steps >= 0], orec["steps"][orec["steps"] >= 0]
+    assert abs(g.mean() - o.mean()) < 0.03 * max(o.mean(), 1.0)
+    return rec, steps, orec, st
+
+
+def test_interior_records_match_oracle_icosphere(api):
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 4, seed=0)
+    gp, op = _params(api, seed=11, walks_per_sample=64, eps=1e-3)
+    _compare_records(api, v, f, smp, False, gp, op)
+
+
+def test_interior_records_uniform_antithetic_multi_component(api):
+    v, f = merge_meshes([icosphere(3), box((0.6, 0.8, 1.0), (3, 3, 3), center=(2.4, 0.2, 0.0)),
+                         torus(1.0, 0.3, 40, 20, axis="z", center=(0, 0, 3.0))])[:2]
+    smp = uniform_samples(v, f, 400, seed=9)
+    gp, op = _params(api, seed=3, walks_per_sample=32, eps=1e-4, importance_sample=False, antithetic=True)
+    _compare_records(api, v, f, smp, False, gp, op)
+
+
+@pytest.mark.parametrize("origin", [(0.0, 0.0, 0.0), (0.3, 0.1, -0.2)])
+def test_exterior_records_and_killing_match_oracle(api, origin):
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 2, seed=1)
+    gp, op = _params(api, seed=5, walks_per_sample=64, eps=1e-3, include_killing=True, n_kill_walks=5000,
+                     kelvin_origin=origin)
+    rec, steps, orec, st = _compare_records(api, v, f, smp, True, gp, op)
+    n_main = len(smp["weight"]) * 64
+    assert len(steps) == n_main + 5000
+    # capacity of the (polyhedral) unit sphere from the killing walks: sum of weights = 4 pi E|t0|
+    wk = _unpack_records(rec)[3][n_main:]
+    assert abs(wk.sum() / (4 * np.pi) - 1.0) < 0.02
+
+
+def test_truncated_and_discarded_walks(api):
+    """max_steps cuts walks (counted, weightless); flipped normals put the tangent ball
+    outside: on a closed convex solid those walks never return and are truncated."""
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 1, seed=2)
+    bvh, S = _setup(api, v, f, smp)
+    gp, op = _params(api, seed=1, walks_per_sample=16, eps=1e-5, max_steps=3)
+    rec, steps, st = api.run_walks(bvh, S, gp, False, want_stats=True)
+    orec, _ = Oracle(mesh_geom(v, f)).run_walks(op, False, smp["tri"], smp["bary"], smp["weight"])
+    steps = steps.cpu().numpy()
+    assert (steps == -1).sum() > 0 and st.n_truncated == (steps == -1).sum()
+    assert ((steps == -1) == (orec["steps"] == -1)).mean() > 0.98
+    tri_t, _, _, wgt = _unpack_records(rec)
+    assert (tri_t[steps == -1] == -1).all() and (wgt[steps == -1] == 0).all()
+    # zero-radius balls: normal override pointing along the surface -> every probe hits
+    nrm = np.zeros((len(smp["weight"]), 3), np.float32)
+    S2 = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"], normal=nrm)
+    rec, steps, st = api.run_walks(bvh, S2, api.Params(walks_per_sample=2, eps=1e-3), False, want_stats=True)
+    assert st.n_discarded == len(smp["weight"]) and (steps.cpu().numpy() == -2).all()
+
+
+# ------------------------------------------------------------------------------
+# A7: deterministic accumulation
+# ------------------------------------------------------------------------------
+def test_accumulate_from_oracle_records_matches_oracle_matrix(api):
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 3, seed=3)
+    orc = Oracle(mesh_geom(v, f))
+    op = OracleParams(seed=2, walks_per_sample=32, eps=1e-3, include_killing=True, n_kill_walks=3000)
+    out = orc.estimate_dtn(op, True, smp["tri"], smp["bary"], smp["weight"])
+    orec = out["records"]
+    rec = np.zeros((len(orec), 4), np.float32)
+    rec[:, 0] = orec["tri_t"].astype(np.int32).view(np.float32)
+    rec[:, 1] = orec["bary_t"][:, 1]
+    rec[:, 2] = orec["bary_t"][:, 2]
+    rec[:, 3] = orec["weight"]
+    bvh, S = _setup(api, v, f, smp)
+    gp = api.Params(seed=2, walks_per_sample=32, eps=1e-3, include_killing=True, n_kill_walks=3000)
+    Sg, st = api.accumulate(bvh, S, gp, _cuda(rec, torch.float32), want_stats=True)
+    Sg = Sg.cpu().numpy().astype(np.float64)
+    So = out["S"]
+    # fp32 sums of ~1e2..1e4 terms per entry
+    assert np.abs(Sg - So).max() <= 3e-5 * np.abs(So).max()
+    assert np.array_equal(Sg, Sg.T)
+    assert st.n_unique <= st.n_entries and st.n_unique >= np.count_nonzero(np.triu(So))
+    # run to run bit identity
+    Sg2 = api.accumulate(bvh, S, gp, _cuda(rec, torch.float32)).cpu().numpy()
+    assert np.array_equal(Sg2.astype(np.float64), Sg)
+
+
+# ------------------------------------------------------------------------------
+# The assembled matrices
+# ------------------------------------------------------------------------------
+def _hit_counts(out, smp, f, K):
+    """Number of oracle walks that contribute to each matrix entry (hat basis: the vertices
+    of the sample's face and of the exit face)."""
+    rec = out["records"]
+    ok = (rec["steps"] >= 0) & (rec["weight"] != 0)
+    r = rec[ok]
+    main = r["sample"] >= 0
+    vt = f[r["tri_t"]].astype(np.int64)
+    vs = np.where(main[:, None], f[np.asarray(smp["tri"])[np.maximum(r["sample"], 0)]].astype(np.int64), vt)
+    idx = np.concatenate([vs, vt], 1)
+    cnt = np.zeros((K, K), np.int64)
+    for p in range(6):
+        for q in range(6):
+            new = np.ones(len(idx), bool)                 # count each (row, col) once per walk
+            for p2 in range(6):
+                for q2 in range(6):
+                    if (p2, q2) < (p, q):
+                        new &= ~((idx[:, p2] == idx[:, p]) & (idx[:, q2] == idx[:, q]))
+            np.add.at(cnt, (idx[new, p], idx[new, q]), 1)
+    return cnt
+
+
+def _assert_within_4se(Sg, out, smp, f, min_hits=32):
+    """BASELINE north_star: entries within 4 Monte Carlo standard errors of the oracle, on
+    entries with >= 32 contributing walks; the variance estimate of an
+    entry hit by a handful of walks says nothing.  The same Philox streams make the two
+    far closer than that overall: Frobenius difference below one standard error."""
+    So, var = out["S"], out["var"]
+    cnt = _hit_counts(out, smp, f, len(So))
+    se = np.sqrt(2.0 * var)                             # both sides carry the same Monte Carlo error
+    scale = np.abs(So).max()
+    sel = cnt >= min_hits
+    assert sel.sum() > 100
+    bad = (np.abs(Sg - So) > 4.0 * se + 2e-6 * scale) & sel
+    assert bad.sum() <= max(1, int(1e-4 * sel.sum())), (bad.sum(), sel.sum())
+    assert np.linalg.norm(Sg - So) <= np.linalg.norm(np.sqrt(var))
+
+
+def test_config0_interior_icosphere_l2(api):
+    """BASELINE config 0: icosphere L2, hat basis, 1024 walks per vertex (G = 8 sample points
+    per vertex x 128 walks), eps 1e-3, cap 2.5 deg, seed 0."""
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 8, seed=0)
+    gp, op = _params(api, seed=0, walks_per_sample=128, eps=1e-3)
+    bvh, S = _setup(api, v, f, smp)
+    Sg, st = api.estimate_dtn_interior(bvh, S, gp, want_stats=True)
+    Sg2 = api.estimate_dtn_interior(bvh, S, gp)
+    assert torch.equal(Sg, Sg2)                          # bit-identical run to run
+    Sg = Sg.cpu().numpy().astype(np.float64)
+    assert st.n_walks == 162 * 1024 and st.n_truncated == 0
+    assert np.array_equal(Sg, Sg.T)                      # exactly symmetric
+    assert np.abs(Sg.sum(1)).max() < 2e-5 * np.abs(Sg).max()     # annihilates constants
+    orc = Oracle(mesh_geom(v, f))
+    out = orc.estimate_dtn(op, False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    _assert_within_4se(Sg, out, smp, f)
+    # spectrum: 0, 1 (x3), 2 (x5), 3 (x7) up to the cap / eps / mesh bias stated in DESIGN.md
+    M = orc.mass_matrix()
+    lam_g, lam_o = steklov_eigs(Sg, M, 16), steklov_eigs(out["S"], M, 16)
+    assert abs(lam_g[0]) < 1e-4
+    assert np.abs(lam_g - lam_o).max() < 0.03
+    for l, sl in ((1, slice(1, 4)), (2, slice(4, 9)), (3, slice(9, 16))):
+        assert abs(lam_g[sl].mean() / l - 1) < 0.12, (l, lam_g[sl])
+    assert np.linalg.eigvalsh(Sg).min() > -1e-5 * np.abs(Sg).max()          # PSD
+
+
+def test_exterior_with_killing_icosphere_l2(api):
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 4, seed=0)
+    gp, op = _params(api, seed=7, walks_per_sample=128, eps=1e-3, include_killing=True,
+                     n_kill_walks=162 * 512, kelvin_origin=(0.2, -0.1, 0.1))
+    bvh, S = _setup(api, v, f, smp)
+    Sg, st = api.estimate_dtn_exterior(bvh, S, gp, want_stats=True)
+    assert torch.equal(Sg, api.estimate_dtn_exterior(bvh, S, gp))
+    Sg = Sg.cpu().numpy().astype(np.float64)
+    assert np.array_equal(Sg, Sg.T)
+    orc = Oracle(mesh_geom(v, f))
+    out = orc.estimate_dtn(op, True, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    _assert_within_4se(Sg, out, smp, f)
+    M = orc.mass_matrix()
+    lam = steklov_eigs(Sg, M, 9)
+    assert abs(lam[0] - 1.0) < 0.08                      # l + 1 with l = 0
+    assert abs(lam[1:4].mean() - 2.0) < 0.2
+    # killing off: constants are annihilated again
+    gp.include_killing = False
+    S0 = api.estimate_dtn_exterior(bvh, S, gp).cpu().numpy().astype(np.float64)
+    assert np.abs(S0.sum(1)).max() < 5e-5 * np.abs(S0).max()
+
+
+def test_interior_does_not_couple_components_exterior_does(api):
+    """PAPER.md:50, 303-309; SURVEY.md 8(c) 'Coupling'."""
+    va, fa = icosphere(2, 1.0, (-1.25, 0, 0))
+    vb, fb = icosphere(2, 1.0, (+1.25, 0, 0))
+    v, f = merge_meshes([(va, fa), (vb, fb)])[:2]
+    smp = vertex_cell_samples(v, f, 2, seed=0)
+    bvh, S = _setup(api, v, f, smp)
+    gp = api.Params(seed=1, walks_per_sample=64, eps=1e-3, kelvin_origin=(-1.25, 0, 0))
+    nA = len(va)
+    Si = api.estimate_dtn_interior(bvh, S, gp).cpu().numpy()
+    assert (Si[:nA, nA:] == 0).all() and (Si[nA:, :nA] == 0).all()
+    Se = api.estimate_dtn_exterior(bvh, S, gp).cpu().numpy()
+    assert np.linalg.norm(Se[:nA, nA:]) > 1e-3 * np.linalg.norm(Se)
+
+
+def test_stress_mesh_subset_against_oracle(api):
+    """In-the-wild style mesh (slivers, duplicates, flips, many components): records agree
+    with the brute-force oracle walk for walk; the matrix is symmetric and reproducible."""
+    v, f, info = stress_mesh(n_faces=6000, n_components=6, seed=3)
+    smp = uniform_samples(v, f, 256, seed=8)
+    gp, op = _params(api, seed=4, walks_per_sample=16, eps=1e-3, max_steps=256)
+    _compare_records(api, v, f, smp, False, gp, op, min_same=0.95)
+    bvh, S = _setup(api, v, f, smp)
+    A = api.estimate_dtn_interior(bvh, S, gp)
+    assert torch.equal(A, api.estimate_dtn_interior(bvh, S, gp)) and torch.equal(A, A.T)
+
+
+def test_estimator_argument_errors(api):
+    v, f = icosphere(1)
+    smp = vertex_cell_samples(v, f, 1, seed=0)
+    bvh, S = _setup(api, v, f, smp)
+    for bad in (dict(eps=0.0), dict(walks_per_sample=0), dict(cap_half_angle_deg=0.0), dict(bisection_iters=0)):
+        with pytest.raises(api.McsError) as e:
+            api.estimate_dtn_interior(bvh, S, api.Params(**{**dict(walks_per_sample=2), **bad}))
+        assert e.value.code == api.MCS_EINVAL
+    with pytest.raises(api.McsError) as e:                # workspace too small
+        api.estimate_dtn_interior(bvh, S, api.Params(walks_per_sample=2), workspace=torch.empty(16, dtype=torch.uint8, device="cuda"),
+                                  _exact_workspace=True)
+    assert e.value.code == api.MCS_ENOMEM
+    badS = api.Samples.from_arrays(np.full_like(smp["tri"], len(f)), smp["bary"], smp["weight"])
+    with pytest.raises(api.McsError) as e:                # sample face out of range
+        api.estimate_dtn_interior(bvh, badS, api.Params(walks_per_sample=2))
+    assert e.value.code == api.MCS_EINVAL
+    with pytest.raises(api.McsError) as e:                # Kelvin origin on a vertex
+        api.estimate_dtn_exterior(bvh, S, api.Params(walks_per_sample=2, kelvin_origin=tuple(float(x) for x in v[0])))
+    assert e.value.code == api.MCS_EDEGENERATE
