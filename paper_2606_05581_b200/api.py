@@ -181,8 +181,8 @@ class Bvh:
 
     def __del__(self):
         h = getattr(self, "_h", None)
-        if h is not None and h.value:
-            lib().mcs_free_bvh(h)
+        if h is not None and h.value and _lib is not None:       # _lib is None at interpreter shutdown
+            _lib.mcs_free_bvh(h)
             self._h = C.c_void_p(0)
 
     @property

@@ -48,49 +48,64 @@ __device__ __forceinline__ float origin_to_segment(float3 a, float3 b, float& t)
     return dot3(c, c);
 }
 
-// Closest point of triangle (a, b, c) to p: Voronoi-region classification
-// (vertex / edge / face), computed on the triangle translated by -p.
+// a*b - c*d with the rounding error of c*d compensated through an FMA (Kahan's
+// difference of products): the result is within ~1.5 ulp of the exact value even under
+// heavy cancellation.  Used for the face normal, so that sliver triangles (aspect
+// ratio > 100, BASELINE.json config 3) keep an accurate supporting plane.
+__device__ __forceinline__ float diff_of_products(float a, float b, float c, float d)
+{
+    const float cd = __fmul_rn(c, d);
+    const float err = __fmaf_rn(-c, d, cd);
+    const float r = __fmaf_rn(a, b, -cd);
+    return __fadd_rn(r, err);
+}
+
+// Closest point of triangle (a, b, c) to p, computed on the triangle translated by -p
+// (A, B, C = vertices seen from p, so every rounding error scales with the distance to
+// the triangle, not with the absolute coordinates):
+//   n = ab x ac (compensated), q = projection of p on the plane = ((A.n)/|n|^2) n,
+//   edge functions w_b = ((C-q) x (A-q)).n, w_c = ((A-q) x (B-q)).n, w_a = |n|^2 - w_b - w_c
+//   (|n|^2-scaled barycentrics of q).  All >= 0: the answer is q.  Otherwise the closest
+//   point lies on an edge whose edge function is negative (at most two): clamp onto those.
+// Removing the normal component before forming the edge functions keeps them accurate for
+// far-away p; the compensated normal keeps them accurate for slivers.
 // Returns the squared distance; (v, w) are the weights of b and c.
-// Zero-area faces (|ab x ac|^2 <= 1e-12 max|e|^4 in fp32) fall back to their three
-// edges (R16).
+// Zero-area faces (|ab x ac|^2 <= 1e-12 max|e|^4) fall back to their three edges
+// (R16).
 __device__ __forceinline__ float closest_point_triangle(float3 p, float3 a, float3 b, float3 c, float& v, float& w)
 {
     const float3 ab = b - a, ac = c - a;
-    const float3 pa = a - p, pb = b - p, pc = c - p;       // vertices seen from p
-    const float3 nrm = cross3(ab, ac);
+    const float3 A = a - p, B = b - p, C = c - p;
+    const float3 n = f3(diff_of_products(ab.y, ac.z, ab.z, ac.y),
+                        diff_of_products(ab.z, ac.x, ab.x, ac.z),
+                        diff_of_products(ab.x, ac.y, ab.y, ac.x));
+    const float nn = dot3(n, n);
     const float e2 = fmaxf(dot3(ab, ab), dot3(ac, ac));
-    if (dot3(nrm, nrm) <= 1e-12f * e2 * e2) {
-        float t, best, d;
-        best = origin_to_segment(pa, pb, t); v = t; w = 0.0f;
-        d = origin_to_segment(pb, pc, t); if (d < best) { best = d; v = 1.0f - t; w = t; }
-        d = origin_to_segment(pc, pa, t); if (d < best) { best = d; v = 0.0f; w = 1.0f - t; }
+    float t, best, d;
+    if (nn <= 1e-12f * e2 * e2) {
+        best = origin_to_segment(A, B, t); v = t; w = 0.0f;
+        d = origin_to_segment(B, C, t); if (d < best) { best = d; v = 1.0f - t; w = t; }
+        d = origin_to_segment(C, A, t); if (d < best) { best = d; v = 0.0f; w = 1.0f - t; }
         return best;
     }
-    // d1 = ab.(p-a) = -ab.pa, ...
-    const float d1 = -dot3(ab, pa), d2 = -dot3(ac, pa);
-    const float d3 = -dot3(ab, pb), d4 = -dot3(ac, pb);
-    const float d5 = -dot3(ab, pc), d6 = -dot3(ac, pc);
-    const float vc = d1 * d4 - d3 * d2;
-    const float vb = d5 * d2 - d1 * d6;
-    const float va = d3 * d6 - d5 * d4;
-    float vv, ww;
-    if (d1 <= 0.0f && d2 <= 0.0f) { vv = 0.0f; ww = 0.0f; }                                   // vertex a
-    else if (d3 >= 0.0f && d4 <= d3) { vv = 1.0f; ww = 0.0f; }                                // vertex b
-    else if (vc <= 0.0f && d1 >= 0.0f && d3 <= 0.0f) { vv = d1 / (d1 - d3); ww = 0.0f; }      // edge ab
-    else if (d6 >= 0.0f && d5 <= d6) { vv = 0.0f; ww = 1.0f; }                                // vertex c
-    else if (vb <= 0.0f && d2 >= 0.0f && d6 <= 0.0f) { vv = 0.0f; ww = d2 / (d2 - d6); }      // edge ac
-    else if (va <= 0.0f && (d4 - d3) >= 0.0f && (d5 - d6) >= 0.0f) {                          // edge bc
-        ww = (d4 - d3) / ((d4 - d3) + (d5 - d6)); vv = 1.0f - ww;
-    } else {                                                                                  // face
-        const float denom = 1.0f / (va + vb + vc);
-        vv = fminf(fmaxf(vb * denom, 0.0f), 1.0f);
-        ww = fminf(fmaxf(vc * denom, 0.0f), 1.0f - vv);
+    const float rnn = 1.0f / nn;
+    const float An = dot3(A, n);
+    const float hq = An * rnn;
+    const float3 q = f3(hq * n.x, hq * n.y, hq * n.z);
+    const float3 Aq = A - q, Bq = B - q, Cq = C - q;
+    const float wb = dot3(cross3(Cq, Aq), n);
+    const float wc = dot3(cross3(Aq, Bq), n);
+    const float wa = nn - wb - wc;
+    if (wa >= 0.0f && wb >= 0.0f && wc >= 0.0f) {                 // face
+        v = fminf(wb * rnn, 1.0f);
+        w = fminf(wc * rnn, 1.0f - v);
+        return An * hq;
     }
-    v = vv; w = ww;
-    const float3 q = f3(fmaf(vv, ab.x, fmaf(ww, ac.x, pa.x)),
-                        fmaf(vv, ab.y, fmaf(ww, ac.y, pa.y)),
-                        fmaf(vv, ab.z, fmaf(ww, ac.z, pa.z)));
-    return dot3(q, q);
+    best = CUDART_INF_F;
+    if (wc < 0.0f) { best = origin_to_segment(A, B, t); v = t; w = 0.0f; }                                    // edge ab
+    if (wa < 0.0f) { d = origin_to_segment(B, C, t); if (d < best) { best = d; v = 1.0f - t; w = t; } }       // edge bc
+    if (wb < 0.0f) { d = origin_to_segment(C, A, t); if (d < best) { best = d; v = 0.0f; w = 1.0f - t; } }    // edge ca
+    return best;
 }
 
 __device__ __forceinline__ float box_dist2(float3 p, float lx, float ly, float lz, float hx, float hy, float hz)
@@ -132,6 +147,12 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
     int sp = 0;
     int node = 0;
     const float bound0 = h.d2;
+    // A sub-tree is pruned when its box is farther than the best distance by more than a
+    // few ulps: the fp32 box distance of a face's own leaf may round above the fp32
+    // distance to the face, and an equal-distance face with a smaller index must still
+    // be reached for the tie rule to hold.
+    const float SLACK = 1.0f + 4e-6f;
+    float lim = h.d2 * SLACK;
     for (;;) {
         const float4* nd = reinterpret_cast<const float4*>(nodes + node);
         const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
@@ -140,15 +161,15 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
         const float d0 = box_dist2(p, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y);
         const float d1 = box_dist2(p, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
         const int c0 = w3.x, c1 = w3.y;
-        bool go0 = d0 <= h.d2, go1 = d1 <= h.d2;
-        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h); if (COUNT) cnt.tris++; go0 = false; }
+        bool go0 = d0 <= lim, go1 = d1 <= lim;
+        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h); if (COUNT) cnt.tris++; go0 = false; lim = h.d2 * SLACK; }
         if (go1 && c1 < 0) {
-            if (d1 <= h.d2) { test_triangle(tris, ~c1, p, h); if (COUNT) cnt.tris++; }
+            if (d1 <= lim) { test_triangle(tris, ~c1, p, h); if (COUNT) cnt.tris++; lim = h.d2 * SLACK; }
             go1 = false;
         }
         if (ANY && h.d2 < bound0) return;
-        go0 = go0 && d0 <= h.d2;
-        go1 = go1 && d1 <= h.d2;
+        go0 = go0 && d0 <= lim;
+        go1 = go1 && d1 <= lim;
         if (go0 && go1) {
             const bool swap = d1 < d0;
             const int nearc = swap ? c1 : c0, farc = swap ? c0 : c1;
@@ -162,7 +183,7 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
             bool found = false;
             while (sp > 0) {
                 --sp;
-                if (stack_d[sp] <= h.d2) { node = stack_n[sp]; found = true; break; }
+                if (stack_d[sp] <= lim) { node = stack_n[sp]; found = true; break; }
             }
             if (!found) return;
         }
