@@ -181,6 +181,23 @@ int mcs_estimate_dtn_exterior(const mcs_bvh* bvh, const mcs_samples* samples, co
                               const mcs_params* params, void* workspace, size_t workspace_bytes,
                               const mcs_matrix* out, mcs_stats* host_stats, void* stream);
 
+/*
+ * The whole path from HOST buffers, for callers that keep their data on the CPU
+ * (and for the end-to-end measurement): uploads the mesh and the samples,
+ * builds the LBVH, runs the requested estimators (operators: bit 0 = interior,
+ * bit 1 = exterior) and downloads the dense K x K matrices (K = V, hat basis).
+ * EVERY pointer here is a HOST pointer, including those inside `samples`
+ * (pinned memory makes the copies asynchronous but is not required);
+ * out_interior / out_exterior are [V][V] fp32 and may be NULL when their bit is
+ * clear.  Device memory is allocated and freed inside the call (stream-ordered);
+ * the call blocks until the results are in the host buffers.  `stats` (host,
+ * may be NULL) receives the counters of the LAST operator run.
+ * Errors: as mcs_build_bvh and mcs_estimate_dtn_*.
+ */
+int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                          const mcs_samples* samples, const mcs_params* params, int operators,
+                          float* out_interior, float* out_exterior, mcs_stats* stats, void* stream);
+
 /* ------------------------------------------------------------------------ */
 /* Test / benchmark hooks for the individual steps of SURVEY.md 8(a).         */
 /* ------------------------------------------------------------------------ */
@@ -238,6 +255,13 @@ typedef struct {
 unsigned long long mcs_launch_count(void);
 int mcs_profile_enable(int on);
 int mcs_profile_last(mcs_phase_times* out /* host */);
+
+/* Roofline denominators measured on this device (bench.py): FP32
+ * CUDA-core throughput of independent FMA chains (TFLOP/s, 2 flop per FMA) and the read
+ * bandwidth of a 24 MiB L2-resident buffer with 16-byte loads (GB/s).  Each allocates a
+ * scratch buffer, times 6 launches with CUDA events on `stream`, returns the best, blocks. */
+int mcs_measure_fp32_tflops(double* tflops /* host */, void* stream);
+int mcs_measure_l2_gbs(double* gbs /* host */, void* stream);
 
 const char* mcs_error_string(int code);
 const char* mcs_version(void);

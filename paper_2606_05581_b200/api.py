@@ -276,6 +276,45 @@ def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats
                      want_stats, out, workspace, _exact_workspace)
 
 
+def estimate_dtn_host(verts, faces, tri, bary, weight, params: Params, interior=True, exterior=True,
+                      out_interior=None, out_exterior=None, normal=None, want_stats=False, device=None):
+    """The whole path from HOST tensors (mcs_estimate_dtn_host): upload, LBVH build, estimators,
+    download.  Inputs are CPU tensors (pinned memory makes the copies asynchronous); the results are
+    written into CPU tensors [V,V] (allocated pinned when not given)."""
+    def host(t, dtype, name):
+        t = torch.as_tensor(t)
+        if t.is_cuda:
+            raise ValueError(f"{name} must be a CPU tensor for the host entry point")
+        return t.to(dtype).contiguous()
+    verts, faces = host(verts, torch.float32, "verts"), host(faces, torch.int32, "faces")
+    tri, bary, weight = host(tri, torch.int32, "tri"), host(bary, torch.float32, "bary"), host(weight, torch.float32, "weight")
+    normal = host(normal, torch.float32, "normal") if normal is not None else None
+    V, F, n_s = int(verts.shape[0]), int(faces.shape[0]), int(tri.shape[0])
+    ops = (1 if interior else 0) | (2 if exterior else 0)
+    if interior and out_interior is None:
+        out_interior = torch.empty((V, V), dtype=torch.float32, pin_memory=True)
+    if exterior and out_exterior is None:
+        out_exterior = torch.empty((V, V), dtype=torch.float32, pin_memory=True)
+    cs = _Samples(tri=tri.data_ptr(), bary=bary.data_ptr(), weight=weight.data_ptr(),
+                  normal=normal.data_ptr() if normal is not None else None, n_s=n_s)
+    cp = params.c()
+    st = Stats() if want_stats else None
+    dev = torch.device("cuda" if device is None else device)
+    with torch.cuda.device(dev):
+        rc = lib().mcs_estimate_dtn_host(_ptr(verts), C.c_int64(V), _ptr(faces), C.c_int64(F), C.byref(cs), C.byref(cp),
+                                         C.c_int(ops), _ptr(out_interior) if interior else None,
+                                         _ptr(out_exterior) if exterior else None,
+                                         C.byref(st) if st is not None else None, _stream(dev))
+    _check(rc, "mcs_estimate_dtn_host")
+    h2d = verts.numel() * 4 + faces.numel() * 4 + n_s * 20 + (n_s * 12 if normal is not None else 0)
+    d2h = (int(interior) + int(exterior)) * V * V * 4
+    res = dict(interior=out_interior if interior else None, exterior=out_exterior if exterior else None,
+               h2d_bytes=h2d, d2h_bytes=d2h)
+    if want_stats:
+        res["stats"] = st
+    return res
+
+
 def tangent_balls(bvh: Bvh, samples: Samples, params: Params, exterior: bool):
     cs, cp = samples.c(), params.c()
     balls = torch.empty((samples.n_s, 8), dtype=torch.float32, device=bvh.device)
@@ -373,3 +412,17 @@ def profile_last() -> PhaseTimes:
 
 def version() -> str:
     return lib().mcs_version().decode()
+
+
+def measure_fp32_tflops(device="cuda") -> float:
+    o = C.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(lib().mcs_measure_fp32_tflops(C.byref(o), _stream(torch.device(device))), "mcs_measure_fp32_tflops")
+    return o.value
+
+
+def measure_l2_gbs(device="cuda") -> float:
+    o = C.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(lib().mcs_measure_l2_gbs(C.byref(o), _stream(torch.device(device))), "mcs_measure_l2_gbs")
+    return o.value

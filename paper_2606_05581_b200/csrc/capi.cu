@@ -139,6 +139,71 @@ extern "C" int mcs_estimate_dtn_exterior(const mcs_bvh* b, const mcs_samples* s,
     return estimate(b, s, basis, p, 1, ws, ws_bytes, out, hs, stream);
 }
 
+extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                                     const mcs_samples* hs, const mcs_params* p, int operators,
+                                     float* out_interior, float* out_exterior, mcs_stats* stats, void* stream)
+{
+    if (stats) memset(stats, 0, sizeof *stats);
+    if (!verts || !faces || !hs || !p || V < 1 || F < 1 || hs->n_s < 1) return MCS_EINVAL;
+    if (!hs->tri || !hs->bary || !hs->weight) return MCS_EINVAL;
+    if ((operators & 3) == 0 || (operators & ~3)) return MCS_EINVAL;
+    if (((operators & 1) && !out_interior) || ((operators & 2) && !out_exterior)) return MCS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n_s = hs->n_s;
+    const size_t nb_v = (size_t)V * 12, nb_f = (size_t)F * 12, nb_m = (size_t)V * V * 4;
+    const size_t nb_tri = (size_t)n_s * 4, nb_bary = (size_t)n_s * 12, nb_w = (size_t)n_s * 4;
+    const size_t nb_n = hs->normal ? (size_t)n_s * 12 : 0;
+    // one staging block: verts | faces | tri | bary | weight | normal
+    size_t off_v = 0, off_f = align_up(off_v + nb_v), off_t = align_up(off_f + nb_f), off_b = align_up(off_t + nb_tri),
+           off_w = align_up(off_b + nb_bary), off_n = align_up(off_w + nb_w), in_total = align_up(off_n + nb_n) + 256;
+    char* d_in = nullptr; float* d_out = nullptr; void* d_ws = nullptr;
+    mcs_bvh* bvh = nullptr;
+    int rc = MCS_OK;
+    cudaError_t e = cudaMallocAsync((void**)&d_in, in_total, st);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&d_out, nb_m, st);
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+    e = cudaMemcpyAsync(d_in + off_v, verts, nb_v, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_f, faces, nb_f, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_t, hs->tri, nb_tri, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_b, hs->bary, nb_bary, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_w, hs->weight, nb_w, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && nb_n) e = cudaMemcpyAsync(d_in + off_n, hs->normal, nb_n, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; goto done; }
+    rc = mcs_build_bvh((const float*)(d_in + off_v), V, (const int32_t*)(d_in + off_f), F, nullptr, stream, &bvh);
+    if (rc != MCS_OK) goto done;
+    {
+        mcs_samples ds;
+        ds.tri = (const int32_t*)(d_in + off_t); ds.bary = (const float*)(d_in + off_b);
+        ds.weight = (const float*)(d_in + off_w); ds.normal = nb_n ? (const float*)(d_in + off_n) : nullptr;
+        ds.n_s = n_s;
+        mcs_basis basis; basis.kind = 0; basis.pad_ = 0; basis.K = V;
+        mcs_matrix m; m.kind = 0; m.pad_ = 0; m.K = V; m.dense = d_out;
+        size_t need = 0;
+        for (int ext = 0; ext < 2; ++ext)
+            if (operators & (1 << ext)) {
+                const size_t b = make_layout(bvh, &ds, &basis, p, ext, true, true).total;
+                need = b > need ? b : need;
+            }
+        e = cudaMallocAsync(&d_ws, need, st);
+        if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+        for (int ext = 0; ext < 2 && rc == MCS_OK; ++ext) {
+            if (!(operators & (1 << ext))) continue;
+            rc = estimate(bvh, &ds, &basis, p, ext, d_ws, need, &m, stats, stream);
+            if (rc != MCS_OK) break;
+            e = cudaMemcpyAsync(ext ? out_exterior : out_interior, d_out, nb_m, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+        }
+    }
+done:
+    if (d_ws) cudaFreeAsync(d_ws, st);
+    if (d_out) cudaFreeAsync(d_out, st);
+    if (d_in) cudaFreeAsync(d_in, st);
+    e = cudaStreamSynchronize(st);
+    if (rc == MCS_OK && e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+    if (bvh) mcs_free_bvh(bvh);
+    return fail(rc, stats);
+}
+
 extern "C" int mcs_tangent_balls(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
                                  float* balls, void* stream)
 {
