@@ -146,6 +146,7 @@ typedef struct {                 /* host; filled when passed non-NULL (forces a 
     int64_t n_nodes_visited, n_tris_tested;   /* traversal work actually done (flop/byte model)    */
     int64_t n_entries, n_unique;          /* (row,col,value) records expanded / after reduction    */
     int64_t workspace_needed;             /* bytes; set on MCS_ENOMEM too                           */
+    int64_t nodes_hist[16];               /* walk-kernel queries by floor(log2(nodes visited)), bin 15 = rest */
     int32_t cuda_error;                   /* cudaError_t on MCS_ECUDA                               */
     int32_t pad_;
 } mcs_stats;

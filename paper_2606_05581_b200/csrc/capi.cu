@@ -58,6 +58,7 @@ void fill_stats(mcs_stats* hs, const unsigned long long* h, const mcs_samples* s
     hs->n_tris_tested = (int64_t)h[ST_TRIS];
     hs->n_entries = (int64_t)h[ST_ENTRIES];
     hs->n_unique = (int64_t)h[ST_UNIQUE];
+    for (int b = 0; b < 16; ++b) hs->nodes_hist[b] = (int64_t)h[ST_HIST + b];
 }
 
 int fail(int rc, mcs_stats* hs)

@@ -206,22 +206,57 @@ __device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& 
     e2 = f3(b, sign + n.y * n.y * a, -n.y);
 }
 
-struct LaneWalk {
-    float3 x;          // interior: position; exterior: Kelvin coordinates y about the origin
-    float  wfac;       // weight without the exit-point factor
-    unsigned sample, walk;
-    int    k;          // jumps taken so far
-    int    slot_hi, slot_lo;   // record slot (64-bit split)
-    int    prev;       // sorted slot of the last closest triangle (-1: none)
+// ---------------------------------------------------------------------------
+// The walk kernel: a per-lane state machine with warp-level phase voting.
+//
+// Every lane owns one walk and, inside it, one closest-point query.  A query is a
+// stack of pending items (inner nodes and leaves of the LBVH, each with the fp32
+// squared distance of its box); the lane's next item decides what KIND of work it
+// wants to do:   NODE (visit an inner node: two box tests, push the far child),
+// TRI (one point-triangle test), TRANS (the query is finished: terminate the walk or
+// take the next WoS jump, refill from the work queue, start the next query).
+// Each pass of the single loop the warp votes and executes ONE kind, the one most
+// lanes wait for; the others keep their state and wait.  No lane ever waits for
+// another lane's query to finish, so a query near the medial axis that visits a
+// thousand nodes costs its own lane only (wavefront compaction at the granularity of
+// single node visits).  What a lane computes does not depend on the vote, so results
+// are independent of the schedule.
+//
+// The traversal stack lives in shared memory ([depth][thread]: a lane always hits its
+// own bank); entries beyond WSTACK spill to local memory (deep LBVH chains only).
+// ---------------------------------------------------------------------------
+constexpr int WSTACK = 24;                       // shared-memory stack entries per lane
+constexpr int CUR_NONE = INT_MIN;
+
+struct LaneStack {
+    int*   s_ref;      // shared: [WSTACK][WT], this lane's column
+    float* s_d;
+    int    l_ref[MCS_STACK - WSTACK];            // local-memory spill
+    float  l_d[MCS_STACK - WSTACK];
 };
 
-// ---------------------------------------------------------------------------
-// The walk kernel.
-// ---------------------------------------------------------------------------
+__device__ __forceinline__ void stack_push(LaneStack& st, int& sp, int ref, float d)
+{
+    if (sp < WSTACK) { st.s_ref[sp * WT] = ref; st.s_d[sp * WT] = d; }
+    else if (sp < MCS_STACK) { st.l_ref[sp - WSTACK] = ref; st.l_d[sp - WSTACK] = d; }
+    ++sp;                                        // sp > MCS_STACK cannot happen: depth <= 63 + log2(F)
+}
+
+__device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, float& d)
+{
+    --sp;
+    if (sp < WSTACK) { ref = st.s_ref[sp * WT]; d = st.s_d[sp * WT]; }
+    else { ref = st.l_ref[sp - WSTACK]; d = st.l_d[sp - WSTACK]; }
+}
+
+enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
+
 template <bool EXT, bool COUNT>
 __global__ void __launch_bounds__(WT)
 walk_kernel(WalkGeom g, WalkArgs a)
 {
+    __shared__ int   sh_ref[WSTACK * WT];
+    __shared__ float sh_d[WSTACK * WT];
     const unsigned FULL = 0xFFFFFFFFu;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -229,146 +264,213 @@ walk_kernel(WalkGeom g, WalkArgs a)
     const long long n_main = a.n_s * a.W;
     const uint2 key = make_uint2(a.key0, a.key1);
     const float3 o = f3(a.ox, a.oy, a.oz);
+    const float SLACK = 1.0f + 4e-6f;            // see bvh_closest_point
+
+    LaneStack stk;
+    stk.s_ref = sh_ref + threadIdx.x;
+    stk.s_d = sh_d + threadIdx.x;
 
     long long chunk_cur = 0, chunk_end = 0;      // warp-uniform
-    bool exhausted = false;
-    bool active = false;
-    float3 x = f3(0.f, 0.f, 0.f);
+    bool exhausted = false;                      // warp-uniform
+    // walk state
+    bool busy = false;                           // lane owns a walk
+    float3 x = f3(0.f, 0.f, 0.f);                // interior: position; exterior: Kelvin coordinates y
     float wfac = 0.f;
     unsigned sample = 0, walk = 0;
     int k = 0, prev = -1;
     long long slot = 0;
-    TraversalCounters cnt; cnt.nodes = 0; cnt.tris = 0;
+    // query state
+    float3 xq = f3(0.f, 0.f, 0.f);
+    float rho = 0.f, far_radius = -1.0f;         // far_radius >= 0: jump radius known without a query (exterior far field)
+    ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.f;
+    float lim = CUDART_INF_F;
+    int cur = CUR_NONE, sp = 0;
+    // statistics
+    unsigned n_nodes = 0, n_tris = 0, q_nodes = 0;
     unsigned n_steps = 0, n_queries = 0, n_trunc = 0;
 
     for (;;) {
-        // ---- refill idle lanes from the warp's chunk ------------------------
-        unsigned idle = __ballot_sync(FULL, !active);
-        while (idle != 0 && !exhausted) {
-            if (chunk_cur >= chunk_end) {
-                long long base = 0;
-                if (lane == 0) base = (long long)atomicAdd(a.work_counter, (unsigned long long)a.chunk);
-                base = __shfl_sync(FULL, base, 0);
-                if (base >= total) { exhausted = true; break; }
-                chunk_cur = base;
-                chunk_end = base + a.chunk < total ? base + a.chunk : total;
+        // ---- next item of every lane that has none --------------------------------
+        if (busy && cur == CUR_NONE) {
+            while (sp > 0) {
+                int ref; float d;
+                stack_pop(stk, sp, ref, d);
+                if (d <= lim) { cur = ref; break; }
             }
-            const int avail = (int)(chunk_end - chunk_cur);
-            const int n_idle = __popc(idle);
-            const int rank = __popc(idle & lt);
-            if (!active && rank < avail) {
-                const long long j = chunk_cur + rank;
-                active = true; k = 0; prev = -1;
-                if (j < n_main) {
-                    const long long pos = j / a.W;
-                    walk = (unsigned)(j - pos * a.W);
-                    sample = a.order[pos];
-                    slot = (long long)sample * a.W + walk;
-                    const float4 b0 = __ldg(&a.balls[2 * (long long)sample]);
-                    const float4 b1 = __ldg(&a.balls[2 * (long long)sample + 1]);
-                    const float r = b0.w;
-                    if (!(r > 0.0f)) {                               // discarded sample
-                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                        if (a.steps) a.steps[slot] = -2;
-                        active = false;
-                    } else {
-                        // SampleBallSurface + BallJumpKernel (Eq. 23; R5-R7)
-                        const unsigned wq = a.antithetic ? (walk >> 1) : walk;
-                        const uint4 rn = philox4x32_10(make_uint4(sample, wq, 0u, MCS_PURPOSE_INIT), key);
-                        const float u1 = u01(rn.x), u2 = u01(rn.y);
-                        float q, factor;
-                        if (a.importance) {
-                            q = 1.0f / (a.inv_q0 - u1 * (a.inv_q0 - 1.0f));
-                            factor = (1.0f / (4.0f * r)) * (a.inv_q0 - 1.0f);
-                        } else {
-                            q = sqrtf(u1);
-                            factor = (q < a.q0) ? 0.0f : 1.0f / (8.0f * r * q * q * q);
-                        }
-                        const float ct = 1.0f - 2.0f * q * q;
-                        const float st = 2.0f * q * sqrtf(fmaxf(0.0f, 1.0f - q * q));
-                        float sphi, cphi;
-                        sincospif(2.0f * u2 + ((a.antithetic && (walk & 1u)) ? 1.0f : 0.0f), &sphi, &cphi);
-                        const float3 pole = f3(b1.x, b1.y, b1.z);
-                        float3 e1, e2;
-                        frame_from_normal(pole, e1, e2);
-                        x = f3(b0.x + r * (ct * pole.x + st * (cphi * e1.x + sphi * e2.x)),
-                               b0.y + r * (ct * pole.y + st * (cphi * e1.y + sphi * e2.y)),
-                               b0.z + r * (ct * pole.z + st * (cphi * e1.z + sphi * e2.z)));
-                        wfac = (__ldg(&a.weight[sample]) / (float)a.W) * factor;
-                        if (EXT) wfac *= b1.w * b1.w * b1.w;          // |s*|^3, Eq. 32
-                        prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
-                    }
-                } else {                                             // killing walk from kappa(inf) = 0
-                    sample = MCS_KILLING_SAMPLE;
-                    walk = (unsigned)(j - n_main);
-                    slot = j;
-                    x = f3(0.f, 0.f, 0.f);
-                    wfac = 4.0f * CUDART_PI_F / (float)a.n_kill;
-                }
-            }
-            chunk_cur += n_idle < avail ? n_idle : avail;
-            idle = __ballot_sync(FULL, !active);
         }
-        if (!__any_sync(FULL, active)) break;
+        const int kind = busy ? (cur == CUR_NONE ? KIND_TRANS : (cur >= 0 ? KIND_NODE : KIND_TRI))
+                              : (exhausted ? KIND_IDLE : KIND_TRANS);
+        const int n_node = __popc(__ballot_sync(FULL, kind == KIND_NODE));
+        const int n_tri = __popc(__ballot_sync(FULL, kind == KIND_TRI));
+        const int n_trans = __popc(__ballot_sync(FULL, kind == KIND_TRANS));
+        if (n_node + n_tri + n_trans == 0) break;
+        // vote: the kind most lanes wait for (ties: NODE, then TRI)
+        int which = KIND_NODE, best = n_node;
+        if (n_tri > best) { which = KIND_TRI; best = n_tri; }
+        if (n_trans > best) { which = KIND_TRANS; best = n_trans; }
 
-        // ---- one walk-on-spheres iteration (R9) ---
-        if (active) {
-            float3 xq = x;
-            float radius = 0.0f, rho = 0.0f;
-            bool need_query = true;
-            if (EXT) {
-                const float yn = sqrtf(dot3(x, x));
-                if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
-                    radius = 1.0f / a.Rmax - yn;
-                    need_query = false;
-                } else {
-                    const float inv = 1.0f / (yn * yn);
-                    xq = f3(fmaf(inv, x.x, o.x), fmaf(inv, x.y, o.y), fmaf(inv, x.z, o.z));
-                    rho = 1.0f / yn;
-                }
+        if (which == KIND_NODE) {
+            if (kind == KIND_NODE) {
+                const float4* nd = reinterpret_cast<const float4*>(g.nodes + cur);
+                const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
+                const int2 ch = __ldg(reinterpret_cast<const int2*>(nd + 3));
+                if (COUNT) { ++n_nodes; ++q_nodes; }
+                const float d0 = box_dist2(xq, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y);
+                const float d1 = box_dist2(xq, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
+                const bool go0 = d0 <= lim, go1 = d1 <= lim;
+                const bool swap = d1 < d0;
+                const int nearc = swap ? ch.y : ch.x, farc = swap ? ch.x : ch.y;
+                if (go0 && go1) { stack_push(stk, sp, farc, swap ? d0 : d1); cur = nearc; }
+                else if (go0) cur = ch.x;
+                else if (go1) cur = ch.y;
+                else cur = CUR_NONE;
             }
-            bool done = false;
-            if (need_query) {
-                ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
-                if (prev >= 0) { test_triangle(g.tris, prev, xq, h); if (COUNT) cnt.tris++; }
-                bvh_closest_point<COUNT, false>(g.nodes, g.tris, xq, h, cnt);
-                ++n_queries;
-                prev = h.k;
-                const float D = sqrtf(h.d2);
-                radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
-                if (radius < a.eps) {
-                    float wgt = wfac;
-                    if (EXT) {
-                        const float3 t = hit_point(g.tris, h) - o;
-                        wgt *= sqrtf(dot3(t, t));                    // 1/|t*| = |t - o|, Eq. 32
+        } else if (which == KIND_TRI) {
+            if (kind == KIND_TRI) {
+                test_triangle(g.tris, ~cur, xq, h);
+                if (COUNT) ++n_tris;
+                lim = h.d2 * SLACK;
+                cur = CUR_NONE;
+            }
+        } else {
+            // ---- (1) finished queries: terminate or jump (R9) ----
+            bool start_query = false;
+            if (busy && kind == KIND_TRANS) {
+                float radius;
+                bool done = false;
+                if (far_radius >= 0.0f) {
+                    radius = far_radius;
+                } else {
+                    ++n_queries;
+                    if (COUNT) { atomicAdd(&a.stats[ST_HIST + (q_nodes > 0 ? min(31 - __clz(q_nodes), 15) : 0)], 1ull); q_nodes = 0; }
+                    prev = h.k;
+                    const float D = sqrtf(h.d2);
+                    radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
+                    if (radius < a.eps) {
+                        float wgt = wfac;
+                        if (EXT) {
+                            const float3 t = hit_point(g.tris, h) - o;
+                            wgt *= sqrtf(dot3(t, t));                    // 1/|t*| = |t - o|, Eq. 32
+                        }
+                        a.records[slot] = make_float4(__int_as_float(h.tri), h.v, h.w, wgt);
+                        if (a.steps) a.steps[slot] = k;
+                        done = true;
                     }
-                    a.records[slot] = make_float4(__int_as_float(h.tri), h.v, h.w, wgt);
-                    if (a.steps) a.steps[slot] = k;
-                    done = true;
+                }
+                if (!done) {
+                    if (k == a.max_steps) {                              // DESIGN.md R10
+                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                        if (a.steps) a.steps[slot] = -1;
+                        ++n_trunc;
+                        done = true;
+                    } else {
+                        ++k; ++n_steps;
+                        const uint4 rn = philox4x32_10(make_uint4(sample, walk, (unsigned)k, MCS_PURPOSE_STEP), key);
+                        const float ct = 1.0f - 2.0f * u01(rn.x);
+                        const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+                        float sphi, cphi;
+                        sincospif(2.0f * u01(rn.y), &sphi, &cphi);
+                        x = f3(fmaf(radius, st * cphi, x.x), fmaf(radius, st * sphi, x.y), fmaf(radius, ct, x.z));
+                        start_query = true;
+                    }
+                }
+                if (done) busy = false;
+            }
+            // ---- (2) refill idle lanes from the warp's chunk of the work queue ------------
+            unsigned idle = __ballot_sync(FULL, !busy);
+            while (idle != 0 && !exhausted) {
+                if (chunk_cur >= chunk_end) {
+                    long long base = 0;
+                    if (lane == 0) base = (long long)atomicAdd(a.work_counter, (unsigned long long)a.chunk);
+                    base = __shfl_sync(FULL, base, 0);
+                    if (base >= total) { exhausted = true; break; }
+                    chunk_cur = base;
+                    chunk_end = base + a.chunk < total ? base + a.chunk : total;
+                }
+                const int avail = (int)(chunk_end - chunk_cur);
+                const int n_idle = __popc(idle);
+                const int rank = __popc(idle & lt);
+                if (!busy && rank < avail) {
+                    const long long j = chunk_cur + rank;
+                    busy = true; k = 0; prev = -1; start_query = true;
+                    if (j < n_main) {
+                        const long long pos = j / a.W;
+                        walk = (unsigned)(j - pos * a.W);
+                        sample = a.order[pos];
+                        slot = (long long)sample * a.W + walk;
+                        const float4 b0 = __ldg(&a.balls[2 * (long long)sample]);
+                        const float4 b1 = __ldg(&a.balls[2 * (long long)sample + 1]);
+                        const float r = b0.w;
+                        if (!(r > 0.0f)) {                               // discarded sample
+                            a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                            if (a.steps) a.steps[slot] = -2;
+                            busy = false; start_query = false;
+                        } else {
+                            // SampleBallSurface + BallJumpKernel (Eq. 23; R5-R7)
+                            const unsigned wq = a.antithetic ? (walk >> 1) : walk;
+                            const uint4 rn = philox4x32_10(make_uint4(sample, wq, 0u, MCS_PURPOSE_INIT), key);
+                            const float u1 = u01(rn.x), u2 = u01(rn.y);
+                            float q, factor;
+                            if (a.importance) {
+                                q = 1.0f / (a.inv_q0 - u1 * (a.inv_q0 - 1.0f));
+                                factor = (1.0f / (4.0f * r)) * (a.inv_q0 - 1.0f);
+                            } else {
+                                q = sqrtf(u1);
+                                factor = (q < a.q0) ? 0.0f : 1.0f / (8.0f * r * q * q * q);
+                            }
+                            const float ct = 1.0f - 2.0f * q * q;
+                            const float st = 2.0f * q * sqrtf(fmaxf(0.0f, 1.0f - q * q));
+                            float sphi, cphi;
+                            sincospif(2.0f * u2 + ((a.antithetic && (walk & 1u)) ? 1.0f : 0.0f), &sphi, &cphi);
+                            const float3 pole = f3(b1.x, b1.y, b1.z);
+                            float3 e1, e2;
+                            frame_from_normal(pole, e1, e2);
+                            x = f3(b0.x + r * (ct * pole.x + st * (cphi * e1.x + sphi * e2.x)),
+                                   b0.y + r * (ct * pole.y + st * (cphi * e1.y + sphi * e2.y)),
+                                   b0.z + r * (ct * pole.z + st * (cphi * e1.z + sphi * e2.z)));
+                            wfac = (__ldg(&a.weight[sample]) / (float)a.W) * factor;
+                            if (EXT) wfac *= b1.w * b1.w * b1.w;          // |s*|^3, Eq. 32
+                            prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
+                        }
+                    } else {                                             // killing walk from kappa(inf) = 0
+                        sample = MCS_KILLING_SAMPLE;
+                        walk = (unsigned)(j - n_main);
+                        slot = j;
+                        x = f3(0.f, 0.f, 0.f);
+                        wfac = 4.0f * CUDART_PI_F / (float)a.n_kill;
+                    }
+                }
+                chunk_cur += n_idle < avail ? n_idle : avail;
+                idle = __ballot_sync(FULL, !busy);
+            }
+            // ---- (3) set up the next closest-point query -------------------------------
+            if (start_query) {
+                xq = x; far_radius = -1.0f;
+                bool need_query = true;
+                if (EXT) {
+                    const float yn = sqrtf(dot3(x, x));
+                    if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
+                        far_radius = 1.0f / a.Rmax - yn;
+                        need_query = false;
+                    } else {
+                        const float inv = 1.0f / (yn * yn);
+                        xq = f3(fmaf(inv, x.x, o.x), fmaf(inv, x.y, o.y), fmaf(inv, x.z, o.z));
+                        rho = 1.0f / yn;
+                    }
+                }
+                h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
+                lim = CUDART_INF_F;
+                sp = 0; cur = CUR_NONE;
+                if (need_query) {
+                    if (prev >= 0) { stack_push(stk, sp, 0, 0.0f); cur = ~prev; }   // last closest face first: a tight bound
+                    else cur = 0;                                                   // root
                 }
             }
-            if (!done) {
-                if (k == a.max_steps) {                              // DESIGN.md R10
-                    a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                    if (a.steps) a.steps[slot] = -1;
-                    ++n_trunc;
-                    done = true;
-                } else {
-                    ++k; ++n_steps;
-                    const uint4 rn = philox4x32_10(make_uint4(sample, walk, (unsigned)k, MCS_PURPOSE_STEP), key);
-                    const float ct = 1.0f - 2.0f * u01(rn.x);
-                    const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-                    float sphi, cphi;
-                    sincospif(2.0f * u01(rn.y), &sphi, &cphi);
-                    x = f3(fmaf(radius, st * cphi, x.x), fmaf(radius, st * sphi, x.y), fmaf(radius, ct, x.z));
-                }
-            }
-            if (done) active = false;
         }
     }
 
     // ---- statistics ----------------------------------------------------------
-    unsigned vals[5] = { n_steps, n_queries, n_trunc, cnt.nodes, cnt.tris };
+    unsigned vals[5] = { n_steps, n_queries, n_trunc, n_nodes, n_tris };
     for (int q = 0; q < 5; ++q) {
         unsigned long long v = vals[q];
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);

@@ -6,7 +6,8 @@ enum {
     ST_WORK = 0,        // work-queue head of the persistent walk kernel
     ST_STEPS, ST_QUERIES, ST_TRUNCATED, ST_DISCARDED, ST_NODES, ST_TRIS,
     ST_ENTRIES, ST_UNIQUE,
-    ST_COUNT = 16
+    ST_HIST = 16,       // 16 bins: queries of the walk kernel by floor(log2(nodes visited))
+    ST_COUNT = 32
 };
 
 struct WalkGeom {
