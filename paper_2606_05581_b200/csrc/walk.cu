@@ -225,7 +225,7 @@ __device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& 
 // The traversal stack lives in shared memory ([depth][thread]: a lane always hits its
 // own bank); entries beyond WSTACK spill to local memory (deep LBVH chains only).
 // ---------------------------------------------------------------------------
-constexpr int WSTACK = 24;                       // shared-memory stack entries per lane
+constexpr int WSTACK = 16;                       // shared-memory stack entries per lane
 constexpr int CUR_NONE = INT_MIN;
 
 struct LaneStack {
@@ -300,11 +300,10 @@ walk_kernel(WalkGeom g, WalkArgs a)
         }
         const int kind = busy ? (cur == CUR_NONE ? KIND_TRANS : (cur >= 0 ? KIND_NODE : KIND_TRI))
                               : (exhausted ? KIND_IDLE : KIND_TRANS);
-        const int n_node = __popc(__ballot_sync(FULL, kind == KIND_NODE));
-        const int n_tri = __popc(__ballot_sync(FULL, kind == KIND_TRI));
-        const int n_trans = __popc(__ballot_sync(FULL, kind == KIND_TRANS));
-        if (n_node + n_tri + n_trans == 0) break;
+        const unsigned m0 = __ballot_sync(FULL, (kind & 1) != 0), m1 = __ballot_sync(FULL, (kind & 2) != 0);
+        if ((m0 | m1) == 0) break;
         // vote: the kind most lanes wait for (ties: NODE, then TRI)
+        const int n_node = __popc(m0 & ~m1), n_tri = __popc(m1 & ~m0), n_trans = __popc(m0 & m1);
         int which = KIND_NODE, best = n_node;
         if (n_tri > best) { which = KIND_TRI; best = n_tri; }
         if (n_trans > best) { which = KIND_TRANS; best = n_trans; }
