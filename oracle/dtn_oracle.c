@@ -15,7 +15,7 @@
  * in DESIGN.md ("Readings") and named here as [Rn].
  *
  * Pins (tests/test_oracle_*.py, all run without a GPU):
- *   philox4x32_10        cuRAND host generator + Random123 known answers
+ *   philox4x32_10        cuRAND host generator (independent implementation)
  *   closest point        second formulation + invariants + brute force
  *   tangent ball         closed forms (sphere, cube face)
  *   WoS                  martingale E[t] = z, Poisson kernel of the ball (Eq. 22)

@@ -1,20 +1,9 @@
 """Pins for the oracle's Philox4x32-10 and uniform mapping (no GPU)."""
 import ctypes as C
-import os
-
 import numpy as np
 import pytest
 
 from oracle import philox4x32_10, u01
-
-
-def test_known_answers(golden_dir):
-    rows = [l.split() for l in open(os.path.join(golden_dir, "philox4x32_10_kat.txt"))
-            if l.strip() and not l.startswith("#")]
-    assert len(rows) == 3
-    for r in rows:
-        w = [int(x, 16) for x in r]
-        assert philox4x32_10(w[0:4], w[4:6]) == tuple(w[6:10])
 
 
 def _curand_host():
@@ -33,11 +22,11 @@ def test_against_curand_host_generator():
     (mapping found by search); every block must equal ours."""
     lib = _curand_host()
     if lib is None:
-        pytest.skip("libcurand not loadable")
+        pytest.fail("libcurand (CUDA toolkit) not loadable: the Philox pin needs it")
     gen = C.c_void_p()
     CURAND_RNG_PSEUDO_PHILOX4_32_10 = 161
     if lib.curandCreateGeneratorHost(C.byref(gen), CURAND_RNG_PSEUDO_PHILOX4_32_10) != 0:
-        pytest.skip("cuRAND host generator unavailable")
+        pytest.fail("cuRAND host generator unavailable: the Philox pin needs it")
     for seed in (0, 77, 0x0123456789ABCDEF):
         assert lib.curandSetPseudoRandomGeneratorSeed(gen, C.c_ulonglong(seed)) == 0
         assert lib.curandSetGeneratorOffset(gen, C.c_ulonglong(0)) == 0
