@@ -122,7 +122,7 @@ typedef struct {
     float    cap_half_angle_deg; /* excluded cap about s, PAPER.md:395 ("~2.5 deg")            */
     float    rmax_scale;         /* r_max = rmax_scale * (shortest AABB side)/2  */
     float    rmax_override;      /* > 0: use this r_max instead of the AABB rule               */
-    int32_t  bisection_iters;    /* LargestTangentBall iterations, PAPER.md:383 (10)           */
+    int32_t  bisection_iters;    /* LargestTangentBall iterations, PAPER.md:383 (10); 1..24    */
     int32_t  importance_sample;  /* 1: z ~ J^B; 0: z uniform on the ball        */
     int32_t  antithetic;         /* 1: walks 2j, 2j+1 are antipodal in azimuth  */
     int32_t  include_killing;    /* exterior only: second expectation of Eq. 32                */
@@ -142,8 +142,9 @@ typedef struct {                 /* host; filled when passed non-NULL (forces a 
     int64_t n_samples, n_discarded;       /* samples whose tangent ball degenerated */
     int64_t n_walks, n_truncated;         /* walks started / cut at max_steps       */
     int64_t n_steps;                      /* position updates x += d*omega                         */
-    int64_t n_queries;                    /* closest-point queries (bisection + every WoS iteration) */
+    int64_t n_queries;                    /* closest-point queries: every WoS iteration + one tangent-ball traversal per sample */
     int64_t n_nodes_visited, n_tris_tested;   /* traversal work actually done (flop/byte model)    */
+    int64_t n_prep_queries, n_prep_nodes, n_prep_tris;  /* of which: the tangent-ball traversals (A2) */
     int64_t n_entries, n_unique;          /* (row,col,value) records expanded / after reduction    */
     int64_t workspace_needed;             /* bytes; set on MCS_ENOMEM too                           */
     int64_t nodes_hist[16];               /* walk-kernel queries by floor(log2(nodes visited)), bin 15 = rest */

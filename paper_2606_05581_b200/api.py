@@ -59,7 +59,8 @@ class _Matrix(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_samples", C.c_int64), ("n_discarded", C.c_int64), ("n_walks", C.c_int64),
                 ("n_truncated", C.c_int64), ("n_steps", C.c_int64), ("n_queries", C.c_int64),
-                ("n_nodes_visited", C.c_int64), ("n_tris_tested", C.c_int64), ("n_entries", C.c_int64),
+                ("n_nodes_visited", C.c_int64), ("n_tris_tested", C.c_int64), ("n_prep_queries", C.c_int64),
+                ("n_prep_nodes", C.c_int64), ("n_prep_tris", C.c_int64), ("n_entries", C.c_int64),
                 ("n_unique", C.c_int64), ("workspace_needed", C.c_int64), ("nodes_hist", C.c_int64 * 16),
                 ("cuda_error", C.c_int32),
                 ("pad_", C.c_int32)]

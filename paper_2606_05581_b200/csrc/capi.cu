@@ -56,6 +56,9 @@ void fill_stats(mcs_stats* hs, const unsigned long long* h, const mcs_samples* s
     hs->n_queries = (int64_t)h[ST_QUERIES];
     hs->n_nodes_visited = (int64_t)h[ST_NODES];
     hs->n_tris_tested = (int64_t)h[ST_TRIS];
+    hs->n_prep_queries = (int64_t)h[ST_PREP_QUERIES];
+    hs->n_prep_nodes = (int64_t)h[ST_PREP_NODES];
+    hs->n_prep_tris = (int64_t)h[ST_PREP_TRIS];
     hs->n_entries = (int64_t)h[ST_ENTRIES];
     hs->n_unique = (int64_t)h[ST_UNIQUE];
     for (int b = 0; b < 16; ++b) hs->nodes_hist[b] = (int64_t)h[ST_HIST + b];

@@ -112,85 +112,178 @@ sample_keys_kernel(const float* __restrict__ verts, const int32_t* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------
-// LargestTangentBall: bisection with `iters` iterations
-// (PAPER.md:383), radius clamped to r_max.  Each probe is a
-// bounded "is any face closer than r - eps/2" traversal (R4).
-// Exterior: the ball lives in the inverted domain and is probed through its
-// primal image (E2).
+// LargestTangentBall: the bisection of PAPER.md:383 with `iters`
+// iterations, radius clamped to r_max (R4).
+//
+// The bisection probes radii on the grid r_j = j * hi / 2^iters and, because the
+// probed balls B(s - r n, r - eps/2) are nested (tangent at s), returns the largest
+// grid radius whose ball no face enters:  r = r_J,  J = min over faces T of
+// j_T = max{ j : T outside ball_j }.  Instead of `iters` separate emptiness proofs
+// (each one visits every node its ball touches), ONE traversal with a shrinking ball
+// computes that minimum: keep the current candidate J, visit only nodes whose box
+// enters ball_J, and when a face enters ball_J find its own j_T by bisection over j
+// on that single face (<= iters point-triangle tests) and shrink J.
+//
+// One warp per sample: the warp shares a node stack and a leaf list in shared
+// memory, pops up to 32 nodes (or 32 leaves) per pass, one per lane, and pushes the
+// surviving children with warp-aggregated offsets.  J is a minimum, so the result
+// does not depend on the order of the traversal.
+// Exterior: the ball lives in the inverted domain and is probed through its primal
+// image (E2), which preserves the nesting.
 // ---------------------------------------------------------------------------
+constexpr int TB_WARPS = 4;
+constexpr int TB_NCAP = 2048;          // node stack entries per warp
+constexpr int TB_LCAP = 128;           // leaf list entries per warp (drained at 32)
+
+struct BallFamily {
+    float3 base, pole, o;
+    float step, ss2, sdn, eps;
+};
+
+// Probe ball of grid index j: centre c and squared threshold thr2 (< 0: nothing can be closer).
 template <bool EXT>
-__global__ void __launch_bounds__(PT)
+__device__ __forceinline__ void probe_ball(const BallFamily& f, int j, float3& c, float& thr2)
+{
+    const float r = (float)j * f.step;
+    c = f3(fmaf(-r, f.pole.x, f.base.x), fmaf(-r, f.pole.y, f.base.y), fmaf(-r, f.pole.z, f.base.z));
+    float thr;
+    if (EXT) {
+        const float den = f.ss2 - 2.0f * r * f.sdn;               // |c*|^2 - r^2
+        c = f3(f.o.x + c.x / den, f.o.y + c.y / den, f.o.z + c.z / den);
+        thr = (r / den) * (1.0f - 0.5f * f.eps / r);
+    } else {
+        thr = r - 0.5f * f.eps;
+    }
+    thr2 = (j > 0 && thr > 0.0f) ? thr * thr : -1.0f;
+}
+
+template <bool EXT>
+__global__ void __launch_bounds__(TB_WARPS * 32)
 tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
                     const float* __restrict__ normal, const uint32_t* __restrict__ order, int64_t n_s,
                     float rmax, float eps, int iters, float3 o,
                     float4* __restrict__ balls, unsigned long long* __restrict__ stats)
 {
-    const int64_t j = (int64_t)blockIdx.x * PT + threadIdx.x;
-    TraversalCounters cnt; cnt.nodes = 0; cnt.tris = 0;
-    unsigned queries = 0, discarded = 0;
-    if (j < n_s) {
-        const int64_t i = order[j];
+    __shared__ int s_nodes[TB_WARPS][TB_NCAP];
+    __shared__ int s_leaves[TB_WARPS][TB_LCAP];
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    int* nstack = s_nodes[wib];
+    int* lstack = s_leaves[wib];
+    const int64_t n_warps = (int64_t)gridDim.x * TB_WARPS;
+    unsigned cnt_nodes = 0, cnt_tris = 0, cnt_queries = 0, cnt_discarded = 0;
+    const float SLACK = 1.0f + 4e-6f;
+
+    for (int64_t jj = (int64_t)blockIdx.x * TB_WARPS + wib; jj < n_s; jj += n_warps) {
+        const int64_t i = order[jj];
         float3 s, n;
         sample_point(g.verts, g.faces, tri, bary, i, s, n);
         if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
-        float3 base = s, pole = n;       // ball centre = base - r * pole
-        float hi = rmax, ss2 = 1.0f, sdn = 0.0f, sstar_norm = 1.0f;
+        BallFamily fam;
+        fam.base = s; fam.pole = n; fam.o = o; fam.ss2 = 1.0f; fam.sdn = 0.0f; fam.eps = eps;
+        float hi = rmax, sstar_norm = 1.0f;
         bool ok = true;
         if (EXT) {
             const float3 st = s - o;
             const float sig = dot3(st, st);
             ok = sig > 0.0f;
             if (ok) {
-                base = (1.0f / sig) * st;                                  // s* = kappa(s - o)
+                fam.base = (1.0f / sig) * st;                              // s* = kappa(s - o)
                 const float sn = dot3(st, n) / sig;
-                pole = f3(-(n.x - 2.0f * st.x * sn), -(n.y - 2.0f * st.y * sn), -(n.z - 2.0f * st.z * sn));   // Eq. 54
-                ss2 = dot3(base, base);
-                sdn = dot3(base, pole);
-                if (sdn > 0.0f) hi = fminf(hi, 0.45f * ss2 / sdn);       // keep 0 = kappa(inf) outside the ball
-                sstar_norm = sqrtf(ss2);
+                fam.pole = f3(-(n.x - 2.0f * st.x * sn), -(n.y - 2.0f * st.y * sn), -(n.z - 2.0f * st.z * sn));   // Eq. 54
+                fam.ss2 = dot3(fam.base, fam.base);
+                fam.sdn = dot3(fam.base, fam.pole);
+                if (fam.sdn > 0.0f) hi = fminf(hi, 0.45f * fam.ss2 / fam.sdn);   // keep 0 = kappa(inf) outside the ball
+                sstar_norm = sqrtf(fam.ss2);
             }
         }
-        float lo = 0.0f;
-        if (ok) {
-            for (int it = 0; it < iters; ++it) {
-                const float r = 0.5f * (lo + hi);
-                float3 c = f3(fmaf(-r, pole.x, base.x), fmaf(-r, pole.y, base.y), fmaf(-r, pole.z, base.z));
-                float thr;
-                if (EXT) {
-                    const float den = ss2 - 2.0f * r * sdn;               // |c*|^2 - r^2
-                    c = f3(o.x + c.x / den, o.y + c.y / den, o.z + c.z / den);
-                    thr = (r / den) * (1.0f - 0.5f * eps / r);
-                } else {
-                    thr = r - 0.5f * eps;
+        const int NJ = 1 << iters;
+        fam.step = hi / (float)NJ;
+        int J = ok ? NJ - 1 : 0;
+        float3 cJ; float thr2J;
+        probe_ball<EXT>(fam, J, cJ, thr2J);
+        int ncount = 0, lcount = 0;
+        if (J > 0 && thr2J > 0.0f) { if (lane == 0) nstack[0] = 0; ncount = 1; }
+        if (lane == 0) ++cnt_queries;
+        __syncwarp();
+        while (J > 0 && (ncount > 0 || lcount > 0)) {
+            if (lcount >= 32 || ncount == 0) {
+                // ---- leaf pass: does the face enter ball_J? ---------------------------
+                const int nl = lcount < 32 ? lcount : 32;
+                int myJ = J;
+                if (lane < nl) {
+                    const int kk = lstack[lcount - nl + lane];
+                    float3 a, b, c; int orig; float v, w;
+                    load_tri(g.tris, kk, a, b, c, orig);
+                    ++cnt_tris;
+                    if (closest_point_triangle(cJ, a, b, c, v, w) < thr2J) {
+                        int lo_j = 0, hi_j = J;                           // ball_0 is empty by definition
+                        while (hi_j - lo_j > 1) {
+                            const int mid = (lo_j + hi_j) >> 1;
+                            float3 cm; float t2;
+                            probe_ball<EXT>(fam, mid, cm, t2);
+                            ++cnt_tris;
+                            if (closest_point_triangle(cm, a, b, c, v, w) < t2) hi_j = mid; else lo_j = mid;
+                        }
+                        myJ = lo_j;
+                    }
                 }
-                bool closer = false;
-                if (thr > 0.0f) {
-                    ClosestHit h; h.d2 = thr * thr; h.tri = -1; h.k = -1; h.v = h.w = 0.0f;
-                    const float bound = h.d2;
-                    bvh_closest_point<true, true>(g.nodes, g.tris, c, h, cnt);
-                    closer = h.d2 < bound;
-                    ++queries;
+                lcount -= nl;
+                for (int off = 16; off > 0; off >>= 1) myJ = min(myJ, __shfl_xor_sync(FULL, myJ, off));
+                if (myJ < J) { J = myJ; probe_ball<EXT>(fam, J, cJ, thr2J); }
+                __syncwarp();
+            } else {
+                // ---- node pass: which children enter ball_J? ---------------------------
+                int np = ncount < 32 ? ncount : 32;
+                if (ncount > TB_NCAP - 96) np = 1;                        // nearly full: plain depth-first
+                bool in0 = false, in1 = false;
+                int c0 = 0, c1 = 0;
+                if (lane < np) {
+                    const int node = nstack[ncount - np + lane];
+                    const float4* nd = reinterpret_cast<const float4*>(g.nodes + node);
+                    const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
+                    const int2 ch = __ldg(reinterpret_cast<const int2*>(nd + 3));
+                    ++cnt_nodes;
+                    c0 = ch.x; c1 = ch.y;
+                    const float lim = thr2J * SLACK;
+                    in0 = box_dist2(cJ, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y) <= lim;
+                    in1 = box_dist2(cJ, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w) <= lim;
                 }
-                if (closer) hi = r; else lo = r;
+                ncount -= np;
+                __syncwarp();                                             // all pops read before any push writes
+                const unsigned mn0 = __ballot_sync(FULL, in0 && c0 >= 0), mn1 = __ballot_sync(FULL, in1 && c1 >= 0);
+                const unsigned ml0 = __ballot_sync(FULL, in0 && c0 < 0), ml1 = __ballot_sync(FULL, in1 && c1 < 0);
+                if (in0 && c0 >= 0) nstack[ncount + __popc(mn0 & lt)] = c0;
+                if (in1 && c1 >= 0) nstack[ncount + __popc(mn0) + __popc(mn1 & lt)] = c1;
+                if (in0 && c0 < 0) lstack[lcount + __popc(ml0 & lt)] = ~c0;
+                if (in1 && c1 < 0) lstack[lcount + __popc(ml0) + __popc(ml1 & lt)] = ~c1;
+                ncount += __popc(mn0) + __popc(mn1);
+                lcount += __popc(ml0) + __popc(ml1);
+                __syncwarp();
             }
         }
-        const float r = lo;
-        if (!(r > 0.0f)) discarded = 1;
-        balls[2 * i] = make_float4(fmaf(-r, pole.x, base.x), fmaf(-r, pole.y, base.y), fmaf(-r, pole.z, base.z), r);
-        balls[2 * i + 1] = make_float4(pole.x, pole.y, pole.z, ok ? sstar_norm : 0.0f);
+        const float r = (float)J * fam.step;
+        if (lane == 0) {
+            if (!(r > 0.0f)) ++cnt_discarded;
+            balls[2 * i] = make_float4(fmaf(-r, fam.pole.x, fam.base.x), fmaf(-r, fam.pole.y, fam.base.y),
+                                       fmaf(-r, fam.pole.z, fam.base.z), r);
+            balls[2 * i + 1] = make_float4(fam.pole.x, fam.pole.y, fam.pole.z, ok ? sstar_norm : 0.0f);
+        }
+        __syncwarp();
     }
     // statistics (integer atomics: order-independent)
-    unsigned vals[4] = { queries, discarded, cnt.nodes, cnt.tris };
+    unsigned vals[4] = { cnt_queries, cnt_discarded, cnt_nodes, cnt_tris };
     for (int q = 0; q < 4; ++q) {
         unsigned v = vals[q];
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
         vals[q] = v;
     }
-    if ((threadIdx.x & 31) == 0) {
-        if (vals[0]) atomicAdd(&stats[ST_QUERIES], (unsigned long long)vals[0]);
+    if (lane == 0) {
+        if (vals[0]) { atomicAdd(&stats[ST_QUERIES], (unsigned long long)vals[0]); atomicAdd(&stats[ST_PREP_QUERIES], (unsigned long long)vals[0]); }
         if (vals[1]) atomicAdd(&stats[ST_DISCARDED], (unsigned long long)vals[1]);
-        if (vals[2]) atomicAdd(&stats[ST_NODES], (unsigned long long)vals[2]);
-        if (vals[3]) atomicAdd(&stats[ST_TRIS], (unsigned long long)vals[3]);
+        if (vals[2]) { atomicAdd(&stats[ST_NODES], (unsigned long long)vals[2]); atomicAdd(&stats[ST_PREP_NODES], (unsigned long long)vals[2]); }
+        if (vals[3]) { atomicAdd(&stats[ST_TRIS], (unsigned long long)vals[3]); atomicAdd(&stats[ST_PREP_TRIS], (unsigned long long)vals[3]); }
     }
 }
 
@@ -502,7 +595,7 @@ int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, in
     if (s->n_s < 1 || !s->tri || !s->bary || !s->weight) return MCS_EINVAL;
     if (p->walks_per_sample < 1 || p->max_steps < 0 || !(p->eps > 0.0f)) return MCS_EINVAL;
     if (!(p->cap_half_angle_deg > 0.0f) || p->cap_half_angle_deg >= 180.0f) return MCS_EINVAL;
-    if (p->bisection_iters < 1 || p->bisection_iters > 64) return MCS_EINVAL;
+    if (p->bisection_iters < 1 || p->bisection_iters > 24) return MCS_EINVAL;
     if (!(p->rmax_scale > 0.0f) && !(p->rmax_override > 0.0f)) return MCS_EINVAL;
     if (s->n_s >= ((int64_t)1 << 32) - 1) return MCS_EINVAL;
     if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
@@ -590,12 +683,20 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     }
     mcs_note_launch(), face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
 
-    if (exterior)
-        mcs_note_launch(), tangent_ball_kernel<true><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
-                                                         p->bisection_iters, o, balls, stats);
-    else
-        mcs_note_launch(), tangent_ball_kernel<false><<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps,
-                                                          p->bisection_iters, o, balls, stats);
+    {
+        int dev_tb = 0, n_sm_tb = 0;
+        MCS_CUDA_TRY(cudaGetDevice(&dev_tb));
+        MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm_tb, cudaDevAttrMultiProcessorCount, dev_tb));
+        int64_t nblk_tb = ceil_div64(n_s, TB_WARPS);
+        const int64_t cap_tb = (int64_t)n_sm_tb * 6;                  // 6 resident blocks of 34 KB shared memory per SM
+        if (nblk_tb > cap_tb) nblk_tb = cap_tb;
+        if (exterior)
+            mcs_note_launch(), tangent_ball_kernel<true><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
+                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, balls, stats);
+        else
+            mcs_note_launch(), tangent_ball_kernel<false><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
+                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, balls, stats);
+    }
     if (balls_out) mcs_note_launch(), balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
     MCS_CUDA_TRY(cudaGetLastError());
     if (balls_only) return MCS_OK;

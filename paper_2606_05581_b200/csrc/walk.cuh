@@ -6,6 +6,7 @@ enum {
     ST_WORK = 0,        // work-queue head of the persistent walk kernel
     ST_STEPS, ST_QUERIES, ST_TRUNCATED, ST_DISCARDED, ST_NODES, ST_TRIS,
     ST_ENTRIES, ST_UNIQUE,
+    ST_PREP_QUERIES, ST_PREP_NODES, ST_PREP_TRIS,   // tangent-ball share of ST_QUERIES / ST_NODES / ST_TRIS
     ST_HIST = 16,       // 16 bins: queries of the walk kernel by floor(log2(nodes visited))
     ST_COUNT = 32
 };
