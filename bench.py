@@ -301,12 +301,14 @@ def run_ours(args):
     roof = {}
     for name, st in (("interior", st_i), ("exterior", st_e)):
         t = float(np.mean(walk_ms[name])) * 1e-3
-        # walk kernel only: subtract the bisection probes' share (counted in the same totals) pro rata by queries
-        flops = 36.0 * st.n_nodes_visited + 80.0 * st.n_tris_tested
-        nbytes = 64.0 * st.n_nodes_visited + 48.0 * st.n_tris_tested
+        # walk kernel only: the tangent-ball traversals (A2) are counted separately
+        nodes, tris = st.n_nodes_visited - st.n_prep_nodes, st.n_tris_tested - st.n_prep_tris
+        queries = st.n_queries - st.n_prep_queries
+        flops = 36.0 * nodes + 80.0 * tris
+        nbytes = 64.0 * nodes + 48.0 * tris
         t_alu, t_mem = flops / (fp32_tflops * 1e12), nbytes / (level_gbs * 1e9)
         roof[name] = dict(t=t, flops=flops, bytes=nbytes, t_alu=t_alu, t_mem=t_mem,
-                          nodes_per_query=st.n_nodes_visited / st.n_queries, tris_per_query=st.n_tris_tested / st.n_queries)
+                          nodes_per_query=nodes / queries, tris_per_query=tris / queries)
     t_kernel = roof["interior"]["t"] + roof["exterior"]["t"]
     nbytes = roof["interior"]["bytes"] + roof["exterior"]["bytes"]
     flops = roof["interior"]["flops"] + roof["exterior"]["flops"]

@@ -4,19 +4,42 @@
 // killing record contributing weight * b(t0) b(t0)^T (Eq. 32, second term).
 //
 // The paper defers the outer products "to be computed in batches to avoid shared
-// memory contention".  Here: expand every walk into its
-// upper-triangular (row, col, value) entries in slot order, stable radix sort by
-// key = row*K + col, sum each run of equal keys left to right, add the run sums
-// to the dense matrix (one writer per entry, so no atomics), and mirror the
-// upper triangle at the end.  The result is bit-identical from run to run and
+// memory contention".  Here the accumulation is a two-level
+// sort-by-key segmented reduction, with no float atomics anywhere:
+//
+//  level 1 (on chip)  A block takes 256 consecutive record slots, sorts them in shared
+//      memory by (sample, exit face) and reduces every run to ONE pair record: the
+//      moments  w = sum wgt,  A_k = sum wgt b_k(t),  M_kl = sum wgt b_k(t) b_l(t)
+//      of the exit-point barycentrics.  All walks of a pair share b(s) and the six
+//      vertices involved, so  sum wgt d d^T  over the pair is a function of
+//      (w, A, M) alone.  With W walks per sample this shrinks the stream that has to
+//      be sorted globally by the number of walks per (sample, exit face) pair.
+//  level 2 (global)   Pair records are expanded to upper-triangular (row*K+col, value)
+//      entries in slot order, stable-radix-sorted by key, every run of equal keys is
+//      summed by a segmented scan of fixed shape, and the run sums are added to the
+//      dense matrix (one writer per entry); runs that cross a tile are completed in
+//      tile order by a second small kernel.  The upper triangle is mirrored at the end.
+//
+// Every sum has a fixed association order (the position of an item after a stable
+// sort, the shape of the scan), so the result is bit-identical from run to run and
 // exactly symmetric.
 #include "walk.cuh"
 
 namespace {
 
 constexpr int AT = 256;
+constexpr int CH = 256;                               // record slots per level-1 block
 constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << 22;
-constexpr int MAX_ENTRIES_PER_WALK = 21;          // upper triangle of a 6 x 6 block
+constexpr int MAX_ENTRIES_PER_PAIR = 21;              // upper triangle of a 6 x 6 block
+constexpr int RT = 1024;                              // entries per tile of the run reduction
+
+struct __align__(16) PairRec {
+    int   sample;            // -1: killing walk (no b(s) part)
+    int   tri_t;
+    float w;                 // sum wgt
+    float A[3];              // sum wgt b_k
+    float M[6];              // sum wgt b_k b_l : 00 01 02 11 12 22
+};
 
 struct AccArgs {
     const float4*  records;
@@ -28,82 +51,259 @@ struct AccArgs {
     long long K;
 };
 
-// d = b(s) - b(t): up to 6 (vertex, value) pairs; shared vertices are merged.
-__device__ __forceinline__ int build_d(const AccArgs& a, long long j, const float4 rec, int idx[6], float val[6])
+// ---------------------------------------------------------------------------
+// Segmented inclusive scan over the CH (or RT) threads of a block, NV values per
+// thread, fixed shape: Hillis-Steele inside a warp restricted to the lane's segment,
+// then the warps' trailing partial sums are chained in warp order.
+// head: this thread starts a new segment.  On return v[] holds the inclusive sum of
+// the thread's segment up to and including itself, as far as the segment lies inside
+// the block.  Returns true when the thread's segment has its head inside the block.
+// ---------------------------------------------------------------------------
+template <int NV, int NWARPS>
+__device__ __forceinline__ bool block_segmented_scan(float (&v)[NV], bool head, float (*s_tail)[NV], int* s_has_head)
 {
-    int n = 0;
-    float sign = 1.0f;
-    if (j < a.n_main) {
-        const long long smp = j / a.W;
-        const long long fs = a.s_tri[smp];
-        for (int k = 0; k < 3; ++k) { idx[n] = a.faces[3 * fs + k]; val[n] = a.s_bary[3 * smp + k]; ++n; }
-        sign = -1.0f;
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned heads = __ballot_sync(FULL, head);
+    const unsigned upto = heads & (0xFFFFFFFFu >> (31 - lane));          // heads at lanes <= lane
+    const int seg_start = upto ? 31 - __clz(upto) : 0;                    // first lane of my segment inside the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            const float t = __shfl_up_sync(FULL, v[q], o);
+            if (lane - o >= seg_start) v[q] += t;
+        }
     }
-    const long long ft = __float_as_int(rec.x);
-    const float bt[3] = { 1.0f - rec.y - rec.z, rec.y, rec.z };
+    if (lane == 31) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) s_tail[warp][q] = v[q];
+        s_has_head[warp] = heads != 0;
+    }
+    __syncthreads();
+    bool headed = upto != 0;
+    if (!headed && warp > 0) {                                            // my segment started in an earlier warp
+        float carry[NV];
+#pragma unroll
+        for (int q = 0; q < NV; ++q) carry[q] = 0.0f;
+        int first = warp - 1;
+        while (first > 0 && !s_has_head[first]) --first;                  // warp holding the segment's head (or warp 0)
+        headed = s_has_head[first] != 0;
+        for (int w = first; w < warp; ++w)                                // chained left to right
+#pragma unroll
+            for (int q = 0; q < NV; ++q) carry[q] += s_tail[w][q];
+#pragma unroll
+        for (int q = 0; q < NV; ++q) v[q] = carry[q] + v[q];
+    }
+    __syncthreads();
+    return headed;
+}
+
+// ---------------------------------------------------------------------------
+// Level 1.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(CH)
+pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ pairs, uint32_t* __restrict__ pair_counts)
+{
+    __shared__ unsigned long long s_key[CH];
+    __shared__ float4 s_rec[CH];
+    __shared__ float s_tail[CH / 32][10];
+    __shared__ int s_has_head[CH / 32];
+    __shared__ int s_warp_runs[CH / 32];
+    const int tid = threadIdx.x;
+    const long long base = j0 + (long long)blockIdx.x * CH;
+    const long long slot = base + tid;
+    const long long first_sample = base < a.n_main ? base / a.W : 0;
+    unsigned long long key = ~0ull;
+    if (slot < j0 + n) {
+        const float4 rec = a.records[slot];
+        s_rec[tid] = rec;
+        const int tri_t = __float_as_int(rec.x);
+        if (tri_t >= 0 && rec.w != 0.0f) {
+            const unsigned long long sl = slot < a.n_main ? (unsigned long long)(slot / a.W - first_sample) : 0x1FFull;
+            key = (sl << 40) | ((unsigned long long)(unsigned)tri_t << 8) | (unsigned long long)tid;
+        }
+    }
+    s_key[tid] = key;
+    __syncthreads();
+    // bitonic sort of CH unique 64-bit keys (the low byte is the slot: ties keep slot order)
+    for (int k = 2; k <= CH; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            const int partner = tid ^ j;
+            if (partner > tid) {
+                const unsigned long long x = s_key[tid], y = s_key[partner];
+                const bool up = (tid & k) == 0;
+                if ((x > y) == up) { s_key[tid] = y; s_key[partner] = x; }
+            }
+            __syncthreads();
+        }
+    }
+    key = s_key[tid];
+    const bool valid = key != ~0ull;
+    const unsigned long long gid = key >> 8;
+    const bool head = valid && (tid == 0 || (s_key[tid - 1] >> 8) != gid);
+    const bool tail = valid && (tid == CH - 1 || (s_key[tid + 1] >> 8) != gid);     // invalid keys sort last
+    float v[10];
+    {
+        const float4 rec = s_rec[valid ? (int)(key & 0xFF) : 0];
+        const float wgt = valid ? rec.w : 0.0f;
+        const float b1 = rec.y, b2 = rec.z, b0 = 1.0f - b1 - b2;
+        v[0] = wgt; v[1] = wgt * b0; v[2] = wgt * b1; v[3] = wgt * b2;
+        v[4] = v[1] * b0; v[5] = v[1] * b1; v[6] = v[1] * b2; v[7] = v[2] * b1; v[8] = v[2] * b2; v[9] = v[3] * b2;
+    }
+    block_segmented_scan<10, CH / 32>(v, head || !valid, s_tail, s_has_head);
+    // rank of my run among the block's runs (runs are counted at their tails)
+    const unsigned tails = __ballot_sync(0xFFFFFFFFu, tail);
+    const int lane = tid & 31, warp = tid >> 5;
+    if (lane == 0) s_warp_runs[warp] = __popc(tails);
+    __syncthreads();
+    int before = 0, total = 0;
+    for (int w = 0; w < CH / 32; ++w) { const int c = s_warp_runs[w]; if (w < warp) before += c; total += c; }
+    if (tail) {
+        const int rank = before + __popc(tails & ((1u << lane) - 1u));
+        PairRec r;
+        const unsigned sl = (unsigned)(gid >> 32);
+        r.sample = sl == 0x1FFu ? -1 : (int)(first_sample + sl);
+        r.tri_t = (int)(gid & 0xFFFFFFFFu);
+        r.w = v[0]; r.A[0] = v[1]; r.A[1] = v[2]; r.A[2] = v[3];
+        for (int q = 0; q < 6; ++q) r.M[q] = v[4 + q];
+        pairs[(long long)blockIdx.x * CH + rank] = r;
+    }
+    if (tid == 0) pair_counts[blockIdx.x] = (uint32_t)total;
+}
+
+// ---------------------------------------------------------------------------
+// Level 2: pair record -> upper-triangular entries.
+// The merged vertex list holds the (<= 3) vertices of the sample's face and the
+// (<= 3) vertices of the exit face, shared vertices once.
+// ---------------------------------------------------------------------------
+struct PairBlock {
+    int   idx[6];
+    float ds[6];          // b_v(s)
+    float At[6];          // sum wgt b_v(t)
+    int   tmask[6];       // corners of the exit face that are this vertex (bit k)
+    int   m;
+};
+
+__device__ __forceinline__ int pair_block_slot(PairBlock& B, int vtx)
+{
+    for (int q = 0; q < B.m; ++q) if (B.idx[q] == vtx) return q;
+    B.idx[B.m] = vtx; B.ds[B.m] = 0.0f; B.At[B.m] = 0.0f; B.tmask[B.m] = 0;
+    return B.m++;
+}
+
+__device__ __forceinline__ void build_pair_block(const AccArgs& a, const PairRec& r, PairBlock& B)
+{
+    B.m = 0;
+    if (r.sample >= 0) {
+        const long long fs = a.s_tri[r.sample];
+        for (int k = 0; k < 3; ++k) B.ds[pair_block_slot(B, a.faces[3 * fs + k])] += a.s_bary[3 * (long long)r.sample + k];
+    }
+    const long long ft = r.tri_t;
     for (int k = 0; k < 3; ++k) {
-        const int v = a.faces[3 * ft + k];
-        int found = -1;
-        for (int m = 0; m < n; ++m) if (idx[m] == v) found = m;
-        if (found >= 0) val[found] += sign * bt[k];
-        else { idx[n] = v; val[n] = sign * bt[k]; ++n; }
+        const int q = pair_block_slot(B, a.faces[3 * ft + k]);
+        B.At[q] += r.A[k];
+        B.tmask[q] |= 1 << k;
     }
-    return n;
+}
+
+__device__ __forceinline__ float moment(const PairRec& r, int k, int l)
+{
+    if (k > l) { const int t = k; k = l; l = t; }
+    return r.M[k == 0 ? l : (k == 1 ? 2 + l : 5)];
+}
+
+// sum wgt b_p(t) b_q(t) for merged vertices p, q
+__device__ __forceinline__ float moment_block(const PairRec& r, int maskp, int maskq)
+{
+    float e = 0.0f;
+    for (int k = 0; k < 3; ++k)
+        if (maskp & (1 << k))
+            for (int l = 0; l < 3; ++l)
+                if (maskq & (1 << l)) e += moment(r, k, l);
+    return e;
 }
 
 __global__ void __launch_bounds__(AT)
-count_entries_kernel(AccArgs a, long long j0, long long n, uint32_t* __restrict__ counts)
+count_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32_t* __restrict__ pair_counts,
+                     long long n_slots, uint32_t* __restrict__ counts)
 {
     const long long i = (long long)blockIdx.x * AT + threadIdx.x;
-    if (i >= n) return;
-    const float4 rec = a.records[j0 + i];
+    if (i >= n_slots) return;
     uint32_t c = 0;
-    if (__float_as_int(rec.x) >= 0 && rec.w != 0.0f) {
-        int idx[6]; float val[6];
-        const int m = build_d(a, j0 + i, rec, idx, val);
-        for (int p = 0; p < m; ++p) for (int q = 0; q < m; ++q) c += (idx[p] <= idx[q]) ? 1u : 0u;
+    if ((uint32_t)(i % CH) < pair_counts[i / CH]) {
+        PairBlock B;
+        build_pair_block(a, pairs[i], B);
+        for (int p = 0; p < B.m; ++p) for (int q = 0; q < B.m; ++q) c += (B.idx[p] <= B.idx[q]) ? 1u : 0u;
     }
     counts[i] = c;
 }
 
 __global__ void __launch_bounds__(AT)
-expand_entries_kernel(AccArgs a, long long j0, long long n, const uint32_t* __restrict__ offsets,
+expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32_t* __restrict__ pair_counts,
+                      long long n_slots, const uint32_t* __restrict__ offsets,
                       uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
 {
     const long long i = (long long)blockIdx.x * AT + threadIdx.x;
-    if (i >= n) return;
-    const float4 rec = a.records[j0 + i];
-    if (__float_as_int(rec.x) < 0 || rec.w == 0.0f) return;
-    int idx[6]; float val[6];
-    const int m = build_d(a, j0 + i, rec, idx, val);
+    if (i >= n_slots) return;
+    if ((uint32_t)(i % CH) >= pair_counts[i / CH]) return;
+    const PairRec r = pairs[i];
+    PairBlock B;
+    build_pair_block(a, r, B);
     uint32_t o = offsets[i];
-    for (int p = 0; p < m; ++p)
-        for (int q = 0; q < m; ++q)
-            if (idx[p] <= idx[q]) {
-                keys[o] = (uint32_t)((long long)idx[p] * a.K + idx[q]);
-                vals[o] = __float_as_uint(rec.w * val[p] * val[q]);
+    for (int p = 0; p < B.m; ++p)
+        for (int q = 0; q < B.m; ++q)
+            if (B.idx[p] <= B.idx[q]) {
+                // sum over the pair's walks of wgt * d_p d_q,  d = b(s) - b(t)
+                float e = r.w * B.ds[p] * B.ds[q] - B.ds[p] * B.At[q] - B.At[p] * B.ds[q];
+                if (B.tmask[p] && B.tmask[q]) e += moment_block(r, B.tmask[p], B.tmask[q]);
+                keys[o] = (uint32_t)((long long)B.idx[p] * a.K + B.idx[q]);
+                vals[o] = __float_as_uint(e);
                 ++o;
             }
 }
 
-// One thread per run of equal keys: sum left to right, add to the dense matrix.
-__global__ void __launch_bounds__(AT)
+// ---------------------------------------------------------------------------
+// Run sums of the sorted entries.  A run whose head lies in this tile is added to the
+// matrix by its last thread in the tile; the leading part of a run that began in an
+// earlier tile goes to carry[tile] and is added by carry_fixup_kernel in tile order.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(RT)
 reduce_runs_dense_kernel(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, long long n,
-                         float* __restrict__ S, unsigned long long* __restrict__ n_unique)
+                         float* __restrict__ S, uint32_t* __restrict__ carry_key, float* __restrict__ carry_sum,
+                         unsigned long long* __restrict__ n_unique)
 {
-    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
-    bool head = false;
-    if (i < n) {
-        const uint32_t key = keys[i];
-        head = (i == 0) || (keys[i - 1] != key);
-        if (head) {
-            float sum = __uint_as_float(vals[i]);
-            for (long long j = i + 1; j < n && keys[j] == key; ++j) sum += __uint_as_float(vals[j]);
-            S[key] += sum;
-        }
+    __shared__ float s_tail[RT / 32][1];
+    __shared__ int s_has_head[RT / 32];
+    const long long i = (long long)blockIdx.x * RT + threadIdx.x;
+    const bool valid = i < n;
+    const uint32_t key = valid ? keys[i] : 0xFFFFFFFFu;
+    const bool head = valid && (i == 0 || keys[i - 1] != key);
+    const bool last = valid && (threadIdx.x == RT - 1 || i + 1 >= n || keys[i + 1] != key);
+    float v[1] = { valid ? __uint_as_float(vals[i]) : 0.0f };
+    const bool headed = block_segmented_scan<1, RT / 32>(v, head || !valid, s_tail, s_has_head);
+    if (threadIdx.x == 0) carry_key[blockIdx.x] = 0xFFFFFFFFu;
+    __syncthreads();
+    if (last) {
+        if (headed) S[key] += v[0];
+        else { carry_key[blockIdx.x] = key; carry_sum[blockIdx.x] = v[0]; }
     }
     const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
     if (n_unique && (threadIdx.x & 31) == 0 && m) atomicAdd(n_unique, (unsigned long long)__popc(m));
+}
+
+__global__ void __launch_bounds__(AT)
+carry_fixup_kernel(const uint32_t* __restrict__ carry_key, const float* __restrict__ carry_sum, long long n_tiles,
+                   float* __restrict__ S)
+{
+    const long long b = (long long)blockIdx.x * AT + threadIdx.x;
+    if (b >= n_tiles) return;
+    const uint32_t key = carry_key[b];
+    if (key == 0xFFFFFFFFu) return;
+    if (b > 0 && carry_key[b - 1] == key) return;                        // not the first carry of this run
+    float total = carry_sum[b];
+    for (long long j = b + 1; j < n_tiles && carry_key[j] == key; ++j) total += carry_sum[j];
+    S[key] += total;
 }
 
 __global__ void __launch_bounds__(AT)
@@ -123,15 +323,39 @@ int key_bits_for(long long K)
     return bits < 1 ? 1 : bits;
 }
 
+struct AccLayout {
+    size_t pairs, pair_counts, counts, keys, vals, carry_key, carry_sum, scan, sort, total;
+    int64_t C, E, n_blocks, n_tiles;
+};
+
+AccLayout acc_layout(int64_t n_records)
+{
+    AccLayout L;
+    L.C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
+    L.n_blocks = ceil_div64(L.C, CH);
+    const int64_t slots = L.n_blocks * CH;
+    L.E = slots * MAX_ENTRIES_PER_PAIR;
+    L.n_tiles = ceil_div64(L.E, RT);
+    size_t off = 0;
+    L.pairs = off;       off += align_up((size_t)slots * sizeof(PairRec));
+    L.pair_counts = off; off += align_up((size_t)L.n_blocks * 4);
+    L.counts = off;      off += align_up((size_t)(slots + 1) * 4);
+    L.keys = off;        off += align_up((size_t)L.E * 4);
+    L.vals = off;        off += align_up((size_t)L.E * 4);
+    L.carry_key = off;   off += align_up((size_t)L.n_tiles * 4);
+    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 4);
+    L.scan = off;        off += align_up(scan_workspace_bytes(slots) + 256);
+    L.sort = off;        off += align_up(sort_workspace_bytes(L.E, 4));
+    L.total = off + 1024;
+    return L;
+}
+
 }  // namespace
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records)
 {
     (void)b; (void)basis;
-    const int64_t C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
-    const int64_t E = C * MAX_ENTRIES_PER_WALK;
-    return align_up((size_t)(C + 1) * 4) + 2 * align_up((size_t)E * 4) + sort_workspace_bytes(E, 4) +
-           scan_workspace_bytes(C) + 1024;
+    return acc_layout(n_records).total;
 }
 
 int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
@@ -143,18 +367,20 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     if (out->kind != 0 || out->K != basis->K || !out->dense) return MCS_EINVAL;
     const long long K = basis->K;
     if (K > 65535) return MCS_EINVAL;                 // dense keys are 32-bit (row*K + col)
-    if (!ws || ws_bytes < accumulate_workspace_bytes(b, basis, n_records)) return MCS_ENOMEM;
+    const AccLayout L = acc_layout(n_records);
+    if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
 
-    const int64_t C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
-    const int64_t E = C * MAX_ENTRIES_PER_WALK;
-    char* ptr = (char*)ws;
-    uint32_t* counts = (uint32_t*)ptr;  ptr += align_up((size_t)(C + 1) * 4);
-    uint32_t* keys = (uint32_t*)ptr;    ptr += align_up((size_t)E * 4);
-    uint32_t* vals = (uint32_t*)ptr;    ptr += align_up((size_t)E * 4);
-    void* scan_ws = ptr;                ptr += scan_workspace_bytes(C) + 256;
-    ptr = (char*)align_up((size_t)ptr);
-    void* sort_ws = ptr;
-    const size_t sort_bytes = ws_bytes - (size_t)(ptr - (char*)ws);
+    char* base = (char*)ws;
+    PairRec* pairs = (PairRec*)(base + L.pairs);
+    uint32_t* pair_counts = (uint32_t*)(base + L.pair_counts);
+    uint32_t* counts = (uint32_t*)(base + L.counts);
+    uint32_t* keys = (uint32_t*)(base + L.keys);
+    uint32_t* vals = (uint32_t*)(base + L.vals);
+    uint32_t* carry_key = (uint32_t*)(base + L.carry_key);
+    float* carry_sum = (float*)(base + L.carry_sum);
+    void* scan_ws = base + L.scan;
+    void* sort_ws = base + L.sort;
+    const size_t scan_bytes = L.sort - L.scan, sort_bytes = L.total - L.sort;
 
     AccArgs a;
     a.records = records; a.faces = b->faces; a.s_tri = s->tri; a.s_bary = s->bary;
@@ -163,22 +389,26 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 
     MCS_CUDA_TRY(cudaMemsetAsync(out->dense, 0, (size_t)K * K * sizeof(float), st));
     unsigned long long entries_total = 0;
-    for (int64_t j0 = 0; j0 < n_records; j0 += C) {
-        const long long n = (n_records - j0) < C ? (n_records - j0) : C;
-        const unsigned nblk = (unsigned)ceil_div64(n, AT);
-        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts);
-        int rc = exclusive_scan_u32(counts, counts, n, counts + n, scan_ws, scan_workspace_bytes(C) + 256, st);
+    for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
+        const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
+        const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
+        mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        const unsigned nblk = (unsigned)ceil_div64(slots, AT);
+        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
+        int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
         uint32_t n_entries = 0;
-        MCS_CUDA_TRY(cudaMemcpyAsync(&n_entries, counts + n, 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaMemcpyAsync(&n_entries, counts + slots, 4, cudaMemcpyDeviceToHost, st));
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (n_entries == 0) continue;
         entries_total += n_entries;
-        mcs_note_launch(), expand_entries_kernel<<<nblk, AT, 0, st>>>(a, j0, n, counts, keys, vals);
+        mcs_note_launch(), expand_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts, keys, vals);
         rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
-        mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)ceil_div64(n_entries, AT), AT, 0, st>>>(
-            keys, vals, n_entries, out->dense, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
+        const long long n_tiles = ceil_div64(n_entries, RT);
+        mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
+            keys, vals, n_entries, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
+        mcs_note_launch(), carry_fixup_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(carry_key, carry_sum, n_tiles, out->dense);
     }
     mcs_note_launch(), mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);
     if (stats_dev)
