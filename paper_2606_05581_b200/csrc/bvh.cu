@@ -185,9 +185,18 @@ pack_refit_kernel(const float* __restrict__ verts, const int32_t* __restrict__ f
     for (int v = 0; v < 3; ++v)
         for (int d = 0; d < 3; ++d) p[v][d] = verts[3 * (int64_t)faces[3 * (int64_t)f + v] + d];
     PackedTri t;
-    t.t0 = make_float4(p[0][0], p[0][1], p[0][2], __int_as_float(f));
-    t.t1 = make_float4(p[1][0], p[1][1], p[1][2], 0.0f);
-    t.t2 = make_float4(p[2][0], p[2][1], p[2][2], 0.0f);
+    {
+        const double abx = (double)p[1][0] - p[0][0], aby = (double)p[1][1] - p[0][1], abz = (double)p[1][2] - p[0][2];
+        const double acx = (double)p[2][0] - p[0][0], acy = (double)p[2][1] - p[0][1], acz = (double)p[2][2] - p[0][2];
+        const float nx = (float)(aby * acz - abz * acy), ny = (float)(abz * acx - abx * acz), nz = (float)(abx * acy - aby * acx);
+        const float nn = nx * nx + ny * ny + nz * nz;
+        const float e2 = fmaxf((float)(abx * abx + aby * aby + abz * abz), (float)(acx * acx + acy * acy + acz * acz));
+        const bool degenerate = !(nn > 1e-12f * e2 * e2) || !(nn > 0.0f) || !isfinite(1.0f / nn);
+        t.t0 = make_float4(p[0][0], p[0][1], p[0][2], __int_as_float(f));
+        t.t1 = make_float4(p[1][0], p[1][1], p[1][2], degenerate ? 0.0f : nn);
+        t.t2 = make_float4(p[2][0], p[2][1], p[2][2], degenerate ? 0.0f : 1.0f / nn);
+        t.t3 = make_float4(nx, ny, nz, degenerate ? 1.0f : 0.0f);
+    }
     tris[k] = t;
     float box[6];
     for (int d = 0; d < 3; ++d) {

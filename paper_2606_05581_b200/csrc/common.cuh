@@ -41,11 +41,14 @@ struct __align__(16) BvhNode {
     int4   w3;
 };
 
-// One packed triangle = 48 bytes = 3 x 16-byte loads, in Morton order:
+// One packed triangle = 64 bytes = 4 x 16-byte loads, in Morton order:
 //   t0 = (v0.x, v0.y, v0.z, original face index as int bits)
-//   t1 = (v1.x, v1.y, v1.z, 0)   t2 = (v2.x, v2.y, v2.z, 0)
+//   t1 = (v1.x, v1.y, v1.z, |n|^2)   t2 = (v2.x, v2.y, v2.z, 1/|n|^2)
+//   t3 = (n.x, n.y, n.z, 1.0 if the face has zero area else 0.0),  n = (v1-v0) x (v2-v0)
+// The vertices are the caller's fp32 numbers; n, |n|^2 are computed in fp64 by the build
+// and rounded once.
 struct __align__(16) PackedTri {
-    float4 t0, t1, t2;
+    float4 t0, t1, t2, t3;
 };
 
 struct mcs_bvh {

@@ -25,13 +25,13 @@ closest_point_kernel(const BvhNode* __restrict__ nodes, const PackedTri* __restr
 }
 
 // Exhaustive scan: every thread tests every face; faces staged through shared memory.
-constexpr int BF_TILE = 256;
+constexpr int BF_TILE = 128;
 __global__ void __launch_bounds__(QT)
 closest_point_bruteforce_kernel(const PackedTri* __restrict__ tris, int64_t F,
                                 const float* __restrict__ q, int64_t Q,
                                 float* __restrict__ dist, int32_t* __restrict__ tri, float* __restrict__ bary)
 {
-    __shared__ float4 s_tri[BF_TILE * 3];
+    __shared__ float4 s_tri[BF_TILE * 4];
     const int64_t i = (int64_t)blockIdx.x * QT + threadIdx.x;
     const bool active = i < Q;
     const float3 p = active ? f3(q[3 * i], q[3 * i + 1], q[3 * i + 2]) : f3(0.f, 0.f, 0.f);
@@ -39,15 +39,15 @@ closest_point_bruteforce_kernel(const PackedTri* __restrict__ tris, int64_t F,
     for (int64_t base = 0; base < F; base += BF_TILE) {
         const int n = (int)min((int64_t)BF_TILE, F - base);
         __syncthreads();
-        for (int j = threadIdx.x; j < n * 3; j += QT)
+        for (int j = threadIdx.x; j < n * 4; j += QT)
             s_tri[j] = reinterpret_cast<const float4*>(tris + base)[j];
         __syncthreads();
         if (active) {
             for (int j = 0; j < n; ++j) {
-                const float4 t0 = s_tri[3 * j], t1 = s_tri[3 * j + 1], t2 = s_tri[3 * j + 2];
-                float v, w;
-                const float d2 = closest_point_triangle(p, f3(t0.x, t0.y, t0.z), f3(t1.x, t1.y, t1.z), f3(t2.x, t2.y, t2.z), v, w);
-                const int orig = __float_as_int(t0.w);
+                const TriData T = unpack_tri(s_tri[4 * j], s_tri[4 * j + 1], s_tri[4 * j + 2], s_tri[4 * j + 3]);
+                float v = 0.0f, w = 0.0f;
+                const float d2 = closest_point_triangle(p, T, CUDART_INF_F, v, w);
+                const int orig = T.orig;
                 if (d2 < h.d2 || (d2 == h.d2 && orig < h.tri)) { h.d2 = d2; h.tri = orig; h.k = (int)(base + j); h.v = v; h.w = w; }
             }
         }

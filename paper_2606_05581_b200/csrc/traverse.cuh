@@ -41,65 +41,74 @@ __device__ __forceinline__ float origin_to_segment(float3 a, float3 b, float& t)
 {
     float3 ab = b - a;
     float den = dot3(ab, ab);
-    float tt = den > 0.0f ? -dot3(a, ab) / den : 0.0f;
+    float tt = den > 0.0f ? __fdividef(-dot3(a, ab), den) : 0.0f;
     tt = fminf(fmaxf(tt, 0.0f), 1.0f);
     t = tt;
     float3 c = f3(fmaf(tt, ab.x, a.x), fmaf(tt, ab.y, a.y), fmaf(tt, ab.z, a.z));
     return dot3(c, c);
 }
 
-// a*b - c*d with the rounding error of c*d compensated through an FMA (Kahan's
-// difference of products): the result is within ~1.5 ulp of the exact value even under
-// heavy cancellation.  Used for the face normal, so that sliver triangles (aspect
-// ratio > 100, BASELINE.json config 3) keep an accurate supporting plane.
-__device__ __forceinline__ float diff_of_products(float a, float b, float c, float d)
+// One packed triangle as the query kernels see it (common.cuh "PackedTri"): the three fp32
+// vertices exactly as given, plus the supporting plane precomputed by the build in fp64 and
+// rounded once: n = (b-a) x (c-a), nn = |n|^2, rnn = 1/nn.  A sliver (aspect ratio > 100,
+// BASELINE.json config 3) loses its plane when the cross product is formed in fp32
+// (relative error eps * aspect); with the fp64 normal the error of the plane is one rounding.
+struct TriData {
+    float3 a, b, c, n;
+    float  nn, rnn;
+    int    orig;           // original face index
+    bool   degenerate;     // zero-area face: absorbs as its three edges (R16)
+};
+
+__device__ __forceinline__ TriData unpack_tri(float4 t0, float4 t1, float4 t2, float4 t3)
 {
-    const float cd = __fmul_rn(c, d);
-    const float err = __fmaf_rn(-c, d, cd);
-    const float r = __fmaf_rn(a, b, -cd);
-    return __fadd_rn(r, err);
+    TriData T;
+    T.a = f3(t0.x, t0.y, t0.z); T.b = f3(t1.x, t1.y, t1.z); T.c = f3(t2.x, t2.y, t2.z);
+    T.n = f3(t3.x, t3.y, t3.z);
+    T.orig = __float_as_int(t0.w); T.nn = t1.w; T.rnn = t2.w; T.degenerate = t3.w != 0.0f;
+    return T;
 }
 
-// Closest point of triangle (a, b, c) to p, computed on the triangle translated by -p
-// (A, B, C = vertices seen from p, so every rounding error scales with the distance to
-// the triangle, not with the absolute coordinates):
-//   n = ab x ac (compensated), q = projection of p on the plane = ((A.n)/|n|^2) n,
+__device__ __forceinline__ TriData load_tri(const PackedTri* __restrict__ tris, int k)
+{
+    const float4* t = reinterpret_cast<const float4*>(tris + k);
+    return unpack_tri(__ldg(t), __ldg(t + 1), __ldg(t + 2), __ldg(t + 3));
+}
+
+// Closest point of triangle T to p, computed on the triangle translated by -p (A, B, C =
+// vertices seen from p, so every rounding error scales with the distance to the triangle,
+// not with the absolute coordinates):
+//   q = projection of p on the plane = ((A.n)/|n|^2) n,
 //   edge functions w_b = ((C-q) x (A-q)).n, w_c = ((A-q) x (B-q)).n, w_a = |n|^2 - w_b - w_c
 //   (|n|^2-scaled barycentrics of q).  All >= 0: the answer is q.  Otherwise the closest
 //   point lies on an edge whose edge function is negative (at most two): clamp onto those.
 // Removing the normal component before forming the edge functions keeps them accurate for
-// far-away p; the compensated normal keeps them accurate for slivers.
-// Returns the squared distance; (v, w) are the weights of b and c.
-// Zero-area faces (|ab x ac|^2 <= 1e-12 max|e|^4) fall back to their three edges
-// (R16).
-__device__ __forceinline__ float closest_point_triangle(float3 p, float3 a, float3 b, float3 c, float& v, float& w)
+// far-away p.  Returns the squared distance; (v, w) are the weights of b and c.
+// `bound`: a triangle whose PLANE is already farther than bound cannot matter to the caller;
+// +inf is returned for it without the in-plane work (v, w untouched).
+__device__ __forceinline__ float closest_point_triangle(float3 p, const TriData& T, float bound, float& v, float& w)
 {
-    const float3 ab = b - a, ac = c - a;
-    const float3 A = a - p, B = b - p, C = c - p;
-    const float3 n = f3(diff_of_products(ab.y, ac.z, ab.z, ac.y),
-                        diff_of_products(ab.z, ac.x, ab.x, ac.z),
-                        diff_of_products(ab.x, ac.y, ab.y, ac.x));
-    const float nn = dot3(n, n);
-    const float e2 = fmaxf(dot3(ab, ab), dot3(ac, ac));
+    const float3 A = T.a - p, B = T.b - p, C = T.c - p;
     float t, best, d;
-    if (nn <= 1e-12f * e2 * e2) {
+    if (T.degenerate) {
         best = origin_to_segment(A, B, t); v = t; w = 0.0f;
         d = origin_to_segment(B, C, t); if (d < best) { best = d; v = 1.0f - t; w = t; }
         d = origin_to_segment(C, A, t); if (d < best) { best = d; v = 0.0f; w = 1.0f - t; }
         return best;
     }
-    const float rnn = 1.0f / nn;
-    const float An = dot3(A, n);
-    const float hq = An * rnn;
-    const float3 q = f3(hq * n.x, hq * n.y, hq * n.z);
+    const float An = dot3(A, T.n);
+    const float hq = An * T.rnn;
+    const float plane_d2 = An * hq;
+    if (plane_d2 > bound) return CUDART_INF_F;
+    const float3 q = f3(hq * T.n.x, hq * T.n.y, hq * T.n.z);
     const float3 Aq = A - q, Bq = B - q, Cq = C - q;
-    const float wb = dot3(cross3(Cq, Aq), n);
-    const float wc = dot3(cross3(Aq, Bq), n);
-    const float wa = nn - wb - wc;
+    const float wb = dot3(cross3(Cq, Aq), T.n);
+    const float wc = dot3(cross3(Aq, Bq), T.n);
+    const float wa = T.nn - wb - wc;
     if (wa >= 0.0f && wb >= 0.0f && wc >= 0.0f) {                 // face
-        v = fminf(wb * rnn, 1.0f);
-        w = fminf(wc * rnn, 1.0f - v);
-        return An * hq;
+        v = fminf(wb * T.rnn, 1.0f);
+        w = fminf(wc * T.rnn, 1.0f - v);
+        return plane_d2;
     }
     best = CUDART_INF_F;
     if (wc < 0.0f) { best = origin_to_segment(A, B, t); v = t; w = 0.0f; }                                    // edge ab
@@ -116,20 +125,14 @@ __device__ __forceinline__ float box_dist2(float3 p, float lx, float ly, float l
     return fmaf(dx, dx, fmaf(dy, dy, dz * dz));
 }
 
-__device__ __forceinline__ void load_tri(const PackedTri* __restrict__ tris, int k, float3& a, float3& b, float3& c, int& orig)
+// Tests sorted triangle k against the running best h; `lim` = h.d2 with the pruning slack.
+__device__ __forceinline__ void test_triangle(const PackedTri* __restrict__ tris, int k, float3 p, ClosestHit& h, float lim)
 {
-    const float4* t = reinterpret_cast<const float4*>(tris + k);
-    const float4 t0 = __ldg(t), t1 = __ldg(t + 1), t2 = __ldg(t + 2);
-    a = f3(t0.x, t0.y, t0.z); b = f3(t1.x, t1.y, t1.z); c = f3(t2.x, t2.y, t2.z);
-    orig = __float_as_int(t0.w);
-}
-
-__device__ __forceinline__ void test_triangle(const PackedTri* __restrict__ tris, int k, float3 p, ClosestHit& h)
-{
-    float3 a, b, c; int orig; float v, w;
-    load_tri(tris, k, a, b, c, orig);
-    const float d2 = closest_point_triangle(p, a, b, c, v, w);
-    if (d2 < h.d2 || (d2 == h.d2 && orig < h.tri)) { h.d2 = d2; h.tri = orig; h.k = k; h.v = v; h.w = w; }
+    const TriData T = load_tri(tris, k);
+    float v = 0.0f, w = 0.0f;
+    (void)lim;     // no plane early-out here: an exact tie (d2 == h.d2, e.g. 0 on a shared edge) must reach the index rule
+    const float d2 = closest_point_triangle(p, T, CUDART_INF_F, v, w);
+    if (d2 < h.d2 || (d2 == h.d2 && T.orig < h.tri)) { h.d2 = d2; h.tri = T.orig; h.k = k; h.v = v; h.w = w; }
 }
 
 // Full closest-point traversal.  `h` carries the initial bound on entry
@@ -162,9 +165,9 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
         const float d1 = box_dist2(p, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
         const int c0 = w3.x, c1 = w3.y;
         bool go0 = d0 <= lim, go1 = d1 <= lim;
-        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h); if (COUNT) cnt.tris++; go0 = false; lim = h.d2 * SLACK; }
+        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h, lim); if (COUNT) cnt.tris++; go0 = false; lim = h.d2 * SLACK; }
         if (go1 && c1 < 0) {
-            if (d1 <= lim) { test_triangle(tris, ~c1, p, h); if (COUNT) cnt.tris++; lim = h.d2 * SLACK; }
+            if (d1 <= lim) { test_triangle(tris, ~c1, p, h, lim); if (COUNT) cnt.tris++; lim = h.d2 * SLACK; }
             go1 = false;
         }
         if (ANY && h.d2 < bound0) return;
@@ -193,12 +196,12 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
 // Barycentric position of hit h in the primal mesh.
 __device__ __forceinline__ float3 hit_point(const PackedTri* __restrict__ tris, const ClosestHit& h)
 {
-    float3 a, b, c; int orig;
-    load_tri(tris, h.k, a, b, c, orig);
+    const float4* t = reinterpret_cast<const float4*>(tris + h.k);
+    const float4 t0 = __ldg(t), t1 = __ldg(t + 1), t2 = __ldg(t + 2);
     const float u = 1.0f - h.v - h.w;
-    return f3(fmaf(u, a.x, fmaf(h.v, b.x, h.w * c.x)),
-              fmaf(u, a.y, fmaf(h.v, b.y, h.w * c.y)),
-              fmaf(u, a.z, fmaf(h.v, b.z, h.w * c.z)));
+    return f3(fmaf(u, t0.x, fmaf(h.v, t1.x, h.w * t2.x)),
+              fmaf(u, t0.y, fmaf(h.v, t1.y, h.w * t2.y)),
+              fmaf(u, t0.z, fmaf(h.v, t1.z, h.w * t2.z)));
 }
 
 // ---------------------------------------------------------------------------

@@ -214,17 +214,17 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
                 int myJ = J;
                 if (lane < nl) {
                     const int kk = lstack[lcount - nl + lane];
-                    float3 a, b, c; int orig; float v, w;
-                    load_tri(g.tris, kk, a, b, c, orig);
+                    const TriData T = load_tri(g.tris, kk);
+                    float v, w;
                     ++cnt_tris;
-                    if (closest_point_triangle(cJ, a, b, c, v, w) < thr2J) {
+                    if (closest_point_triangle(cJ, T, thr2J, v, w) < thr2J) {
                         int lo_j = 0, hi_j = J;                           // ball_0 is empty by definition
                         while (hi_j - lo_j > 1) {
                             const int mid = (lo_j + hi_j) >> 1;
                             float3 cm; float t2;
                             probe_ball<EXT>(fam, mid, cm, t2);
                             ++cnt_tris;
-                            if (closest_point_triangle(cm, a, b, c, v, w) < t2) hi_j = mid; else lo_j = mid;
+                            if (closest_point_triangle(cm, T, t2, v, w) < t2) hi_j = mid; else lo_j = mid;
                         }
                         myJ = lo_j;
                     }
@@ -419,7 +419,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
             }
         } else if (which == KIND_TRI) {
             if (kind == KIND_TRI) {
-                test_triangle(g.tris, ~cur, xq, h);
+                test_triangle(g.tris, ~cur, xq, h, lim);
                 if (COUNT) ++n_tris;
                 lim = h.d2 * SLACK;
                 cur = CUR_NONE;
