@@ -15,6 +15,20 @@
 
 #define MCS_STACK 96      // >= 63 Morton bits + log2(F) index-tie levels
 
+// 256-bit read-only global load (sm_100: LDG.E.256).  A divergent warp pays one L1
+// wavefront per lane and per load instruction whatever its width, and that wavefront rate
+// (one per cycle per SM) is what bounds the walk kernel: 32-byte loads halve the wavefronts
+// of a 64-byte node or triangle.  p must be 32-byte aligned.
+struct __align__(32) Vec8 { float4 lo, hi; };
+__device__ __forceinline__ Vec8 ldg256(const void* p)
+{
+    Vec8 r;
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+                 : "l"(p));
+    return r;
+}
+
 struct ClosestHit {
     float d2;      // squared distance
     int   tri;     // ORIGINAL face index (-1: none)
@@ -71,8 +85,8 @@ __device__ __forceinline__ TriData unpack_tri(float4 t0, float4 t1, float4 t2, f
 
 __device__ __forceinline__ TriData load_tri(const PackedTri* __restrict__ tris, int k)
 {
-    const float4* t = reinterpret_cast<const float4*>(tris + k);
-    return unpack_tri(__ldg(t), __ldg(t + 1), __ldg(t + 2), __ldg(t + 3));
+    const Vec8 u0 = ldg256(tris + k), u1 = ldg256(reinterpret_cast<const char*>(tris + k) + 32);
+    return unpack_tri(u0.lo, u0.hi, u1.lo, u1.hi);
 }
 
 // Closest point of triangle T to p, computed on the triangle translated by -p (A, B, C =
@@ -157,9 +171,9 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
     const float SLACK = 1.0f + 4e-6f;
     float lim = h.d2 * SLACK;
     for (;;) {
-        const float4* nd = reinterpret_cast<const float4*>(nodes + node);
-        const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
-        const int4 w3 = __ldg(reinterpret_cast<const int4*>(nd + 3));
+        const Vec8 n0 = ldg256(nodes + node), n1 = ldg256(reinterpret_cast<const char*>(nodes + node) + 32);
+        const float4 w0 = n0.lo, w1 = n0.hi, w2 = n1.lo;
+        const int4 w3 = make_int4(__float_as_int(n1.hi.x), __float_as_int(n1.hi.y), __float_as_int(n1.hi.z), __float_as_int(n1.hi.w));
         if (COUNT) cnt.nodes++;
         const float d0 = box_dist2(p, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y);
         const float d1 = box_dist2(p, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);

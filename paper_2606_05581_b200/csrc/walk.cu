@@ -241,9 +241,9 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
                 int c0 = 0, c1 = 0;
                 if (lane < np) {
                     const int node = nstack[ncount - np + lane];
-                    const float4* nd = reinterpret_cast<const float4*>(g.nodes + node);
-                    const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
-                    const int2 ch = __ldg(reinterpret_cast<const int2*>(nd + 3));
+                    const Vec8 n0 = ldg256(g.nodes + node), n1 = ldg256(reinterpret_cast<const char*>(g.nodes + node) + 32);
+                    const float4 w0 = n0.lo, w1 = n0.hi, w2 = n1.lo;
+                    const int2 ch = make_int2(__float_as_int(n1.hi.x), __float_as_int(n1.hi.y));
                     ++cnt_nodes;
                     c0 = ch.x; c1 = ch.y;
                     const float lim = thr2J * SLACK;
@@ -403,9 +403,9 @@ walk_kernel(WalkGeom g, WalkArgs a)
 
         if (which == KIND_NODE) {
             if (kind == KIND_NODE) {
-                const float4* nd = reinterpret_cast<const float4*>(g.nodes + cur);
-                const float4 w0 = __ldg(nd), w1 = __ldg(nd + 1), w2 = __ldg(nd + 2);
-                const int2 ch = __ldg(reinterpret_cast<const int2*>(nd + 3));
+                const Vec8 n0 = ldg256(g.nodes + cur), n1 = ldg256(reinterpret_cast<const char*>(g.nodes + cur) + 32);
+                const float4 w0 = n0.lo, w1 = n0.hi, w2 = n1.lo;
+                const int2 ch = make_int2(__float_as_int(n1.hi.x), __float_as_int(n1.hi.y));
                 if (COUNT) { ++n_nodes; ++q_nodes; }
                 const float d0 = box_dist2(xq, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y);
                 const float d1 = box_dist2(xq, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
