@@ -393,13 +393,17 @@ walk_kernel(WalkGeom g, WalkArgs a)
         }
         const int kind = busy ? (cur == CUR_NONE ? KIND_TRANS : (cur >= 0 ? KIND_NODE : KIND_TRI))
                               : (exhausted ? KIND_IDLE : KIND_TRANS);
-        const unsigned m0 = __ballot_sync(FULL, (kind & 1) != 0), m1 = __ballot_sync(FULL, (kind & 2) != 0);
-        if ((m0 | m1) == 0) break;
-        // vote: the kind most lanes wait for (ties: NODE, then TRI)
-        const int n_node = __popc(m0 & ~m1), n_tri = __popc(m1 & ~m0), n_trans = __popc(m0 & m1);
-        int which = KIND_NODE, best = n_node;
-        if (n_tri > best) { which = KIND_TRI; best = n_tri; }
-        if (n_trans > best) { which = KIND_TRANS; best = n_trans; }
+        // fast path: at least half of the warp waits for a node visit
+        const unsigned m_node = __ballot_sync(FULL, kind == KIND_NODE);
+        int which = KIND_NODE;
+        if (__popc(m_node) < 16) {
+            const unsigned m_tri = __ballot_sync(FULL, kind == KIND_TRI), m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
+            if ((m_node | m_tri | m_trans) == 0) break;
+            // vote: the kind most lanes wait for (ties: NODE, then TRI)
+            int best = __popc(m_node);
+            if (__popc(m_tri) > best) { which = KIND_TRI; best = __popc(m_tri); }
+            if (__popc(m_trans) > best) { which = KIND_TRANS; }
+        }
 
         if (which == KIND_NODE) {
             if (kind == KIND_NODE) {
