@@ -622,6 +622,34 @@ static void fill_sample(const orc_geom *g, const int32_t *tri, const float *bary
     if (normal) for (int k = 0; k < 3; ++k) S->n[k] = normal[3*i+k];
 }
 
+/* One walk (sample i, walk w) of Alg. 2 lines 273-285 / Eq. 32 from the tangent ball B of
+ * sample S: start point, walk-on-spheres, exit record, weight. */
+static void run_one_walk(const orc_geom *g, const orc_params *P, int exterior, const orc_sample *S,
+                         const orc_ball *Bp, int64_t i, int w, orc_record *R)
+{
+    const int W = P->walks_per_sample;
+    const orc_ball B = *Bp;
+    memset(R, 0, sizeof *R);
+    R->sample = i; R->tri_t = -1;
+    if (!(B.r > 0.0)) { R->steps = -2; return; }           /* discarded sample */
+    double factor = sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, R->z);
+    orc_hit h;
+    int steps = exterior ? walk_on_spheres_kelvin(g, P, (uint32_t)i, (uint32_t)w, R->z, &h)
+                         : walk_on_spheres(g, P, (uint32_t)i, (uint32_t)w, R->z, &h);
+    R->steps = steps;
+    if (steps < 0) return;                                   /* truncated: contributes nothing */
+    R->tri_t = h.tri;
+    memcpy(R->bary_t, h.bary, sizeof h.bary);
+    memcpy(R->t, h.cp, sizeof h.cp);
+    double wgt = (S->a / W) * factor;                        /* |dOmega| |dB| J / (2N), Alg. 2 */
+    if (exterior) {
+        double tt[3]; sub3(h.cp, P->origin, tt);
+        /* |s*|^3 / |t*|, Eq. 32;  1/|t*| = |t - o| */
+        wgt *= B.sstar_norm * B.sstar_norm * B.sstar_norm * norm3(tt);
+    }
+    R->weight = wgt;
+}
+
 /*
  * Run every walk of every sample and write one record per walk at slot
  * sample*W + walk (then the killing walks).  exterior = 0: Alg. 2; 1: Eq. 32.
@@ -642,28 +670,8 @@ int64_t orc_run_walks(const orc_geom *g, const orc_params *P, int exterior,
         if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
         else          orc_tangent_ball_interior(g, P, &S, &B);
         if (balls_out) { balls_out[5*i] = B.r; balls_out[5*i+1] = B.c[0]; balls_out[5*i+2] = B.c[1]; balls_out[5*i+3] = B.c[2]; balls_out[5*i+4] = B.sstar_norm; }
-        for (int w = 0; w < W; ++w) {
-            orc_record *R = rec + i * W + w;
-            memset(R, 0, sizeof *R);
-            R->sample = i; R->tri_t = -1;
-            if (!(B.r > 0.0)) { R->steps = -2; continue; }      /* discarded sample */
-            double factor = sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, R->z);
-            orc_hit h;
-            int steps = exterior ? walk_on_spheres_kelvin(g, P, (uint32_t)i, (uint32_t)w, R->z, &h)
-                                 : walk_on_spheres(g, P, (uint32_t)i, (uint32_t)w, R->z, &h);
-            R->steps = steps;
-            if (steps < 0) continue;                              /* truncated: contributes nothing */
-            R->tri_t = h.tri;
-            memcpy(R->bary_t, h.bary, sizeof h.bary);
-            memcpy(R->t, h.cp, sizeof h.cp);
-            double wgt = (S.a / W) * factor;                      /* |dOmega| |dB| J / (2N), Alg. 2 */
-            if (exterior) {
-                double tt[3]; sub3(h.cp, P->origin, tt);
-                /* |s*|^3 / |t*|, Eq. 32;  1/|t*| = |t - o| */
-                wgt *= B.sstar_norm * B.sstar_norm * B.sstar_norm * norm3(tt);
-            }
-            R->weight = wgt;
-        }
+        for (int w = 0; w < W; ++w)
+            run_one_walk(g, P, exterior, &S, &B, i, w, rec + i * W + w);
     }
     int64_t n_rec = n_s * W;
     if (exterior && P->include_killing) {
@@ -684,6 +692,50 @@ int64_t orc_run_walks(const orc_geom *g, const orc_params *P, int exterior,
             R->weight = 4.0 * ORC_PI * norm3(tt) / (double)P->n_kill_walks;    /* 4 pi / |t0*| */
         }
         n_rec += P->n_kill_walks;
+    }
+    return n_rec;
+}
+
+/*
+ * Sampled outputs of the same run (parity at sizes the full oracle cannot finish): the
+ * records of walks w = 0..n_w-1 of the listed samples, rec[k*n_w + w] for sample ids[k],
+ * and of the first n_kill_first killing walks after them.  Same Philox counters as the
+ * full run: the counter holds the sample's index in the full arrays, not k.
+ */
+int64_t orc_run_walks_subset(const orc_geom *g, const orc_params *P, int exterior,
+                             const int32_t *tri, const float *bary, const float *weight,
+                             const float *normal, const int64_t *ids, int64_t n_ids, int n_w,
+                             int64_t n_kill_first, orc_record *rec)
+{
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < n_ids; ++k) {
+        const int64_t i = ids[k];
+        orc_sample S;
+        orc_ball B;
+        fill_sample(g, tri, bary, weight, normal, NULL, i, &S);
+        if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
+        else          orc_tangent_ball_interior(g, P, &S, &B);
+        for (int w = 0; w < n_w; ++w)
+            run_one_walk(g, P, exterior, &S, &B, i, w, rec + k * n_w + w);
+    }
+    int64_t n_rec = n_ids * n_w;
+    if (exterior && P->include_killing) {
+        #pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t j = 0; j < n_kill_first; ++j) {
+            orc_record *R = rec + n_rec + j;
+            memset(R, 0, sizeof *R);
+            R->sample = -1; R->tri_t = -1;
+            orc_hit h;
+            int steps = walk_on_spheres_kelvin(g, P, ORC_KILLING_SAMPLE, (uint32_t)j, R->z, &h);
+            R->steps = steps;
+            if (steps < 0) continue;
+            R->tri_t = h.tri;
+            memcpy(R->bary_t, h.bary, sizeof h.bary);
+            memcpy(R->t, h.cp, sizeof h.cp);
+            double tt[3]; sub3(h.cp, P->origin, tt);
+            R->weight = 4.0 * ORC_PI * norm3(tt) / (double)P->n_kill_walks;    /* 4 pi / |t0*| */
+        }
+        n_rec += n_kill_first;
     }
     return n_rec;
 }

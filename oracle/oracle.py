@@ -26,6 +26,7 @@ def _load():
         _lib.orc_max_vertex_norm.restype = C.c_double
         _lib.orc_total_area.restype = C.c_double
         _lib.orc_run_walks.restype = C.c_int64
+        _lib.orc_run_walks_subset.restype = C.c_int64
         _lib.orc_num_threads.restype = C.c_int
         for f in ("orc_sizeof_record", "orc_sizeof_params", "orc_sizeof_geom"):
             getattr(_lib, f).restype = C.c_size_t
@@ -215,6 +216,26 @@ class Oracle:
                                    C.c_int64(n_s), ptr(rec), ptr(balls))
         assert n == len(rec)
         return rec, balls
+
+    def run_walks_subset(self, params: OracleParams, exterior: bool, tri, bary, weight, ids, n_w,
+                         n_kill_first=0, normal=None):
+        """Records of walks 0..n_w-1 of the samples `ids` of the FULL arrays (same Philox
+        counters as the full run), then of the first n_kill_first killing walks."""
+        tri = np.ascontiguousarray(tri, np.int32)
+        bary = np.ascontiguousarray(bary, np.float32)
+        weight = np.ascontiguousarray(weight, np.float32)
+        ids = np.ascontiguousarray(ids, np.int64)
+        if normal is not None:
+            normal = np.ascontiguousarray(normal, np.float32)
+        cp = self._params(params, exterior)
+        nk = int(n_kill_first) if (exterior and params.include_killing) else 0
+        rec = np.zeros(len(ids) * n_w + nk, RECORD_DTYPE)
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        n = self.lib.orc_run_walks_subset(C.byref(self.geom.c), C.byref(cp), C.c_int(int(exterior)),
+                                          ptr(tri), ptr(bary), ptr(weight), ptr(normal), ptr(ids),
+                                          C.c_int64(len(ids)), C.c_int(int(n_w)), C.c_int64(nk), ptr(rec))
+        assert n == len(rec)
+        return rec
 
     def accumulate_hat(self, rec, tri, bary, want_var=False):
         K = self.geom.c.V

@@ -353,3 +353,25 @@ def test_interior_blocks_vanish_and_exterior_couples_with_decay():
             assert abs(series - 1.4553) < 1e-3
             assert 0.90 * series < cap < 1.01 * series          # level-1 polyhedra are a bit smaller
     assert norms[0] > 0 and norms[1] > 0 and norms[1] < 0.7 * norms[0]
+
+
+def test_subset_entry_reproduces_the_full_run():
+    """orc_run_walks_subset (sampled outputs for full-size GPU parity) must return exactly the
+    records of the full run: same Philox counters (index in the full arrays), same arithmetic."""
+    from synth import icosphere, vertex_cell_samples
+    v, f = icosphere(1)
+    smp = vertex_cell_samples(v, f, 3, seed=5)
+    orc = Oracle(mesh_geom(v, f))
+    for ext in (False, True):
+        p = OracleParams(seed=9, walks_per_sample=6, eps=1e-3, include_killing=ext, n_kill_walks=40 if ext else 0,
+                         origin=(0.1, 0.0, -0.05))
+        full, _ = orc.run_walks(p, ext, smp["tri"], smp["bary"], smp["weight"])
+        ids = np.array([0, 7, 31, len(smp["weight"]) - 1])
+        sub = orc.run_walks_subset(p, ext, smp["tri"], smp["bary"], smp["weight"], ids, 4, n_kill_first=10)
+        for k, i in enumerate(ids):
+            for w in range(4):
+                a, b = full[i * 6 + w], sub[k * 4 + w]
+                assert a.tobytes() == b.tobytes()
+        if ext:
+            n_main = len(smp["weight"]) * 6
+            assert full[n_main:n_main + 10].tobytes() == sub[len(ids) * 4:].tobytes()
