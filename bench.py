@@ -172,6 +172,40 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------
+# multi-rank host logic (replicas only); covered on CPU with gloo
+# ------------------------------------------------------------------------------
+def replica_seed(seed: int, rank: int) -> int:
+    """Rank r of an N-replica run uses Philox seed + r: independent walks, same workload."""
+    return seed + rank
+
+
+def max_over_ranks(x: float, device, world: int) -> float:
+    """Device-timed durations are reduced with MAX over ranks (never wall clock)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float, device, world: int) -> float:
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_step: float, world: int, seconds_per_step: float) -> float:
+    """Weak scaling: every rank processes units_per_rank_step per step; the job's rate is the sum."""
+    return world * units_per_rank_step / seconds_per_step
+
+
+# ------------------------------------------------------------------------------
 # this repo's CUDA path
 # ------------------------------------------------------------------------------
 def run_ours(args):
@@ -191,7 +225,7 @@ def run_ours(args):
     api.lib()
 
     # replicas only: rank r runs the same workload with Philox seed + r
-    seed = args.seed + rank
+    seed = replica_seed(args.seed, rank)
     wl = make_workload(args.level, args.walks_per_vertex, args.points_per_vertex, args.seed)
     n_walks = wl["n_s"] * wl["W"]
     v_h = torch.as_tensor(wl["v"]).pin_memory()
@@ -254,12 +288,11 @@ def run_ours(args):
     clk = clocks.stop()
     api.profile_enable(False)
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev, world)
     ms_per_step = ms / args.steps
-    value = world * steps_per_step / (ms_per_step * 1e-3)
+    job_steps = sum_over_ranks(steps_per_step, dev, world)        # replicas differ by their Philox seed
+    job_queries = sum_over_ranks(queries_per_step, dev, world)
+    value = job_steps / (ms_per_step * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     oi_h = torch.empty((wl["V"], wl["V"]), dtype=torch.float32, pin_memory=True)
@@ -275,11 +308,8 @@ def run_ours(args):
         flush.fill_(1)
     barrier()
     e2e_t = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_t], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_t = float(t.item())
-    e2e_value = world * steps_per_step / e2e_t
+    e2e_t = max_over_ranks(e2e_t, dev, world)
+    e2e_value = job_steps / e2e_t
 
     if rank != 0:
         if world > 1:
@@ -340,7 +370,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": config_dict(wl, args),
-            "queries_per_s": world * queries_per_step / (ms_per_step * 1e-3),
+            "queries_per_s": job_queries / (ms_per_step * 1e-3),
             "dtn_matrices_per_s": world * 2.0 / (ms_per_step * 1e-3),
             "walk_steps_per_step": steps_per_step, "queries_per_step": queries_per_step,
             "phase_ms_per_step": {"prep": float(np.sum(prep_ms)) / args.steps, "walk": t_kernel * 1e3,
