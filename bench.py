@@ -70,9 +70,11 @@ class ClockSampler:
         self.thread = None
 
     def start(self):
+        if os.environ.get("MCS_BENCH_NO_CLOCKS"):
+            return
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -268,15 +270,16 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    clocks = ClockSampler(local)
+    clocks.start()                 # before the warm-up: nvidia-smi's own start-up stays out of the timed region
     for _ in range(args.warmup):
         step(False)
         flush.fill_(1)
     api.profile_enable(True)
     stream = torch.cuda.current_stream(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    clocks = ClockSampler(local)
-    clocks.start()
     barrier()
+    clocks.rows.clear()            # keep the samples taken during the timed region only
     launches0 = api.launch_count()
     e0.record(stream)
     for _ in range(args.steps):
@@ -388,7 +391,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--level", type=int, default=4, help="icosphere subdivision level (configs[1]: 4)")

@@ -160,6 +160,13 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
     // one staging block: verts | faces | tri | bary | weight | normal
     size_t off_v = 0, off_f = align_up(off_v + nb_v), off_t = align_up(off_f + nb_f), off_b = align_up(off_t + nb_tri),
            off_w = align_up(off_b + nb_bary), off_n = align_up(off_w + nb_w), in_total = align_up(off_n + nb_n) + 256;
+    {   // keep the stream-ordered pool's memory across calls (default: released at every synchronisation)
+        int dev = 0; cudaMemPool_t pool;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
     char* d_in = nullptr; float* d_out = nullptr; void* d_ws = nullptr;
     mcs_bvh* bvh = nullptr;
     int rc = MCS_OK;
