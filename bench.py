@@ -112,6 +112,20 @@ class ClockSampler:
                 "power_w_max": float(max(power)), "samples": len(sm)}
 
 
+def read_traffic():
+    """DRAM bytes of the walk-kernel launches of one step, from the committed ncu capture (profiles/)."""
+    path = os.path.join(ROOT, "profiles", "walk_kernel_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    total = 0
+    with open(path) as fh:
+        for line in fh.read().splitlines()[1:]:
+            p = line.split(",")
+            if len(p) == 3:
+                total += int(p[1]) + int(p[2])
+    return total or None
+
+
 def read_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -355,7 +369,8 @@ def run_ours(args):
         "peak": level_gbs if mem_bound else fp32_tflops,
         "unit": "GB/s" if mem_bound else "TFLOP/s",
         "frac": max(t_mem, t_alu) / t_kernel,
-        "traffic": None,
+        "traffic": read_traffic(),
+        "traffic_note": "dram bytes read+write of the two walk_kernel launches of one step (ncu --set full, profiles/walk_kernel_traffic.csv); algorithmic node+triangle bytes are served from L2",
         "peak_source": (f"{level} read bandwidth measured live by mcs_measure_l2_gbs (tree is {tree_bytes / 1e6:.2f} MB, "
                         f"{level}-resident); HBM {hbm_gbs:.0f} GB/s {hbm_src}; FP32 {fp32_tflops:.1f} TFLOP/s measured live"),
         "algorithmic": "bytes = 64 B x nodes visited + 48 B x triangles tested; flops = 36 x nodes + 80 x triangles (DESIGN.md)",
