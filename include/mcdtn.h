@@ -140,7 +140,7 @@ typedef struct {
 
 typedef struct {                 /* host; filled when passed non-NULL (forces a stream sync) */
     int64_t n_samples, n_discarded;       /* samples whose tangent ball degenerated */
-    int64_t n_walks, n_truncated;         /* walks started / cut at max_steps       */
+    int64_t n_walks, n_truncated;         /* walks started / cut at max_steps or outside the AABB */
     int64_t n_steps;                      /* position updates x += d*omega                         */
     int64_t n_queries;                    /* closest-point queries: every WoS iteration + one tangent-ball traversal per sample */
     int64_t n_nodes_visited, n_tris_tested;   /* traversal work actually done (flop/byte model)    */
@@ -219,7 +219,8 @@ size_t mcs_walk_workspace_bytes(const mcs_samples* samples);
 size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_basis* basis, int64_t n_records);
 
 /* A2-A6: run every walk and write records [n_s*W (+ n_kill_walks)] and, if non-NULL,
- * steps [same length] (jumps taken; -1 truncated; -2 sample discarded). */
+ * steps [same length] (jumps taken; -1 truncated at max_steps; -2 sample discarded; -3 interior
+ * walker left the bounding box of the mesh, cut and counted as truncated: DESIGN.md R10b). */
 int mcs_run_walks(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_params* params,
                   int exterior, void* workspace, size_t workspace_bytes,
                   mcs_record* records, int32_t* steps, mcs_stats* host_stats, void* stream);

@@ -327,6 +327,20 @@ static void face_normal_area(const orc_geom *g, int64_t f, double n[3], double *
     if (l > 0.0) { n[0] /= l; n[1] /= l; n[2] /= l; }
 }
 
+/* Diagonal of the AABB of the vertices referenced by faces (escape test [R10b]). */
+double orc_aabb_diagonal(const orc_geom *g)
+{
+    if (g->kind != 0 || g->F < 1) return 0.0;
+    double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    for (int64_t f = 0; f < g->F; ++f)
+        for (int c = 0; c < 3; ++c) {
+            double p[3]; load_vertex(g, g->faces[3*f + c], p);
+            for (int k = 0; k < 3; ++k) { if (p[k] < lo[k]) lo[k] = p[k]; if (p[k] > hi[k]) hi[k] = p[k]; }
+        }
+    double d[3] = { hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2] };
+    return norm3(d);
+}
+
 /* r_max = half of the shortest AABB side ("maximum diameter ... shortest side
  * length of the mesh's axis-aligned bounding box").  For the
  * exterior the box is that of the Kelvin-inverted vertices kappa(v - origin). */
@@ -391,6 +405,7 @@ typedef struct {
     int64_t n_kill_walks;
     double origin[3];               /* Kelvin origin [R12]               */
     double Rmax_norm;               /* orc_max_vertex_norm(), exterior only             */
+    double escape_radius;           /* [R10b] interior: AABB diagonal; 0 = no escape test */
 } orc_params;
 
 typedef struct {                    /* one boundary sample            */
@@ -534,7 +549,11 @@ static void step_direction(uint64_t seed, uint32_t sample, uint32_t walk, uint32
  * WalkOnSpheres in the primal domain  [R9]:
  * repeat { closest point; stop if D < eps; jump to a uniform point of the
  * sphere of radius D }.  Returns the number of jumps, or -1 if max_steps
- * jumps did not reach the shell [R10].
+ * jumps did not reach the shell [R10], or -3 if the walker left the bounding box
+ * of the surface [R10b]: every point of the AABB is within its diagonal of every
+ * surface point, so D > diagonal proves the walker is outside the box, hence
+ * outside the solid -- an "unbounded" walk of an open or mis-oriented surface
+ * (PAPER.md:548, 638-640).  Such a walk contributes nothing, like a truncated one.
  */
 static int walk_on_spheres(const orc_geom *g, const orc_params *P, uint32_t sample, uint32_t walk,
                            const double z[3], orc_hit *h)
@@ -543,6 +562,7 @@ static int walk_on_spheres(const orc_geom *g, const orc_params *P, uint32_t samp
     for (int k = 0; ; ++k) {
         orc_closest_point(g, x, h);
         if (h->dist < P->eps) return k;
+        if (P->escape_radius > 0.0 && h->dist > P->escape_radius) return -3;
         if (k == P->max_steps) return -1;
         double w[3];
         step_direction(P->seed, sample, walk, (uint32_t)(k + 1), w);

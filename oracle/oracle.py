@@ -23,6 +23,7 @@ def _load():
         _lib.orc_closest_point_triangle.restype = C.c_double
         _lib.orc_closest_point_triangle_alt.restype = C.c_double
         _lib.orc_rmax.restype = C.c_double
+        _lib.orc_aabb_diagonal.restype = C.c_double
         _lib.orc_max_vertex_norm.restype = C.c_double
         _lib.orc_total_area.restype = C.c_double
         _lib.orc_run_walks.restype = C.c_int64
@@ -48,7 +49,8 @@ class _Params(C.Structure):
                 ("eps", C.c_double), ("cap_half_angle_deg", C.c_double), ("rmax", C.c_double),
                 ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32),
-                ("n_kill_walks", C.c_int64), ("origin", C.c_double * 3), ("Rmax_norm", C.c_double)]
+                ("n_kill_walks", C.c_int64), ("origin", C.c_double * 3), ("Rmax_norm", C.c_double),
+                ("escape_radius", C.c_double)]
 
 
 RECORD_DTYPE = np.dtype([("sample", np.int64), ("tri_t", np.int64), ("bary_t", np.float64, 3),
@@ -187,6 +189,7 @@ class Oracle:
             cp.rmax = float(p.rmax)
         else:
             cp.rmax = float(np.float32(p.rmax_scale)) * self.rmax(exterior, p.origin)
+        cp.escape_radius = 0.0 if exterior else float(np.float32(self.lib.orc_aabb_diagonal(C.byref(self.geom.c))))
         if p.Rmax_norm is not None:
             cp.Rmax_norm = float(p.Rmax_norm)
         elif self.geom.c.kind == 0:

@@ -453,6 +453,12 @@ walk_kernel(WalkGeom g, WalkArgs a)
                         done = true;
                     }
                 }
+                if (!done && !EXT && radius > a.escape) {                // left the bounding box: DESIGN.md R10b
+                    a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                    if (a.steps) a.steps[slot] = -3;
+                    ++n_trunc;
+                    done = true;
+                }
                 if (!done) {
                     if (k == a.max_steps) {                              // DESIGN.md R10
                         a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
@@ -714,6 +720,10 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.inv_q0 = 1.0f / a.q0;
     a.importance = p->importance_sample; a.antithetic = p->antithetic;
     a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
+    {
+        const float dx = hi.x - lo.x, dy = hi.y - lo.y, dz = hi.z - lo.z;
+        a.escape = exterior ? 3.0e38f : sqrtf(dx * dx + dy * dy + dz * dz);
+    }
     a.key0 = (uint32_t)(p->seed & 0xFFFFFFFFu); a.key1 = (uint32_t)(p->seed >> 32);
     a.records = records; a.steps = steps;
     a.work_counter = stats + ST_WORK; a.stats = stats;

@@ -28,6 +28,7 @@ struct WalkArgs {
     int   importance, antithetic;
     float eps, q0, inv_q0;
     float ox, oy, oz, Rmax;
+    float escape;                  // interior: AABB diagonal (R10b); exterior: +inf
     uint32_t key0, key1;
     float4* records;               // mcs_record viewed as float4
     int32_t* steps;

@@ -375,3 +375,24 @@ def test_subset_entry_reproduces_the_full_run():
         if ext:
             n_main = len(smp["weight"]) * 6
             assert full[n_main:n_main + 10].tobytes() == sub[len(ids) * 4:].tobytes()
+
+
+def test_escape_rule_r10b():
+    """[R10b] an interior walker whose jump radius exceeds the AABB diagonal is outside the box: cut (-3).
+    Correctly oriented closed mesh: never happens.  Normals flipped: the tangent ball sits outside the
+    solid; the walkers that leave for good are cut long before max_steps, the others land."""
+    from synth import icosphere, vertex_cell_samples
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 1, seed=0)
+    orc = Oracle(mesh_geom(v, f))
+    p = OracleParams(seed=1, walks_per_sample=8, eps=1e-3, max_steps=4096, rmax=0.5)
+    rec, _ = orc.run_walks(p, False, smp["tri"], smp["bary"], smp["weight"])
+    assert (rec["steps"] >= 0).all()
+    vv = v[f[smp["tri"]]].astype(np.float64)
+    nrm = np.cross(vv[:, 1] - vv[:, 0], vv[:, 2] - vv[:, 0])
+    nrm /= np.linalg.norm(nrm, axis=1, keepdims=True)
+    rec, _ = orc.run_walks(p, False, smp["tri"], smp["bary"], smp["weight"], normal=-nrm.astype(np.float32))
+    st = rec["steps"]
+    assert (st == -1).sum() == 0                       # nobody needs 4096 jumps: escapes are detected
+    assert 0.005 < (st == -3).mean() < 0.5             # starts hug the surface (importance sampling): most return, some leave for good
+    assert (rec["weight"][st == -3] == 0).all() and (rec["tri_t"][st == -3] == -1).all()
