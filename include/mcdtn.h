@@ -128,14 +128,24 @@ typedef struct {
     int32_t  include_killing;    /* exterior only: second expectation of Eq. 32                */
     int64_t  n_kill_walks;       /* exterior only                                              */
     float    kelvin_origin[3];   /* exterior only: a point strictly inside the solid */
-    int32_t  output_kind;        /* 0: dense row-major fp32 [K][K]                             */
+    int32_t  output_kind;        /* 0: dense row-major fp32 [K][K] (K <= 65535);
+                                    1: sparse COO, upper triangle (any K < 2^31)                */
+    int64_t  coo_capacity;       /* output_kind 1: entries mcs_matrix.coo_* can hold (sizes the workspace) */
 } mcs_params;
 
 typedef struct {
     int32_t kind;                /* must equal params.output_kind                    */
     int32_t pad_;
     int64_t K;
-    float*  dense;               /* [K][K] row-major, overwritten                    */
+    float*  dense;               /* kind 0: [K][K] row-major, overwritten             */
+    /* kind 1: the UPPER triangle (row <= col) of the symmetric matrix in coordinate form,
+     * sorted by (row, col), one entry per (row, col); S[col][row] = S[row][col] is implied. */
+    int64_t  coo_capacity;       /* entries each of the three arrays can hold (= params.coo_capacity) */
+    int32_t* coo_row;
+    int32_t* coo_col;
+    float*   coo_val;
+    int64_t* coo_nnz;            /* device scalar: entries written.  MCS_ENOMEM when more than
+                                    coo_capacity are needed; then it holds a lower bound of the need */
 } mcs_matrix;
 
 typedef struct {                 /* host; filled when passed non-NULL (forces a stream sync) */
@@ -216,7 +226,8 @@ int mcs_tangent_balls(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_
 
 /* Workspace (bytes) of mcs_run_walks and of mcs_accumulate. */
 size_t mcs_walk_workspace_bytes(const mcs_samples* samples);
-size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_basis* basis, int64_t n_records);
+size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_basis* basis, const mcs_params* params,
+                                      int64_t n_records);
 
 /* A2-A6: run every walk and write records [n_s*W (+ n_kill_walks)] and, if non-NULL,
  * steps [same length] (jumps taken; -1 truncated at max_steps; -2 sample discarded; -3 interior

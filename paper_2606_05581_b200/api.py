@@ -49,11 +49,13 @@ class _Params(C.Structure):
                 ("eps", C.c_float), ("cap_half_angle_deg", C.c_float), ("rmax_scale", C.c_float),
                 ("rmax_override", C.c_float), ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
-                ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32)]
+                ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64)]
 
 
 class _Matrix(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64), ("dense", C.c_void_p)]
+    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64), ("dense", C.c_void_p),
+                ("coo_capacity", C.c_int64), ("coo_row", C.c_void_p), ("coo_col", C.c_void_p), ("coo_val", C.c_void_p),
+                ("coo_nnz", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -126,6 +128,8 @@ class Params:
     include_killing: bool = False
     n_kill_walks: int = 0
     kelvin_origin: tuple = (0.0, 0.0, 0.0)
+    output_kind: int = 0                 # 0 dense, 1 sparse COO (upper triangle)
+    coo_capacity: int = 0
 
     def c(self) -> _Params:
         p = _Params(seed=self.seed, walks_per_sample=self.walks_per_sample, max_steps=self.max_steps,
@@ -133,7 +137,7 @@ class Params:
                     rmax_override=self.rmax_override, bisection_iters=self.bisection_iters,
                     importance_sample=int(self.importance_sample), antithetic=int(self.antithetic),
                     include_killing=int(self.include_killing), n_kill_walks=int(self.n_kill_walks),
-                    output_kind=0)
+                    output_kind=int(self.output_kind), coo_capacity=int(self.coo_capacity))
         p.kelvin_origin[:] = [float(x) for x in self.kelvin_origin]
         return p
 
@@ -356,7 +360,7 @@ def accumulate(bvh: Bvh, samples: Samples, params: Params, records, want_stats=F
     n = records.shape[0]
     K = bvh.V
     out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
-    need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cb), C.c_int64(n)))
+    need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cb), C.byref(cp), C.c_int64(n)))
     ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
     m = _Matrix(kind=0, K=K, dense=out.data_ptr())
     st = Stats() if want_stats else None
@@ -428,3 +432,67 @@ def measure_l2_gbs(device="cuda") -> float:
     with torch.cuda.device(device):
         _check(lib().mcs_measure_l2_gbs(C.byref(o), _stream(torch.device(device))), "mcs_measure_l2_gbs")
     return o.value
+
+
+# ------------------------------------------------------------------------------
+# sparse output (output_kind 1)
+# ------------------------------------------------------------------------------
+@dataclass
+class CooMatrix:
+    """Upper triangle (row <= col) of the symmetric DtN matrix, sorted by (row, col)."""
+    K: int
+    row: torch.Tensor
+    col: torch.Tensor
+    val: torch.Tensor
+
+    @property
+    def nnz(self):
+        return int(self.row.numel())
+
+    def to_dense(self):
+        S = torch.zeros((self.K, self.K), dtype=torch.float32, device=self.val.device)
+        r, c = self.row.long(), self.col.long()
+        S[r, c] = self.val
+        S[c, r] = self.val
+        return S
+
+
+def _coo_buffers(K, capacity, device):
+    row = torch.empty(capacity, dtype=torch.int32, device=device)
+    col = torch.empty(capacity, dtype=torch.int32, device=device)
+    val = torch.empty(capacity, dtype=torch.float32, device=device)
+    nnz = torch.zeros(1, dtype=torch.int64, device=device)
+    m = _Matrix(kind=1, K=K, dense=None, coo_capacity=capacity, coo_row=row.data_ptr(), coo_col=col.data_ptr(),
+                coo_val=val.data_ptr(), coo_nnz=nnz.data_ptr())
+    return row, col, val, nnz, m
+
+
+def estimate_dtn_coo(bvh: Bvh, samples: Samples, params: Params, exterior: bool, capacity: int | None = None,
+                     want_stats=False, max_retries=6):
+    """DtN matrix in sparse COO form (any K): mcs_estimate_dtn_* with output_kind 1.  When the capacity
+    guess is too small the library reports MCS_ENOMEM with a lower bound of the need; the call is
+    repeated with a larger buffer."""
+    import dataclasses
+    K = bvh.V
+    n_rec = num_records(samples, params, exterior)
+    cap = int(capacity) if capacity else max(4096, min(K * (K + 1) // 2, 4 * n_rec))
+    fn = lib().mcs_estimate_dtn_exterior if exterior else lib().mcs_estimate_dtn_interior
+    for _ in range(max_retries):
+        p = dataclasses.replace(params, output_kind=1, coo_capacity=cap)
+        cs, cb, cp = samples.c(), _basis(bvh), p.c()
+        need = int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
+        ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+        row, col, val, nnz, m = _coo_buffers(K, cap, bvh.device)
+        st = Stats()
+        with torch.cuda.device(bvh.device):
+            rc = fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(ws), C.c_size_t(need), C.byref(m),
+                    C.byref(st), _stream(bvh.device))
+        if rc == MCS_ENOMEM and int(nnz.item()) > cap:
+            cap = min(K * (K + 1) // 2, max(2 * cap, 2 * int(nnz.item())))
+            del ws, row, col, val
+            continue
+        _check(rc, "mcs_estimate_dtn (coo)")
+        n = int(nnz.item())
+        out = CooMatrix(K, row[:n], col[:n], val[:n])
+        return (out, st) if want_stats else out
+    raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")

@@ -239,10 +239,11 @@ count_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32_
     counts[i] = c;
 }
 
+template <typename KeyT>
 __global__ void __launch_bounds__(AT)
 expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32_t* __restrict__ pair_counts,
                       long long n_slots, const uint32_t* __restrict__ offsets,
-                      uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
+                      KeyT* __restrict__ keys, uint32_t* __restrict__ vals)
 {
     const long long i = (long long)blockIdx.x * AT + threadIdx.x;
     if (i >= n_slots) return;
@@ -257,7 +258,7 @@ expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32
                 // sum over the pair's walks of wgt * d_p d_q,  d = b(s) - b(t)
                 float e = r.w * B.ds[p] * B.ds[q] - B.ds[p] * B.At[q] - B.At[p] * B.ds[q];
                 if (B.tmask[p] && B.tmask[q]) e += moment_block(r, B.tmask[p], B.tmask[q]);
-                keys[o] = (uint32_t)((long long)B.idx[p] * a.K + B.idx[q]);
+                keys[o] = (KeyT)((long long)B.idx[p] * a.K + B.idx[q]);
                 vals[o] = __float_as_uint(e);
                 ++o;
             }
@@ -304,6 +305,88 @@ carry_fixup_kernel(const uint32_t* __restrict__ carry_key, const float* __restri
     float total = carry_sum[b];
     for (long long j = b + 1; j < n_tiles && carry_key[j] == key; ++j) total += carry_sum[j];
     S[key] += total;
+}
+
+// ---------------------------------------------------------------------------
+// Sparse output (output_kind 1): the same run sums, written compactly.  Pass 1 counts the
+// run heads of every tile; after an exclusive scan a run's output slot is
+// (heads before its tile) + (heads in the tile up to its own) - 1.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(RT)
+count_heads_kernel(const unsigned long long* __restrict__ keys, long long n, uint32_t* __restrict__ tile_heads)
+{
+    __shared__ int s_cnt[RT / 32];
+    const long long i = (long long)blockIdx.x * RT + threadIdx.x;
+    const bool head = i < n && (i == 0 || keys[i - 1] != keys[i]);
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+    if ((threadIdx.x & 31) == 0) s_cnt[threadIdx.x >> 5] = __popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int w = 0; w < RT / 32; ++w) t += s_cnt[w];
+        tile_heads[blockIdx.x] = (uint32_t)t;
+    }
+}
+
+__global__ void __launch_bounds__(RT)
+reduce_runs_compact_kernel(const unsigned long long* __restrict__ keys, const uint32_t* __restrict__ vals, long long n,
+                           const uint32_t* __restrict__ tile_offset,
+                           unsigned long long* __restrict__ out_keys, float* __restrict__ out_vals,
+                           unsigned long long* __restrict__ carry_key, float* __restrict__ carry_sum)
+{
+    __shared__ float s_tail[RT / 32][1];
+    __shared__ int s_has_head[RT / 32];
+    __shared__ int s_cnt[RT / 32];
+    const long long i = (long long)blockIdx.x * RT + threadIdx.x;
+    const bool valid = i < n;
+    const unsigned long long key = valid ? keys[i] : ~0ull;
+    const bool head = valid && (i == 0 || keys[i - 1] != key);
+    const bool last = valid && (threadIdx.x == RT - 1 || i + 1 >= n || keys[i + 1] != key);
+    float v[1] = { valid ? __uint_as_float(vals[i]) : 0.0f };
+    const bool headed = block_segmented_scan<1, RT / 32>(v, head || !valid, s_tail, s_has_head);
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) s_cnt[warp] = __popc(m);
+    if (threadIdx.x == 0) carry_key[blockIdx.x] = ~0ull;
+    __syncthreads();
+    if (last) {
+        if (headed) {
+            int heads_upto = __popc(m & (0xFFFFFFFFu >> (31 - lane)));           // heads at or before me: my run's head is the last
+            for (int w = 0; w < warp; ++w) heads_upto += s_cnt[w];
+            const long long slot = (long long)tile_offset[blockIdx.x] + heads_upto - 1;
+            out_keys[slot] = key; out_vals[slot] = v[0];
+        } else {
+            carry_key[blockIdx.x] = key; carry_sum[blockIdx.x] = v[0];
+        }
+    }
+}
+
+// Leading parts of runs that began in an earlier tile, added in tile order.  The run's slot is
+// the last one opened before the tile: tile_offset[tile] - 1.
+__global__ void __launch_bounds__(AT)
+carry_fixup_compact_kernel(const unsigned long long* __restrict__ carry_key, const float* __restrict__ carry_sum,
+                           long long n_tiles, const uint32_t* __restrict__ tile_offset, float* __restrict__ out_vals)
+{
+    const long long b = (long long)blockIdx.x * AT + threadIdx.x;
+    if (b >= n_tiles) return;
+    const unsigned long long key = carry_key[b];
+    if (key == ~0ull) return;
+    if (b > 0 && carry_key[b - 1] == key) return;
+    float total = carry_sum[b];
+    for (long long j = b + 1; j < n_tiles && carry_key[j] == key; ++j) total += carry_sum[j];
+    out_vals[(long long)tile_offset[b] - 1] += total;
+}
+
+__global__ void __launch_bounds__(AT)
+coo_write_kernel(const unsigned long long* __restrict__ keys, const float* __restrict__ vals, long long n, long long K,
+                 int32_t* __restrict__ row, int32_t* __restrict__ col, float* __restrict__ val)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n) return;
+    const unsigned long long k = keys[i];
+    row[i] = (int32_t)(k / (unsigned long long)K);
+    col[i] = (int32_t)(k % (unsigned long long)K);
+    val[i] = vals[i];
 }
 
 __global__ void __launch_bounds__(AT)
@@ -402,7 +485,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (n_entries == 0) continue;
         entries_total += n_entries;
-        mcs_note_launch(), expand_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts, keys, vals);
+        mcs_note_launch(), expand_entries_kernel<uint32_t><<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts, keys, vals);
         rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
         const long long n_tiles = ceil_div64(n_entries, RT);
@@ -415,5 +498,146 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_ENTRIES, &entries_total, 8, cudaMemcpyHostToDevice, st));
     MCS_CUDA_TRY(cudaGetLastError());
     if (stats_dev) MCS_CUDA_TRY(cudaStreamSynchronize(st));     // entries_total lives on this stack frame
+    return MCS_OK;
+}
+
+// ---------------------------------------------------------------------------
+// Sparse (COO) accumulation, any K < 2^31: 64-bit keys.  The list of unique entries found
+// so far sits at the front of the key buffer; every chunk appends its entries behind it,
+// the whole is stable-sorted and reduced into the other buffer.  The running list comes
+// first in the buffer, so the order of every sum is fixed.
+// ---------------------------------------------------------------------------
+namespace {
+
+struct CooLayout {
+    size_t pairs, pair_counts, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, scan, sort, total;
+    int64_t C, E, cap, n_blocks, n_tiles;
+};
+
+CooLayout coo_layout(int64_t n_records, int64_t coo_capacity)
+{
+    CooLayout L;
+    L.C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
+    L.n_blocks = ceil_div64(L.C, CH);
+    const int64_t slots = L.n_blocks * CH;
+    L.E = slots * MAX_ENTRIES_PER_PAIR;
+    L.cap = L.E + (coo_capacity > 0 ? coo_capacity : 0);
+    L.n_tiles = ceil_div64(L.cap, RT);
+    size_t off = 0;
+    L.pairs = off;       off += align_up((size_t)slots * sizeof(PairRec));
+    L.pair_counts = off; off += align_up((size_t)L.n_blocks * 4);
+    L.counts = off;      off += align_up((size_t)(slots + 1) * 4);
+    for (int q = 0; q < 2; ++q) {
+        L.keys[q] = off; off += align_up((size_t)L.cap * 8);
+        L.vals[q] = off; off += align_up((size_t)L.cap * 4);
+    }
+    L.tile_heads = off;  off += align_up((size_t)(L.n_tiles + 1) * 4);
+    L.carry_key = off;   off += align_up((size_t)L.n_tiles * 8);
+    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 4);
+    const int64_t scan_n = slots > L.n_tiles ? slots : L.n_tiles;
+    L.scan = off;        off += align_up(scan_workspace_bytes(scan_n) + 256);
+    L.sort = off;        off += align_up(sort_workspace_bytes(L.cap, 8));
+    L.total = off + 1024;
+    return L;
+}
+
+int key_bits_for64(long long K)
+{
+    unsigned long long m = (unsigned long long)K * (unsigned long long)K - 1ull;
+    int bits = 0;
+    while (m) { ++bits; m >>= 1; }
+    return bits < 1 ? 1 : bits;
+}
+
+}  // namespace
+
+size_t accumulate_coo_workspace_bytes(int64_t n_records, int64_t coo_capacity)
+{
+    return coo_layout(n_records, coo_capacity).total;
+}
+
+int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+                       const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
+                       const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
+{
+    if (!b || !s || !basis || !out || !records || n_records < 0) return MCS_EINVAL;
+    if (basis->kind != 0 || basis->K != b->V) return MCS_EINVAL;
+    if (out->kind != 1 || out->K != basis->K || out->coo_capacity < 1) return MCS_EINVAL;
+    if (!out->coo_row || !out->coo_col || !out->coo_val || !out->coo_nnz) return MCS_EINVAL;
+    const long long K = basis->K;
+    const CooLayout L = coo_layout(n_records, out->coo_capacity);
+    if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
+    if (L.cap >= ((int64_t)1 << 32)) return MCS_EINVAL;
+
+    char* base = (char*)ws;
+    PairRec* pairs = (PairRec*)(base + L.pairs);
+    uint32_t* pair_counts = (uint32_t*)(base + L.pair_counts);
+    uint32_t* counts = (uint32_t*)(base + L.counts);
+    unsigned long long* keys[2] = { (unsigned long long*)(base + L.keys[0]), (unsigned long long*)(base + L.keys[1]) };
+    uint32_t* vals[2] = { (uint32_t*)(base + L.vals[0]), (uint32_t*)(base + L.vals[1]) };
+    uint32_t* tile_heads = (uint32_t*)(base + L.tile_heads);
+    unsigned long long* carry_key = (unsigned long long*)(base + L.carry_key);
+    float* carry_sum = (float*)(base + L.carry_sum);
+    void* scan_ws = base + L.scan;
+    void* sort_ws = base + L.sort;
+    const size_t scan_bytes = L.sort - L.scan, sort_bytes = L.total - L.sort;
+
+    AccArgs a;
+    a.records = records; a.faces = b->faces; a.s_tri = s->tri; a.s_bary = s->bary;
+    a.n_main = (long long)s->n_s * W; a.W = W; a.K = K;
+    const int bits = key_bits_for64(K);
+
+    unsigned long long entries_total = 0;
+    long long n_u = 0;
+    int cur = 0;
+    for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
+        const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
+        const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
+        mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        const unsigned nblk = (unsigned)ceil_div64(slots, AT);
+        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
+        int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
+        if (rc != MCS_OK) return rc;
+        uint32_t n_entries = 0;
+        MCS_CUDA_TRY(cudaMemcpyAsync(&n_entries, counts + slots, 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (n_entries == 0) continue;
+        entries_total += n_entries;
+        mcs_note_launch(), expand_entries_kernel<unsigned long long><<<nblk, AT, 0, st>>>(
+            a, pairs, pair_counts, slots, counts, keys[cur] + n_u, vals[cur] + n_u);
+        const long long n_tot = n_u + n_entries;
+        rc = sort_pairs_u64((uint64_t*)keys[cur], vals[cur], n_tot, bits, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) return rc;
+        const long long n_tiles = ceil_div64(n_tot, RT);
+        mcs_note_launch(), count_heads_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(keys[cur], n_tot, tile_heads);
+        rc = exclusive_scan_u32(tile_heads, tile_heads, n_tiles, tile_heads + n_tiles, scan_ws, scan_bytes, st);
+        if (rc != MCS_OK) return rc;
+        uint32_t n_heads = 0;
+        MCS_CUDA_TRY(cudaMemcpyAsync(&n_heads, tile_heads + n_tiles, 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if ((long long)n_heads > out->coo_capacity) {
+            const long long need = n_heads;                                 // a lower bound on the final count
+            MCS_CUDA_TRY(cudaMemcpyAsync(out->coo_nnz, &need, 8, cudaMemcpyHostToDevice, st));
+            MCS_CUDA_TRY(cudaStreamSynchronize(st));
+            return MCS_ENOMEM;
+        }
+        mcs_note_launch(), reduce_runs_compact_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
+            keys[cur], vals[cur], n_tot, tile_heads, keys[1 - cur], (float*)vals[1 - cur], carry_key, carry_sum);
+        mcs_note_launch(), carry_fixup_compact_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(
+            carry_key, carry_sum, n_tiles, tile_heads, (float*)vals[1 - cur]);
+        cur = 1 - cur;
+        n_u = n_heads;
+    }
+    if (n_u > 0)
+        mcs_note_launch(), coo_write_kernel<<<(unsigned)ceil_div64(n_u, AT), AT, 0, st>>>(
+            keys[cur], (const float*)vals[cur], n_u, K, out->coo_row, out->coo_col, out->coo_val);
+    const unsigned long long h2[2] = { entries_total, (unsigned long long)n_u };
+    MCS_CUDA_TRY(cudaMemcpyAsync(out->coo_nnz, &n_u, 8, cudaMemcpyHostToDevice, st));
+    if (stats_dev) {
+        MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_ENTRIES, &h2[0], 8, cudaMemcpyHostToDevice, st));
+        MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_UNIQUE, &h2[1], 8, cudaMemcpyHostToDevice, st));
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    MCS_CUDA_TRY(cudaStreamSynchronize(st));                               // host scalars above live on this frame
     return MCS_OK;
 }

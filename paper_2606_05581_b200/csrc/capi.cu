@@ -28,6 +28,21 @@ void mcs_prof_mark(int which, cudaStream_t st)
 
 namespace {
 
+size_t acc_ws_bytes(const mcs_bvh* b, const mcs_basis* basis, const mcs_params* p, int64_t n_records)
+{
+    return p->output_kind == 1 ? accumulate_coo_workspace_bytes(n_records, p->coo_capacity)
+                               : accumulate_workspace_bytes(b, basis, n_records);
+}
+
+int acc_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, const mcs_params* p,
+            const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
+            const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
+{
+    if (p->output_kind == 1)
+        return accumulate_coo_run(b, s, basis, p->walks_per_sample, records, n_records, ws, ws_bytes, out, stats_dev, st);
+    return accumulate_run(b, s, basis, p->walks_per_sample, records, n_records, ws, ws_bytes, out, stats_dev, st);
+}
+
 struct Layout {
     size_t records_off, walk_off, acc_off, total;
     int64_t n_records;
@@ -41,7 +56,7 @@ Layout make_layout(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     size_t off = 0;
     L.records_off = off; if (with_records) off += align_up((size_t)L.n_records * sizeof(mcs_record));
     L.walk_off = off;    off += align_up(walk_workspace_bytes(s));
-    L.acc_off = off;     if (with_acc) off += align_up(accumulate_workspace_bytes(b, basis, L.n_records));
+    L.acc_off = off;     if (with_acc) off += align_up(acc_ws_bytes(b, basis, p, L.n_records));
     L.total = off + 256;
     return L;
 }
@@ -75,7 +90,8 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
 {
     if (hs) memset(hs, 0, sizeof *hs);
     if (!b || !s || !basis || !p || !out) return MCS_EINVAL;
-    if (p->output_kind != 0 || out->kind != p->output_kind) return MCS_EINVAL;
+    if ((p->output_kind != 0 && p->output_kind != 1) || out->kind != p->output_kind) return MCS_EINVAL;
+    if (p->output_kind == 1 && (p->coo_capacity < 1 || out->coo_capacity != p->coo_capacity)) return MCS_EINVAL;
     if (p->walks_per_sample < 1 || s->n_s < 1) return MCS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Layout L = make_layout(b, s, basis, p, exterior, true, true);
@@ -88,8 +104,8 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
     int rc = walk_run(b, s, p, exterior, base + L.walk_off, align_up(walk_workspace_bytes(s)), records, nullptr,
                       false, nullptr, hs != nullptr, &stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
-    rc = accumulate_run(b, s, basis, p->walks_per_sample, records, L.n_records, base + L.acc_off,
-                        align_up(accumulate_workspace_bytes(b, basis, L.n_records)), out, stats_dev, st);
+    rc = acc_run(b, s, basis, p, records, L.n_records, base + L.acc_off,
+                 align_up(acc_ws_bytes(b, basis, p, L.n_records)), out, stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
     mcs_prof_mark(MCS_MARK_END, st);
     if (hs) {
@@ -150,7 +166,7 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
     if (stats) memset(stats, 0, sizeof *stats);
     if (!verts || !faces || !hs || !p || V < 1 || F < 1 || hs->n_s < 1) return MCS_EINVAL;
     if (!hs->tri || !hs->bary || !hs->weight) return MCS_EINVAL;
-    if ((operators & 3) == 0 || (operators & ~3)) return MCS_EINVAL;
+    if ((operators & 3) == 0 || (operators & ~3) || p->output_kind != 0) return MCS_EINVAL;
     if (((operators & 1) && !out_interior) || ((operators & 2) && !out_exterior)) return MCS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t n_s = hs->n_s;
@@ -188,7 +204,7 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
         ds.weight = (const float*)(d_in + off_w); ds.normal = nb_n ? (const float*)(d_in + off_n) : nullptr;
         ds.n_s = n_s;
         mcs_basis basis; basis.kind = 0; basis.pad_ = 0; basis.K = V;
-        mcs_matrix m; m.kind = 0; m.pad_ = 0; m.K = V; m.dense = d_out;
+        mcs_matrix m; memset(&m, 0, sizeof m); m.kind = 0; m.K = V; m.dense = d_out;
         size_t need = 0;
         for (int ext = 0; ext < 2; ++ext)
             if (operators & (1 << ext)) {
@@ -260,14 +276,15 @@ extern "C" int mcs_accumulate(const mcs_bvh* b, const mcs_samples* s, const mcs_
     if (hs) memset(hs, 0, sizeof *hs);
     if (!b || !s || !basis || !p || !records || !out) return MCS_EINVAL;
     if (n_records < s->n_s * (int64_t)p->walks_per_sample) return MCS_EINVAL;
-    const size_t need = align_up(accumulate_workspace_bytes(b, basis, n_records)) + 512;
+    if ((p->output_kind != 0 && p->output_kind != 1) || out->kind != p->output_kind) return MCS_EINVAL;
+    if (p->output_kind == 1 && (p->coo_capacity < 1 || out->coo_capacity != p->coo_capacity)) return MCS_EINVAL;
+    const size_t need = align_up(acc_ws_bytes(b, basis, p, n_records)) + 512;
     if (hs) hs->workspace_needed = (int64_t)need;
     if (!ws || ws_bytes < need) return MCS_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned long long* stats_dev = (unsigned long long*)ws;       // first 512 bytes: counters
     MCS_CUDA_TRY(cudaMemsetAsync(stats_dev, 0, ST_COUNT * 8, st));
-    int rc = accumulate_run(b, s, basis, p->walks_per_sample, (const float4*)records, n_records,
-                            (char*)ws + 512, ws_bytes - 512, out, stats_dev, st);
+    int rc = acc_run(b, s, basis, p, (const float4*)records, n_records, (char*)ws + 512, ws_bytes - 512, out, stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
     if (hs) {
         unsigned long long h[ST_COUNT];
@@ -279,10 +296,11 @@ extern "C" int mcs_accumulate(const mcs_bvh* b, const mcs_samples* s, const mcs_
     return MCS_OK;
 }
 
-extern "C" size_t mcs_accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records)
+extern "C" size_t mcs_accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, const mcs_params* p,
+                                                 int64_t n_records)
 {
-    if (!b || !basis) return 0;
-    return align_up(accumulate_workspace_bytes(b, basis, n_records)) + 512;
+    if (!b || !basis || !p) return 0;
+    return align_up(acc_ws_bytes(b, basis, p, n_records)) + 512;
 }
 
 extern "C" size_t mcs_walk_workspace_bytes(const mcs_samples* s)
