@@ -124,10 +124,21 @@ __device__ __forceinline__ float closest_point_triangle(float3 p, const TriData&
         w = fminf(wc * T.rnn, 1.0f - v);
         return plane_d2;
     }
-    best = CUDART_INF_F;
-    if (wc < 0.0f) { best = origin_to_segment(A, B, t); v = t; w = 0.0f; }                                    // edge ab
-    if (wa < 0.0f) { d = origin_to_segment(B, C, t); if (d < best) { best = d; v = 1.0f - t; w = t; } }       // edge bc
-    if (wb < 0.0f) { d = origin_to_segment(C, A, t); if (d < best) { best = d; v = 0.0f; w = 1.0f - t; } }    // edge ca
+    // first edge with a negative edge function (order ab, bc, ca), selected so that all lanes run ONE clamp
+    const int e1 = wc < 0.0f ? 0 : (wa < 0.0f ? 1 : 2);
+    {
+        const float3 P = e1 == 0 ? A : (e1 == 1 ? B : C), Q = e1 == 0 ? B : (e1 == 1 ? C : A);
+        best = origin_to_segment(P, Q, t);
+        v = e1 == 0 ? t : (e1 == 1 ? 1.0f - t : 0.0f);
+        w = e1 == 0 ? 0.0f : (e1 == 1 ? t : 1.0f - t);
+    }
+    // a second one (vertex regions): ab & bc -> bc, ab & ca -> ca, bc & ca -> ca
+    const int e2 = (e1 == 0 && wa < 0.0f) ? 1 : ((e1 < 2 && wb < 0.0f) ? 2 : -1);
+    if (e2 >= 0) {
+        const float3 P = e2 == 1 ? B : C, Q = e2 == 1 ? C : A;
+        d = origin_to_segment(P, Q, t);
+        if (d < best) { best = d; v = e2 == 1 ? 1.0f - t : 0.0f; w = e2 == 1 ? t : 1.0f - t; }
+    }
     return best;
 }
 
