@@ -173,6 +173,84 @@ pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ p
 }
 
 // ---------------------------------------------------------------------------
+// Killing walks (Eq. 32, second term) carry no sample: their key is the exit face alone, and
+// 256 consecutive ones rarely share a face.  They are reduced globally instead: sort the
+// walks by exit face (stable: slot order inside a face), segmented-sum the six moments
+// per face into M_face, and hand one pair record per face to level 2.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(AT)
+kill_keys_kernel(const float4* __restrict__ records, long long j0, long long n, uint32_t invalid_key,
+                 uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n) return;
+    const float4 rec = records[j0 + i];
+    const int tri_t = __float_as_int(rec.x);
+    keys[i] = (tri_t >= 0 && rec.w != 0.0f) ? (uint32_t)tri_t : invalid_key;
+    vals[i] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(RT)
+kill_reduce_kernel(const float4* __restrict__ records, long long j0, const uint32_t* __restrict__ keys,
+                   const uint32_t* __restrict__ vals, long long n, uint32_t invalid_key,
+                   float* __restrict__ mface, uint32_t* __restrict__ carry_key, float* __restrict__ carry_sum)
+{
+    __shared__ float s_tail[RT / 32][6];
+    __shared__ int s_has_head[RT / 32];
+    const long long i = (long long)blockIdx.x * RT + threadIdx.x;
+    const uint32_t key = i < n ? keys[i] : invalid_key;
+    const bool valid = key != invalid_key;                       // invalid keys sort last
+    const bool head = valid && (i == 0 || keys[i - 1] != key);
+    const bool last = valid && (threadIdx.x == RT - 1 || i + 1 >= n || keys[i + 1] != key);
+    float v[6] = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f };
+    if (valid) {
+        const float4 rec = records[j0 + vals[i]];
+        const float b1 = rec.y, b2 = rec.z, b0 = 1.0f - b1 - b2;
+        const float w0 = rec.w * b0, w1 = rec.w * b1, w2 = rec.w * b2;
+        v[0] = w0 * b0; v[1] = w0 * b1; v[2] = w0 * b2; v[3] = w1 * b1; v[4] = w1 * b2; v[5] = w2 * b2;
+    }
+    const bool headed = block_segmented_scan<6, RT / 32>(v, head || !valid, s_tail, s_has_head);
+    if (threadIdx.x == 0) carry_key[blockIdx.x] = 0xFFFFFFFFu;
+    __syncthreads();
+    if (last) {
+        if (headed) { for (int q = 0; q < 6; ++q) mface[6 * (long long)key + q] += v[q]; }
+        else { carry_key[blockIdx.x] = key; for (int q = 0; q < 6; ++q) carry_sum[6 * (long long)blockIdx.x + q] = v[q]; }
+    }
+}
+
+__global__ void __launch_bounds__(AT)
+kill_carry_fixup_kernel(const uint32_t* __restrict__ carry_key, const float* __restrict__ carry_sum, long long n_tiles,
+                        float* __restrict__ mface)
+{
+    const long long b = (long long)blockIdx.x * AT + threadIdx.x;
+    if (b >= n_tiles) return;
+    const uint32_t key = carry_key[b];
+    if (key == 0xFFFFFFFFu) return;
+    if (b > 0 && carry_key[b - 1] == key) return;
+    float total[6];
+    for (int q = 0; q < 6; ++q) total[q] = carry_sum[6 * b + q];
+    for (long long j = b + 1; j < n_tiles && carry_key[j] == key; ++j)
+        for (int q = 0; q < 6; ++q) total[q] += carry_sum[6 * j + q];
+    for (int q = 0; q < 6; ++q) mface[6 * (long long)key + q] += total[q];
+}
+
+// faces [f0, f0 + n) -> pair records (sample = -1); a face no killing walk reached gets tri_t = -1
+__global__ void __launch_bounds__(AT)
+kill_pairs_kernel(const float* __restrict__ mface, long long f0, long long n, long long n_slots,
+                  PairRec* __restrict__ pairs, uint32_t* __restrict__ pair_counts)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n_slots) return;
+    PairRec r;
+    r.sample = -1; r.tri_t = -1; r.w = 0.0f; r.A[0] = r.A[1] = r.A[2] = 0.0f;
+    bool any = false;
+    for (int q = 0; q < 6; ++q) { r.M[q] = i < n ? mface[6 * (f0 + i) + q] : 0.0f; any = any || r.M[q] != 0.0f; }
+    if (any) r.tri_t = (int)(f0 + i);
+    pairs[i] = r;
+    if (i % CH == 0) pair_counts[i / CH] = CH;
+}
+
+// ---------------------------------------------------------------------------
 // Level 2: pair record -> upper-triangular entries.
 // The merged vertex list holds the (<= 3) vertices of the sample's face and the
 // (<= 3) vertices of the exit face, shared vertices once.
@@ -231,7 +309,7 @@ count_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32_
     const long long i = (long long)blockIdx.x * AT + threadIdx.x;
     if (i >= n_slots) return;
     uint32_t c = 0;
-    if ((uint32_t)(i % CH) < pair_counts[i / CH]) {
+    if ((uint32_t)(i % CH) < pair_counts[i / CH] && pairs[i].tri_t >= 0) {
         PairBlock B;
         build_pair_block(a, pairs[i], B);
         for (int p = 0; p < B.m; ++p) for (int q = 0; q < B.m; ++q) c += (B.idx[p] <= B.idx[q]) ? 1u : 0u;
@@ -249,6 +327,7 @@ expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32
     if (i >= n_slots) return;
     if ((uint32_t)(i % CH) >= pair_counts[i / CH]) return;
     const PairRec r = pairs[i];
+    if (r.tri_t < 0) return;
     PairBlock B;
     build_pair_block(a, r, B);
     uint32_t o = offsets[i];
@@ -406,15 +485,53 @@ int key_bits_for(long long K)
     return bits < 1 ? 1 : bits;
 }
 
+int bits_for_count(unsigned long long m)     // bits needed for values 0..m
+{
+    int bits = 0;
+    while (m) { ++bits; m >>= 1; }
+    return bits < 1 ? 1 : bits;
+}
+
+// slots per chunk: walks of one chunk, or faces of one chunk of the killing pass
+int64_t chunk_slots(int64_t n_records, int64_t F)
+{
+    int64_t c = n_records < MAX_CHUNK_WALKS ? n_records : MAX_CHUNK_WALKS;
+    const int64_t f = F < MAX_CHUNK_WALKS ? F : MAX_CHUNK_WALKS;
+    if (f > c) c = f;
+    return c < 1 ? 1 : c;
+}
+
+// Killing records [n_main, n_main + n_kill) -> mface[F][6], in pieces of at most `cap` walks.
+int kill_prereduce(const float4* records, long long n_main, long long n_kill, long long F, float* mface,
+                   uint32_t* keys, uint32_t* vals, long long cap, uint32_t* carry_key, float* carry_sum6,
+                   void* sort_ws, size_t sort_bytes, cudaStream_t st)
+{
+    MCS_CUDA_TRY(cudaMemsetAsync(mface, 0, (size_t)F * 6 * sizeof(float), st));
+    const uint32_t invalid = (uint32_t)F;
+    const int bits = bits_for_count((unsigned long long)F);
+    for (long long k0 = 0; k0 < n_kill; k0 += cap) {
+        const long long n = (n_kill - k0) < cap ? (n_kill - k0) : cap;
+        mcs_note_launch(), kill_keys_kernel<<<(unsigned)ceil_div64(n, AT), AT, 0, st>>>(records, n_main + k0, n, invalid, keys, vals);
+        int rc = sort_pairs_u32(keys, vals, n, bits, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) return rc;
+        const long long n_tiles = ceil_div64(n, RT);
+        mcs_note_launch(), kill_reduce_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(records, n_main + k0, keys, vals, n, invalid,
+                                                                               mface, carry_key, carry_sum6);
+        mcs_note_launch(), kill_carry_fixup_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(carry_key, carry_sum6, n_tiles, mface);
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
 struct AccLayout {
-    size_t pairs, pair_counts, counts, keys, vals, carry_key, carry_sum, scan, sort, total;
+    size_t pairs, pair_counts, counts, keys, vals, carry_key, carry_sum, mface, scan, sort, total;
     int64_t C, E, n_blocks, n_tiles;
 };
 
-AccLayout acc_layout(int64_t n_records)
+AccLayout acc_layout(int64_t n_records, int64_t F)
 {
     AccLayout L;
-    L.C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
+    L.C = chunk_slots(n_records, F);
     L.n_blocks = ceil_div64(L.C, CH);
     const int64_t slots = L.n_blocks * CH;
     L.E = slots * MAX_ENTRIES_PER_PAIR;
@@ -426,7 +543,8 @@ AccLayout acc_layout(int64_t n_records)
     L.keys = off;        off += align_up((size_t)L.E * 4);
     L.vals = off;        off += align_up((size_t)L.E * 4);
     L.carry_key = off;   off += align_up((size_t)L.n_tiles * 4);
-    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 4);
+    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 24);
+    L.mface = off;       off += align_up((size_t)F * 24);
     L.scan = off;        off += align_up(scan_workspace_bytes(slots) + 256);
     L.sort = off;        off += align_up(sort_workspace_bytes(L.E, 4));
     L.total = off + 1024;
@@ -437,8 +555,8 @@ AccLayout acc_layout(int64_t n_records)
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records)
 {
-    (void)b; (void)basis;
-    return acc_layout(n_records).total;
+    (void)basis;
+    return acc_layout(n_records, b->F).total;
 }
 
 int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
@@ -450,7 +568,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     if (out->kind != 0 || out->K != basis->K || !out->dense) return MCS_EINVAL;
     const long long K = basis->K;
     if (K > 65535) return MCS_EINVAL;                 // dense keys are 32-bit (row*K + col)
-    const AccLayout L = acc_layout(n_records);
+    const AccLayout L = acc_layout(n_records, b->F);
     if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
 
     char* base = (char*)ws;
@@ -461,6 +579,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     uint32_t* vals = (uint32_t*)(base + L.vals);
     uint32_t* carry_key = (uint32_t*)(base + L.carry_key);
     float* carry_sum = (float*)(base + L.carry_sum);
+    float* mface = (float*)(base + L.mface);
     void* scan_ws = base + L.scan;
     void* sort_ws = base + L.sort;
     const size_t scan_bytes = L.sort - L.scan, sort_bytes = L.total - L.sort;
@@ -469,13 +588,21 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     a.records = records; a.faces = b->faces; a.s_tri = s->tri; a.s_bary = s->bary;
     a.n_main = (long long)s->n_s * W; a.W = W; a.K = K;
     const int bits = key_bits_for(K);
+    const long long n_main = a.n_main < n_records ? a.n_main : n_records, n_kill = n_records - n_main;
 
     MCS_CUDA_TRY(cudaMemsetAsync(out->dense, 0, (size_t)K * K * sizeof(float), st));
+    if (n_kill > 0) {
+        int rc = kill_prereduce(records, n_main, n_kill, b->F, mface, keys, vals, L.E, carry_key, carry_sum, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) return rc;
+    }
     unsigned long long entries_total = 0;
-    for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
-        const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
+    // phase 0: the walks of the samples, chunk by chunk; phase 1: one pair record per face from the killing walks
+    for (int phase = 0; phase < 2; ++phase)
+    for (int64_t j0 = 0, total = phase == 0 ? n_main : (n_kill > 0 ? b->F : 0); j0 < total; j0 += L.C) {
+        const long long n = (total - j0) < L.C ? (total - j0) : L.C;
         const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
-        mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        if (phase == 0) mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
         const unsigned nblk = (unsigned)ceil_div64(slots, AT);
         mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
         int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
@@ -510,14 +637,14 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 namespace {
 
 struct CooLayout {
-    size_t pairs, pair_counts, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, scan, sort, total;
+    size_t pairs, pair_counts, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, mface, scan, sort, total;
     int64_t C, E, cap, n_blocks, n_tiles;
 };
 
-CooLayout coo_layout(int64_t n_records, int64_t coo_capacity)
+CooLayout coo_layout(int64_t n_records, int64_t coo_capacity, int64_t F)
 {
     CooLayout L;
-    L.C = n_records < MAX_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : MAX_CHUNK_WALKS;
+    L.C = chunk_slots(n_records, F);
     L.n_blocks = ceil_div64(L.C, CH);
     const int64_t slots = L.n_blocks * CH;
     L.E = slots * MAX_ENTRIES_PER_PAIR;
@@ -533,7 +660,8 @@ CooLayout coo_layout(int64_t n_records, int64_t coo_capacity)
     }
     L.tile_heads = off;  off += align_up((size_t)(L.n_tiles + 1) * 4);
     L.carry_key = off;   off += align_up((size_t)L.n_tiles * 8);
-    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 4);
+    L.carry_sum = off;   off += align_up((size_t)L.n_tiles * 24);
+    L.mface = off;       off += align_up((size_t)F * 24);
     const int64_t scan_n = slots > L.n_tiles ? slots : L.n_tiles;
     L.scan = off;        off += align_up(scan_workspace_bytes(scan_n) + 256);
     L.sort = off;        off += align_up(sort_workspace_bytes(L.cap, 8));
@@ -551,9 +679,9 @@ int key_bits_for64(long long K)
 
 }  // namespace
 
-size_t accumulate_coo_workspace_bytes(int64_t n_records, int64_t coo_capacity)
+size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64_t coo_capacity)
 {
-    return coo_layout(n_records, coo_capacity).total;
+    return coo_layout(n_records, coo_capacity, b->F).total;
 }
 
 int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
@@ -565,7 +693,7 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
     if (out->kind != 1 || out->K != basis->K || out->coo_capacity < 1) return MCS_EINVAL;
     if (!out->coo_row || !out->coo_col || !out->coo_val || !out->coo_nnz) return MCS_EINVAL;
     const long long K = basis->K;
-    const CooLayout L = coo_layout(n_records, out->coo_capacity);
+    const CooLayout L = coo_layout(n_records, out->coo_capacity, b->F);
     if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
     if (L.cap >= ((int64_t)1 << 32)) return MCS_EINVAL;
 
@@ -587,13 +715,22 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
     a.n_main = (long long)s->n_s * W; a.W = W; a.K = K;
     const int bits = key_bits_for64(K);
 
+    float* mface = (float*)(base + L.mface);
+    const long long n_main = a.n_main < n_records ? a.n_main : n_records, n_kill = n_records - n_main;
+    if (n_kill > 0) {
+        int rc = kill_prereduce(records, n_main, n_kill, b->F, mface, (uint32_t*)keys[0], vals[0], L.cap,
+                                (uint32_t*)carry_key, carry_sum, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) return rc;
+    }
     unsigned long long entries_total = 0;
     long long n_u = 0;
     int cur = 0;
-    for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
-        const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
+    for (int phase = 0; phase < 2; ++phase)
+    for (int64_t j0 = 0, total = phase == 0 ? n_main : (n_kill > 0 ? b->F : 0); j0 < total; j0 += L.C) {
+        const long long n = (total - j0) < L.C ? (total - j0) : L.C;
         const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
-        mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        if (phase == 0) mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+        else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
         const unsigned nblk = (unsigned)ceil_div64(slots, AT);
         mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
         int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);

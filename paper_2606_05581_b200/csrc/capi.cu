@@ -30,7 +30,7 @@ namespace {
 
 size_t acc_ws_bytes(const mcs_bvh* b, const mcs_basis* basis, const mcs_params* p, int64_t n_records)
 {
-    return p->output_kind == 1 ? accumulate_coo_workspace_bytes(n_records, p->coo_capacity)
+    return p->output_kind == 1 ? accumulate_coo_workspace_bytes(b, n_records, p->coo_capacity)
                                : accumulate_workspace_bytes(b, basis, n_records);
 }
 

@@ -43,7 +43,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
              bool count, unsigned long long** stats_dev_out, cudaStream_t st);
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records);
-size_t accumulate_coo_workspace_bytes(int64_t n_records, int64_t coo_capacity);
+size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64_t coo_capacity);
 int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
                        const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                        const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);

@@ -41,7 +41,10 @@ def test_coo_equals_dense_upper_triangle_bitwise(api, exterior):
     key = coo.row.long() * bvh.V + coo.col.long()
     assert (key[1:] > key[:-1]).all()                                  # sorted, one entry per (row, col)
     up = torch.triu(dense)
-    assert torch.equal(coo.to_dense(), dense)                          # one chunk: the same sums bit for bit
+    if exterior:    # two passes (sample walks, then per-face killing moments): dense adds pass by pass, COO merges lists
+        assert (coo.to_dense() - dense).abs().max().item() <= 2e-6 * dense.abs().max().item()
+    else:
+        assert torch.equal(coo.to_dense(), dense)                      # one chunk: the same sums bit for bit
     assert coo.nnz == int((up != 0).sum().item()) or coo.nnz >= int((up != 0).sum().item())
     # too small a capacity: the library says so and the binding retries
     coo2 = api.estimate_dtn_coo(bvh, S, P, exterior, capacity=100)
