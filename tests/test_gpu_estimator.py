@@ -322,3 +322,35 @@ def test_estimator_argument_errors(api):
     with pytest.raises(api.McsError) as e:                # Kelvin origin on a vertex
         api.estimate_dtn_exterior(bvh, S, api.Params(walks_per_sample=2, kelvin_origin=tuple(float(x) for x in v[0])))
     assert e.value.code == api.MCS_EDEGENERATE
+
+
+def test_config2a_two_spheres_capacity_and_coupling_decay(api):
+    """BASELINE config 2 (spheres-only variant 2a, SURVEY.md 8(c) 'Killing / escape', 'Coupling'):
+    the killing term sums to 4 pi * capacity; two unit spheres with centres 2.5 apart have capacity
+    1.4553 (classical image series 2 a sinh(beta) sum_n (-1)^(n+1) / sinh(n beta), cosh(beta) = d / 2a);
+    the exterior coupling block decays with the separation, the interior one is exactly zero."""
+    def series(d, a=1.0, n=200):
+        beta = np.arccosh(d / (2 * a))
+        k = np.arange(1, n + 1)
+        return 2 * a * np.sinh(beta) * np.sum((-1.0) ** (k + 1) / np.sinh(k * beta))
+    assert abs(series(2.5) - 1.4553) < 2e-4
+    norms = []
+    for d in (2.5, 3.0, 4.0, 6.0):
+        level = 3
+        va, fa = icosphere(level, 1.0, (-d / 2, 0, 0))
+        vb, fb = icosphere(level, 1.0, (+d / 2, 0, 0))
+        v, f = merge_meshes([(va, fa), (vb, fb)])[:2]
+        smp = vertex_cell_samples(v, f, 2, seed=0)
+        bvh, S = _setup(api, v, f, smp)
+        nA = len(va)
+        P = api.Params(seed=3, walks_per_sample=128, eps=1e-3, include_killing=True, n_kill_walks=400_000,
+                       kelvin_origin=(-d / 2, 0, 0))
+        Se = api.estimate_dtn_exterior(bvh, S, P).cpu().numpy().astype(np.float64)
+        cap = Se.sum() / (4 * np.pi)                     # jump part annihilates constants
+        assert abs(cap / series(d) - 1) < 0.02, (d, cap, series(d))     # polyhedral spheres + 4e5 walks
+        # total weight of the walks that start on one sphere and exit on the other (a sum: robust to MC noise)
+        norms.append(-Se[:nA, nA:].sum() / np.trace(Se[:nA, :nA]))
+        if d == 2.5:
+            Si = api.estimate_dtn_interior(bvh, S, api.Params(seed=3, walks_per_sample=128, eps=1e-3)).cpu().numpy()
+            assert (Si[:nA, nA:] == 0).all()
+    assert norms[0] > norms[1] > norms[2] > norms[3] > 0, norms
