@@ -351,8 +351,8 @@ def run_ours(args):
         # walk kernel only: the tangent-ball traversals (A2) are counted separately
         nodes, tris = st.n_nodes_visited - st.n_prep_nodes, st.n_tris_tested - st.n_prep_tris
         queries = st.n_queries - st.n_prep_queries
-        flops = 36.0 * nodes + 80.0 * tris
-        nbytes = 64.0 * nodes + 48.0 * tris
+        flops = 72.0 * nodes + 80.0 * tris          # 4-wide nodes: four 18-flop box tests per visit
+        nbytes = 128.0 * nodes + 48.0 * tris
         t_alu, t_mem = flops / (fp32_tflops * 1e12), nbytes / (level_gbs * 1e9)
         roof[name] = dict(t=t, flops=flops, bytes=nbytes, t_alu=t_alu, t_mem=t_mem,
                           nodes_per_query=nodes / queries, tris_per_query=tris / queries)
@@ -373,7 +373,7 @@ def run_ours(args):
         "traffic_note": "dram bytes read+write of the two walk_kernel launches of one step (ncu --set full, profiles/walk_kernel_traffic.csv); algorithmic node+triangle bytes are served from L2",
         "peak_source": (f"{level} read bandwidth measured live by mcs_measure_l2_gbs (tree is {tree_bytes / 1e6:.2f} MB, "
                         f"{level}-resident); HBM {hbm_gbs:.0f} GB/s {hbm_src}; FP32 {fp32_tflops:.1f} TFLOP/s measured live"),
-        "algorithmic": "bytes = 64 B x nodes visited + 48 B x triangles tested; flops = 36 x nodes + 80 x triangles (DESIGN.md)",
+        "algorithmic": "bytes = 128 B x 4-wide nodes visited + 48 B x triangles tested; flops = 72 x nodes + 80 x triangles (DESIGN.md)",
         "alu_frac": t_alu / t_kernel, "mem_frac": t_mem / t_kernel,
         "kernel_ms_per_step": t_kernel * 1e3, "kernel_share_of_step": t_kernel * 1e3 / ms_per_step,
         "nodes_per_query": {k: roof[k]["nodes_per_query"] for k in roof},

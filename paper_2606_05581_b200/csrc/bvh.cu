@@ -9,6 +9,7 @@
 // connected mesh: every face is a leaf (all triangles absorb).
 #include "common.cuh"
 
+#include <limits.h>
 #include <new>
 #include <string.h>
 
@@ -249,12 +250,55 @@ depth_kernel(const int32_t* __restrict__ node_words, const int32_t* __restrict__
     if ((threadIdx.x & 31) == 0 && depth > 0) atomicMax(&sc->max_depth, depth);
 }
 
+// ---------------------------------------------------------------------------
+// 4-wide collapse for the walk kernel: binary nodes at even depth become wide nodes.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(BT)
+even_depth_kernel(const int32_t* __restrict__ node_words, int64_t n_nodes, uint32_t* __restrict__ even)
+{
+    const int64_t i = (int64_t)blockIdx.x * BT + threadIdx.x;
+    if (i >= n_nodes) return;
+    int depth = 0;
+    for (int32_t p = node_words[16 * i + 14]; p >= 0; p = node_words[16 * (int64_t)p + 14]) ++depth;
+    even[i] = (depth & 1) ? 0u : 1u;
+}
+
+__global__ void __launch_bounds__(BT)
+wide_pack_kernel(const int32_t* __restrict__ node_words, int64_t n_nodes, const uint32_t* __restrict__ even,
+                 const uint32_t* __restrict__ widx, WideNode* __restrict__ wide)
+{
+    const int64_t i = (int64_t)blockIdx.x * BT + threadIdx.x;
+    if (i >= n_nodes || !even[i]) return;
+    const float* fw = reinterpret_cast<const float*>(node_words);
+    WideNode w;
+    int n = 0;
+    for (int side = 0; side < 2; ++side) {
+        const int32_t c = node_words[16 * i + 12 + side];
+        if (c < 0) {                                           // leaf child: its box is stored in i
+            for (int q = 0; q < 6; ++q) w.f[6 * n + q] = fw[16 * i + 6 * side + q];
+            w.c[n++] = c;
+        } else {                                               // inner child at odd depth: take its two children
+            for (int s2 = 0; s2 < 2; ++s2) {
+                const int32_t g = node_words[16 * (int64_t)c + 12 + s2];
+                for (int q = 0; q < 6; ++q) w.f[6 * n + q] = fw[16 * (int64_t)c + 6 * s2 + q];
+                w.c[n++] = g < 0 ? g : (int32_t)widx[g];
+            }
+        }
+    }
+    w.pad[0] = n; w.pad[1] = (int)i; w.pad[2] = 0; w.pad[3] = 0;
+    for (; n < 4; ++n) {
+        for (int q = 0; q < 3; ++q) { w.f[6 * n + q] = CUDART_INF_F; w.f[6 * n + 3 + q] = -CUDART_INF_F; }
+        w.c[n] = INT_MIN;
+    }
+    wide[widx[i]] = w;
+}
+
 }  // namespace
 
 extern "C" void mcs_free_bvh(mcs_bvh* b)
 {
     if (!b) return;
-    cudaFree(b->verts); cudaFree(b->faces); cudaFree(b->nodes); cudaFree(b->tris);
+    cudaFree(b->verts); cudaFree(b->faces); cudaFree(b->nodes); cudaFree(b->wide); cudaFree(b->tris);
     cudaFree(b->leaf_tri); cudaFree(b->face_slot); cudaFree(b->morton);
     delete b;
 }
@@ -283,7 +327,7 @@ extern "C" int mcs_build_bvh(const float* verts, int64_t V, const int32_t* faces
 #define ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
     ALLOC(b->verts, nb_verts); ALLOC(b->faces, nb_faces); ALLOC(b->nodes, nb_nodes); ALLOC(b->tris, nb_tris);
     ALLOC(b->leaf_tri, (size_t)F * 4); ALLOC(b->face_slot, (size_t)F * 4); ALLOC(b->morton, (size_t)F * 8);
-    ALLOC(sc, sizeof(BuildScratch)); ALLOC(partials, (size_t)nblk * 8); ALLOC(vals, (size_t)F * 4);
+    ALLOC(sc, sizeof(BuildScratch) + 256); ALLOC(partials, (size_t)nblk * 8); ALLOC(vals, (size_t)F * 4);
     ALLOC(leaf_parent, (size_t)F * 4); ALLOC(arrivals, (size_t)b->n_nodes * 4); ALLOC(sort_ws, sort_bytes);
 #undef ALLOC
     BuildScratch h;
@@ -318,6 +362,25 @@ extern "C" int mcs_build_bvh(const float* verts, int64_t V, const int32_t* faces
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) { rc = MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+    {   // 4-wide collapse (binary nodes at even depth), compacted with a prefix sum
+        uint32_t* even = (uint32_t*)arrivals;                  // arrivals are done: reuse as flags
+        uint32_t* widx = vals;                                 // sorted face ids are packed: reuse (n_nodes <= F)
+        uint32_t n_wide = 0;
+        mcs_note_launch(), even_depth_kernel<<<(int)ceil_div64(b->n_nodes, BT), BT, 0, st>>>((const int32_t*)b->nodes, b->n_nodes, even);
+        uint32_t* total_dev = (uint32_t*)sc + 16;              // scratch word behind BuildScratch
+        rc = exclusive_scan_u32(even, widx, b->n_nodes, total_dev, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) goto done;
+        e = cudaMemcpyAsync(&n_wide, total_dev, 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&b->wide, (size_t)(n_wide ? n_wide : 1) * sizeof(WideNode));
+        if (e != cudaSuccess) { rc = (e == cudaErrorMemoryAllocation) ? MCS_ENOMEM : MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+        b->n_wide = n_wide;
+        b->device_bytes += (size_t)n_wide * sizeof(WideNode);
+        mcs_note_launch(), wide_pack_kernel<<<(int)ceil_div64(b->n_nodes, BT), BT, 0, st>>>((const int32_t*)b->nodes, b->n_nodes, even, widx, b->wide);
+        e = cudaStreamSynchronize(st);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) { rc = MCS_ECUDA; mcs_set_last_cuda_error((int)e); goto done; }
+    }
     b->max_depth = h.max_depth;
     b->n_degenerate = h.n_degenerate;
     b->area = h.area;

@@ -51,11 +51,25 @@ struct __align__(16) PackedTri {
     float4 t0, t1, t2, t3;
 };
 
+// One 4-wide node of the walk kernel = 128 bytes = 4 x 32-byte loads: every second level of the
+// binary tree collapsed (a binary node at even depth with its grandchildren, or a leaf child where
+// the tree ends earlier).
+//   f[6k .. 6k+5] = box of child k (lo.xyz, hi.xyz), k = 0..3;  an empty slot has lo = +inf
+//   c[k]          = child k: >= 0 wide node index, < 0 leaf ~c = sorted triangle slot
+//   pad[4]        = (number of children, binary node index, 0, 0)
+struct __align__(32) WideNode {
+    float f[24];
+    int   c[4];
+    int   pad[4];
+};
+
 struct mcs_bvh {
     int64_t V, F, n_nodes;
     float*     verts;      // [V][3] copy of the input
     int32_t*   faces;      // [F][3] copy of the input
     BvhNode*   nodes;      // [max(F-1,1)]
+    WideNode*  wide;       // [n_wide] 4-wide collapse of `nodes` (walk kernel); root = 0
+    int64_t    n_wide;
     PackedTri* tris;       // [F] Morton order
     int32_t*   leaf_tri;   // [F] original face index of sorted leaf k
     int32_t*   face_slot;  // [F] sorted slot of original face f (inverse of leaf_tri)

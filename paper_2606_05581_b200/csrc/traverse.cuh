@@ -13,7 +13,7 @@
 #pragma once
 #include "common.cuh"
 
-#define MCS_STACK 96      // >= 63 Morton bits + log2(F) index-tie levels
+#define MCS_STACK 160     // binary tree: >= 63 Morton bits + log2(F) index-tie levels; 4-wide walk: 3 pushes per two levels
 
 // 256-bit read-only global load (sm_100: LDG.E.256).  A divergent warp pays one L1
 // wavefront per lane and per load instruction whatever its width, and that wavefront rate

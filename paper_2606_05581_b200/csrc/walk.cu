@@ -321,6 +321,9 @@ __device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& 
 constexpr int WALK_MIN_BLOCKS = 8;                  // 64 registers per thread; 10 (48 registers, spills) measured 9 % slower
 constexpr int WSTACK = 16;                       // shared-memory stack entries per lane
 constexpr int CUR_NONE = INT_MIN;
+#ifndef TRANS_MIN
+#define TRANS_MIN 16
+#endif
 
 struct LaneStack {
     int*   s_ref;      // shared: [WSTACK][WT], this lane's column
@@ -377,7 +380,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
     float3 xq = f3(0.f, 0.f, 0.f);
     float rho = 0.f, far_radius = -1.0f;         // far_radius >= 0: jump radius known without a query (exterior far field)
     ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.f;
-    float lim = CUDART_INF_F;
+    float lim = 3.0e38f;
     int cur = CUR_NONE, sp = 0;
     // statistics
     unsigned n_nodes = 0, n_tris = 0, q_nodes = 0;
@@ -403,24 +406,32 @@ walk_kernel(WalkGeom g, WalkArgs a)
             // vote: the kind most lanes wait for (ties: NODE, then TRI)
             int best = __popc(m_node);
             if (__popc(m_tri) > best) { which = KIND_TRI; best = __popc(m_tri); }
-            if (__popc(m_trans) > best) { which = KIND_TRANS; }
+            // TRANS is the long pass (Philox, sincos, record, refill): run it when enough lanes wait for it
+            // or when little else is left to do
+            if (__popc(m_trans) >= TRANS_MIN || (best < 8 && __popc(m_trans) > 0)) { which = KIND_TRANS; }
         }
 
         if (which == KIND_NODE) {
             if (kind == KIND_NODE) {
-                const Vec8 n0 = ldg256(g.nodes + cur), n1 = ldg256(reinterpret_cast<const char*>(g.nodes + cur) + 32);
-                const float4 w0 = n0.lo, w1 = n0.hi, w2 = n1.lo;
-                const int2 ch = make_int2(__float_as_int(n1.hi.x), __float_as_int(n1.hi.y));
+                // 4-wide node: four box tests, the children that survive sorted by distance; the nearest
+                // is visited next, the others go on the stack farthest first
+                const char* wn = reinterpret_cast<const char*>(g.wide + cur);
+                const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32), q2 = ldg256(wn + 64), q3 = ldg256(wn + 96);
                 if (COUNT) { ++n_nodes; ++q_nodes; }
-                const float d0 = box_dist2(xq, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y);
-                const float d1 = box_dist2(xq, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
-                const bool go0 = d0 <= lim, go1 = d1 <= lim;
-                const bool swap = d1 < d0;
-                const int nearc = swap ? ch.y : ch.x, farc = swap ? ch.x : ch.y;
-                if (go0 && go1) { stack_push(stk, sp, farc, swap ? d0 : d1); cur = nearc; }
-                else if (go0) cur = ch.x;
-                else if (go1) cur = ch.y;
-                else cur = CUR_NONE;
+                float d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
+                float d1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
+                float d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
+                float d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
+                int c0 = __float_as_int(q3.lo.x), c1 = __float_as_int(q3.lo.y), c2 = __float_as_int(q3.lo.z), c3 = __float_as_int(q3.lo.w);
+                // sorting network on (distance, child): (0,1)(2,3)(0,2)(1,3)(1,2); empty slots have d = +inf
+#define MCS_CSWAP(da, ca, db, cb) { const bool s_ = db < da; const float td_ = s_ ? da : db; const int tc_ = s_ ? ca : cb; \
+                                    da = s_ ? db : da; ca = s_ ? cb : ca; db = td_; cb = tc_; }
+                MCS_CSWAP(d0, c0, d1, c1) MCS_CSWAP(d2, c2, d3, c3) MCS_CSWAP(d0, c0, d2, c2) MCS_CSWAP(d1, c1, d3, c3) MCS_CSWAP(d1, c1, d2, c2)
+#undef MCS_CSWAP
+                if (d3 <= lim) stack_push(stk, sp, c3, d3);
+                if (d2 <= lim) stack_push(stk, sp, c2, d2);
+                if (d1 <= lim) stack_push(stk, sp, c1, d1);
+                cur = d0 <= lim ? c0 : CUR_NONE;
             }
         } else if (which == KIND_TRI) {
             if (kind == KIND_TRI) {
@@ -562,7 +573,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                     }
                 }
                 h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
-                lim = CUDART_INF_F;
+                lim = 3.0e38f;                               // finite: the +inf of an empty node slot never passes
                 sp = 0; cur = CUR_NONE;
                 if (need_query) {
                     if (prev >= 0) { stack_push(stk, sp, 0, 0.0f); cur = ~prev; }   // last closest face first: a tight bound
@@ -653,7 +664,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     if (stats_dev_out) *stats_dev_out = stats;
 
     WalkGeom g;
-    g.nodes = b->nodes; g.tris = b->tris; g.verts = b->verts; g.faces = b->faces;
+    g.nodes = b->nodes; g.wide = b->wide; g.tris = b->tris; g.verts = b->verts; g.faces = b->faces;
 
     MCS_CUDA_TRY(cudaMemsetAsync(stats, 0, ST_COUNT * 8 + 64, st));
     const float3 lo = f3(b->aabb_lo[0], b->aabb_lo[1], b->aabb_lo[2]);

@@ -13,6 +13,7 @@ enum {
 
 struct WalkGeom {
     const BvhNode*   nodes;
+    const WideNode*  wide;         // 4-wide collapse of `nodes` (walk kernel)
     const PackedTri* tris;
     const float*     verts;
     const int32_t*   faces;
