@@ -321,8 +321,14 @@ __device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& 
 constexpr int WALK_MIN_BLOCKS = 8;                  // 64 registers per thread; 10 (48 registers, spills) measured 9 % slower
 constexpr int WSTACK = 16;                       // shared-memory stack entries per lane
 constexpr int CUR_NONE = INT_MIN;
-#ifndef TRANS_MIN
-#define TRANS_MIN 16
+#ifndef VOTE_NODE
+#define VOTE_NODE 8
+#endif
+#ifndef VOTE_TRI
+#define VOTE_TRI 8
+#endif
+#ifndef VOTE_TRANS
+#define VOTE_TRANS 20
 #endif
 
 struct LaneStack {
@@ -397,18 +403,18 @@ walk_kernel(WalkGeom g, WalkArgs a)
         }
         const int kind = busy ? (cur == CUR_NONE ? KIND_TRANS : (cur >= 0 ? KIND_NODE : KIND_TRI))
                               : (exhausted ? KIND_IDLE : KIND_TRANS);
-        // fast path: at least half of the warp waits for a node visit
+        // Which kind runs this pass: NODE while at least VOTE_NODE lanes want it (one ballot), else TRI when
+        // at least VOTE_TRI lanes wait, else TRANS (the long pass: Philox, sincos, record, refill) when at least
+        // VOTE_TRANS lanes wait; otherwise the kind most lanes wait for.  Draining one kind lets the others fill.
         const unsigned m_node = __ballot_sync(FULL, kind == KIND_NODE);
         int which = KIND_NODE;
-        if (__popc(m_node) < 16) {
+        if (__popc(m_node) < VOTE_NODE) {
             const unsigned m_tri = __ballot_sync(FULL, kind == KIND_TRI), m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
             if ((m_node | m_tri | m_trans) == 0) break;
-            // vote: the kind most lanes wait for (ties: NODE, then TRI)
-            int best = __popc(m_node);
-            if (__popc(m_tri) > best) { which = KIND_TRI; best = __popc(m_tri); }
-            // TRANS is the long pass (Philox, sincos, record, refill): run it when enough lanes wait for it
-            // or when little else is left to do
-            if (__popc(m_trans) >= TRANS_MIN || (best < 8 && __popc(m_trans) > 0)) { which = KIND_TRANS; }
+            const int nn = __popc(m_node), nt = __popc(m_tri), nx = __popc(m_trans);
+            if (nt >= VOTE_TRI) which = KIND_TRI;
+            else if (nx >= VOTE_TRANS) which = KIND_TRANS;
+            else which = (nx > nn && nx > nt) ? KIND_TRANS : (nt > nn ? KIND_TRI : KIND_NODE);
         }
 
         if (which == KIND_NODE) {
