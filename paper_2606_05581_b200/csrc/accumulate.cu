@@ -9,10 +9,10 @@
 //
 //  level 1 (on chip)  A block takes 256 consecutive record slots, sorts them in shared
 //      memory by (sample, exit face) and reduces every run to ONE pair record: the
-//      moments  w = sum wgt,  A_k = sum wgt b_k(t),  M_kl = sum wgt b_k(t) b_l(t)
-//      of the exit-point barycentrics.  All walks of a pair share b(s) and the six
-//      vertices involved, so  sum wgt d d^T  over the pair is a function of
-//      (w, A, M) alone.  With W walks per sample this shrinks the stream that has to
+//      moments  w = sum wgt,  A_k = sum wgt eta_k,  M_kl = sum wgt eta_k eta_l  of the
+//      exit-point barycentrics about a reference r (the pair's first exit point),
+//      eta = b(t) - r.  All walks of a pair share b(s) and the six vertices involved, so
+//      sum wgt d d^T  over the pair, d = (b(s) - r) - eta, is a function of (w, A, M, r) alone.  With W walks per sample this shrinks the stream that has to
 //      be sorted globally by the number of walks per (sample, exit face) pair.
 //  level 2 (global)   Pair records are expanded to upper-triangular (row*K+col, value)
 //      entries in slot order, stable-radix-sorted by key, every run of equal keys is
@@ -33,12 +33,17 @@ constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << 22;
 constexpr int MAX_ENTRIES_PER_PAIR = 21;              // upper triangle of a 6 x 6 block
 constexpr int RT = 1024;                              // entries per tile of the run reduction
 
+// Moments of a pair are taken about a reference exit point (the barycentrics r of the pair's first walk):
+// eta = b(t) - r.  Most of the weight sits in walks that land close to their sample, where d = b(s) - b(t)
+// is small; sums of raw b b^T would lose three digits to cancellation there, sums of eta eta^T do not.
 struct __align__(16) PairRec {
     int   sample;            // -1: killing walk (no b(s) part)
     int   tri_t;
     float w;                 // sum wgt
-    float A[3];              // sum wgt b_k
-    float M[6];              // sum wgt b_k b_l : 00 01 02 11 12 22
+    float A[3];              // sum wgt eta_k
+    float M[6];              // sum wgt eta_k eta_l : 00 01 02 11 12 22
+    float ref1, ref2;        // reference barycentrics r_1, r_2 (r_0 = 1 - r_1 - r_2); killing: 0, 0, eta = b
+    float pad_[2];
 };
 
 struct AccArgs {
@@ -108,6 +113,7 @@ pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ p
     __shared__ unsigned long long s_key[CH];
     __shared__ float4 s_rec[CH];
     __shared__ float s_tail[CH / 32][10];
+    __shared__ float s_tail2[CH / 32][2];
     __shared__ int s_has_head[CH / 32];
     __shared__ int s_warp_runs[CH / 32];
     const int tid = threadIdx.x;
@@ -143,13 +149,18 @@ pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ p
     const unsigned long long gid = key >> 8;
     const bool head = valid && (tid == 0 || (s_key[tid - 1] >> 8) != gid);
     const bool tail = valid && (tid == CH - 1 || (s_key[tid + 1] >> 8) != gid);     // invalid keys sort last
-    float v[10];
+    float v[10], ref[2];
     {
         const float4 rec = s_rec[valid ? (int)(key & 0xFF) : 0];
         const float wgt = valid ? rec.w : 0.0f;
-        const float b1 = rec.y, b2 = rec.z, b0 = 1.0f - b1 - b2;
-        v[0] = wgt; v[1] = wgt * b0; v[2] = wgt * b1; v[3] = wgt * b2;
-        v[4] = v[1] * b0; v[5] = v[1] * b1; v[6] = v[1] * b2; v[7] = v[2] * b1; v[8] = v[2] * b2; v[9] = v[3] * b2;
+        const bool killing = (gid >> 32) == 0x1FFull;
+        // reference of the run = barycentrics of its first walk, broadcast by a segmented sum of (r at the head, 0 elsewhere)
+        ref[0] = (head && !killing) ? rec.y : 0.0f; ref[1] = (head && !killing) ? rec.z : 0.0f;
+        block_segmented_scan<2, CH / 32>(ref, head || !valid, s_tail2, s_has_head);
+        const float e1 = rec.y - ref[0], e2 = rec.z - ref[1];
+        const float e0 = killing ? 1.0f - rec.y - rec.z : -(e1 + e2);
+        v[0] = wgt; v[1] = wgt * e0; v[2] = wgt * e1; v[3] = wgt * e2;
+        v[4] = v[1] * e0; v[5] = v[1] * e1; v[6] = v[1] * e2; v[7] = v[2] * e1; v[8] = v[2] * e2; v[9] = v[3] * e2;
     }
     block_segmented_scan<10, CH / 32>(v, head || !valid, s_tail, s_has_head);
     // rank of my run among the block's runs (runs are counted at their tails)
@@ -167,6 +178,7 @@ pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ p
         r.tri_t = (int)(gid & 0xFFFFFFFFu);
         r.w = v[0]; r.A[0] = v[1]; r.A[1] = v[2]; r.A[2] = v[3];
         for (int q = 0; q < 6; ++q) r.M[q] = v[4 + q];
+        r.ref1 = ref[0]; r.ref2 = ref[1]; r.pad_[0] = r.pad_[1] = 0.0f;
         pairs[(long long)blockIdx.x * CH + rank] = r;
     }
     if (tid == 0) pair_counts[blockIdx.x] = (uint32_t)total;
@@ -243,6 +255,7 @@ kill_pairs_kernel(const float* __restrict__ mface, long long f0, long long n, lo
     if (i >= n_slots) return;
     PairRec r;
     r.sample = -1; r.tri_t = -1; r.w = 0.0f; r.A[0] = r.A[1] = r.A[2] = 0.0f;
+    r.ref1 = r.ref2 = 0.0f; r.pad_[0] = r.pad_[1] = 0.0f;
     bool any = false;
     for (int q = 0; q < 6; ++q) { r.M[q] = i < n ? mface[6 * (f0 + i) + q] : 0.0f; any = any || r.M[q] != 0.0f; }
     if (any) r.tri_t = (int)(f0 + i);
@@ -257,8 +270,8 @@ kill_pairs_kernel(const float* __restrict__ mface, long long f0, long long n, lo
 // ---------------------------------------------------------------------------
 struct PairBlock {
     int   idx[6];
-    float ds[6];          // b_v(s)
-    float At[6];          // sum wgt b_v(t)
+    float ds[6];          // D_v = b_v(s) - r_v(t): the pair's d at the reference exit point
+    float At[6];          // sum wgt eta_v(t)
     int   tmask[6];       // corners of the exit face that are this vertex (bit k)
     int   m;
 };
@@ -278,8 +291,11 @@ __device__ __forceinline__ void build_pair_block(const AccArgs& a, const PairRec
         for (int k = 0; k < 3; ++k) B.ds[pair_block_slot(B, a.faces[3 * fs + k])] += a.s_bary[3 * (long long)r.sample + k];
     }
     const long long ft = r.tri_t;
+    const bool killing = r.sample < 0;
+    const float rb[3] = { killing ? 0.0f : 1.0f - r.ref1 - r.ref2, r.ref1, r.ref2 };
     for (int k = 0; k < 3; ++k) {
         const int q = pair_block_slot(B, a.faces[3 * ft + k]);
+        B.ds[q] -= rb[k];
         B.At[q] += r.A[k];
         B.tmask[q] |= 1 << k;
     }
@@ -334,7 +350,7 @@ expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32
     for (int p = 0; p < B.m; ++p)
         for (int q = 0; q < B.m; ++q)
             if (B.idx[p] <= B.idx[q]) {
-                // sum over the pair's walks of wgt * d_p d_q,  d = b(s) - b(t)
+                // sum over the pair's walks of wgt * d_p d_q,  d = b(s) - b(t) = D - eta
                 float e = r.w * B.ds[p] * B.ds[q] - B.ds[p] * B.At[q] - B.At[p] * B.ds[q];
                 if (B.tmask[p] && B.tmask[q]) e += moment_block(r, B.tmask[p], B.tmask[q]);
                 keys[o] = (KeyT)((long long)B.idx[p] * a.K + B.idx[q]);

@@ -354,3 +354,56 @@ def test_config2a_two_spheres_capacity_and_coupling_decay(api):
             Si = api.estimate_dtn_interior(bvh, S, api.Params(seed=3, walks_per_sample=128, eps=1e-3)).cpu().numpy()
             assert (Si[:nA, nA:] == 0).all()
     assert norms[0] > norms[1] > norms[2] > norms[3] > 0, norms
+
+
+def test_w1_many_samples_per_chunk_and_odd_sizes(api):
+    """Alg. 2 as printed: one walk per sample (W = 1), so a level-1 block of the accumulation holds 256
+    different samples; odd counts exercise the ragged tails (samples, walks, killing walks)."""
+    v, f = icosphere(2)
+    smp = uniform_samples(v, f, 3001, seed=13)
+    gp, op = _params(api, seed=21, walks_per_sample=1, eps=1e-3, include_killing=True, n_kill_walks=777,
+                     kelvin_origin=(0.05, 0.1, 0.0))
+    bvh, S = _setup(api, v, f, smp)
+    orc = Oracle(mesh_geom(v, f))
+    for ext in (False, True):
+        fn = api.estimate_dtn_exterior if ext else api.estimate_dtn_interior
+        Sg = fn(bvh, S, gp)
+        assert torch.equal(Sg, fn(bvh, S, gp)) and torch.equal(Sg, Sg.T)
+        out = orc.estimate_dtn(op, ext, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+        Sg = Sg.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(Sg - out["S"]) <= np.linalg.norm(np.sqrt(out["var"]))
+        # the library's accumulation of its own records equals the oracle's accumulation of them
+        rec, steps = api.run_walks(bvh, S, gp, ext)
+        r = rec.cpu().numpy()
+        from oracle import RECORD_DTYPE
+        orec = np.zeros(len(r), RECORD_DTYPE)
+        tri_t = r[:, 0].copy().view(np.int32)
+        n_main = len(smp["tri"])
+        orec["sample"] = np.where(np.arange(len(r)) < n_main, np.arange(len(r)), -1)
+        orec["tri_t"] = tri_t
+        orec["bary_t"][:, 1] = r[:, 1]; orec["bary_t"][:, 2] = r[:, 2]
+        orec["bary_t"][:, 0] = 1.0 - r[:, 1].astype(np.float32) - r[:, 2].astype(np.float32)
+        orec["weight"] = np.where(tri_t >= 0, r[:, 3], 0.0)
+        orec["steps"] = np.where(tri_t >= 0, 0, -1)
+        So = orc.accumulate_hat(orec, smp["tri"], smp["bary"])
+        assert np.abs(Sg - So).max() <= 3e-5 * np.abs(So).max()
+
+
+def test_tiny_meshes_and_normal_override(api):
+    """A tetrahedron (4 faces) runs the whole path; an explicit normal array equal to the face normals gives
+    the same matrix bit for bit."""
+    v = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1]], np.float32)
+    f = np.array([[0, 2, 1], [0, 1, 3], [0, 3, 2], [1, 2, 3]], np.int32)          # outward winding
+    smp = uniform_samples(v, f, 64, seed=2)
+    bvh, S = _setup(api, v, f, smp)
+    P = api.Params(seed=5, walks_per_sample=32, eps=1e-3)
+    A, st = api.estimate_dtn_interior(bvh, S, P, want_stats=True)
+    assert st.n_truncated == 0 and torch.equal(A, A.T)
+    Sg = A.cpu().numpy().astype(np.float64)
+    assert np.abs(Sg.sum(1)).max() < 5e-5 * np.abs(Sg).max() and np.linalg.eigvalsh(Sg).min() > -1e-5 * np.abs(Sg).max()
+    vv = v[f[smp["tri"]]].astype(np.float64)
+    nrm = np.cross(vv[:, 1] - vv[:, 0], vv[:, 2] - vv[:, 0]).astype(np.float32)
+    nrm /= np.linalg.norm(nrm, axis=1, keepdims=True)
+    S2 = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"], normal=nrm)
+    B = api.estimate_dtn_interior(bvh, S2, P)
+    assert (A - B).abs().max().item() <= 1e-5 * A.abs().max().item()
