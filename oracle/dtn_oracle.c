@@ -406,6 +406,9 @@ typedef struct {
     double origin[3];               /* Kelvin origin [R12]               */
     double Rmax_norm;               /* orc_max_vertex_norm(), exterior only             */
     double escape_radius;           /* [R10b] interior: AABB diagonal; 0 = no escape test */
+    int32_t estimator;              /* 0: Alg. 2 (tangent-ball jump kernel); 1: Alg. 1 (naive finite difference), interior only */
+    int32_t pad_;
+    double inset;                   /* Alg. 1: inset distance of the evaluation point x = s - inset n_s */
 } orc_params;
 
 typedef struct {                    /* one boundary sample            */
@@ -651,8 +654,16 @@ static void run_one_walk(const orc_geom *g, const orc_params *P, int exterior, c
     const orc_ball B = *Bp;
     memset(R, 0, sizeof *R);
     R->sample = i; R->tri_t = -1;
-    if (!(B.r > 0.0)) { R->steps = -2; return; }           /* discarded sample */
-    double factor = sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, R->z);
+    double factor;
+    if (P->estimator == 1 && !exterior) {
+        /* Alg. 1 (Eq. 13-16; [G2]): the walk starts at the inset point x = s - eps n_s
+         * and the update is (|dOmega| / (N eps)) b_s (b_s - b_t)^T: no tangent ball, no sampling weight. */
+        for (int k = 0; k < 3; ++k) R->z[k] = S->s[k] - P->inset * S->n[k];
+        factor = 1.0 / P->inset;
+    } else {
+        if (!(B.r > 0.0)) { R->steps = -2; return; }       /* discarded sample */
+        factor = sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, R->z);
+    }
     orc_hit h;
     int steps = exterior ? walk_on_spheres_kelvin(g, P, (uint32_t)i, (uint32_t)w, R->z, &h)
                          : walk_on_spheres(g, P, (uint32_t)i, (uint32_t)w, R->z, &h);
@@ -687,8 +698,9 @@ int64_t orc_run_walks(const orc_geom *g, const orc_params *P, int exterior,
         orc_sample S;
         orc_ball B;
         fill_sample(g, tri, bary, weight, normal, pos, i, &S);
-        if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
-        else          orc_tangent_ball_interior(g, P, &S, &B);
+        if (P->estimator == 1 && !exterior) { memset(&B, 0, sizeof B); B.sstar_norm = 1.0; }   /* Alg. 1 has no ball */
+        else if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
+        else               orc_tangent_ball_interior(g, P, &S, &B);
         if (balls_out) { balls_out[5*i] = B.r; balls_out[5*i+1] = B.c[0]; balls_out[5*i+2] = B.c[1]; balls_out[5*i+3] = B.c[2]; balls_out[5*i+4] = B.sstar_norm; }
         for (int w = 0; w < W; ++w)
             run_one_walk(g, P, exterior, &S, &B, i, w, rec + i * W + w);
@@ -733,8 +745,9 @@ int64_t orc_run_walks_subset(const orc_geom *g, const orc_params *P, int exterio
         orc_sample S;
         orc_ball B;
         fill_sample(g, tri, bary, weight, normal, NULL, i, &S);
-        if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
-        else          orc_tangent_ball_interior(g, P, &S, &B);
+        if (P->estimator == 1 && !exterior) { memset(&B, 0, sizeof B); B.sstar_norm = 1.0; }   /* Alg. 1 has no ball */
+        else if (exterior) orc_tangent_ball_exterior(g, P, &S, &B);
+        else               orc_tangent_ball_interior(g, P, &S, &B);
         for (int w = 0; w < n_w; ++w)
             run_one_walk(g, P, exterior, &S, &B, i, w, rec + k * n_w + w);
     }
@@ -795,9 +808,9 @@ static int build_d(const orc_geom *g, const orc_record *R, const int32_t *tri, c
     return n;
 }
 
-void orc_accumulate_hat(const orc_geom *g, const orc_record *rec, int64_t n_rec,
-                        const int32_t *tri, const float *bary, int64_t K,
-                        double *S /* [K][K] zeroed by caller */, double *S2 /* [K][K] or NULL */)
+static void accumulate_hat_impl(const orc_geom *g, const orc_record *rec, int64_t n_rec,
+                                const int32_t *tri, const float *bary, int64_t K,
+                                double *S, double *S2, int naive)
 {
     orc_entry *buf = NULL;
     int64_t cap = 0;
@@ -813,8 +826,16 @@ void orc_accumulate_hat(const orc_geom *g, const orc_record *rec, int64_t n_rec,
             if (R->steps < 0 || R->weight == 0.0) continue;
             int64_t idx[6]; double val[6];
             int n = build_d(g, R, tri, bary, idx, val);
+            double bsv[6] = { 0, 0, 0, 0, 0, 0 };              /* b_s on the merged vertex list (Alg. 1) */
+            if (naive && R->sample >= 0) {
+                const int32_t *fs = g->faces + 3 * (int64_t)tri[R->sample];
+                for (int m = 0; m < n; ++m) for (int k = 0; k < 3; ++k)
+                    if (idx[m] == fs[k]) bsv[m] += (double)bary[3 * R->sample + k];
+            }
             for (int p = 0; p < n; ++p) for (int q = 0; q < n; ++q) {
-                double x = R->weight * val[p] * val[q];
+                /* Alg. 2: w d d^T.  Alg. 1: w b_s d^T, symmetrised as in its last line: (S + S^T)/2 */
+                double x = naive ? R->weight * 0.5 * (bsv[p] * val[q] + bsv[q] * val[p])
+                                 : R->weight * val[p] * val[q];
                 S[idx[p] * K + idx[q]] += x;
                 if (S2) { buf[n_e].key = idx[p] * K + idx[q]; buf[n_e].val = x; ++n_e; }
             }
@@ -833,6 +854,20 @@ void orc_accumulate_hat(const orc_geom *g, const orc_record *rec, int64_t n_rec,
         g0 = g1;
     }
     free(buf);
+}
+
+void orc_accumulate_hat(const orc_geom *g, const orc_record *rec, int64_t n_rec,
+                        const int32_t *tri, const float *bary, int64_t K,
+                        double *S /* [K][K] zeroed by caller */, double *S2 /* [K][K] or NULL */)
+{
+    accumulate_hat_impl(g, rec, n_rec, tri, bary, K, S, S2, 0);
+}
+
+/* Alg. 1's update  S += w b_s (b_s - b_t)^T  followed by its symmetrisation. */
+void orc_accumulate_hat_naive(const orc_geom *g, const orc_record *rec, int64_t n_rec,
+                              const int32_t *tri, const float *bary, int64_t K, double *S, double *S2)
+{
+    accumulate_hat_impl(g, rec, n_rec, tri, bary, K, S, S2, 1);
 }
 
 int orc_num_threads(void)

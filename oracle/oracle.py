@@ -50,7 +50,7 @@ class _Params(C.Structure):
                 ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32),
                 ("n_kill_walks", C.c_int64), ("origin", C.c_double * 3), ("Rmax_norm", C.c_double),
-                ("escape_radius", C.c_double)]
+                ("escape_radius", C.c_double), ("estimator", C.c_int32), ("pad_", C.c_int32), ("inset", C.c_double)]
 
 
 RECORD_DTYPE = np.dtype([("sample", np.int64), ("tri_t", np.int64), ("bary_t", np.float64, 3),
@@ -72,6 +72,8 @@ class OracleParams:
     include_killing: bool = False
     n_kill_walks: int = 0
     origin: tuple = (0.0, 0.0, 0.0)
+    estimator: int = 0                   # 0: Alg. 2; 1: Alg. 1 (naive finite difference, interior only)
+    inset: float = 0.0                   # Alg. 1: x = s - inset * n_s
     rmax: float | None = None            # overrides the AABB rule (analytic sphere pins)
     Rmax_norm: float | None = None
 
@@ -183,7 +185,7 @@ class Oracle:
                      eps=p.eps, cap_half_angle_deg=p.cap_half_angle_deg,
                      bisection_iters=p.bisection_iters, importance_sample=int(p.importance_sample),
                      antithetic=int(p.antithetic), include_killing=int(p.include_killing),
-                     n_kill_walks=int(p.n_kill_walks))
+                     n_kill_walks=int(p.n_kill_walks), estimator=int(p.estimator), inset=float(p.inset))
         cp.origin[:] = [float(x) for x in p.origin]
         if p.rmax is not None:
             cp.rmax = float(p.rmax)
@@ -240,14 +242,15 @@ class Oracle:
         assert n == len(rec)
         return rec
 
-    def accumulate_hat(self, rec, tri, bary, want_var=False):
+    def accumulate_hat(self, rec, tri, bary, want_var=False, naive=False):
         K = self.geom.c.V
         tri = np.ascontiguousarray(tri, np.int32)
         bary = np.ascontiguousarray(bary, np.float32)
         rec = np.ascontiguousarray(rec)
         S = np.zeros((K, K))
         S2 = np.zeros((K, K)) if want_var else None
-        self.lib.orc_accumulate_hat(C.byref(self.geom.c), rec.ctypes.data_as(C.c_void_p),
+        fn = self.lib.orc_accumulate_hat_naive if naive else self.lib.orc_accumulate_hat
+        fn(C.byref(self.geom.c), rec.ctypes.data_as(C.c_void_p),
                                     C.c_int64(len(rec)), tri.ctypes.data_as(C.c_void_p),
                                     bary.ctypes.data_as(C.c_void_p), C.c_int64(K),
                                     S.ctypes.data_as(C.c_void_p),
@@ -258,7 +261,7 @@ class Oracle:
                      want_var=False):
         """Dense hat-basis DtN matrix (Alg. 2 / Eq. 32) plus records and balls."""
         rec, balls = self.run_walks(params, exterior, tri, bary, weight, normal)
-        out = self.accumulate_hat(rec, tri, bary, want_var)
+        out = self.accumulate_hat(rec, tri, bary, want_var, naive=(params.estimator == 1 and not exterior))
         S, var = out if want_var else (out, None)
         return dict(S=S, var=var, records=rec, balls=balls)
 

@@ -12,8 +12,9 @@
 //      moments  w = sum wgt,  A_k = sum wgt eta_k,  M_kl = sum wgt eta_k eta_l  of the
 //      exit-point barycentrics about a reference r (the pair's first exit point),
 //      eta = b(t) - r.  All walks of a pair share b(s) and the six vertices involved, so
-//      sum wgt d d^T  over the pair, d = (b(s) - r) - eta, is a function of (w, A, M, r) alone.  With W walks per sample this shrinks the stream that has to
-//      be sorted globally by the number of walks per (sample, exit face) pair.
+//      sum wgt d d^T  over the pair, d = (b(s) - r) - eta, is a function of (w, A, M, r) alone.
+//      With W walks per sample this shrinks the stream that has to be sorted globally by the
+//      number of walks per (sample, exit face) pair.
 //  level 2 (global)   Pair records are expanded to upper-triangular (row*K+col, value)
 //      entries in slot order, stable-radix-sorted by key, every run of equal keys is
 //      summed by a segmented scan of fixed shape, and the run sums are added to the

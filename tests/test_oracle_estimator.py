@@ -396,3 +396,59 @@ def test_escape_rule_r10b():
     assert (st == -1).sum() == 0                       # nobody needs 4096 jumps: escapes are detected
     assert 0.005 < (st == -3).mean() < 0.5             # starts hug the surface (importance sampling): most return, some leave for good
     assert (rec["weight"][st == -3] == 0).all() and (rec["tri_t"][st == -3] == -1).all()
+
+
+# --------------------------------------------------------------------------
+# Alg. 1, the naive finite-difference estimator (Eq. 13-16)
+# --------------------------------------------------------------------------
+def test_naive_estimator_unit_ball_finite_difference_spectrum():
+    """On the unit ball the harmonic extension of Y_l is r^l Y_l, so Eq. 14 gives exactly
+    (1 - (1 - eps)^l) / eps for degree l (l - l(l-1) eps / 2 + ...): a closed form that pins the start point
+    x = s - eps n, the weight |dOmega| / (N eps) and the sign of b_s (b_s - b_t)^T."""
+    n_s, W, inset = 4000, 64, 0.05
+    pos = fibonacci_sphere(n_s)
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    P = OracleParams(seed=4, walks_per_sample=W, eps=1e-4, estimator=1, inset=inset)
+    rec, _ = orc.run_walks(P, False, weight=np.full(n_s, 4 * np.pi / n_s, np.float32), pos=pos)
+    assert (rec["steps"] >= 1).all()                                     # the inset point is outside the shell
+    assert np.allclose(np.linalg.norm(rec["z"], axis=1), 1.0 - inset, atol=1e-12)
+    assert np.allclose(rec["weight"], 4 * np.pi / n_s / W / inset, rtol=1e-6)
+    Ys = real_sph_harm(pos)[rec["sample"]]
+    Yt = real_sph_harm(rec["t"])
+    S = (Ys * rec["weight"][:, None]).T @ (Ys - Yt)
+    want = np.array([(1 - (1 - inset) ** l) / inset for l in DEGREES])
+    assert abs(S[0, 0]) < 1e-9
+    assert np.abs(np.diag(S) - want).max() < 0.08, (np.diag(S), want)
+    assert np.abs(S - np.diag(np.diag(S))).max() < 0.12
+
+
+def test_naive_estimator_on_mesh_is_symmetrised_not_psd_and_noisier():
+    """PAPER.md:163 (last line) and the two deficiencies listed after Eq. 16: the symmetrised naive estimate
+    is symmetric, but PSD only in expectation, and at equal walk count its entries are
+    noisier than those of Alg. 2 (Fig. 12's ordering)."""
+    from synth import icosphere, vertex_cell_samples
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 4, seed=0)
+    orc = Oracle(mesh_geom(v, f))
+    naive = orc.estimate_dtn(OracleParams(seed=3, walks_per_sample=32, eps=1e-4, estimator=1, inset=0.02), False,
+                             smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    jump = orc.estimate_dtn(OracleParams(seed=3, walks_per_sample=32, eps=1e-4), False,
+                            smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    Sn, Sj = naive["S"], jump["S"]
+    assert np.abs(Sn - Sn.T).max() < 1e-15 * np.abs(Sn).max() + 1e-18
+    # b_s d^T annihilates constants on the right only (d sums to 0); after symmetrisation the row sums are
+    # (1/2) sum_w w d, zero in expectation: the total over the whole matrix is exactly 0
+    assert abs(Sn.sum()) < 1e-6 * np.abs(Sn).sum()                       # fp32 barycentrics sum to 1 within 1e-7
+    assert np.linalg.eigvalsh(Sn).min() < -1e-3 * np.abs(Sn).max()       # not PSD at finite N
+    assert np.linalg.eigvalsh(Sj).min() > -1e-12 * np.abs(Sj).max()      # Alg. 2 is, by construction
+    # "the variance blows up as eps is decreased to reduce bias" (deficiency 2): ~1/eps, and above Alg. 2's
+    fine = orc.estimate_dtn(OracleParams(seed=3, walks_per_sample=32, eps=1e-5, estimator=1, inset=0.002), False,
+                            smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    assert fine["var"].mean() > 4.0 * naive["var"].mean()
+    assert fine["var"].mean() > 2.0 * jump["var"].mean()
+    # still the same operator in expectation: the coordinate functions are the l = 1 harmonics, for which the
+    # finite difference is exact on a ball ((1 - (1 - eps)) / eps = 1); Rayleigh quotients, not eigenvalues (not PSD)
+    M = orc.mass_matrix()
+    for k in range(3):
+        g = v[:, k].astype(np.float64)
+        assert abs(g @ Sn @ g / (g @ M @ g) - 1.0) < 0.1
