@@ -131,6 +131,11 @@ typedef struct {
     int32_t  output_kind;        /* 0: dense row-major fp32 [K][K] (K <= 65535);
                                     1: sparse COO, upper triangle (any K < 2^31)                */
     int64_t  coo_capacity;       /* output_kind 1: entries mcs_matrix.coo_* can hold (sizes the workspace) */
+    int32_t  estimator;          /* 0: Alg. 2, the tangent-ball jump-kernel estimator;
+                                    1: Alg. 1, the naive finite-difference estimator (Eq. 16),
+                                       interior only: walks start at s - inset * n_s, update
+                                       (a_i / (W inset)) b_s (b_s - b_t)^T, symmetrised; NOT PSD at finite N */
+    float    inset;              /* estimator 1: inset distance (the paper's epsilon of Eq. 13), > 0 */
 } mcs_params;
 
 typedef struct {

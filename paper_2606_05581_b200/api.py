@@ -49,7 +49,8 @@ class _Params(C.Structure):
                 ("eps", C.c_float), ("cap_half_angle_deg", C.c_float), ("rmax_scale", C.c_float),
                 ("rmax_override", C.c_float), ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
-                ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64)]
+                ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64),
+                ("estimator", C.c_int32), ("inset", C.c_float)]
 
 
 class _Matrix(C.Structure):
@@ -130,6 +131,8 @@ class Params:
     kelvin_origin: tuple = (0.0, 0.0, 0.0)
     output_kind: int = 0                 # 0 dense, 1 sparse COO (upper triangle)
     coo_capacity: int = 0
+    estimator: int = 0                   # 0: Alg. 2; 1: Alg. 1 (naive finite difference, interior only)
+    inset: float = 0.0                   # Alg. 1: walks start at s - inset * n_s
 
     def c(self) -> _Params:
         p = _Params(seed=self.seed, walks_per_sample=self.walks_per_sample, max_steps=self.max_steps,
@@ -137,7 +140,8 @@ class Params:
                     rmax_override=self.rmax_override, bisection_iters=self.bisection_iters,
                     importance_sample=int(self.importance_sample), antithetic=int(self.antithetic),
                     include_killing=int(self.include_killing), n_kill_walks=int(self.n_kill_walks),
-                    output_kind=int(self.output_kind), coo_capacity=int(self.coo_capacity))
+                    output_kind=int(self.output_kind), coo_capacity=int(self.coo_capacity),
+                    estimator=int(self.estimator), inset=float(self.inset))
         p.kelvin_origin[:] = [float(x) for x in self.kelvin_origin]
         return p
 

@@ -54,6 +54,7 @@ struct AccArgs {
     const float*   s_bary;
     long long n_main;       // records below this index belong to sample (index / W)
     int W;
+    int naive;              // Alg. 1: entries of (1/2)(b_s d^T + d b_s^T) instead of d d^T
     long long K;
 };
 
@@ -271,6 +272,7 @@ kill_pairs_kernel(const float* __restrict__ mface, long long f0, long long n, lo
 // ---------------------------------------------------------------------------
 struct PairBlock {
     int   idx[6];
+    float bs[6];          // b_v(s)
     float ds[6];          // D_v = b_v(s) - r_v(t): the pair's d at the reference exit point
     float At[6];          // sum wgt eta_v(t)
     int   tmask[6];       // corners of the exit face that are this vertex (bit k)
@@ -280,7 +282,7 @@ struct PairBlock {
 __device__ __forceinline__ int pair_block_slot(PairBlock& B, int vtx)
 {
     for (int q = 0; q < B.m; ++q) if (B.idx[q] == vtx) return q;
-    B.idx[B.m] = vtx; B.ds[B.m] = 0.0f; B.At[B.m] = 0.0f; B.tmask[B.m] = 0;
+    B.idx[B.m] = vtx; B.bs[B.m] = 0.0f; B.ds[B.m] = 0.0f; B.At[B.m] = 0.0f; B.tmask[B.m] = 0;
     return B.m++;
 }
 
@@ -289,7 +291,11 @@ __device__ __forceinline__ void build_pair_block(const AccArgs& a, const PairRec
     B.m = 0;
     if (r.sample >= 0) {
         const long long fs = a.s_tri[r.sample];
-        for (int k = 0; k < 3; ++k) B.ds[pair_block_slot(B, a.faces[3 * fs + k])] += a.s_bary[3 * (long long)r.sample + k];
+        for (int k = 0; k < 3; ++k) {
+            const int q = pair_block_slot(B, a.faces[3 * fs + k]);
+            const float bk = a.s_bary[3 * (long long)r.sample + k];
+            B.bs[q] += bk; B.ds[q] += bk;
+        }
     }
     const long long ft = r.tri_t;
     const bool killing = r.sample < 0;
@@ -352,8 +358,14 @@ expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32
         for (int q = 0; q < B.m; ++q)
             if (B.idx[p] <= B.idx[q]) {
                 // sum over the pair's walks of wgt * d_p d_q,  d = b(s) - b(t) = D - eta
-                float e = r.w * B.ds[p] * B.ds[q] - B.ds[p] * B.At[q] - B.At[p] * B.ds[q];
-                if (B.tmask[p] && B.tmask[q]) e += moment_block(r, B.tmask[p], B.tmask[q]);
+                float e;
+                if (a.naive) {
+                    // Alg. 1: sum wgt (1/2)(b_s,p d_q + b_s,q d_p),  sum wgt d = w D - A
+                    e = 0.5f * (B.bs[p] * (r.w * B.ds[q] - B.At[q]) + B.bs[q] * (r.w * B.ds[p] - B.At[p]));
+                } else {
+                    e = r.w * B.ds[p] * B.ds[q] - B.ds[p] * B.At[q] - B.At[p] * B.ds[q];
+                    if (B.tmask[p] && B.tmask[q]) e += moment_block(r, B.tmask[p], B.tmask[q]);
+                }
                 keys[o] = (KeyT)((long long)B.idx[p] * a.K + B.idx[q]);
                 vals[o] = __float_as_uint(e);
                 ++o;
@@ -576,7 +588,7 @@ size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int6
     return acc_layout(n_records, b->F).total;
 }
 
-int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W, int naive,
                    const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                    const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
 {
@@ -603,7 +615,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 
     AccArgs a;
     a.records = records; a.faces = b->faces; a.s_tri = s->tri; a.s_bary = s->bary;
-    a.n_main = (long long)s->n_s * W; a.W = W; a.K = K;
+    a.n_main = (long long)s->n_s * W; a.W = W; a.naive = naive; a.K = K;
     const int bits = key_bits_for(K);
     const long long n_main = a.n_main < n_records ? a.n_main : n_records, n_kill = n_records - n_main;
 
@@ -701,7 +713,7 @@ size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64
     return coo_layout(n_records, coo_capacity, b->F).total;
 }
 
-int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W, int naive,
                        const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                        const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
 {
@@ -729,7 +741,7 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
 
     AccArgs a;
     a.records = records; a.faces = b->faces; a.s_tri = s->tri; a.s_bary = s->bary;
-    a.n_main = (long long)s->n_s * W; a.W = W; a.K = K;
+    a.n_main = (long long)s->n_s * W; a.W = W; a.naive = naive; a.K = K;
     const int bits = key_bits_for64(K);
 
     float* mface = (float*)(base + L.mface);

@@ -39,8 +39,8 @@ int acc_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, cons
             const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
 {
     if (p->output_kind == 1)
-        return accumulate_coo_run(b, s, basis, p->walks_per_sample, records, n_records, ws, ws_bytes, out, stats_dev, st);
-    return accumulate_run(b, s, basis, p->walks_per_sample, records, n_records, ws, ws_bytes, out, stats_dev, st);
+        return accumulate_coo_run(b, s, basis, p->walks_per_sample, p->estimator == 1, records, n_records, ws, ws_bytes, out, stats_dev, st);
+    return accumulate_run(b, s, basis, p->walks_per_sample, p->estimator == 1, records, n_records, ws, ws_bytes, out, stats_dev, st);
 }
 
 struct Layout {

@@ -287,6 +287,21 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
     }
 }
 
+// Alg. 1: no tangent ball; the walk of sample i starts at the inset point
+// x = s - inset * n_s.  Written in the layout of the tangent balls: (x, 1), (n, 1).
+__global__ void __launch_bounds__(PT)
+naive_start_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
+                   const float* __restrict__ normal, int64_t n_s, float inset, float4* __restrict__ balls)
+{
+    const int64_t i = (int64_t)blockIdx.x * PT + threadIdx.x;
+    if (i >= n_s) return;
+    float3 s, n;
+    sample_point(g.verts, g.faces, tri, bary, i, s, n);
+    if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
+    balls[2 * i] = make_float4(fmaf(-inset, n.x, s.x), fmaf(-inset, n.y, s.y), fmaf(-inset, n.z, s.z), 1.0f);
+    balls[2 * i + 1] = make_float4(n.x, n.y, n.z, 1.0f);
+}
+
 // Orthonormal frame (e1, e2, n) of a unit vector n: branchless construction of
 // Duff et al. (JCGT 2017), restated (R6b: the frame rule is part of
 // the definition of a walk's start point).
@@ -525,6 +540,10 @@ walk_kernel(WalkGeom g, WalkArgs a)
                             a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
                             if (a.steps) a.steps[slot] = -2;
                             busy = false; start_query = false;
+                        } else if (a.naive) {                            // Alg. 1: start at the inset point, weight a_i / (W eps)
+                            x = f3(b0.x, b0.y, b0.z);
+                            wfac = (__ldg(&a.weight[sample]) / (float)a.W) * a.inv_inset;
+                            prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
                         } else {
                             // SampleBallSurface + BallJumpKernel (Eq. 23; R5-R7)
                             const unsigned wq = a.antithetic ? (walk >> 1) : walk;
@@ -626,6 +645,8 @@ int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, in
     if (p->bisection_iters < 1 || p->bisection_iters > 24) return MCS_EINVAL;
     if (!(p->rmax_scale > 0.0f) && !(p->rmax_override > 0.0f)) return MCS_EINVAL;
     if (s->n_s >= ((int64_t)1 << 32) - 1) return MCS_EINVAL;
+    if (p->estimator != 0 && p->estimator != 1) return MCS_EINVAL;
+    if (p->estimator == 1 && (exterior || !(p->inset > 0.0f))) return MCS_EINVAL;      // Alg. 1 is the interior estimator
     if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
     if (s->n_s * (int64_t)p->walks_per_sample >= ((int64_t)1 << 40)) return MCS_EINVAL;
     return MCS_OK;
@@ -711,7 +732,9 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     }
     mcs_note_launch(), face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
 
-    {
+    if (p->estimator == 1) {
+        mcs_note_launch(), naive_start_kernel<<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, n_s, p->inset, balls);
+    } else {
         int dev_tb = 0, n_sm_tb = 0;
         MCS_CUDA_TRY(cudaGetDevice(&dev_tb));
         MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm_tb, cudaDevAttrMultiProcessorCount, dev_tb));
@@ -737,6 +760,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.q0 = (float)sin(0.5 * (double)p->cap_half_angle_deg * 3.14159265358979323846 / 180.0);
     a.inv_q0 = 1.0f / a.q0;
     a.importance = p->importance_sample; a.antithetic = p->antithetic;
+    a.naive = p->estimator == 1; a.inv_inset = p->estimator == 1 ? 1.0f / p->inset : 0.0f;
     a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
     {
         const float dx = hi.x - lo.x, dy = hi.y - lo.y, dz = hi.z - lo.z;

@@ -27,6 +27,8 @@ struct WalkArgs {
     long long n_s, n_kill;
     int   W, max_steps, chunk;
     int   importance, antithetic;
+    int   naive;                   // Alg. 1: balls hold the start point, no ball sampling
+    float inv_inset;
     float eps, q0, inv_q0;
     float ox, oy, oz, Rmax;
     float escape;                  // interior: AABB diagonal (R10b); exterior: +inf
@@ -45,9 +47,9 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records);
 size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64_t coo_capacity);
-int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W, int naive,
                        const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                        const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);
-int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W, int naive,
                    const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                    const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);

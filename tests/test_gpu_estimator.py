@@ -407,3 +407,28 @@ def test_tiny_meshes_and_normal_override(api):
     S2 = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"], normal=nrm)
     B = api.estimate_dtn_interior(bvh, S2, P)
     assert (A - B).abs().max().item() <= 1e-5 * A.abs().max().item()
+
+
+# ------------------------------------------------------------------------------
+# Alg. 1, the naive finite-difference estimator
+# ------------------------------------------------------------------------------
+def test_naive_estimator_records_and_matrix_match_oracle(api):
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 4, seed=0)
+    gp, op = _params(api, seed=6, walks_per_sample=64, eps=1e-4, estimator=1, inset=0.02)
+    rec, steps, orec, st = _compare_records(api, v, f, smp, False, gp, op)
+    assert st.n_discarded == 0 and (steps >= 1).all()                   # the inset point is outside the shell
+    bvh, S = _setup(api, v, f, smp)
+    A = api.estimate_dtn_interior(bvh, S, gp)
+    assert torch.equal(A, api.estimate_dtn_interior(bvh, S, gp)) and torch.equal(A, A.T)
+    Sg = A.cpu().numpy().astype(np.float64)
+    out = Oracle(mesh_geom(v, f)).estimate_dtn(op, False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    _assert_within_4se(Sg, out, smp, f)
+    assert np.linalg.eigvalsh(Sg).min() < -1e-3 * np.abs(Sg).max()      # PSD only in expectation (PAPER.md, after Eq. 16)
+    coo = api.estimate_dtn_coo(bvh, S, gp, False)
+    assert torch.equal(coo.to_dense(), A)
+    with pytest.raises(api.McsError) as e:                               # Alg. 1 is the interior estimator
+        api.estimate_dtn_exterior(bvh, S, gp)
+    assert e.value.code == api.MCS_EINVAL
+    with pytest.raises(api.McsError):
+        api.estimate_dtn_interior(bvh, S, api.Params(walks_per_sample=2, estimator=1, inset=0.0))
