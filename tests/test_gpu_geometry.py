@@ -219,3 +219,23 @@ def test_build_edge_cases_and_errors(api):
     bvh = _bvh(api, v2, f2)
     d, t, _ = api.closest_point(bvh, _cuda(np.array([[0.9, 0.9, 1.0]]), torch.float32))
     assert t.item() == 1 and abs(d.item() - 1.0) < 1e-6
+
+
+def test_closest_point_one_million_queries(api):
+    """SURVEY.md 8(c) 'LBVH (GPU)': query result = brute force on >= 1e6 queries.  The exhaustive device scan
+    (same fp32 point-triangle routine, every face) is the brute force at this count; the fp64 oracle checks a
+    seeded sample of them, tie-free by its own gap filter."""
+    v, f = two_spheres_torus_scene(level=4, distance=2.5, with_torus=True)[:2]
+    q = np.concatenate([near_surface_queries(v, f, 700_000, seed=21), far_field_queries(v, 300_000, seed=22)])
+    bvh = _bvh(api, v, f)
+    qd = _cuda(q, torch.float32)
+    d1, t1, b1 = api.closest_point(bvh, qd)
+    d2, t2, b2 = api.closest_point_bruteforce(bvh, qd)
+    assert torch.equal(d1, d2) and torch.equal(t1, t2) and torch.equal(b1, b2)
+    idx = np.random.default_rng(3).choice(len(q), 4000, replace=False)
+    orc = Oracle(mesh_geom(v, f))
+    keep, r = _tie_free(orc, q[idx])
+    assert keep.sum() > 1500                                       # symmetric scene: many far-field queries are near-ties
+    assert np.array_equal(t1.cpu().numpy()[idx][keep], r["tri"][keep])
+    D, dg = r["dist"], d1.cpu().numpy()[idx]
+    assert (np.abs(dg - D) <= 1e-6 * D + 2e-7 * float(np.abs(v).max())).all()
