@@ -22,6 +22,8 @@
  *   interior weights     analytic unit ball: S -> diag(l) minus the cap term
  *   exterior weights     analytic sphere, centred and off-centre: l, l+1, capacity
  *   mesh estimators      symmetry, PSD, zero row sums, multiplicities 1,3,5,7
+ *   Alg. 1 (naive)       unit ball: (1 - (1 - eps)^l) / eps; mesh: not PSD, variance ~ 1/eps
+ *   point basis (k-NN)   numpy neighbour search, weight special cases, sphere spectrum l through the estimator
  * Parity unpinned: nothing in this file.
  */
 #include <math.h>
@@ -869,6 +871,125 @@ void orc_accumulate_hat_naive(const orc_geom *g, const orc_record *rec, int64_t 
 {
     accumulate_hat_impl(g, rec, n_rec, tri, bary, K, S, S2, 1);
 }
+
+/* ------------------------------------------------------------------------- */
+/* Point-based function space: k-NN bilateral interpolator (PAPER.md:373-379;  */
+/* App. B, Eq. 44-45).  The basis functions live on a point  */
+/* cloud (x_i, n_i), i < K; the value of a boundary function at a query point  */
+/* q with normal n_q is  sum_{i in N_k(q)} w_i(q) phi(x_i),                     */
+/*   w~_i = exp(-|q - x_i|^2 / (2 sigma^2)) exp(-(1 - <n_q, n_i>) / tau_n),    */
+/*   w_i = w~_i / sum_j w~_j,                                                  */
+/* so the vector b(q) of Alg. 2 has the k non-zeros w_i(q).                    */
+/* Readings: [Rk1] the w~ are formed relative to the largest       */
+/* exponent (identical after normalisation; no 0/0 when q is many sigma away   */
+/* from every point); [Rk2] neighbours by squared distance, ties by smaller    */
+/* index; [Rk3] k is clamped to K; [Rk4] n_q is the sample's normal at s and    */
+/* the normal of the exit face at t.                                           */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    const float *points;        /* [K][3] */
+    const float *normals;       /* [K][3] unit */
+    int64_t K;
+    int32_t k;                  /* neighbours (paper: 8) */
+    int32_t pad_;
+    double sigma, tau_n;        /* paper: 0.025, 0.8 */
+} orc_point_basis;
+
+#define ORC_KNN_MAX 32
+
+void orc_knn_weights(const orc_point_basis *PB, const double q[3], const double nq[3],
+                     int64_t *idx /* [k] */, double *w /* [k] */)
+{
+    int k = PB->k < PB->K ? PB->k : (int)PB->K;
+    if (k > ORC_KNN_MAX) k = ORC_KNN_MAX;
+    double bd[ORC_KNN_MAX]; int64_t bi[ORC_KNN_MAX];
+    int n = 0;
+    for (int64_t i = 0; i < PB->K; ++i) {                      /* brute force over all points */
+        double d[3] = { q[0] - (double)PB->points[3*i], q[1] - (double)PB->points[3*i+1], q[2] - (double)PB->points[3*i+2] };
+        double d2 = dot3(d, d);
+        if (n == k && !(d2 < bd[k-1])) continue;                /* strict <: on a tie the smaller index stays */
+        int pos = n < k ? n : k - 1;
+        while (pos > 0 && d2 < bd[pos-1]) { bd[pos] = bd[pos-1]; bi[pos] = bi[pos-1]; --pos; }
+        bd[pos] = d2; bi[pos] = i;
+        if (n < k) ++n;
+    }
+    double lg[ORC_KNN_MAX], lmax = -INFINITY, sum = 0.0;
+    for (int j = 0; j < k; ++j) {
+        const float *ni = PB->normals + 3 * bi[j];
+        double c = nq[0] * (double)ni[0] + nq[1] * (double)ni[1] + nq[2] * (double)ni[2];
+        lg[j] = -bd[j] / (2.0 * PB->sigma * PB->sigma) - (1.0 - c) / PB->tau_n;     /* Eq. 45 */
+        if (lg[j] > lmax) lmax = lg[j];
+    }
+    for (int j = 0; j < k; ++j) { w[j] = exp(lg[j] - lmax); sum += w[j]; }          /* [Rk1] */
+    for (int j = 0; j < k; ++j) { w[j] /= sum; idx[j] = bi[j]; }
+    for (int j = k; j < PB->k; ++j) { idx[j] = -1; w[j] = 0.0; }
+}
+
+/* S += weight d d^T with d = b(s) - b(t) in the point basis (killing: weight b(t) b(t)^T), plus the
+ * per-entry variance estimate of orc_accumulate_hat.  s and n_s come from the sample arrays (mesh:
+ * tri/bary, sphere: pos), t from the record, n_t from the exit face (sphere: radial)  [Rk4]. */
+void orc_accumulate_points(const orc_geom *g, const orc_point_basis *PB, const orc_record *rec, int64_t n_rec,
+                           const int32_t *tri, const float *bary, const float *weight, const float *normal,
+                           const double *pos, double *S /* [K][K] zeroed */, double *S2 /* or NULL */)
+{
+    const int64_t K = PB->K;
+    const int k = PB->k;
+    orc_entry *buf = NULL;
+    int64_t cap = 0;
+    for (int64_t g0 = 0; g0 < n_rec; ) {
+        int64_t g1 = g0, sample = rec[g0].sample;
+        while (g1 < n_rec && rec[g1].sample == sample) ++g1;
+        int64_t is[ORC_KNN_MAX]; double ws[ORC_KNN_MAX];
+        if (sample >= 0) {
+            orc_sample SS;
+            fill_sample(g, tri, bary, weight, normal, pos, sample, &SS);
+            orc_knn_weights(PB, SS.s, SS.n, is, ws);
+        }
+        int64_t n_e = 0;
+        const int64_t per = (int64_t)(2 * k) * (2 * k);
+        if (S2 && per * (g1 - g0) > cap) { cap = per * (g1 - g0); buf = (orc_entry *)realloc(buf, cap * sizeof *buf); }
+        for (int64_t r = g0; r < g1; ++r) {
+            const orc_record *R = rec + r;
+            if (R->steps < 0 || R->weight == 0.0) continue;
+            double nt[3], area;
+            if (g->kind == 0) face_normal_area(g, R->tri_t, nt, &area);
+            else { double d[3]; sub3(R->t, g->centre, d); double l = norm3(d); for (int c = 0; c < 3; ++c) nt[c] = d[c] / l; }
+            int64_t it[ORC_KNN_MAX]; double wt[ORC_KNN_MAX];
+            orc_knn_weights(PB, R->t, nt, it, wt);
+            int64_t idx[2 * ORC_KNN_MAX]; double val[2 * ORC_KNN_MAX];
+            int n = 0;
+            if (sample >= 0) for (int j = 0; j < k; ++j) if (is[j] >= 0) { idx[n] = is[j]; val[n] = ws[j]; ++n; }
+            const double sign = sample >= 0 ? -1.0 : 1.0;
+            for (int j = 0; j < k; ++j) {
+                if (it[j] < 0) continue;
+                int found = -1;
+                for (int m = 0; m < n; ++m) if (idx[m] == it[j]) found = m;
+                if (found >= 0) val[found] += sign * wt[j];
+                else { idx[n] = it[j]; val[n] = sign * wt[j]; ++n; }
+            }
+            for (int p = 0; p < n; ++p) for (int q = 0; q < n; ++q) {
+                double x = R->weight * val[p] * val[q];
+                S[idx[p] * K + idx[q]] += x;
+                if (S2) { buf[n_e].key = idx[p] * K + idx[q]; buf[n_e].val = x; ++n_e; }
+            }
+        }
+        if (S2 && n_e > 0) {
+            double Wg = (double)(g1 - g0);
+            qsort(buf, (size_t)n_e, sizeof *buf, entry_cmp);
+            for (int64_t e0 = 0; e0 < n_e; ) {
+                int64_t e1 = e0; double s1 = 0.0, s2 = 0.0;
+                while (e1 < n_e && buf[e1].key == buf[e0].key) { s1 += buf[e1].val; s2 += buf[e1].val * buf[e1].val; ++e1; }
+                double var = (Wg > 1.0) ? Wg / (Wg - 1.0) * (s2 - s1 * s1 / Wg) : s2;
+                S2[buf[e0].key] += var > 0.0 ? var : 0.0;
+                e0 = e1;
+            }
+        }
+        g0 = g1;
+    }
+    free(buf);
+}
+
+size_t orc_sizeof_point_basis(void) { return sizeof(orc_point_basis); }
 
 int orc_num_threads(void)
 {

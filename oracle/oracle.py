@@ -34,6 +34,8 @@ def _load():
         assert _lib.orc_sizeof_record() == RECORD_DTYPE.itemsize
         assert _lib.orc_sizeof_params() == C.sizeof(_Params)
         assert _lib.orc_sizeof_geom() == C.sizeof(_Geom)
+        _lib.orc_sizeof_point_basis.restype = C.c_size_t
+        assert _lib.orc_sizeof_point_basis() == C.sizeof(_PointBasis)
     return _lib
 
 
@@ -51,6 +53,27 @@ class _Params(C.Structure):
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32),
                 ("n_kill_walks", C.c_int64), ("origin", C.c_double * 3), ("Rmax_norm", C.c_double),
                 ("escape_radius", C.c_double), ("estimator", C.c_int32), ("pad_", C.c_int32), ("inset", C.c_double)]
+
+
+class _PointBasis(C.Structure):
+    _fields_ = [("points", C.c_void_p), ("normals", C.c_void_p), ("K", C.c_int64), ("k", C.c_int32),
+                ("pad_", C.c_int32), ("sigma", C.c_double), ("tau_n", C.c_double)]
+
+
+@dataclass
+class PointBasis:
+    """Point-based function space: points, unit normals, k, sigma, tau_n."""
+    points: np.ndarray
+    normals: np.ndarray
+    k: int = 8
+    sigma: float = 0.025
+    tau_n: float = 0.8
+
+    def c(self):
+        self._p = np.ascontiguousarray(self.points, np.float32)
+        self._n = np.ascontiguousarray(self.normals, np.float32)
+        return _PointBasis(points=self._p.ctypes.data, normals=self._n.ctypes.data, K=len(self._p), k=int(self.k),
+                           sigma=float(self.sigma), tau_n=float(self.tau_n))
 
 
 RECORD_DTYPE = np.dtype([("sample", np.int64), ("tri_t", np.int64), ("bary_t", np.float64, 3),
@@ -256,6 +279,46 @@ class Oracle:
                                     S.ctypes.data_as(C.c_void_p),
                                     S2.ctypes.data_as(C.c_void_p) if want_var else None)
         return (S, S2) if want_var else S
+
+    def knn_weights(self, basis: "PointBasis", q, nq):
+        """(idx [n,k], w [n,k]) of the k-NN bilateral interpolator at points q with normals nq (Eq. 44-45)."""
+        pb = basis.c()
+        q = np.ascontiguousarray(q, np.float64).reshape(-1, 3)
+        nq = np.ascontiguousarray(nq, np.float64).reshape(-1, 3)
+        idx = np.empty((len(q), basis.k), np.int64)
+        w = np.empty((len(q), basis.k))
+        for i in range(len(q)):
+            self.lib.orc_knn_weights(C.byref(pb), q[i].ctypes.data_as(C.c_void_p), nq[i].ctypes.data_as(C.c_void_p),
+                                     idx[i].ctypes.data_as(C.c_void_p), w[i].ctypes.data_as(C.c_void_p))
+        return idx, w
+
+    def accumulate_points(self, basis: "PointBasis", rec, tri=None, bary=None, weight=None, normal=None, pos=None,
+                          want_var=False):
+        pb = basis.c()
+        K = len(basis.points)
+        rec = np.ascontiguousarray(rec)
+        weight = np.ascontiguousarray(weight, np.float32)
+        if self.geom.c.kind == 0:
+            tri = np.ascontiguousarray(tri, np.int32)
+            bary = np.ascontiguousarray(bary, np.float32)
+        else:
+            pos = np.ascontiguousarray(pos, np.float64)
+        if normal is not None:
+            normal = np.ascontiguousarray(normal, np.float32)
+        S = np.zeros((K, K))
+        S2 = np.zeros((K, K)) if want_var else None
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        self.lib.orc_accumulate_points(C.byref(self.geom.c), C.byref(pb), ptr(rec), C.c_int64(len(rec)), ptr(tri), ptr(bary),
+                                       ptr(weight), ptr(normal), ptr(pos), ptr(S), ptr(S2))
+        return (S, S2) if want_var else S
+
+    def estimate_dtn_points(self, basis: "PointBasis", params: OracleParams, exterior: bool, tri, bary, weight,
+                            normal=None, want_var=False):
+        """Dense DtN matrix in the point basis (K = number of points) plus records."""
+        rec, balls = self.run_walks(params, exterior, tri, bary, weight, normal)
+        out = self.accumulate_points(basis, rec, tri, bary, weight, normal, want_var=want_var)
+        S, var = out if want_var else (out, None)
+        return dict(S=S, var=var, records=rec, balls=balls)
 
     def estimate_dtn(self, params: OracleParams, exterior: bool, tri, bary, weight, normal=None,
                      want_var=False):
