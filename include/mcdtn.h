@@ -109,9 +109,18 @@ typedef struct {                 /* boundary samples: point s with its face, PAP
 } mcs_samples;
 
 typedef struct {                 /* boundary basis functions b(.) of Alg. 2 */
-    int32_t kind;                /* 0 = hat functions on the mesh vertices (K = V)            */
+    int32_t kind;                /* 0 = hat functions on the mesh vertices (K = V);
+                                    1 = point-based k-NN bilateral interpolator (App. B
+                                        Eq. 44-45): K = number of points, b(q) has the k weights w_i(q)   */
     int32_t pad_;
     int64_t K;
+    /* kind 1 only (ignored for kind 0) */
+    const float* points;         /* [K][3] positions x_i                                                */
+    const float* normals;        /* [K][3] unit normals n_i                                             */
+    int32_t k;                   /* neighbours, 1..16 (paper: 8); clamped to K                          */
+    float   sigma;               /* spatial falloff (paper: 0.025)                                      */
+    float   tau_n;               /* normal falloff (paper: 0.8)                                         */
+    int32_t pad2_;
 } mcs_basis;
 
 typedef struct {
@@ -231,8 +240,8 @@ int mcs_tangent_balls(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_
 
 /* Workspace (bytes) of mcs_run_walks and of mcs_accumulate. */
 size_t mcs_walk_workspace_bytes(const mcs_samples* samples);
-size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_basis* basis, const mcs_params* params,
-                                      int64_t n_records);
+size_t mcs_accumulate_workspace_bytes(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                                      const mcs_params* params, int64_t n_records);
 
 /* A2-A6: run every walk and write records [n_s*W (+ n_kill_walks)] and, if non-NULL,
  * steps [same length] (jumps taken; -1 truncated at max_steps; -2 sample discarded; -3 interior
@@ -247,6 +256,12 @@ int mcs_accumulate(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_bas
                    const mcs_params* params, const mcs_record* records, int64_t n_records,
                    void* workspace, size_t workspace_bytes, const mcs_matrix* out,
                    mcs_stats* host_stats, void* stream);
+
+/* k-NN bilateral weights of a kind-1 basis at Q query points q [Q][3] with unit normals nq [Q][3]
+ * (Eq. 44-45): idx [Q][k] (neighbours by increasing distance, ties by smaller index; -1 beyond K),
+ * w [Q][k] (sum 1).  Exhaustive search over the K points.  Asynchronous on `stream`. */
+int mcs_knn_weights(const mcs_basis* basis, const float* q, const float* nq, int64_t Q,
+                    int32_t* idx, float* w, void* stream);
 
 /* Philox4x32-10 words for counters [n][4] and one key [2] (host): out [n][4].
  * Lets the tests pin the device generator against the known answers. */

@@ -41,7 +41,9 @@ class _Samples(C.Structure):
 
 
 class _Basis(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64)]
+    _fields_ = [("kind", C.c_int32), ("pad_", C.c_int32), ("K", C.c_int64), ("points", C.c_void_p),
+                ("normals", C.c_void_p), ("k", C.c_int32), ("sigma", C.c_float), ("tau_n", C.c_float),
+                ("pad2_", C.c_int32)]
 
 
 class _Params(C.Structure):
@@ -246,21 +248,60 @@ def closest_point_bruteforce(bvh: Bvh, q):
     return _closest(lib().mcs_closest_point_bruteforce, "mcs_closest_point_bruteforce", bvh, q)
 
 
-def _basis(bvh: Bvh) -> _Basis:
-    return _Basis(kind=0, K=bvh.V)
+@dataclass
+class PointBasis:
+    """Point-based function space (mcs_basis.kind 1; App. B): device tensors points [K,3], unit normals
+    [K,3]; k neighbours, sigma, tau_n."""
+    points: torch.Tensor
+    normals: torch.Tensor
+    k: int = 8
+    sigma: float = 0.025
+    tau_n: float = 0.8
+
+    @classmethod
+    def from_arrays(cls, points, normals, k=8, sigma=0.025, tau_n=0.8, device="cuda"):
+        p = torch.as_tensor(points).to(device=device, dtype=torch.float32).contiguous()
+        n = torch.as_tensor(normals).to(device=device, dtype=torch.float32).contiguous()
+        return cls(p, n, k, sigma, tau_n)
+
+    @property
+    def K(self):
+        return int(self.points.shape[0])
+
+    def c(self) -> _Basis:
+        assert self.points.is_cuda and self.normals.is_cuda and self.points.shape == self.normals.shape
+        return _Basis(kind=1, K=self.K, points=self.points.data_ptr(), normals=self.normals.data_ptr(), k=int(self.k),
+                      sigma=float(self.sigma), tau_n=float(self.tau_n))
 
 
-def workspace_bytes(bvh: Bvh, samples: Samples, params: Params, exterior: bool) -> int:
-    cs, cb, cp = samples.c(), _basis(bvh), params.c()
+def _basis(bvh: Bvh, basis=None) -> _Basis:
+    return basis.c() if basis is not None else _Basis(kind=0, K=bvh.V)
+
+
+def knn_weights(basis: PointBasis, q, nq):
+    """(idx [Q,k] int32, w [Q,k] fp32) of the k-NN bilateral interpolator (mcs_knn_weights)."""
+    q, nq = _dev(q, torch.float32, "q"), _dev(nq, torch.float32, "nq")
+    Q = int(q.shape[0])
+    idx = torch.empty((Q, basis.k), dtype=torch.int32, device=q.device)
+    w = torch.empty((Q, basis.k), dtype=torch.float32, device=q.device)
+    cb = basis.c()
+    with torch.cuda.device(q.device):
+        _check(lib().mcs_knn_weights(C.byref(cb), _ptr(q), _ptr(nq), C.c_int64(Q), _ptr(idx), _ptr(w), _stream(q.device)),
+               "mcs_knn_weights")
+    return idx, w
+
+
+def workspace_bytes(bvh: Bvh, samples: Samples, params: Params, exterior: bool, basis=None) -> int:
+    cs, cb, cp = samples.c(), _basis(bvh, basis), params.c()
     return int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
 
 
-def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace, _exact_workspace=False):
-    cs, cb, cp = samples.c(), _basis(bvh), params.c()
-    K = bvh.V
+def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace, _exact_workspace=False, basis=None):
+    cs, cb, cp = samples.c(), _basis(bvh, basis), params.c()
+    K = basis.K if basis is not None else bvh.V
     if out is None:
         out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
-    need = workspace_bytes(bvh, samples, params, exterior)
+    need = workspace_bytes(bvh, samples, params, exterior, basis)
     if workspace is None or (workspace.numel() < need and not _exact_workspace):
         workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
     m = _Matrix(kind=0, K=K, dense=out.data_ptr())
@@ -273,17 +314,18 @@ def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspa
 
 
 def estimate_dtn_interior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
-                          _exact_workspace=False):
-    """Interior DtN matrix, Alg. 2: dense [K,K] fp32 on the device."""
+                          _exact_workspace=False, basis=None):
+    """Interior DtN matrix, Alg. 2: dense [K,K] fp32 on the device (K = V, or the number of
+    points of a PointBasis)."""
     return _estimate(lib().mcs_estimate_dtn_interior, "mcs_estimate_dtn_interior", bvh, samples, params, False,
-                     want_stats, out, workspace, _exact_workspace)
+                     want_stats, out, workspace, _exact_workspace, basis)
 
 
 def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
-                          _exact_workspace=False):
+                          _exact_workspace=False, basis=None):
     """Exterior DtN matrix, Eq. 32."""
     return _estimate(lib().mcs_estimate_dtn_exterior, "mcs_estimate_dtn_exterior", bvh, samples, params, True,
-                     want_stats, out, workspace, _exact_workspace)
+                     want_stats, out, workspace, _exact_workspace, basis)
 
 
 def estimate_dtn_host(verts, faces, tri, bary, weight, params: Params, interior=True, exterior=True,
@@ -358,13 +400,13 @@ def run_walks(bvh: Bvh, samples: Samples, params: Params, exterior: bool, want_s
     return (rec, steps, st) if want_stats else (rec, steps)
 
 
-def accumulate(bvh: Bvh, samples: Samples, params: Params, records, want_stats=False):
-    cs, cb, cp = samples.c(), _basis(bvh), params.c()
+def accumulate(bvh: Bvh, samples: Samples, params: Params, records, want_stats=False, basis=None):
+    cs, cb, cp = samples.c(), _basis(bvh, basis), params.c()
     records = _dev(records, torch.float32, "records")
     n = records.shape[0]
-    K = bvh.V
+    K = basis.K if basis is not None else bvh.V
     out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
-    need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cb), C.byref(cp), C.c_int64(n)))
+    need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int64(n)))
     ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
     m = _Matrix(kind=0, K=K, dense=out.data_ptr())
     st = Stats() if want_stats else None

@@ -807,3 +807,349 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
     MCS_CUDA_TRY(cudaStreamSynchronize(st));                               // host scalars above live on this frame
     return MCS_OK;
 }
+
+// ===========================================================================
+// Point-based function space (mcs_basis.kind 1): k-NN bilateral interpolator of
+// PAPER.md App. B (Eq. 44-45).  b(q) has the k weights
+//   w_i(q) ~ exp(-|q - x_i|^2 / (2 sigma^2)) exp(-(1 - <n_q, n_i>) / tau_n)
+// over the k nearest points, normalised; d = b(s) - b(t) has up to 2k non-zeros, so
+// a walk expands to up to 2k(2k+1)/2 upper-triangular entries, which go through the
+// same stable sort + fixed-shape run sums as the hat basis.
+// Readings (DESIGN.md Rk1-Rk4): weights formed relative to the largest exponent;
+// neighbours by fp32 squared distance, ties by smaller index; k clamped to K;
+// n_q = sample normal at s, normal of the exit face at t.
+// ===========================================================================
+namespace {
+
+constexpr int KNN_MAX = 16;
+constexpr int KNN_TILE = 256;
+constexpr int64_t PB_CHUNK_WALKS = (int64_t)1 << 19;
+
+struct PointBasisDev {
+    const float* points;
+    const float* normals;
+    long long K;
+    int k;
+    float inv2s2, inv_tau;
+};
+
+// Exhaustive k-NN of one query per thread, points staged through shared memory; the k best are kept
+// sorted in registers (static indices only).  Every thread of the block must call this.
+__device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool active, float3 q, float3 nq,
+                                                   float4* s_pts, int* idx_out, float* w_out)
+{
+    float bd[KNN_MAX]; int bi[KNN_MAX];
+#pragma unroll
+    for (int j = 0; j < KNN_MAX; ++j) { bd[j] = CUDART_INF_F; bi[j] = -1; }
+    const int k = pb.k;
+    for (long long base = 0; base < pb.K; base += KNN_TILE) {
+        const int n = (int)((pb.K - base) < KNN_TILE ? (pb.K - base) : KNN_TILE);
+        __syncthreads();
+        for (int j = threadIdx.x; j < n; j += blockDim.x)
+            s_pts[j] = make_float4(pb.points[3 * (base + j)], pb.points[3 * (base + j) + 1], pb.points[3 * (base + j) + 2], 0.0f);
+        __syncthreads();
+        if (active) {
+            for (int j = 0; j < n; ++j) {
+                const float4 p = s_pts[j];
+                const float dx = q.x - p.x, dy = q.y - p.y, dz = q.z - p.z;
+                const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (d2 < bd[KNN_MAX - 1]) {                    // strict: on a tie the smaller index stays in front
+                    bd[KNN_MAX - 1] = d2; bi[KNN_MAX - 1] = (int)(base + j);
+#pragma unroll
+                    for (int m = KNN_MAX - 1; m > 0; --m)
+                        if (bd[m] < bd[m - 1]) {
+                            const float td = bd[m]; bd[m] = bd[m - 1]; bd[m - 1] = td;
+                            const int ti = bi[m]; bi[m] = bi[m - 1]; bi[m - 1] = ti;
+                        }
+                }
+            }
+        }
+    }
+    if (!active) return;
+    // only the first k count: the list holds the KNN_MAX nearest in order
+    float lg[KNN_MAX], lmax = -CUDART_INF_F;
+#pragma unroll
+    for (int j = 0; j < KNN_MAX; ++j) {
+        const bool use = j < k && bi[j] >= 0;
+        float c = 0.0f;
+        if (use) {
+            const float* ni = pb.normals + 3 * (long long)bi[j];
+            c = fmaf(nq.x, ni[0], fmaf(nq.y, ni[1], nq.z * ni[2]));
+        }
+        lg[j] = use ? -bd[j] * pb.inv2s2 - (1.0f - c) * pb.inv_tau : -CUDART_INF_F;
+        lmax = fmaxf(lmax, lg[j]);
+    }
+    float sum = 0.0f;
+#pragma unroll
+    for (int j = 0; j < KNN_MAX; ++j) { lg[j] = (j < k && bi[j] >= 0) ? expf(lg[j] - lmax) : 0.0f; sum += lg[j]; }
+    const float inv = 1.0f / sum;
+#pragma unroll
+    for (int j = 0; j < KNN_MAX; ++j)
+        if (j < k) { idx_out[j] = bi[j]; w_out[j] = lg[j] * inv; }
+}
+
+__global__ void __launch_bounds__(AT)
+knn_queries_kernel(PointBasisDev pb, const float* __restrict__ q, const float* __restrict__ nq, long long Q,
+                   int32_t* __restrict__ idx, float* __restrict__ w)
+{
+    __shared__ float4 s_pts[KNN_TILE];
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    const bool active = i < Q;
+    float3 qq = make_float3(0.f, 0.f, 0.f), nn = make_float3(0.f, 0.f, 1.f);
+    if (active) { qq = make_float3(q[3 * i], q[3 * i + 1], q[3 * i + 2]); nn = make_float3(nq[3 * i], nq[3 * i + 1], nq[3 * i + 2]); }
+    int io[KNN_MAX]; float wo[KNN_MAX];
+    knn_weights_device(pb, active, qq, nn, s_pts, io, wo);
+    if (active)
+        for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
+}
+
+__device__ __forceinline__ void face_point_normal(const float* __restrict__ verts, const int32_t* __restrict__ faces,
+                                                  long long f, float b0, float b1, float b2, float3& p, float3& n)
+{
+    const long long i0 = faces[3 * f], i1 = faces[3 * f + 1], i2 = faces[3 * f + 2];
+    const float3 a = make_float3(verts[3 * i0], verts[3 * i0 + 1], verts[3 * i0 + 2]);
+    const float3 b = make_float3(verts[3 * i1], verts[3 * i1 + 1], verts[3 * i1 + 2]);
+    const float3 c = make_float3(verts[3 * i2], verts[3 * i2 + 1], verts[3 * i2 + 2]);
+    p = make_float3(fmaf(b0, a.x, fmaf(b1, b.x, b2 * c.x)), fmaf(b0, a.y, fmaf(b1, b.y, b2 * c.y)), fmaf(b0, a.z, fmaf(b1, b.z, b2 * c.z)));
+    const float ux = b.x - a.x, uy = b.y - a.y, uz = b.z - a.z, vx = c.x - a.x, vy = c.y - a.y, vz = c.z - a.z;
+    n = make_float3(uy * vz - uz * vy, uz * vx - ux * vz, ux * vy - uy * vx);
+    const float l = sqrtf(fmaf(n.x, n.x, fmaf(n.y, n.y, n.z * n.z)));
+    if (l > 0.0f) { n.x /= l; n.y /= l; n.z /= l; }
+}
+
+// b(s) of every sample
+__global__ void __launch_bounds__(AT)
+knn_samples_kernel(PointBasisDev pb, const float* __restrict__ verts, const int32_t* __restrict__ faces,
+                   const int32_t* __restrict__ s_tri, const float* __restrict__ s_bary, const float* __restrict__ s_normal,
+                   long long n_s, int32_t* __restrict__ idx, float* __restrict__ w)
+{
+    __shared__ float4 s_pts[KNN_TILE];
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    const bool active = i < n_s;
+    float3 p = make_float3(0.f, 0.f, 0.f), n = make_float3(0.f, 0.f, 1.f);
+    if (active) {
+        face_point_normal(verts, faces, s_tri[i], s_bary[3 * i], s_bary[3 * i + 1], s_bary[3 * i + 2], p, n);
+        if (s_normal) n = make_float3(s_normal[3 * i], s_normal[3 * i + 1], s_normal[3 * i + 2]);
+    }
+    int io[KNN_MAX]; float wo[KNN_MAX];
+    knn_weights_device(pb, active, p, n, s_pts, io, wo);
+    if (active)
+        for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
+}
+
+// b(t) of the records [j0, j0 + n): idx = -1 everywhere for a record without contribution
+__global__ void __launch_bounds__(AT)
+knn_records_kernel(PointBasisDev pb, const float* __restrict__ verts, const int32_t* __restrict__ faces,
+                   const float4* __restrict__ records, long long j0, long long n,
+                   int32_t* __restrict__ idx, float* __restrict__ w)
+{
+    __shared__ float4 s_pts[KNN_TILE];
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    bool active = i < n;
+    float3 p = make_float3(0.f, 0.f, 0.f), nrm = make_float3(0.f, 0.f, 1.f);
+    if (active) {
+        const float4 rec = records[j0 + i];
+        const int tri_t = __float_as_int(rec.x);
+        if (tri_t >= 0 && rec.w != 0.0f) face_point_normal(verts, faces, tri_t, 1.0f - rec.y - rec.z, rec.y, rec.z, p, nrm);
+        else { active = false; for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = -1; w[i * pb.k + j] = 0.0f; } }
+    }
+    int io[KNN_MAX]; float wo[KNN_MAX];
+    knn_weights_device(pb, active, p, nrm, s_pts, io, wo);
+    if (active)
+        for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
+}
+
+}  // namespace
+
+namespace {
+
+// d = b(s) - b(t) of record i as a merged list (shared points once); killing walks: d = b(t).
+__device__ __forceinline__ int build_d_points(int k, bool has_s, const int32_t* __restrict__ is, const float* __restrict__ ws,
+                                              const int32_t* __restrict__ it, const float* __restrict__ wt,
+                                              int* idx, float* val)
+{
+    int m = 0;
+    if (has_s)
+        for (int j = 0; j < k; ++j) if (is[j] >= 0) { idx[m] = is[j]; val[m] = ws[j]; ++m; }
+    const float sign = has_s ? -1.0f : 1.0f;
+    for (int j = 0; j < k; ++j) {
+        if (it[j] < 0) continue;
+        int found = -1;
+        for (int q = 0; q < m; ++q) if (idx[q] == it[j]) found = q;
+        if (found >= 0) val[found] += sign * wt[j];
+        else { idx[m] = it[j]; val[m] = sign * wt[j]; ++m; }
+    }
+    return m;
+}
+
+__global__ void __launch_bounds__(AT)
+count_entries_points_kernel(int k, long long j0, long long n, long long n_main, int W,
+                            const int32_t* __restrict__ is, const float* __restrict__ ws,
+                            const int32_t* __restrict__ it, const float* __restrict__ wt, uint32_t* __restrict__ counts)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n) return;
+    uint32_t c = 0;
+    if (it[i * k] >= 0) {
+        const bool has_s = j0 + i < n_main;
+        const long long smp = has_s ? (j0 + i) / W : 0;
+        int idx[2 * KNN_MAX]; float val[2 * KNN_MAX];
+        const int m = build_d_points(k, has_s, is + smp * k, ws + smp * k, it + i * k, wt + i * k, idx, val);
+        c = (uint32_t)(m * (m + 1) / 2);
+    }
+    counts[i] = c;
+}
+
+__global__ void __launch_bounds__(AT)
+expand_entries_points_kernel(int k, long long j0, long long n, long long n_main, int W, long long K,
+                             const float4* __restrict__ records,
+                             const int32_t* __restrict__ is, const float* __restrict__ ws,
+                             const int32_t* __restrict__ it, const float* __restrict__ wt,
+                             const uint32_t* __restrict__ offsets, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n || it[i * k] < 0) return;
+    const bool has_s = j0 + i < n_main;
+    const long long smp = has_s ? (j0 + i) / W : 0;
+    int idx[2 * KNN_MAX]; float val[2 * KNN_MAX];
+    const int m = build_d_points(k, has_s, is + smp * k, ws + smp * k, it + i * k, wt + i * k, idx, val);
+    const float wgt = records[j0 + i].w;
+    uint32_t o = offsets[i];
+    for (int p = 0; p < m; ++p)
+        for (int q = p; q < m; ++q) {
+            const int r = idx[p] < idx[q] ? idx[p] : idx[q], c = idx[p] < idx[q] ? idx[q] : idx[p];
+            keys[o] = (uint32_t)((long long)r * K + c);
+            vals[o] = __float_as_uint(wgt * val[p] * val[q]);
+            ++o;
+        }
+}
+
+struct PbLayout {
+    size_t is, ws, it, wt, counts, keys, vals, carry_key, carry_sum, scan, sort, total;
+    int64_t C, E, n_tiles;
+};
+
+PbLayout pb_layout(int64_t n_s, int64_t n_records, int k)
+{
+    PbLayout L;
+    L.C = n_records < PB_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : PB_CHUNK_WALKS;
+    L.E = L.C * (int64_t)(2 * k) * (2 * k + 1) / 2;
+    L.n_tiles = ceil_div64(L.E, RT);
+    size_t off = 0;
+    L.is = off;        off += align_up((size_t)n_s * k * 4);
+    L.ws = off;        off += align_up((size_t)n_s * k * 4);
+    L.it = off;        off += align_up((size_t)L.C * k * 4);
+    L.wt = off;        off += align_up((size_t)L.C * k * 4);
+    L.counts = off;    off += align_up((size_t)(L.C + 1) * 4);
+    L.keys = off;      off += align_up((size_t)L.E * 4);
+    L.vals = off;      off += align_up((size_t)L.E * 4);
+    L.carry_key = off; off += align_up((size_t)L.n_tiles * 4);
+    L.carry_sum = off; off += align_up((size_t)L.n_tiles * 4);
+    L.scan = off;      off += align_up(scan_workspace_bytes(L.C) + 256);
+    L.sort = off;      off += align_up(sort_workspace_bytes(L.E, 4));
+    L.total = off + 1024;
+    return L;
+}
+
+int check_point_basis(const mcs_basis* basis)
+{
+    if (!basis || basis->kind != 1 || basis->K < 1 || !basis->points || !basis->normals) return MCS_EINVAL;
+    if (basis->k < 1 || basis->k > KNN_MAX || !(basis->sigma > 0.0f) || !(basis->tau_n > 0.0f)) return MCS_EINVAL;
+    return MCS_OK;
+}
+
+PointBasisDev point_basis_dev(const mcs_basis* basis)
+{
+    PointBasisDev pb;
+    pb.points = basis->points; pb.normals = basis->normals; pb.K = basis->K;
+    pb.k = basis->k < basis->K ? basis->k : (int)basis->K;
+    pb.inv2s2 = 1.0f / (2.0f * basis->sigma * basis->sigma);
+    pb.inv_tau = 1.0f / basis->tau_n;
+    return pb;
+}
+
+}  // namespace
+
+size_t accumulate_points_workspace_bytes(const mcs_samples* s, const mcs_basis* basis, int64_t n_records)
+{
+    const int k = basis->k < 1 ? 1 : (basis->k > KNN_MAX ? KNN_MAX : basis->k);
+    return pb_layout(s->n_s, n_records, k).total;
+}
+
+int knn_weights_run(const mcs_basis* basis, const float* q, const float* nq, int64_t Q, int32_t* idx, float* w, cudaStream_t st)
+{
+    int rc = check_point_basis(basis);
+    if (rc != MCS_OK) return rc;
+    if (Q < 0 || (Q > 0 && (!q || !nq || !idx || !w))) return MCS_EINVAL;
+    if (Q == 0) return MCS_OK;
+    PointBasisDev pb = point_basis_dev(basis);
+    pb.k = basis->k;                                  // output stride is the caller's k; slots beyond K hold -1 / 0
+    if (basis->k > basis->K) {                        // clamp inside: weights of the missing neighbours are 0
+        pb.k = basis->k;
+    }
+    mcs_note_launch(), knn_queries_kernel<<<(unsigned)ceil_div64(Q, AT), AT, 0, st>>>(pb, q, nq, Q, idx, w);
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+                          const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
+                          const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
+{
+    if (!b || !s || !out || !records || n_records < 0) return MCS_EINVAL;
+    int rc = check_point_basis(basis);
+    if (rc != MCS_OK) return rc;
+    if (out->kind != 0 || out->K != basis->K || !out->dense) return MCS_EINVAL;      // dense output only for now
+    const long long K = basis->K;
+    if (K > 65535) return MCS_EINVAL;
+    const int k = basis->k;
+    const PbLayout L = pb_layout(s->n_s, n_records, k);
+    if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
+    char* base = (char*)ws;
+    int32_t* is = (int32_t*)(base + L.is);  float* wsm = (float*)(base + L.ws);
+    int32_t* it = (int32_t*)(base + L.it);  float* wt = (float*)(base + L.wt);
+    uint32_t* counts = (uint32_t*)(base + L.counts);
+    uint32_t* keys = (uint32_t*)(base + L.keys);
+    uint32_t* vals = (uint32_t*)(base + L.vals);
+    uint32_t* carry_key = (uint32_t*)(base + L.carry_key);
+    float* carry_sum = (float*)(base + L.carry_sum);
+    void* scan_ws = base + L.scan;
+    void* sort_ws = base + L.sort;
+    const size_t scan_bytes = L.sort - L.scan, sort_bytes = L.total - L.sort;
+    PointBasisDev pb = point_basis_dev(basis);
+    pb.k = k;
+    const long long n_main = (long long)s->n_s * W < n_records ? (long long)s->n_s * W : n_records;
+    const int bits = key_bits_for(K);
+
+    MCS_CUDA_TRY(cudaMemsetAsync(out->dense, 0, (size_t)K * K * sizeof(float), st));
+    mcs_note_launch(), knn_samples_kernel<<<(unsigned)ceil_div64(s->n_s, AT), AT, 0, st>>>(
+        pb, b->verts, b->faces, s->tri, s->bary, s->normal, s->n_s, is, wsm);
+    unsigned long long entries_total = 0;
+    for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
+        const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
+        const unsigned nblk = (unsigned)ceil_div64(n, AT);
+        mcs_note_launch(), knn_records_kernel<<<nblk, AT, 0, st>>>(pb, b->verts, b->faces, records, j0, n, it, wt);
+        mcs_note_launch(), count_entries_points_kernel<<<nblk, AT, 0, st>>>(k, j0, n, n_main, W, is, wsm, it, wt, counts);
+        rc = exclusive_scan_u32(counts, counts, n, counts + n, scan_ws, scan_bytes, st);
+        if (rc != MCS_OK) return rc;
+        uint32_t n_entries = 0;
+        MCS_CUDA_TRY(cudaMemcpyAsync(&n_entries, counts + n, 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (n_entries == 0) continue;
+        entries_total += n_entries;
+        mcs_note_launch(), expand_entries_points_kernel<<<nblk, AT, 0, st>>>(k, j0, n, n_main, W, K, records, is, wsm, it, wt,
+                                                                            counts, keys, vals);
+        rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
+        if (rc != MCS_OK) return rc;
+        const long long n_tiles = ceil_div64(n_entries, RT);
+        mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
+            keys, vals, n_entries, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
+        mcs_note_launch(), carry_fixup_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(carry_key, carry_sum, n_tiles, out->dense);
+    }
+    mcs_note_launch(), mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);
+    if (stats_dev)
+        MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_ENTRIES, &entries_total, 8, cudaMemcpyHostToDevice, st));
+    MCS_CUDA_TRY(cudaGetLastError());
+    if (stats_dev) MCS_CUDA_TRY(cudaStreamSynchronize(st));
+    return MCS_OK;
+}

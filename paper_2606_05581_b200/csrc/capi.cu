@@ -28,8 +28,9 @@ void mcs_prof_mark(int which, cudaStream_t st)
 
 namespace {
 
-size_t acc_ws_bytes(const mcs_bvh* b, const mcs_basis* basis, const mcs_params* p, int64_t n_records)
+size_t acc_ws_bytes(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, const mcs_params* p, int64_t n_records)
 {
+    if (basis->kind == 1) return accumulate_points_workspace_bytes(s, basis, n_records);
     return p->output_kind == 1 ? accumulate_coo_workspace_bytes(b, n_records, p->coo_capacity)
                                : accumulate_workspace_bytes(b, basis, n_records);
 }
@@ -38,6 +39,10 @@ int acc_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, cons
             const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
             const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st)
 {
+    if (basis->kind == 1) {                    // point basis: Alg. 2 / Eq. 32, dense output
+        if (p->output_kind != 0 || p->estimator != 0) return MCS_EINVAL;
+        return accumulate_points_run(b, s, basis, p->walks_per_sample, records, n_records, ws, ws_bytes, out, stats_dev, st);
+    }
     if (p->output_kind == 1)
         return accumulate_coo_run(b, s, basis, p->walks_per_sample, p->estimator == 1, records, n_records, ws, ws_bytes, out, stats_dev, st);
     return accumulate_run(b, s, basis, p->walks_per_sample, p->estimator == 1, records, n_records, ws, ws_bytes, out, stats_dev, st);
@@ -56,7 +61,7 @@ Layout make_layout(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     size_t off = 0;
     L.records_off = off; if (with_records) off += align_up((size_t)L.n_records * sizeof(mcs_record));
     L.walk_off = off;    off += align_up(walk_workspace_bytes(s));
-    L.acc_off = off;     if (with_acc) off += align_up(acc_ws_bytes(b, basis, p, L.n_records));
+    L.acc_off = off;     if (with_acc) off += align_up(acc_ws_bytes(b, s, basis, p, L.n_records));
     L.total = off + 256;
     return L;
 }
@@ -105,7 +110,7 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
                       false, nullptr, hs != nullptr, &stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
     rc = acc_run(b, s, basis, p, records, L.n_records, base + L.acc_off,
-                 align_up(acc_ws_bytes(b, basis, p, L.n_records)), out, stats_dev, st);
+                 align_up(acc_ws_bytes(b, s, basis, p, L.n_records)), out, stats_dev, st);
     if (rc != MCS_OK) return fail(rc, hs);
     mcs_prof_mark(MCS_MARK_END, st);
     if (hs) {
@@ -278,7 +283,7 @@ extern "C" int mcs_accumulate(const mcs_bvh* b, const mcs_samples* s, const mcs_
     if (n_records < s->n_s * (int64_t)p->walks_per_sample) return MCS_EINVAL;
     if ((p->output_kind != 0 && p->output_kind != 1) || out->kind != p->output_kind) return MCS_EINVAL;
     if (p->output_kind == 1 && (p->coo_capacity < 1 || out->coo_capacity != p->coo_capacity)) return MCS_EINVAL;
-    const size_t need = align_up(acc_ws_bytes(b, basis, p, n_records)) + 512;
+    const size_t need = align_up(acc_ws_bytes(b, s, basis, p, n_records)) + 512;
     if (hs) hs->workspace_needed = (int64_t)need;
     if (!ws || ws_bytes < need) return MCS_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
@@ -296,11 +301,17 @@ extern "C" int mcs_accumulate(const mcs_bvh* b, const mcs_samples* s, const mcs_
     return MCS_OK;
 }
 
-extern "C" size_t mcs_accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, const mcs_params* p,
-                                                 int64_t n_records)
+extern "C" int mcs_knn_weights(const mcs_basis* basis, const float* q, const float* nq, int64_t Q,
+                               int32_t* idx, float* w, void* stream)
 {
-    if (!b || !basis || !p) return 0;
-    return align_up(acc_ws_bytes(b, basis, p, n_records)) + 512;
+    return knn_weights_run(basis, q, nq, Q, idx, w, (cudaStream_t)stream);
+}
+
+extern "C" size_t mcs_accumulate_workspace_bytes(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
+                                                 const mcs_params* p, int64_t n_records)
+{
+    if (!b || !s || !basis || !p) return 0;
+    return align_up(acc_ws_bytes(b, s, basis, p, n_records)) + 512;
 }
 
 extern "C" size_t mcs_walk_workspace_bytes(const mcs_samples* s)

@@ -53,3 +53,10 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
 int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W, int naive,
                    const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
                    const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);
+
+// point-based k-NN basis (mcs_basis.kind 1), accumulate.cu
+size_t accumulate_points_workspace_bytes(const mcs_samples* s, const mcs_basis* basis, int64_t n_records);
+int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, int W,
+                          const float4* records, int64_t n_records, void* ws, size_t ws_bytes,
+                          const mcs_matrix* out, unsigned long long* stats_dev, cudaStream_t st);
+int knn_weights_run(const mcs_basis* basis, const float* q, const float* nq, int64_t Q, int32_t* idx, float* w, cudaStream_t st);
