@@ -52,7 +52,7 @@ def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
             sys.stderr.write(f"--- nvcc {src} ---\n{out}\n")
         failed = failed or p.returncode != 0
     if failed:
-        raise RuntimeError("nvcc failed")
+        raise RuntimeError("nvcc failed: error (see the compiler output above)")
     subprocess.run([_nvcc(), "-shared", "-o", LIB, *objs, "-lcudart"], check=True)
     return LIB
 

@@ -345,6 +345,9 @@ constexpr int CUR_NONE = INT_MIN;
 #ifndef VOTE_TRANS
 #define VOTE_TRANS 20
 #endif
+#ifndef VOTE_AGE
+#define VOTE_AGE 32
+#endif
 
 struct LaneStack {
     int*   s_ref;      // shared: [WSTACK][WT], this lane's column
@@ -369,12 +372,146 @@ __device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, floa
 
 enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 
-template <bool EXT, bool COUNT>
+// ---------------------------------------------------------------------------
+// Warp-cooperative completion of ONE heavy query.  A query that has already visited COOP_MIN nodes
+// (near a medial axis every box is about equally far: hundreds to thousands of nodes) would keep its
+// lane busy for as many passes while the kernel's run time is the longest single-lane chain.  The whole
+// warp takes such a query over: its pending items move to a warp-shared node stack and leaf list, every
+// pass 32 lanes test 32 wide nodes (or 32 triangles), children are pushed with warp-aggregated offsets,
+// and the best hit is a warp arg-min under the tie rule (smaller d2, then smaller face index).  The
+// result is the same minimum the lane would have found; the order of the traversal does not matter.
+// ---------------------------------------------------------------------------
+#ifndef COOP_MIN_NODES
+#define COOP_MIN_NODES 96
+#endif
+constexpr int COOP_MIN = COOP_MIN_NODES;                      // nodes visited by a lane's query before the warp takes it over
+constexpr int COOP_NCAP = 512;                    // warp node stack
+constexpr int COOP_LCAP = 160;                    // warp leaf list (drained at 32; a node pass adds <= 128)
+
+// The hot per-lane variables of the walk kernel are handed over BY VALUE in this struct (a temporary at the
+// call site): passing them by reference to a function that is not inlined would pin them in local memory
+// for the whole kernel.
+struct CoopState {
+    float3 xq;
+    ClosestHit h;
+    float lim;
+    int sp, cur;
+    unsigned n_nodes, n_tris, q_nodes;       // increments (COUNT builds)
+};
+
+template <bool COUNT>
+__device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, const WideNode* __restrict__ wide,
+                                               const PackedTri* __restrict__ tris, int L, float SLACK,
+                                               int* __restrict__ co_nodes, int* __restrict__ co_leaves,
+                                               int* s_ref, float* s_d, int* l_ref, float* l_d, CoopState* stp)
+{
+    (void)nodes_unused;
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    CoopState& S = *stp;
+    const float3 xq_own = S.xq;
+    ClosestHit& h = S.h;
+    float& lim = S.lim;
+    int& sp = S.sp;
+    int& cur = S.cur;
+    unsigned& n_nodes = S.n_nodes;
+    unsigned& n_tris = S.n_tris;
+    unsigned& q_nodes = S.q_nodes;
+    // the query of lane L, known to all lanes
+    const float3 xq = f3(__shfl_sync(FULL, xq_own.x, L), __shfl_sync(FULL, xq_own.y, L), __shfl_sync(FULL, xq_own.z, L));
+    float bd2 = __shfl_sync(FULL, h.d2, L), bv = __shfl_sync(FULL, h.v, L), bw = __shfl_sync(FULL, h.w, L);
+    int btri = __shfl_sync(FULL, h.tri, L), bk = __shfl_sync(FULL, h.k, L);
+    float wlim = __shfl_sync(FULL, lim, L);
+    // lane L moves its pending items to the warp lists
+    int ncount = 0, lcount = 0;
+    if (lane == L) {
+        if (cur != CUR_NONE) { if (cur >= 0) co_nodes[ncount++] = cur; else co_leaves[lcount++] = ~cur; }
+        while (sp > 0) {
+            int ref; float d;
+            --sp;
+            if (sp < WSTACK) { ref = s_ref[sp * WT]; d = s_d[sp * WT]; }
+            else { ref = l_ref[sp - WSTACK]; d = l_d[sp - WSTACK]; }
+            if (d <= lim) { if (ref >= 0) co_nodes[ncount++] = ref; else co_leaves[lcount++] = ~ref; }
+        }
+        cur = CUR_NONE;
+    }
+    ncount = __shfl_sync(FULL, ncount, L); lcount = __shfl_sync(FULL, lcount, L);
+    __syncwarp();
+    unsigned visited = 0;
+    while (ncount > 0 || lcount > 0) {
+        if (lcount >= 32 || ncount == 0) {
+            // ---- leaf pass: 32 triangles, warp arg-min ------------------------------------
+            const int nl = lcount < 32 ? lcount : 32;
+            float d2 = CUDART_INF_F, v = 0.f, w = 0.f; int orig = INT_MAX, kk = -1;
+            if (lane < nl) {
+                kk = co_leaves[lcount - nl + lane];
+                const TriData T = load_tri(tris, kk);
+                d2 = closest_point_triangle(xq, T, CUDART_INF_F, v, w);
+                orig = T.orig;
+                if (COUNT) ++n_tris;
+            }
+            lcount -= nl;
+            float md2 = d2; int morig = orig, mlane = lane;
+            for (int off = 16; off > 0; off >>= 1) {
+                const float od2 = __shfl_xor_sync(FULL, md2, off);
+                const int oorig = __shfl_xor_sync(FULL, morig, off), olane = __shfl_xor_sync(FULL, mlane, off);
+                if (od2 < md2 || (od2 == md2 && oorig < morig)) { md2 = od2; morig = oorig; mlane = olane; }
+            }
+            if (md2 < bd2 || (md2 == bd2 && morig < btri)) {
+                bd2 = md2; btri = morig;
+                bk = __shfl_sync(FULL, kk, mlane); bv = __shfl_sync(FULL, v, mlane); bw = __shfl_sync(FULL, w, mlane);
+                wlim = bd2 * SLACK;
+            }
+            __syncwarp();
+        } else {
+            // ---- node pass: 32 wide nodes, four boxes each -----------------------------------
+            int np = ncount < 32 ? ncount : 32;
+            if (ncount > COOP_NCAP - 128) np = 1;                        // nearly full: depth-first, one node at a time
+            bool in0 = false, in1 = false, in2 = false, in3 = false;
+            int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+            if (lane < np) {
+                const char* wn = reinterpret_cast<const char*>(wide + co_nodes[ncount - np + lane]);
+                const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32), q2 = ldg256(wn + 64), q3 = ldg256(wn + 96);
+                if (COUNT) ++n_nodes;
+                in0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y) <= wlim;
+                in1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w) <= wlim;
+                in2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y) <= wlim;
+                in3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w) <= wlim;
+                c0 = __float_as_int(q3.lo.x); c1 = __float_as_int(q3.lo.y); c2 = __float_as_int(q3.lo.z); c3 = __float_as_int(q3.lo.w);
+            }
+            visited += (unsigned)np;
+            ncount -= np;
+            __syncwarp();                                                // all pops read before any push writes
+#define MCS_COOP_PUSH(inj, cj)                                                                      \
+            {                                                                                       \
+                const unsigned mn_ = __ballot_sync(FULL, inj && cj >= 0), ml_ = __ballot_sync(FULL, inj && cj < 0); \
+                if (inj && cj >= 0) co_nodes[ncount + __popc(mn_ & lt)] = cj;                         \
+                if (inj && cj < 0) co_leaves[lcount + __popc(ml_ & lt)] = ~cj;                        \
+                ncount += __popc(mn_); lcount += __popc(ml_);                                       \
+            }
+            MCS_COOP_PUSH(in0, c0) MCS_COOP_PUSH(in1, c1) MCS_COOP_PUSH(in2, c2) MCS_COOP_PUSH(in3, c3)
+#undef MCS_COOP_PUSH
+            __syncwarp();
+        }
+    }
+    if (lane == L) {
+        h.d2 = bd2; h.tri = btri; h.k = bk; h.v = bv; h.w = bw;
+        lim = wlim;
+        if (COUNT) q_nodes += visited;
+    }
+}
+
+template <bool EXT, bool COUNT, bool COOP>
 __global__ void __launch_bounds__(WT, WALK_MIN_BLOCKS)
 walk_kernel(WalkGeom g, WalkArgs a)
 {
     __shared__ int   sh_ref[WSTACK * WT];
     __shared__ float sh_d[WSTACK * WT];
+    // warp lists of the cooperative path: global scratch (L2-resident, used by monster queries only); shared
+    // memory here would take 10 KB per block away from the L1 that serves every node read
+    int* const co_nodes = a.coop_scratch + ((size_t)blockIdx.x * (WT / 32) + (threadIdx.x >> 5)) * (COOP_NCAP + COOP_LCAP);
+    int* const co_leaves = co_nodes + COOP_NCAP;
     const unsigned FULL = 0xFFFFFFFFu;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -405,7 +542,9 @@ walk_kernel(WalkGeom g, WalkArgs a)
     int cur = CUR_NONE, sp = 0;
     // statistics
     unsigned n_nodes = 0, n_tris = 0, q_nodes = 0;
+    int q_visits = 0;                            // nodes visited by the current query (hand-over to the warp at COOP_MIN)
     unsigned n_steps = 0, n_queries = 0, n_trunc = 0;
+    int age_tri = 0, age_trans = 0;              // warp-uniform: passes since the kind last ran (or was last unwanted)
 
     for (;;) {
         // ---- next item of every lane that has none --------------------------------
@@ -421,16 +560,26 @@ walk_kernel(WalkGeom g, WalkArgs a)
         // Which kind runs this pass: NODE while at least VOTE_NODE lanes want it (one ballot), else TRI when
         // at least VOTE_TRI lanes wait, else TRANS (the long pass: Philox, sincos, record, refill) when at least
         // VOTE_TRANS lanes wait; otherwise the kind most lanes wait for.  Draining one kind lets the others fill.
+        // Aging keeps the wait bounded: a kind that has not run for VOTE_AGE passes runs next if any lane wants it
+        // (a few lanes inside thousand-node queries must not park the rest of the warp).
         const unsigned m_node = __ballot_sync(FULL, kind == KIND_NODE);
         int which = KIND_NODE;
-        if (__popc(m_node) < VOTE_NODE) {
+        ++age_tri; ++age_trans;
+        if (__popc(m_node) < VOTE_NODE || age_tri >= VOTE_AGE || age_trans >= VOTE_AGE) {
             const unsigned m_tri = __ballot_sync(FULL, kind == KIND_TRI), m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
             if ((m_node | m_tri | m_trans) == 0) break;
             const int nn = __popc(m_node), nt = __popc(m_tri), nx = __popc(m_trans);
-            if (nt >= VOTE_TRI) which = KIND_TRI;
+            if (nx > 0 && age_trans >= VOTE_AGE) which = KIND_TRANS;
+            else if (nt > 0 && age_tri >= VOTE_AGE) which = KIND_TRI;
+            else if (nn >= VOTE_NODE) which = KIND_NODE;
+            else if (nt >= VOTE_TRI) which = KIND_TRI;
             else if (nx >= VOTE_TRANS) which = KIND_TRANS;
             else which = (nx > nn && nx > nt) ? KIND_TRANS : (nt > nn ? KIND_TRI : KIND_NODE);
+            if (nt == 0) age_tri = 0;
+            if (nx == 0) age_trans = 0;
         }
+        if (which == KIND_TRI) age_tri = 0;
+        if (which == KIND_TRANS) age_trans = 0;
 
         if (which == KIND_NODE) {
             if (kind == KIND_NODE) {
@@ -439,6 +588,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 const char* wn = reinterpret_cast<const char*>(g.wide + cur);
                 const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32), q2 = ldg256(wn + 64), q3 = ldg256(wn + 96);
                 if (COUNT) { ++n_nodes; ++q_nodes; }
+                if (COOP) ++q_visits;
                 float d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
                 float d1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
                 float d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
@@ -453,6 +603,17 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 if (d2 <= lim) stack_push(stk, sp, c2, d2);
                 if (d1 <= lim) stack_push(stk, sp, c1, d1);
                 cur = d0 <= lim ? c0 : CUR_NONE;
+            }
+            // a lane whose query keeps going hands it to the warp (one query per pass)
+            const unsigned heavy = COOP ? __ballot_sync(FULL, kind == KIND_NODE && q_visits >= COOP_MIN) : 0u;
+            if (COOP && heavy) {
+                const int L = __ffs(heavy) - 1;
+                CoopState cs;
+                cs.xq = xq; cs.h = h; cs.lim = lim; cs.sp = sp; cs.cur = cur; cs.n_nodes = 0; cs.n_tris = 0; cs.q_nodes = 0;
+                coop_finish_query<COUNT>(g.nodes, g.wide, g.tris, L, SLACK, co_nodes, co_leaves,
+                                         stk.s_ref, stk.s_d, stk.l_ref, stk.l_d, &cs);
+                if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; }
+                if (COUNT) { n_nodes += cs.n_nodes; n_tris += cs.n_tris; q_nodes += cs.q_nodes; }
             }
         } else if (which == KIND_TRI) {
             if (kind == KIND_TRI) {
@@ -599,7 +760,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 }
                 h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
                 lim = 3.0e38f;                               // finite: the +inf of an empty node slot never passes
-                sp = 0; cur = CUR_NONE;
+                sp = 0; cur = CUR_NONE; q_visits = 0;
                 if (need_query) {
                     if (prev >= 0) { stack_push(stk, sp, 0, 0.0f); cur = ~prev; }   // last closest face first: a tight bound
                     else cur = 0;                                                   // root
@@ -661,10 +822,13 @@ int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior
     return n;
 }
 
+constexpr int64_t MAX_WALK_BLOCKS = 4096;         // grid cap of the persistent walk kernel (sizes the cooperative scratch)
+
 size_t walk_workspace_bytes(const mcs_samples* s)
 {
     const int64_t n = s->n_s;
-    return align_up((size_t)n * 32)                 // balls
+    return align_up((size_t)MAX_WALK_BLOCKS * (WT / 32) * (COOP_NCAP + COOP_LCAP) * 4)   // cooperative-path warp lists
+         + align_up((size_t)n * 32)                 // balls
          + align_up((size_t)n * 4) * 3              // keys, order, sample_slot
          + align_up(ST_COUNT * 8 + 64)              // counters
          + sort_workspace_bytes(n, 4) + 256;
@@ -680,6 +844,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     if (!ws || ws_bytes < walk_workspace_bytes(s)) return MCS_ENOMEM;
     const int64_t n_s = s->n_s;
     char* ptr = (char*)ws;
+    int* coop_scratch = (int*)ptr;                ptr += align_up((size_t)MAX_WALK_BLOCKS * (WT / 32) * (COOP_NCAP + COOP_LCAP) * 4);
     float4* balls = (float4*)ptr;                 ptr += align_up((size_t)n_s * 32);
     uint32_t* keys = (uint32_t*)ptr;              ptr += align_up((size_t)n_s * 4);
     uint32_t* order = (uint32_t*)ptr;             ptr += align_up((size_t)n_s * 4);
@@ -767,16 +932,25 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         a.escape = exterior ? 3.0e38f : sqrtf(dx * dx + dy * dy + dz * dz);
     }
     a.key0 = (uint32_t)(p->seed & 0xFFFFFFFFu); a.key1 = (uint32_t)(p->seed >> 32);
-    a.records = records; a.steps = steps;
+    a.records = records; a.steps = steps; a.coop_scratch = coop_scratch;
     a.work_counter = stats + ST_WORK; a.stats = stats;
 
     // persistent grid: resident blocks per SM x number of SMs
     int dev = 0, n_sm = 0, per_sm = 0;
     MCS_CUDA_TRY(cudaGetDevice(&dev));
     MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    const void* fn = exterior ? (count ? (const void*)walk_kernel<true, true> : (const void*)walk_kernel<true, false>)
-                              : (count ? (const void*)walk_kernel<false, true> : (const void*)walk_kernel<false, false>);
-    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, WT, 0));
+    // The warp-cooperative completion of heavy queries bounds the longest single-lane chain, which is what the
+    // kernel's run time is when walks are few or queries are long-tailed (large or messy meshes).  On a small
+    // tree with millions of walks (throughput-bound: BASELINE configs 0-1) its code costs registers and nothing
+    // is gained, so it is compiled out there.
+    const long long total_walks = s->n_s * (long long)p->walks_per_sample + ((exterior && p->include_killing) ? p->n_kill_walks : 0);
+    const bool coop = b->F > 20000 || total_walks < (long long)n_sm * 2048 * 16;
+    typedef void (*walk_fn)(WalkGeom, WalkArgs);
+    static const walk_fn table[8] = {
+        walk_kernel<false, false, false>, walk_kernel<false, false, true>, walk_kernel<false, true, false>, walk_kernel<false, true, true>,
+        walk_kernel<true, false, false>,  walk_kernel<true, false, true>,  walk_kernel<true, true, false>,  walk_kernel<true, true, true> };
+    const walk_fn fn = table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)];
+    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
     if (per_sm < 1) per_sm = 1;
     const long long total = a.n_s * a.W + a.n_kill;
     long long grid = (long long)n_sm * per_sm;
@@ -787,15 +961,10 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.chunk = (int)chunk;
     const long long need_blocks = ceil_div64(ceil_div64(total, chunk), WT / 32);
     if (grid > need_blocks) grid = need_blocks;
+    if (grid > MAX_WALK_BLOCKS) grid = MAX_WALK_BLOCKS;
     if (grid < 1) grid = 1;
     mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
-    if (exterior) {
-        if (count) mcs_note_launch(), walk_kernel<true, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
-        else       mcs_note_launch(), walk_kernel<true, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
-    } else {
-        if (count) mcs_note_launch(), walk_kernel<false, true><<<(unsigned)grid, WT, 0, st>>>(g, a);
-        else       mcs_note_launch(), walk_kernel<false, false><<<(unsigned)grid, WT, 0, st>>>(g, a);
-    }
+    mcs_note_launch(), fn<<<(unsigned)grid, WT, 0, st>>>(g, a);
     mcs_prof_mark(MCS_MARK_WALK_END, st);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;

@@ -35,6 +35,7 @@ struct WalkArgs {
     uint32_t key0, key1;
     float4* records;               // mcs_record viewed as float4
     int32_t* steps;
+    int*     coop_scratch;         // [grid][warps][COOP_NCAP + COOP_LCAP] warp lists of the cooperative path
     unsigned long long* work_counter;
     unsigned long long* stats;
 };
