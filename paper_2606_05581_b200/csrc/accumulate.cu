@@ -825,16 +825,83 @@ constexpr int KNN_MAX = 16;
 constexpr int KNN_TILE = 256;
 constexpr int64_t PB_CHUNK_WALKS = (int64_t)1 << 19;
 
+// Uniform grid over the points (used when K > KNN_GRID_MIN): points sorted by cell, start/count per cell.
+struct PointGrid {
+    const uint32_t* cell_start;
+    const uint32_t* cell_count;
+    const uint32_t* sorted_idx;     // point index at sorted position
+    float lox, loy, loz, h, inv_h;
+    int nx, ny, nz;
+};
+
 struct PointBasisDev {
     const float* points;
     const float* normals;
     long long K;
     int k;
     float inv2s2, inv_tau;
+    int use_grid;
+    PointGrid grid;
 };
 
-// Exhaustive k-NN of one query per thread, points staged through shared memory; the k best are kept
-// sorted in registers (static indices only).  Every thread of the block must call this.
+constexpr int KNN_GRID_MIN = 1024;
+
+// Insert candidate (d2, idx) into the sorted list of the KNN_MAX best: order by d2, then by smaller index [Rk2].
+__device__ __forceinline__ void knn_insert(float (&bd)[KNN_MAX], int (&bi)[KNN_MAX], float d2, int idx)
+{
+    if (d2 < bd[KNN_MAX - 1] || (d2 == bd[KNN_MAX - 1] && idx < bi[KNN_MAX - 1])) {
+        bd[KNN_MAX - 1] = d2; bi[KNN_MAX - 1] = idx;
+#pragma unroll
+        for (int m = KNN_MAX - 1; m > 0; --m)
+            if (bd[m] < bd[m - 1] || (bd[m] == bd[m - 1] && bi[m] < bi[m - 1])) {
+                const float td = bd[m]; bd[m] = bd[m - 1]; bd[m - 1] = td;
+                const int ti = bi[m]; bi[m] = bi[m - 1]; bi[m - 1] = ti;
+            }
+    }
+}
+
+// Grid search: rings of cells about the query's cell.  After ring r every point within r*h - off of q has been
+// seen (off = distance from q to its clamped cell), so the search stops when the k-th best is closer than that.
+__device__ __forceinline__ void knn_gather_grid(const PointBasisDev& pb, float3 q, float (&bd)[KNN_MAX], int (&bi)[KNN_MAX])
+{
+    const PointGrid& G = pb.grid;
+    const float fx = (q.x - G.lox) * G.inv_h, fy = (q.y - G.loy) * G.inv_h, fz = (q.z - G.loz) * G.inv_h;
+    const int cx = min(max((int)floorf(fx), 0), G.nx - 1), cy = min(max((int)floorf(fy), 0), G.ny - 1), cz = min(max((int)floorf(fz), 0), G.nz - 1);
+    // distance from q to its (clamped) cell box, 0 when inside
+    const float ox = fmaxf(fmaxf((float)cx - fx, fx - (float)(cx + 1)), 0.0f), oy = fmaxf(fmaxf((float)cy - fy, fy - (float)(cy + 1)), 0.0f),
+                oz = fmaxf(fmaxf((float)cz - fz, fz - (float)(cz + 1)), 0.0f);
+    const float off = sqrtf(ox * ox + oy * oy + oz * oz) * G.h;
+    const int kk = pb.k < pb.K ? pb.k : (int)pb.K;
+    const int rmax = max(G.nx, max(G.ny, G.nz));
+    for (int r = 0; r <= rmax; ++r) {
+        for (int dz = -r; dz <= r; ++dz) {
+            const int z = cz + dz;
+            if (z < 0 || z >= G.nz) continue;
+            for (int dy = -r; dy <= r; ++dy) {
+                const int y = cy + dy;
+                if (y < 0 || y >= G.ny) continue;
+                const bool face = (dz == -r || dz == r || dy == -r || dy == r);
+                for (int dx = -r; dx <= r; dx += (face || r == 0) ? 1 : 2 * r) {     // only the shell of the cube
+                    const int x = cx + dx;
+                    if (x < 0 || x >= G.nx) continue;
+                    const long long c = ((long long)z * G.ny + y) * G.nx + x;
+                    const uint32_t s0 = G.cell_start[c], n = G.cell_count[c];
+                    for (uint32_t j = 0; j < n; ++j) {
+                        const int i = (int)G.sorted_idx[s0 + j];
+                        const float dxp = q.x - pb.points[3 * (long long)i], dyp = q.y - pb.points[3 * (long long)i + 1],
+                                    dzp = q.z - pb.points[3 * (long long)i + 2];
+                        knn_insert(bd, bi, fmaf(dxp, dxp, fmaf(dyp, dyp, dzp * dzp)), i);
+                    }
+                }
+            }
+        }
+        const float reach = fmaxf((float)r * G.h - off, 0.0f);
+        if (bi[kk - 1] >= 0 && bd[kk - 1] < reach * reach) break;
+    }
+}
+
+// k-NN of one query per thread: exhaustive (points staged through shared memory; every thread of the block must
+// call this) or through the grid; the k best are kept sorted in registers (static indices only).
 __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool active, float3 q, float3 nq,
                                                    float4* s_pts, int* idx_out, float* w_out)
 {
@@ -842,25 +909,20 @@ __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool
 #pragma unroll
     for (int j = 0; j < KNN_MAX; ++j) { bd[j] = CUDART_INF_F; bi[j] = -1; }
     const int k = pb.k;
-    for (long long base = 0; base < pb.K; base += KNN_TILE) {
-        const int n = (int)((pb.K - base) < KNN_TILE ? (pb.K - base) : KNN_TILE);
-        __syncthreads();
-        for (int j = threadIdx.x; j < n; j += blockDim.x)
-            s_pts[j] = make_float4(pb.points[3 * (base + j)], pb.points[3 * (base + j) + 1], pb.points[3 * (base + j) + 2], 0.0f);
-        __syncthreads();
-        if (active) {
-            for (int j = 0; j < n; ++j) {
-                const float4 p = s_pts[j];
-                const float dx = q.x - p.x, dy = q.y - p.y, dz = q.z - p.z;
-                const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                if (d2 < bd[KNN_MAX - 1]) {                    // strict: on a tie the smaller index stays in front
-                    bd[KNN_MAX - 1] = d2; bi[KNN_MAX - 1] = (int)(base + j);
-#pragma unroll
-                    for (int m = KNN_MAX - 1; m > 0; --m)
-                        if (bd[m] < bd[m - 1]) {
-                            const float td = bd[m]; bd[m] = bd[m - 1]; bd[m - 1] = td;
-                            const int ti = bi[m]; bi[m] = bi[m - 1]; bi[m - 1] = ti;
-                        }
+    if (pb.use_grid) {
+        if (active) knn_gather_grid(pb, q, bd, bi);
+    } else {
+        for (long long base = 0; base < pb.K; base += KNN_TILE) {
+            const int n = (int)((pb.K - base) < KNN_TILE ? (pb.K - base) : KNN_TILE);
+            __syncthreads();
+            for (int j = threadIdx.x; j < n; j += blockDim.x)
+                s_pts[j] = make_float4(pb.points[3 * (base + j)], pb.points[3 * (base + j) + 1], pb.points[3 * (base + j) + 2], 0.0f);
+            __syncthreads();
+            if (active) {
+                for (int j = 0; j < n; ++j) {
+                    const float4 p = s_pts[j];
+                    const float dx = q.x - p.x, dy = q.y - p.y, dz = q.z - p.z;
+                    knn_insert(bd, bi, fmaf(dx, dx, fmaf(dy, dy, dz * dz)), (int)(base + j));
                 }
             }
         }
@@ -886,6 +948,45 @@ __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool
 #pragma unroll
     for (int j = 0; j < KNN_MAX; ++j)
         if (j < k) { idx_out[j] = bi[j]; w_out[j] = lg[j] * inv; }
+}
+
+// ---- grid build ------------------------------------------------------------
+__device__ __forceinline__ int pg_float_to_ordered(float f) { int i = __float_as_int(f); return i >= 0 ? i : i ^ 0x7FFFFFFF; }
+
+__global__ void __launch_bounds__(AT)
+points_bbox_kernel(const float* __restrict__ pts, long long K, int* __restrict__ out /* lo[3], hi[3] ordered */)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= K) return;
+    for (int d = 0; d < 3; ++d) {
+        const int v = pg_float_to_ordered(pts[3 * i + d]);
+        atomicMin(&out[d], v); atomicMax(&out[3 + d], v);
+    }
+}
+
+__global__ void __launch_bounds__(AT)
+points_cell_kernel(const float* __restrict__ pts, long long K, PointGrid G, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= K) return;
+    const int x = min(max((int)floorf((pts[3 * i] - G.lox) * G.inv_h), 0), G.nx - 1);
+    const int y = min(max((int)floorf((pts[3 * i + 1] - G.loy) * G.inv_h), 0), G.ny - 1);
+    const int z = min(max((int)floorf((pts[3 * i + 2] - G.loz) * G.inv_h), 0), G.nz - 1);
+    keys[i] = (uint32_t)(((long long)z * G.ny + y) * G.nx + x);
+    vals[i] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(AT)
+points_ranges_kernel(const uint32_t* __restrict__ keys, long long K, uint32_t* __restrict__ cell_start, uint32_t* __restrict__ cell_count)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= K) return;
+    const uint32_t c = keys[i];
+    if (i == 0 || keys[i - 1] != c) {
+        long long j = i + 1;
+        while (j < K && keys[j] == c) ++j;            // cells hold a handful of points
+        cell_start[c] = (uint32_t)i; cell_count[c] = (uint32_t)(j - i);
+    }
 }
 
 __global__ void __launch_bounds__(AT)
@@ -1025,11 +1126,62 @@ expand_entries_points_kernel(int k, long long j0, long long n, long long n_main,
 }
 
 struct PbLayout {
-    size_t is, ws, it, wt, counts, keys, vals, carry_key, carry_sum, scan, sort, total;
+    size_t is, ws, it, wt, counts, keys, vals, carry_key, carry_sum, scan, sort, grid, total;
     int64_t C, E, n_tiles;
 };
 
-PbLayout pb_layout(int64_t n_s, int64_t n_records, int k)
+// scratch of the point grid: keys[K] | vals[K] | cell_start[cells] | cell_count[cells] | bbox ints | sort workspace
+int64_t grid_max_cells(int64_t K) { return 16 * K + 64; }
+size_t grid_scratch_bytes(int64_t K)
+{
+    return 2 * align_up((size_t)K * 4) + 2 * align_up((size_t)grid_max_cells(K) * 4) + 256 + align_up(sort_workspace_bytes(K, 4));
+}
+
+// Builds the grid over the points in `scratch` (blocks the host once, to read the bounding box).
+int build_point_grid(const mcs_basis* basis, void* scratch, PointGrid* G, cudaStream_t st)
+{
+    const int64_t K = basis->K;
+    char* p = (char*)scratch;
+    uint32_t* keys = (uint32_t*)p;  p += align_up((size_t)K * 4);
+    uint32_t* vals = (uint32_t*)p;  p += align_up((size_t)K * 4);
+    uint32_t* start = (uint32_t*)p; p += align_up((size_t)grid_max_cells(K) * 4);
+    uint32_t* count = (uint32_t*)p; p += align_up((size_t)grid_max_cells(K) * 4);
+    int* box = (int*)p;             p += 256;
+    void* sort_ws = p;
+    int h[6] = { 0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF, (int)0x80000000, (int)0x80000000, (int)0x80000000 };
+    MCS_CUDA_TRY(cudaMemcpyAsync(box, h, sizeof h, cudaMemcpyHostToDevice, st));
+    mcs_note_launch(), points_bbox_kernel<<<(unsigned)ceil_div64(K, AT), AT, 0, st>>>(basis->points, K, box);
+    MCS_CUDA_TRY(cudaMemcpyAsync(h, box, sizeof h, cudaMemcpyDeviceToHost, st));
+    MCS_CUDA_TRY(cudaStreamSynchronize(st));
+    float lo[3], hi[3];
+    for (int d = 0; d < 6; ++d) { int v = h[d] >= 0 ? h[d] : h[d] ^ 0x7FFFFFFF; memcpy(d < 3 ? &lo[d] : &hi[d - 3], &v, 4); }
+    const float ex = hi[0] - lo[0], ey = hi[1] - lo[1], ez = hi[2] - lo[2];
+    if (!(ex >= 0.0f) || !(ey >= 0.0f) || !(ez >= 0.0f)) return MCS_EDEGENERATE;          // non-finite point
+    const float diag = sqrtf(ex * ex + ey * ey + ez * ez);
+    float cell = diag > 0.0f ? diag / sqrtf((float)K) : 1.0f;                             // ~ one point spacing on a surface
+    int nx, ny, nz;
+    for (;;) {
+        nx = (int)(ex / cell) + 1; ny = (int)(ey / cell) + 1; nz = (int)(ez / cell) + 1;
+        if ((int64_t)nx * ny * nz <= grid_max_cells(K) - 64) break;
+        cell *= 1.25f;
+    }
+    G->cell_start = start; G->cell_count = count; G->sorted_idx = vals;
+    G->lox = lo[0]; G->loy = lo[1]; G->loz = lo[2]; G->h = cell; G->inv_h = 1.0f / cell;
+    G->nx = nx; G->ny = ny; G->nz = nz;
+    const int64_t cells = (int64_t)nx * ny * nz;
+    MCS_CUDA_TRY(cudaMemsetAsync(start, 0, (size_t)cells * 4, st));
+    MCS_CUDA_TRY(cudaMemsetAsync(count, 0, (size_t)cells * 4, st));
+    mcs_note_launch(), points_cell_kernel<<<(unsigned)ceil_div64(K, AT), AT, 0, st>>>(basis->points, K, *G, keys, vals);
+    int bits = 1;
+    while (((int64_t)1 << bits) < cells) ++bits;
+    int rc = sort_pairs_u32(keys, vals, K, bits, sort_ws, sort_workspace_bytes(K, 4), st);
+    if (rc != MCS_OK) return rc;
+    mcs_note_launch(), points_ranges_kernel<<<(unsigned)ceil_div64(K, AT), AT, 0, st>>>(keys, K, start, count);
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+PbLayout pb_layout(int64_t n_s, int64_t n_records, int k, int64_t K)
 {
     PbLayout L;
     L.C = n_records < PB_CHUNK_WALKS ? (n_records < 1 ? 1 : n_records) : PB_CHUNK_WALKS;
@@ -1047,6 +1199,7 @@ PbLayout pb_layout(int64_t n_s, int64_t n_records, int k)
     L.carry_sum = off; off += align_up((size_t)L.n_tiles * 4);
     L.scan = off;      off += align_up(scan_workspace_bytes(L.C) + 256);
     L.sort = off;      off += align_up(sort_workspace_bytes(L.E, 4));
+    L.grid = off;      off += K > KNN_GRID_MIN ? align_up(grid_scratch_bytes(K)) : 0;
     L.total = off + 1024;
     return L;
 }
@@ -1065,6 +1218,8 @@ PointBasisDev point_basis_dev(const mcs_basis* basis)
     pb.k = basis->k < basis->K ? basis->k : (int)basis->K;
     pb.inv2s2 = 1.0f / (2.0f * basis->sigma * basis->sigma);
     pb.inv_tau = 1.0f / basis->tau_n;
+    pb.use_grid = 0;
+    memset(&pb.grid, 0, sizeof pb.grid);
     return pb;
 }
 
@@ -1073,7 +1228,7 @@ PointBasisDev point_basis_dev(const mcs_basis* basis)
 size_t accumulate_points_workspace_bytes(const mcs_samples* s, const mcs_basis* basis, int64_t n_records)
 {
     const int k = basis->k < 1 ? 1 : (basis->k > KNN_MAX ? KNN_MAX : basis->k);
-    return pb_layout(s->n_s, n_records, k).total;
+    return pb_layout(s->n_s, n_records, k, basis->K).total;
 }
 
 int knn_weights_run(const mcs_basis* basis, const float* q, const float* nq, int64_t Q, int32_t* idx, float* w, cudaStream_t st)
@@ -1084,11 +1239,18 @@ int knn_weights_run(const mcs_basis* basis, const float* q, const float* nq, int
     if (Q == 0) return MCS_OK;
     PointBasisDev pb = point_basis_dev(basis);
     pb.k = basis->k;                                  // output stride is the caller's k; slots beyond K hold -1 / 0
-    if (basis->k > basis->K) {                        // clamp inside: weights of the missing neighbours are 0
-        pb.k = basis->k;
+    void* scratch = nullptr;
+    if (basis->K > KNN_GRID_MIN) {                    // test hook: its own scratch for the grid
+        cudaError_t e = cudaMalloc(&scratch, grid_scratch_bytes(basis->K));
+        if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return MCS_ENOMEM; }
+        rc = build_point_grid(basis, scratch, &pb.grid, st);
+        if (rc != MCS_OK) { cudaFree(scratch); return rc; }
+        pb.use_grid = 1;
     }
     mcs_note_launch(), knn_queries_kernel<<<(unsigned)ceil_div64(Q, AT), AT, 0, st>>>(pb, q, nq, Q, idx, w);
-    MCS_CUDA_TRY(cudaGetLastError());
+    cudaError_t e = cudaGetLastError();
+    if (scratch) { cudaStreamSynchronize(st); cudaFree(scratch); }
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return MCS_ECUDA; }
     return MCS_OK;
 }
 
@@ -1103,7 +1265,7 @@ int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basi
     const long long K = basis->K;
     if (K > 65535) return MCS_EINVAL;
     const int k = basis->k;
-    const PbLayout L = pb_layout(s->n_s, n_records, k);
+    const PbLayout L = pb_layout(s->n_s, n_records, k, basis->K);
     if (!ws || ws_bytes < L.total) return MCS_ENOMEM;
     char* base = (char*)ws;
     int32_t* is = (int32_t*)(base + L.is);  float* wsm = (float*)(base + L.ws);
@@ -1118,6 +1280,11 @@ int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basi
     const size_t scan_bytes = L.sort - L.scan, sort_bytes = L.total - L.sort;
     PointBasisDev pb = point_basis_dev(basis);
     pb.k = k;
+    if (basis->K > KNN_GRID_MIN) {
+        rc = build_point_grid(basis, base + L.grid, &pb.grid, st);
+        if (rc != MCS_OK) return rc;
+        pb.use_grid = 1;
+    }
     const long long n_main = (long long)s->n_s * W < n_records ? (long long)s->n_s * W : n_records;
     const int bits = key_bits_for(K);
 

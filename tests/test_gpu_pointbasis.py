@@ -137,3 +137,49 @@ def test_point_basis_stress_mesh_config4_style(api):
     assert np.linalg.norm(Sg - out["S"]) <= np.linalg.norm(np.sqrt(out["var"]))
     with pytest.raises(api.McsError):                                   # sparse output / Alg. 1 not offered for this basis
         api.estimate_dtn_interior(bvh, S, api.Params(walks_per_sample=2, estimator=1, inset=0.01), basis=pb)
+
+
+def test_knn_grid_path_matches_oracle_and_exhaustive(api):
+    """K > 1024: the neighbour search runs through the uniform grid.  Same neighbours and weights as the oracle's
+    exhaustive search on tie-free queries, including queries far outside the points' bounding box."""
+    v, f = merge_meshes([icosphere(4), torus(1.0, 0.3, 80, 40, axis="z", center=(0, 0, 2.5))])[:2]
+    pts, nrm, _ = _points_on(v, f, 5000, seed=5)
+    k, sigma = 8, 0.05
+    rng = np.random.default_rng(7)
+    q = np.concatenate([pts[rng.integers(0, len(pts), 4000)] + rng.normal(scale=0.02, size=(4000, 3)),
+                        rng.uniform(-6, 6, size=(300, 3))]).astype(np.float32)
+    nq = rng.normal(size=(len(q), 3)); nq /= np.linalg.norm(nq, axis=1, keepdims=True)
+    nq = nq.astype(np.float32)
+    idx_o, w_o = Oracle(mesh_geom(v, f)).knn_weights(OrcPointBasis(pts, nrm, k=k, sigma=sigma, tau_n=0.8), q, nq)
+    pb = api.PointBasis.from_arrays(pts, nrm, k=k, sigma=sigma, tau_n=0.8)
+    idx_g, w_g = api.knn_weights(pb, _cuda(q, torch.float32), _cuda(nq, torch.float32))
+    idx_g, w_g = idx_g.cpu().numpy(), w_g.cpu().numpy()
+    d2 = ((q[:, None, :].astype(np.float64) - pts[None].astype(np.float64)) ** 2).sum(2)
+    ds = np.sort(d2, axis=1)[:, :k + 1]
+    keep = (np.diff(ds, axis=1) > 1e-5 * ds[:, 1:]).all(1)
+    assert keep.mean() > 0.9
+    assert np.array_equal(idx_g[keep], idx_o[keep])
+    near = np.arange(len(q)) < 4000
+    assert np.abs(w_g[keep & near] - w_o[keep & near]).max() < 5e-5
+    # queries 100 sigma away: the exponents are ~1e4 and their fp32 rounding shows in the weights
+    assert np.abs(w_g[keep & ~near] - w_o[keep & ~near]).max() < 5e-3
+    assert np.abs(w_g.sum(1) - 1).max() < 1e-5
+
+
+def test_point_basis_matrix_grid_path(api):
+    """The estimator with K = 3000 nodes (grid search inside the accumulation) against the oracle."""
+    v, f = icosphere(4)
+    pts, nrm, _ = _points_on(v, f, 3000, seed=6)
+    smp = vertex_cell_samples(v, f, 1, seed=0)
+    sigma = 0.5 * float(np.sqrt(4 * np.pi / 3000))
+    kw = dict(seed=4, walks_per_sample=16, eps=1e-3)
+    bvh = api.build_bvh(_cuda(v, torch.float32), _cuda(f, torch.int32))
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    pb = api.PointBasis.from_arrays(pts, nrm, k=8, sigma=sigma, tau_n=0.8)
+    A = api.estimate_dtn_interior(bvh, S, api.Params(**kw), basis=pb)
+    assert torch.equal(A, api.estimate_dtn_interior(bvh, S, api.Params(**kw), basis=pb)) and torch.equal(A, A.T)
+    Sg = A.cpu().numpy().astype(np.float64)
+    out = Oracle(mesh_geom(v, f)).estimate_dtn_points(OrcPointBasis(pts, nrm, k=8, sigma=sigma, tau_n=0.8), OracleParams(**kw),
+                                                      False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
+    assert np.linalg.norm(Sg - out["S"]) <= np.linalg.norm(np.sqrt(out["var"]))
+    assert np.abs(Sg.sum(1)).max() < 5e-5 * np.abs(Sg).max()
