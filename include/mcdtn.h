@@ -290,6 +290,18 @@ unsigned long long mcs_launch_count(void);
 int mcs_profile_enable(int on);
 int mcs_profile_last(mcs_phase_times* out /* host */);
 
+/* Smallest Steklov eigenpairs of estimated DtN matrices:
+ *     S psi = lambda M psi,  M = diag(mass)  (lumped boundary mass),
+ * for a batch of `batch` dense symmetric matrices S [batch][K][K] (symmetrised inside) with mass [batch][K] > 0.
+ * evals [batch][n_eig] ascending; evecs [batch][n_eig][K] (may be NULL), M-orthonormal: psi_i^T M psi_j = delta_ij.
+ * One-sided Jacobi in fp32 on M^-1/2 S M^-1/2 (all eigenpairs are computed; the n_eig smallest are returned).
+ * sweeps_out (host, may be NULL): Jacobi sweeps used.  Blocks the host once per sweep (convergence flag).
+ * K <= 16384.  Errors: MCS_EINVAL, MCS_ENOMEM (workspace), MCS_ECUDA. */
+size_t mcs_steklov_eigs_workspace_bytes(int64_t K, int64_t batch);
+int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig,
+                     float* evals, float* evecs, void* workspace, size_t workspace_bytes,
+                     int32_t* sweeps_out /* host */, void* stream);
+
 /* Roofline denominators measured on this device (bench.py): FP32
  * CUDA-core throughput of independent FMA chains (TFLOP/s, 2 flop per FMA) and the read
  * bandwidth of a 24 MiB L2-resident buffer with 16-byte loads (GB/s).  Each allocates a

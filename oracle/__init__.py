@@ -7,8 +7,8 @@ algorithm (restated from PAPER.md) and for the list of pins.
 """
 from .oracle import (Oracle, OracleParams, mesh_geom, sphere_geom, philox4x32_10, u01,
                      closest_point_triangle, closest_point_triangle_alt,
-                     RECORD_DTYPE, steklov_eigs, PointBasis)
+                     RECORD_DTYPE, steklov_eigs, steklov_eigpairs, PointBasis)
 
 __all__ = ["Oracle", "OracleParams", "mesh_geom", "sphere_geom", "philox4x32_10", "u01",
            "closest_point_triangle", "closest_point_triangle_alt", "RECORD_DTYPE",
-           "steklov_eigs", "PointBasis"]
+           "steklov_eigs", "steklov_eigpairs", "PointBasis"]

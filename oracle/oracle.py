@@ -340,3 +340,14 @@ def steklov_eigs(S, M, k):
     Ssym = 0.5 * (S + S.T)
     w = sla.eigh(Ssym, M, eigvals_only=True, subset_by_index=[0, min(k, len(S)) - 1])
     return w
+
+
+def steklov_eigpairs(S, mass, k):
+    """Smallest k eigenpairs of S psi = lambda diag(mass) psi (lumped boundary mass), fp64.
+    Returns (lambda [k] ascending, psi [k][K] with psi_i^T M psi_j = delta_ij).  LAPACK (scipy) serves as the step."""
+    import scipy.linalg as sla
+    S = np.asarray(S, dtype=np.float64)
+    mass = np.asarray(mass, dtype=np.float64)
+    w, V = sla.eigh(0.5 * (S + S.T), np.diag(mass), subset_by_index=[0, min(k, len(S)) - 1])
+    return w, V.T.copy()
+

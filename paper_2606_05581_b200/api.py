@@ -542,3 +542,28 @@ def estimate_dtn_coo(bvh: Bvh, samples: Samples, params: Params, exterior: bool,
         out = CooMatrix(K, row[:n], col[:n], val[:n])
         return (out, st) if want_stats else out
     raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")
+
+
+def steklov_eigs(S, mass, n_eig, want_vectors=True):
+    """Smallest n_eig eigenpairs of S psi = lambda diag(mass) psi (mcs_steklov_eigs).  S: [K,K] or [B,K,K] CUDA fp32;
+    mass: [K] or [B,K].  Returns (evals [B,n_eig] or [n_eig], evecs [B,n_eig,K] or [n_eig,K] or None, sweeps)."""
+    S = _dev(S, torch.float32, "S")
+    mass = _dev(mass, torch.float32, "mass")
+    single = S.ndim == 2
+    if single:
+        S, mass = S[None], mass[None]
+    B, K = int(S.shape[0]), int(S.shape[1])
+    f = lib().mcs_steklov_eigs_workspace_bytes
+    f.restype = C.c_size_t
+    need = int(f(C.c_int64(K), C.c_int64(B)))
+    ws = torch.empty(need, dtype=torch.uint8, device=S.device)
+    evals = torch.empty((B, n_eig), dtype=torch.float32, device=S.device)
+    evecs = torch.empty((B, n_eig, K), dtype=torch.float32, device=S.device) if want_vectors else None
+    sweeps = C.c_int32(0)
+    with torch.cuda.device(S.device):
+        _check(lib().mcs_steklov_eigs(_ptr(S), _ptr(mass), C.c_int64(K), C.c_int64(B), C.c_int32(n_eig), _ptr(evals),
+                                      _ptr(evecs), _ptr(ws), C.c_size_t(need), C.byref(sweeps), _stream(S.device)),
+               "mcs_steklov_eigs")
+    if single:
+        return evals[0], (evecs[0] if evecs is not None else None), sweeps.value
+    return evals, evecs, sweeps.value
