@@ -586,7 +586,8 @@ static int walk_on_spheres(const orc_geom *g, const orc_params *P, uint32_t samp
  * is a valid radius.  Far field (|y| R_max <= 1/2): the ball about 0 of radius
  * 1/R_max is the image of the outside of the bounding sphere, so
  * R* = 1/R_max - |y| needs no query.  Stop when R* < eps; the exit point is
- * the primal closest point.
+ * the primal closest point.  Returns the number of jumps, -1 (truncated, [R10]) or
+ * -3 (the walker is inside the solid that holds the inversion centre, [R10c]).
  */
 static int walk_on_spheres_kelvin(const orc_geom *g, const orc_params *P, uint32_t sample, uint32_t walk,
                                   const double z[3], orc_hit *h)
@@ -602,6 +603,13 @@ static int walk_on_spheres_kelvin(const orc_geom *g, const orc_params *P, uint32
             orc_closest_point(g, x, h);
             Rstar = h->dist / (rho * fmin(P->Rmax_norm, rho + h->dist));
             if (Rstar < P->eps) return k;
+            /* [R10c] The empty ball about x holds the inversion centre (D > |x - o| = rho): x lies in the same
+             * component of space as the centre, i.e. INSIDE the solid.  On a closed, consistently oriented
+             * surface this cannot happen (the segment from x to the centre crosses the surface, so D <= rho);
+             * on an open or mis-oriented one it is the exterior twin of [R10b]: in
+             * Kelvin coordinates such a walker runs off to infinity, doubling |y| every jump.  It contributes
+             * nothing, like a truncated walk. */
+            if (h->dist > rho) return -3;
         }
         if (k == P->max_steps) return -1;
         double w[3];

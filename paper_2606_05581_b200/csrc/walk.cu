@@ -236,7 +236,7 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
             } else {
                 // ---- node pass: which children enter ball_J? ---------------------------
                 int np = ncount < 32 ? ncount : 32;
-                if (ncount > TB_NCAP - 96) np = 1;                        // nearly full: plain depth-first
+                if (ncount > TB_NCAP - 256) np = 1;                       // nearly full: plain depth-first (+1 per level of the binary tree)
                 bool in0 = false, in1 = false;
                 int c0 = 0, c1 = 0;
                 if (lane < np) {
@@ -385,8 +385,13 @@ enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 #define COOP_MIN_NODES 96
 #endif
 constexpr int COOP_MIN = COOP_MIN_NODES;                      // nodes visited by a lane's query before the warp takes it over
-constexpr int COOP_NCAP = 512;                    // warp node stack
-constexpr int COOP_LCAP = 160;                    // warp leaf list (drained at 32; a node pass adds <= 128)
+// Capacities.  Nodes: a 32-node pass runs only while ncount <= COOP_SOFT, so it leaves at most COOP_SOFT - 32 + 128
+// = 480 entries; above COOP_SOFT the warp goes depth-first (one node per pass: net +3 per level of the wide tree,
+// whose depth is at most (63 + log2 F) / 2 < 48), so ncount < 480 + 3 * 48 = 624 < COOP_NCAP.  Leaves: the lane's
+// own stack hands over at most MCS_STACK + 1 = 161 entries; afterwards a node pass starts with < 32 and adds <= 128.
+constexpr int COOP_NCAP = 1024;                   // warp node stack
+constexpr int COOP_SOFT = 384;                    // above this: depth-first
+constexpr int COOP_LCAP = 192;                    // warp leaf list (drained at 32)
 
 // The hot per-lane variables of the walk kernel are handed over BY VALUE in this struct (a temporary at the
 // call site): passing them by reference to a function that is not inlined would pin them in local memory
@@ -461,13 +466,13 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
             if (md2 < bd2 || (md2 == bd2 && morig < btri)) {
                 bd2 = md2; btri = morig;
                 bk = __shfl_sync(FULL, kk, mlane); bv = __shfl_sync(FULL, v, mlane); bw = __shfl_sync(FULL, w, mlane);
-                wlim = bd2 * SLACK;
+                wlim = fminf(bd2 * SLACK, 3.0e38f);
             }
             __syncwarp();
         } else {
             // ---- node pass: 32 wide nodes, four boxes each -----------------------------------
             int np = ncount < 32 ? ncount : 32;
-            if (ncount > COOP_NCAP - 128) np = 1;                        // nearly full: depth-first, one node at a time
+            if (ncount > COOP_SOFT) np = 1;                              // depth-first, one node at a time: bounded growth
             bool in0 = false, in1 = false, in2 = false, in3 = false;
             int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
             if (lane < np) {
@@ -485,9 +490,10 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
             __syncwarp();                                                // all pops read before any push writes
 #define MCS_COOP_PUSH(inj, cj)                                                                      \
             {                                                                                       \
-                const unsigned mn_ = __ballot_sync(FULL, inj && cj >= 0), ml_ = __ballot_sync(FULL, inj && cj < 0); \
+                const bool lf_ = inj && cj < 0 && cj != INT_MIN;               /* INT_MIN marks an empty slot */ \
+                const unsigned mn_ = __ballot_sync(FULL, inj && cj >= 0), ml_ = __ballot_sync(FULL, lf_); \
                 if (inj && cj >= 0) co_nodes[ncount + __popc(mn_ & lt)] = cj;                         \
-                if (inj && cj < 0) co_leaves[lcount + __popc(ml_ & lt)] = ~cj;                        \
+                if (lf_) co_leaves[lcount + __popc(ml_ & lt)] = ~cj;                                  \
                 ncount += __popc(mn_); lcount += __popc(ml_);                                       \
             }
             MCS_COOP_PUSH(in0, c0) MCS_COOP_PUSH(in1, c1) MCS_COOP_PUSH(in2, c2) MCS_COOP_PUSH(in3, c3)
@@ -619,7 +625,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
             if (kind == KIND_TRI) {
                 test_triangle(g.tris, ~cur, xq, h, lim);
                 if (COUNT) ++n_tris;
-                lim = h.d2 * SLACK;
+                lim = fminf(h.d2 * SLACK, 3.0e38f);          // finite: an empty slot (box distance +inf) never passes
                 cur = CUR_NONE;
             }
         } else {
@@ -647,7 +653,9 @@ walk_kernel(WalkGeom g, WalkArgs a)
                         done = true;
                     }
                 }
-                if (!done && !EXT && radius > a.escape) {                // left the bounding box: DESIGN.md R10b
+                // left the bounding box (R10b) / inside the solid that holds the inversion centre: the empty
+                // ball about the query point contains the centre, D > |x - o| = rho (R10c)
+                if (!done && (EXT ? (far_radius < 0.0f && sqrtf(h.d2) > rho) : radius > a.escape)) {
                     a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
                     if (a.steps) a.steps[slot] = -3;
                     ++n_trunc;
@@ -749,7 +757,16 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 bool need_query = true;
                 if (EXT) {
                     const float yn = sqrtf(dot3(x, x));
-                    if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
+                    if (!(yn < 3.0e38f)) {
+                        // Safety net behind R10c: the Kelvin coordinate left fp32.  Every later radius would be
+                        // inf or NaN (a NaN query point is inside every box), so the walk could only run to
+                        // max_steps and be truncated there.  Same outcome now.
+                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
+                        if (a.steps) a.steps[slot] = -1;
+                        ++n_trunc;
+                        busy = false; need_query = false;
+                        far_radius = 0.0f;
+                    } else if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
                         far_radius = 1.0f / a.Rmax - yn;
                         need_query = false;
                     } else {
@@ -822,7 +839,7 @@ int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior
     return n;
 }
 
-constexpr int64_t MAX_WALK_BLOCKS = 4096;         // grid cap of the persistent walk kernel (sizes the cooperative scratch)
+constexpr int64_t MAX_WALK_BLOCKS = 2048;         // grid cap of the persistent walk kernel (sizes the cooperative scratch)
 
 size_t walk_workspace_bytes(const mcs_samples* s)
 {

@@ -303,6 +303,38 @@ def test_stress_mesh_subset_against_oracle(api):
     assert torch.equal(A, api.estimate_dtn_interior(bvh, S, gp)) and torch.equal(A, A.T)
 
 
+def test_exterior_on_a_leaky_mesh_cuts_inside_walkers(api):
+    """Regression + R10c.  A noise-displaced sphere with slivers, duplicates and flipped faces (config 3/4 style):
+    exterior walks that start on the wrong side of a flipped face run inside the solid, where the Kelvin
+    coordinate doubles per jump.  They are cut (-3) as soon as their empty ball holds the inversion centre; no
+    walk overflows, whole-tree queries are completed by the warp (this mesh once broke that path), and sampled
+    walks agree with the oracle walk for walk."""
+    from synth import fps_samples
+    v, f, info = stress_mesh(n_faces=52410, n_components=1, seed=100)
+    smp = fps_samples(v, f, 512, n_candidates=12000, seed=0)
+    origin = tuple(float(x) for x in 0.5 * (v.min(0) + v.max(0)))
+    bvh, S = _setup(api, v, f, smp)
+    W = 256
+    kw = dict(seed=1, walks_per_sample=W, eps=1e-3, max_steps=512, include_killing=True, n_kill_walks=4096)
+    gp = api.Params(kelvin_origin=origin, **kw)
+    rec, steps, st = api.run_walks(bvh, S, gp, True, want_stats=True)
+    rec2, steps2 = api.run_walks(bvh, S, gp, True)
+    assert torch.equal(rec.view(torch.int32), rec2.view(torch.int32)) and torch.equal(steps, steps2)
+    steps = steps.cpu().numpy()
+    assert st.n_truncated == int(((steps == -1) | (steps == -3)).sum())
+    assert (steps == -3).sum() > 0 and (steps == -1).mean() < 1e-3
+    assert st.n_steps < 40 * len(steps)                               # no walker runs for hundreds of doubling jumps
+    ids = np.sort(np.random.default_rng(5).choice(512, 24, replace=False))
+    n_w, n_kill = 4, 16
+    orec = Oracle(mesh_geom(v, f)).run_walks_subset(OracleParams(origin=origin, **kw), True, smp["tri"], smp["bary"],
+                                                     smp["weight"], ids, n_w, n_kill_first=n_kill)
+    slots = np.concatenate([(ids[:, None] * W + np.arange(n_w)[None, :]).ravel(), 512 * W + np.arange(n_kill)])
+    same = steps[slots] == orec["steps"]
+    assert same.mean() >= 0.9, (same.mean(), steps[slots], orec["steps"])
+    A = api.estimate_dtn_coo(bvh, S, gp, exterior=True)
+    assert A.nnz > 0
+
+
 def test_estimator_argument_errors(api):
     v, f = icosphere(1)
     smp = vertex_cell_samples(v, f, 1, seed=0)

@@ -398,6 +398,34 @@ def test_escape_rule_r10b():
     assert (rec["weight"][st == -3] == 0).all() and (rec["tri_t"][st == -3] == -1).all()
 
 
+def test_inside_rule_r10c():
+    """[R10c] exterior twin of R10b: a walker whose empty ball holds the inversion centre (D > |x - o|) is inside
+    the solid: cut (-3).  Closed, outward-oriented mesh: never fires, whatever the centre.  Normals flipped: the
+    tangent ball sits inside the solid; every walk either lands on the surface or is cut, long before max_steps
+    (in Kelvin coordinates an uncut walker would double |y| per jump), and a cut walker was indeed inside."""
+    from synth import icosphere, vertex_cell_samples
+    v, f = icosphere(2)
+    smp = vertex_cell_samples(v, f, 1, seed=0)
+    orc = Oracle(mesh_geom(v, f))
+    for origin in [(0.0, 0.0, 0.0), (0.3, -0.2, 0.4)]:
+        p = OracleParams(seed=1, walks_per_sample=8, eps=1e-3, max_steps=4096, origin=origin, include_killing=True, n_kill_walks=64)
+        rec, _ = orc.run_walks(p, True, smp["tri"], smp["bary"], smp["weight"])
+        assert (rec["steps"] >= 0).all()
+    vv = v[f[smp["tri"]]].astype(np.float64)
+    nrm = np.cross(vv[:, 1] - vv[:, 0], vv[:, 2] - vv[:, 0])
+    nrm /= np.linalg.norm(nrm, axis=1, keepdims=True)
+    p = OracleParams(seed=1, walks_per_sample=8, eps=1e-3, max_steps=4096, origin=(0.3, -0.2, 0.4))
+    rec, _ = orc.run_walks(p, True, smp["tri"], smp["bary"], smp["weight"], normal=-nrm.astype(np.float32))
+    st = rec["steps"]
+    assert (st == -1).sum() == 0 and (st != -2).all()
+    assert 0.005 < (st == -3).mean() < 0.9
+    assert (rec["weight"][st == -3] == 0).all() and (rec["tri_t"][st == -3] == -1).all()
+    # the walks of these samples start inside the unit sphere: Kelvin start z, physical start o + z / |z|^2
+    z = rec["z"][st != -2]
+    x0 = np.asarray(p.origin) + z / (z ** 2).sum(1, keepdims=True)
+    assert (np.linalg.norm(x0, axis=1) < 1.0).all()
+
+
 # --------------------------------------------------------------------------
 # Alg. 1, the naive finite-difference estimator (PAPER.md:161-163, Eq. 13-16)
 # --------------------------------------------------------------------------
