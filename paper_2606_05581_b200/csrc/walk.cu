@@ -382,8 +382,12 @@ enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 // result is the same minimum the lane would have found; the order of the traversal does not matter.
 // ---------------------------------------------------------------------------
 #ifndef COOP_MIN_NODES
-#define COOP_MIN_NODES 96
+#define COOP_MIN_NODES 24
 #endif
+#ifndef COOP_MIN_MERGED_NODES
+#define COOP_MIN_MERGED_NODES 8
+#endif
+constexpr int COOP_MIN_MERGED = COOP_MIN_MERGED_NODES;     // the same in the merged-pass variant (small jobs: idle lanes are free)
 constexpr int COOP_MIN = COOP_MIN_NODES;                      // nodes visited by a lane's query before the warp takes it over
 // Capacities.  Nodes: a 32-node pass runs only while ncount <= COOP_SOFT, so it leaves at most COOP_SOFT - 32 + 128
 // = 480 entries; above COOP_SOFT the warp goes depth-first (one node per pass: net +3 per level of the wide tree,
@@ -508,8 +512,13 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
     }
 }
 
-template <bool EXT, bool COUNT, bool COOP>
-__global__ void __launch_bounds__(WT, WALK_MIN_BLOCKS)
+// MERGED (small jobs: a few walks per lane, so nearly the whole run is the tail where a warp holds a handful of
+// live walkers in different phases and the cost is the number of passes, each one memory round trip): a pass
+// serves the lanes that wait for a node AND the lanes that wait for a triangle -- both loads are issued before
+// either is used -- and then the lanes that wait for a transition, instead of one kind per pass: every live lane
+// advances every pass.  The arithmetic of a visit is unchanged.
+template <bool EXT, bool COUNT, bool COOP, bool MERGED>
+__global__ void __launch_bounds__(WT, MERGED ? 4 : WALK_MIN_BLOCKS)      // small jobs: registers instead of occupancy
 walk_kernel(WalkGeom g, WalkArgs a)
 {
     __shared__ int   sh_ref[WSTACK * WT];
@@ -568,10 +577,16 @@ walk_kernel(WalkGeom g, WalkArgs a)
         // VOTE_TRANS lanes wait; otherwise the kind most lanes wait for.  Draining one kind lets the others fill.
         // Aging keeps the wait bounded: a kind that has not run for VOTE_AGE passes runs next if any lane wants it
         // (a few lanes inside thousand-node queries must not park the rest of the warp).
-        const unsigned m_node = __ballot_sync(FULL, kind == KIND_NODE);
+        const unsigned m_node = __ballot_sync(FULL, MERGED ? (kind == KIND_NODE || kind == KIND_TRI) : kind == KIND_NODE);
         int which = KIND_NODE;
         ++age_tri; ++age_trans;
-        if (__popc(m_node) < VOTE_NODE || age_tri >= VOTE_AGE || age_trans >= VOTE_AGE) {
+        bool run_trav, run_trans;
+        if (MERGED) {
+            // every lane advances every pass: traversal items first, then the transitions
+            const unsigned m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
+            if ((m_node | m_trans) == 0) break;
+            run_trav = m_node != 0; run_trans = m_trans != 0;
+        } else if (__popc(m_node) < VOTE_NODE || age_tri >= VOTE_AGE || age_trans >= VOTE_AGE) {
             const unsigned m_tri = __ballot_sync(FULL, kind == KIND_TRI), m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
             if ((m_node | m_tri | m_trans) == 0) break;
             const int nn = __popc(m_node), nt = __popc(m_tri), nx = __popc(m_trans);
@@ -586,13 +601,26 @@ walk_kernel(WalkGeom g, WalkArgs a)
         }
         if (which == KIND_TRI) age_tri = 0;
         if (which == KIND_TRANS) age_trans = 0;
+        if (!MERGED) { run_trav = which == KIND_NODE; run_trans = which == KIND_TRANS; }
 
-        if (which == KIND_NODE) {
-            if (kind == KIND_NODE) {
+        if (run_trav) {
+            const bool tri_lane = MERGED && kind == KIND_TRI;
+            if (kind == KIND_NODE || tri_lane) {
                 // 4-wide node: four box tests, the children that survive sorted by distance; the nearest
                 // is visited next, the others go on the stack farthest first
-                const char* wn = reinterpret_cast<const char*>(g.wide + cur);
-                const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32), q2 = ldg256(wn + 64), q3 = ldg256(wn + 96);
+                const char* wn = tri_lane ? reinterpret_cast<const char*>(g.tris + ~cur) : reinterpret_cast<const char*>(g.wide + cur);
+                const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32);
+                Vec8 q2 = q0, q3 = q0;
+                if (!tri_lane) { q2 = ldg256(wn + 64); q3 = ldg256(wn + 96); }
+              if (tri_lane) {
+                const TriData T = unpack_tri(q0.lo, q0.hi, q1.lo, q1.hi);
+                float tv = 0.0f, tw = 0.0f;
+                const float td2 = closest_point_triangle(xq, T, CUDART_INF_F, tv, tw);
+                if (td2 < h.d2 || (td2 == h.d2 && T.orig < h.tri)) { h.d2 = td2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
+                if (COUNT) ++n_tris;
+                lim = fminf(h.d2 * SLACK, 3.0e38f);
+                cur = CUR_NONE;
+              } else {
                 if (COUNT) { ++n_nodes; ++q_nodes; }
                 if (COOP) ++q_visits;
                 float d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
@@ -609,9 +637,10 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 if (d2 <= lim) stack_push(stk, sp, c2, d2);
                 if (d1 <= lim) stack_push(stk, sp, c1, d1);
                 cur = d0 <= lim ? c0 : CUR_NONE;
+              }
             }
             // a lane whose query keeps going hands it to the warp (one query per pass)
-            const unsigned heavy = COOP ? __ballot_sync(FULL, kind == KIND_NODE && q_visits >= COOP_MIN) : 0u;
+            const unsigned heavy = COOP ? __ballot_sync(FULL, kind == KIND_NODE && q_visits >= (MERGED ? COOP_MIN_MERGED : COOP_MIN)) : 0u;
             if (COOP && heavy) {
                 const int L = __ffs(heavy) - 1;
                 CoopState cs;
@@ -621,14 +650,16 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; }
                 if (COUNT) { n_nodes += cs.n_nodes; n_tris += cs.n_tris; q_nodes += cs.q_nodes; }
             }
-        } else if (which == KIND_TRI) {
+        }
+        if (!MERGED && which == KIND_TRI) {
             if (kind == KIND_TRI) {
                 test_triangle(g.tris, ~cur, xq, h, lim);
                 if (COUNT) ++n_tris;
                 lim = fminf(h.d2 * SLACK, 3.0e38f);          // finite: an empty slot (box distance +inf) never passes
                 cur = CUR_NONE;
             }
-        } else {
+        }
+        if (run_trans) {
             // ---- (1) finished queries: terminate or jump (R9) ----
             bool start_query = false;
             if (busy && kind == KIND_TRANS) {
@@ -962,11 +993,15 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     // is gained, so it is compiled out there.
     const long long total_walks = s->n_s * (long long)p->walks_per_sample + ((exterior && p->include_killing) ? p->n_kill_walks : 0);
     const bool coop = b->F > 20000 || total_walks < (long long)n_sm * 2048 * 16;
+    // Small jobs (a few walks per lane) run the merged-pass variant, always with the cooperative path.
+    const bool merged = total_walks < (long long)n_sm * 2048 * 4;
     typedef void (*walk_fn)(WalkGeom, WalkArgs);
-    static const walk_fn table[8] = {
-        walk_kernel<false, false, false>, walk_kernel<false, false, true>, walk_kernel<false, true, false>, walk_kernel<false, true, true>,
-        walk_kernel<true, false, false>,  walk_kernel<true, false, true>,  walk_kernel<true, true, false>,  walk_kernel<true, true, true> };
-    const walk_fn fn = table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)];
+    static const walk_fn table[12] = {
+        walk_kernel<false, false, false, false>, walk_kernel<false, false, true, false>, walk_kernel<false, true, false, false>, walk_kernel<false, true, true, false>,
+        walk_kernel<true, false, false, false>,  walk_kernel<true, false, true, false>,  walk_kernel<true, true, false, false>,  walk_kernel<true, true, true, false>,
+        walk_kernel<false, false, true, true>,   walk_kernel<false, true, true, true>,   walk_kernel<true, false, true, true>,   walk_kernel<true, true, true, true> };
+    const walk_fn fn = merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)]
+                              : table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)];
     MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
     if (per_sm < 1) per_sm = 1;
     const long long total = a.n_s * a.W + a.n_kill;
