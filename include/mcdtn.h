@@ -62,6 +62,10 @@ typedef struct {
  * Build.  verts [V][3] fp32 and faces [F][3] int32 are read on `stream`; the
  * handle keeps its own copies, so the caller may free them after the call.
  * Blocks the host until the build has finished (it reads back error flags).
+ * The handle's device memory comes from the device's stream-ordered pool
+ * (cudaMallocAsync on `stream`; the pool's release threshold is raised so that
+ * build/free cycles reuse memory).  mcs_free_bvh returns it in the order of the
+ * legacy default stream, i.e. after all work submitted so far; it does not block.
  * Errors: MCS_EINVAL (null pointer, V < 1, F < 1, face index outside [0,V)),
  * MCS_EDEGENERATE (non-finite vertex, zero total area), MCS_ENOMEM, MCS_ECUDA.
  */
