@@ -280,6 +280,26 @@ class Oracle:
                                     S2.ctypes.data_as(C.c_void_p) if want_var else None)
         return (S, S2) if want_var else S
 
+    def winding_number(self, p, exclude=None):
+        """Generalised winding number of the mesh at points p [n,3]; exclude [n]: face left out (-1: none)."""
+        p = np.ascontiguousarray(p, np.float64).reshape(-1, 3)
+        w = np.empty(len(p))
+        ex = None if exclude is None else np.ascontiguousarray(exclude, np.int64)
+        self.lib.orc_winding_number(C.byref(self.geom.c), p.ctypes.data_as(C.c_void_p), C.c_int64(len(p)),
+                                    ex.ctypes.data_as(C.c_void_p) if ex is not None else None, w.ctypes.data_as(C.c_void_p))
+        return w
+
+    def orient_samples(self, tri, bary, h_scale=1.0):
+        """(outward normal [n,3], d [n]) of boundary samples by the winding-number rule G-R1."""
+        tri = np.ascontiguousarray(tri, np.int32)
+        bary = np.ascontiguousarray(bary, np.float32)
+        nrm = np.empty((len(tri), 3))
+        d = np.empty(len(tri))
+        self.lib.orc_orient_samples(C.byref(self.geom.c), tri.ctypes.data_as(C.c_void_p), bary.ctypes.data_as(C.c_void_p),
+                                    C.c_int64(len(tri)), C.c_double(h_scale), nrm.ctypes.data_as(C.c_void_p),
+                                    d.ctypes.data_as(C.c_void_p))
+        return nrm, d
+
     def knn_weights(self, basis: "PointBasis", q, nq):
         """(idx [n,k], w [n,k]) of the k-NN bilateral interpolator at points q with normals nq (Eq. 44-45)."""
         pb = basis.c()
