@@ -294,6 +294,24 @@ unsigned long long mcs_launch_count(void);
 int mcs_profile_enable(int on);
 int mcs_profile_last(mcs_phase_times* out /* host */);
 
+/* Generalised winding number of the mesh (Jacobson et al. 2013):
+ *     w(p) = (1 / 4 pi) sum_f Omega_f(p),  Omega_f = signed solid angle of face f seen from p (Van Oosterom-Strackee),
+ * 1 inside a closed surface wound counter-clockwise seen from outside, 0 outside.  Exhaustive over all faces.
+ * points [n][3] device fp32; exclude [n] device int32 or NULL: original index of a face left out for that point
+ * (-1: none); w_out [n] device.  workspace >= mcs_winding_workspace_bytes(bvh, n).  Asynchronous on `stream`.
+ *
+ * mcs_orient_samples: sidedness of boundary samples by rule G-R1 of DESIGN.md.  For sample i on face f with face
+ * normal n_f (winding order) and h = h_scale * sqrt(area_f):  d_i = w_-f(s - h n_f) - w_-f(s + h n_f), w_-f = the
+ * winding number without face f.  d > 0: n_f points out of the solid.  normal_out [n_s][3] device = sign(d) n_f,
+ * usable as mcs_samples.normal; d_out [n_s] device or NULL.  samples->weight and ->normal are not read.
+ * workspace >= mcs_winding_workspace_bytes(bvh, n_s).  Blocks the host (it reads back an error flag).
+ * Errors: MCS_EINVAL (null pointer, n < 1, h_scale <= 0, sample face out of range), MCS_ENOMEM, MCS_ECUDA. */
+size_t mcs_winding_workspace_bytes(const mcs_bvh* bvh, int64_t n);
+int mcs_winding_number(const mcs_bvh* bvh, const float* points, const int32_t* exclude /* may be NULL */, int64_t n,
+                       float* w_out, void* workspace, size_t workspace_bytes, void* stream);
+int mcs_orient_samples(const mcs_bvh* bvh, const mcs_samples* samples, float h_scale, float* normal_out,
+                       float* d_out /* may be NULL */, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Smallest Steklov eigenpairs of estimated DtN matrices:
  *     S psi = lambda M psi,  M = diag(mass)  (lumped boundary mass),
  * for a batch of `batch` dense symmetric matrices S [batch][K][K] (symmetrised inside) with mass [batch][K] > 0.

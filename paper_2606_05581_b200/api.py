@@ -567,3 +567,38 @@ def steklov_eigs(S, mass, n_eig, want_vectors=True):
     if single:
         return evals[0], (evecs[0] if evecs is not None else None), sweeps.value
     return evals, evecs, sweeps.value
+
+
+def _winding_ws(bvh, n, device):
+    f = lib().mcs_winding_workspace_bytes
+    f.restype = C.c_size_t
+    need = int(f(bvh.handle, C.c_int64(n)))
+    return torch.empty(need, dtype=torch.uint8, device=device), need
+
+
+def winding_number(bvh, points, exclude=None):
+    """Generalised winding number of the mesh at points [n,3] (mcs_winding_number); exclude [n] int32: face left out."""
+    points = _dev(points, torch.float32, "points").reshape(-1, 3)
+    n = int(points.shape[0])
+    ex = _dev(exclude, torch.int32, "exclude") if exclude is not None else None
+    w = torch.empty(n, dtype=torch.float32, device=points.device)
+    with torch.cuda.device(points.device):
+        ws, need = _winding_ws(bvh, n, points.device)
+        _check(lib().mcs_winding_number(bvh.handle, _ptr(points), _ptr(ex), C.c_int64(n), _ptr(w), _ptr(ws),
+                                        C.c_size_t(need), _stream(points.device)), "mcs_winding_number")
+    return w
+
+
+def orient_samples(bvh, samples, h_scale=1.0):
+    """(normal [n_s,3] pointing out of the solid, d [n_s]) by the winding-number rule G-R1 (mcs_orient_samples).
+    Pass the normals back as Samples(..., normal=...) to draw the tangent balls on the right side of flipped faces."""
+    dev = samples.tri.device
+    n = int(samples.tri.shape[0])
+    nrm = torch.empty((n, 3), dtype=torch.float32, device=dev)
+    d = torch.empty(n, dtype=torch.float32, device=dev)
+    cs = samples.c()
+    with torch.cuda.device(dev):
+        ws, need = _winding_ws(bvh, n, dev)
+        _check(lib().mcs_orient_samples(bvh.handle, C.byref(cs), C.c_float(h_scale), _ptr(nrm), _ptr(d), _ptr(ws),
+                                        C.c_size_t(need), _stream(dev)), "mcs_orient_samples")
+    return nrm, d

@@ -1,0 +1,96 @@
+"""GPU parity of mcs_winding_number / mcs_orient_samples (DESIGN.md G-R1)
+against the oracle's fp64 brute force: values to fp32 accuracy of a sum of F solid angles, the excluded face,
+bit-identical reruns, sizes that span several tiles, chunks and a ragged tail, and the sidedness decision equal
+wherever the oracle's margin |d| is above the fp32 error."""
+import time
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import Oracle, mesh_geom                                            # noqa: E402
+from synth import fps_samples, icosphere, merge_meshes, stress_mesh, torus      # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    from paper_2606_05581_b200 import api as _api
+    _api.lib()
+    return _api
+
+
+def _bvh(api, v, f):
+    return api.build_bvh(torch.from_numpy(np.ascontiguousarray(v, np.float32)).cuda(), torch.from_numpy(np.ascontiguousarray(f, np.int32)).cuda())
+
+
+@pytest.mark.parametrize("n", [1, 127, 129, 1000])
+def test_winding_number_matches_oracle(api, n):
+    v, f = merge_meshes([icosphere(3), torus(1.0, 0.3, 37, 19, axis="z", center=(0, 0, 2.5))])[:2]      # 1280 + 1406 faces: ragged
+    rng = np.random.default_rng(n)
+    p = rng.uniform(-2, 4, size=(n, 3)).astype(np.float32)
+    ex = rng.integers(-1, len(f), n).astype(np.int32)
+    orc = Oracle(mesh_geom(v, f))
+    bvh = _bvh(api, v, f)
+    for excl in (None, ex):
+        w = api.winding_number(bvh, torch.from_numpy(p).cuda(), None if excl is None else torch.from_numpy(excl).cuda())
+        w2 = api.winding_number(bvh, torch.from_numpy(p).cuda(), None if excl is None else torch.from_numpy(excl).cuda())
+        assert torch.equal(w, w2)
+        wo = orc.winding_number(p.astype(np.float64), excl)
+        assert np.abs(w.cpu().numpy() - wo).max() < 2e-5
+
+
+def test_closed_surface_values_and_many_chunks(api):
+    """Few points, many faces: the faces are split over chunks (grid.y > 1).  1 inside, 0 outside, 2 in a nested solid."""
+    v, f = merge_meshes([icosphere(5), icosphere(3, radius=0.4)])[:2]            # 20480 + 1280 faces
+    bvh = _bvh(api, v, f)
+    p = torch.tensor([[0.0, 0, 0], [0.7, 0, 0], [0, 1.5, 0], [0.2, -0.1, 0.25]], device="cuda")
+    w = api.winding_number(bvh, p).cpu().numpy()
+    assert np.abs(w - [2, 1, 0, 2]).max() < 2e-5
+
+
+def test_orient_samples_on_a_stress_mesh(api):
+    """Config-3/4 style mesh with flipped faces: the GPU takes the oracle's decision wherever the oracle's margin is
+    above fp32 noise, d agrees, and feeding the normals back to the estimator discards fewer samples."""
+    v, f, info = stress_mesh(n_faces=12000, n_components=5, seed=11)
+    smp = fps_samples(v, f, 600, n_candidates=8000, seed=2)
+    bvh = _bvh(api, v, f)
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    nrm, d = api.orient_samples(bvh, S, h_scale=1.0)
+    nrm2, d2 = api.orient_samples(bvh, S, h_scale=1.0)
+    assert torch.equal(nrm, nrm2) and torch.equal(d, d2)
+    no, do = Oracle(mesh_geom(v, f)).orient_samples(smp["tri"], smp["bary"], h_scale=1.0)
+    d, nrm = d.cpu().numpy(), nrm.cpu().numpy()
+    assert np.abs(d - do).max() < 1e-4
+    sure = np.abs(do) > 1e-3
+    assert sure.mean() > 0.95
+    assert np.abs(nrm[sure] - no[sure]).max() < 1e-5
+    flipped = info["flipped"][smp["tri"]] if "flipped" in info else None
+    if flipped is not None:
+        # most samples on reversed faces are found (overlapping components make the rest ambiguous by construction)
+        assert ((do < 0) == flipped)[sure].mean() > 0.9
+    with pytest.raises(api.McsError):
+        api.orient_samples(bvh, S, h_scale=0.0)
+
+
+def test_sidedness_on_sphere_with_flipped_faces_and_timing(api):
+    rng = np.random.default_rng(3)
+    v, f = icosphere(5)
+    flip = rng.random(len(f)) < 0.1
+    f2 = f.copy(); f2[flip] = f2[flip][:, ::-1]
+    bvh = _bvh(api, v, f2)
+    n = 20000
+    tri = rng.integers(0, len(f), n).astype(np.int32)
+    bary = rng.dirichlet([1, 1, 1], n).astype(np.float32)
+    S = api.Samples.from_arrays(tri, bary, np.ones(n, np.float32))
+    torch.cuda.synchronize(); t = time.time()
+    nrm, d = api.orient_samples(bvh, S)
+    torch.cuda.synchronize(); dt = time.time() - t
+    s = np.einsum("qk,qkd->qd", bary.astype(np.float64), v[f2[tri]].astype(np.float64))
+    assert (np.einsum("qd,qd->q", nrm.cpu().numpy().astype(np.float64), s) > 0).all()
+    assert ((d.cpu().numpy() > 0) == ~flip[tri]).all()
+    print(f"orient_samples: {2 * n} probes x {len(f)} faces in {dt * 1e3:.1f} ms = {2 * n * len(f) / dt / 1e9:.1f} G pairs/s")
