@@ -53,17 +53,27 @@ radix_hist_kernel(const K* __restrict__ keys, int64_t n, int shift, uint32_t* __
     if (threadIdx.x < 256) counts[(size_t)threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
 }
 
+// Stable scatter of one tile.  The keys of a tile are first put in digit order in shared memory (their stable
+// local rank is known), then written out: consecutive threads write consecutive addresses of one digit's run, so
+// the global writes are coalesced (a direct scatter writes 4-8 bytes into 32 different sectors per warp).
 template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS)
 radix_scatter_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin,
                      K* __restrict__ kout, uint32_t* __restrict__ vout,
                      int64_t n, int shift, const uint32_t* __restrict__ offsets, int nblocks)
 {
-    __shared__ uint32_t cnt[SORT_WARPS][256];
+    extern __shared__ __align__(16) unsigned char sort_smem[];
+    K* skey = reinterpret_cast<K*>(sort_smem);                                   // [SORT_TILE]
+    uint32_t* sval = reinterpret_cast<uint32_t*>(skey + SORT_TILE);              // [SORT_TILE]
+    uint32_t (*cnt)[256] = reinterpret_cast<uint32_t (*)[256]>(sval + SORT_TILE); // [SORT_WARPS][256]
+    uint32_t* lstart = &cnt[0][0] + SORT_WARPS * 256;                            // [256] first local slot of a digit
+    uint32_t* gbase = lstart + 256;                                              // [256] first global slot of a digit (this tile)
+    uint32_t* wsum = gbase + 256;                                                // [8]
     for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t warp_base = (int64_t)blockIdx.x * SORT_TILE + (int64_t)warp * 32 * SORT_ITEMS;
+    const int64_t block_base = (int64_t)blockIdx.x * SORT_TILE;
+    const int64_t warp_base = block_base + (int64_t)warp * 32 * SORT_ITEMS;
     K key[SORT_ITEMS];
     uint32_t rank[SORT_ITEMS];
 #pragma unroll
@@ -81,10 +91,22 @@ radix_scatter_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin
         __syncwarp();
     }
     __syncthreads();
+    // per digit: counts of the warps -> exclusive offsets inside the digit; digit totals -> exclusive scan over digits
+    uint32_t total = 0;
     if (threadIdx.x < 256) {
-        uint32_t run = offsets[(size_t)threadIdx.x * nblocks + blockIdx.x];
 #pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w) { uint32_t c = cnt[w][threadIdx.x]; cnt[w][threadIdx.x] = run; run += c; }
+        for (int w = 0; w < SORT_WARPS; ++w) { uint32_t c = cnt[w][threadIdx.x]; cnt[w][threadIdx.x] = total; total += c; }
+        gbase[threadIdx.x] = offsets[(size_t)threadIdx.x * nblocks + blockIdx.x];
+    }
+    uint32_t inc = total;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o); if (lane >= o) inc += t; }
+    if (threadIdx.x < 256 && lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (threadIdx.x < 256) {
+        uint32_t before = 0;
+        for (int w = 0; w < warp; ++w) before += wsum[w];
+        lstart[threadIdx.x] = before + inc - total;
     }
     __syncthreads();
 #pragma unroll
@@ -92,12 +114,25 @@ radix_scatter_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin
         int64_t pos = warp_base + r * 32 + lane;
         if (pos < n) {
             unsigned d = (unsigned)((key[r] >> shift) & 0xFF);
-            uint32_t dst = cnt[warp][d] + rank[r];
-            kout[dst] = key[r];
-            vout[dst] = vin[pos];
+            uint32_t lp = lstart[d] + cnt[warp][d] + rank[r];
+            skey[lp] = key[r];
+            sval[lp] = vin[pos];
         }
     }
+    __syncthreads();
+    const int64_t left = n - block_base;
+    const int count = (int)(left < SORT_TILE ? left : SORT_TILE);
+    for (int j = threadIdx.x; j < count; j += SORT_THREADS) {
+        const K k = skey[j];
+        const unsigned d = (unsigned)((k >> shift) & 0xFF);
+        const uint32_t dst = gbase[d] + ((uint32_t)j - lstart[d]);
+        kout[dst] = k;
+        vout[dst] = sval[j];
+    }
 }
+
+template <typename K>
+constexpr size_t scatter_smem_bytes() { return (size_t)SORT_TILE * (sizeof(K) + 4) + (size_t)SORT_WARPS * 256 * 4 + 2 * 256 * 4 + 64; }
 
 // ------------------------------ scan ---------------------------------------
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
@@ -163,12 +198,19 @@ int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, 
     size_t scan_ws_bytes = ws_bytes - (size_t)(p - (char*)ws);
     K* kin = keys; uint32_t* vin = vals; K* kout = kalt; uint32_t* vout = valt;
     const int passes = (key_bits + 7) / 8;
+    {
+        static bool attr_set = false;                       // per instantiation (K)
+        if (!attr_set) {
+            MCS_CUDA_TRY(cudaFuncSetAttribute(radix_scatter_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)scatter_smem_bytes<K>()));
+            attr_set = true;
+        }
+    }
     for (int pass = 0; pass < passes; ++pass) {
         int shift = pass * 8;
         mcs_note_launch(), radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks);
         int rc = exclusive_scan_u32(counts, counts, (int64_t)256 * nblocks, nullptr, scan_ws, scan_ws_bytes, st);
         if (rc != MCS_OK) return rc;
-        mcs_note_launch(), radix_scatter_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
+        mcs_note_launch(), radix_scatter_kernel<K><<<nblocks, SORT_THREADS, scatter_smem_bytes<K>(), st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
         K* tk = kin; kin = kout; kout = tk;
         uint32_t* tv = vin; vin = vout; vout = tv;
     }
