@@ -280,6 +280,22 @@ class Oracle:
                                     S2.ctypes.data_as(C.c_void_p) if want_var else None)
         return (S, S2) if want_var else S
 
+    def accumulate_reduced(self, rec, tri, bary, Phi):
+        """Reduced Ritz-Galerkin DtN matrix: basis functions phi_k = sum_v Phi[v,k] hat_v,
+        so b(p) = Phi^T iota(p) with iota(p) the hat-basis vector of p (3 non-zeros), and every walk adds
+        weight * d d^T with d = b(s) - b(t) (Alg. 2; killing walks add weight * b(t) b(t)^T, Eq. 32).
+        Written as the deferred batched outer product D^T diag(w) D over all records.  Phi: [V, K] fp64."""
+        Phi = np.asarray(Phi, np.float64)
+        faces = np.ctypeslib.as_array(C.cast(self.geom.c.faces, C.POINTER(C.c_int32)), shape=(self.geom.c.F, 3))
+        rec = rec[(rec["tri_t"] >= 0) & (rec["weight"] != 0)]
+        bt = np.einsum("qk,qkc->qc", rec["bary_t"], Phi[faces[rec["tri_t"]]])                 # b(t)
+        main = rec["sample"] >= 0
+        smp = rec["sample"][main]
+        bs = np.einsum("qk,qkc->qc", np.asarray(bary, np.float64)[smp], Phi[faces[np.asarray(tri)[smp]]])
+        D = bt.copy()
+        D[main] = bs - bt[main]
+        return (D * rec["weight"][:, None]).T @ D
+
     def winding_number(self, p, exclude=None):
         """Generalised winding number of the mesh at points p [n,3]; exclude [n]: face left out (-1: none)."""
         p = np.ascontiguousarray(p, np.float64).reshape(-1, 3)
