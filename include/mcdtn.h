@@ -312,6 +312,16 @@ int mcs_winding_number(const mcs_bvh* bvh, const float* points, const int32_t* e
 int mcs_orient_samples(const mcs_bvh* bvh, const mcs_samples* samples, float h_scale, float* normal_out,
                        float* d_out /* may be NULL */, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Reduced Ritz-Galerkin DtN matrix: for basis functions
+ * phi_k = sum_v Phi[v][k] hat_v (Phi [V][K] device fp32, row-major: e.g. low-frequency Laplacian eigenmodes at the
+ * vertices) the matrix the paper accumulates from dense vectors b(p) = Phi^T iota(p) equals Phi^T S Phi for the
+ * nodal matrix S [V][V] of mcs_estimate_dtn_* (dense output).  out [K][K] device, exactly symmetric.
+ * workspace >= mcs_project_workspace_bytes(V, K).  Asynchronous on `stream`.  V, K <= 65535.
+ * Errors: MCS_EINVAL, MCS_ENOMEM, MCS_ECUDA. */
+size_t mcs_project_workspace_bytes(int64_t V, int64_t K);
+int mcs_project_galerkin(const float* S, const float* Phi, int64_t V, int64_t K, float* out,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
 /* Smallest Steklov eigenpairs of estimated DtN matrices:
  *     S psi = lambda M psi,  M = diag(mass)  (lumped boundary mass),
  * for a batch of `batch` dense symmetric matrices S [batch][K][K] (symmetrised inside) with mass [batch][K] > 0.

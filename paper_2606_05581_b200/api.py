@@ -602,3 +602,21 @@ def orient_samples(bvh, samples, h_scale=1.0):
         _check(lib().mcs_orient_samples(bvh.handle, C.byref(cs), C.c_float(h_scale), _ptr(nrm), _ptr(d), _ptr(ws),
                                         C.c_size_t(need), _stream(dev)), "mcs_orient_samples")
     return nrm, d
+
+
+def project_galerkin(S, Phi):
+    """Reduced Ritz-Galerkin matrix Phi^T S Phi (mcs_project_galerkin).  S [V,V], Phi [V,K] CUDA fp32 -> [K,K]."""
+    S = _dev(S, torch.float32, "S")
+    Phi = _dev(Phi, torch.float32, "Phi")
+    V, K = int(Phi.shape[0]), int(Phi.shape[1])
+    if tuple(S.shape) != (V, V):
+        raise ValueError("S must be [V, V] with V = Phi.shape[0]")
+    f = lib().mcs_project_workspace_bytes
+    f.restype = C.c_size_t
+    need = int(f(C.c_int64(V), C.c_int64(K)))
+    ws = torch.empty(need, dtype=torch.uint8, device=S.device)
+    out = torch.empty((K, K), dtype=torch.float32, device=S.device)
+    with torch.cuda.device(S.device):
+        _check(lib().mcs_project_galerkin(_ptr(S), _ptr(Phi), C.c_int64(V), C.c_int64(K), _ptr(out), _ptr(ws),
+                                          C.c_size_t(need), _stream(S.device)), "mcs_project_galerkin")
+    return out
