@@ -206,6 +206,10 @@ int mcs_estimate_dtn_interior(const mcs_bvh* bvh, const mcs_samples* samples, co
  * Kelvin-inverted domain about params.kelvin_origin with the factor
  * |s*|^3 / |t*|, plus (include_killing) n_kill_walks walks from kappa(infinity)
  * adding (4 pi / |t0*|) b(t0) b(t0)^T / n_kill_walks.
+ * Walks end with steps >= 0 (landed), -1 (max_steps jumps, R10), -2 (sample discarded)
+ * or -3: interior, the jump radius exceeds the AABB diagonal (the walker is outside the box, R10b); exterior,
+ * the distance to the surface exceeds the distance to kelvin_origin (the walker is inside the solid, R10c).
+ * -1 and -3 contribute nothing and are counted in mcs_stats.n_truncated.
  */
 int mcs_estimate_dtn_exterior(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
                               const mcs_params* params, void* workspace, size_t workspace_bytes,
