@@ -325,6 +325,15 @@ int mcs_orient_samples(const mcs_bvh* bvh, const mcs_samples* samples, float h_s
 size_t mcs_project_workspace_bytes(int64_t V, int64_t K);
 int mcs_project_galerkin(const float* S, const float* Phi, int64_t V, int64_t K, float* out,
                          void* workspace, size_t workspace_bytes, void* stream);
+/* The same from the sparse output (mcs_matrix kind 1): row, col, val [nnz] device, the upper triangle sorted by
+ * (row, col) with one entry per position, as mcs_estimate_dtn_* writes it; any V < 2^31 (the reduced basis is how a
+ * K x K operator is obtained on meshes whose V x V matrix cannot be dense).  Deterministic (no atomics).
+ * workspace >= mcs_project_coo_workspace_bytes(V, K).  Blocks the host (it reads back an error flag).
+ * Errors: MCS_EINVAL (also: an entry below the diagonal or out of range, rows not sorted), MCS_ENOMEM, MCS_ECUDA. */
+size_t mcs_project_coo_workspace_bytes(int64_t V, int64_t K);
+int mcs_project_galerkin_coo(const int32_t* row, const int32_t* col, const float* val, int64_t nnz,
+                             const float* Phi, int64_t V, int64_t K, float* out,
+                             void* workspace, size_t workspace_bytes, void* stream);
 
 /* Smallest Steklov eigenpairs of estimated DtN matrices:
  *     S psi = lambda M psi,  M = diag(mass)  (lumped boundary mass),

@@ -620,3 +620,22 @@ def project_galerkin(S, Phi):
         _check(lib().mcs_project_galerkin(_ptr(S), _ptr(Phi), C.c_int64(V), C.c_int64(K), _ptr(out), _ptr(ws),
                                           C.c_size_t(need), _stream(S.device)), "mcs_project_galerkin")
     return out
+
+
+def project_galerkin_coo(coo, Phi):
+    """Reduced Ritz-Galerkin matrix Phi^T S Phi from the sparse output (CooMatrix of estimate_dtn_coo); Phi [V,K]."""
+    Phi = _dev(Phi, torch.float32, "Phi")
+    V, K = int(Phi.shape[0]), int(Phi.shape[1])
+    if V != coo.K:
+        raise ValueError("Phi must have one row per basis function of the sparse matrix")
+    row, col, val = _dev(coo.row, torch.int32, "row"), _dev(coo.col, torch.int32, "col"), _dev(coo.val, torch.float32, "val")
+    f = lib().mcs_project_coo_workspace_bytes
+    f.restype = C.c_size_t
+    need = int(f(C.c_int64(V), C.c_int64(K)))
+    ws = torch.empty(need, dtype=torch.uint8, device=Phi.device)
+    out = torch.empty((K, K), dtype=torch.float32, device=Phi.device)
+    with torch.cuda.device(Phi.device):
+        _check(lib().mcs_project_galerkin_coo(_ptr(row), _ptr(col), _ptr(val), C.c_int64(int(row.numel())), _ptr(Phi),
+                                              C.c_int64(V), C.c_int64(K), _ptr(out), _ptr(ws), C.c_size_t(need),
+                                              _stream(Phi.device)), "mcs_project_galerkin_coo")
+    return out
