@@ -288,6 +288,161 @@ int eig_block_sweep_vec(EigArgs a, int64_t batch, cudaStream_t st)
     return MCS_OK;
 }
 
+// Gram form of the blocked sweep (K <= 768).  For the 32 staged rows X of G the inner tournament is run on their
+// 32 x 32 Gram matrix W = X X^T instead of on the rows: a one-sided rotation of rows p, q is the two-sided rotation
+// W <- R W R^T (same alpha = W_pp, beta = W_qq, gamma = W_pq, same c and s), so the same rotations come out, at
+// 32 numbers per row instead of K.  They are accumulated in J (32 x 32); the rows of G and of Q are then updated
+// once, X <- J X, Q <- J Q, as register-tiled products written straight to global memory.  Shared-memory traffic
+// per block pair: about 25 passes over the staged rows instead of 250.  Convergence is judged on the freshly
+// computed Gram matrix of every visit, so rounding inside W cannot accumulate from visit to visit.
+template <int NV>
+__global__ void __launch_bounds__(512)
+eig_block_gram_kernel(EigArgs a, int nblk_p)
+{
+    constexpr int BR = 16, R2 = 32, RS = 32 * NV;             // rows per block, staged rows, row stride in float4
+    extern __shared__ float4 s_rows4[];
+    float4* sX = s_rows4;
+    float4* sQ = s_rows4 + R2 * RS;
+    float (*sW)[R2 + 1] = reinterpret_cast<float (*)[R2 + 1]>(s_rows4 + 2 * R2 * RS);
+    float (*sJ)[R2 + 1] = sW + R2;
+    const long long K = a.K, b = blockIdx.y;
+    int I, Jb;
+    tournament_pair(nblk_p, a.round, blockIdx.x, I, Jb);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    auto global_row = [&](int r) -> long long {
+        const long long g = (long long)(r < BR ? I : Jb) * BR + (r < BR ? r : r - BR);
+        return g < K ? g : -1;
+    };
+    for (int r = warp; r < R2; r += BR) {
+        const long long g = global_row(r);
+        float* dg = (float*)(sX + r * RS);
+        float* dq = (float*)(sQ + r * RS);
+        if (g < 0) { for (int j = lane; j < 4 * RS; j += 32) { dg[j] = 0.0f; dq[j] = 0.0f; } continue; }
+        const float* src_g = a.G + (b * K + g) * K;
+        const float* src_q = a.Q + (b * K + g) * K;
+        if ((K & 3) == 0) {                                   // rows are 16-byte aligned: 128-bit loads
+            const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int j = lane; j < RS; j += 32) {
+                const bool in = 4 * j < K;
+                sX[r * RS + j] = in ? reinterpret_cast<const float4*>(src_g)[j] : z4;
+                sQ[r * RS + j] = in ? reinterpret_cast<const float4*>(src_q)[j] : z4;
+            }
+        } else {
+            for (int j = lane; j < 4 * RS; j += 32) { dg[j] = j < K ? src_g[j] : 0.0f; dq[j] = j < K ? src_q[j] : 0.0f; }
+        }
+    }
+    for (int i = threadIdx.x; i < R2 * (R2 + 1); i += 512) { (&sJ[0][0])[i] = 0.0f; }
+    __syncthreads();
+    if (threadIdx.x < R2) sJ[threadIdx.x][threadIdx.x] = 1.0f;
+    // W = X X^T: warp w owns rows w and w + 16 (kept in registers), against every row j >= its own
+    for (int i = warp; i < R2; i += BR) {
+        float4 x[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) x[v] = sX[i * RS + lane + 32 * v];
+        for (int j0 = i; j0 < R2; j0 += 4) {                  // four dot products in flight
+            float d[4] = { 0.f, 0.f, 0.f, 0.f };
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int j = j0 + u < R2 ? j0 + u : R2 - 1;
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    const float4 y = sX[j * RS + lane + 32 * v];
+                    d[u] = fmaf(x[v].x, y.x, d[u]); d[u] = fmaf(x[v].y, y.y, d[u]); d[u] = fmaf(x[v].z, y.z, d[u]); d[u] = fmaf(x[v].w, y.w, d[u]);
+                }
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) d[u] += __shfl_xor_sync(0xFFFFFFFFu, d[u], o);
+            }
+            if (lane < 4 && j0 + lane < R2) { const float dv = lane == 0 ? d[0] : lane == 1 ? d[1] : lane == 2 ? d[2] : d[3]; sW[i][j0 + lane] = dv; sW[j0 + lane][i] = dv; }
+        }
+    }
+    __syncthreads();
+    const float nul = 1e-6f * __uint_as_float(a.scale_bits[b]);
+    bool rotated = false;
+    for (int round = 0; round < R2 - 1; ++round) {
+        int p = 0, q = 1;
+        float c = 1.0f, sn = 0.0f;
+        if (warp < BR) {
+            tournament_pair(R2, round, warp, p, q);
+            const float al = sW[p][p], be = sW[q][q], ga = sW[p][q];
+            if (global_row(p) >= 0 && global_row(q) >= 0 && !(al < nul * nul || be < nul * nul) && fabsf(ga) > a.tol * sqrtf(al * be)) {
+                rotated = true;
+                const float zeta = (be - al) / (2.0f * ga);
+                const float t = copysignf(1.0f, zeta) / (fabsf(zeta) + sqrtf(fmaf(zeta, zeta, 1.0f)));
+                c = 1.0f / sqrtf(fmaf(t, t, 1.0f)); sn = c * t;
+            }
+        }
+        __syncthreads();                                      // every pair has read its alpha, beta, gamma
+        if (sn != 0.0f) {                                     // rows p, q of W and of J (lane = column)
+            const float wp = sW[p][lane], wq = sW[q][lane];
+            sW[p][lane] = fmaf(c, wp, -sn * wq); sW[q][lane] = fmaf(sn, wp, c * wq);
+            const float jp = sJ[p][lane], jq = sJ[q][lane];
+            sJ[p][lane] = fmaf(c, jp, -sn * jq); sJ[q][lane] = fmaf(sn, jp, c * jq);
+        }
+        __syncthreads();
+        if (sn != 0.0f) {                                     // columns p, q of W (lane = row)
+            const float wp = sW[lane][p], wq = sW[lane][q];
+            sW[lane][p] = fmaf(c, wp, -sn * wq); sW[lane][q] = fmaf(sn, wp, c * wq);
+        }
+        __syncthreads();
+    }
+    if (rotated && lane == 0) *a.not_converged = 1u;
+    const unsigned any = __syncthreads_or(rotated ? 1 : 0);
+    if (!any) return;                                         // nothing rotated in this block pair: rows unchanged
+    // X <- J X, Q <- J Q: warp w computes output rows w and w + 16 over all columns, reading every staged row once
+    for (int m = 0; m < 2; ++m) {
+        const float4* src = m == 0 ? sX : sQ;
+        float* dst_base = m == 0 ? a.G : a.Q;
+        float4 acc0[NV], acc1[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { acc0[v] = make_float4(0.f, 0.f, 0.f, 0.f); acc1[v] = acc0[v]; }
+        for (int j = 0; j < R2; ++j) {
+            const float j0 = sJ[warp][j], j1 = sJ[warp + BR][j];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const float4 y = src[j * RS + lane + 32 * v];
+                acc0[v].x = fmaf(j0, y.x, acc0[v].x); acc0[v].y = fmaf(j0, y.y, acc0[v].y); acc0[v].z = fmaf(j0, y.z, acc0[v].z); acc0[v].w = fmaf(j0, y.w, acc0[v].w);
+                acc1[v].x = fmaf(j1, y.x, acc1[v].x); acc1[v].y = fmaf(j1, y.y, acc1[v].y); acc1[v].z = fmaf(j1, y.z, acc1[v].z); acc1[v].w = fmaf(j1, y.w, acc1[v].w);
+            }
+        }
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const long long g = global_row(warp + half * BR);
+            if (g < 0) continue;
+            float* dst = dst_base + (b * K + g) * K;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const float4 o = half == 0 ? acc0[v] : acc1[v];
+                const int col = 4 * (lane + 32 * v);
+                if ((K & 3) == 0) { if (col < K) reinterpret_cast<float4*>(dst)[lane + 32 * v] = o; continue; }
+                if (col < K) dst[col] = o.x;
+                if (col + 1 < K) dst[col + 1] = o.y;
+                if (col + 2 < K) dst[col + 2] = o.z;
+                if (col + 3 < K) dst[col + 3] = o.w;
+            }
+        }
+    }
+}
+
+template <int NV>
+int eig_block_sweep_gram(EigArgs a, int64_t batch, cudaStream_t st)
+{
+    const size_t smem = (size_t)4 * 16 * 128 * NV * sizeof(float) + (size_t)2 * 32 * 33 * sizeof(float);
+    static bool attr_set = false;
+    if (!attr_set) {
+        MCS_CUDA_TRY(cudaFuncSetAttribute(eig_block_gram_kernel<NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    const int nblk = (int)ceil_div64(a.K, 16);
+    const int nblk_p = nblk < 2 ? 2 : nblk + (nblk & 1);
+    for (int r = 0; r < nblk_p - 1; ++r) {
+        a.round = r;
+        mcs_note_launch(), eig_block_gram_kernel<NV><<<dim3((unsigned)(nblk_p / 2), (unsigned)batch), 512, smem, st>>>(a, nblk_p);
+    }
+    return MCS_OK;
+}
+
 template <int BR>
 int eig_block_sweep(EigArgs a, int64_t batch, cudaStream_t st)
 {
@@ -389,12 +544,12 @@ extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, in
             MCS_CUDA_TRY(cudaMemsetAsync(flag, 0, 4, st));
             // rows staged in shared memory while 2 x 2 BR rows fit (BR = 16 to K = 896, BR = 8 to K = 1760); else row pairs from L2/HBM
             int rc = MCS_OK;
-            if (K <= 128) rc = eig_block_sweep_vec<16, 1>(a, batch, st);
-            else if (K <= 256) rc = eig_block_sweep_vec<16, 2>(a, batch, st);
-            else if (K <= 384) rc = eig_block_sweep_vec<16, 3>(a, batch, st);
-            else if (K <= 512) rc = eig_block_sweep_vec<16, 4>(a, batch, st);
-            else if (K <= 640) rc = eig_block_sweep_vec<16, 5>(a, batch, st);
-            else if (K <= 768) rc = eig_block_sweep_vec<16, 6>(a, batch, st);
+            if (K <= 128) rc = eig_block_sweep_gram<1>(a, batch, st);
+            else if (K <= 256) rc = eig_block_sweep_gram<2>(a, batch, st);
+            else if (K <= 384) rc = eig_block_sweep_gram<3>(a, batch, st);
+            else if (K <= 512) rc = eig_block_sweep_gram<4>(a, batch, st);
+            else if (K <= 640) rc = eig_block_sweep_gram<5>(a, batch, st);
+            else if (K <= 768) rc = eig_block_sweep_gram<6>(a, batch, st);
             else if (K <= 896) rc = eig_block_sweep_vec<16, 7>(a, batch, st);
             else if (K <= 1760) rc = eig_block_sweep<8>(a, batch, st);
             else
