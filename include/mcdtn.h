@@ -216,6 +216,27 @@ int mcs_estimate_dtn_exterior(const mcs_bvh* bvh, const mcs_samples* samples, co
                               const mcs_matrix* out, mcs_stats* host_stats, void* stream);
 
 /*
+ * Both operators of one mesh in one call (the unit BASELINE configs 1-4 ask for: "interior and exterior DtN"):
+ * the same two estimates as mcs_estimate_dtn_interior(params_interior) and mcs_estimate_dtn_exterior(params_exterior),
+ * bit for bit (walks are keyed by (seed, sample, walk, step) and accumulated in a fixed order, so the result does
+ * not depend on the schedule), with the two persistent walk kernels overlapped: all preparation runs on `stream`,
+ * then the interior's walk + accumulation go to a library-owned high-priority stream and the exterior's to a
+ * low-priority one (the interior's blocks are dispatched first; the exterior's fill the SM slots its tail gives up),
+ * both waiting for the preparation; `stream` waits for both before the call's work is complete, so the caller sees
+ * ordinary stream semantics.  out_interior and out_exterior must be different buffers;
+ * workspace >= mcs_workspace_bytes_both (the two operators' workspaces side by side).
+ * Asynchronous on `stream` up to the exterior's read-back of its Kelvin bounds (a few microseconds of device
+ * work) unless a stats pointer is given.  Errors: as mcs_estimate_dtn_*.
+ */
+size_t mcs_workspace_bytes_both(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                                const mcs_params* params_interior, const mcs_params* params_exterior);
+int mcs_estimate_dtn_both(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
+                          const mcs_params* params_interior, const mcs_params* params_exterior,
+                          void* workspace, size_t workspace_bytes,
+                          const mcs_matrix* out_interior, const mcs_matrix* out_exterior,
+                          mcs_stats* host_stats_interior, mcs_stats* host_stats_exterior, void* stream);
+
+/*
  * The whole path from HOST buffers, for callers that keep their data on the CPU
  * (and for the end-to-end measurement): uploads the mesh and the samples,
  * builds the LBVH, runs the requested estimators (operators: bit 0 = interior,
@@ -224,6 +245,7 @@ int mcs_estimate_dtn_exterior(const mcs_bvh* bvh, const mcs_samples* samples, co
  * (pinned memory makes the copies asynchronous but is not required);
  * out_interior / out_exterior are [V][V] fp32 and may be NULL when their bit is
  * clear.  Device memory is allocated and freed inside the call (stream-ordered);
+ * with both bits set the two operators run as in mcs_estimate_dtn_both;
  * the call blocks until the results are in the host buffers.  `stats` (host,
  * may be NULL) receives the counters of the LAST operator run.
  * Errors: as mcs_build_bvh and mcs_estimate_dtn_*.
@@ -293,6 +315,9 @@ typedef struct {
     float walk_ms;               /* A3-A6: the persistent walk kernel           */
     float accumulate_ms;         /* A7                                          */
     float total_ms;
+    /* mcs_estimate_dtn_both only (else 0): start of the interior walk kernel to the end of the interior / exterior
+     * kernel; walk_ms is the larger, accumulate_ms what follows it */
+    float walk_interior_ms, walk_exterior_ms;
 } mcs_phase_times;
 unsigned long long mcs_launch_count(void);
 int mcs_profile_enable(int on);

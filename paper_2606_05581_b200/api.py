@@ -328,6 +328,41 @@ def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats
                      want_stats, out, workspace, _exact_workspace, basis)
 
 
+def workspace_bytes_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params, basis=None) -> int:
+    cs, cb = samples.c(), _basis(bvh, basis)
+    ci, ce = params_interior.c(), params_exterior.c()
+    fn = lib().mcs_workspace_bytes_both
+    fn.restype = C.c_size_t
+    return int(fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(ci), C.byref(ce)))
+
+
+def estimate_dtn_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params, want_stats=False,
+                      out_interior=None, out_exterior=None, workspace=None, basis=None):
+    """Interior and exterior DtN matrices of one mesh in one call (mcs_estimate_dtn_both): the same results as the
+    two single calls, bit for bit, with the two walk kernels overlapped on two streams."""
+    cs, cb = samples.c(), _basis(bvh, basis)
+    ci, ce = params_interior.c(), params_exterior.c()
+    K = basis.K if basis is not None else bvh.V
+    if out_interior is None:
+        out_interior = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
+    if out_exterior is None:
+        out_exterior = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
+    need = workspace_bytes_both(bvh, samples, params_interior, params_exterior, basis)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+    mi = _Matrix(kind=0, K=K, dense=out_interior.data_ptr())
+    me = _Matrix(kind=0, K=K, dense=out_exterior.data_ptr())
+    si = Stats() if want_stats else None
+    se = Stats() if want_stats else None
+    with torch.cuda.device(bvh.device):
+        rc = lib().mcs_estimate_dtn_both(bvh.handle, C.byref(cs), C.byref(cb), C.byref(ci), C.byref(ce), _ptr(workspace),
+                                         C.c_size_t(workspace.numel()), C.byref(mi), C.byref(me),
+                                         C.byref(si) if si is not None else None, C.byref(se) if se is not None else None,
+                                         _stream(bvh.device))
+    _check(rc, "mcs_estimate_dtn_both")
+    return (out_interior, out_exterior, si, se) if want_stats else (out_interior, out_exterior)
+
+
 def estimate_dtn_host(verts, faces, tri, bary, weight, params: Params, interior=True, exterior=True,
                       out_interior=None, out_exterior=None, normal=None, want_stats=False, device=None):
     """The whole path from HOST tensors (mcs_estimate_dtn_host): upload, LBVH build, estimators,
@@ -443,7 +478,7 @@ def sort_pairs_u64(keys, vals, key_bits=64):
 
 class PhaseTimes(C.Structure):
     _fields_ = [("prep_ms", C.c_float), ("walk_ms", C.c_float), ("accumulate_ms", C.c_float),
-                ("total_ms", C.c_float)]
+                ("total_ms", C.c_float), ("walk_interior_ms", C.c_float), ("walk_exterior_ms", C.c_float)]
 
 
 def launch_count() -> int:

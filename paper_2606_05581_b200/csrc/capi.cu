@@ -123,7 +123,118 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
     return MCS_OK;
 }
 
+// Both operators of one mesh with their walk kernels overlapped ("The tail"): everything that
+// precedes the two walk kernels runs on `st` (the exterior's preparation reads back its Kelvin bounds), then the
+// interior walk and its accumulation go to a library-owned high-priority stream and the exterior's to a low-priority
+// one, both waiting for the preparation; `st` waits for both at the end.  The exterior's blocks take the SM slots the interior
+// launch gives up in its tail, and the interior's accumulation fills the exterior's tail.
+// which: 0 = the interior's stream (highest priority: its blocks are dispatched first, so the exterior's bulk runs
+// beside the interior's long tail and not the other way round), 1 = the exterior's stream (lowest priority).
+cudaStream_t side_stream(int which)
+{
+    static thread_local cudaStream_t ss[2] = { nullptr, nullptr };
+    static thread_local int ss_dev = -1;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    if (!ss[0] || ss_dev != dev) {
+        int least = 0, greatest = 0;
+        if (cudaDeviceGetStreamPriorityRange(&least, &greatest) != cudaSuccess) return nullptr;
+        if (cudaStreamCreateWithPriority(&ss[0], cudaStreamNonBlocking, greatest) != cudaSuccess ||
+            cudaStreamCreateWithPriority(&ss[1], cudaStreamNonBlocking, least) != cudaSuccess) { ss[0] = nullptr; return nullptr; }
+        ss_dev = dev;
+    }
+    return ss[which];
+}
+
+int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
+                  const mcs_params* p_int, const mcs_params* p_ext, void* ws, size_t ws_bytes,
+                  const mcs_matrix* out_int, const mcs_matrix* out_ext, mcs_stats* hs_int, mcs_stats* hs_ext, void* stream)
+{
+    if (hs_int) memset(hs_int, 0, sizeof *hs_int);
+    if (hs_ext) memset(hs_ext, 0, sizeof *hs_ext);
+    if (!b || !s || !basis || !p_int || !p_ext || !out_int || !out_ext) return MCS_EINVAL;
+    const mcs_params* pp[2] = { p_int, p_ext };
+    const mcs_matrix* oo[2] = { out_int, out_ext };
+    mcs_stats* hh[2] = { hs_int, hs_ext };
+    for (int x = 0; x < 2; ++x) {
+        const mcs_params* p = pp[x];
+        if ((p->output_kind != 0 && p->output_kind != 1) || oo[x]->kind != p->output_kind) return MCS_EINVAL;
+        if (p->output_kind == 1 && (p->coo_capacity < 1 || oo[x]->coo_capacity != p->coo_capacity)) return MCS_EINVAL;
+        if (p->walks_per_sample < 1) return MCS_EINVAL;
+    }
+    if (s->n_s < 1) return MCS_EINVAL;
+    if (out_int->kind == out_ext->kind && (out_int->kind == 0 ? out_int->dense == out_ext->dense : out_int->coo_val == out_ext->coo_val))
+        return MCS_EINVAL;                            // the two operators run concurrently: separate outputs
+    cudaStream_t st = (cudaStream_t)stream, st1 = side_stream(0), st2 = side_stream(1);
+    if (!st1 || !st2) return MCS_ECUDA;
+    Layout L[2];
+    for (int x = 0; x < 2; ++x) L[x] = make_layout(b, s, basis, pp[x], x, true, true);
+    const size_t total = L[0].total + L[1].total;
+    for (int x = 0; x < 2; ++x) if (hh[x]) hh[x]->workspace_needed = (int64_t)total;
+    if (!ws || ws_bytes < total) return MCS_ENOMEM;
+    char* base[2] = { (char*)ws, (char*)ws + L[0].total };
+    static thread_local cudaEvent_t ev_prep = nullptr, ev_done = nullptr, ev_done1 = nullptr;
+    if (!ev_prep) {
+        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_prep, cudaEventDisableTiming));
+        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
+        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_done1, cudaEventDisableTiming));
+    }
+    unsigned long long* stats_dev[2] = { nullptr, nullptr };
+    WalkLaunch wl[2];
+    mcs_prof_mark(MCS_MARK_BEGIN, st);
+    for (int x = 1; x >= 0; --x) {                    // exterior first: its host read-back happens before anything long runs
+        int rc = walk_run(b, s, pp[x], x, base[x] + L[x].walk_off, align_up(walk_workspace_bytes(s)),
+                          (float4*)(base[x] + L[x].records_off), nullptr, false, nullptr, hh[x] != nullptr, &stats_dev[x], st, &wl[x]);
+        if (rc != MCS_OK) return fail(rc, hh[x]);
+    }
+    MCS_CUDA_TRY(cudaEventRecord(ev_prep, st));
+    MCS_CUDA_TRY(cudaStreamWaitEvent(st1, ev_prep, 0));
+    MCS_CUDA_TRY(cudaStreamWaitEvent(st2, ev_prep, 0));
+    mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
+    int rc = walk_launch(&wl[0], st1);
+    mcs_prof_mark(MCS_MARK_WALK_END2, st1);
+    if (rc == MCS_OK) rc = walk_launch(&wl[1], st2);
+    mcs_prof_mark(MCS_MARK_WALK_END, st2);            // walk_ms: both walk kernels, from the first block to the last
+    cudaStream_t ss[2] = { st1, st2 };
+    for (int x = 0; x < 2 && rc == MCS_OK; ++x)
+        rc = acc_run(b, s, basis, pp[x], (const float4*)(base[x] + L[x].records_off), L[x].n_records, base[x] + L[x].acc_off,
+                     align_up(acc_ws_bytes(b, s, basis, pp[x], L[x].n_records)), oo[x], stats_dev[x], ss[x]);
+    // join even after an error: the caller's stream must not run ahead of work queued on the second one
+    cudaError_t e = cudaEventRecord(ev_done, st2);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done, 0);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_done1, st1);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done1, 0);
+    if (rc != MCS_OK) return fail(rc, hs_ext);
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return fail(MCS_ECUDA, hs_ext); }
+    mcs_prof_mark(MCS_MARK_END, st);
+    for (int x = 0; x < 2; ++x) {
+        if (!hh[x]) continue;
+        unsigned long long h[ST_COUNT];
+        e = cudaMemcpyAsync(h, stats_dev[x], sizeof h, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return fail(MCS_ECUDA, hh[x]); }
+        fill_stats(hh[x], h, s, L[x].n_records);
+        hh[x]->workspace_needed = (int64_t)total;
+    }
+    return MCS_OK;
+}
+
 }  // namespace
+
+extern "C" size_t mcs_workspace_bytes_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
+                                           const mcs_params* p_int, const mcs_params* p_ext)
+{
+    if (!b || !s || !basis || !p_int || !p_ext || s->n_s < 1 || p_int->walks_per_sample < 1 || p_ext->walks_per_sample < 1) return 0;
+    return make_layout(b, s, basis, p_int, 0, true, true).total + make_layout(b, s, basis, p_ext, 1, true, true).total;
+}
+
+extern "C" int mcs_estimate_dtn_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
+                                     const mcs_params* p_int, const mcs_params* p_ext, void* ws, size_t ws_bytes,
+                                     const mcs_matrix* out_int, const mcs_matrix* out_ext,
+                                     mcs_stats* hs_int, mcs_stats* hs_ext, void* stream)
+{
+    return estimate_both(b, s, basis, p_int, p_ext, ws, ws_bytes, out_int, out_ext, hs_int, hs_ext, stream);
+}
 
 extern "C" unsigned long long mcs_launch_count(void) { return g_launches.load(); }
 
@@ -134,12 +245,19 @@ extern "C" int mcs_profile_last(mcs_phase_times* out)
     if (!out) return MCS_EINVAL;
     memset(out, 0, sizeof *out);
     if (!g_prof_have) return MCS_EINVAL;
-    for (int i = 0; i < MCS_MARK_COUNT; ++i) if (!g_prof_marked[i]) return MCS_EINVAL;
+    for (int i = 0; i < MCS_MARK_COUNT; ++i) if (!g_prof_marked[i] && i != MCS_MARK_WALK_END2) return MCS_EINVAL;
     MCS_CUDA_TRY(cudaEventSynchronize(g_prof_ev[MCS_MARK_END]));
     MCS_CUDA_TRY(cudaEventElapsedTime(&out->prep_ms, g_prof_ev[MCS_MARK_BEGIN], g_prof_ev[MCS_MARK_WALK_BEGIN]));
     MCS_CUDA_TRY(cudaEventElapsedTime(&out->walk_ms, g_prof_ev[MCS_MARK_WALK_BEGIN], g_prof_ev[MCS_MARK_WALK_END]));
     MCS_CUDA_TRY(cudaEventElapsedTime(&out->accumulate_ms, g_prof_ev[MCS_MARK_WALK_END], g_prof_ev[MCS_MARK_END]));
     MCS_CUDA_TRY(cudaEventElapsedTime(&out->total_ms, g_prof_ev[MCS_MARK_BEGIN], g_prof_ev[MCS_MARK_END]));
+    if (g_prof_marked[MCS_MARK_WALK_END2]) {          // two overlapped walk kernels: the span up to the later end
+        float w2 = 0.0f;
+        MCS_CUDA_TRY(cudaEventElapsedTime(&w2, g_prof_ev[MCS_MARK_WALK_BEGIN], g_prof_ev[MCS_MARK_WALK_END2]));
+        out->walk_interior_ms = w2; out->walk_exterior_ms = out->walk_ms;
+        if (w2 > out->walk_ms) out->walk_ms = w2;
+        out->accumulate_ms = out->total_ms - out->prep_ms - out->walk_ms;
+    }
     return MCS_OK;
 }
 
@@ -192,7 +310,7 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
     mcs_bvh* bvh = nullptr;
     int rc = MCS_OK;
     cudaError_t e = cudaMallocAsync((void**)&d_in, in_total, st);
-    if (e == cudaSuccess) e = cudaMallocAsync((void**)&d_out, nb_m, st);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&d_out, operators == 3 ? 2 * nb_m : nb_m, st);
     if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
     e = cudaMemcpyAsync(d_in + off_v, verts, nb_v, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_f, faces, nb_f, cudaMemcpyHostToDevice, st);
@@ -216,6 +334,18 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
                 const size_t b = make_layout(bvh, &ds, &basis, p, ext, true, true).total;
                 need = b > need ? b : need;
             }
+        if (operators == 3) {                         // both: walk kernels overlapped on two streams
+            mcs_matrix m2 = m; m2.dense = d_out + (size_t)V * V;
+            need = make_layout(bvh, &ds, &basis, p, 0, true, true).total + make_layout(bvh, &ds, &basis, p, 1, true, true).total;
+            e = cudaMallocAsync(&d_ws, need, st);
+            if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+            rc = estimate_both(bvh, &ds, &basis, p, p, d_ws, need, &m, &m2, nullptr, stats, stream);
+            if (rc != MCS_OK) goto done;
+            e = cudaMemcpyAsync(out_interior, d_out, nb_m, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(out_exterior, m2.dense, nb_m, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+            goto done;
+        }
         e = cudaMallocAsync(&d_ws, need, st);
         if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
         for (int ext = 0; ext < 2 && rc == MCS_OK; ++ext) {

@@ -18,7 +18,7 @@
 // Launch counter (bench.py's gpu_launches) and phase marks (CUDA events on the
 // caller's stream, recorded only while mcs_profile_enable(1) is in effect).
 void mcs_note_launch();
-enum { MCS_MARK_BEGIN = 0, MCS_MARK_WALK_BEGIN, MCS_MARK_WALK_END, MCS_MARK_END, MCS_MARK_COUNT };
+enum { MCS_MARK_BEGIN = 0, MCS_MARK_WALK_BEGIN, MCS_MARK_WALK_END, MCS_MARK_END, MCS_MARK_WALK_END2 /* optional: second walk kernel */, MCS_MARK_COUNT };
 void mcs_prof_mark(int which, cudaStream_t st);
 
 void mcs_set_last_cuda_error(int e);

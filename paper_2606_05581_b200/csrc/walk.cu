@@ -886,7 +886,7 @@ size_t walk_workspace_bytes(const mcs_samples* s)
 // Runs A2-A6.  Layout of `ws`: see walk_workspace_bytes.
 int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
              void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
-             bool count, unsigned long long** stats_dev_out, cudaStream_t st)
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st, WalkLaunch* defer)
 {
     int rc = check_params(b, s, p, exterior);
     if (rc != MCS_OK) return rc;
@@ -1016,9 +1016,20 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     if (grid > need_blocks) grid = need_blocks;
     if (grid > MAX_WALK_BLOCKS) grid = MAX_WALK_BLOCKS;
     if (grid < 1) grid = 1;
+    if (defer) {                                      // the caller launches it (two operators on two streams)
+        defer->fn = fn; defer->grid = (unsigned)grid; defer->g = g; defer->a = a;
+        return MCS_OK;
+    }
     mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
     mcs_note_launch(), fn<<<(unsigned)grid, WT, 0, st>>>(g, a);
     mcs_prof_mark(MCS_MARK_WALK_END, st);
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+int walk_launch(const WalkLaunch* w, cudaStream_t st)
+{
+    mcs_note_launch(), w->fn<<<w->grid, WT, 0, st>>>(w->g, w->a);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

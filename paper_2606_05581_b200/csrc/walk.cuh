@@ -44,7 +44,17 @@ int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior
 size_t  walk_workspace_bytes(const mcs_samples* s);
 int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
              void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
-             bool count, unsigned long long** stats_dev_out, cudaStream_t st);
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st, struct WalkLaunch* defer = nullptr);
+
+// A prepared launch of the walk kernel (walk_run with `defer`): everything before the kernel has been
+// enqueued on walk_run's stream; walk_launch may enqueue the kernel on another stream that waits for it.
+struct WalkLaunch {
+    void (*fn)(WalkGeom, WalkArgs);
+    unsigned grid;
+    WalkGeom g;
+    WalkArgs a;
+};
+int walk_launch(const WalkLaunch* w, cudaStream_t st);
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records);
 size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64_t coo_capacity);

@@ -464,3 +464,51 @@ def test_naive_estimator_records_and_matrix_match_oracle(api):
     assert e.value.code == api.MCS_EINVAL
     with pytest.raises(api.McsError):
         api.estimate_dtn_interior(bvh, S, api.Params(walks_per_sample=2, estimator=1, inset=0.0))
+
+
+# ------------------------------------------------------------------------------
+# both operators in one call (mcs_estimate_dtn_both): walk kernels overlapped on two streams
+# ------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["sphere", "components"])
+def test_both_operators_in_one_call_equal_the_single_calls_bit_for_bit(api, case):
+    if case == "sphere":
+        v, f = icosphere(3)
+        smp = vertex_cell_samples(v, f, 4, seed=2)
+        W, kill = 64, 4096
+    else:
+        v, f = merge_meshes([icosphere(2), torus(1.0, 0.3, 24, 12, center=(3.0, 0.0, 0.0)),
+                             box((0.6, 0.8, 1.0), (3, 3, 3), center=(0.0, 2.5, 0.0))])[:2]
+        smp = uniform_samples(v, f, 1777, seed=9)
+        W, kill = 37, 5001
+    bvh, S = _setup(api, v, f, smp)
+    Pi = api.Params(seed=11, walks_per_sample=W, eps=1e-3)
+    Pe = api.Params(seed=12, walks_per_sample=W, eps=1e-3, include_killing=True, n_kill_walks=kill,
+                    kelvin_origin=(0.05, -0.02, 0.03))
+    Si = api.estimate_dtn_interior(bvh, S, Pi).clone()
+    Se = api.estimate_dtn_exterior(bvh, S, Pe).clone()
+    Bi, Be, st_i, st_e = api.estimate_dtn_both(bvh, S, Pi, Pe, want_stats=True)
+    assert torch.equal(Bi, Si) and torch.equal(Be, Se)
+    assert st_i.n_walks == S.n_s * W and st_e.n_walks == S.n_s * W + kill
+    assert st_i.n_steps > 0 and st_e.n_steps > 0
+    # again without the counters (the instance bench.py times), on a side stream, several times in a row
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        for _ in range(3):
+            Ci, Ce = api.estimate_dtn_both(bvh, S, Pi, Pe)
+            # work queued behind the call on the caller's stream sees both results
+            di, de = (Ci - Si).abs().max(), (Ce - Se).abs().max()
+    side.synchronize()
+    assert float(di) == 0.0 and float(de) == 0.0
+
+
+def test_both_operators_argument_errors(api):
+    v, f = icosphere(1)
+    smp = vertex_cell_samples(v, f, 2, seed=0)
+    bvh, S = _setup(api, v, f, smp)
+    P = api.Params(seed=1, walks_per_sample=8, eps=1e-3)
+    out = torch.empty((bvh.V, bvh.V), dtype=torch.float32, device="cuda")
+    with pytest.raises(api.McsError):          # the operators run concurrently: one buffer for both is refused
+        api.estimate_dtn_both(bvh, S, P, P, out_interior=out, out_exterior=out)
+    need = api.workspace_bytes_both(bvh, S, P, P)
+    assert need == api.workspace_bytes(bvh, S, P, False) + api.workspace_bytes(bvh, S, P, True)
