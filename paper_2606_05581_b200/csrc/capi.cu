@@ -148,7 +148,8 @@ cudaStream_t side_stream(int which)
 
 int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
                   const mcs_params* p_int, const mcs_params* p_ext, void* ws, size_t ws_bytes,
-                  const mcs_matrix* out_int, const mcs_matrix* out_ext, mcs_stats* hs_int, mcs_stats* hs_ext, void* stream)
+                  const mcs_matrix* out_int, const mcs_matrix* out_ext, mcs_stats* hs_int, mcs_stats* hs_ext, void* stream,
+                  float* host_int = nullptr, float* host_ext = nullptr)   // host copies of dense outputs, each on its operator's stream
 {
     if (hs_int) memset(hs_int, 0, sizeof *hs_int);
     if (hs_ext) memset(hs_ext, 0, sizeof *hs_ext);
@@ -199,6 +200,12 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     for (int x = 0; x < 2 && rc == MCS_OK; ++x)
         rc = acc_run(b, s, basis, pp[x], (const float4*)(base[x] + L[x].records_off), L[x].n_records, base[x] + L[x].acc_off,
                      align_up(acc_ws_bytes(b, s, basis, pp[x], L[x].n_records)), oo[x], stats_dev[x], ss[x]);
+    float* host_out[2] = { host_int, host_ext };
+    for (int x = 0; x < 2 && rc == MCS_OK; ++x)
+        if (host_out[x] && oo[x]->kind == 0) {        // the interior's download runs beside the exterior's accumulation
+            cudaError_t ec = cudaMemcpyAsync(host_out[x], oo[x]->dense, (size_t)oo[x]->K * oo[x]->K * 4, cudaMemcpyDeviceToHost, ss[x]);
+            if (ec != cudaSuccess) { mcs_set_last_cuda_error((int)ec); rc = MCS_ECUDA; }
+        }
     // join even after an error: the caller's stream must not run ahead of work queued on the second one
     cudaError_t e = cudaEventRecord(ev_done, st2);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done, 0);
@@ -339,11 +346,7 @@ extern "C" int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_
             need = make_layout(bvh, &ds, &basis, p, 0, true, true).total + make_layout(bvh, &ds, &basis, p, 1, true, true).total;
             e = cudaMallocAsync(&d_ws, need, st);
             if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
-            rc = estimate_both(bvh, &ds, &basis, p, p, d_ws, need, &m, &m2, nullptr, stats, stream);
-            if (rc != MCS_OK) goto done;
-            e = cudaMemcpyAsync(out_interior, d_out, nb_m, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaMemcpyAsync(out_exterior, m2.dense, nb_m, cudaMemcpyDeviceToHost, st);
-            if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+            rc = estimate_both(bvh, &ds, &basis, p, p, d_ws, need, &m, &m2, nullptr, stats, stream, out_interior, out_exterior);
             goto done;
         }
         e = cudaMallocAsync(&d_ws, need, st);

@@ -512,3 +512,24 @@ def test_both_operators_argument_errors(api):
         api.estimate_dtn_both(bvh, S, P, P, out_interior=out, out_exterior=out)
     need = api.workspace_bytes_both(bvh, S, P, P)
     assert need == api.workspace_bytes(bvh, S, P, False) + api.workspace_bytes(bvh, S, P, True)
+
+
+@pytest.mark.parametrize("ops", [(True, False), (False, True), (True, True)])
+def test_host_entry_point_equals_the_device_calls_bit_for_bit(api, ops):
+    """mcs_estimate_dtn_host (upload, build, estimate, download; with both operators: the overlapped call with each
+    download on its operator's stream) against build_bvh + estimate_dtn_* on device tensors."""
+    interior, exterior = ops
+    v, f = merge_meshes([icosphere(2), box((0.6, 0.8, 1.0), (3, 3, 3), center=(2.2, 0.1, 0.0))])[:2]
+    smp = uniform_samples(v, f, 1501, seed=3)
+    bvh, S = _setup(api, v, f, smp)
+    P = api.Params(seed=5, walks_per_sample=48, eps=1e-3, include_killing=True, n_kill_walks=7777,
+                   kelvin_origin=(0.02, 0.01, -0.03))
+    res = api.estimate_dtn_host(torch.as_tensor(v, dtype=torch.float32), torch.as_tensor(f, dtype=torch.int32),
+                                torch.as_tensor(smp["tri"]), torch.as_tensor(smp["bary"]), torch.as_tensor(smp["weight"]),
+                                P, interior=interior, exterior=exterior, want_stats=True)
+    if interior:
+        assert torch.equal(res["interior"], api.estimate_dtn_interior(bvh, S, P).cpu())
+    if exterior:
+        assert torch.equal(res["exterior"], api.estimate_dtn_exterior(bvh, S, P).cpu())
+        assert res["stats"].n_walks == S.n_s * 48 + 7777
+    assert res["d2h_bytes"] == (int(interior) + int(exterior)) * bvh.V * bvh.V * 4
