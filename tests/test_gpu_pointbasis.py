@@ -10,7 +10,8 @@ torch = pytest.importorskip("torch")
 
 from oracle import Oracle, OracleParams, mesh_geom                            # noqa: E402
 from oracle import PointBasis as OrcPointBasis                                 # noqa: E402
-from synth import fps_samples, icosphere, merge_meshes, stress_mesh, torus, vertex_cell_samples   # noqa: E402
+from synth import (box, fps_samples, icosphere, merge_meshes, stress_mesh, torus, uniform_samples,   # noqa: E402
+                   vertex_cell_samples)
 
 
 @pytest.fixture(scope="module")
@@ -183,3 +184,19 @@ def test_point_basis_matrix_grid_path(api):
                                                       False, smp["tri"], smp["bary"], smp["weight"], want_var=True)
     assert np.linalg.norm(Sg - out["S"]) <= np.linalg.norm(np.sqrt(out["var"]))
     assert np.abs(Sg.sum(1)).max() < 5e-5 * np.abs(Sg).max()
+
+
+def test_point_basis_both_operators_in_one_call(api):
+    """mcs_estimate_dtn_both with the k-NN point basis: the overlapped call equals the two single calls bit for bit."""
+    v, f = merge_meshes([icosphere(3), box((0.7, 0.5, 0.9), (4, 4, 4), center=(2.4, 0.0, 0.1))])[:2]
+    pts, nrm, _ = _points_on(v, f, 300, seed=5)
+    smp = uniform_samples(v, f, 900, seed=6)
+    bvh = api.build_bvh(_cuda(v, torch.float32), _cuda(f, torch.int32))
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    pb = api.PointBasis.from_arrays(pts, nrm, k=8, sigma=0.1, tau_n=0.8)
+    Pi = api.Params(seed=3, walks_per_sample=32, eps=1e-3)
+    Pe = api.Params(seed=3, walks_per_sample=32, eps=1e-3, include_killing=True, n_kill_walks=3000, kelvin_origin=(0.05, 0.0, 0.02))
+    Ai = api.estimate_dtn_interior(bvh, S, Pi, basis=pb).clone()
+    Ae = api.estimate_dtn_exterior(bvh, S, Pe, basis=pb).clone()
+    Bi, Be = api.estimate_dtn_both(bvh, S, Pi, Pe, basis=pb)
+    assert Bi.shape == (300, 300) and torch.equal(Bi, Ai) and torch.equal(Be, Ae)
