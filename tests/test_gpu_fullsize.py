@@ -99,3 +99,22 @@ def test_config1_exterior_full_size(api, cfg1):
     assert 0.95 < lam[0] < 1.02, lam[0]                                         # l + 1 with l = 0
     assert 0.9 < lam[1:4].mean() / 2.0 < 1.01 and lam[1:4].max() - lam[1:4].min() < 0.1, lam[1:4]
     assert 0.9 < lam[4:9].mean() / 3.0 < 1.01, lam[4:9]
+
+
+def test_config1_both_operators_full_size_in_the_configuration_bench_times(api, cfg1):
+    """bench.py's step: mcs_estimate_dtn_both with bench.py's parameters (cap 2.5 deg, killing on, seed 0), the two
+    walk kernels overlapped.  Bit-identical to the single calls checked above and to itself across reruns."""
+    wl, bvh, S, orc = cfg1
+    n_walks = wl["n_s"] * wl["W"]
+    Pi = api.Params(seed=0, walks_per_sample=wl["W"], eps=1e-3, cap_half_angle_deg=2.5)
+    Pe = api.Params(seed=0, walks_per_sample=wl["W"], eps=1e-3, cap_half_angle_deg=2.5, include_killing=True, n_kill_walks=n_walks)
+    Ai = api.estimate_dtn_interior(bvh, S, Pi).clone()
+    Ae = api.estimate_dtn_exterior(bvh, S, Pe).clone()
+    ws = torch.empty(api.workspace_bytes_both(bvh, S, Pi, Pe), dtype=torch.uint8, device="cuda")
+    for _ in range(3):
+        Bi, Be = api.estimate_dtn_both(bvh, S, Pi, Pe, workspace=ws)
+        assert torch.equal(Bi, Ai) and torch.equal(Be, Ae)
+    Sg = Bi.cpu().numpy().astype(np.float64)
+    assert np.abs(Sg.sum(1)).max() < 5e-5 * np.abs(Sg).max()
+    cap = Be.double().sum().item() / (4 * np.pi)
+    assert 0.985 < cap < 1.001, cap
