@@ -579,6 +579,37 @@ def estimate_dtn_coo(bvh: Bvh, samples: Samples, params: Params, exterior: bool,
     raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")
 
 
+def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params,
+                          capacity: int | None = None, max_retries=6):
+    """Interior and exterior DtN matrices in sparse COO form from one mcs_estimate_dtn_both call (walk kernels
+    overlapped).  Same entries as two estimate_dtn_coo calls; one capacity for both, grown on MCS_ENOMEM."""
+    import dataclasses
+    K = bvh.V
+    n_rec = max(num_records(samples, params_interior, False), num_records(samples, params_exterior, True))
+    cap = int(capacity) if capacity else max(4096, min(K * (K + 1) // 2, 4 * n_rec))
+    for _ in range(max_retries):
+        pi = dataclasses.replace(params_interior, output_kind=1, coo_capacity=cap)
+        pe = dataclasses.replace(params_exterior, output_kind=1, coo_capacity=cap)
+        need = workspace_bytes_both(bvh, samples, pi, pe)
+        ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+        bi, be = _coo_buffers(K, cap, bvh.device), _coo_buffers(K, cap, bvh.device)
+        cs, cb, ci, ce = samples.c(), _basis(bvh), pi.c(), pe.c()
+        with torch.cuda.device(bvh.device):
+            rc = lib().mcs_estimate_dtn_both(bvh.handle, C.byref(cs), C.byref(cb), C.byref(ci), C.byref(ce), _ptr(ws),
+                                             C.c_size_t(need), C.byref(bi[4]), C.byref(be[4]), None, None,
+                                             _stream(bvh.device))
+            torch.cuda.current_stream(bvh.device).synchronize()
+        worst = max(int(bi[3].item()), int(be[3].item()))
+        if rc == MCS_ENOMEM and worst > cap:
+            cap = min(K * (K + 1) // 2, max(2 * cap, 2 * worst))
+            del ws, bi, be
+            continue
+        _check(rc, "mcs_estimate_dtn_both (coo)")
+        ni, ne = int(bi[3].item()), int(be[3].item())
+        return (CooMatrix(K, bi[0][:ni], bi[1][:ni], bi[2][:ni]), CooMatrix(K, be[0][:ne], be[1][:ne], be[2][:ne]))
+    raise McsError(MCS_ENOMEM, "estimate_dtn_coo_both", "capacity retries exhausted")
+
+
 def steklov_eigs(S, mass, n_eig, want_vectors=True):
     """Smallest n_eig eigenpairs of S psi = lambda diag(mass) psi (mcs_steklov_eigs).  S: [K,K] or [B,K,K] CUDA fp32;
     mass: [K] or [B,K].  Returns (evals [B,n_eig] or [n_eig], evecs [B,n_eig,K] or [n_eig,K] or None, sweeps)."""

@@ -93,3 +93,22 @@ def test_coo_large_K_against_oracle_on_touched_submesh(api):
     Sg[cc, rr] = vv
     assert np.abs(Sg - So).max() <= 3e-5 * np.abs(So).max()
     assert np.abs(Sg.sum(1)).max() < 5e-5 * np.abs(Sg).max()           # interior operator annihilates constants
+
+
+def test_coo_both_operators_in_one_call_equal_the_single_calls(api):
+    """mcs_estimate_dtn_both with sparse outputs: same lists as two estimate_dtn_coo calls, also after a capacity retry."""
+    v, f = icosphere(3)
+    smp = uniform_samples(v, f, 2001, seed=4)
+    bvh = api.build_bvh(_cuda(v, torch.float32), _cuda(f, torch.int32))
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    Pi = api.Params(seed=6, walks_per_sample=32, eps=1e-3)
+    Pe = api.Params(seed=6, walks_per_sample=32, eps=1e-3, include_killing=True, n_kill_walks=6000, kelvin_origin=(0.1, 0.0, 0.05))
+    ci = api.estimate_dtn_coo(bvh, S, Pi, False)
+    ce = api.estimate_dtn_coo(bvh, S, Pe, True)
+    for cap in (None, 500):
+        bi, be = api.estimate_dtn_coo_both(bvh, S, Pi, Pe, capacity=cap)
+        for a, b in ((bi, ci), (be, ce)):
+            assert torch.equal(a.row, b.row) and torch.equal(a.col, b.col) and torch.equal(a.val, b.val)
+    with pytest.raises(api.McsError) as e:
+        api.estimate_dtn_coo_both(bvh, S, Pi, Pe, capacity=500, max_retries=1)
+    assert e.value.code == api.MCS_ENOMEM
