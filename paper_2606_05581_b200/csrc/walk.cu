@@ -373,6 +373,19 @@ __device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, floa
 enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 
 // ---------------------------------------------------------------------------
+// Pruning limit for a running best squared distance d2 of query p.  A sub-tree is skipped when its box is farther than
+// the limit, so the limit must exceed d2 by more than the error of the COMPUTED triangle distances: otherwise a
+// triangle whose computed distance is the minimum can be skipped after a near-tie has been found first and kept when it
+// comes first, and the result depends on the traversal order -- which differs between the lane path and the
+// warp-cooperative path, i.e. on the schedule (found on the 2 M-face stress mesh: 1 walk in 82 M changed between
+// reruns).  The vertices seen from p carry an absolute rounding error of a few ulp of the coordinates involved, whatever
+// the distance, so the margin is absolute in the DISTANCE: (sqrt(d2) + eta)^2 with eta = 8 eps32 (|p|_1 + mesh scale).
+__device__ __forceinline__ float prune_limit(float d2, float3 p, float scale)
+{
+    const float eta = 9.6e-7f * (fabsf(p.x) + fabsf(p.y) + fabsf(p.z) + scale);
+    return fminf(fmaf(2.0f * eta, sqrtf(d2), d2 * (1.0f + 4e-6f)) + eta * eta, 3.0e38f);
+}
+
 // Warp-cooperative completion of ONE heavy query.  A query that has already visited COOP_MIN nodes
 // (near a medial axis every box is about equally far: hundreds to thousands of nodes) would keep its
 // lane busy for as many passes while the kernel's run time is the longest single-lane chain.  The whole
@@ -410,7 +423,7 @@ struct CoopState {
 
 template <bool COUNT>
 __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, const WideNode* __restrict__ wide,
-                                               const PackedTri* __restrict__ tris, int L, float SLACK,
+                                               const PackedTri* __restrict__ tris, int L, float mesh_scale,
                                                int* __restrict__ co_nodes, int* __restrict__ co_leaves,
                                                int* s_ref, float* s_d, int* l_ref, float* l_d, CoopState* stp)
 {
@@ -470,7 +483,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
             if (md2 < bd2 || (md2 == bd2 && morig < btri)) {
                 bd2 = md2; btri = morig;
                 bk = __shfl_sync(FULL, kk, mlane); bv = __shfl_sync(FULL, v, mlane); bw = __shfl_sync(FULL, w, mlane);
-                wlim = fminf(bd2 * SLACK, 3.0e38f);
+                wlim = prune_limit(bd2, xq, mesh_scale);
             }
             __syncwarp();
         } else {
@@ -617,7 +630,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 const float td2 = closest_point_triangle(xq, T, CUDART_INF_F, tv, tw);
                 if (td2 < h.d2 || (td2 == h.d2 && T.orig < h.tri)) { h.d2 = td2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
                 if (COUNT) ++n_tris;
-                lim = fminf(h.d2 * SLACK, 3.0e38f);
+                lim = prune_limit(h.d2, xq, a.mesh_scale);
                 cur = CUR_NONE;
               } else {
                 if (COUNT) { ++n_nodes; ++q_nodes; }
@@ -646,7 +659,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 const int L = __ffs(heavy) - 1;
                 CoopState cs;
                 cs.xq = xq; cs.h = h; cs.lim = lim; cs.sp = sp; cs.cur = cur; cs.n_nodes = 0; cs.n_tris = 0; cs.q_nodes = 0;
-                coop_finish_query<COUNT>(g.nodes, g.wide, g.tris, L, SLACK, co_nodes, co_leaves,
+                coop_finish_query<COUNT>(g.nodes, g.wide, g.tris, L, a.mesh_scale, co_nodes, co_leaves,
                                          stk.s_ref, stk.s_d, stk.l_ref, stk.l_d, &cs);
                 if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; }
                 if (COUNT) { n_nodes += cs.n_nodes; n_tris += cs.n_tris; q_nodes += cs.q_nodes; }
@@ -656,7 +669,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
             if (kind == KIND_TRI) {
                 test_triangle(g.tris, ~cur, xq, h, lim);
                 if (COUNT) ++n_tris;
-                lim = fminf(h.d2 * SLACK, 3.0e38f);          // finite: an empty slot (box distance +inf) never passes
+                lim = prune_limit(h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
                 cur = CUR_NONE;
             }
         }
@@ -976,6 +989,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.importance = p->importance_sample; a.antithetic = p->antithetic;
     a.naive = p->estimator == 1; a.inv_inset = p->estimator == 1 ? 1.0f / p->inset : 0.0f;
     a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
+    a.mesh_scale = fmaxf(fabsf(lo.x), fabsf(hi.x)) + fmaxf(fabsf(lo.y), fabsf(hi.y)) + fmaxf(fabsf(lo.z), fabsf(hi.z));
     {
         const float dx = hi.x - lo.x, dy = hi.y - lo.y, dz = hi.z - lo.z;
         a.escape = exterior ? 3.0e38f : sqrtf(dx * dx + dy * dy + dz * dz);

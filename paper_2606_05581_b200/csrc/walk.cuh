@@ -31,6 +31,7 @@ struct WalkArgs {
     float inv_inset;
     float eps, q0, inv_q0;
     float ox, oy, oz, Rmax;
+    float mesh_scale;              // |coordinates|_1 bound of the mesh (prune_limit)
     float escape;                  // interior: AABB diagonal (R10b); exterior: +inf
     uint32_t key0, key1;
     float4* records;               // mcs_record viewed as float4
