@@ -10,7 +10,7 @@ constexpr int QT = 128;
 
 __global__ void __launch_bounds__(QT)
 closest_point_kernel(const BvhNode* __restrict__ nodes, const PackedTri* __restrict__ tris,
-                     const float* __restrict__ q, int64_t Q,
+                     const float* __restrict__ q, int64_t Q, float mesh_scale,
                      float* __restrict__ dist, int32_t* __restrict__ tri, float* __restrict__ bary)
 {
     const int64_t i = (int64_t)blockIdx.x * QT + threadIdx.x;
@@ -18,7 +18,7 @@ closest_point_kernel(const BvhNode* __restrict__ nodes, const PackedTri* __restr
     const float3 p = f3(q[3 * i], q[3 * i + 1], q[3 * i + 2]);
     ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = 0.0f; h.w = 0.0f;
     TraversalCounters cnt;
-    bvh_closest_point<false, false>(nodes, tris, p, h, cnt);
+    bvh_closest_point<false, false>(nodes, tris, p, h, cnt, mesh_scale);
     if (dist) dist[i] = sqrtf(h.d2);
     if (tri) tri[i] = h.k >= 0 ? h.tri : -1;
     if (bary) { bary[3 * i] = fmaxf(1.0f - h.v - h.w, 0.0f); bary[3 * i + 1] = h.v; bary[3 * i + 2] = h.w; }
@@ -74,7 +74,9 @@ extern "C" int mcs_closest_point(const mcs_bvh* b, const float* q, int64_t Q,
 {
     if (!b || Q < 0 || (Q > 0 && !q)) return MCS_EINVAL;
     if (Q == 0) return MCS_OK;
-    mcs_note_launch(), closest_point_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->nodes, b->tris, q, Q, dist, tri, bary);
+    float scale = 0.0f;                                // |coordinates|_1 bound of the mesh (prune_limit)
+    for (int d = 0; d < 3; ++d) scale += fmaxf(fabsf(b->aabb_lo[d]), fabsf(b->aabb_hi[d]));
+    mcs_note_launch(), closest_point_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->nodes, b->tris, q, Q, scale, dist, tri, bary);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

@@ -150,6 +150,19 @@ __device__ __forceinline__ float box_dist2(float3 p, float lx, float ly, float l
     return fmaf(dx, dx, fmaf(dy, dy, dz * dz));
 }
 
+// Pruning limit for a running best squared distance d2 of query p.  A sub-tree is skipped when its box is farther than
+// the limit, so the limit must exceed d2 by more than the error of the COMPUTED triangle distances: otherwise a
+// triangle whose computed distance is the minimum can be skipped after a near-tie has been found first and kept when it
+// comes first, and the result depends on the traversal order -- which differs between the lane path and the
+// warp-cooperative path, i.e. on the schedule (found on the 2 M-face stress mesh: 1 walk in 82 M changed between
+// reruns).  The vertices seen from p carry an absolute rounding error of a few ulp of the coordinates involved, whatever
+// the distance, so the margin is absolute in the DISTANCE: (sqrt(d2) + eta)^2 with eta = 8 eps32 (|p|_1 + mesh scale).
+__device__ __forceinline__ float prune_limit(float d2, float3 p, float scale)
+{
+    const float eta = 9.6e-7f * (fabsf(p.x) + fabsf(p.y) + fabsf(p.z) + scale);
+    return fminf(fmaf(2.0f * eta, sqrtf(d2), d2 * (1.0f + 4e-6f)) + eta * eta, 3.0e38f);
+}
+
 // Tests sorted triangle k against the running best h; `lim` = h.d2 with the pruning slack.
 __device__ __forceinline__ void test_triangle(const PackedTri* __restrict__ tris, int k, float3 p, ClosestHit& h, float lim)
 {
@@ -168,19 +181,16 @@ __device__ __forceinline__ void test_triangle(const PackedTri* __restrict__ tris
 // the caller sets h.tri = -1 so that equal distances do not count.
 template <bool COUNT, bool ANY>
 __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ nodes, const PackedTri* __restrict__ tris,
-                                                  float3 p, ClosestHit& h, TraversalCounters& cnt)
+                                                  float3 p, ClosestHit& h, TraversalCounters& cnt, float mesh_scale)
 {
     int   stack_n[MCS_STACK];
     float stack_d[MCS_STACK];
     int sp = 0;
     int node = 0;
     const float bound0 = h.d2;
-    // A sub-tree is pruned when its box is farther than the best distance by more than a
-    // few ulps: the fp32 box distance of a face's own leaf may round above the fp32
-    // distance to the face, and an equal-distance face with a smaller index must still
-    // be reached for the tie rule to hold.
-    const float SLACK = 1.0f + 4e-6f;
-    float lim = h.d2 * SLACK;
+    // A sub-tree is pruned when its box is farther than prune_limit(best): every face that can hold the computed
+    // minimum, or tie with it, is reached, so the result equals the exhaustive minimum under the index tie rule.
+    float lim = prune_limit(h.d2, p, mesh_scale);
     for (;;) {
         const Vec8 n0 = ldg256(nodes + node), n1 = ldg256(reinterpret_cast<const char*>(nodes + node) + 32);
         const float4 w0 = n0.lo, w1 = n0.hi, w2 = n1.lo;
@@ -190,9 +200,9 @@ __device__ __forceinline__ void bvh_closest_point(const BvhNode* __restrict__ no
         const float d1 = box_dist2(p, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w);
         const int c0 = w3.x, c1 = w3.y;
         bool go0 = d0 <= lim, go1 = d1 <= lim;
-        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h, lim); if (COUNT) cnt.tris++; go0 = false; lim = h.d2 * SLACK; }
+        if (go0 && c0 < 0) { test_triangle(tris, ~c0, p, h, lim); if (COUNT) cnt.tris++; go0 = false; lim = prune_limit(h.d2, p, mesh_scale); }
         if (go1 && c1 < 0) {
-            if (d1 <= lim) { test_triangle(tris, ~c1, p, h, lim); if (COUNT) cnt.tris++; lim = h.d2 * SLACK; }
+            if (d1 <= lim) { test_triangle(tris, ~c1, p, h, lim); if (COUNT) cnt.tris++; lim = prune_limit(h.d2, p, mesh_scale); }
             go1 = false;
         }
         if (ANY && h.d2 < bound0) return;

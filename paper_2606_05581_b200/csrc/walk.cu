@@ -373,19 +373,6 @@ __device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, floa
 enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 
 // ---------------------------------------------------------------------------
-// Pruning limit for a running best squared distance d2 of query p.  A sub-tree is skipped when its box is farther than
-// the limit, so the limit must exceed d2 by more than the error of the COMPUTED triangle distances: otherwise a
-// triangle whose computed distance is the minimum can be skipped after a near-tie has been found first and kept when it
-// comes first, and the result depends on the traversal order -- which differs between the lane path and the
-// warp-cooperative path, i.e. on the schedule (found on the 2 M-face stress mesh: 1 walk in 82 M changed between
-// reruns).  The vertices seen from p carry an absolute rounding error of a few ulp of the coordinates involved, whatever
-// the distance, so the margin is absolute in the DISTANCE: (sqrt(d2) + eta)^2 with eta = 8 eps32 (|p|_1 + mesh scale).
-__device__ __forceinline__ float prune_limit(float d2, float3 p, float scale)
-{
-    const float eta = 9.6e-7f * (fabsf(p.x) + fabsf(p.y) + fabsf(p.z) + scale);
-    return fminf(fmaf(2.0f * eta, sqrtf(d2), d2 * (1.0f + 4e-6f)) + eta * eta, 3.0e38f);
-}
-
 // Warp-cooperative completion of ONE heavy query.  A query that has already visited COOP_MIN nodes
 // (near a medial axis every box is about equally far: hundreds to thousands of nodes) would keep its
 // lane busy for as many passes while the kernel's run time is the longest single-lane chain.  The whole
