@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- headline measurement of the Monte Carlo DtN hot path on B200.
 
-One "step" = one pass of the whole hot path over the
-workload BASELINE.json's metric is quoted on (configs[1]): LBVH build of the
-icosphere-L4 mesh, then the interior AND the exterior (killing term on) DtN
-matrices, 2562 vertices x 4096 walks per operator.  Prints ONE JSON line (the
-contract is in DESIGN.md "Measurement").
+BASELINE.json's metric ("walk steps/s and DtN matrices/s on 1 B200; fraction of traversal roofline") names no
+config, so the headline workload is the largest single-GPU one, configs[3]: the seeded 2 M-face in-the-wild stress
+mesh (30 components, 5 % slivers, 1 % duplicated and 2 % flipped faces), 20 000 boundary samples chosen by
+farthest-point sampling, 4096 walks each, interior AND exterior operator, sparse (COO) output in the hat basis.
+One "step" = one pass of the whole hot path over it: LBVH build, sidedness pre-pass
+(winding number), tangent balls, walks and accumulation of both operators.  configs[1] (the
+closed-form sphere case of round 1) and a sample of configs[4] (meshes/s end to end, eigenpairs included) are
+measured in the same run and reported as sub-records of the same JSON line.  Prints ONE JSON line.
 
   python bench.py                       # N=1, this repo's CUDA path
-  python bench.py --impl reference      # the CPU oracle, as it stands, on a bounded sample
+  python bench.py --impl reference      # the CPU oracle, as it stands, on a bounded sample of the same workload
   torchrun ... bench.py --gpus N        # N independent replicas
 """
 from __future__ import annotations
@@ -18,6 +21,7 @@ import json
 import os
 import subprocess
 import sys
+import tempfile
 import threading
 import time
 
@@ -32,27 +36,65 @@ UNIT = "walk steps/s"
 
 
 # ------------------------------------------------------------------------------
-# workload = BASELINE.json configs[1]
+# workloads (seeded synthetic stand-ins)
 # ------------------------------------------------------------------------------
-def make_workload(level: int, walks_per_vertex: int, points_per_vertex: int, seed: int):
+def _cache_dir():
+    d = os.path.join(tempfile.gettempdir(), "mcdtn_bench_cache")
+    os.makedirs(d, exist_ok=True)
+    return d
+
+
+def make_cfg3(args):
+    """configs[3]: stress mesh + FPS samples + Kelvin origin.  Generated once per box (a few seconds) and kept as an
+    .npz in the temp directory; always outside the timed region."""
+    from synth import fps_samples, stress_mesh
+    tag = f"cfg3_F{args.faces}_C{args.components}_S{args.samples}_N{args.candidates}_seed{args.mesh_seed}.npz"
+    path = os.path.join(_cache_dir(), tag)
+    if os.path.exists(path) and not args.no_cache:
+        try:
+            z = np.load(path)
+            return dict(v=z["v"], f=z["f"], tri=z["tri"], bary=z["bary"], weight=z["weight"], origin=tuple(float(x) for x in z["origin"]),
+                        n_components=int(z["n_components"]), flipped=float(z["flipped"]), sliver=float(z["sliver"]), dup=float(z["dup"]))
+        except Exception:
+            pass
+    v, f, info = stress_mesh(n_faces=args.faces, n_components=args.components, seed=args.mesh_seed)
+    smp = fps_samples(v, f, args.samples, n_candidates=args.candidates, seed=args.mesh_seed)
+    # Kelvin origin strictly inside the solid (PAPER.md:335): the centre of the component with the most faces
+    comp = int(np.bincount(info["face_component"]).argmax())
+    cv = v[np.unique(f[info["face_component"] == comp])]
+    origin = tuple(float(x) for x in 0.5 * (cv.min(0) + cv.max(0)))
+    wl = dict(v=v, f=f, tri=smp["tri"], bary=smp["bary"], weight=smp["weight"], origin=origin,
+              n_components=int(info["n_components"]), flipped=float(info["flipped"].mean()),
+              sliver=float(info["sliver"].mean()), dup=float(info["duplicate"].mean()))
+    try:
+        np.savez(path, **{k: np.asarray(x) for k, x in wl.items()})
+    except OSError:
+        pass
+    return wl
+
+
+def cfg3_config(wl, args, extra=None):
+    V, F, n_s = len(wl["v"]), len(wl["f"]), len(wl["tri"])
+    c = {"workload": f"configs[3]: stress mesh seed {args.mesh_seed} ({V} vertices, {F} faces, {wl['n_components']} components, "
+                     f"{100 * wl['sliver']:.1f}% slivers, {100 * wl['dup']:.1f}% duplicated, {100 * wl['flipped']:.1f}% flipped faces), "
+                     f"{n_s} FPS samples of {args.candidates} candidates x {args.walks} walks per operator, interior + exterior "
+                     f"(killing off: the paper's default, PAPER.md:383), sidedness pre-pass, hat basis, sparse COO output, "
+                     f"eps={args.eps:g}, cap={args.cap:g} deg, Philox seed {args.seed}",
+         "operators": ["interior", "exterior"], "walks_per_operator": n_s * args.walks,
+         "includes_bvh_build": True, "includes_sidedness_prepass": True, "output": "coo (upper triangle)",
+         "l2_policy": "inputs larger than L2 (tree 256 MB + records 2.6 GB per step) and a 256 MiB buffer written between timed steps",
+         "parallelism": "replicas" if args.gpus > 1 else "single"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def make_cfg1(level=4, walks_per_vertex=4096, points_per_vertex=16, seed=0):
     from synth import icosphere, vertex_cell_samples
     v, f = icosphere(level)
     smp = vertex_cell_samples(v, f, points_per_vertex, seed=seed)
     W = walks_per_vertex // points_per_vertex
     return dict(v=v, f=f, smp=smp, W=W, name=f"icosphere_L{level}", V=len(v), F=len(f), n_s=len(smp["tri"]))
-
-
-def config_dict(wl, args, extra=None):
-    c = {"workload": f"configs[1]: {wl['name']} ({wl['V']} vertices, {wl['F']} faces), interior + exterior(killing on) "
-                     f"DtN, hat basis, {args.walks_per_vertex} walks/vertex = {wl['n_s']} sample points x {wl['W']} walks "
-                     f"per operator, eps={args.eps:g}, cap={args.cap:g} deg, Philox seed {args.seed}",
-         "operators": ["interior", "exterior+killing"], "walks_per_operator": wl["n_s"] * wl["W"],
-         "kill_walks": wl["n_s"] * wl["W"], "includes_bvh_build": True,
-         "l2_policy": "256 MiB buffer written between timed steps (L2 flush); the 0.6 MB tree is re-read from HBM/L2 each step",
-         "parallelism": "replicas" if args.gpus > 1 else "single"}
-    if extra:
-        c.update(extra)
-    return c
 
 
 # ------------------------------------------------------------------------------
@@ -79,6 +121,7 @@ class ClockSampler:
         except OSError:
             self.proc = None
             return
+
         def pump():
             for line in self.proc.stdout:
                 self.rows.append(line.strip())
@@ -112,9 +155,10 @@ class ClockSampler:
                 "power_w_max": float(max(power)), "samples": len(sm)}
 
 
-def read_traffic():
-    """DRAM bytes of the walk-kernel launches of one step, from the committed ncu capture (profiles/)."""
-    path = os.path.join(ROOT, "profiles", "walk_kernel_traffic.csv")
+def read_traffic(name):
+    """DRAM bytes (read + write) of the walk-kernel launches of one step, from the committed ncu capture under
+    profiles/ (a csv of kernel, dram_read_bytes, dram_write_bytes); None when there is no capture."""
+    path = os.path.join(ROOT, "profiles", name)
     if not os.path.exists(path):
         return None
     total = 0
@@ -138,28 +182,29 @@ def read_peaks():
 # ------------------------------------------------------------------------------
 # the CPU oracle on a bounded sample of the same workload (cpu_baseline / --impl reference)
 # ------------------------------------------------------------------------------
-def oracle_sample_run(wl, args, n_samples: int):
-    """Runs interior + exterior(killing) through oracle/ on every (n_s // n_samples)-th sample point.
-    Returns (walk steps, seconds, cores, description)."""
+def oracle_sample_cfg3(wl, args, n_samples: int, n_walks: int):
+    """Interior + exterior walks of `n_walks` walks of every (n_s // n_samples)-th sample point through oracle/
+    (brute-force fp64 closest point over all faces; same Philox counters as the full run), then the oracle's
+    accumulation of those records.  Returns (walk steps, seconds, cores, description)."""
     from oracle import Oracle, OracleParams, mesh_geom
-    smp = wl["smp"]
-    stride = max(1, wl["n_s"] // n_samples)
-    idx = np.arange(0, wl["n_s"], stride)[:n_samples]
-    tri, bary, wgt = smp["tri"][idx], smp["bary"][idx], smp["weight"][idx]
+    n_s = len(wl["tri"])
+    stride = max(1, n_s // n_samples)
+    ids = np.arange(0, n_s, stride)[:n_samples]
     orc = Oracle(mesh_geom(wl["v"], wl["f"]))
     steps = 0
     t0 = time.perf_counter()
+    nrm, _ = orc.orient_samples(wl["tri"][ids], wl["bary"][ids])            # the sidedness pre-pass, on the sample
+    normal = np.zeros((n_s, 3), np.float32)
+    normal[ids] = nrm
     for ext in (False, True):
-        n_walks = len(idx) * wl["W"]
-        p = OracleParams(seed=args.seed, walks_per_sample=wl["W"], eps=args.eps, cap_half_angle_deg=args.cap,
-                         include_killing=ext, n_kill_walks=n_walks if ext else 0)
-        res = orc.estimate_dtn(p, ext, tri, bary, wgt)
-        st = res["records"]["steps"]
+        p = OracleParams(seed=args.seed, walks_per_sample=args.walks, eps=args.eps, cap_half_angle_deg=args.cap,
+                         origin=wl["origin"])
+        rec = orc.run_walks_subset(p, ext, wl["tri"], wl["bary"], wl["weight"], ids, n_walks, normal=normal)
+        st = rec["steps"]
         steps += int(st[st > 0].sum())
     dt = time.perf_counter() - t0
-    desc = (f"{len(idx)} of {wl['n_s']} sample points (every {stride}th) x {wl['W']} walks, interior + exterior "
-            f"(+ {len(idx) * wl['W']} killing walks), brute-force fp64 closest point over {wl['F']} faces, then the dense "
-            f"hat-basis accumulation")
+    desc = (f"{len(ids)} of {n_s} sample points (every {stride}th) x {n_walks} of {args.walks} walks, interior + exterior, "
+            f"sidedness by the oracle's winding number on those points, brute-force fp64 closest point over {len(wl['f'])} faces")
     return steps, dt, orc.num_threads, desc
 
 
@@ -167,19 +212,19 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    wl = make_workload(args.level, args.walks_per_vertex, args.points_per_vertex, args.seed)
+    wl = make_cfg3(args)
     for _ in range(args.warmup):
-        oracle_sample_run(wl, args, max(1, args.ref_samples // 8))
+        oracle_sample_cfg3(wl, args, 2, 2)
     total_steps, total_t, cores, desc = 0, 0.0, 0, ""
     for _ in range(args.steps):
-        s, dt, cores, desc = oracle_sample_run(wl, args, args.ref_samples)
+        s, dt, cores, desc = oracle_sample_cfg3(wl, args, args.ref_samples, args.ref_walks)
         total_steps += s
         total_t += dt
     value = total_steps / total_t
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(wl, args, {"reference_sample": desc}),
+            "config": cfg3_config(wl, args),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -222,6 +267,189 @@ def whole_job_value(units_per_rank_step: float, world: int, seconds_per_step: fl
 
 
 # ------------------------------------------------------------------------------
+# roofline of the walk kernel from its own node / triangle counts
+# ------------------------------------------------------------------------------
+def walk_roofline(stats, t_kernel_s, level_gbs, level, fp32_tflops, note, tri_bytes=48.0):
+    nodes = tris = queries = 0.0
+    per = {}
+    for name, st in stats.items():
+        n = st.n_nodes_visited - st.n_prep_nodes
+        t = st.n_tris_tested - st.n_prep_tris
+        q = st.n_queries - st.n_prep_queries
+        per[name] = dict(nodes_per_query=n / max(q, 1), tris_per_query=t / max(q, 1))
+        nodes += n; tris += t; queries += q
+    flops = 72.0 * nodes + 80.0 * tris              # 4-wide nodes: four 18-flop box tests per visit
+    nbytes = 128.0 * nodes + tri_bytes * tris
+    t_mem, t_alu = nbytes / (level_gbs * 1e9), flops / (fp32_tflops * 1e12)
+    mem_bound = t_mem >= t_alu
+    return {
+        "kernel": note,
+        "bound": level if mem_bound else "alu",
+        "achieved": (nbytes / t_kernel_s / 1e9) if mem_bound else (flops / t_kernel_s / 1e12),
+        "peak": level_gbs if mem_bound else fp32_tflops,
+        "unit": "GB/s" if mem_bound else "TFLOP/s",
+        "frac": max(t_mem, t_alu) / t_kernel_s,
+        "algorithmic": "bytes = 128 B x 4-wide nodes visited + 48 B x triangles tested; flops = 72 x nodes + 80 x triangles (DESIGN.md section 6)",
+        "alu_frac": t_alu / t_kernel_s, "mem_frac": t_mem / t_kernel_s,
+        "kernel_ms_per_step": t_kernel_s * 1e3,
+        "nodes_per_query": {k: per[k]["nodes_per_query"] for k in per},
+        "tris_per_query": {k: per[k]["tris_per_query"] for k in per},
+        "algorithmic_bytes_per_step": nbytes, "algorithmic_flops_per_step": flops,
+    }
+
+
+# ------------------------------------------------------------------------------
+# sub-record: configs[1] (icosphere L4, dense output, killing on) -- round 1's headline, kept for continuity
+# ------------------------------------------------------------------------------
+def bench_cfg1(api, torch, dev, args, seed, steps, warmup, flush, fp32_tflops, l2_gbs):
+    wl = make_cfg1()
+    n_walks = wl["n_s"] * wl["W"]
+    v_h, f_h = torch.as_tensor(wl["v"]).pin_memory(), torch.as_tensor(wl["f"]).pin_memory()
+    tri_h, bary_h = torch.as_tensor(wl["smp"]["tri"]).pin_memory(), torch.as_tensor(wl["smp"]["bary"]).pin_memory()
+    w_h = torch.as_tensor(wl["smp"]["weight"]).pin_memory()
+    vd, fd = v_h.to(dev), f_h.to(dev)
+    S = api.Samples(tri_h.to(dev), bary_h.to(dev), w_h.to(dev))
+    P_int = api.Params(seed=seed, walks_per_sample=wl["W"], eps=1e-3, cap_half_angle_deg=2.5)
+    P_ext = api.Params(seed=seed, walks_per_sample=wl["W"], eps=1e-3, cap_half_angle_deg=2.5, include_killing=True, n_kill_walks=n_walks)
+    bvh0 = api.build_bvh(vd, fd)
+    ws = torch.empty(api.workspace_bytes_both(bvh0, S, P_int, P_ext), dtype=torch.uint8, device=dev)
+    out_int = torch.empty((wl["V"], wl["V"]), dtype=torch.float32, device=dev)
+    out_ext = torch.empty_like(out_int)
+    _, st_i = api.estimate_dtn_interior(bvh0, S, P_int, want_stats=True, out=out_int, workspace=ws)
+    _, st_e = api.estimate_dtn_exterior(bvh0, S, P_ext, want_stats=True, out=out_ext, workspace=ws)
+    del bvh0
+    phases = []
+
+    def step(profile):
+        bvh = api.build_bvh(vd, fd)
+        api.estimate_dtn_both(bvh, S, P_int, P_ext, out_interior=out_int, out_exterior=out_ext, workspace=ws)
+        if profile:
+            phases.append(api.profile_last())
+
+    for _ in range(warmup):
+        step(False); flush.fill_(1)
+    api.profile_enable(True)
+    stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    l0 = api.launch_count()
+    e0.record(stream)
+    for _ in range(steps):
+        step(True); flush.fill_(1)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    launches = api.launch_count() - l0
+    api.profile_enable(False)
+    ms = e0.elapsed_time(e1) / steps
+    walk_steps = st_i.n_steps + st_e.n_steps
+    t_kernel = float(np.mean([p.walk_ms for p in phases])) * 1e-3
+    roof = walk_roofline({"interior": st_i, "exterior": st_e}, t_kernel, l2_gbs, "l2", fp32_tflops,
+                         "walk_kernel (interior + exterior launch of one step, overlapped: span of both)")
+    roof["peak_source"] = "L2 read bandwidth measured live by mcs_measure_l2_gbs (the 0.6 MB tree is L2-resident)"
+    roof["traffic"] = read_traffic("walk_kernel_traffic.csv")
+    # end to end through the host entry point (dense matrices back to pinned host memory)
+    oi_h = torch.empty((wl["V"], wl["V"]), dtype=torch.float32, pin_memory=True)
+    oe_h = torch.empty_like(oi_h).pin_memory()
+    for _ in range(4):
+        r = api.estimate_dtn_host(v_h, f_h, tri_h, bary_h, w_h, P_ext, out_interior=oi_h, out_exterior=oe_h, device=dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    n_e2e = max(1, min(steps, 5))
+    for _ in range(n_e2e):
+        r = api.estimate_dtn_host(v_h, f_h, tri_h, bary_h, w_h, P_ext, out_interior=oi_h, out_exterior=oe_h, device=dev)
+        flush.fill_(1)
+    torch.cuda.synchronize()
+    e2e_t = (time.perf_counter() - t0) / n_e2e
+    return {"workload": f"configs[1]: {wl['name']} ({wl['V']} vertices, {wl['F']} faces), interior + exterior(killing on), hat basis, dense "
+                        f"output, 4096 walks/vertex = {wl['n_s']} sample points x {wl['W']} walks per operator, eps=1e-3, cap=2.5 deg",
+            "metric": METRIC, "value": walk_steps / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps, "warmup": warmup,
+            "dtn_matrices_per_s": 2.0 / (ms * 1e-3), "walk_steps_per_step": walk_steps,
+            "queries_per_s": (st_i.n_queries + st_e.n_queries) / (ms * 1e-3),
+            "phase_ms_per_step": {"prep": float(np.mean([p.prep_ms for p in phases])), "walk": t_kernel * 1e3,
+                                  "accumulate": float(np.mean([p.accumulate_ms for p in phases]))},
+            "e2e": {"value": walk_steps / e2e_t, "unit": UNIT, "ms_per_step": e2e_t * 1e3, "h2d_bytes_per_step": r["h2d_bytes"],
+                    "d2h_bytes_per_step": r["d2h_bytes"], "call": "mcs_estimate_dtn_host (pinned host buffers)"},
+            "gpu_launches": launches, "roofline": roof}
+
+
+# ------------------------------------------------------------------------------
+# sub-record: a sample of configs[4] (meshes/s end to end: build, sidedness, both operators, top-64 eigenpairs)
+# ------------------------------------------------------------------------------
+def make_cfg4_sample(n_meshes, seed0=0):
+    """Meshes seeds seed0.. of BASELINE configs[4]: faces log-uniform in [5k, 200k], 1-50 components, stress style;
+    512 FPS samples that are also the nodes of the k-NN point basis (R3)."""
+    from synth import fps_samples, stress_mesh
+    out = []
+    for s in range(seed0, seed0 + n_meshes):
+        rng = np.random.default_rng(10_000 + s)
+        n_faces = int(round(np.exp(rng.uniform(np.log(5_000), np.log(200_000)))))
+        n_comp = int(rng.integers(1, 51))
+        v, f, info = stress_mesh(n_faces=n_faces, n_components=n_comp, seed=s)
+        smp = fps_samples(v, f, 512, n_candidates=20_000, seed=s)
+        comp = int(np.bincount(info["face_component"]).argmax())
+        cv = v[np.unique(f[info["face_component"] == comp])]
+        origin = tuple(float(x) for x in 0.5 * (cv.min(0) + cv.max(0)))
+        a, b, c = v[f[smp["tri"], 0]], v[f[smp["tri"], 1]], v[f[smp["tri"], 2]]
+        pts = (smp["bary"][:, 0:1] * a + smp["bary"][:, 1:2] * b + smp["bary"][:, 2:3] * c).astype(np.float32)
+        out.append(dict(v=v, f=f, tri=smp["tri"], bary=smp["bary"], weight=smp["weight"], pts=pts, origin=origin, seed=s))
+    return out
+
+
+def bench_cfg4_sample(api, torch, dev, args, seed, n_meshes, flush):
+    meshes = make_cfg4_sample(n_meshes)
+    W, n_eig = 1024, 64
+    pinned = [{k: torch.as_tensor(m[k]).pin_memory() for k in ("v", "f", "tri", "bary", "weight", "pts")} for m in meshes]
+    Si = torch.empty((n_meshes, 512, 512), dtype=torch.float32, device=dev)
+    Se = torch.empty_like(Si)
+    mass = torch.empty((n_meshes, 512), dtype=torch.float32, device=dev)
+    total_steps = 0
+
+    def one_pass(count):
+        nonlocal total_steps
+        for i, (m, h) in enumerate(zip(meshes, pinned)):
+            vd, fd = h["v"].to(dev, non_blocking=True), h["f"].to(dev, non_blocking=True)
+            S0 = api.Samples(h["tri"].to(dev, non_blocking=True), h["bary"].to(dev, non_blocking=True), h["weight"].to(dev, non_blocking=True))
+            pts = h["pts"].to(dev, non_blocking=True)
+            bvh = api.build_bvh(vd, fd)
+            nrm, _ = api.orient_samples(bvh, S0)
+            S = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
+            basis = api.PointBasis(pts, nrm, k=8, sigma=0.025, tau_n=0.8)
+            Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3)
+            Pe = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, kelvin_origin=m["origin"])
+            if count:
+                _, _, sti, ste = api.estimate_dtn_both(bvh, S, Pi, Pe, want_stats=True, out_interior=Si[i], out_exterior=Se[i], basis=basis)
+                total_steps += sti.n_steps + ste.n_steps
+            else:
+                api.estimate_dtn_both(bvh, S, Pi, Pe, out_interior=Si[i], out_exterior=Se[i], basis=basis)
+            mass[i] = S0.weight
+        # Steklov eigenpairs of all matrices of the pass in two batched calls (lumped mass = the samples' weights)
+        ei, _, _ = api.steklov_eigs(Si, mass, n_eig)
+        ee, _, _ = api.steklov_eigs(Se, mass, n_eig)
+        return ei, ee
+
+    one_pass(True)                                  # warm-up, and the deterministic step counts
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = api.launch_count()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    one_pass(False)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    ms = e0.elapsed_time(e1)
+    faces = [len(m["f"]) for m in meshes]
+    return {"workload": f"configs[4] sample: {n_meshes} stress-style meshes (seeds 0..{n_meshes - 1}, {min(faces)}-{max(faces)} faces), per mesh: "
+                        f"upload from pinned host memory, LBVH build, sidedness pre-pass, 512 FPS samples = nodes of the k-NN point basis "
+                        f"(k=8), {W} walks per sample, interior + exterior (killing off), then top-{n_eig} Steklov eigenpairs of all "
+                        f"{2 * n_meshes} matrices in two batched calls",
+            "metric": "meshes_per_s", "value": n_meshes / (ms * 1e-3), "unit": "meshes/s", "ms_per_mesh": ms / n_meshes,
+            "wall_ms_per_mesh": wall * 1e3 / n_meshes, "walk_steps_per_s": total_steps / (ms * 1e-3),
+            "gpu_launches": api.launch_count() - l0, "meshes": n_meshes, "mean_faces": float(np.mean(faces))}
+
+
+# ------------------------------------------------------------------------------
 # this repo's CUDA path
 # ------------------------------------------------------------------------------
 def run_ours(args):
@@ -242,49 +470,40 @@ def run_ours(args):
 
     # replicas only: rank r runs the same workload with Philox seed + r
     seed = replica_seed(args.seed, rank)
-    wl = make_workload(args.level, args.walks_per_vertex, args.points_per_vertex, args.seed)
-    n_walks = wl["n_s"] * wl["W"]
-    v_h = torch.as_tensor(wl["v"]).pin_memory()
-    f_h = torch.as_tensor(wl["f"]).pin_memory()
-    tri_h = torch.as_tensor(wl["smp"]["tri"]).pin_memory()
-    bary_h = torch.as_tensor(wl["smp"]["bary"]).pin_memory()
-    w_h = torch.as_tensor(wl["smp"]["weight"]).pin_memory()
+    wl = make_cfg3(args)
+    V, F, n_s, W = len(wl["v"]), len(wl["f"]), len(wl["tri"]), args.walks
+    v_h, f_h = torch.as_tensor(wl["v"]).pin_memory(), torch.as_tensor(wl["f"]).pin_memory()
+    tri_h, bary_h, w_h = (torch.as_tensor(wl[k]).pin_memory() for k in ("tri", "bary", "weight"))
     vd, fd = v_h.to(dev), f_h.to(dev)
-    S = api.Samples(tri_h.to(dev), bary_h.to(dev), w_h.to(dev))
-    P_int = api.Params(seed=seed, walks_per_sample=wl["W"], eps=args.eps, cap_half_angle_deg=args.cap)
-    P_ext = api.Params(seed=seed, walks_per_sample=wl["W"], eps=args.eps, cap_half_angle_deg=args.cap,
-                       include_killing=True, n_kill_walks=n_walks)
-    bvh0 = api.build_bvh(vd, fd)
-    ws_bytes = max(api.workspace_bytes(bvh0, S, P_int, False), api.workspace_bytes(bvh0, S, P_ext, True),
-                   api.workspace_bytes_both(bvh0, S, P_int, P_ext))
-    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
-    out_int = torch.empty((wl["V"], wl["V"]), dtype=torch.float32, device=dev)
-    out_ext = torch.empty_like(out_int)
+    S0 = api.Samples(tri_h.to(dev), bary_h.to(dev), w_h.to(dev))
+    P_int = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap)
+    P_ext = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, kelvin_origin=wl["origin"])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
-    # deterministic work counts of one step (counter build of the kernels; outside the timed region)
-    _, st_i = api.estimate_dtn_interior(bvh0, S, P_int, want_stats=True, out=out_int, workspace=ws)
-    _, st_e = api.estimate_dtn_exterior(bvh0, S, P_ext, want_stats=True, out=out_ext, workspace=ws)
+    # deterministic work counts of one step (counter build of the kernels) and the size of the sparse outputs;
+    # outside the timed region
+    bvh0 = api.build_bvh(vd, fd)
+    info = bvh0.info()
+    nrm0, _ = api.orient_samples(bvh0, S0)
+    S = api.Samples(S0.tri, S0.bary, S0.weight, nrm0)
+    ci, st_i = api.estimate_dtn_coo(bvh0, S, P_int, False, want_stats=True)
+    ce, st_e = api.estimate_dtn_coo(bvh0, S, P_ext, True, want_stats=True)
+    nnz = (ci.nnz, ce.nnz)
+    cap = int(max(nnz) * 1.02) + 4096
+    del ci, ce, bvh0, S, nrm0
+    torch.cuda.empty_cache()
     steps_per_step = st_i.n_steps + st_e.n_steps
     queries_per_step = st_i.n_queries + st_e.n_queries
-    del bvh0
-
     phases = []
 
     def step(profile):
         bvh = api.build_bvh(vd, fd)
-        if not args.serial:
-            # one call for both operators: the two walk kernels overlap on two streams
-            api.estimate_dtn_both(bvh, S, P_int, P_ext, out_interior=out_int, out_exterior=out_ext, workspace=ws)
-            if profile:
-                phases.append(("both", api.profile_last()))
-            return
-        api.estimate_dtn_interior(bvh, S, P_int, out=out_int, workspace=ws)
+        nrm, _ = api.orient_samples(bvh, S0)
+        Sx = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
+        out = api.estimate_dtn_coo_both(bvh, Sx, P_int, P_ext, capacity=cap)
         if profile:
-            phases.append(("interior", api.profile_last()))
-        api.estimate_dtn_exterior(bvh, S, P_ext, out=out_ext, workspace=ws)
-        if profile:
-            phases.append(("exterior", api.profile_last()))
+            phases.append(api.profile_last())
+        return out
 
     def barrier():
         if world > 1:
@@ -317,103 +536,81 @@ def run_ours(args):
     job_steps = sum_over_ranks(steps_per_step, dev, world)        # replicas differ by their Philox seed
     job_queries = sum_over_ranks(queries_per_step, dev, world)
     value = job_steps / (ms_per_step * 1e-3)
+    torch.cuda.empty_cache()
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    oi_h = torch.empty((wl["V"], wl["V"]), dtype=torch.float32, pin_memory=True)
-    oe_h = torch.empty_like(oi_h).pin_memory()
-    e2e_steps = max(1, min(args.steps, 10))
-    # warm-up: the device idles while nvidia-smi is stopped and the host buffers are pinned, and the first ~0.3 s of
-    # calls after that ran 6 % slower than the following ones (measured per call: 51.6, 51.6, 51.5, 48.4 ms)
-    for _ in range(max(args.warmup, 8)):
-        r = api.estimate_dtn_host(v_h, f_h, tri_h, bary_h, w_h, P_ext, out_interior=oi_h, out_exterior=oe_h, device=dev)
+    host_out = [tuple(torch.empty(cap, dtype=dt, pin_memory=True) for dt in (torch.int32, torch.int32, torch.float32)) for _ in range(2)]
+    e2e_steps = max(1, min(args.steps, 3))
+    for _ in range(2):
+        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, device=dev)
     barrier()
     t0 = time.perf_counter()
     e2e_each = []
     for _ in range(e2e_steps):
-        # one call runs interior (killing flag ignored there) and exterior on one upload of the mesh
         tc = time.perf_counter()
-        r = api.estimate_dtn_host(v_h, f_h, tri_h, bary_h, w_h, P_ext, out_interior=oi_h, out_exterior=oe_h, device=dev)
-        e2e_each.append((time.perf_counter() - tc) * 1e3)      # the call blocks until the matrices are in host memory
+        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, device=dev)
+        e2e_each.append((time.perf_counter() - tc) * 1e3)      # the call blocks until the entries are in host memory
         flush.fill_(1)
     barrier()
     e2e_t = (time.perf_counter() - t0) / e2e_steps
     e2e_t = max_over_ranks(e2e_t, dev, world)
     e2e_value = job_steps / e2e_t
+    del host_out
+    torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (the persistent walk kernel), DESIGN.md "Roofline"
-    walk_ms = {"interior": [], "exterior": [], "both": []}
-    prep_ms, acc_ms = [], []
-    for name, ph in phases:
-        walk_ms[name].append(ph.walk_ms)
-        prep_ms.append(ph.prep_ms)
-        acc_ms.append(ph.accumulate_ms)
+    # ---- roofline of the dominant kernel (the persistent walk kernel)
     fp32_tflops = api.measure_fp32_tflops(dev)
     l2_gbs = api.measure_l2_gbs(dev)
     hbm_gbs, hbm_src = read_peaks()
-    tree_bytes = 64 * (wl["F"] - 1) + 48 * wl["F"]
-    level_gbs, level = (l2_gbs, "l2") if tree_bytes < 100e6 else (hbm_gbs, "hbm")
-    roof = {}
-    for name, st in (("interior", st_i), ("exterior", st_e)):
-        t = float(np.mean(walk_ms[name])) * 1e-3 if args.serial else 0.0
-        # walk kernel only: the tangent-ball traversals (A2) are counted separately
-        nodes, tris = st.n_nodes_visited - st.n_prep_nodes, st.n_tris_tested - st.n_prep_tris
-        queries = st.n_queries - st.n_prep_queries
-        flops = 72.0 * nodes + 80.0 * tris          # 4-wide nodes: four 18-flop box tests per visit
-        nbytes = 128.0 * nodes + 48.0 * tris
-        t_alu, t_mem = flops / (fp32_tflops * 1e12), nbytes / (level_gbs * 1e9)
-        roof[name] = dict(t=t, flops=flops, bytes=nbytes, t_alu=t_alu, t_mem=t_mem,
-                          nodes_per_query=nodes / queries, tris_per_query=tris / queries)
-    # overlapped launches: the denominator is the span from the interior kernel's start to the exterior kernel's
-    # end (events on the two streams), which also holds whatever else ran in that span
-    t_kernel = roof["interior"]["t"] + roof["exterior"]["t"] if args.serial else float(np.mean(walk_ms["both"])) * 1e-3
-    nbytes = roof["interior"]["bytes"] + roof["exterior"]["bytes"]
-    flops = roof["interior"]["flops"] + roof["exterior"]["flops"]
-    t_mem = nbytes / (level_gbs * 1e9)
-    t_alu = flops / (fp32_tflops * 1e12)
-    mem_bound = t_mem >= t_alu
-    roofline = {
-        "kernel": "walk_kernel (interior launch + exterior launch of one step" + (")" if args.serial else ", overlapped on two streams: span of both)"),
-        "bound": level if mem_bound else "alu",
-        "achieved": (nbytes / t_kernel / 1e9) if mem_bound else (flops / t_kernel / 1e12),
-        "peak": level_gbs if mem_bound else fp32_tflops,
-        "unit": "GB/s" if mem_bound else "TFLOP/s",
-        "frac": max(t_mem, t_alu) / t_kernel,
-        "traffic": read_traffic(),
-        "traffic_note": "dram bytes read+write of the two walk_kernel launches of one step (ncu --set full, profiles/walk_kernel_traffic.csv); algorithmic node+triangle bytes are served from L2",
-        "peak_source": (f"{level} read bandwidth measured live by mcs_measure_l2_gbs (tree is {tree_bytes / 1e6:.2f} MB, "
-                        f"{level}-resident); HBM {hbm_gbs:.0f} GB/s {hbm_src}; FP32 {fp32_tflops:.1f} TFLOP/s measured live"),
-        "algorithmic": "bytes = 128 B x 4-wide nodes visited + 48 B x triangles tested; flops = 72 x nodes + 80 x triangles (DESIGN.md)",
-        "alu_frac": t_alu / t_kernel, "mem_frac": t_mem / t_kernel,
-        "kernel_ms_per_step": t_kernel * 1e3, "kernel_share_of_step": t_kernel * 1e3 / ms_per_step,
-        "nodes_per_query": {k: roof[k]["nodes_per_query"] for k in roof},
-        "tris_per_query": {k: roof[k]["tris_per_query"] for k in roof},
-    }
+    tree_bytes = int(info.device_bytes)
+    t_kernel = float(np.mean([p.walk_ms for p in phases])) * 1e-3
+    roofline = walk_roofline({"interior": st_i, "exterior": st_e}, t_kernel, hbm_gbs, "hbm", fp32_tflops,
+                             "walk_kernel (interior launch + exterior launch of one step, overlapped on two streams: span of both)")
+    roofline["peak_source"] = (f"HBM {hbm_gbs:.0f} GB/s {hbm_src}: packed tree + triangles are {tree_bytes / 1e6:.0f} MB > L2; "
+                               f"FP32 {fp32_tflops:.1f} TFLOP/s and L2 {l2_gbs:.0f} GB/s measured live")
+    roofline["l2_frac"] = roofline["algorithmic_bytes_per_step"] / (l2_gbs * 1e9) / t_kernel
+    roofline["traffic"] = read_traffic("r02_cfg3_walk_traffic.csv")
+    roofline["traffic_note"] = "dram bytes read+write of the two walk_kernel launches of one step (ncu --set full, profiles/r02_cfg3_walk_traffic.csv)"
+    roofline["kernel_share_of_step"] = t_kernel * 1e3 / ms_per_step
+    cut = (st_i.n_truncated + st_e.n_truncated) / float(st_i.n_walks + st_e.n_walks)
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        s, dt, cores, desc = oracle_sample_run(wl, args, args.cpu_samples)
+        s, dt, cores, desc = oracle_sample_cfg3(wl, args, args.cpu_samples, args.cpu_walks)
         cpu = {"value": s / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
+
+    sub = {}
+    if world == 1 and not args.no_sub:
+        sub["configs[1]"] = bench_cfg1(api, torch, dev, args, seed, min(args.steps, 5), 3, flush, fp32_tflops, l2_gbs)
+        sub["configs[4] sample"] = bench_cfg4_sample(api, torch, dev, args, seed, args.cfg4_meshes, flush)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic", "config": config_dict(wl, args),
+            "dtype": "f32", "data": "synthetic", "config": cfg3_config(wl, args),
             "queries_per_s": job_queries / (ms_per_step * 1e-3),
             "dtn_matrices_per_s": world * 2.0 / (ms_per_step * 1e-3),
             "walk_steps_per_step": steps_per_step, "queries_per_step": queries_per_step,
-            "call": "mcs_build_bvh + " + ("mcs_estimate_dtn_interior + mcs_estimate_dtn_exterior" if args.serial else "mcs_estimate_dtn_both"),
-            "phase_ms_per_step": {"prep": float(np.sum(prep_ms)) / args.steps, "walk": t_kernel * 1e3,
-                                  "accumulate": float(np.sum(acc_ms)) / args.steps},
-            "walk_end_ms": None if args.serial else {"interior": float(np.mean([ph.walk_interior_ms for _, ph in phases])),
-                                                     "exterior": float(np.mean([ph.walk_exterior_ms for _, ph in phases]))},
+            "nnz": {"interior": nnz[0], "exterior": nnz[1]},
+            "cut_fraction": cut, "cut_walks": {"interior": st_i.n_truncated, "exterior": st_e.n_truncated,
+                                               "rule": "R10 max_steps / R10b left the bounding box / R10c inside the solid (DESIGN.md section 2)"},
+            "discarded_samples": {"interior": st_i.n_discarded, "exterior": st_e.n_discarded},
+            "bvh": {"faces": int(info.F), "nodes": int(info.n_nodes), "max_depth": int(info.max_depth), "device_bytes": tree_bytes},
+            "call": "mcs_build_bvh + mcs_orient_samples + mcs_estimate_dtn_both (output_kind 1)",
+            "phase_ms_per_step": {"build+sidedness+flush": ms_per_step - float(np.mean([p.total_ms for p in phases])),
+                                  "prep": float(np.mean([p.prep_ms for p in phases])), "walk": t_kernel * 1e3,
+                                  "accumulate": float(np.mean([p.accumulate_ms for p in phases]))},
+            "walk_end_ms": {"interior": float(np.mean([p.walk_interior_ms for p in phases])),
+                            "exterior": float(np.mean([p.walk_exterior_ms for p in phases]))},
             "clocks": clk,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": r["h2d_bytes"], "d2h_bytes_per_step": r["d2h_bytes"],
-                    "ms_per_step": e2e_t * 1e3, "ms_per_call": e2e_each, "steps": e2e_steps, "call": "mcs_estimate_dtn_host (pinned host buffers)"},
-            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+                    "ms_per_step": e2e_t * 1e3, "ms_per_call": e2e_each, "steps": e2e_steps,
+                    "call": "mcs_estimate_dtn_host_coo (pinned host buffers: mesh + samples up, COO entries of both operators down)"},
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "sub_records": sub}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -423,19 +620,26 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--level", type=int, default=4, help="icosphere subdivision level (configs[1]: 4)")
-    ap.add_argument("--walks-per-vertex", type=int, default=4096)
-    ap.add_argument("--points-per-vertex", type=int, default=16, help="G of DESIGN.md reading R1")
+    ap.add_argument("--faces", type=int, default=2_000_000, help="configs[3]: faces of the stress mesh")
+    ap.add_argument("--components", type=int, default=30)
+    ap.add_argument("--samples", type=int, default=20_000, help="boundary samples by farthest-point sampling")
+    ap.add_argument("--candidates", type=int, default=1_000_000, help="area-uniform candidates of the FPS")
+    ap.add_argument("--walks", type=int, default=4096, help="walks per sample and operator")
+    ap.add_argument("--mesh-seed", type=int, default=3)
     ap.add_argument("--eps", type=float, default=1e-3)
     ap.add_argument("--cap", type=float, default=2.5)
     ap.add_argument("--seed", type=int, default=0)
-    ap.add_argument("--cpu-samples", type=int, default=768, help="sample points of the cpu_baseline leg (about 12 s on 16 cores)")
-    ap.add_argument("--ref-samples", type=int, default=96, help="sample points per step of --impl reference")
+    ap.add_argument("--cpu-samples", type=int, default=16, help="sample points of the cpu_baseline leg")
+    ap.add_argument("--cpu-walks", type=int, default=8, help="walks per sample point of the cpu_baseline leg")
+    ap.add_argument("--ref-samples", type=int, default=8, help="sample points per step of --impl reference")
+    ap.add_argument("--ref-walks", type=int, default=4, help="walks per sample point per step of --impl reference")
+    ap.add_argument("--cfg4-meshes", type=int, default=16, help="meshes of the configs[4] sample sub-record")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--serial", action="store_true", help="two single-operator calls back to back instead of mcs_estimate_dtn_both")
+    ap.add_argument("--no-sub", action="store_true", help="skip the configs[1] / configs[4] sub-records")
+    ap.add_argument("--no-cache", action="store_true", help="regenerate the workload instead of reading the temp-dir cache")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -254,6 +254,29 @@ int mcs_estimate_dtn_host(const float* verts, int64_t V, const int32_t* faces, i
                           const mcs_samples* samples, const mcs_params* params, int operators,
                           float* out_interior, float* out_exterior, mcs_stats* stats, void* stream);
 
+/*
+ * The same from HOST buffers with the SPARSE output, for meshes whose V x V matrix cannot be dense (BASELINE
+ * config 3: 2 M faces): upload of the mesh and the samples, LBVH build, optionally the sidedness
+ * pre-pass (orient_h_scale > 0: mcs_orient_samples with that h_scale decides the side of every sample and replaces
+ * samples->normal), BOTH estimators as in mcs_estimate_dtn_both with output_kind 1, download.
+ * EVERY pointer is a HOST pointer.  out_*: capacity = entries the three arrays can hold; on return nnz = entries
+ * written (upper triangle, sorted by (row, col)).  MCS_ENOMEM when a capacity is too small: nnz then holds a lower
+ * bound of the need and nothing is copied.  params_*->output_kind / coo_capacity are ignored (taken from out_*).
+ * Device memory is allocated and freed inside the call (stream-ordered pool); blocks until the results are in the
+ * host buffers.  Errors: as mcs_build_bvh, mcs_orient_samples and mcs_estimate_dtn_*.
+ */
+typedef struct {
+    int64_t  capacity;           /* in: entries row/col/val can hold                          */
+    int32_t* row;                /* host [capacity]                                           */
+    int32_t* col;
+    float*   val;
+    int64_t  nnz;                /* out                                                       */
+} mcs_host_coo;
+int mcs_estimate_dtn_host_coo(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                              const mcs_samples* samples, const mcs_params* params_interior, const mcs_params* params_exterior,
+                              float orient_h_scale, mcs_host_coo* out_interior, mcs_host_coo* out_exterior,
+                              mcs_stats* stats_interior, mcs_stats* stats_exterior, void* stream);
+
 /* ------------------------------------------------------------------------ */
 /* Test / benchmark hooks for the individual steps of SURVEY.md 8(a).         */
 /* ------------------------------------------------------------------------ */
@@ -383,7 +406,7 @@ const char* mcs_error_string(int code);
 const char* mcs_version(void);
 /* sizeof of the ABI structs, for bindings to check their mirrors against:
  * 0 mcs_samples, 1 mcs_basis, 2 mcs_params, 3 mcs_matrix, 4 mcs_stats, 5 mcs_bvh_info_t,
- * 6 mcs_record; anything else: 0. */
+ * 6 mcs_record, 7 mcs_host_coo; anything else: 0. */
 size_t mcs_abi_sizeof(int which);
 
 #ifdef __cplusplus

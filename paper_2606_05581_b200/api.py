@@ -402,6 +402,58 @@ def estimate_dtn_host(verts, faces, tri, bary, weight, params: Params, interior=
     return res
 
 
+class _HostCoo(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("row", C.c_void_p), ("col", C.c_void_p), ("val", C.c_void_p), ("nnz", C.c_int64)]
+
+
+def estimate_dtn_host_coo(verts, faces, tri, bary, weight, params_interior: Params, params_exterior: Params,
+                          out_interior, out_exterior, orient_h_scale=0.0, normal=None, want_stats=False, device=None):
+    """The whole path from HOST tensors with sparse output (mcs_estimate_dtn_host_coo): upload, LBVH build, optional
+    sidedness pre-pass, both estimators, download.  out_*: (row int32, col int32, val fp32) CPU tensors of equal
+    length = capacity (pinned memory makes the copies asynchronous).  Returns dict(nnz_interior, nnz_exterior,
+    h2d_bytes, d2h_bytes[, stats_interior, stats_exterior]); raises McsError(MCS_ENOMEM) with .need = (ni, ne) when a
+    capacity is too small."""
+    def host(t, dtype, name):
+        t = torch.as_tensor(t)
+        if t.is_cuda:
+            raise ValueError(f"{name} must be a CPU tensor for the host entry point")
+        return t.to(dtype).contiguous()
+    verts, faces = host(verts, torch.float32, "verts"), host(faces, torch.int32, "faces")
+    tri, bary, weight = host(tri, torch.int32, "tri"), host(bary, torch.float32, "bary"), host(weight, torch.float32, "weight")
+    normal = host(normal, torch.float32, "normal") if normal is not None else None
+    V, F, n_s = int(verts.shape[0]), int(faces.shape[0]), int(tri.shape[0])
+    outs = []
+    for name, o in (("out_interior", out_interior), ("out_exterior", out_exterior)):
+        r, c, v = o
+        if r.is_cuda or c.is_cuda or v.is_cuda or r.dtype != torch.int32 or c.dtype != torch.int32 or v.dtype != torch.float32:
+            raise ValueError(f"{name} must be CPU tensors (int32, int32, float32)")
+        if not (r.is_contiguous() and c.is_contiguous() and v.is_contiguous()) or not (r.numel() == c.numel() == v.numel() > 0):
+            raise ValueError(f"{name}: three contiguous tensors of equal, non-zero length")
+        outs.append(_HostCoo(capacity=r.numel(), row=r.data_ptr(), col=c.data_ptr(), val=v.data_ptr(), nnz=0))
+    cs = _Samples(tri=tri.data_ptr(), bary=bary.data_ptr(), weight=weight.data_ptr(),
+                  normal=normal.data_ptr() if normal is not None else None, n_s=n_s)
+    ci, ce = params_interior.c(), params_exterior.c()
+    si = Stats() if want_stats else None
+    se = Stats() if want_stats else None
+    dev = torch.device("cuda" if device is None else device)
+    with torch.cuda.device(dev):
+        rc = lib().mcs_estimate_dtn_host_coo(_ptr(verts), C.c_int64(V), _ptr(faces), C.c_int64(F), C.byref(cs), C.byref(ci),
+                                             C.byref(ce), C.c_float(float(orient_h_scale)), C.byref(outs[0]), C.byref(outs[1]),
+                                             C.byref(si) if si is not None else None, C.byref(se) if se is not None else None,
+                                             _stream(dev))
+    ni, ne = int(outs[0].nnz), int(outs[1].nnz)
+    if rc == MCS_ENOMEM and (ni > outs[0].capacity or ne > outs[1].capacity):
+        err = McsError(rc, "mcs_estimate_dtn_host_coo", "sparse output capacity too small")
+        err.need = (ni, ne)
+        raise err
+    _check(rc, "mcs_estimate_dtn_host_coo")
+    h2d = verts.numel() * 4 + faces.numel() * 4 + n_s * 20 + (n_s * 12 if (normal is not None and not orient_h_scale > 0) else 0)
+    res = dict(nnz_interior=ni, nnz_exterior=ne, h2d_bytes=h2d, d2h_bytes=12 * (ni + ne) + 16)
+    if want_stats:
+        res["stats_interior"], res["stats_exterior"] = si, se
+    return res
+
+
 def tangent_balls(bvh: Bvh, samples: Samples, params: Params, exterior: bool):
     cs, cp = samples.c(), params.c()
     balls = torch.empty((samples.n_s, 8), dtype=torch.float32, device=bvh.device)

@@ -381,6 +381,112 @@ done:
     return fail(rc, stats);
 }
 
+// The same from host buffers with the SPARSE output (any V: BASELINE config 3, 2 M faces, ~1 M vertices): upload,
+// LBVH build, optional sidedness pre-pass (G-R1), both estimators into device COO buffers of the caller's capacity,
+// download of the entries that were written.
+extern "C" int mcs_estimate_dtn_host_coo(const float* verts, int64_t V, const int32_t* faces, int64_t F,
+                                         const mcs_samples* hs, const mcs_params* p_int, const mcs_params* p_ext,
+                                         float orient_h_scale, mcs_host_coo* out_interior, mcs_host_coo* out_exterior,
+                                         mcs_stats* stats_interior, mcs_stats* stats_exterior, void* stream)
+{
+    if (stats_interior) memset(stats_interior, 0, sizeof *stats_interior);
+    if (stats_exterior) memset(stats_exterior, 0, sizeof *stats_exterior);
+    if (!verts || !faces || !hs || !p_int || !p_ext || !out_interior || !out_exterior || V < 1 || F < 1 || hs->n_s < 1) return MCS_EINVAL;
+    if (!hs->tri || !hs->bary || !hs->weight) return MCS_EINVAL;
+    mcs_host_coo* ho[2] = { out_interior, out_exterior };
+    for (int x = 0; x < 2; ++x) {
+        if (ho[x]->capacity < 1 || !ho[x]->row || !ho[x]->col || !ho[x]->val) return MCS_EINVAL;
+        ho[x]->nnz = 0;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n_s = hs->n_s;
+    const size_t nb_v = (size_t)V * 12, nb_f = (size_t)F * 12;
+    const size_t nb_tri = (size_t)n_s * 4, nb_bary = (size_t)n_s * 12, nb_w = (size_t)n_s * 4, nb_n = (size_t)n_s * 12;
+    const bool orient = orient_h_scale > 0.0f;
+    const bool have_n = orient || hs->normal;
+    size_t off_v = 0, off_f = align_up(off_v + nb_v), off_t = align_up(off_f + nb_f), off_b = align_up(off_t + nb_tri),
+           off_w = align_up(off_b + nb_bary), off_n = align_up(off_w + nb_w), in_total = align_up(off_n + nb_n) + 256;
+    {
+        int dev = 0; cudaMemPool_t pool;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
+    char* d_in = nullptr; char* d_out = nullptr; void* d_ws = nullptr; void* d_wws = nullptr;
+    mcs_bvh* bvh = nullptr;
+    int rc = MCS_OK;
+    size_t out_off[2], out_total = 0;
+    for (int x = 0; x < 2; ++x) { out_off[x] = out_total; out_total += align_up((size_t)ho[x]->capacity * 12 + 64); }
+    cudaError_t e = cudaMallocAsync((void**)&d_in, in_total, st);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&d_out, out_total, st);
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+    e = cudaMemcpyAsync(d_in + off_v, verts, nb_v, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_f, faces, nb_f, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_t, hs->tri, nb_tri, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_b, hs->bary, nb_bary, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_in + off_w, hs->weight, nb_w, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && hs->normal && !orient) e = cudaMemcpyAsync(d_in + off_n, hs->normal, nb_n, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; goto done; }
+    rc = mcs_build_bvh((const float*)(d_in + off_v), V, (const int32_t*)(d_in + off_f), F, nullptr, stream, &bvh);
+    if (rc != MCS_OK) goto done;
+    {
+        mcs_samples ds;
+        ds.tri = (const int32_t*)(d_in + off_t); ds.bary = (const float*)(d_in + off_b);
+        ds.weight = (const float*)(d_in + off_w); ds.normal = nullptr; ds.n_s = n_s;
+        if (orient) {                                 // sidedness by the winding number (DESIGN.md G-R1)
+            const size_t wb = mcs_winding_workspace_bytes(bvh, n_s);
+            e = cudaMallocAsync(&d_wws, wb, st);
+            if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+            rc = mcs_orient_samples(bvh, &ds, orient_h_scale, (float*)(d_in + off_n), nullptr, d_wws, wb, stream);
+            if (rc != MCS_OK) goto done;
+        }
+        if (have_n) ds.normal = (const float*)(d_in + off_n);
+        mcs_basis basis; memset(&basis, 0, sizeof basis); basis.kind = 0; basis.K = V;
+        mcs_params pp[2] = { *p_int, *p_ext };
+        mcs_matrix mm[2];
+        for (int x = 0; x < 2; ++x) {
+            pp[x].output_kind = 1; pp[x].coo_capacity = ho[x]->capacity;
+            memset(&mm[x], 0, sizeof mm[x]);
+            char* o = d_out + out_off[x];
+            mm[x].kind = 1; mm[x].K = V; mm[x].coo_capacity = ho[x]->capacity;
+            mm[x].coo_nnz = (int64_t*)o;
+            mm[x].coo_row = (int32_t*)(o + 64); mm[x].coo_col = mm[x].coo_row + ho[x]->capacity;
+            mm[x].coo_val = (float*)(mm[x].coo_col + ho[x]->capacity);
+        }
+        const size_t need = make_layout(bvh, &ds, &basis, &pp[0], 0, true, true).total + make_layout(bvh, &ds, &basis, &pp[1], 1, true, true).total;
+        e = cudaMallocAsync(&d_ws, need, st);
+        if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }
+        rc = estimate_both(bvh, &ds, &basis, &pp[0], &pp[1], d_ws, need, &mm[0], &mm[1], stats_interior, stats_exterior, stream);
+        // entry counts first (on MCS_ENOMEM they hold a lower bound of the need), then the entries that were written
+        int64_t nnz[2] = { 0, 0 };
+        for (int x = 0; x < 2; ++x) {
+            cudaError_t ec = cudaMemcpyAsync(&nnz[x], mm[x].coo_nnz, 8, cudaMemcpyDeviceToHost, st);
+            if (ec != cudaSuccess && rc == MCS_OK) { mcs_set_last_cuda_error((int)ec); rc = MCS_ECUDA; }
+        }
+        e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess && rc == MCS_OK) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+        for (int x = 0; x < 2; ++x) ho[x]->nnz = nnz[x];
+        if (rc != MCS_OK) goto done;
+        for (int x = 0; x < 2 && e == cudaSuccess; ++x) {
+            const size_t nb = (size_t)nnz[x] * 4;
+            e = cudaMemcpyAsync(ho[x]->row, mm[x].coo_row, nb, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(ho[x]->col, mm[x].coo_col, nb, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(ho[x]->val, mm[x].coo_val, nb, cudaMemcpyDeviceToHost, st);
+        }
+        if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+    }
+done:
+    if (d_ws) cudaFreeAsync(d_ws, st);
+    if (d_wws) cudaFreeAsync(d_wws, st);
+    if (d_out) cudaFreeAsync(d_out, st);
+    if (d_in) cudaFreeAsync(d_in, st);
+    e = cudaStreamSynchronize(st);
+    if (rc == MCS_OK && e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+    if (bvh) mcs_free_bvh(bvh);
+    return fail(rc, stats_exterior);
+}
+
 extern "C" int mcs_tangent_balls(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
                                  float* balls, void* stream)
 {
@@ -496,6 +602,7 @@ extern "C" size_t mcs_abi_sizeof(int which)
         case 4: return sizeof(mcs_stats);
         case 5: return sizeof(mcs_bvh_info_t);
         case 6: return sizeof(mcs_record);
+        case 7: return sizeof(mcs_host_coo);
         default: return 0;
     }
 }

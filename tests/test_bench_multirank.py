@@ -59,9 +59,12 @@ def test_reference_arm_line_shape():
     env = dict(os.environ)
     env.pop("RANK", None)
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
-                        "--warmup", "0", "--ref-samples", "4"], env=env, capture_output=True, text=True, timeout=600)
+                        "--warmup", "0", "--ref-samples", "4", "--ref-walks", "2", "--faces", "20000", "--components", "5",
+                        "--samples", "200", "--candidates", "5000", "--walks", "64", "--no-cache"],
+                       env=env, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stderr
     d = json.loads(r.stdout.strip().splitlines()[-1])
     assert d["impl"] == "reference" and d["metric"] == "walk_steps_per_s" and d["vs_baseline"] is None
+    assert d["config"]["workload"].startswith("configs[3]")
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"] and d["gpu_launches"] == 0
