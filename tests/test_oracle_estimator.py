@@ -480,3 +480,128 @@ def test_naive_estimator_on_mesh_is_symmetrised_not_psd_and_noisier():
     for k in range(3):
         g = v[:, k].astype(np.float64)
         assert abs(g @ Sn @ g / (g @ M @ g) - 1.0) < 0.1
+
+
+# --------------------------------------------------------------------------
+# antithetic sampling on the tangent ball ("antithetical sampling on each tangent ball"; reading R7:
+# walks 2j and 2j+1 share the INIT draw of counter walk = j and start at azimuths phi and phi + pi; their STEP
+# streams stay those of their own walk index)
+# --------------------------------------------------------------------------
+def _antithetic_setup(W=32, n_s=300, r=0.5, seed=11, eps=1e-3):
+    pos = fibonacci_sphere(n_s)
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    w = np.full(n_s, 4 * np.pi / n_s, np.float32)
+    kw = dict(seed=seed, walks_per_sample=W, eps=eps, rmax=r * 1024 / 1023, cap_half_angle_deg=2.5)
+    rec_a, balls = orc.run_walks(OracleParams(antithetic=True, **kw), False, weight=w, pos=pos)
+    rec_n, _ = orc.run_walks(OracleParams(antithetic=False, **kw), False, weight=w, pos=pos)
+    return pos, balls, rec_a.reshape(n_s, W), rec_n.reshape(n_s, W)
+
+
+def test_antithetic_partners_are_mirror_images_about_the_pole_axis():
+    """The partners' start points have the same polar angle and opposite tangential parts:
+    z_{2j} + z_{2j+1} - 2 (c + r cos(theta) n) = 0, (z - c).n equal, |z - c| = r, equal weights; the even partner
+    is the start point the plain run gives walk j (shared INIT draw, no shift)."""
+    pos, balls, ra, rn = _antithetic_setup()
+    r, c = balls[:, 0], balls[:, 1:4]
+    n = (pos - c) / r[:, None]                                    # pole: from the centre to the tangent point
+    assert np.allclose(np.linalg.norm(n, axis=1), 1.0, atol=1e-12)
+    a = ra["z"][:, 0::2] - c[:, None, :]
+    b = ra["z"][:, 1::2] - c[:, None, :]
+    an = np.einsum("swk,sk->sw", a, n)
+    bn = np.einsum("swk,sk->sw", b, n)
+    assert np.abs(an - bn).max() < 1e-12
+    assert np.abs(a + b - 2 * an[..., None] * n[:, None, :]).max() < 1e-12          # the mirror identity
+    assert np.abs(np.linalg.norm(a, axis=2) - r[:, None]).max() < 1e-12
+    at = a - an[..., None] * n[:, None, :]
+    assert np.linalg.norm(at, axis=2).min() > 1e-6                # outside the cap: the two points are distinct
+    assert np.array_equal(ra["weight"][:, 0::2], ra["weight"][:, 1::2])
+    W = ra.shape[1]
+    assert np.abs(ra["z"][:, 0::2] - rn["z"][:, :W // 2]).max() == 0.0               # even partner = plain walk j's start
+
+
+def test_antithetic_partners_keep_their_own_step_streams():
+    """Each partner's jumps are drawn from Philox(seed; sample, ITS OWN walk index, step, STEP): re-walking from the
+    recorded start point on the analytic unit ball (distance 1 - |x|) with those counters, through the generator that
+    is pinned against cuRAND, lands on the recorded exit point.  Sharing the stream between partners (walk >> 1)
+    would not."""
+    from oracle import philox4x32_10, u01
+    seed, eps = 11, 1e-3
+    pos, balls, ra, rn = _antithetic_setup(W=8, n_s=40, seed=seed, eps=eps)
+    shared_would_differ = 0
+    for i in range(ra.shape[0]):
+        for w in range(ra.shape[1]):
+            for stream in (w, w >> 1):
+                x = ra["z"][i, w].copy()
+                k = 0
+                while True:
+                    d = 1.0 - np.linalg.norm(x)
+                    if d < eps:
+                        break
+                    k += 1
+                    words = philox4x32_10((i, stream, k, 2), (seed & 0xFFFFFFFF, seed >> 32))
+                    ct = 1.0 - 2.0 * u01(words[0])
+                    st = np.sqrt(max(0.0, 1.0 - ct * ct))
+                    phi = 2.0 * np.pi * u01(words[1])
+                    x += d * np.array([st * np.cos(phi), st * np.sin(phi), ct])
+                t = x / np.linalg.norm(x)
+                if stream == w:
+                    assert k == ra["steps"][i, w]
+                    assert np.abs(t - ra["t"][i, w]).max() < 1e-9
+                elif w >= 2 and k > 0:                            # walks 0, 1: w >> 1 == 0 is walk 0's own stream
+                    shared_would_differ += int(np.abs(t - ra["t"][i, w]).max() > 1e-6)
+    assert shared_would_differ > 50                               # the check above has teeth
+
+
+def test_interior_unit_ball_whole_ball_cap_spectrum_holds_with_antithetic_pairs():
+    """Antithetic partners are each distributed as a plain start point, so the expectation is unchanged: the
+    whole-ball case (no walk) must still give the cap quadrature (phi + pi/2, or a pair sharing one point, would not
+    change this; the mirror identity above pins those)."""
+    n_s, W = 8000, 64            # partners share their polar angle, so even functionals (d d^T) see half as many draws
+    pos = fibonacci_sphere(n_s)
+    orc = Oracle(sphere_geom((0, 0, 0), 1.0))
+    P = OracleParams(seed=1, walks_per_sample=W, eps=1e-2, rmax=1.0 * 1024 / 1023, cap_half_angle_deg=2.5, antithetic=True)
+    rec, balls = orc.run_walks(P, False, weight=np.full(n_s, 4 * np.pi / n_s, np.float32), pos=pos)
+    assert (rec["steps"] == 0).all()
+    S, _ = _galerkin_from_records(rec, pos, np.zeros(3))
+    want = np.array([_cap_spectrum(l, 2.5) for l in DEGREES])
+    assert np.abs(np.diag(S) - want).max() < 0.03, (np.diag(S), want)
+    assert np.abs(S - np.diag(np.diag(S))).max() < 0.03
+
+
+def test_antithetic_pairs_cancel_odd_tangential_moments():
+    """What the pairing buys: a functional that is odd in the tangential offset of the start point has a pair sum of
+    exactly zero at the start points (here: the tangential part of z - c), and the pair means of first-order
+    quantities of the exit points, E[t - s] projected on a tangent direction, have a smaller variance than means over
+    independent pairs."""
+    pos, balls, ra, rn = _antithetic_setup(W=64, n_s=400, eps=1e-4)
+    r, c = balls[:, 0], balls[:, 1:4]
+    n = (pos - c) / r[:, None]
+    e = np.cross(n, np.array([0.3, -0.5, 0.8]))
+    e /= np.linalg.norm(e, axis=1, keepdims=True)                  # a tangent direction per sample
+    fa = np.einsum("swk,sk->sw", ra["t"] - pos[:, None, :], e)
+    fn = np.einsum("swk,sk->sw", rn["t"] - pos[:, None, :], e)
+    var_pairs_anti = (0.5 * (fa[:, 0::2] + fa[:, 1::2])).var()
+    var_pairs_plain = (0.5 * (fn[:, 0::2] + fn[:, 1::2])).var()
+    assert var_pairs_anti < 0.8 * var_pairs_plain, (var_pairs_anti, var_pairs_plain)
+
+
+# --------------------------------------------------------------------------
+# thin spots named by the round-1 review: r_max of the exterior rule and the AABB diagonal of R10b
+# --------------------------------------------------------------------------
+def test_aabb_diagonal_and_exterior_rmax_closed_forms():
+    import ctypes as C
+    v, f = box((1.0, 2.0, 3.0), (2, 2, 2))
+    orc = Oracle(mesh_geom(v, f))
+    orc.lib.orc_aabb_diagonal.restype = C.c_double
+    assert abs(orc.lib.orc_aabb_diagonal(C.byref(orc.geom.c)) - np.sqrt(14.0)) < 1e-6      # half of it would fail
+    assert abs(orc.rmax() - 0.5) < 1e-7                                                    # half the shortest side
+    # exterior: AABB of the inverted vertices (PAPER.md:642 applied in the inverted domain, R11).  Unit sphere about
+    # its centre: kappa fixes the sphere, sides 2, r_max = 1.  About an interior point at distance a from the centre
+    # the image is a sphere of radius R / (R^2 - a^2): r_max = that radius (up to the tessellation).
+    v, f = icosphere(4)
+    orc = Oracle(mesh_geom(v, f))
+    assert abs(orc.rmax(True, (0.0, 0.0, 0.0)) - 1.0) < 2e-3
+    a = 0.3
+    assert abs(orc.rmax(True, (a, 0.0, 0.0)) - 1.0 / (1.0 - a * a)) < 5e-3
+    v2, f2 = icosphere(4, radius=2.0)
+    assert abs(Oracle(mesh_geom(v2, f2)).rmax(True, (0.0, 0.5, 0.0)) - 2.0 / (4.0 - 0.25)) < 5e-3
