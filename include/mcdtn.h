@@ -44,18 +44,30 @@ typedef struct mcs_bvh mcs_bvh;
 /* the build assumes nothing about manifoldness, orientation, area or the     */
 /* number of components.                                                       */
 /* ------------------------------------------------------------------------ */
-typedef struct {
-    int32_t reserved;            /* must be 0 */
+typedef struct {                 /* all zero = defaults */
+    int32_t no_split;            /* 1: one leaf per face.  0: long thin faces enter the tree as several leaf references,
+                                    one per slab across their longest edge (sliver-heavy CAD meshes;
+                                    the box of a rotated sliver is almost all empty space).  Query results are the same
+                                    either way: every reference carries the whole triangle                              */
+    int32_t max_pieces;          /* references per face at most (0: 64)                                                 */
+    float   split_length;        /* a face is cut when its longest edge exceeds this many mean edge lengths and its
+                                    aspect L^2 / 2A exceeds 8; pieces are about this long (0: 4)                         */
+    float   split_budget;        /* extra references per face on average at most; the piece length is raised until
+                                    this holds (0: 1)                                                                    */
 } mcs_build_opts;
 
 typedef struct {
     int64_t V, F;                /* vertices, faces                                  */
-    int64_t n_nodes;             /* internal nodes of the packed tree                */
+    int64_t n_nodes;             /* internal nodes of the packed tree (n_leaves - 1) */
     int32_t max_depth;           /* deepest leaf (root = 0)                          */
     int32_t n_degenerate;        /* zero-area faces (kept: they absorb as segments)  */
     float   aabb_lo[3], aabb_hi[3];   /* box of the vertices referenced by faces     */
     double  area;                /* total surface area |dOmega|                      */
     size_t  device_bytes;        /* device memory owned by the handle                */
+    int64_t n_leaves;            /* leaf references: F plus the extra slabs of split faces */
+    double  sah_cost;            /* surface-area cost of the tree: sum over child boxes of area x (1 inner, 80/18 leaf)
+                                    / area of the root box -- expected box tests + weighted triangle tests of a random
+                                    line; a quality readout, lower is better                                             */
 } mcs_bvh_info_t;
 
 /*
@@ -65,7 +77,10 @@ typedef struct {
  * The handle's device memory comes from the device's stream-ordered pool
  * (cudaMallocAsync on `stream`; the pool's release threshold is raised so that
  * build/free cycles reuse memory).  mcs_free_bvh returns it in the order of the
- * legacy default stream, i.e. after all work submitted so far; it does not block.
+ * legacy default stream after making that stream wait for the last call that used the handle (the handle
+ * records an event on the stream of every call that reads the tree), so kernels still queued on a non-blocking
+ * stream finish first; it does not block the host.  A handle used on several streams at once must be
+ * synchronised by the caller before it is freed (only the last call's stream is tracked).
  * Errors: MCS_EINVAL (null pointer, V < 1, F < 1, face index outside [0,V)),
  * MCS_EDEGENERATE (non-finite vertex, zero total area), MCS_ENOMEM, MCS_ECUDA.
  */
@@ -78,8 +93,8 @@ int  mcs_bvh_info(const mcs_bvh* bvh, mcs_bvh_info_t* out /* host */);
 /*
  * Structure dump for the invariant tests (SURVEY.md 8(c) "LBVH (GPU)").
  * Each output may be NULL.  nodes: [n_nodes][16] 32-bit words, the packed node
- * (see DESIGN.md "BVH node"); leaf_tri: [F] original face index of the k-th
- * leaf in Morton order; morton: [F] sorted 63-bit keys.  Blocks the host.
+ * (see DESIGN.md "BVH node"); leaf_tri: [n_leaves] original face index of the k-th
+ * leaf in Morton order; morton: [n_leaves] sorted 63-bit keys.  Blocks the host.
  */
 int  mcs_bvh_dump(const mcs_bvh* bvh, uint32_t* nodes, int32_t* leaf_tri, uint64_t* morton,
                   void* stream);

@@ -26,13 +26,13 @@ class McsError(RuntimeError):
 
 
 class _BuildOpts(C.Structure):
-    _fields_ = [("reserved", C.c_int32)]
+    _fields_ = [("no_split", C.c_int32), ("max_pieces", C.c_int32), ("split_length", C.c_float), ("split_budget", C.c_float)]
 
 
 class BvhInfo(C.Structure):
     _fields_ = [("V", C.c_int64), ("F", C.c_int64), ("n_nodes", C.c_int64), ("max_depth", C.c_int32),
                 ("n_degenerate", C.c_int32), ("aabb_lo", C.c_float * 3), ("aabb_hi", C.c_float * 3),
-                ("area", C.c_double), ("device_bytes", C.c_size_t)]
+                ("area", C.c_double), ("device_bytes", C.c_size_t), ("n_leaves", C.c_int64), ("sah_cost", C.c_double)]
 
 
 class _Samples(C.Structure):
@@ -179,7 +179,7 @@ class Samples:
 class Bvh:
     """Opaque LBVH handle (mcs_build_bvh / mcs_free_bvh)."""
 
-    def __init__(self, verts, faces):
+    def __init__(self, verts, faces, split=True, max_pieces=0, split_length=0.0, split_budget=0.0):
         self.verts = _dev(verts, torch.float32, "verts")
         self.faces = _dev(faces, torch.int32, "faces")
         if self.verts.ndim != 2 or self.verts.shape[1] != 3 or self.faces.ndim != 2 or self.faces.shape[1] != 3:
@@ -187,8 +187,10 @@ class Bvh:
         self.device = self.verts.device
         self._h = C.c_void_p(0)
         with torch.cuda.device(self.device):
+            opts = _BuildOpts(no_split=int(not split), max_pieces=int(max_pieces), split_length=float(split_length),
+                              split_budget=float(split_budget))
             rc = lib().mcs_build_bvh(_ptr(self.verts), C.c_int64(self.verts.shape[0]), _ptr(self.faces),
-                                     C.c_int64(self.faces.shape[0]), None, _stream(self.device), C.byref(self._h))
+                                     C.c_int64(self.faces.shape[0]), C.byref(opts), _stream(self.device), C.byref(self._h))
         _check(rc, "mcs_build_bvh")
 
     def __del__(self):
@@ -217,16 +219,18 @@ class Bvh:
     def dump(self):
         info = self.info()
         nodes = torch.empty((info.n_nodes, 16), dtype=torch.int32, device=self.device)
-        leaf_tri = torch.empty(info.F, dtype=torch.int32, device=self.device)
-        morton = torch.empty(info.F, dtype=torch.int64, device=self.device)
+        leaf_tri = torch.empty(info.n_leaves, dtype=torch.int32, device=self.device)
+        morton = torch.empty(info.n_leaves, dtype=torch.int64, device=self.device)
         with torch.cuda.device(self.device):
             _check(lib().mcs_bvh_dump(self._h, _ptr(nodes), _ptr(leaf_tri), _ptr(morton), _stream(self.device)),
                    "mcs_bvh_dump")
         return nodes, leaf_tri, morton
 
 
-def build_bvh(verts, faces) -> Bvh:
-    return Bvh(verts, faces)
+def build_bvh(verts, faces, split=True, max_pieces=0, split_length=0.0, split_budget=0.0) -> Bvh:
+    """LBVH over the triangle soup (mcs_build_bvh).  split: long thin faces enter the tree as several leaf references
+    (mcs_build_opts); the query results do not depend on it."""
+    return Bvh(verts, faces, split, max_pieces, split_length, split_budget)
 
 
 def _closest(fn, name, bvh: Bvh, q):

@@ -111,6 +111,7 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
     if (rc != MCS_OK) return fail(rc, hs);
     rc = acc_run(b, s, basis, p, records, L.n_records, base + L.acc_off,
                  align_up(acc_ws_bytes(b, s, basis, p, L.n_records)), out, stats_dev, st);
+    mcs_bvh_touch(b, st);
     if (rc != MCS_OK) return fail(rc, hs);
     mcs_prof_mark(MCS_MARK_END, st);
     if (hs) {
@@ -223,6 +224,7 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done, 0);
     if (e == cudaSuccess) e = cudaEventRecord(ev_done1, st1);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done1, 0);
+    mcs_bvh_touch(b, st);                             // after the join: covers both side streams
     if (rc != MCS_OK) return fail(rc, hs_ext);
     if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return fail(MCS_ECUDA, hs_ext); }
     mcs_prof_mark(MCS_MARK_END, st);
@@ -514,6 +516,7 @@ extern "C" int mcs_run_walks(const mcs_bvh* b, const mcs_samples* s, const mcs_p
     if (!ws || ws_bytes < need) return MCS_ENOMEM;
     unsigned long long* stats_dev = nullptr;
     int rc = walk_run(b, s, p, exterior, ws, ws_bytes, (float4*)records, steps, false, nullptr, hs != nullptr, &stats_dev, st);
+    mcs_bvh_touch(b, st);
     if (rc != MCS_OK) return fail(rc, hs);
     if (hs) {
         unsigned long long h[ST_COUNT];
@@ -541,6 +544,7 @@ extern "C" int mcs_accumulate(const mcs_bvh* b, const mcs_samples* s, const mcs_
     unsigned long long* stats_dev = (unsigned long long*)ws;       // first 512 bytes: counters
     MCS_CUDA_TRY(cudaMemsetAsync(stats_dev, 0, ST_COUNT * 8, st));
     int rc = acc_run(b, s, basis, p, (const float4*)records, n_records, (char*)ws + 512, ws_bytes - 512, out, stats_dev, st);
+    mcs_bvh_touch(b, st);
     if (rc != MCS_OK) return fail(rc, hs);
     if (hs) {
         unsigned long long h[ST_COUNT];

@@ -44,7 +44,8 @@ struct __align__(16) BvhNode {
 // One packed triangle = 64 bytes = 4 x 16-byte loads, in Morton order:
 //   t0 = (v0.x, v0.y, v0.z, original face index as int bits)
 //   t1 = (v1.x, v1.y, v1.z, |n|^2)   t2 = (v2.x, v2.y, v2.z, 1/|n|^2)
-//   t3 = (n.x, n.y, n.z, 1.0 if the face has zero area else 0.0),  n = (v1-v0) x (v2-v0)
+//   t3 = (n.x, n.y, n.z, flags as int bits: bit 0 = zero-area face, bit 1 = not the first leaf reference of its face),
+//        n = (v1-v0) x (v2-v0)
 // The vertices are the caller's fp32 numbers; n, |n|^2 are computed in fp64 by the build
 // and rounded once.
 struct __align__(16) PackedTri {
@@ -65,23 +66,29 @@ struct __align__(32) WideNode {
 
 struct mcs_bvh {
     int64_t V, F, n_nodes;
+    int64_t n_leaves;      // leaf references: F, plus the extra slabs of split slivers (bvh.cu)
     float*     verts;      // [V][3] copy of the input
     int32_t*   faces;      // [F][3] copy of the input
     BvhNode*   nodes;      // [max(F-1,1)]
     WideNode*  wide;       // [n_wide] 4-wide collapse of `nodes` (walk kernel); root = 0
     int64_t    n_wide;
-    PackedTri* tris;       // [F] Morton order
-    int32_t*   leaf_tri;   // [F] original face index of sorted leaf k
-    int32_t*   face_slot;  // [F] sorted slot of original face f (inverse of leaf_tri)
-    uint64_t*  morton;     // [F] sorted keys
+    PackedTri* tris;       // [n_leaves] Morton order; leaf k holds the whole triangle of its face
+    int32_t*   leaf_tri;   // [n_leaves] original face index of sorted leaf k
+    int32_t*   face_slot;  // [F] first sorted leaf of original face f
+    uint64_t*  morton;     // [n_leaves] sorted keys
     int32_t    root;       // index of the root node (0)
     int32_t    max_depth;
     int32_t    n_degenerate;
     float      aabb_lo[3], aabb_hi[3];
     double     area;
+    double     sah_cost;   // surface-area cost of the packed tree (bvh.cu sah_partial_kernel)
     size_t     device_bytes;
     int        device;
+    mutable cudaEvent_t last_use;   // recorded on the stream of every call that reads the tree (mcs_free_bvh waits for it)
 };
+
+// Every entry point that enqueues work reading the tree calls this with its stream when it is done enqueuing.
+void mcs_bvh_touch(const mcs_bvh* b, cudaStream_t st);
 
 // ---------------------------------------------------------------------------
 // radix sort / scan (sort.cu)

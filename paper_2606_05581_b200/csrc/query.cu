@@ -77,6 +77,7 @@ extern "C" int mcs_closest_point(const mcs_bvh* b, const float* q, int64_t Q,
     float scale = 0.0f;                                // |coordinates|_1 bound of the mesh (prune_limit)
     for (int d = 0; d < 3; ++d) scale += fmaxf(fabsf(b->aabb_lo[d]), fabsf(b->aabb_hi[d]));
     mcs_note_launch(), closest_point_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->nodes, b->tris, q, Q, scale, dist, tri, bary);
+    mcs_bvh_touch(b, (cudaStream_t)stream);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }
@@ -86,7 +87,8 @@ extern "C" int mcs_closest_point_bruteforce(const mcs_bvh* b, const float* q, in
 {
     if (!b || Q < 0 || (Q > 0 && !q)) return MCS_EINVAL;
     if (Q == 0) return MCS_OK;
-    mcs_note_launch(), closest_point_bruteforce_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->tris, b->F, q, Q, dist, tri, bary);
+    mcs_note_launch(), closest_point_bruteforce_kernel<<<(unsigned)ceil_div64(Q, QT), QT, 0, (cudaStream_t)stream>>>(b->tris, b->n_leaves, q, Q, dist, tri, bary);
+    mcs_bvh_touch(b, (cudaStream_t)stream);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

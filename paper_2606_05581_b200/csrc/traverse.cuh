@@ -7,9 +7,10 @@
 // feature size and not with the absolute coordinates.
 //
 // Tie rule (R15): smaller fp32 squared distance, then smaller
-// ORIGINAL face index.  Sub-trees are pruned only when their box distance is
-// strictly larger than the best distance so far, so the result does not depend
-// on the traversal order.
+// ORIGINAL face index.  Sub-trees are pruned only when their box distance exceeds
+// prune_limit(best): the best squared distance so far plus an absolute margin that
+// covers the rounding of the computed triangle distances, so every face that can hold
+// the computed minimum is tested and the result does not depend on the traversal order.
 #pragma once
 #include "common.cuh"
 
@@ -79,7 +80,7 @@ __device__ __forceinline__ TriData unpack_tri(float4 t0, float4 t1, float4 t2, f
     TriData T;
     T.a = f3(t0.x, t0.y, t0.z); T.b = f3(t1.x, t1.y, t1.z); T.c = f3(t2.x, t2.y, t2.z);
     T.n = f3(t3.x, t3.y, t3.z);
-    T.orig = __float_as_int(t0.w); T.nn = t1.w; T.rnn = t2.w; T.degenerate = t3.w != 0.0f;
+    T.orig = __float_as_int(t0.w); T.nn = t1.w; T.rnn = t2.w; T.degenerate = (__float_as_int(t3.w) & 1) != 0;
     return T;
 }
 

@@ -161,7 +161,7 @@ template <bool EXT>
 __global__ void __launch_bounds__(TB_WARPS * 32)
 tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
                     const float* __restrict__ normal, const uint32_t* __restrict__ order, int64_t n_s,
-                    float rmax, float eps, int iters, float3 o,
+                    float rmax, float eps, int iters, float3 o, float mesh_scale,
                     float4* __restrict__ balls, unsigned long long* __restrict__ stats)
 {
     __shared__ int s_nodes[TB_WARPS][TB_NCAP];
@@ -173,7 +173,6 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
     int* lstack = s_leaves[wib];
     const int64_t n_warps = (int64_t)gridDim.x * TB_WARPS;
     unsigned cnt_nodes = 0, cnt_tris = 0, cnt_queries = 0, cnt_discarded = 0;
-    const float SLACK = 1.0f + 4e-6f;
 
     for (int64_t jj = (int64_t)blockIdx.x * TB_WARPS + wib; jj < n_s; jj += n_warps) {
         const int64_t i = order[jj];
@@ -246,7 +245,9 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
                     const int2 ch = make_int2(__float_as_int(n1.hi.x), __float_as_int(n1.hi.y));
                     ++cnt_nodes;
                     c0 = ch.x; c1 = ch.y;
-                    const float lim = thr2J * SLACK;
+                    // same limit as the walk kernel's queries: a face whose COMPUTED distance enters the ball is reached
+                    // whatever its box distance rounds to, so J is the minimum over all faces and does not depend on the tree
+                    const float lim = prune_limit(thr2J, cJ, mesh_scale);
                     in0 = box_dist2(cJ, w0.x, w0.y, w0.z, w0.w, w1.x, w1.y) <= lim;
                     in1 = box_dist2(cJ, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w) <= lim;
                 }
@@ -534,7 +535,6 @@ walk_kernel(WalkGeom g, WalkArgs a)
     const long long n_main = a.n_s * a.W;
     const uint2 key = make_uint2(a.key0, a.key1);
     const float3 o = f3(a.ox, a.oy, a.oz);
-    const float SLACK = 1.0f + 4e-6f;            // see bvh_closest_point
 
     LaneStack stk;
     stk.s_ref = sh_ref + threadIdx.x;
@@ -912,6 +912,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     const float3 hi = f3(b->aabb_hi[0], b->aabb_hi[1], b->aabb_hi[2]);
     const float3 o = exterior ? f3(p->kelvin_origin[0], p->kelvin_origin[1], p->kelvin_origin[2]) : f3(0.f, 0.f, 0.f);
     const unsigned nblk_s = (unsigned)ceil_div64(n_s, PT);
+    const float mesh_scale = fmaxf(fabsf(lo.x), fabsf(hi.x)) + fmaxf(fabsf(lo.y), fabsf(hi.y)) + fmaxf(fabsf(lo.z), fabsf(hi.z));
 
     // r_max and, for the exterior, R_max
     float side = fminf(hi.x - lo.x, fminf(hi.y - lo.y, hi.z - lo.z));
@@ -957,10 +958,10 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         if (nblk_tb > cap_tb) nblk_tb = cap_tb;
         if (exterior)
             mcs_note_launch(), tangent_ball_kernel<true><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
-                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, balls, stats);
+                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
         else
             mcs_note_launch(), tangent_ball_kernel<false><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
-                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, balls, stats);
+                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
     }
     if (balls_out) mcs_note_launch(), balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
     MCS_CUDA_TRY(cudaGetLastError());
@@ -976,7 +977,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.importance = p->importance_sample; a.antithetic = p->antithetic;
     a.naive = p->estimator == 1; a.inv_inset = p->estimator == 1 ? 1.0f / p->inset : 0.0f;
     a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
-    a.mesh_scale = fmaxf(fabsf(lo.x), fabsf(hi.x)) + fmaxf(fabsf(lo.y), fabsf(hi.y)) + fmaxf(fabsf(lo.z), fabsf(hi.z));
+    a.mesh_scale = mesh_scale;
     {
         const float dx = hi.x - lo.x, dy = hi.y - lo.y, dz = hi.z - lo.z;
         a.escape = exterior ? 3.0e38f : sqrtf(dx * dx + dy * dy + dz * dz);

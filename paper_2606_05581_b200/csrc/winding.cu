@@ -15,7 +15,7 @@ namespace {
 constexpr int WQ = 128;           // query points per block = faces per tile
 
 __global__ void __launch_bounds__(WQ)
-winding_partial_kernel(const PackedTri* __restrict__ tris, long long F, const float* __restrict__ pts,
+winding_partial_kernel(const float* __restrict__ verts, const int32_t* __restrict__ faces, long long F, const float* __restrict__ pts,
                        const int32_t* __restrict__ exclude, long long n, long long faces_per_chunk,
                        float* __restrict__ partial)
 {
@@ -29,9 +29,11 @@ winding_partial_kernel(const PackedTri* __restrict__ tris, long long F, const fl
     float sum = 0.0f, comp = 0.0f;                                    // Kahan: a chunk holds up to ~10^5 terms
     for (long long t0 = f0; t0 < f1; t0 += WQ) {
         const long long k = t0 + threadIdx.x;
-        if (k < f1) {
-            const float4* t = reinterpret_cast<const float4*>(tris + k);
-            sA[threadIdx.x] = __ldg(t); sB[threadIdx.x] = __ldg(t + 1); sC[threadIdx.x] = __ldg(t + 2);
+        if (k < f1) {                                                 // every face once, from the mesh itself (the tree's
+            const long long i0 = faces[3 * k], i1 = faces[3 * k + 1], i2 = faces[3 * k + 2];   // leaves hold split faces several times)
+            sA[threadIdx.x] = make_float4(verts[3 * i0], verts[3 * i0 + 1], verts[3 * i0 + 2], __int_as_float((int)k));
+            sB[threadIdx.x] = make_float4(verts[3 * i1], verts[3 * i1 + 1], verts[3 * i1 + 2], 0.0f);
+            sC[threadIdx.x] = make_float4(verts[3 * i2], verts[3 * i2 + 1], verts[3 * i2 + 2], 0.0f);
         }
         __syncthreads();
         const int cnt = (int)((f1 - t0) < WQ ? (f1 - t0) : WQ);
@@ -121,8 +123,9 @@ int winding_run(const mcs_bvh* b, const float* pts, const int32_t* excl, long lo
     const int n_chunks = winding_chunks(b->F, n);
     const long long fpc = ceil_div64(ceil_div64(b->F, n_chunks), WQ) * WQ;
     const dim3 grid((unsigned)ceil_div64(n, WQ), (unsigned)n_chunks);
-    mcs_note_launch(), winding_partial_kernel<<<grid, WQ, 0, st>>>(b->tris, b->F, pts, excl, n, fpc, partial);
+    mcs_note_launch(), winding_partial_kernel<<<grid, WQ, 0, st>>>(b->verts, b->faces, b->F, pts, excl, n, fpc, partial);
     mcs_note_launch(), winding_reduce_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(partial, n, n_chunks, w);
+    mcs_bvh_touch(b, st);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

@@ -73,36 +73,73 @@ MESHES = {
 }
 
 
+@pytest.mark.parametrize("split", [False, True])
 @pytest.mark.parametrize("name", list(MESHES))
-def test_lbvh_invariants(api, name):
+def test_lbvh_invariants(api, name, split):
+    """Structure of the packed tree.  split=False: one leaf per face.  split=True (the default build): long thin
+    faces enter as several leaf references, one per slab across their longest edge; every face
+    keeps at least one leaf, an unsplit face has exactly its vertex box, and the slab boxes of a split face cover it."""
     v, f = MESHES[name]()
     F = len(f)
-    bvh = _bvh(api, v, f)
+    bvh = api.build_bvh(_cuda(v, torch.float32), _cuda(f, torch.int32), split=split)
     info = bvh.info()
-    assert info.F == F and info.n_nodes == F - 1 and info.V == len(v)
+    R = info.n_leaves
+    assert info.F == F and info.n_nodes == R - 1 and info.V == len(v)
+    assert R == F if not split else F <= R <= 2 * F                   # default budget: one extra leaf per face on average
     nodes, leaf_tri, morton = bvh.dump()
     box0, box1, c0, c1, parent = _unpack_nodes(nodes)
     m = morton.cpu().numpy().astype(np.uint64)
-    assert (m[1:] >= m[:-1]).all()                                    # keys sorted
+    assert len(m) == R and (m[1:] >= m[:-1]).all()                    # keys sorted
     lt = leaf_tri.cpu().numpy()
-    assert np.array_equal(np.sort(lt), np.arange(F))                  # every face in exactly one leaf
+    per_face = np.bincount(lt, minlength=F)
+    assert len(lt) == R and per_face.min() >= 1 and per_face.sum() == R   # every face in at least one leaf
+    if not split:
+        assert per_face.max() == 1
     children = np.concatenate([c0, c1])
     leaves = ~children[children < 0]
     inner = children[children >= 0]
-    assert np.array_equal(np.sort(leaves), np.arange(F))
-    assert np.array_equal(np.sort(inner), np.arange(1, F - 1))        # every node but the root has one parent
+    assert np.array_equal(np.sort(leaves), np.arange(R))              # every leaf reference hangs in the tree once
+    assert np.array_equal(np.sort(inner), np.arange(1, R - 1))        # every node but the root has one parent
     assert parent[0] == -1
+    leaf_box = np.zeros((R, 6), np.float32)
     for c, boxes in ((c0, box0), (c1, box1)):
         isleaf = c < 0
-        # triangle inside its leaf box (exactly: the box is the min/max of its fp32 vertices)
-        tv = v[f[lt[~c[isleaf]]]]
-        assert np.array_equal(boxes[isleaf][:, :3], tv.min(1)) and np.array_equal(boxes[isleaf][:, 3:], tv.max(1))
+        leaf_box[~c[isleaf]] = boxes[isleaf]
         # child box = union of the grandchildren's boxes, and parent links agree
         ii = c[~isleaf]
         lo = np.minimum(box0[ii][:, :3], box1[ii][:, :3])
         hi = np.maximum(box0[ii][:, 3:], box1[ii][:, 3:])
         assert np.array_equal(boxes[~isleaf][:, :3], lo) and np.array_equal(boxes[~isleaf][:, 3:], hi)
         assert np.array_equal(parent[ii], np.nonzero(~isleaf)[0])
+    # an unsplit face lies in its leaf box exactly (the box is the min/max of its fp32 vertices)
+    single = per_face[lt] == 1
+    tv = v[f[lt[single]]]
+    assert np.array_equal(leaf_box[single][:, :3], tv.min(1)) and np.array_equal(leaf_box[single][:, 3:], tv.max(1))
+    # a split face: long and thin, and every point of it lies in at least one of its slab boxes
+    multi = np.flatnonzero(per_face > 1)
+    if split and name == "stress20k":
+        assert len(multi) > 50
+    if len(multi):
+        vv = v.astype(np.float64)
+        a, b, c = vv[f[multi, 0]], vv[f[multi, 1]], vv[f[multi, 2]]
+        L2 = np.maximum(np.maximum(((b - a) ** 2).sum(1), ((c - b) ** 2).sum(1)), ((a - c) ** 2).sum(1))
+        area2 = np.linalg.norm(np.cross(b - a, c - a), axis=1)
+        assert (L2 > 7.9 * area2).all()                               # aspect L^2 / 2A > 8
+        rng = np.random.default_rng(0)
+        w = rng.dirichlet(np.ones(3), size=64)                        # random interior points ...
+        w = np.concatenate([w, np.eye(3), [[0.5, 0.5, 0], [0, 0.5, 0.5], [0.5, 0, 0.5]],     # ... corners, edge midpoints,
+                            np.stack([np.linspace(0, 1, 33), 1 - np.linspace(0, 1, 33), np.zeros(33)], 1),   # and the edges
+                            np.stack([np.zeros(33), np.linspace(0, 1, 33), 1 - np.linspace(0, 1, 33)], 1),
+                            np.stack([1 - np.linspace(0, 1, 33), np.zeros(33), np.linspace(0, 1, 33)], 1)])
+        order = np.argsort(lt, kind="stable")
+        start = np.concatenate([[0], np.cumsum(per_face)])
+        for k, face in enumerate(multi[:400]):
+            pts = w @ np.stack([a[k], b[k], c[k]])
+            bx = leaf_box[order[start[face]:start[face + 1]]].astype(np.float64)
+            inside = ((pts[:, None, :] >= bx[None, :, :3]) & (pts[:, None, :] <= bx[None, :, 3:])).all(2).any(1)
+            assert inside.all(), (face, per_face[face])
+            tvf = v[f[face]]
+            assert (bx[:, :3].min(0) <= tvf.min(0)).all() and (bx[:, 3:].max(0) >= tvf.max(0)).all()
     # area and AABB against numpy on the same fp32 inputs
     vv = v.astype(np.float64)
     area = 0.5 * np.linalg.norm(np.cross(vv[f[:, 1]] - vv[f[:, 0]], vv[f[:, 2]] - vv[f[:, 0]]), axis=1).sum()
@@ -110,6 +147,35 @@ def test_lbvh_invariants(api, name):
     used = np.unique(f)
     assert np.array_equal(np.array(info.aabb_lo[:]), v[used].min(0)) and np.array_equal(np.array(info.aabb_hi[:]), v[used].max(0))
     assert info.max_depth >= int(np.ceil(np.log2(F)))
+    assert info.sah_cost > 0.0
+
+
+def test_sliver_splitting_lowers_the_tree_cost_and_changes_no_query(api):
+    """Stress mesh with rotated sliver strips: the surface-area cost of the tree drops with the default build, the
+    closest-point results are bit-identical with and without splitting (every reference carries the whole triangle),
+    and so are the walk records of both operators."""
+    v, f, info = stress_mesh(n_faces=60_000, n_components=12, seed=5)
+    vd, fd = _cuda(v, torch.float32), _cuda(f, torch.int32)
+    b0, b1 = api.build_bvh(vd, fd, split=False), api.build_bvh(vd, fd)
+    i0, i1 = b0.info(), b1.info()
+    assert i1.n_leaves > i0.n_leaves == len(f)
+    assert i1.sah_cost < 0.7 * i0.sah_cost, (i0.sah_cost, i1.sah_cost)
+    q = np.concatenate([near_surface_queries(v, f, 30000, seed=5), far_field_queries(v, 10000, seed=6)])
+    qd = _cuda(q, torch.float32)
+    r0, r1 = api.closest_point(b0, qd), api.closest_point(b1, qd)
+    assert all(torch.equal(x, y) for x, y in zip(r0, r1))
+    from synth import fps_samples
+    smp = fps_samples(v, f, 256, n_candidates=10_000, seed=1)
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    comp = int(np.bincount(info["face_component"]).argmax())
+    cv = v[np.unique(f[info["face_component"] == comp])]
+    origin = tuple(float(x) for x in 0.5 * (cv.min(0) + cv.max(0)))
+    for ext in (False, True):
+        P = api.Params(seed=2, walks_per_sample=128, eps=1e-3, kelvin_origin=origin)
+        ra, sa, sta = api.run_walks(b0, S, P, ext, want_stats=True)
+        rb, sb, stb = api.run_walks(b1, S, P, ext, want_stats=True)
+        assert torch.equal(ra.view(torch.int32), rb.view(torch.int32)) and torch.equal(sa, sb)
+        assert stb.n_tris_tested < sta.n_tris_tested               # fewer triangle tests for the same walks
 
 
 def _tie_free(orc, q, rel_gap=1e-4):
