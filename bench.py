@@ -79,7 +79,8 @@ def cfg3_config(wl, args, extra=None):
                      f"{100 * wl['sliver']:.1f}% slivers, {100 * wl['dup']:.1f}% duplicated, {100 * wl['flipped']:.1f}% flipped faces), "
                      f"{n_s} FPS samples of {args.candidates} candidates x {args.walks} walks per operator, interior + exterior "
                      f"(killing off: the paper's default, PAPER.md:383), sidedness pre-pass, hat basis, sparse COO output, "
-                     f"eps={args.eps:g}, cap={args.cap:g} deg, Philox seed {args.seed}",
+                     f"eps={args.eps:g}, cap={args.cap:g} deg, Philox seed {args.seed}, "
+                     + (f"far-field queries by lower bound (far_alpha={args.far_alpha:g}, near={args.far_near:g} eps)" if args.far_alpha > 0 else "exact closest-point queries"),
          "operators": ["interior", "exterior"], "walks_per_operator": n_s * args.walks,
          "includes_bvh_build": True, "includes_sidedness_prepass": True, "output": "coo (upper triangle)",
          "l2_policy": "inputs larger than L2 (tree 256 MB + records 2.6 GB per step) and a 256 MiB buffer written between timed steps",
@@ -476,8 +477,9 @@ def run_ours(args):
     tri_h, bary_h, w_h = (torch.as_tensor(wl[k]).pin_memory() for k in ("tri", "bary", "weight"))
     vd, fd = v_h.to(dev), f_h.to(dev)
     S0 = api.Samples(tri_h.to(dev), bary_h.to(dev), w_h.to(dev))
-    P_int = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap)
-    P_ext = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, kelvin_origin=wl["origin"])
+    far = dict(far_alpha=args.far_alpha, far_near_factor=args.far_near)
+    P_int = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, **far)
+    P_ext = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, kelvin_origin=wl["origin"], **far)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     # deterministic work counts of one step (counter build of the kernels) and the size of the sparse outputs;
@@ -596,6 +598,7 @@ def run_ours(args):
             "dtn_matrices_per_s": world * 2.0 / (ms_per_step * 1e-3),
             "walk_steps_per_step": steps_per_step, "queries_per_step": queries_per_step,
             "nnz": {"interior": nnz[0], "exterior": nnz[1]},
+            "far_query_fraction": (st_i.n_far_queries + st_e.n_far_queries) / float(max(queries_per_step, 1)),
             "cut_fraction": cut, "cut_walks": {"interior": st_i.n_truncated, "exterior": st_e.n_truncated,
                                                "rule": "R10 max_steps / R10b left the bounding box / R10c inside the solid (DESIGN.md section 2)"},
             "discarded_samples": {"interior": st_i.n_discarded, "exterior": st_e.n_discarded},
@@ -632,6 +635,8 @@ def main():
     ap.add_argument("--eps", type=float, default=1e-3)
     ap.add_argument("--cap", type=float, default=2.5)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--far-alpha", type=float, default=0.0, help="mcs_params.far_alpha: > 0 answers far-field queries with a lower bound of the distance")
+    ap.add_argument("--far-near", type=float, default=4.0, help="mcs_params.far_near_factor (multiples of eps)")
     ap.add_argument("--cpu-samples", type=int, default=16, help="sample points of the cpu_baseline leg")
     ap.add_argument("--cpu-walks", type=int, default=8, help="walks per sample point of the cpu_baseline leg")
     ap.add_argument("--ref-samples", type=int, default=8, help="sample points per step of --impl reference")

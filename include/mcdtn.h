@@ -164,6 +164,14 @@ typedef struct {
                                        interior only: walks start at s - inset * n_s, update
                                        (a_i / (W inset)) b_s (b_s - b_t)^T, symmetrised; NOT PSD at finite N */
     float    inset;              /* estimator 1: inset distance (the paper's epsilon of Eq. 13), > 0 */
+    float    far_alpha;          /* 0: every closest-point query is exact (default).  > 0: far-field queries return a LOWER
+                                    BOUND of the distance: a sub-tree whose box diagonal is <= far_alpha x its box distance
+                                    is not descended, its box distance stands for its faces.  The walker then jumps with a
+                                    radius between D / (1 + far_alpha) and D.  WoS only needs a ball inside the domain
+                                    (PAPER.md:155), so the estimator is unchanged in expectation; single walks differ from
+                                    the exact run.  The shell test and the exit point always come from an exact query.
+                                    Deterministic (independent of the schedule).  Typical: 0.5                          */
+    float    far_near_factor;    /* far_alpha > 0: boxes closer than this many eps are always descended (0: 16; >= 2)  */
 } mcs_params;
 
 typedef struct {
@@ -190,6 +198,7 @@ typedef struct {                 /* host; filled when passed non-NULL (forces a 
     int64_t n_prep_queries, n_prep_nodes, n_prep_tris;  /* of which: the tangent-ball traversals (A2) */
     int64_t n_entries, n_unique;          /* (row,col,value) records expanded / after reduction    */
     int64_t workspace_needed;             /* bytes; set on MCS_ENOMEM too                           */
+    int64_t n_far_queries;                /* walk-kernel queries answered by a lower bound (far_alpha > 0; counter build) */
     int64_t nodes_hist[16];               /* walk-kernel queries by floor(log2(nodes visited)), bin 15 = rest */
     int32_t cuda_error;                   /* cudaError_t on MCS_ECUDA                               */
     int32_t pad_;

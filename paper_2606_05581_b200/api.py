@@ -52,7 +52,7 @@ class _Params(C.Structure):
                 ("rmax_override", C.c_float), ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
                 ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64),
-                ("estimator", C.c_int32), ("inset", C.c_float)]
+                ("estimator", C.c_int32), ("inset", C.c_float), ("far_alpha", C.c_float), ("far_near_factor", C.c_float)]
 
 
 class _Matrix(C.Structure):
@@ -66,7 +66,7 @@ class Stats(C.Structure):
                 ("n_truncated", C.c_int64), ("n_steps", C.c_int64), ("n_queries", C.c_int64),
                 ("n_nodes_visited", C.c_int64), ("n_tris_tested", C.c_int64), ("n_prep_queries", C.c_int64),
                 ("n_prep_nodes", C.c_int64), ("n_prep_tris", C.c_int64), ("n_entries", C.c_int64),
-                ("n_unique", C.c_int64), ("workspace_needed", C.c_int64), ("nodes_hist", C.c_int64 * 16),
+                ("n_unique", C.c_int64), ("workspace_needed", C.c_int64), ("n_far_queries", C.c_int64), ("nodes_hist", C.c_int64 * 16),
                 ("cuda_error", C.c_int32),
                 ("pad_", C.c_int32)]
 
@@ -135,6 +135,8 @@ class Params:
     coo_capacity: int = 0
     estimator: int = 0                   # 0: Alg. 2; 1: Alg. 1 (naive finite difference, interior only)
     inset: float = 0.0                   # Alg. 1: walks start at s - inset * n_s
+    far_alpha: float = 0.0               # > 0: far-field queries return a lower bound of the distance (mcs_params.far_alpha)
+    far_near_factor: float = 0.0         # boxes closer than this many eps are always descended (0: 16)
 
     def c(self) -> _Params:
         p = _Params(seed=self.seed, walks_per_sample=self.walks_per_sample, max_steps=self.max_steps,
@@ -143,7 +145,8 @@ class Params:
                     importance_sample=int(self.importance_sample), antithetic=int(self.antithetic),
                     include_killing=int(self.include_killing), n_kill_walks=int(self.n_kill_walks),
                     output_kind=int(self.output_kind), coo_capacity=int(self.coo_capacity),
-                    estimator=int(self.estimator), inset=float(self.inset))
+                    estimator=int(self.estimator), inset=float(self.inset), far_alpha=float(self.far_alpha),
+                    far_near_factor=float(self.far_near_factor))
         p.kelvin_origin[:] = [float(x) for x in self.kelvin_origin]
         return p
 

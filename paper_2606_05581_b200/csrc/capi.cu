@@ -81,6 +81,7 @@ void fill_stats(mcs_stats* hs, const unsigned long long* h, const mcs_samples* s
     hs->n_prep_tris = (int64_t)h[ST_PREP_TRIS];
     hs->n_entries = (int64_t)h[ST_ENTRIES];
     hs->n_unique = (int64_t)h[ST_UNIQUE];
+    hs->n_far_queries = (int64_t)h[ST_FAR];
     for (int b = 0; b < 16; ++b) hs->nodes_hist[b] = (int64_t)h[ST_HIST + b];
 }
 

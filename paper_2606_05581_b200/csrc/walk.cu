@@ -405,11 +405,19 @@ struct CoopState {
     float3 xq;
     ClosestHit h;
     float lim;
+    float lb2, dnear2, alpha2;               // far-field lower bound (FAR builds): running minimum, near threshold, alpha^2
     int sp, cur;
     unsigned n_nodes, n_tris, q_nodes;       // increments (COUNT builds)
 };
 
-template <bool COUNT>
+// Squared diagonal of child box k of a wide node held in q0, q1, q2 (24 floats: lo.xyz, hi.xyz per child).
+#define MCS_SQ(x) ((x) * (x))
+#define MCS_DIAG0(q0, q1, q2) (MCS_SQ(q0.lo.w - q0.lo.x) + MCS_SQ(q0.hi.x - q0.lo.y) + MCS_SQ(q0.hi.y - q0.lo.z))
+#define MCS_DIAG1(q0, q1, q2) (MCS_SQ(q1.lo.y - q0.hi.z) + MCS_SQ(q1.lo.z - q0.hi.w) + MCS_SQ(q1.lo.w - q1.lo.x))
+#define MCS_DIAG2(q0, q1, q2) (MCS_SQ(q1.hi.w - q1.hi.x) + MCS_SQ(q2.lo.x - q1.hi.y) + MCS_SQ(q2.lo.y - q1.hi.z))
+#define MCS_DIAG3(q0, q1, q2) (MCS_SQ(q2.hi.y - q2.lo.z) + MCS_SQ(q2.hi.z - q2.lo.w) + MCS_SQ(q2.hi.w - q2.hi.x))
+
+template <bool COUNT, bool FAR>
 __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, const WideNode* __restrict__ wide,
                                                const PackedTri* __restrict__ tris, int L, float mesh_scale,
                                                int* __restrict__ co_nodes, int* __restrict__ co_leaves,
@@ -433,6 +441,9 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
     float bd2 = __shfl_sync(FULL, h.d2, L), bv = __shfl_sync(FULL, h.v, L), bw = __shfl_sync(FULL, h.w, L);
     int btri = __shfl_sync(FULL, h.tri, L), bk = __shfl_sync(FULL, h.k, L);
     float wlim = __shfl_sync(FULL, lim, L);
+    float wlb = FAR ? __shfl_sync(FULL, S.lb2, L) : CUDART_INF_F;
+    const float wnear2 = FAR ? __shfl_sync(FULL, S.dnear2, L) : 0.0f;
+    const float alpha2 = S.alpha2;                                   // warp-uniform
     // lane L moves its pending items to the warp lists
     int ncount = 0, lcount = 0;
     if (lane == L) {
@@ -471,7 +482,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
             if (md2 < bd2 || (md2 == bd2 && morig < btri)) {
                 bd2 = md2; btri = morig;
                 bk = __shfl_sync(FULL, kk, mlane); bv = __shfl_sync(FULL, v, mlane); bw = __shfl_sync(FULL, w, mlane);
-                wlim = prune_limit(bd2, xq, mesh_scale);
+                wlim = prune_limit(FAR ? fminf(bd2, wlb) : bd2, xq, mesh_scale);
             }
             __syncwarp();
         } else {
@@ -480,6 +491,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
             if (ncount > COOP_SOFT) np = 1;                              // depth-first, one node at a time: bounded growth
             bool in0 = false, in1 = false, in2 = false, in3 = false;
             int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+            float mylb = CUDART_INF_F;
             if (lane < np) {
                 const char* wn = reinterpret_cast<const char*>(wide + co_nodes[ncount - np + lane]);
                 const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32), q2 = ldg256(wn + 64), q3 = ldg256(wn + 96);
@@ -489,6 +501,22 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
                 in2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y) <= wlim;
                 in3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w) <= wlim;
                 c0 = __float_as_int(q3.lo.x); c1 = __float_as_int(q3.lo.y); c2 = __float_as_int(q3.lo.z); c3 = __float_as_int(q3.lo.w);
+                if (FAR) {
+                    // a sub-tree whose box is small against its distance stands for its faces: its box distance is a lower
+                    // bound of theirs (see walk_kernel); it is not descended
+                    const float e0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
+                    const float e1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
+                    const float e2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
+                    const float e3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
+                    if (in0 && c0 >= 0 && e0 >= wnear2 && MCS_DIAG0(q0, q1, q2) <= alpha2 * e0) { mylb = fminf(mylb, e0); in0 = false; }
+                    if (in1 && c1 >= 0 && e1 >= wnear2 && MCS_DIAG1(q0, q1, q2) <= alpha2 * e1) { mylb = fminf(mylb, e1); in1 = false; }
+                    if (in2 && c2 >= 0 && e2 >= wnear2 && MCS_DIAG2(q0, q1, q2) <= alpha2 * e2) { mylb = fminf(mylb, e2); in2 = false; }
+                    if (in3 && c3 >= 0 && e3 >= wnear2 && MCS_DIAG3(q0, q1, q2) <= alpha2 * e3) { mylb = fminf(mylb, e3); in3 = false; }
+                }
+            }
+            if (FAR) {
+                for (int off = 16; off > 0; off >>= 1) mylb = fminf(mylb, __shfl_xor_sync(FULL, mylb, off));
+                if (mylb < wlb) { wlb = mylb; wlim = fminf(wlim, prune_limit(wlb, xq, mesh_scale)); }
             }
             visited += (unsigned)np;
             ncount -= np;
@@ -509,6 +537,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
     if (lane == L) {
         h.d2 = bd2; h.tri = btri; h.k = bk; h.v = bv; h.w = bw;
         lim = wlim;
+        if (FAR) S.lb2 = wlb;
         if (COUNT) q_nodes += visited;
     }
 }
@@ -518,7 +547,22 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 // serves the lanes that wait for a node AND the lanes that wait for a triangle -- both loads are issued before
 // either is used -- and then the lanes that wait for a transition, instead of one kind per pass: every live lane
 // advances every pass.  The arithmetic of a visit is unchanged.
-template <bool EXT, bool COUNT, bool COOP, bool MERGED>
+// FAR (mcs_params.far_alpha > 0): far-field queries answered by a LOWER BOUND of the distance.  Walk-on-spheres needs a
+// ball about the walker that lies inside the domain, not the largest one, and an exact query from far
+// away is expensive for a reason no tree removes: every face whose box enters the ball of radius D about the query
+// point has to be tested, and on a finely tessellated surface that is hundreds of faces (BASELINE config 3: 70-150
+// triangle tests per query; the paper names the exterior's far queries as its bottleneck).  During
+// the traversal a sub-tree whose box is small against its distance -- diagonal <= alpha x box distance, and box
+// distance >= the near threshold -- is not descended: its box distance stands for its faces (they are at most
+// (1 + alpha) times farther).  The query then returns the minimum over a CUT of the tree (such boxes, and real faces
+// where no ancestor qualified).  Which nodes qualify depends on the query point only, pruning is against that running
+// minimum with the usual margin, so the result does not depend on the traversal order or the schedule.  If the
+// minimum is a real face the query is exact as before (exit point, termination test); if it is a box the walker
+// jumps with that lower bound as its radius, at least 1 / (1 + alpha) of the largest possible one, and the shell test
+// is never taken from it: boxes closer than the near threshold (a multiple of eps, in the exterior the distance whose
+// Kelvin radius is that multiple) are always descended.  The estimator is the same in expectation; single walks differ
+// from the exact run, so record-level parity tests run with far_alpha = 0 and matrices are compared statistically.
+template <bool EXT, bool COUNT, bool COOP, bool MERGED, bool FAR>
 __global__ void __launch_bounds__(WT, MERGED ? 4 : WALK_MIN_BLOCKS)      // small jobs: registers instead of occupancy
 walk_kernel(WalkGeom g, WalkArgs a)
 {
@@ -554,9 +598,10 @@ walk_kernel(WalkGeom g, WalkArgs a)
     float rho = 0.f, far_radius = -1.0f;         // far_radius >= 0: jump radius known without a query (exterior far field)
     ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.f;
     float lim = 3.0e38f;
+    float lb2 = CUDART_INF_F, dnear2 = 0.0f;     // FAR: smallest box distance of the sub-trees taken as a whole; near threshold
     int cur = CUR_NONE, sp = 0;
     // statistics
-    unsigned n_nodes = 0, n_tris = 0, q_nodes = 0;
+    unsigned n_nodes = 0, n_tris = 0, q_nodes = 0, n_far = 0;
     int q_visits = 0;                            // nodes visited by the current query (hand-over to the warp at COOP_MIN)
     unsigned n_steps = 0, n_queries = 0, n_trunc = 0;
     int age_tri = 0, age_trans = 0;              // warp-uniform: passes since the kind last ran (or was last unwanted)
@@ -617,7 +662,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 const float td2 = closest_point_triangle(xq, T, CUDART_INF_F, tv, tw);
                 if (td2 < h.d2 || (td2 == h.d2 && T.orig < h.tri)) { h.d2 = td2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
                 if (COUNT) ++n_tris;
-                lim = prune_limit(h.d2, xq, a.mesh_scale);
+                lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);
                 cur = CUR_NONE;
               } else {
                 if (COUNT) { ++n_nodes; ++q_nodes; }
@@ -627,6 +672,14 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 float d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
                 float d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
                 int c0 = __float_as_int(q3.lo.x), c1 = __float_as_int(q3.lo.y), c2 = __float_as_int(q3.lo.z), c3 = __float_as_int(q3.lo.w);
+                if (FAR) {
+                    bool any = false;
+                    if (c0 >= 0 && d0 >= dnear2 && d0 <= lim && MCS_DIAG0(q0, q1, q2) <= a.far_alpha2 * d0) { lb2 = fminf(lb2, d0); d0 = CUDART_INF_F; any = true; }
+                    if (c1 >= 0 && d1 >= dnear2 && d1 <= lim && MCS_DIAG1(q0, q1, q2) <= a.far_alpha2 * d1) { lb2 = fminf(lb2, d1); d1 = CUDART_INF_F; any = true; }
+                    if (c2 >= 0 && d2 >= dnear2 && d2 <= lim && MCS_DIAG2(q0, q1, q2) <= a.far_alpha2 * d2) { lb2 = fminf(lb2, d2); d2 = CUDART_INF_F; any = true; }
+                    if (c3 >= 0 && d3 >= dnear2 && d3 <= lim && MCS_DIAG3(q0, q1, q2) <= a.far_alpha2 * d3) { lb2 = fminf(lb2, d3); d3 = CUDART_INF_F; any = true; }
+                    if (any) lim = fminf(lim, prune_limit(lb2, xq, a.mesh_scale));
+                }
                 // partial sorting network on (distance, child): (0,1)(2,3)(0,2) puts the nearest child first; the other
                 // three go on the stack as they are (the full network, two more comparators, visits 0.15 % fewer nodes
                 // and costs 1.5 % more time); empty slots have d = +inf
@@ -646,9 +699,10 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 const int L = __ffs(heavy) - 1;
                 CoopState cs;
                 cs.xq = xq; cs.h = h; cs.lim = lim; cs.sp = sp; cs.cur = cur; cs.n_nodes = 0; cs.n_tris = 0; cs.q_nodes = 0;
-                coop_finish_query<COUNT>(g.nodes, g.wide, g.tris, L, a.mesh_scale, co_nodes, co_leaves,
-                                         stk.s_ref, stk.s_d, stk.l_ref, stk.l_d, &cs);
-                if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; }
+                cs.lb2 = lb2; cs.dnear2 = dnear2; cs.alpha2 = a.far_alpha2;
+                coop_finish_query<COUNT, FAR>(g.nodes, g.wide, g.tris, L, a.mesh_scale, co_nodes, co_leaves,
+                                              stk.s_ref, stk.s_d, stk.l_ref, stk.l_d, &cs);
+                if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; if (FAR) lb2 = cs.lb2; }
                 if (COUNT) { n_nodes += cs.n_nodes; n_tris += cs.n_tris; q_nodes += cs.q_nodes; }
             }
         }
@@ -656,7 +710,7 @@ walk_kernel(WalkGeom g, WalkArgs a)
             if (kind == KIND_TRI) {
                 test_triangle(g.tris, ~cur, xq, h, lim);
                 if (COUNT) ++n_tris;
-                lim = prune_limit(h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
+                lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
                 cur = CUR_NONE;
             }
         }
@@ -672,9 +726,13 @@ walk_kernel(WalkGeom g, WalkArgs a)
                     ++n_queries;
                     if (COUNT) { atomicAdd(&a.stats[ST_HIST + (q_nodes > 0 ? min(31 - __clz(q_nodes), 15) : 0)], 1ull); q_nodes = 0; }
                     prev = h.k;
-                    const float D = sqrtf(h.d2);
+                    // FAR: the minimum over the cut is a box, not a face: jump with the lower bound, no shell test
+                    const bool far_hit = FAR && lb2 < h.d2;
+                    if (FAR && COUNT && far_hit) ++n_far;
+                    const float D = sqrtf(far_hit ? lb2 : h.d2);
+                    if (FAR) h.d2 = D * D;                        // the rules below read the distance from h.d2
                     radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
-                    if (radius < a.eps) {
+                    if (!far_hit && radius < a.eps) {
                         float wgt = wfac;
                         if (EXT) {
                             const float3 t = hit_point(g.tris, h) - o;
@@ -810,6 +868,17 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
                 lim = 3.0e38f;                               // finite: the +inf of an empty node slot never passes
                 sp = 0; cur = CUR_NONE; q_visits = 0;
+                if (FAR) {
+                    lb2 = CUDART_INF_F;
+                    if (EXT) {
+                        // smallest primal distance whose Kelvin radius D / (rho (rho + D)) <= R* reaches far_near = k eps
+                        const float tr = a.far_near * rho;
+                        const float dn = tr < 0.5f ? tr * rho / (1.0f - tr) : 3.0e18f;
+                        dnear2 = dn * dn;
+                    } else {
+                        dnear2 = a.far_near * a.far_near;
+                    }
+                }
                 if (need_query) {
                     if (prev >= 0) { stack_push(stk, sp, 0, 0.0f); cur = ~prev; }   // last closest face first: a tight bound
                     else cur = 0;                                                   // root
@@ -819,12 +888,12 @@ walk_kernel(WalkGeom g, WalkArgs a)
     }
 
     // ---- statistics ----------------------------------------------------------
-    unsigned vals[5] = { n_steps, n_queries, n_trunc, n_nodes, n_tris };
-    for (int q = 0; q < 5; ++q) {
+    unsigned vals[6] = { n_steps, n_queries, n_trunc, n_nodes, n_tris, n_far };
+    for (int q = 0; q < 6; ++q) {
         unsigned long long v = vals[q];
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
         if (lane == 0 && v) {
-            const int idx = q == 0 ? ST_STEPS : q == 1 ? ST_QUERIES : q == 2 ? ST_TRUNCATED : q == 3 ? ST_NODES : ST_TRIS;
+            const int idx = q == 0 ? ST_STEPS : q == 1 ? ST_QUERIES : q == 2 ? ST_TRUNCATED : q == 3 ? ST_NODES : q == 4 ? ST_TRIS : ST_FAR;
             atomicAdd(&a.stats[idx], v);
         }
     }
@@ -859,6 +928,7 @@ int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, in
     if (p->estimator == 1 && (exterior || !(p->inset > 0.0f))) return MCS_EINVAL;      // Alg. 1 is the interior estimator
     if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
     if (s->n_s * (int64_t)p->walks_per_sample >= ((int64_t)1 << 40)) return MCS_EINVAL;
+    if (!(p->far_alpha >= 0.0f) || p->far_alpha > 4.0f || !(p->far_near_factor >= 0.0f)) return MCS_EINVAL;
     return MCS_OK;
 }
 
@@ -978,6 +1048,8 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.naive = p->estimator == 1; a.inv_inset = p->estimator == 1 ? 1.0f / p->inset : 0.0f;
     a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
     a.mesh_scale = mesh_scale;
+    a.far_alpha2 = p->far_alpha * p->far_alpha;
+    a.far_near = (p->far_near_factor > 0.0f ? fmaxf(p->far_near_factor, 2.0f) : 16.0f) * p->eps;   // never below 2 eps
     {
         const float dx = hi.x - lo.x, dy = hi.y - lo.y, dz = hi.z - lo.z;
         a.escape = exterior ? 3.0e38f : sqrtf(dx * dx + dy * dy + dz * dz);
@@ -999,12 +1071,15 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     // Small jobs (a few walks per lane) run the merged-pass variant, always with the cooperative path.
     const bool merged = total_walks < (long long)n_sm * 2048 * 4;
     typedef void (*walk_fn)(WalkGeom, WalkArgs);
-    static const walk_fn table[12] = {
-        walk_kernel<false, false, false, false>, walk_kernel<false, false, true, false>, walk_kernel<false, true, false, false>, walk_kernel<false, true, true, false>,
-        walk_kernel<true, false, false, false>,  walk_kernel<true, false, true, false>,  walk_kernel<true, true, false, false>,  walk_kernel<true, true, true, false>,
-        walk_kernel<false, false, true, true>,   walk_kernel<false, true, true, true>,   walk_kernel<true, false, true, true>,   walk_kernel<true, true, true, true> };
-    const walk_fn fn = merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)]
-                              : table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)];
+#define MCS_WK(E, C, P, M) { walk_kernel<E, C, P, M, false>, walk_kernel<E, C, P, M, true> }
+    static const walk_fn table[12][2] = {
+        MCS_WK(false, false, false, false), MCS_WK(false, false, true, false), MCS_WK(false, true, false, false), MCS_WK(false, true, true, false),
+        MCS_WK(true, false, false, false),  MCS_WK(true, false, true, false),  MCS_WK(true, true, false, false),  MCS_WK(true, true, true, false),
+        MCS_WK(false, false, true, true),   MCS_WK(false, true, true, true),   MCS_WK(true, false, true, true),   MCS_WK(true, true, true, true) };
+#undef MCS_WK
+    const int far = p->far_alpha > 0.0f ? 1 : 0;
+    const walk_fn fn = merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)][far]
+                              : table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)][far];
     MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
     if (per_sm < 1) per_sm = 1;
     const long long total = a.n_s * a.W + a.n_kill;

@@ -7,6 +7,7 @@ enum {
     ST_STEPS, ST_QUERIES, ST_TRUNCATED, ST_DISCARDED, ST_NODES, ST_TRIS,
     ST_ENTRIES, ST_UNIQUE,
     ST_PREP_QUERIES, ST_PREP_NODES, ST_PREP_TRIS,   // tangent-ball share of ST_QUERIES / ST_NODES / ST_TRIS
+    ST_FAR,             // queries answered by a lower bound (far_alpha > 0)
     ST_HIST = 16,       // 16 bins: queries of the walk kernel by floor(log2(nodes visited))
     ST_COUNT = 32
 };
@@ -33,6 +34,7 @@ struct WalkArgs {
     float ox, oy, oz, Rmax;
     float mesh_scale;              // |coordinates|_1 bound of the mesh (prune_limit)
     float escape;                  // interior: AABB diagonal (R10b); exterior: +inf
+    float far_alpha2, far_near;    // far-field lower-bound queries: alpha^2 (0: exact queries only), near threshold k eps
     uint32_t key0, key1;
     float4* records;               // mcs_record viewed as float4
     int32_t* steps;
