@@ -486,7 +486,7 @@ def run_ours(args):
     # outside the timed region
     bvh0 = api.build_bvh(vd, fd)
     info = bvh0.info()
-    nrm0, _ = api.orient_samples(bvh0, S0)
+    nrm0, _ = api.orient_samples_fast(bvh0, S0, beta=args.orient_beta) if args.orient_beta > 0 else api.orient_samples(bvh0, S0)
     S = api.Samples(S0.tri, S0.bary, S0.weight, nrm0)
     ci, st_i = api.estimate_dtn_coo(bvh0, S, P_int, False, want_stats=True)
     ce, st_e = api.estimate_dtn_coo(bvh0, S, P_ext, True, want_stats=True)
@@ -500,7 +500,7 @@ def run_ours(args):
 
     def step(profile):
         bvh = api.build_bvh(vd, fd)
-        nrm, _ = api.orient_samples(bvh, S0)
+        nrm, _ = api.orient_samples_fast(bvh, S0, beta=args.orient_beta) if args.orient_beta > 0 else api.orient_samples(bvh, S0)
         Sx = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
         out = api.estimate_dtn_coo_both(bvh, Sx, P_int, P_ext, capacity=cap)
         if profile:
@@ -544,13 +544,13 @@ def run_ours(args):
     host_out = [tuple(torch.empty(cap, dtype=dt, pin_memory=True) for dt in (torch.int32, torch.int32, torch.float32)) for _ in range(2)]
     e2e_steps = max(1, min(args.steps, 3))
     for _ in range(2):
-        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, device=dev)
+        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, orient_beta=args.orient_beta, device=dev)
     barrier()
     t0 = time.perf_counter()
     e2e_each = []
     for _ in range(e2e_steps):
         tc = time.perf_counter()
-        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, device=dev)
+        r = api.estimate_dtn_host_coo(v_h, f_h, tri_h, bary_h, w_h, P_int, P_ext, host_out[0], host_out[1], orient_h_scale=1.0, orient_beta=args.orient_beta, device=dev)
         e2e_each.append((time.perf_counter() - tc) * 1e3)      # the call blocks until the entries are in host memory
         flush.fill_(1)
     barrier()
@@ -603,7 +603,7 @@ def run_ours(args):
                                                "rule": "R10 max_steps / R10b left the bounding box / R10c inside the solid (DESIGN.md section 2)"},
             "discarded_samples": {"interior": st_i.n_discarded, "exterior": st_e.n_discarded},
             "bvh": {"faces": int(info.F), "nodes": int(info.n_nodes), "max_depth": int(info.max_depth), "device_bytes": tree_bytes},
-            "call": "mcs_build_bvh + mcs_orient_samples + mcs_estimate_dtn_both (output_kind 1)",
+            "call": "mcs_build_bvh + " + ("mcs_orient_samples_fast" if args.orient_beta > 0 else "mcs_orient_samples") + " + mcs_estimate_dtn_both (output_kind 1)",
             "phase_ms_per_step": {"build+sidedness+flush": ms_per_step - float(np.mean([p.total_ms for p in phases])),
                                   "prep": float(np.mean([p.prep_ms for p in phases])), "walk": t_kernel * 1e3,
                                   "accumulate": float(np.mean([p.accumulate_ms for p in phases]))},
@@ -635,6 +635,7 @@ def main():
     ap.add_argument("--eps", type=float, default=1e-3)
     ap.add_argument("--cap", type=float, default=2.5)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--orient-beta", type=float, default=2.5, help="sidedness pre-pass: opening parameter of mcs_orient_samples_fast (0: exhaustive mcs_orient_samples)")
     ap.add_argument("--far-alpha", type=float, default=0.0, help="mcs_params.far_alpha: > 0 answers far-field queries with a lower bound of the distance")
     ap.add_argument("--far-near", type=float, default=4.0, help="mcs_params.far_near_factor (multiples of eps)")
     ap.add_argument("--cpu-samples", type=int, default=16, help="sample points of the cpu_baseline leg")

@@ -414,7 +414,8 @@ class _HostCoo(C.Structure):
 
 
 def estimate_dtn_host_coo(verts, faces, tri, bary, weight, params_interior: Params, params_exterior: Params,
-                          out_interior, out_exterior, orient_h_scale=0.0, normal=None, want_stats=False, device=None):
+                          out_interior, out_exterior, orient_h_scale=0.0, orient_beta=0.0, normal=None, want_stats=False,
+                          device=None):
     """The whole path from HOST tensors with sparse output (mcs_estimate_dtn_host_coo): upload, LBVH build, optional
     sidedness pre-pass, both estimators, download.  out_*: (row int32, col int32, val fp32) CPU tensors of equal
     length = capacity (pinned memory makes the copies asynchronous).  Returns dict(nnz_interior, nnz_exterior,
@@ -445,7 +446,8 @@ def estimate_dtn_host_coo(verts, faces, tri, bary, weight, params_interior: Para
     dev = torch.device("cuda" if device is None else device)
     with torch.cuda.device(dev):
         rc = lib().mcs_estimate_dtn_host_coo(_ptr(verts), C.c_int64(V), _ptr(faces), C.c_int64(F), C.byref(cs), C.byref(ci),
-                                             C.byref(ce), C.c_float(float(orient_h_scale)), C.byref(outs[0]), C.byref(outs[1]),
+                                             C.byref(ce), C.c_float(float(orient_h_scale)), C.c_float(float(orient_beta)),
+                                             C.byref(outs[0]), C.byref(outs[1]),
                                              C.byref(si) if si is not None else None, C.byref(se) if se is not None else None,
                                              _stream(dev))
     ni, ne = int(outs[0].nnz), int(outs[1].nnz)
@@ -638,6 +640,31 @@ def estimate_dtn_coo(bvh: Bvh, samples: Samples, params: Params, exterior: bool,
     raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")
 
 
+def accumulate_coo(bvh: Bvh, samples: Samples, params: Params, records, capacity: int | None = None, max_retries=6):
+    """A7 alone with sparse output (mcs_accumulate, output_kind 1): records [n,4] fp32 as run_walks returns them."""
+    import dataclasses
+    records = _dev(records, torch.float32, "records")
+    n = int(records.shape[0])
+    K = bvh.V
+    cap = int(capacity) if capacity else max(4096, min(K * (K + 1) // 2, 21 * n))
+    for _ in range(max_retries):
+        p = dataclasses.replace(params, output_kind=1, coo_capacity=cap)
+        cs, cb, cp = samples.c(), _basis(bvh), p.c()
+        need = int(lib().mcs_accumulate_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int64(n)))
+        ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+        row, col, val, nnz, m = _coo_buffers(K, cap, bvh.device)
+        with torch.cuda.device(bvh.device):
+            rc = lib().mcs_accumulate(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(records), C.c_int64(n),
+                                      _ptr(ws), C.c_size_t(need), C.byref(m), None, _stream(bvh.device))
+        if rc == MCS_ENOMEM and int(nnz.item()) > cap:
+            cap = min(K * (K + 1) // 2, max(2 * cap, 2 * int(nnz.item())))
+            continue
+        _check(rc, "mcs_accumulate (coo)")
+        k = int(nnz.item())
+        return CooMatrix(K, row[:k], col[:k], val[:k])
+    raise McsError(MCS_ENOMEM, "accumulate_coo", "capacity retries exhausted")
+
+
 def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params,
                           capacity: int | None = None, max_retries=6):
     """Interior and exterior DtN matrices in sparse COO form from one mcs_estimate_dtn_both call (walk kernels
@@ -726,6 +753,19 @@ def orient_samples(bvh, samples, h_scale=1.0):
         ws, need = _winding_ws(bvh, n, dev)
         _check(lib().mcs_orient_samples(bvh.handle, C.byref(cs), C.c_float(h_scale), _ptr(nrm), _ptr(d), _ptr(ws),
                                         C.c_size_t(need), _stream(dev)), "mcs_orient_samples")
+    return nrm, d
+
+
+def orient_samples_fast(bvh, samples, h_scale=1.0, beta=2.5):
+    """(normal [n_s,3], d [n_s]) as orient_samples, from the hierarchical evaluation (mcs_orient_samples_fast)."""
+    dev = samples.tri.device
+    n = int(samples.tri.shape[0])
+    nrm = torch.empty((n, 3), dtype=torch.float32, device=dev)
+    d = torch.empty(n, dtype=torch.float32, device=dev)
+    cs = samples.c()
+    with torch.cuda.device(dev):
+        _check(lib().mcs_orient_samples_fast(bvh.handle, C.byref(cs), C.c_float(h_scale), C.c_float(beta), _ptr(nrm), _ptr(d),
+                                             _stream(dev)), "mcs_orient_samples_fast")
     return nrm, d
 
 

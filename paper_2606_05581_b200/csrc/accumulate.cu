@@ -31,6 +31,9 @@ namespace {
 constexpr int AT = 256;
 constexpr int CH = 256;                               // record slots per level-1 block
 constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << 22;
+// Sparse output: the running list of unique entries is re-sorted with every chunk's new entries, so fewer, larger chunks
+// pay (B200: 180 GB; a 16 Mi-walk chunk takes about 17 GB of workspace per operator at BASELINE config 3's sizes).
+constexpr int64_t MAX_CHUNK_WALKS_COO = (int64_t)1 << 24;
 constexpr int MAX_ENTRIES_PER_PAIR = 21;              // upper triangle of a 6 x 6 block
 constexpr int RT = 1024;                              // entries per tile of the run reduction
 
@@ -184,6 +187,62 @@ pair_reduce_kernel(AccArgs a, long long j0, long long n, PairRec* __restrict__ p
         pairs[(long long)blockIdx.x * CH + rank] = r;
     }
     if (tid == 0) pair_counts[blockIdx.x] = (uint32_t)total;
+}
+
+// ---------------------------------------------------------------------------
+// Level 1b: pairs of one chunk that share (sample, exit face) are merged.  A sample's W walks span W / 256 level-1
+// blocks, and most of them land on the same few hundred faces, so the same pair comes out of many blocks (BASELINE
+// config 3, W = 4096: 5 pair records per distinct pair).  The chunk's pair records are stable-sorted by (sample, face)
+// and every run is folded into its first record, in slot order, after moving the moments to that record's reference
+// point: with delta = r_j - r_0,  A' = A + w delta,  M' = M + A delta^T + delta A^T + w delta delta^T.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(AT)
+pair_keys_kernel(const PairRec* __restrict__ pairs, const uint32_t* __restrict__ pair_counts, long long n_slots,
+                 long long first_sample, int face_bits, unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n_slots) return;
+    unsigned long long key = ~0ull >> 1;                                    // invalid slots sort last (63-bit keys)
+    if ((uint32_t)(i % CH) < pair_counts[i / CH]) {
+        const int sample = pairs[i].sample, tri = pairs[i].tri_t;
+        if (tri >= 0 && sample >= 0)
+            key = ((unsigned long long)((long long)sample - first_sample) << face_bits) | (unsigned long long)(unsigned)tri;
+    }
+    keys[i] = key;
+    vals[i] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(AT)
+pair_merge_kernel(const PairRec* __restrict__ pairs, const unsigned long long* __restrict__ keys, const uint32_t* __restrict__ vals,
+                  long long n_slots, PairRec* __restrict__ merged, uint32_t* __restrict__ merged_counts)
+{
+    const long long i = (long long)blockIdx.x * AT + threadIdx.x;
+    if (i >= n_slots) return;
+    if (i % CH == 0) merged_counts[i / CH] = CH;                            // every slot is looked at; tri_t = -1 marks the empty ones
+    const unsigned long long key = keys[i];
+    PairRec r;
+    r.sample = -1; r.tri_t = -1; r.w = 0.0f; r.A[0] = r.A[1] = r.A[2] = 0.0f;
+    for (int q = 0; q < 6; ++q) r.M[q] = 0.0f;
+    r.ref1 = r.ref2 = 0.0f; r.pad_[0] = r.pad_[1] = 0.0f;
+    if (key != (~0ull >> 1) && (i == 0 || keys[i - 1] != key)) {            // head of a run: fold the run into it
+        r = pairs[vals[i]];
+        for (long long j = i + 1; j < n_slots && keys[j] == key; ++j) {
+            const PairRec o = pairs[vals[j]];
+            const float d1 = o.ref1 - r.ref1, d2 = o.ref2 - r.ref2;
+            const float dl[3] = { -(d1 + d2), d1, d2 };
+            // moments of o about r's reference
+            float A[3], M[6];
+            for (int k = 0; k < 3; ++k) A[k] = fmaf(o.w, dl[k], o.A[k]);
+            int q = 0;
+            for (int k = 0; k < 3; ++k)
+                for (int l = k; l < 3; ++l, ++q)
+                    M[q] = o.M[q] + o.A[k] * dl[l] + dl[k] * o.A[l] + o.w * dl[k] * dl[l];
+            r.w += o.w;
+            for (int k = 0; k < 3; ++k) r.A[k] += A[k];
+            for (int k = 0; k < 6; ++k) r.M[k] += M[k];
+        }
+    }
+    merged[i] = r;
 }
 
 // ---------------------------------------------------------------------------
@@ -522,10 +581,10 @@ int bits_for_count(unsigned long long m)     // bits needed for values 0..m
 }
 
 // slots per chunk: walks of one chunk, or faces of one chunk of the killing pass
-int64_t chunk_slots(int64_t n_records, int64_t F)
+int64_t chunk_slots(int64_t n_records, int64_t F, int64_t max_walks = MAX_CHUNK_WALKS)
 {
-    int64_t c = n_records < MAX_CHUNK_WALKS ? n_records : MAX_CHUNK_WALKS;
-    const int64_t f = F < MAX_CHUNK_WALKS ? F : MAX_CHUNK_WALKS;
+    int64_t c = n_records < max_walks ? n_records : max_walks;
+    const int64_t f = F < max_walks ? F : max_walks;
     if (f > c) c = f;
     return c < 1 ? 1 : c;
 }
@@ -552,8 +611,24 @@ int kill_prereduce(const float4* records, long long n_main, long long n_kill, lo
     return MCS_OK;
 }
 
+// Level 1b on the host side: sort the chunk's pair records by (sample, exit face) and fold the runs (see pair_merge_kernel).
+// key_buf / val_buf: scratch for n_slots 64-bit keys and 32-bit indices (the entry buffers, not in use yet).
+int merge_pairs(const PairRec* pairs, const uint32_t* pair_counts, long long n_slots, long long first_sample, long long n_samples,
+                long long F, unsigned long long* key_buf, uint32_t* val_buf, void* sort_ws, size_t sort_bytes,
+                PairRec* merged, uint32_t* merged_counts, cudaStream_t st)
+{
+    const int face_bits = bits_for_count((unsigned long long)F);
+    const int bits = face_bits + bits_for_count((unsigned long long)n_samples) + 1;    // + 1: the invalid key
+    const unsigned nblk = (unsigned)ceil_div64(n_slots, AT);
+    mcs_note_launch(), pair_keys_kernel<<<nblk, AT, 0, st>>>(pairs, pair_counts, n_slots, first_sample, face_bits, key_buf, val_buf);
+    int rc = sort_pairs_u64((uint64_t*)key_buf, val_buf, n_slots, bits > 63 ? 63 : bits, sort_ws, sort_bytes, st);
+    if (rc != MCS_OK) return rc;
+    mcs_note_launch(), pair_merge_kernel<<<nblk, AT, 0, st>>>(pairs, key_buf, val_buf, n_slots, merged, merged_counts);
+    return MCS_OK;
+}
+
 struct AccLayout {
-    size_t pairs, pair_counts, counts, keys, vals, carry_key, carry_sum, mface, scan, sort, total;
+    size_t pairs, pairs2, pair_counts, pair_counts2, counts, keys, vals, carry_key, carry_sum, mface, scan, sort, total;
     int64_t C, E, n_blocks, n_tiles;
 };
 
@@ -567,7 +642,9 @@ AccLayout acc_layout(int64_t n_records, int64_t F)
     L.n_tiles = ceil_div64(L.E, RT);
     size_t off = 0;
     L.pairs = off;       off += align_up((size_t)slots * sizeof(PairRec));
+    L.pairs2 = off;      off += align_up((size_t)slots * sizeof(PairRec));
     L.pair_counts = off; off += align_up((size_t)L.n_blocks * 4);
+    L.pair_counts2 = off; off += align_up((size_t)L.n_blocks * 4);
     L.counts = off;      off += align_up((size_t)(slots + 1) * 4);
     L.keys = off;        off += align_up((size_t)L.E * 4);
     L.vals = off;        off += align_up((size_t)L.E * 4);
@@ -602,7 +679,9 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 
     char* base = (char*)ws;
     PairRec* pairs = (PairRec*)(base + L.pairs);
+    PairRec* pairs2 = (PairRec*)(base + L.pairs2);
     uint32_t* pair_counts = (uint32_t*)(base + L.pair_counts);
+    uint32_t* pair_counts2 = (uint32_t*)(base + L.pair_counts2);
     uint32_t* counts = (uint32_t*)(base + L.counts);
     uint32_t* keys = (uint32_t*)(base + L.keys);
     uint32_t* vals = (uint32_t*)(base + L.vals);
@@ -630,10 +709,18 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
     for (int64_t j0 = 0, total = phase == 0 ? n_main : (n_kill > 0 ? b->F : 0); j0 < total; j0 += L.C) {
         const long long n = (total - j0) < L.C ? (total - j0) : L.C;
         const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
-        if (phase == 0) mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
-        else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
+        const PairRec* pp = pairs; const uint32_t* pc = pair_counts;
+        if (phase == 0) {
+            mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+            if (a.W > CH / 2) {                        // a sample spans several level-1 blocks: fold its repeated pairs (level 1b)
+                int rcm = merge_pairs(pairs, pair_counts, slots, j0 / a.W, n / a.W + 2, b->F, (unsigned long long*)keys, vals,
+                                      sort_ws, sort_bytes, pairs2, pair_counts2, st);
+                if (rcm != MCS_OK) return rcm;
+                pp = pairs2; pc = pair_counts2;
+            }
+        } else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
         const unsigned nblk = (unsigned)ceil_div64(slots, AT);
-        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
+        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pp, pc, slots, counts);
         int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
         uint32_t n_entries = 0;
@@ -641,7 +728,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         MCS_CUDA_TRY(cudaStreamSynchronize(st));
         if (n_entries == 0) continue;
         entries_total += n_entries;
-        mcs_note_launch(), expand_entries_kernel<uint32_t><<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts, keys, vals);
+        mcs_note_launch(), expand_entries_kernel<uint32_t><<<nblk, AT, 0, st>>>(a, pp, pc, slots, counts, keys, vals);
         rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
         const long long n_tiles = ceil_div64(n_entries, RT);
@@ -666,14 +753,14 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 namespace {
 
 struct CooLayout {
-    size_t pairs, pair_counts, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, mface, scan, sort, total;
+    size_t pairs, pairs2, pair_counts, pair_counts2, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, mface, scan, sort, total;
     int64_t C, E, cap, n_blocks, n_tiles;
 };
 
 CooLayout coo_layout(int64_t n_records, int64_t coo_capacity, int64_t F)
 {
     CooLayout L;
-    L.C = chunk_slots(n_records, F);
+    L.C = chunk_slots(n_records, F, MAX_CHUNK_WALKS_COO);
     L.n_blocks = ceil_div64(L.C, CH);
     const int64_t slots = L.n_blocks * CH;
     L.E = slots * MAX_ENTRIES_PER_PAIR;
@@ -681,7 +768,9 @@ CooLayout coo_layout(int64_t n_records, int64_t coo_capacity, int64_t F)
     L.n_tiles = ceil_div64(L.cap, RT);
     size_t off = 0;
     L.pairs = off;       off += align_up((size_t)slots * sizeof(PairRec));
+    L.pairs2 = off;      off += align_up((size_t)slots * sizeof(PairRec));
     L.pair_counts = off; off += align_up((size_t)L.n_blocks * 4);
+    L.pair_counts2 = off; off += align_up((size_t)L.n_blocks * 4);
     L.counts = off;      off += align_up((size_t)(slots + 1) * 4);
     for (int q = 0; q < 2; ++q) {
         L.keys[q] = off; off += align_up((size_t)L.cap * 8);
@@ -728,7 +817,9 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
 
     char* base = (char*)ws;
     PairRec* pairs = (PairRec*)(base + L.pairs);
+    PairRec* pairs2 = (PairRec*)(base + L.pairs2);
     uint32_t* pair_counts = (uint32_t*)(base + L.pair_counts);
+    uint32_t* pair_counts2 = (uint32_t*)(base + L.pair_counts2);
     uint32_t* counts = (uint32_t*)(base + L.counts);
     unsigned long long* keys[2] = { (unsigned long long*)(base + L.keys[0]), (unsigned long long*)(base + L.keys[1]) };
     uint32_t* vals[2] = { (uint32_t*)(base + L.vals[0]), (uint32_t*)(base + L.vals[1]) };
@@ -758,10 +849,18 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
     for (int64_t j0 = 0, total = phase == 0 ? n_main : (n_kill > 0 ? b->F : 0); j0 < total; j0 += L.C) {
         const long long n = (total - j0) < L.C ? (total - j0) : L.C;
         const long long nblk1 = ceil_div64(n, CH), slots = nblk1 * CH;
-        if (phase == 0) mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
-        else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
+        const PairRec* pp = pairs; const uint32_t* pc = pair_counts;
+        if (phase == 0) {
+            mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
+            if (a.W > CH / 2) {                        // level 1b: fold the pairs a sample repeats over its level-1 blocks
+                int rcm = merge_pairs(pairs, pair_counts, slots, j0 / a.W, n / a.W + 2, b->F, keys[cur] + n_u, vals[cur] + n_u,
+                                      sort_ws, sort_bytes, pairs2, pair_counts2, st);
+                if (rcm != MCS_OK) return rcm;
+                pp = pairs2; pc = pair_counts2;
+            }
+        } else mcs_note_launch(), kill_pairs_kernel<<<(unsigned)ceil_div64(slots, AT), AT, 0, st>>>(mface, j0, n, slots, pairs, pair_counts);
         const unsigned nblk = (unsigned)ceil_div64(slots, AT);
-        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pairs, pair_counts, slots, counts);
+        mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pp, pc, slots, counts);
         int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
         uint32_t n_entries = 0;
@@ -770,7 +869,7 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
         if (n_entries == 0) continue;
         entries_total += n_entries;
         mcs_note_launch(), expand_entries_kernel<unsigned long long><<<nblk, AT, 0, st>>>(
-            a, pairs, pair_counts, slots, counts, keys[cur] + n_u, vals[cur] + n_u);
+            a, pp, pc, slots, counts, keys[cur] + n_u, vals[cur] + n_u);
         const long long n_tot = n_u + n_entries;
         rc = sort_pairs_u64((uint64_t*)keys[cur], vals[cur], n_tot, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;

@@ -469,7 +469,8 @@ extern "C" void mcs_free_bvh(mcs_bvh* b)
     // (like this library's own) are non-blocking, so without the event a kernel still queued on such a stream could
     // read the tree after the pool had handed its memory to someone else.
     if (b->last_use) cudaStreamWaitEvent((cudaStream_t)0, b->last_use, 0);
-    void* ptrs[8] = { b->verts, b->faces, b->nodes, b->wide, b->tris, b->leaf_tri, b->face_slot, b->morton };
+    void* ptrs[11] = { b->verts, b->faces, b->nodes, b->wide, b->tris, b->leaf_tri, b->face_slot, b->morton,
+                       b->wn_nodes, b->wn_order, b->wn_face_pos };
     for (void* p : ptrs) if (p) cudaFreeAsync(p, (cudaStream_t)0);
     if (b->last_use) cudaEventDestroy(b->last_use);
     if (cur != b->device) cudaSetDevice(cur);

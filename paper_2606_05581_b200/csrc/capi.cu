@@ -389,7 +389,7 @@ done:
 // download of the entries that were written.
 extern "C" int mcs_estimate_dtn_host_coo(const float* verts, int64_t V, const int32_t* faces, int64_t F,
                                          const mcs_samples* hs, const mcs_params* p_int, const mcs_params* p_ext,
-                                         float orient_h_scale, mcs_host_coo* out_interior, mcs_host_coo* out_exterior,
+                                         float orient_h_scale, float orient_beta, mcs_host_coo* out_interior, mcs_host_coo* out_exterior,
                                          mcs_stats* stats_interior, mcs_stats* stats_exterior, void* stream)
 {
     if (stats_interior) memset(stats_interior, 0, sizeof *stats_interior);
@@ -437,7 +437,10 @@ extern "C" int mcs_estimate_dtn_host_coo(const float* verts, int64_t V, const in
         mcs_samples ds;
         ds.tri = (const int32_t*)(d_in + off_t); ds.bary = (const float*)(d_in + off_b);
         ds.weight = (const float*)(d_in + off_w); ds.normal = nullptr; ds.n_s = n_s;
-        if (orient) {                                 // sidedness by the winding number (DESIGN.md G-R1)
+        if (orient && orient_beta > 0.0f) {           // sidedness from the hierarchical evaluation
+            rc = mcs_orient_samples_fast(bvh, &ds, orient_h_scale, orient_beta, (float*)(d_in + off_n), nullptr, stream);
+            if (rc != MCS_OK) goto done;
+        } else if (orient) {                          // sidedness by the winding number (DESIGN.md G-R1)
             const size_t wb = mcs_winding_workspace_bytes(bvh, n_s);
             e = cudaMallocAsync(&d_wws, wb, st);
             if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ENOMEM; goto done; }

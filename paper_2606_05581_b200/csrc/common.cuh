@@ -3,6 +3,7 @@
 #pragma once
 
 #include <cuda_runtime.h>
+#include <mutex>
 #include <math_constants.h>
 #include <stdint.h>
 #include <stddef.h>
@@ -85,6 +86,13 @@ struct mcs_bvh {
     size_t     device_bytes;
     int        device;
     mutable cudaEvent_t last_use;   // recorded on the stream of every call that reads the tree (mcs_free_bvh waits for it)
+    // face hierarchy of mcs_orient_samples_fast (winding.cu), built on first use
+    mutable std::mutex wn_mutex;
+    mutable void*      wn_nodes;    // float4 [2 G][2]: (centroid, radius), (area vector, area); heap order, root = 1
+    mutable uint32_t*  wn_order;    // [F] faces along the Z-order curve
+    mutable int32_t*   wn_face_pos; // [F] position of a face in wn_order
+    mutable long long  wn_G;        // leaf groups, padded to a power of two
+    mutable int        wn_levels;   // level of the leaf groups (root = 0)
 };
 
 // Every entry point that enqueues work reading the tree calls this with its stream when it is done enqueuing.

@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 
-from bench import make_workload                                               # noqa: E402
+from bench import make_cfg1                                                      # noqa: E402
 from oracle import Oracle, OracleParams, mesh_geom, steklov_eigs              # noqa: E402
 
 
@@ -26,7 +26,7 @@ def api():
 
 @pytest.fixture(scope="module")
 def cfg1(api):
-    wl = make_workload(4, 4096, 16, 0)
+    wl = make_cfg1(4, 4096, 16, 0)
     vd = torch.as_tensor(wl["v"]).cuda()
     fd = torch.as_tensor(wl["f"]).cuda()
     bvh = api.build_bvh(vd, fd)

@@ -33,7 +33,7 @@ def big(api):
 def test_build_2m_faces(api, big):
     v, f, info, bvh, orc = big
     bi = bvh.info()
-    assert bi.F == 2_000_000 and bi.n_nodes == bi.F - 1
+    assert bi.F == 2_000_000 and bi.n_nodes == bi.n_leaves - 1 and bi.F < bi.n_leaves <= 2 * bi.F
     assert 21 <= bi.max_depth <= 96                                   # log2(2M) = 20.9; traversal stack bound
     area = orc.total_area()
     assert abs(bi.area - area) <= 1e-9 * area
@@ -41,7 +41,12 @@ def test_build_2m_faces(api, big):
     m = morton.cpu().numpy().astype(np.uint64)
     assert (m[1:] >= m[:-1]).all()
     lt = leaf_tri.cpu().numpy()
-    assert np.array_equal(np.bincount(lt, minlength=bi.F), np.ones(bi.F, np.int64))
+    per_face = np.bincount(lt, minlength=bi.F)
+    assert per_face.min() >= 1 and per_face.sum() == bi.n_leaves     # every face has a leaf; long slivers have several
+    assert info["sliver"][per_face > 1].all()                         # only slivers were cut (aspect > 100 among them all)
+    # tree quality readout: the rotated strips dominate the surface-area cost of the unsplit tree
+    plain = api.build_bvh(torch.as_tensor(v).cuda(), torch.as_tensor(f).cuda(), split=False).info()
+    assert plain.n_leaves == bi.F and bi.sah_cost < 0.2 * plain.sah_cost, (bi.sah_cost, plain.sah_cost)
 
 
 def test_closest_point_2m_faces(api, big):
@@ -89,20 +94,27 @@ def test_walks_2m_faces_sampled_against_oracle(api, big, exterior):
     steps, rec = steps.cpu().numpy(), rec.cpu().numpy()
     assert st.n_truncated == int(((steps == -1) | (steps == -3)).sum()) and st.n_discarded * 64 == int((steps == -2).sum())
     assert (steps >= 0).mean() > 0.5                                  # flipped faces / overlaps cost some walks, not most
-    ids = np.sort(np.random.default_rng(2).choice(len(smp["weight"]), 20, replace=False))
-    n_w, n_kill = 4, 16
+    ids = np.sort(np.random.default_rng(2).choice(len(smp["weight"]), 48, replace=False))
+    n_w, n_kill = 4, 32
     orec = orc.run_walks_subset(OracleParams(origin=origin, **kw), exterior, smp["tri"], smp["bary"], smp["weight"],
                                 ids, n_w, n_kill_first=n_kill)
     slots = (ids[:, None] * 64 + np.arange(n_w)[None, :]).ravel()
     if exterior:
         slots = np.concatenate([slots, len(smp["weight"]) * 64 + np.arange(n_kill)])
+    # Flipped faces are NOT repaired here (no sidedness pre-pass), so some sampled walks start on the wrong side and are
+    # cut by R10b / R10c or by max_steps on both sides; the outcome class must agree walk for walk.
+    assert ((steps[slots] >= 0) == (orec["steps"] >= 0)).mean() >= 0.98
     same = steps[slots] == orec["steps"]
-    assert same.mean() >= 0.9, (same.mean(), steps[slots], orec["steps"])
+    assert same.mean() >= 0.95, (same.mean(), steps[slots], orec["steps"])
     ok = same & (steps[slots] >= 0)
     tri_t = rec[slots, 0].copy().view(np.int32)
     key = np.sort(f.astype(np.int64), axis=1)
     same_face = np.array([np.array_equal(key[a], key[b]) for a, b in zip(tri_t[ok], orec["tri_t"][ok])])
-    assert same_face.mean() > 0.9
+    assert same_face.mean() >= 0.95
+    bt = np.stack([1 - rec[slots, 1] - rec[slots, 2], rec[slots, 1], rec[slots, 2]], 1).astype(np.float64)
+    t_gpu = np.einsum("qk,qkd->qd", bt[ok], v[f[tri_t[ok]]].astype(np.float64))
+    err = np.linalg.norm(t_gpu - orec["t"][ok], axis=1)
+    assert np.quantile(err, 0.95) < 5e-4 and np.median(err) < 2e-5, np.quantile(err, [0.5, 0.95, 1.0])
 
 
 @pytest.mark.parametrize("exterior", [False, True])
@@ -127,3 +139,70 @@ def test_walks_2m_faces_config3_size_bit_identical_reruns(api, big, exterior):
         rec, steps = api.run_walks(bvh, S, P, exterior)
         assert torch.equal(rec.view(torch.int32), r0) and torch.equal(steps, steps0)
         del rec, steps
+
+
+def test_config3_sparse_matrix_entries_against_the_oracle_on_a_sample_subset(api):
+    """BASELINE config 3 as bench.py builds it (2 M-face stress mesh, 20 000 FPS samples, Kelvin origin, sidedness
+    pre-pass): every 1250th sample point (16 of 20 000, a 1/1250 subset) with 8 walks each, both operators, sparse
+    output.  (1) The library's accumulation of the ORACLE's records equals the oracle's own accumulation (on the
+    sub-mesh of touched faces: pure re-indexing) to fp32 rounding.  (2) The library's own walks + accumulation give
+    entries within 4 Monte Carlo standard errors of the oracle's (same Philox counters, so in practice far closer)."""
+    import argparse
+    from bench import make_cfg3
+    from oracle import RECORD_DTYPE
+    args = argparse.Namespace(faces=2_000_000, components=30, samples=20_000, candidates=1_000_000, mesh_seed=3, no_cache=False)
+    wl = make_cfg3(args)
+    v, f = wl["v"], wl["f"]
+    bvh = api.build_bvh(torch.as_tensor(v).cuda(), torch.as_tensor(f).cuda())
+    ids = np.arange(0, len(wl["tri"]), 1250)
+    tri, bary, wgt = wl["tri"][ids], wl["bary"][ids], wl["weight"][ids]
+    S0 = api.Samples.from_arrays(tri, bary, wgt)
+    nrm, _ = api.orient_samples(bvh, S0)
+    S = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
+    nrm_h = nrm.cpu().numpy()
+    orc = Oracle(mesh_geom(v, f))
+    W = 8
+    for exterior in (False, True):
+        kw = dict(seed=0, walks_per_sample=W, eps=1e-3)
+        P = api.Params(kelvin_origin=wl["origin"], **kw)
+        orec, _ = orc.run_walks(OracleParams(origin=wl["origin"], **kw), exterior, tri, bary, wgt, normal=nrm_h)
+        ok = orec["tri_t"] >= 0
+        assert ok.mean() > 0.9
+        # ---- sub-mesh of touched faces, oracle accumulation with variances
+        faces_used = np.unique(np.concatenate([tri, orec["tri_t"][ok]]))
+        verts_used, inv = np.unique(f[faces_used], return_inverse=True)
+        f_sub = inv.reshape(-1, 3).astype(np.int32)
+        face_new = -np.ones(len(f), np.int64); face_new[faces_used] = np.arange(len(faces_used))
+        vert_new = -np.ones(len(v), np.int64); vert_new[verts_used] = np.arange(len(verts_used))
+        sub = orec.copy()
+        sub["tri_t"] = np.where(ok, face_new[np.maximum(orec["tri_t"], 0)], -1)
+        osub = Oracle(mesh_geom(v[verts_used], f_sub))
+        So, var = osub.accumulate_hat(sub, face_new[tri].astype(np.int32), bary, want_var=True)
+        # ---- (1) the oracle's records through the library's sparse accumulation
+        r = np.zeros((len(orec), 4), np.float32)
+        r[:, 0] = np.where(ok, orec["tri_t"], -1).astype(np.int32).view(np.float32)
+        r[:, 1], r[:, 2], r[:, 3] = orec["bary_t"][:, 1], orec["bary_t"][:, 2], np.where(ok, orec["weight"], 0.0)
+        coo = api.accumulate_coo(bvh, S, P, torch.as_tensor(r).cuda())
+        rr, cc = vert_new[coo.row.cpu().numpy()], vert_new[coo.col.cpu().numpy()]
+        assert (rr >= 0).all() and (cc >= 0).all()
+        Sg = np.zeros_like(So)
+        Sg[rr, cc] = coo.val.cpu().numpy(); Sg[cc, rr] = coo.val.cpu().numpy()
+        assert np.abs(Sg - So).max() <= 3e-5 * np.abs(So).max()
+        # ---- (2) the library's own walks
+        coo2, st = api.estimate_dtn_coo(bvh, S, P, exterior, want_stats=True)
+        rec, steps = api.run_walks(bvh, S, P, exterior)
+        same = steps.cpu().numpy() == orec["steps"]
+        assert same.mean() >= 0.95, same.mean()
+        r2, c2 = coo2.row.cpu().numpy(), coo2.col.cpu().numpy()
+        inside = (vert_new[r2] >= 0) & (vert_new[c2] >= 0)
+        S2 = np.zeros_like(So)
+        S2[vert_new[r2[inside]], vert_new[c2[inside]]] = coo2.val.cpu().numpy()[inside]
+        S2 = np.triu(S2) + np.triu(S2, 1).T
+        se = np.sqrt(np.maximum(var, 0.0))
+        scale = np.abs(So).max()
+        bad = np.abs(S2 - So) > 4.0 * np.sqrt(2.0) * se + 2e-6 * scale
+        assert bad.sum() <= max(1, int(1e-3 * (So != 0).sum())), (bad.sum(), (So != 0).sum())
+        # entries of walks that ended elsewhere than the oracle's (a few per cent) fall outside the sub-mesh: small in norm
+        out_norm = np.sqrt((coo2.val.cpu().numpy()[~inside].astype(np.float64) ** 2).sum())
+        assert out_norm <= 0.2 * np.linalg.norm(So), (out_norm, np.linalg.norm(So))
+        assert np.linalg.norm(S2 - So) <= np.linalg.norm(se) + 0.05 * np.linalg.norm(So)

@@ -94,3 +94,40 @@ def test_sidedness_on_sphere_with_flipped_faces_and_timing(api):
     assert (np.einsum("qd,qd->q", nrm.cpu().numpy().astype(np.float64), s) > 0).all()
     assert ((d.cpu().numpy() > 0) == ~flip[tri]).all()
     print(f"orient_samples: {2 * n} probes x {len(f)} faces in {dt * 1e3:.1f} ms = {2 * n * len(f) / dt / 1e9:.1f} G pairs/s")
+
+
+def test_orient_samples_fast_against_oracle_and_exhaustive(api):
+    """The hierarchical evaluation (dipole terms for far groups of faces, same cut for both probes) against the fp64
+    oracle and the exhaustive GPU sum: d within 5e-3, the decision equal wherever the oracle's margin exceeds 2e-2,
+    bit-identical reruns; tighter with a larger opening parameter."""
+    v, f, info = stress_mesh(n_faces=60_000, n_components=9, seed=11)
+    smp = fps_samples(v, f, 800, n_candidates=10_000, seed=2)
+    bvh = _bvh(api, v, f)
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    no, do = Oracle(mesh_geom(v, f)).orient_samples(smp["tri"], smp["bary"], h_scale=1.0)
+    nx, dx = api.orient_samples(bvh, S, h_scale=1.0)
+    errs = {}
+    for beta in (2.0, 2.5, 4.0):
+        nrm, d = api.orient_samples_fast(bvh, S, h_scale=1.0, beta=beta)
+        nrm2, d2 = api.orient_samples_fast(bvh, S, h_scale=1.0, beta=beta)
+        assert torch.equal(nrm, nrm2) and torch.equal(d, d2)
+        d, nrm = d.cpu().numpy(), nrm.cpu().numpy()
+        errs[beta] = np.abs(d - do).max()
+        sure = np.abs(do) > 2e-2
+        assert sure.mean() > 0.9
+        assert np.abs(nrm[sure] - no[sure]).max() < 1e-5                  # same decision, same normal
+        assert ((d < 0) == (dx.cpu().numpy() < 0))[sure].all()
+    assert errs[2.5] < 5e-3 and errs[4.0] < 2e-3 and errs[4.0] <= errs[2.0], errs
+    flipped = info["flipped"][smp["tri"]]
+    sure = np.abs(do) > 2e-2
+    nrm, d = api.orient_samples_fast(bvh, S)
+    assert ((d.cpu().numpy() < 0) == flipped)[sure].mean() > 0.9
+    with pytest.raises(api.McsError):
+        api.orient_samples_fast(bvh, S, beta=1.0)
+    # tiny meshes (fewer faces than one group, a single face)
+    v1, f1 = icosphere(0)
+    b1 = _bvh(api, v1, f1)
+    S1 = api.Samples.from_arrays(np.arange(20, dtype=np.int32), np.full((20, 3), 1 / 3, np.float32), np.ones(20, np.float32))
+    n1, d1 = api.orient_samples_fast(b1, S1)
+    n1x, d1x = api.orient_samples(b1, S1)
+    assert np.abs(d1.cpu().numpy() - d1x.cpu().numpy()).max() < 1e-5 and torch.equal(n1, n1x)
