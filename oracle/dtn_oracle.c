@@ -454,9 +454,9 @@ void orc_tangent_ball_interior(const orc_geom *g, const orc_params *P, const orc
  * Exterior: the tangent ball lives in the inverted domain Omega*_ext
  * (PAPER.md:348-353).  s* = kappa(s - o); the unit normal at s* pointing out of
  * Omega*_ext is n* = -H_shat n (Eq. 54).  The ball B_r(c*),
- * c* = s* - r n*, is tested through its primal image, which is again a ball as
- * long as 0 is outside it: centre c* / (|c*|^2 - r^2), radius r / (|c*|^2 - r^2)
- * [DESIGN.md reading E2].  r is limited so that 0 stays outside
+ * c* = s* - r n*, is tested through the primal image of its eps/2-shrunken copy, which is again a ball as
+ * long as 0 is outside it: a Kelvin ball (c*, rho) maps to centre c* / (|c*|^2 - rho^2), radius rho / (|c*|^2 - rho^2)
+ * [DESIGN.md readings E2, R4].  r is limited so that 0 stays outside
  * (r < |s*|^2 / (2 s*.n*)) and by r_max of the inverted box.
  */
 void orc_tangent_ball_exterior(const orc_geom *g, const orc_params *P, const orc_sample *S, orc_ball *B)
@@ -478,12 +478,18 @@ void orc_tangent_ball_exterior(const orc_geom *g, const orc_params *P, const orc
     for (int it = 0; it < P->bisection_iters; ++it) {
         double r = 0.5 * (lo + hi);
         double cs[3] = { sstar[0] - r * nstar[0], sstar[1] - r * nstar[1], sstar[2] - r * nstar[2] };
-        double den = dot3(cs, cs) - r * r;
+        /* [R4] the probe ball is B(c*, r - eps/2) IN KELVIN COORDINATES (the walk domain: a point of the tangent ball
+         * that pokes out by < eps/2 is inside the shell); it is tested through ITS OWN primal image.  (Shrinking the
+         * primal image of B(c*, r) by the relative amount eps / 2r instead moves its near side by eps / (2 (|c*|^2 - r^2))
+         * in primal units, many eps when that image is large.) */
+        double rk = r - 0.5 * P->eps;
+        if (!(rk > 0.0)) { lo = r; continue; }
+        double den = dot3(cs, cs) - rk * rk;
         double cprime[3] = { P->origin[0] + cs[0] / den, P->origin[1] + cs[1] / den, P->origin[2] + cs[2] / den };
-        double rprime = r / den;
+        double rprime = rk / den;
         orc_hit h;
         orc_closest_point(g, cprime, &h);
-        if (h.dist >= rprime * (1.0 - 0.5 * P->eps / r)) lo = r; else hi = r;
+        if (h.dist >= rprime) lo = r; else hi = r;
     }
     B->r = lo;
     for (int k = 0; k < 3; ++k) { B->c[k] = sstar[k] - lo * nstar[k]; B->pole[k] = nstar[k]; }

@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libmcdtn.so")
+LIB_PATH = os.environ.get("MCDTN_LIB") or os.path.join(HERE, "libmcdtn.so")     # MCDTN_LIB: another build of the same library
 
 MCS_OK, MCS_EINVAL, MCS_EDEGENERATE, MCS_ENOMEM, MCS_ECUDA = 0, -1, -2, -3, -4
 

@@ -431,10 +431,14 @@ wide_pack_kernel(const int32_t* __restrict__ node_words, int64_t n_nodes, const 
             }
         }
     }
-    w.pad[0] = n; w.pad[1] = (int)i; w.pad[2] = 0; w.pad[3] = 0;
     for (; n < 4; ++n) {
         for (int q = 0; q < 3; ++q) { w.f[6 * n + q] = CUDART_INF_F; w.f[6 * n + 3 + q] = -CUDART_INF_F; }
         w.c[n] = INT_MIN;
+    }
+    for (int k = 0; k < 4; ++k) {                                  // squared diagonal of every child box (far-field test of the walk kernel)
+        const float ex = w.f[6 * k + 3] - w.f[6 * k], ey = w.f[6 * k + 4] - w.f[6 * k + 1], ez = w.f[6 * k + 5] - w.f[6 * k + 2];
+        const float g = w.c[k] == INT_MIN ? CUDART_INF_F : (ex * ex + ey * ey + ez * ez) * (1.0f + 4e-7f);   // rounded up
+        w.pad[k] = __float_as_int(g);
     }
     wide[widx[i]] = w;
 }

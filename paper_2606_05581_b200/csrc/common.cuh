@@ -58,7 +58,7 @@ struct __align__(16) PackedTri {
 // the tree ends earlier).
 //   f[6k .. 6k+5] = box of child k (lo.xyz, hi.xyz), k = 0..3;  an empty slot has lo = +inf
 //   c[k]          = child k: >= 0 wide node index, < 0 leaf ~c = sorted triangle slot
-//   pad[4]        = (number of children, binary node index, 0, 0)
+//   pad[4]        = squared diagonal of the box of child k as float bits (+inf for an empty slot)
 struct __align__(32) WideNode {
     float f[24];
     int   c[4];

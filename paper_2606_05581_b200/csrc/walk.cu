@@ -148,9 +148,11 @@ __device__ __forceinline__ void probe_ball(const BallFamily& f, int j, float3& c
     c = f3(fmaf(-r, f.pole.x, f.base.x), fmaf(-r, f.pole.y, f.base.y), fmaf(-r, f.pole.z, f.base.z));
     float thr;
     if (EXT) {
-        const float den = f.ss2 - 2.0f * r * f.sdn;               // |c*|^2 - r^2
+        // the Kelvin ball B(c*, r - eps/2) through its own primal image (R4 / E2): centre c* / den, radius rk / den
+        const float rk = r - 0.5f * f.eps;
+        const float den = (f.ss2 - 2.0f * r * f.sdn) + (r - rk) * (r + rk);   // |c*|^2 - rk^2,  |c*|^2 = ss2 - 2 r sdn + r^2
         c = f3(f.o.x + c.x / den, f.o.y + c.y / den, f.o.z + c.z / den);
-        thr = (r / den) * (1.0f - 0.5f * f.eps / r);
+        thr = rk / den;
     } else {
         thr = r - 0.5f * f.eps;
     }
@@ -335,6 +337,13 @@ __device__ __forceinline__ void frame_from_normal(float3 n, float3& e1, float3& 
 // own bank); entries beyond WSTACK spill to local memory (deep LBVH chains only).
 // ---------------------------------------------------------------------------
 constexpr int WALK_MIN_BLOCKS = 8;                  // 64 registers per thread; 10 (48 registers, spills) measured 9 % slower
+// Blocks per SM of the variants with the warp-cooperative path (large or messy meshes): they need ~96 registers; at
+// 8 blocks (64 registers) ncu counted 19 G spill instructions and more local-memory sectors than global ones on BASELINE
+// config 3 (profiles/r02_cfg3_walk_kernel.md).  Measured on that workload (both operators, W = 1024): 8 blocks 358 ms,
+// 6: 308, 5: 284, 4: 314.
+#ifndef WALK_COOP_BLOCKS
+#define WALK_COOP_BLOCKS 5
+#endif
 constexpr int WSTACK = 16;                       // shared-memory stack entries per lane
 constexpr int CUR_NONE = INT_MIN;
 #ifndef VOTE_NODE
@@ -409,13 +418,6 @@ struct CoopState {
     int sp, cur;
     unsigned n_nodes, n_tris, q_nodes;       // increments (COUNT builds)
 };
-
-// Squared diagonal of child box k of a wide node held in q0, q1, q2 (24 floats: lo.xyz, hi.xyz per child).
-#define MCS_SQ(x) ((x) * (x))
-#define MCS_DIAG0(q0, q1, q2) (MCS_SQ(q0.lo.w - q0.lo.x) + MCS_SQ(q0.hi.x - q0.lo.y) + MCS_SQ(q0.hi.y - q0.lo.z))
-#define MCS_DIAG1(q0, q1, q2) (MCS_SQ(q1.lo.y - q0.hi.z) + MCS_SQ(q1.lo.z - q0.hi.w) + MCS_SQ(q1.lo.w - q1.lo.x))
-#define MCS_DIAG2(q0, q1, q2) (MCS_SQ(q1.hi.w - q1.hi.x) + MCS_SQ(q2.lo.x - q1.hi.y) + MCS_SQ(q2.lo.y - q1.hi.z))
-#define MCS_DIAG3(q0, q1, q2) (MCS_SQ(q2.hi.y - q2.lo.z) + MCS_SQ(q2.hi.z - q2.lo.w) + MCS_SQ(q2.hi.w - q2.hi.x))
 
 template <bool COUNT, bool FAR>
 __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, const WideNode* __restrict__ wide,
@@ -502,16 +504,16 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
                 in3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w) <= wlim;
                 c0 = __float_as_int(q3.lo.x); c1 = __float_as_int(q3.lo.y); c2 = __float_as_int(q3.lo.z); c3 = __float_as_int(q3.lo.w);
                 if (FAR) {
-                    // a sub-tree whose box is small against its distance stands for its faces: its box distance is a lower
-                    // bound of theirs (see walk_kernel); it is not descended
+                    // a child whose box is small against its distance stands for its faces: its box distance is a lower
+                    // bound of theirs (see walk_kernel); it is not descended / not tested.  INT_MIN marks an empty slot.
                     const float e0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
                     const float e1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
                     const float e2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
                     const float e3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
-                    if (in0 && c0 >= 0 && e0 >= wnear2 && MCS_DIAG0(q0, q1, q2) <= alpha2 * e0) { mylb = fminf(mylb, e0); in0 = false; }
-                    if (in1 && c1 >= 0 && e1 >= wnear2 && MCS_DIAG1(q0, q1, q2) <= alpha2 * e1) { mylb = fminf(mylb, e1); in1 = false; }
-                    if (in2 && c2 >= 0 && e2 >= wnear2 && MCS_DIAG2(q0, q1, q2) <= alpha2 * e2) { mylb = fminf(mylb, e2); in2 = false; }
-                    if (in3 && c3 >= 0 && e3 >= wnear2 && MCS_DIAG3(q0, q1, q2) <= alpha2 * e3) { mylb = fminf(mylb, e3); in3 = false; }
+                    if (in0 && e0 >= wnear2 && q3.hi.x <= alpha2 * e0) { mylb = fminf(mylb, e0); in0 = false; }
+                    if (in1 && e1 >= wnear2 && q3.hi.y <= alpha2 * e1) { mylb = fminf(mylb, e1); in1 = false; }
+                    if (in2 && e2 >= wnear2 && q3.hi.z <= alpha2 * e2) { mylb = fminf(mylb, e2); in2 = false; }
+                    if (in3 && e3 >= wnear2 && q3.hi.w <= alpha2 * e3) { mylb = fminf(mylb, e3); in3 = false; }
                 }
             }
             if (FAR) {
@@ -552,10 +554,10 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 // away is expensive for a reason no tree removes: every face whose box enters the ball of radius D about the query
 // point has to be tested, and on a finely tessellated surface that is hundreds of faces (BASELINE config 3: 70-150
 // triangle tests per query; the paper names the exterior's far queries as its bottleneck).  During
-// the traversal a sub-tree whose box is small against its distance -- diagonal <= alpha x box distance, and box
-// distance >= the near threshold -- is not descended: its box distance stands for its faces (they are at most
-// (1 + alpha) times farther).  The query then returns the minimum over a CUT of the tree (such boxes, and real faces
-// where no ancestor qualified).  Which nodes qualify depends on the query point only, pruning is against that running
+// the traversal a child (sub-tree or single face) whose box is small against its distance -- diagonal <= alpha x box
+// distance, and box distance >= the near threshold -- is not descended or tested: its box distance stands for its
+// faces (they are at most (1 + alpha) times farther).  The query then returns the minimum over a CUT of the tree (such
+// boxes, and real faces where neither they nor an ancestor qualified).  Which nodes qualify depends on the query point only, pruning is against that running
 // minimum with the usual margin, so the result does not depend on the traversal order or the schedule.  If the
 // minimum is a real face the query is exact as before (exit point, termination test); if it is a box the walker
 // jumps with that lower bound as its radius, at least 1 / (1 + alpha) of the largest possible one, and the shell test
@@ -563,7 +565,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 // Kelvin radius is that multiple) are always descended.  The estimator is the same in expectation; single walks differ
 // from the exact run, so record-level parity tests run with far_alpha = 0 and matrices are compared statistically.
 template <bool EXT, bool COUNT, bool COOP, bool MERGED, bool FAR>
-__global__ void __launch_bounds__(WT, MERGED ? 4 : WALK_MIN_BLOCKS)      // small jobs: registers instead of occupancy
+__global__ void __launch_bounds__(WT, MERGED ? 4 : (COOP ? WALK_COOP_BLOCKS : WALK_MIN_BLOCKS))      // small jobs: registers instead of occupancy
 walk_kernel(WalkGeom g, WalkArgs a)
 {
     __shared__ int   sh_ref[WSTACK * WT];
@@ -673,11 +675,12 @@ walk_kernel(WalkGeom g, WalkArgs a)
                 float d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
                 int c0 = __float_as_int(q3.lo.x), c1 = __float_as_int(q3.lo.y), c2 = __float_as_int(q3.lo.z), c3 = __float_as_int(q3.lo.w);
                 if (FAR) {
+                    // q3.hi = squared diagonals of the four child boxes (+inf for an empty slot, so it never qualifies)
                     bool any = false;
-                    if (c0 >= 0 && d0 >= dnear2 && d0 <= lim && MCS_DIAG0(q0, q1, q2) <= a.far_alpha2 * d0) { lb2 = fminf(lb2, d0); d0 = CUDART_INF_F; any = true; }
-                    if (c1 >= 0 && d1 >= dnear2 && d1 <= lim && MCS_DIAG1(q0, q1, q2) <= a.far_alpha2 * d1) { lb2 = fminf(lb2, d1); d1 = CUDART_INF_F; any = true; }
-                    if (c2 >= 0 && d2 >= dnear2 && d2 <= lim && MCS_DIAG2(q0, q1, q2) <= a.far_alpha2 * d2) { lb2 = fminf(lb2, d2); d2 = CUDART_INF_F; any = true; }
-                    if (c3 >= 0 && d3 >= dnear2 && d3 <= lim && MCS_DIAG3(q0, q1, q2) <= a.far_alpha2 * d3) { lb2 = fminf(lb2, d3); d3 = CUDART_INF_F; any = true; }
+                    if (d0 >= dnear2 && d0 <= lim && q3.hi.x <= a.far_alpha2 * d0) { lb2 = fminf(lb2, d0); d0 = CUDART_INF_F; any = true; }
+                    if (d1 >= dnear2 && d1 <= lim && q3.hi.y <= a.far_alpha2 * d1) { lb2 = fminf(lb2, d1); d1 = CUDART_INF_F; any = true; }
+                    if (d2 >= dnear2 && d2 <= lim && q3.hi.z <= a.far_alpha2 * d2) { lb2 = fminf(lb2, d2); d2 = CUDART_INF_F; any = true; }
+                    if (d3 >= dnear2 && d3 <= lim && q3.hi.w <= a.far_alpha2 * d3) { lb2 = fminf(lb2, d3); d3 = CUDART_INF_F; any = true; }
                     if (any) lim = fminf(lim, prune_limit(lb2, xq, a.mesh_scale));
                 }
                 // partial sorting network on (distance, child): (0,1)(2,3)(0,2) puts the nearest child first; the other

@@ -605,3 +605,42 @@ def test_aabb_diagonal_and_exterior_rmax_closed_forms():
     assert abs(orc.rmax(True, (a, 0.0, 0.0)) - 1.0 / (1.0 - a * a)) < 5e-3
     v2, f2 = icosphere(4, radius=2.0)
     assert abs(Oracle(mesh_geom(v2, f2)).rmax(True, (0.0, 0.5, 0.0)) - 2.0 / (4.0 - 0.25)) < 5e-3
+
+
+def test_exterior_tangent_ball_stays_out_of_a_neighbouring_solid():
+    """Readings E2 + R4: the accepted Kelvin ball may poke out of the inverted domain by at most eps/2 IN KELVIN
+    COORDINATES.  BASELINE config 2b in small (two unit spheres 2.5 apart, the torus between them, inversion centre =
+    centre of the first sphere A, whose image is the unit sphere |y| = 1 with A's inside OUTSIDE it): tangent balls of
+    torus samples grow until they meet the image of A, and some of them pass close to 0 = kappa(infinity), where their
+    primal image is a huge ball.  Every accepted ball must stay within |y| <= 1 + eps.  An earlier form of the test
+    shrank the primal image by the RELATIVE amount eps / 2r, i.e. by eps / (2 (|c*|^2 - r^2)) in primal units, and let
+    such balls reach 0.014 into A (found by the full-size GPU test of config 2b: walks started inside A, two of 83 M
+    were cut by R10c on both sides)."""
+    from synth import torus
+    parts = [icosphere(3, 1.0, (-1.25, 0, 0)), icosphere(3, 1.0, (1.25, 0, 0)), torus(1.0, 0.3, 60, 30, axis="x")]
+    v, f, vid, fid = merge_meshes(parts)
+    orc = Oracle(mesh_geom(v, f))
+    origin = (-1.25, 0.0, 0.0)
+    tor = np.flatnonzero(fid == 2)
+    eps = 1e-3
+    P = OracleParams(walks_per_sample=1, eps=eps, origin=origin)
+    rec, balls = orc.run_walks(P, True, tor.astype(np.int32), np.full((len(tor), 3), 1 / 3, np.float32), np.ones(len(tor), np.float32))
+    r, c = balls[:, 0], balls[:, 1:4]
+    ok = r > 0
+    assert ok.mean() > 0.95
+    near_origin = ok & ((np.linalg.norm(c, axis=1) ** 2 - r ** 2) < 0.05)      # balls whose primal image is large
+    assert near_origin.sum() > 20
+    pick = np.flatnonzero(near_origin)[:60]
+    # points on those Kelvin balls, mapped back to primal space: how deep do they sit inside a solid?
+    u = fibonacci_sphere(96)
+    y = (c[pick, None, :] + r[pick, None, None] * u[None, :, :]).reshape(-1, 3)
+    x = np.asarray(origin) + y / (y ** 2).sum(1, keepdims=True)
+    D = orc.closest_points(x.astype(np.float32))["dist"]
+    inside = orc.winding_number(x) > 0.5
+    rho = np.linalg.norm(x - np.asarray(origin), axis=1)
+    # allowed: eps/2 in Kelvin coordinates = (eps/2) rho^2 in primal ones (|kappa(x) - kappa(p)| = |x - p| / (|x||p|))
+    depth = np.where(inside, D, 0.0)
+    assert inside.sum() < 0.02 * len(x)
+    assert (depth <= 0.75 * eps * np.maximum(rho, 1.0) ** 2 + 1e-5).all(), (depth.max(), rho[depth.argmax()])
+    reach = np.linalg.norm(c, axis=1) + r
+    assert reach[ok].max() > 0.97                                  # some balls are limited by A: they nearly touch its image
