@@ -666,9 +666,11 @@ def accumulate_coo(bvh: Bvh, samples: Samples, params: Params, records, capacity
 
 
 def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params,
-                          capacity: int | None = None, max_retries=6):
+                          capacity: int | None = None, max_retries=6, scratch: dict | None = None):
     """Interior and exterior DtN matrices in sparse COO form from one mcs_estimate_dtn_both call (walk kernels
-    overlapped).  Same entries as two estimate_dtn_coo calls; one capacity for both, grown on MCS_ENOMEM."""
+    overlapped).  Same entries as two estimate_dtn_coo calls; one capacity for both, grown on MCS_ENOMEM.
+    scratch: a dict the caller keeps between calls; the workspace and the output buffers are kept in it and reused
+    while they are large enough (the returned matrices are then views into it, valid until the next call)."""
     import dataclasses
     K = bvh.V
     n_rec = max(num_records(samples, params_interior, False), num_records(samples, params_exterior, True))
@@ -677,18 +679,32 @@ def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, p
         pi = dataclasses.replace(params_interior, output_kind=1, coo_capacity=cap)
         pe = dataclasses.replace(params_exterior, output_kind=1, coo_capacity=cap)
         need = workspace_bytes_both(bvh, samples, pi, pe)
-        ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
-        bi, be = _coo_buffers(K, cap, bvh.device), _coo_buffers(K, cap, bvh.device)
+        ws = scratch.get("ws") if scratch is not None else None
+        if ws is None or ws.numel() < need or ws.device != bvh.device:
+            ws = None
+            if scratch is not None:
+                scratch.pop("ws", None)
+            ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+            if scratch is not None:
+                scratch["ws"] = ws
+        bufs = scratch.get("bufs") if scratch is not None else None
+        if bufs is None or bufs[0] != (K, cap):
+            bufs = ((K, cap), _coo_buffers(K, cap, bvh.device), _coo_buffers(K, cap, bvh.device))
+            if scratch is not None:
+                scratch["bufs"] = bufs
+        bi, be = bufs[1], bufs[2]
         cs, cb, ci, ce = samples.c(), _basis(bvh), pi.c(), pe.c()
         with torch.cuda.device(bvh.device):
             rc = lib().mcs_estimate_dtn_both(bvh.handle, C.byref(cs), C.byref(cb), C.byref(ci), C.byref(ce), _ptr(ws),
-                                             C.c_size_t(need), C.byref(bi[4]), C.byref(be[4]), None, None,
+                                             C.c_size_t(ws.numel()), C.byref(bi[4]), C.byref(be[4]), None, None,
                                              _stream(bvh.device))
             torch.cuda.current_stream(bvh.device).synchronize()
         worst = max(int(bi[3].item()), int(be[3].item()))
         if rc == MCS_ENOMEM and worst > cap:
             cap = min(K * (K + 1) // 2, max(2 * cap, 2 * worst))
-            del ws, bi, be
+            del ws, bi, be, bufs
+            if scratch is not None:
+                scratch.clear()
             continue
         _check(rc, "mcs_estimate_dtn_both (coo)")
         ni, ne = int(bi[3].item()), int(be[3].item())

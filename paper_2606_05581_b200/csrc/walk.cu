@@ -178,6 +178,7 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
 
     for (int64_t jj = (int64_t)blockIdx.x * TB_WARPS + wib; jj < n_s; jj += n_warps) {
         const int64_t i = order[jj];
+        const int own_face = tri[i];
         float3 s, n;
         sample_point(g.verts, g.faces, tri, bary, i, s, n);
         if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
@@ -218,7 +219,11 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
                     const TriData T = load_tri(g.tris, kk);
                     float v, w;
                     ++cnt_tris;
-                    if (closest_point_triangle(cJ, T, thr2J, v, w) < thr2J) {
+                    // The sample's own face is tangent to every ball of the family at s (distance exactly r): it can never
+                    // enter one.  In fp32 s sits up to ~2e-7 off its plane, which is more than eps/2 at the paper's
+                    // eps = 1e-6 and made the face "enter" every ball (38 of 41 000 samples discarded on
+                    // the unit icosphere; none in the fp64 oracle).  It is left out.
+                    if (T.orig != own_face && closest_point_triangle(cJ, T, thr2J, v, w) < thr2J) {
                         int lo_j = 0, hi_j = J;                           // ball_0 is empty by definition
                         while (hi_j - lo_j > 1) {
                             const int mid = (lo_j + hi_j) >> 1;
