@@ -259,6 +259,136 @@ void orc_closest_point(const orc_geom *g, const double x[3], orc_hit *h)
     h->dist = sqrt(best);
 }
 
+/* ------------------------------------------------------------------------- */
+/* Exact distance to the Kelvin image of a flat triangle  [DESIGN.md reading E4]. */
+/*                                                                            */
+/* The paper runs its exterior walks on "inverted triangle meshes with        */
+/* spherical-triangular elements and ... (non-planar) distance queries"       */
+/* (its stated exterior bottleneck): the     */
+/* Kelvin image of a flat face is a patch of the sphere through 0 that is the */
+/* image of the face's plane.  The distance from a point y of the inverted    */
+/* domain to that patch needs no spherical geometry: with x = kappa(y) and    */
+/* the distance identity of the inversion,                                    */
+/*     |kappa(x) - kappa(p)| = |x - p| / (|x| |p|),                            */
+/* it is  (1/|x|) min over p in T of |x - p| / |p|  (all coordinates about    */
+/* the inversion centre).  The level sets of |x - p| / |p| = k are the        */
+/* spheres of Apollonius, centre x / (1 - k^2), radius k |x| / |1 - k^2|, so  */
+/* the minimum over the triangle is attained                                  */
+/*   - where such a sphere touches the face's plane n.p = h:                  */
+/*       (n.x - h (1 - u))^2 = u |x|^2,  u = k^2  (the smaller root), at the  */
+/*       foot of the sphere's centre on the plane, if that foot lies in T, or */
+/*   - on an edge a + t e: the ratio of two quadratics with the same leading  */
+/*       coefficient, N(t)/D(t); N'D - ND' = 0 is a quadratic in t, or        */
+/*   - at a vertex.                                                            */
+/* Returns min |x - p|^2 / |p|^2 and the barycentrics of the minimiser.       */
+/* ------------------------------------------------------------------------- */
+static double ratio2_at(const double x[3], const double p[3])
+{
+    double d[3]; sub3(x, p, d);
+    double pp = dot3(p, p);
+    return pp > 0.0 ? dot3(d, d) / pp : INFINITY;
+}
+
+double orc_inverted_ratio2_triangle(const double x[3], const double a[3], const double b[3], const double c[3],
+                                    double bary[3])
+{
+    const double *vtx[3] = { a, b, c };
+    double best = INFINITY;
+    bary[0] = 1.0; bary[1] = bary[2] = 0.0;
+    /* vertices and edges */
+    for (int k = 0; k < 3; ++k) {
+        const double *P = vtx[k], *Q = vtx[(k + 1) % 3];
+        double e[3], xp[3]; sub3(Q, P, e); sub3(x, P, xp);
+        const double n0 = dot3(xp, xp), n1 = -2.0 * dot3(xp, e), n2 = dot3(e, e);
+        const double d0 = dot3(P, P), d1 = 2.0 * dot3(P, e);
+        double cand[4] = { 0.0, 1.0, -1.0, -1.0 };
+        const double qa = n2 * (d1 - n1), qb = 2.0 * n2 * (d0 - n0), qc = n1 * d0 - n0 * d1;
+        if (fabs(qa) > 1e-300) {
+            const double disc = qb * qb - 4.0 * qa * qc;
+            if (disc >= 0.0) {
+                const double sq = sqrt(disc);
+                /* numerically stable pair of roots */
+                const double q = -0.5 * (qb + (qb >= 0.0 ? sq : -sq));
+                cand[2] = q / qa;
+                if (fabs(q) > 0.0) cand[3] = qc / q;
+            }
+        } else if (fabs(qb) > 1e-300) {
+            cand[2] = -qc / qb;
+        }
+        for (int j = 0; j < 4; ++j) {
+            const double t = cand[j];
+            if (!(t >= 0.0 && t <= 1.0)) continue;
+            const double N = n0 + t * (n1 + t * n2), D = d0 + t * (d1 + t * n2);
+            const double f = D > 0.0 ? N / D : INFINITY;
+            if (f < best) {
+                best = f;
+                bary[0] = bary[1] = bary[2] = 0.0;
+                bary[k] = 1.0 - t; bary[(k + 1) % 3] = t;
+            }
+        }
+    }
+    /* interior: the Apollonius sphere that touches the plane */
+    double ab[3], ac[3], n[3];
+    sub3(b, a, ab); sub3(c, a, ac); cross3(ab, ac, n);
+    const double nn = dot3(n, n);
+    const double e2 = fmax(dot3(ab, ab), dot3(ac, ac));
+    if (nn > 1e-24 * e2 * e2) {
+        const double inv = 1.0 / sqrt(nn);
+        const double nh[3] = { n[0] * inv, n[1] * inv, n[2] * inv };
+        const double h = dot3(nh, a), hx = dot3(nh, x), xx = dot3(x, x);
+        double u = -1.0;
+        const double A2 = h * h, B2 = 2.0 * h * (hx - h) - xx, C2 = (hx - h) * (hx - h);
+        if (A2 > 1e-30 * xx) {
+            const double disc = B2 * B2 - 4.0 * A2 * C2;
+            if (disc >= 0.0) {
+                /* smaller root, written without cancellation: B2 < 0 whenever the roots are positive */
+                const double q = -0.5 * (B2 - sqrt(disc));
+                u = q > 0.0 ? C2 / q : -1.0;
+            }
+        } else if (xx > 0.0) {
+            u = C2 / xx;                                 /* plane through the inversion centre */
+        }
+        if (u >= 0.0 && fabs(1.0 - u) > 1e-12) {
+            double cc[3] = { x[0] / (1.0 - u), x[1] / (1.0 - u), x[2] / (1.0 - u) };
+            const double off = dot3(nh, cc) - h;
+            double p0[3] = { cc[0] - off * nh[0], cc[1] - off * nh[1], cc[2] - off * nh[2] };
+            /* barycentrics of p0 */
+            double ap[3]; sub3(p0, a, ap);
+            const double d00 = dot3(ab, ab), d01 = dot3(ab, ac), d11 = dot3(ac, ac), d20 = dot3(ap, ab), d21 = dot3(ap, ac);
+            const double den = d00 * d11 - d01 * d01;
+            const double v = (d11 * d20 - d01 * d21) / den, w = (d00 * d21 - d01 * d20) / den;
+            if (v >= 0.0 && w >= 0.0 && v + w <= 1.0) {
+                const double f = ratio2_at(x, p0);
+                if (f < best) { best = f; bary[0] = 1.0 - v - w; bary[1] = v; bary[2] = w; }
+            }
+        }
+    }
+    return best;
+}
+
+/* Brute force over all faces: h->dist receives the RATIO min_p |x - p| / |p - o| (dimensionless; the distance in
+ * Kelvin coordinates is ratio / |x - o|), h->cp the minimiser on the primal mesh.  Ties: smaller ratio, then smaller
+ * face index, as in orc_closest_point. */
+void orc_closest_point_inverted(const orc_geom *g, const double x[3], const double origin[3], orc_hit *h)
+{
+    double xr[3]; sub3(x, origin, xr);
+    double best = INFINITY;
+    h->tri = -1;
+    for (int64_t f = 0; f < g->F; ++f) {
+        double a[3], b[3], c[3], bary[3];
+        load_vertex(g, g->faces[3*f], a); load_vertex(g, g->faces[3*f+1], b); load_vertex(g, g->faces[3*f+2], c);
+        double ar[3], br[3], cr[3];
+        sub3(a, origin, ar); sub3(b, origin, br); sub3(c, origin, cr);
+        double r2 = orc_inverted_ratio2_triangle(xr, ar, br, cr, bary);
+        if (r2 < best) {
+            best = r2; h->tri = f;
+            memcpy(h->bary, bary, sizeof bary);
+            for (int k = 0; k < 3; ++k) h->cp[k] = bary[0] * a[k] + bary[1] * b[k] + bary[2] * c[k];
+        }
+    }
+    h->dist = sqrt(best);
+}
+
 /* Batch form for the parity tests: queries in fp32 (same numbers the GPU gets).
  * second[q] = smallest distance over faces that share no vertex with the winner
  * (for the tie filter of SURVEY.md 8(c)); may be NULL. */
@@ -412,6 +542,8 @@ typedef struct {
     int32_t estimator;              /* 0: Alg. 2 (tangent-ball jump kernel); 1: Alg. 1 (naive finite difference), interior only */
     int32_t pad_;
     double inset;                   /* Alg. 1: inset distance of the evaluation point x = s - inset n_s */
+    int32_t exterior_query;         /* 0: flat-triangle query + conservative radius [E3]; 1: exact distance to the inverted faces [E4] */
+    int32_t pad2_;
 } orc_params;
 
 typedef struct {                    /* one boundary sample            */
@@ -607,8 +739,16 @@ static int walk_on_spheres_kelvin(const orc_geom *g, const orc_params *P, uint32
         } else {
             double x[3] = { P->origin[0] + y[0] / (yn * yn), P->origin[1] + y[1] / (yn * yn), P->origin[2] + y[2] / (yn * yn) };
             double rho = 1.0 / yn;
-            orc_closest_point(g, x, h);
-            Rstar = h->dist / (rho * fmin(P->Rmax_norm, rho + h->dist));
+            if (P->exterior_query == 1 && g->kind == 0) {
+                /* [E4] the paper's own query: exact distance from y to the Kelvin-inverted faces = ratio / |x| */
+                orc_closest_point_inverted(g, x, P->origin, h);
+                Rstar = h->dist / rho;
+                double dd[3]; sub3(x, h->cp, dd);
+                h->dist = norm3(dd);                 /* primal distance to the exit point, for the [R10c] test below */
+            } else {
+                orc_closest_point(g, x, h);
+                Rstar = h->dist / (rho * fmin(P->Rmax_norm, rho + h->dist));
+            }
             if (Rstar < P->eps) return k;
             /* [R10c] The empty ball about x holds the inversion centre (D > |x - o| = rho): x lies in the same
              * component of space as the centre, i.e. INSIDE the solid.  On a closed, consistently oriented

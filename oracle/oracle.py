@@ -22,6 +22,7 @@ def _load():
         _lib.orc_u01.argtypes = [C.c_uint32]
         _lib.orc_closest_point_triangle.restype = C.c_double
         _lib.orc_closest_point_triangle_alt.restype = C.c_double
+        _lib.orc_inverted_ratio2_triangle.restype = C.c_double
         _lib.orc_rmax.restype = C.c_double
         _lib.orc_aabb_diagonal.restype = C.c_double
         _lib.orc_max_vertex_norm.restype = C.c_double
@@ -52,7 +53,8 @@ class _Params(C.Structure):
                 ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32),
                 ("n_kill_walks", C.c_int64), ("origin", C.c_double * 3), ("Rmax_norm", C.c_double),
-                ("escape_radius", C.c_double), ("estimator", C.c_int32), ("pad_", C.c_int32), ("inset", C.c_double)]
+                ("escape_radius", C.c_double), ("estimator", C.c_int32), ("pad_", C.c_int32), ("inset", C.c_double),
+                ("exterior_query", C.c_int32), ("pad2_", C.c_int32)]
 
 
 class _PointBasis(C.Structure):
@@ -97,6 +99,7 @@ class OracleParams:
     origin: tuple = (0.0, 0.0, 0.0)
     estimator: int = 0                   # 0: Alg. 2; 1: Alg. 1 (naive finite difference, interior only)
     inset: float = 0.0                   # Alg. 1: x = s - inset * n_s
+    exterior_query: int = 0              # 0: flat-triangle query + conservative radius (E3); 1: exact inverted faces (E4)
     rmax: float | None = None            # overrides the AABB rule (analytic sphere pins)
     Rmax_norm: float | None = None
 
@@ -153,6 +156,15 @@ def closest_point_triangle_alt(p, a, b, c):
     return d2, np.array(cp)
 
 
+def inverted_ratio2_triangle(x, a, b, c):
+    """min over the flat triangle (a, b, c) of |x - p|^2 / |p|^2 (coordinates about the inversion centre) and the
+    barycentrics of the minimiser: the exact distance to the Kelvin image of the face is sqrt(.) / |x| (reading E4)."""
+    lib = _load()
+    bary = (C.c_double * 3)()
+    r2 = lib.orc_inverted_ratio2_triangle(_d3(x), _d3(a), _d3(b), _d3(c), bary)
+    return r2, np.array(bary)
+
+
 class Oracle:
     """Brute-force CPU estimator over one geometry (mesh or analytic sphere)."""
 
@@ -187,6 +199,14 @@ class Oracle:
                                t.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
         return out
 
+    def closest_point_inverted(self, x, origin=(0, 0, 0)):
+        """(ratio, face, closest primal point, barycentrics): min over the mesh of |x - p| / |p - o| (reading E4)."""
+        class _Hit(C.Structure):
+            _fields_ = [("dist", C.c_double), ("cp", C.c_double * 3), ("bary", C.c_double * 3), ("tri", C.c_int64)]
+        h = _Hit()
+        self.lib.orc_closest_point_inverted(C.byref(self.geom.c), _d3(x), _d3(origin), C.byref(h))
+        return h.dist, int(h.tri), np.array(h.cp), np.array(h.bary)
+
     def rmax(self, exterior=False, origin=(0, 0, 0)):
         return self.lib.orc_rmax(C.byref(self.geom.c), C.c_int(int(exterior)), _d3(origin))
 
@@ -208,7 +228,8 @@ class Oracle:
                      eps=p.eps, cap_half_angle_deg=p.cap_half_angle_deg,
                      bisection_iters=p.bisection_iters, importance_sample=int(p.importance_sample),
                      antithetic=int(p.antithetic), include_killing=int(p.include_killing),
-                     n_kill_walks=int(p.n_kill_walks), estimator=int(p.estimator), inset=float(p.inset))
+                     n_kill_walks=int(p.n_kill_walks), estimator=int(p.estimator), inset=float(p.inset),
+                     exterior_query=int(p.exterior_query))
         cp.origin[:] = [float(x) for x in p.origin]
         if p.rmax is not None:
             cp.rmax = float(p.rmax)

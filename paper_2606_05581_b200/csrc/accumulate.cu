@@ -712,7 +712,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         const PairRec* pp = pairs; const uint32_t* pc = pair_counts;
         if (phase == 0) {
             mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
-            if (a.W > CH / 2) {                        // a sample spans several level-1 blocks: fold its repeated pairs (level 1b)
+            if (a.W > CH) {                            // a sample spans several level-1 blocks: fold its repeated pairs (level 1b)
                 int rcm = merge_pairs(pairs, pair_counts, slots, j0 / a.W, n / a.W + 2, b->F, (unsigned long long*)keys, vals,
                                       sort_ws, sort_bytes, pairs2, pair_counts2, st);
                 if (rcm != MCS_OK) return rcm;
@@ -852,7 +852,7 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
         const PairRec* pp = pairs; const uint32_t* pc = pair_counts;
         if (phase == 0) {
             mcs_note_launch(), pair_reduce_kernel<<<(unsigned)nblk1, CH, 0, st>>>(a, j0, n, pairs, pair_counts);
-            if (a.W > CH / 2) {                        // level 1b: fold the pairs a sample repeats over its level-1 blocks
+            if (a.W > CH) {                            // level 1b: fold the pairs a sample repeats over its level-1 blocks
                 int rcm = merge_pairs(pairs, pair_counts, slots, j0 / a.W, n / a.W + 2, b->F, keys[cur] + n_u, vals[cur] + n_u,
                                       sort_ws, sort_bytes, pairs2, pair_counts2, st);
                 if (rcm != MCS_OK) return rcm;
