@@ -172,6 +172,12 @@ typedef struct {
                                     the exact run.  The shell test and the exit point always come from an exact query.
                                     Deterministic (independent of the schedule).  Typical: 0.5                          */
     float    far_near_factor;    /* far_alpha > 0: boxes closer than this many eps are always descended (0: 16; >= 2)  */
+    int32_t  exterior_query;     /* exterior only.  0 (default): flat-triangle query at x = kappa(y) on the primal tree with
+                                    the conservative radius D / (rho min(R_max, rho + D)) (E3).  1: the paper's own
+                                    query, the EXACT distance from y to the Kelvin-inverted faces = (1/|x|) min
+                                    over the mesh of |x - p| / |p - o| (E4): larger balls, fewer jumps, a dearer
+                                    query; same estimator.  Not combinable with far_alpha                              */
+    int32_t  pad3_;
 } mcs_params;
 
 typedef struct {

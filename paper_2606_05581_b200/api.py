@@ -52,7 +52,8 @@ class _Params(C.Structure):
                 ("rmax_override", C.c_float), ("bisection_iters", C.c_int32), ("importance_sample", C.c_int32),
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
                 ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64),
-                ("estimator", C.c_int32), ("inset", C.c_float), ("far_alpha", C.c_float), ("far_near_factor", C.c_float)]
+                ("estimator", C.c_int32), ("inset", C.c_float), ("far_alpha", C.c_float), ("far_near_factor", C.c_float),
+                ("exterior_query", C.c_int32), ("pad3_", C.c_int32)]
 
 
 class _Matrix(C.Structure):
@@ -137,6 +138,7 @@ class Params:
     inset: float = 0.0                   # Alg. 1: walks start at s - inset * n_s
     far_alpha: float = 0.0               # > 0: far-field queries return a lower bound of the distance (mcs_params.far_alpha)
     far_near_factor: float = 0.0         # boxes closer than this many eps are always descended (0: 16)
+    exterior_query: int = 0              # exterior: 0 conservative radius on flat faces (E3); 1 exact inverted faces (E4)
 
     def c(self) -> _Params:
         p = _Params(seed=self.seed, walks_per_sample=self.walks_per_sample, max_steps=self.max_steps,
@@ -146,7 +148,7 @@ class Params:
                     include_killing=int(self.include_killing), n_kill_walks=int(self.n_kill_walks),
                     output_kind=int(self.output_kind), coo_capacity=int(self.coo_capacity),
                     estimator=int(self.estimator), inset=float(self.inset), far_alpha=float(self.far_alpha),
-                    far_near_factor=float(self.far_near_factor))
+                    far_near_factor=float(self.far_near_factor), exterior_query=int(self.exterior_query))
         p.kelvin_origin[:] = [float(x) for x in self.kelvin_origin]
         return p
 

@@ -143,6 +143,101 @@ __device__ __forceinline__ float closest_point_triangle(float3 p, const TriData&
     return best;
 }
 
+// ---------------------------------------------------------------------------
+// Exact distance to the Kelvin image of a flat face (reading E4; the paper's "spherical-triangular
+// elements" with "non-planar distance queries").  With x = kappa(y) and the distance identity of the
+// inversion, dist(y, kappa(T)) = (1/|x|) min over p in T of |x - p| / |p| (coordinates about the inversion centre), so
+// the query minimises the ratio over the FLAT face: where the Apollonius sphere {|x - p| = k |p|} (centre x / (1 - k^2))
+// touches the face's plane, if that point lies in the face; else on an edge (N(t)/D(t), two quadratics with the same
+// leading coefficient: the stationary points solve a quadratic) or at a vertex.  Every candidate's value is recomputed
+// from the candidate point itself, |x - p|^2 / |p|^2 with the differences taken directly, so the cancellation-prone
+// closed forms only choose WHERE, not the value.  X, and the vertices in T, are relative to the inversion centre.
+// Returns the squared ratio; (v, w) = weights of b and c.
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ float ratio2_point(float3 X, float3 P)
+{
+    const float3 d = X - P;
+    const float pp = dot3(P, P);
+    return pp > 0.0f ? __fdividef(dot3(d, d), pp) : CUDART_INF_F;
+}
+
+__device__ __forceinline__ float inverted_ratio2_triangle(float3 X, float3 A, float3 B, float3 C, float3 n, float nn, bool degenerate,
+                                                          float& v, float& w)
+{
+    float best = ratio2_point(X, A); v = 0.0f; w = 0.0f;
+    { const float f = ratio2_point(X, B); if (f < best) { best = f; v = 1.0f; w = 0.0f; } }
+    { const float f = ratio2_point(X, C); if (f < best) { best = f; v = 0.0f; w = 1.0f; } }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const float3 P = k == 0 ? A : (k == 1 ? B : C), Q = k == 0 ? B : (k == 1 ? C : A);
+        const float3 e = Q - P, xp = X - P;
+        const float n0 = dot3(xp, xp), n1 = -2.0f * dot3(xp, e), n2 = dot3(e, e);
+        const float d0 = dot3(P, P), d1 = 2.0f * dot3(P, e);
+        const float qa = n2 * (d1 - n1), qb = 2.0f * n2 * (d0 - n0), qc = n1 * d0 - n0 * d1;
+        const float disc = qb * qb - 4.0f * qa * qc;
+        if (disc >= 0.0f) {
+            const float q = -0.5f * (qb + copysignf(sqrtf(disc), qb));
+            const float t1 = qa != 0.0f ? q / qa : -1.0f, t2 = q != 0.0f ? qc / q : -1.0f;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const float t = j ? t2 : t1;
+                if (t > 0.0f && t < 1.0f) {
+                    const float3 Pt = f3(fmaf(t, e.x, P.x), fmaf(t, e.y, P.y), fmaf(t, e.z, P.z));
+                    const float f = ratio2_point(X, Pt);
+                    if (f < best) {
+                        best = f;
+                        v = k == 0 ? t : (k == 1 ? 1.0f - t : 0.0f);
+                        w = k == 0 ? 0.0f : (k == 1 ? t : 1.0f - t);
+                    }
+                }
+            }
+        }
+    }
+    if (!degenerate) {
+        const float inv = rsqrtf(nn);
+        const float3 nh = inv * n;
+        const float h = dot3(nh, A), hx = dot3(nh, X), xx = dot3(X, X);
+        const float A2 = h * h, B2 = 2.0f * h * (hx - h) - xx, C2 = (hx - h) * (hx - h);
+        float u = -1.0f;
+        if (A2 > 1e-12f * xx) {
+            const float disc = B2 * B2 - 4.0f * A2 * C2;
+            if (disc >= 0.0f) { const float q = -0.5f * (B2 - sqrtf(disc)); u = q > 0.0f ? C2 / q : -1.0f; }
+        } else if (xx > 0.0f) {
+            u = C2 / xx;
+        }
+        if (u >= 0.0f && fabsf(1.0f - u) > 1e-6f) {
+            const float s = 1.0f / (1.0f - u);
+            const float3 cc = s * X;
+            const float off = dot3(nh, cc) - h;
+            const float3 p0 = f3(cc.x - off * nh.x, cc.y - off * nh.y, cc.z - off * nh.z);
+            // |n|^2-scaled barycentrics of p0 by edge functions, as in closest_point_triangle
+            const float3 Aq = A - p0, Bq = B - p0, Cq = C - p0;
+            const float wb = dot3(cross3(Cq, Aq), n), wc = dot3(cross3(Aq, Bq), n), wa = nn - wb - wc;
+            if (wa >= 0.0f && wb >= 0.0f && wc >= 0.0f) {
+                const float rnn = 1.0f / nn;
+                const float vv = fminf(wb * rnn, 1.0f), ww = fminf(wc * rnn, 1.0f - vv);
+                const float uu = 1.0f - vv - ww;
+                const float3 pt = f3(fmaf(uu, A.x, fmaf(vv, B.x, ww * C.x)), fmaf(uu, A.y, fmaf(vv, B.y, ww * C.y)), fmaf(uu, A.z, fmaf(vv, B.z, ww * C.z)));
+                const float f = ratio2_point(X, pt);
+                if (f < best) { best = f; v = vv; w = ww; }
+            }
+        }
+    }
+    return best;
+}
+
+// Lower bound of |x - p|^2 / |p - o|^2 over a box: squared distance of x to the box over the squared distance of the
+// box's farthest corner from o.
+__device__ __forceinline__ float box_ratio2(float3 x, float3 o, float lx, float ly, float lz, float hx, float hy, float hz)
+{
+    const float d2 = fmaf(fmaxf(fmaxf(lx - x.x, x.x - hx), 0.0f), fmaxf(fmaxf(lx - x.x, x.x - hx), 0.0f),
+                     fmaf(fmaxf(fmaxf(ly - x.y, x.y - hy), 0.0f), fmaxf(fmaxf(ly - x.y, x.y - hy), 0.0f),
+                          fmaxf(fmaxf(lz - x.z, x.z - hz), 0.0f) * fmaxf(fmaxf(lz - x.z, x.z - hz), 0.0f)));
+    const float fx = fmaxf(fabsf(lx - o.x), fabsf(hx - o.x)), fy = fmaxf(fabsf(ly - o.y), fabsf(hy - o.y)), fz = fmaxf(fabsf(lz - o.z), fabsf(hz - o.z));
+    const float far2 = fmaf(fx, fx, fmaf(fy, fy, fz * fz));
+    return far2 < 3.0e38f ? __fdividef(d2, far2) * (1.0f - 4e-7f) : CUDART_INF_F;      // empty slot (lo = +inf): never visited
+}
+
 __device__ __forceinline__ float box_dist2(float3 p, float lx, float ly, float lz, float hx, float hy, float hz)
 {
     const float dx = fmaxf(fmaxf(lx - p.x, p.x - hx), 0.0f);

@@ -569,8 +569,13 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 // is never taken from it: boxes closer than the near threshold (a multiple of eps, in the exterior the distance whose
 // Kelvin radius is that multiple) are always descended.  The estimator is the same in expectation; single walks differ
 // from the exact run, so record-level parity tests run with far_alpha = 0 and matrices are compared statistically.
-template <bool EXT, bool COUNT, bool COOP, bool MERGED, bool FAR>
-__global__ void __launch_bounds__(WT, MERGED ? 4 : (COOP ? WALK_COOP_BLOCKS : WALK_MIN_BLOCKS))      // small jobs: registers instead of occupancy
+// KEX (exterior, mcs_params.exterior_query = 1): the paper's own exterior query, the exact distance from the walker to
+// the Kelvin-inverted faces (reading E4), instead of the flat-triangle query with the conservative radius E3.
+// The traversal runs on the SAME primal tree: a box is bounded below by box_ratio2, a face is tested by
+// inverted_ratio2_triangle; h.d2 holds the best squared ratio, the radius in Kelvin coordinates is ratio / |x - o|.
+// Lane path only (no cooperative take-over, no merged passes, no far-field cut): a cross-check variant.
+template <bool EXT, bool COUNT, bool COOP, bool MERGED, bool FAR, bool KEX = false>
+__global__ void __launch_bounds__(WT, MERGED ? 4 : (COOP ? WALK_COOP_BLOCKS : (KEX ? 6 : WALK_MIN_BLOCKS)))      // small jobs: registers instead of occupancy
 walk_kernel(WalkGeom g, WalkArgs a)
 {
     __shared__ int   sh_ref[WSTACK * WT];
@@ -674,10 +679,18 @@ walk_kernel(WalkGeom g, WalkArgs a)
               } else {
                 if (COUNT) { ++n_nodes; ++q_nodes; }
                 if (COOP) ++q_visits;
-                float d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
-                float d1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
-                float d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
-                float d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
+                float d0, d1, d2, d3;
+                if (KEX) {
+                    d0 = box_ratio2(xq, o, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
+                    d1 = box_ratio2(xq, o, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
+                    d2 = box_ratio2(xq, o, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
+                    d3 = box_ratio2(xq, o, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
+                } else {
+                    d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
+                    d1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
+                    d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
+                    d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
+                }
                 int c0 = __float_as_int(q3.lo.x), c1 = __float_as_int(q3.lo.y), c2 = __float_as_int(q3.lo.z), c3 = __float_as_int(q3.lo.w);
                 if (FAR) {
                     // q3.hi = squared diagonals of the four child boxes (+inf for an empty slot, so it never qualifies)
@@ -716,9 +729,17 @@ walk_kernel(WalkGeom g, WalkArgs a)
         }
         if (!MERGED && which == KIND_TRI) {
             if (kind == KIND_TRI) {
-                test_triangle(g.tris, ~cur, xq, h, lim);
+                if (KEX) {
+                    const TriData T = load_tri(g.tris, ~cur);
+                    float tv = 0.0f, tw = 0.0f;
+                    const float r2 = inverted_ratio2_triangle(xq - o, T.a - o, T.b - o, T.c - o, T.n, T.nn, T.degenerate, tv, tw);
+                    if (r2 < h.d2 || (r2 == h.d2 && T.orig < h.tri)) { h.d2 = r2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
+                    lim = fminf(fmaf(h.d2, 4e-4f, h.d2) + 1e-14f, 3.0e38f);            // relative margin: lane path only, so the order is fixed
+                } else {
+                    test_triangle(g.tris, ~cur, xq, h, lim);
+                    lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
+                }
                 if (COUNT) ++n_tris;
-                lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
                 cur = CUR_NONE;
             }
         }
@@ -737,9 +758,18 @@ walk_kernel(WalkGeom g, WalkArgs a)
                     // FAR: the minimum over the cut is a box, not a face: jump with the lower bound, no shell test
                     const bool far_hit = FAR && lb2 < h.d2;
                     if (FAR && COUNT && far_hit) ++n_far;
-                    const float D = sqrtf(far_hit ? lb2 : h.d2);
-                    if (FAR) h.d2 = D * D;                        // the rules below read the distance from h.d2
-                    radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
+                    float D = sqrtf(far_hit ? lb2 : h.d2);
+                    if (KEX) {
+                        // D is the ratio |x - p| / |p - o| at its minimiser p: the exact distance to the inverted surface is
+                        // ratio / rho.  The primal distance to p is kept for the R10c test below.
+                        radius = D / rho;
+                        const float3 dp = hit_point(g.tris, h) - xq;
+                        D = sqrtf(dot3(dp, dp));
+                        h.d2 = D * D;
+                    } else {
+                        if (FAR) h.d2 = D * D;                    // the rules below read the distance from h.d2
+                        radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
+                    }
                     if (!far_hit && radius < a.eps) {
                         float wgt = wfac;
                         if (EXT) {
@@ -937,6 +967,8 @@ int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, in
     if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
     if (s->n_s * (int64_t)p->walks_per_sample >= ((int64_t)1 << 40)) return MCS_EINVAL;
     if (!(p->far_alpha >= 0.0f) || p->far_alpha > 4.0f || !(p->far_near_factor >= 0.0f)) return MCS_EINVAL;
+    if (p->exterior_query != 0 && p->exterior_query != 1) return MCS_EINVAL;
+    if (p->exterior_query == 1 && (!exterior || p->far_alpha > 0.0f)) return MCS_EINVAL;      // E4 is an exterior query; the far-field cut belongs to E3
     return MCS_OK;
 }
 
@@ -1086,7 +1118,10 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         MCS_WK(false, false, true, true),   MCS_WK(false, true, true, true),   MCS_WK(true, false, true, true),   MCS_WK(true, true, true, true) };
 #undef MCS_WK
     const int far = p->far_alpha > 0.0f ? 1 : 0;
-    const walk_fn fn = merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)][far]
+    static const walk_fn kex_table[2] = { walk_kernel<true, false, false, false, false, true>, walk_kernel<true, true, false, false, false, true> };
+    const bool kex = exterior && p->exterior_query == 1;
+    const walk_fn fn = kex ? kex_table[count ? 1 : 0]
+                     : merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)][far]
                               : table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)][far];
     MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
     if (per_sm < 1) per_sm = 1;
