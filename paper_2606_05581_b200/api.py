@@ -613,33 +613,36 @@ def _coo_buffers(K, capacity, device):
 
 def estimate_dtn_coo(bvh: Bvh, samples: Samples, params: Params, exterior: bool, capacity: int | None = None,
                      want_stats=False, max_retries=6):
-    """DtN matrix in sparse COO form (any K): mcs_estimate_dtn_* with output_kind 1.  When the capacity
-    guess is too small the library reports MCS_ENOMEM with a lower bound of the need; the call is
-    repeated with a larger buffer."""
+    """DtN matrix in sparse COO form (any K): mcs_estimate_dtn_* with output_kind 1.  When the capacity guess is too
+    small the library reports MCS_ENOMEM with a lower bound of the need; the walks are NOT repeated: their records are
+    still at the head of the workspace, and only the accumulation (mcs_accumulate) is run again with a larger buffer."""
     import dataclasses
     K = bvh.V
     n_rec = num_records(samples, params, exterior)
     cap = int(capacity) if capacity else max(4096, min(K * (K + 1) // 2, 4 * n_rec))
     fn = lib().mcs_estimate_dtn_exterior if exterior else lib().mcs_estimate_dtn_interior
-    for _ in range(max_retries):
-        p = dataclasses.replace(params, output_kind=1, coo_capacity=cap)
-        cs, cb, cp = samples.c(), _basis(bvh), p.c()
-        need = int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
-        ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
-        row, col, val, nnz, m = _coo_buffers(K, cap, bvh.device)
-        st = Stats()
-        with torch.cuda.device(bvh.device):
-            rc = fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(ws), C.c_size_t(need), C.byref(m),
-                    C.byref(st), _stream(bvh.device))
-        if rc == MCS_ENOMEM and int(nnz.item()) > cap:
-            cap = min(K * (K + 1) // 2, max(2 * cap, 2 * int(nnz.item())))
-            del ws, row, col, val
-            continue
-        _check(rc, "mcs_estimate_dtn (coo)")
-        n = int(nnz.item())
-        out = CooMatrix(K, row[:n], col[:n], val[:n])
+    p = dataclasses.replace(params, output_kind=1, coo_capacity=cap)
+    cs, cb, cp = samples.c(), _basis(bvh), p.c()
+    need = int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
+    ws = torch.empty(need, dtype=torch.uint8, device=bvh.device)
+    row, col, val, nnz, m = _coo_buffers(K, cap, bvh.device)
+    st = Stats()
+    with torch.cuda.device(bvh.device):
+        rc = fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(ws), C.c_size_t(need), C.byref(m),
+                C.byref(st), _stream(bvh.device))
+    if rc == MCS_ENOMEM and int(nnz.item()) > cap:
+        if max_retries <= 1:
+            raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")
+        # records: [n_rec][4] fp32 at offset 0 of the workspace (capi.cu make_layout); the walk counters are already in st
+        records = ws[: n_rec * 16].view(torch.float32).view(n_rec, 4).clone()
+        del ws, row, col, val
+        out = accumulate_coo(bvh, samples, params, records, capacity=max(2 * cap, 2 * int(nnz.item())), max_retries=max_retries - 1)
+        st.n_unique = out.nnz
         return (out, st) if want_stats else out
-    raise McsError(MCS_ENOMEM, "estimate_dtn_coo", "capacity retries exhausted")
+    _check(rc, "mcs_estimate_dtn (coo)")
+    n = int(nnz.item())
+    out = CooMatrix(K, row[:n], col[:n], val[:n])
+    return (out, st) if want_stats else out
 
 
 def accumulate_coo(bvh: Bvh, samples: Samples, params: Params, records, capacity: int | None = None, max_retries=6):
@@ -703,11 +706,20 @@ def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, p
             torch.cuda.current_stream(bvh.device).synchronize()
         worst = max(int(bi[3].item()), int(be[3].item()))
         if rc == MCS_ENOMEM and worst > cap:
-            cap = min(K * (K + 1) // 2, max(2 * cap, 2 * worst))
+            if max_retries <= 1:
+                raise McsError(MCS_ENOMEM, "estimate_dtn_coo_both", "capacity retries exhausted")
+            # The walks are not repeated: both operators' records sit at the head of their halves of the workspace
+            # (capi.cu estimate_both: interior at 0, exterior behind the interior's layout); only A7 runs again.
+            n_i, n_e = num_records(samples, pi, False), num_records(samples, pe, True)
+            off = workspace_bytes(bvh, samples, pi, False)
+            rec_i = ws[: n_i * 16].view(torch.float32).view(n_i, 4).clone()
+            rec_e = ws[off: off + n_e * 16].view(torch.float32).view(n_e, 4).clone()
             del ws, bi, be, bufs
             if scratch is not None:
                 scratch.clear()
-            continue
+            big = max(2 * cap, 2 * worst)
+            return (accumulate_coo(bvh, samples, params_interior, rec_i, capacity=big, max_retries=max_retries - 1),
+                    accumulate_coo(bvh, samples, params_exterior, rec_e, capacity=big, max_retries=max_retries - 1))
         _check(rc, "mcs_estimate_dtn_both (coo)")
         ni, ne = int(bi[3].item()), int(be[3].item())
         return (CooMatrix(K, bi[0][:ni], bi[1][:ni], bi[2][:ni]), CooMatrix(K, be[0][:ne], be[1][:ne], be[2][:ne]))

@@ -178,10 +178,14 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
 
     for (int64_t jj = (int64_t)blockIdx.x * TB_WARPS + wib; jj < n_s; jj += n_warps) {
         const int64_t i = order[jj];
-        const int own_face = tri[i];
         float3 s, n;
         sample_point(g.verts, g.faces, tri, bary, i, s, n);
-        if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
+        int own_face = tri[i];
+        if (normal) {
+            const float3 nf = n;
+            n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
+            if (!(fabsf(dot3(n, nf)) > 0.999999f)) own_face = -1;      // an override off the face's normal line: the ball is not tangent to the face
+        }
         BallFamily fam;
         fam.base = s; fam.pole = n; fam.o = o; fam.ss2 = 1.0f; fam.sdn = 0.0f; fam.eps = eps;
         float hi = rmax, sstar_norm = 1.0f;
