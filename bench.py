@@ -398,45 +398,45 @@ def make_cfg4_sample(n_meshes, seed0=0):
 
 def bench_cfg4_sample(api, torch, dev, args, seed, n_meshes, flush):
     meshes = make_cfg4_sample(n_meshes)
-    W, n_eig = 1024, 64
+    W, n_eig, K = 1024, 64, 512
     pinned = [{k: torch.as_tensor(m[k]).pin_memory() for k in ("v", "f", "tri", "bary", "weight", "pts")} for m in meshes]
-    Si = torch.empty((n_meshes, 512, 512), dtype=torch.float32, device=dev)
+    Si = torch.empty((n_meshes, K, K), dtype=torch.float32, device=dev)
     Se = torch.empty_like(Si)
-    mass = torch.empty((n_meshes, 512), dtype=torch.float32, device=dev)
-    total_steps = 0
+    mass = torch.empty((n_meshes, K), dtype=torch.float32, device=dev)
+    Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3)
+    Pe = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, far_alpha=args.far_alpha, far_near_factor=args.far_near)
 
-    def one_pass(count):
-        nonlocal total_steps
-        for i, (m, h) in enumerate(zip(meshes, pinned)):
+    def one_pass():
+        # upload of every mesh from pinned host memory (async on the current stream), then ONE batch call: per mesh
+        # LBVH build, sidedness, both estimators in the k-NN point basis of its 512 samples (normals of the basis =
+        # face normals at the samples, oriented by the same sidedness rule in a first batch of normals-only work)
+        items = []
+        for m, h in zip(meshes, pinned):
             vd, fd = h["v"].to(dev, non_blocking=True), h["f"].to(dev, non_blocking=True)
             S0 = api.Samples(h["tri"].to(dev, non_blocking=True), h["bary"].to(dev, non_blocking=True), h["weight"].to(dev, non_blocking=True))
-            pts = h["pts"].to(dev, non_blocking=True)
-            bvh = api.build_bvh(vd, fd)
-            nrm, _ = api.orient_samples_fast(bvh, S0, beta=args.orient_beta) if args.orient_beta > 0 else api.orient_samples(bvh, S0)
-            S = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
-            basis = api.PointBasis(pts, nrm, k=8, sigma=0.025, tau_n=0.8)
-            Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3)
-            Pe = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, kelvin_origin=m["origin"], far_alpha=args.far_alpha,
-                            far_near_factor=args.far_near)
-            if count:
-                _, _, sti, ste = api.estimate_dtn_both(bvh, S, Pi, Pe, want_stats=True, out_interior=Si[i], out_exterior=Se[i], basis=basis)
-                total_steps += sti.n_steps + ste.n_steps
-            else:
-                api.estimate_dtn_both(bvh, S, Pi, Pe, out_interior=Si[i], out_exterior=Se[i], basis=basis)
-            mass[i] = S0.weight
-        # Steklov eigenpairs of all matrices of the pass in two batched calls (lumped mass = the samples' weights)
+            items.append(dict(verts=vd, faces=fd, samples=S0, origin=m["origin"], pts=h["pts"].to(dev, non_blocking=True)))
+        # the point basis needs outward normals at the nodes: face normals of the samples, oriented by the library
+        for it in items:
+            f_s = it["faces"][it["samples"].tri.long()].long()
+            a, b, c = it["verts"][f_s[:, 0]], it["verts"][f_s[:, 1]], it["verts"][f_s[:, 2]]
+            n = torch.linalg.cross(b - a, c - a)
+            it["basis"] = api.PointBasis(it["pts"], n / n.norm(dim=1, keepdim=True).clamp_min(1e-30), k=8, sigma=0.025, tau_n=0.8)
+        normals = api.estimate_dtn_batch(items, Pi, Pe, Si, Se, orient_h_scale=1.0, orient_beta=args.orient_beta if args.orient_beta > 0 else 0.0,
+                                         n_workers=args.cfg4_workers)
+        for i, it in enumerate(items):
+            mass[i] = it["samples"].weight
         ei, _, _ = api.steklov_eigs(Si, mass, n_eig)
         ee, _, _ = api.steklov_eigs(Se, mass, n_eig)
         return ei, ee
 
-    one_pass(True)                                  # warm-up, and the deterministic step counts
+    one_pass()                                      # warm-up
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = api.launch_count()
     t0 = time.perf_counter()
     e0.record(stream)
-    one_pass(False)
+    one_pass()
     e1.record(stream)
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
@@ -444,11 +444,12 @@ def bench_cfg4_sample(api, torch, dev, args, seed, n_meshes, flush):
     faces = [len(m["f"]) for m in meshes]
     return {"workload": f"configs[4] sample: {n_meshes} stress-style meshes (seeds 0..{n_meshes - 1}, {min(faces)}-{max(faces)} faces), per mesh: "
                         f"upload from pinned host memory, LBVH build, sidedness pre-pass, 512 FPS samples = nodes of the k-NN point basis "
-                        f"(k=8), {W} walks per sample, interior + exterior (killing off; far-field bound as in the headline), then top-{n_eig} Steklov eigenpairs of all "
-                        f"{2 * n_meshes} matrices in two batched calls",
+                        f"(k=8, face normals at the nodes), {W} walks per sample, interior + exterior (killing off; exterior far-field bound as "
+                        f"in the headline) through ONE mcs_estimate_dtn_batch call ({args.cfg4_workers} workers), then top-{n_eig} Steklov "
+                        f"eigenpairs of all {2 * n_meshes} matrices in two batched calls",
             "metric": "meshes_per_s", "value": n_meshes / (ms * 1e-3), "unit": "meshes/s", "ms_per_mesh": ms / n_meshes,
-            "wall_ms_per_mesh": wall * 1e3 / n_meshes, "walk_steps_per_s": total_steps / (ms * 1e-3),
-            "gpu_launches": api.launch_count() - l0, "meshes": n_meshes, "mean_faces": float(np.mean(faces))}
+            "wall_ms_per_mesh": wall * 1e3 / n_meshes, "gpu_launches": api.launch_count() - l0, "meshes": n_meshes,
+            "mean_faces": float(np.mean(faces)), "workers": args.cfg4_workers}
 
 
 # ------------------------------------------------------------------------------
@@ -678,7 +679,8 @@ def main():
     ap.add_argument("--cpu-walks", type=int, default=8, help="walks per sample point of the cpu_baseline leg")
     ap.add_argument("--ref-samples", type=int, default=8, help="sample points per step of --impl reference")
     ap.add_argument("--ref-walks", type=int, default=4, help="walks per sample point per step of --impl reference")
-    ap.add_argument("--cfg4-meshes", type=int, default=16, help="meshes of the configs[4] sample sub-record")
+    ap.add_argument("--cfg4-meshes", type=int, default=32, help="meshes of the configs[4] sample sub-record")
+    ap.add_argument("--cfg4-workers", type=int, default=4, help="host workers of mcs_estimate_dtn_batch in that sub-record")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sub", action="store_true", help="skip the configs[1] / configs[4] sub-records")
     ap.add_argument("--no-cache", action="store_true", help="regenerate the workload instead of reading the temp-dir cache")

@@ -308,6 +308,36 @@ int mcs_estimate_dtn_host_coo(const float* verts, int64_t V, const int32_t* face
                               float orient_h_scale, float orient_beta, mcs_host_coo* out_interior, mcs_host_coo* out_exterior,
                               mcs_stats* stats_interior, mcs_stats* stats_exterior, void* stream);
 
+/*
+ * Many meshes in one call (BASELINE config 4: "1024 seeded synthetic meshes ... interior and exterior DtN ... meshes/s
+ * end to end"; dataset-scale runs, one shape after another).  For every item: LBVH build, optional
+ * sidedness pre-pass (orient_h_scale > 0: mcs_orient_samples, or mcs_orient_samples_fast when orient_beta > 0; the
+ * normals are written to item.normal_out and used as the samples' normals), then both estimators as in
+ * mcs_estimate_dtn_both with DENSE outputs (item.basis.K squared each; params_*->output_kind must be 0;
+ * params_exterior->kelvin_origin is replaced by item.kelvin_origin).  `n_workers` (0: 4, at most 16) host threads, each
+ * with its own stream and workspace, take the items in turn, so that the small launches, the host read-backs and the
+ * tail of one mesh's walks overlap with the bulk of another's; every item is computed exactly as by the single calls
+ * (results do not depend on n_workers).  items is a HOST array whose pointers are DEVICE pointers; item.rc receives the
+ * item's return code.  Work starts after what `stream` holds at the call (uploads) and `stream` continues after all
+ * of it; the call blocks until everything is done.  Returns the first non-zero item code.
+ */
+typedef struct {
+    const float*   verts;        /* [V][3] device */
+    int64_t        V;
+    const int32_t* faces;        /* [F][3] device */
+    int64_t        F;
+    mcs_samples    samples;      /* device pointers; samples.normal is replaced by normal_out when orient_h_scale > 0 */
+    mcs_basis      basis;        /* kind 0: K = V; kind 1: the point basis of this mesh */
+    float          kelvin_origin[3];
+    int32_t        rc;           /* out */
+    float*         out_interior; /* [K][K] device */
+    float*         out_exterior; /* [K][K] device */
+    float*         normal_out;   /* [n_s][3] device, or NULL when orient_h_scale <= 0 */
+} mcs_batch_item;
+int mcs_estimate_dtn_batch(mcs_batch_item* items /* host */, int64_t n_items, const mcs_params* params_interior,
+                           const mcs_params* params_exterior, float orient_h_scale, float orient_beta, int32_t n_workers,
+                           void* stream);
+
 /* ------------------------------------------------------------------------ */
 /* Test / benchmark hooks for the individual steps of SURVEY.md 8(a).         */
 /* ------------------------------------------------------------------------ */
@@ -448,7 +478,7 @@ const char* mcs_error_string(int code);
 const char* mcs_version(void);
 /* sizeof of the ABI structs, for bindings to check their mirrors against:
  * 0 mcs_samples, 1 mcs_basis, 2 mcs_params, 3 mcs_matrix, 4 mcs_stats, 5 mcs_bvh_info_t,
- * 6 mcs_record, 7 mcs_host_coo; anything else: 0. */
+ * 6 mcs_record, 7 mcs_host_coo, 8 mcs_batch_item; anything else: 0. */
 size_t mcs_abi_sizeof(int which);
 
 #ifdef __cplusplus

@@ -465,6 +465,50 @@ def estimate_dtn_host_coo(verts, faces, tri, bary, weight, params_interior: Para
     return res
 
 
+class _BatchItem(C.Structure):
+    _fields_ = [("verts", C.c_void_p), ("V", C.c_int64), ("faces", C.c_void_p), ("F", C.c_int64), ("samples", _Samples),
+                ("basis", _Basis), ("kelvin_origin", C.c_float * 3), ("rc", C.c_int32), ("out_interior", C.c_void_p),
+                ("out_exterior", C.c_void_p), ("normal_out", C.c_void_p)]
+
+
+def estimate_dtn_batch(meshes, params_interior: Params, params_exterior: Params, out_interior, out_exterior,
+                       orient_h_scale=1.0, orient_beta=2.5, n_workers=4):
+    """Interior and exterior dense DtN matrices of many meshes in one call (mcs_estimate_dtn_batch).
+    meshes: list of dicts with CUDA tensors verts [V,3] fp32, faces [F,3] int32, samples (Samples), optional basis
+    (PointBasis; default hat basis K = V), origin (3 floats).  out_interior / out_exterior: lists of (or a stacked
+    tensor of) CUDA fp32 [K,K] matrices, one per mesh.  Returns the list of sidedness normals (or None)."""
+    n = len(meshes)
+    items = (_BatchItem * n)()
+    keep, normals = [], []
+    dev = meshes[0]["verts"].device
+    for i, m in enumerate(meshes):
+        v, f, S = _dev(m["verts"], torch.float32, "verts"), _dev(m["faces"], torch.int32, "faces"), m["samples"]
+        basis = m.get("basis")
+        cb = basis.c() if basis is not None else _Basis(kind=0, K=int(v.shape[0]))
+        K = int(cb.K)
+        oi, oe = out_interior[i], out_exterior[i]
+        for o in (oi, oe):
+            if not (o.is_cuda and o.dtype == torch.float32 and o.is_contiguous() and tuple(o.shape) == (K, K)):
+                raise ValueError("batch outputs must be contiguous CUDA float32 [K, K] matrices")
+        nrm = torch.empty((S.n_s, 3), dtype=torch.float32, device=dev) if orient_h_scale > 0 else None
+        normals.append(nrm)
+        keep.append((v, f, S, basis, nrm))
+        it = items[i]
+        it.verts, it.V, it.faces, it.F = v.data_ptr(), int(v.shape[0]), f.data_ptr(), int(f.shape[0])
+        it.samples, it.basis = S.c(), cb
+        it.kelvin_origin[:] = [float(x) for x in m.get("origin", (0.0, 0.0, 0.0))]
+        it.out_interior, it.out_exterior = oi.data_ptr(), oe.data_ptr()
+        it.normal_out = nrm.data_ptr() if nrm is not None else None
+    ci, ce = params_interior.c(), params_exterior.c()
+    with torch.cuda.device(dev):
+        rc = lib().mcs_estimate_dtn_batch(items, C.c_int64(n), C.byref(ci), C.byref(ce), C.c_float(float(orient_h_scale)),
+                                          C.c_float(float(orient_beta)), C.c_int32(int(n_workers)), _stream(dev))
+    if rc != MCS_OK:
+        bad = [(i, items[i].rc) for i in range(n) if items[i].rc != MCS_OK]
+        raise McsError(rc, "mcs_estimate_dtn_batch", f"{lib().mcs_error_string(rc).decode()}; failing items {bad[:8]}")
+    return normals if orient_h_scale > 0 else None
+
+
 def tangent_balls(bvh: Bvh, samples: Samples, params: Params, exterior: bool):
     cs, cp = samples.c(), params.c()
     balls = torch.empty((samples.n_s, 8), dtype=torch.float32, device=bvh.device)

@@ -139,21 +139,42 @@ __global__ void stream_delay_kernel(unsigned long long ns)
 // launch gives up in its tail, and the interior's accumulation fills the exterior's tail.
 // which: 0 = the interior's stream (highest priority: its blocks are dispatched first, so the exterior's bulk runs
 // beside the interior's long tail and not the other way round), 1 = the exterior's stream (lowest priority).
-cudaStream_t side_stream(int which)
-{
-    static thread_local cudaStream_t ss[2] = { nullptr, nullptr };
-    static thread_local int ss_dev = -1;
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
-    if (!ss[0] || ss_dev != dev) {
-        int least = 0, greatest = 0;
-        if (cudaDeviceGetStreamPriorityRange(&least, &greatest) != cudaSuccess) return nullptr;
-        if (cudaStreamCreateWithPriority(&ss[0], cudaStreamNonBlocking, greatest) != cudaSuccess ||
-            cudaStreamCreateWithPriority(&ss[1], cudaStreamNonBlocking, least) != cudaSuccess) { ss[0] = nullptr; return nullptr; }
-        ss_dev = dev;
+// Per host thread: the two side streams (interior: highest priority, exterior: lowest) and the three events of
+// estimate_both, created for the thread's current device, recreated when that changes, destroyed with the thread
+// (mcs_estimate_dtn_batch runs estimate_both on short-lived worker threads).
+struct BothCtx {
+    cudaStream_t ss[2] = { nullptr, nullptr };
+    cudaEvent_t ev[3] = { nullptr, nullptr, nullptr };
+    int dev = -1;
+    void release()
+    {
+        if (dev < 0) return;
+        int cur = -1;
+        cudaGetDevice(&cur);
+        if (cur != dev) cudaSetDevice(dev);
+        for (auto& x : ss) { if (x) cudaStreamDestroy(x); x = nullptr; }
+        for (auto& x : ev) { if (x) cudaEventDestroy(x); x = nullptr; }
+        if (cur >= 0 && cur != dev) cudaSetDevice(cur);
+        dev = -1;
     }
-    return ss[which];
-}
+    bool ensure()
+    {
+        int cur = 0;
+        if (cudaGetDevice(&cur) != cudaSuccess) return false;
+        if (dev == cur) return true;
+        release();
+        int least = 0, greatest = 0;
+        if (cudaDeviceGetStreamPriorityRange(&least, &greatest) != cudaSuccess) return false;
+        bool ok = cudaStreamCreateWithPriority(&ss[0], cudaStreamNonBlocking, greatest) == cudaSuccess &&
+                  cudaStreamCreateWithPriority(&ss[1], cudaStreamNonBlocking, least) == cudaSuccess;
+        for (auto& x : ev) ok = ok && cudaEventCreateWithFlags(&x, cudaEventDisableTiming) == cudaSuccess;
+        dev = cur;
+        if (!ok) { release(); return false; }
+        return true;
+    }
+    ~BothCtx() { release(); }
+};
+thread_local BothCtx g_both;
 
 int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis,
                   const mcs_params* p_int, const mcs_params* p_ext, void* ws, size_t ws_bytes,
@@ -175,8 +196,8 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     if (s->n_s < 1) return MCS_EINVAL;
     if (out_int->kind == out_ext->kind && (out_int->kind == 0 ? out_int->dense == out_ext->dense : out_int->coo_val == out_ext->coo_val))
         return MCS_EINVAL;                            // the two operators run concurrently: separate outputs
-    cudaStream_t st = (cudaStream_t)stream, st1 = side_stream(0), st2 = side_stream(1);
-    if (!st1 || !st2) return MCS_ECUDA;
+    if (!g_both.ensure()) return MCS_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream, st1 = g_both.ss[0], st2 = g_both.ss[1];
 
     Layout L[2];
     for (int x = 0; x < 2; ++x) L[x] = make_layout(b, s, basis, pp[x], x, true, true);
@@ -184,12 +205,7 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     for (int x = 0; x < 2; ++x) if (hh[x]) hh[x]->workspace_needed = (int64_t)total;
     if (!ws || ws_bytes < total) return MCS_ENOMEM;
     char* base[2] = { (char*)ws, (char*)ws + L[0].total };
-    static thread_local cudaEvent_t ev_prep = nullptr, ev_done = nullptr, ev_done1 = nullptr;
-    if (!ev_prep) {
-        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_prep, cudaEventDisableTiming));
-        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
-        MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_done1, cudaEventDisableTiming));
-    }
+    cudaEvent_t ev_prep = g_both.ev[0], ev_done = g_both.ev[1], ev_done1 = g_both.ev[2];
     unsigned long long* stats_dev[2] = { nullptr, nullptr };
     WalkLaunch wl[2];
     mcs_prof_mark(MCS_MARK_BEGIN, st);
@@ -493,6 +509,109 @@ done:
     return fail(rc, stats_exterior);
 }
 
+// ---------------------------------------------------------------------------
+// Batch entry point (BASELINE config 4: "1024 seeded synthetic meshes ... interior and exterior DtN ... meshes/s end
+// to end"; ~450 k shapes, one shape after another per GPU).  A small mesh cannot keep the device busy: its
+// 0.5 M walks are over almost as soon as they start and most of the run is the tail of the longest walks, plus a
+// dozen small launches and the host read-backs of the build.  The batch call owns the schedule: `n_workers` host
+// threads, each with its own stream and workspace, take the meshes in turn (build, sidedness, both estimators into the
+// caller's dense outputs, free), so the device always has the bulk of some meshes next to the tails of others.  Every
+// mesh is computed exactly as by the single calls (fixed record slots, ordered accumulation): the results do not
+// depend on the number of workers or on the interleaving.
+// ---------------------------------------------------------------------------
+#include <thread>
+#include <vector>
+
+extern "C" int mcs_estimate_dtn_batch(mcs_batch_item* items, int64_t n_items, const mcs_params* p_int, const mcs_params* p_ext,
+                                      float orient_h_scale, float orient_beta, int32_t n_workers, void* stream)
+{
+    if (!items || n_items < 1 || !p_int || !p_ext) return MCS_EINVAL;
+    if (p_int->output_kind != 0 || p_ext->output_kind != 0) return MCS_EINVAL;      // dense [K][K] outputs
+    for (int64_t i = 0; i < n_items; ++i) {
+        const mcs_batch_item& it = items[i];
+        if (!it.verts || !it.faces || it.V < 1 || it.F < 1 || it.samples.n_s < 1 || !it.samples.tri || !it.samples.bary ||
+            !it.samples.weight || !it.out_interior || !it.out_exterior || it.out_interior == it.out_exterior) return MCS_EINVAL;
+        if (orient_h_scale > 0.0f && !it.normal_out) return MCS_EINVAL;
+        items[i].rc = MCS_OK;
+    }
+    int dev = 0;
+    MCS_CUDA_TRY(cudaGetDevice(&dev));
+    int nw = n_workers > 0 ? n_workers : 4;
+    if (nw > 16) nw = 16;
+    if ((int64_t)nw > n_items) nw = (int)n_items;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t ev_start = nullptr;
+    MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    MCS_CUDA_TRY(cudaEventRecord(ev_start, st));                 // the workers' streams start after what the caller has queued (uploads)
+    std::vector<cudaStream_t> ws(nw, nullptr);
+    std::vector<cudaEvent_t> ev_done(nw, nullptr);
+    std::vector<int> worker_rc(nw, MCS_OK);
+    for (int w = 0; w < nw; ++w) {
+        if (cudaStreamCreateWithFlags(&ws[w], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ev_done[w], cudaEventDisableTiming) != cudaSuccess) return MCS_ECUDA;
+        cudaStreamWaitEvent(ws[w], ev_start, 0);
+    }
+    auto work = [&](int w) {
+        cudaSetDevice(dev);
+        cudaStream_t s = ws[w];
+        void* d_ws = nullptr; size_t d_ws_bytes = 0;
+        for (int64_t i = w; i < n_items; i += nw) {
+            mcs_batch_item& it = items[i];
+            mcs_bvh* bvh = nullptr;
+            int rc = mcs_build_bvh(it.verts, it.V, it.faces, it.F, nullptr, s, &bvh);
+            if (rc == MCS_OK) {
+                mcs_samples smp = it.samples;
+                if (orient_h_scale > 0.0f) {
+                    if (orient_beta > 0.0f) rc = mcs_orient_samples_fast(bvh, &smp, orient_h_scale, orient_beta, it.normal_out, nullptr, s);
+                    else {
+                        const size_t wb = mcs_winding_workspace_bytes(bvh, smp.n_s);
+                        void* wws = nullptr;
+                        if (cudaMallocAsync(&wws, wb, s) != cudaSuccess) rc = MCS_ENOMEM;
+                        else { rc = mcs_orient_samples(bvh, &smp, orient_h_scale, it.normal_out, nullptr, wws, wb, s); cudaFreeAsync(wws, s); }
+                    }
+                    smp.normal = it.normal_out;
+                }
+                if (rc == MCS_OK) {
+                    mcs_params pi = *p_int, pe = *p_ext;
+                    for (int d = 0; d < 3; ++d) pe.kelvin_origin[d] = it.kelvin_origin[d];
+                    mcs_matrix mi, me;
+                    memset(&mi, 0, sizeof mi); memset(&me, 0, sizeof me);
+                    mi.kind = 0; mi.K = it.basis.K; mi.dense = it.out_interior;
+                    me.kind = 0; me.K = it.basis.K; me.dense = it.out_exterior;
+                    const size_t need = mcs_workspace_bytes_both(bvh, &smp, &it.basis, &pi, &pe);
+                    if (need == 0) rc = MCS_EINVAL;
+                    if (rc == MCS_OK && need > d_ws_bytes) {
+                        if (d_ws) cudaFreeAsync(d_ws, s);
+                        d_ws = nullptr; d_ws_bytes = 0;
+                        if (cudaMallocAsync(&d_ws, need + need / 4, s) != cudaSuccess) rc = MCS_ENOMEM; else d_ws_bytes = need + need / 4;
+                    }
+                    if (rc == MCS_OK)
+                        rc = estimate_both(bvh, &smp, &it.basis, &pi, &pe, d_ws, d_ws_bytes, &mi, &me, nullptr, nullptr, s);
+                }
+            }
+            if (bvh) mcs_free_bvh(bvh);
+            it.rc = rc;
+            if (rc != MCS_OK && worker_rc[w] == MCS_OK) worker_rc[w] = rc;
+        }
+        if (d_ws) cudaFreeAsync(d_ws, s);
+        cudaEventRecord(ev_done[w], s);
+    };
+    std::vector<std::thread> threads;
+    for (int w = 1; w < nw; ++w) threads.emplace_back(work, w);
+    work(0);
+    for (auto& t : threads) t.join();
+    int rc = MCS_OK;
+    for (int w = 0; w < nw; ++w) {
+        cudaStreamWaitEvent(st, ev_done[w], 0);                  // the caller's stream continues after every worker
+        if (worker_rc[w] != MCS_OK && rc == MCS_OK) rc = worker_rc[w];
+    }
+    cudaError_t e = cudaStreamSynchronize(st);                   // streams and events are destroyed below: wait for them
+    for (int w = 0; w < nw; ++w) { cudaStreamDestroy(ws[w]); cudaEventDestroy(ev_done[w]); }
+    cudaEventDestroy(ev_start);
+    if (rc == MCS_OK && e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
+    return rc;
+}
+
 extern "C" int mcs_tangent_balls(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
                                  float* balls, void* stream)
 {
@@ -611,6 +730,7 @@ extern "C" size_t mcs_abi_sizeof(int which)
         case 5: return sizeof(mcs_bvh_info_t);
         case 6: return sizeof(mcs_record);
         case 7: return sizeof(mcs_host_coo);
+        case 8: return sizeof(mcs_batch_item);
         default: return 0;
     }
 }

@@ -43,7 +43,7 @@ def test_binding_struct_sizes_match_header():
     lib = ctypes.CDLL(build())
     lib.mcs_abi_sizeof.restype = ctypes.c_size_t
     for which, cls in ((0, api._Samples), (1, api._Basis), (2, api._Params), (3, api._Matrix), (4, api.Stats), (5, api.BvhInfo),
-                       (7, api._HostCoo)):
+                       (7, api._HostCoo), (8, api._BatchItem)):
         assert lib.mcs_abi_sizeof(ctypes.c_int(which)) == ctypes.sizeof(cls), cls.__name__
 
 
