@@ -454,12 +454,34 @@ static void keep_pool_memory()
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
         unsigned long long keep = ~0ull;
         cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        // Memory freed on one stream may be handed to an allocation on another only when that free has COMPLETED
+        // (opportunistic reuse), never by making the allocating stream wait for it: with several meshes in flight on
+        // their own streams (mcs_estimate_dtn_batch) such inserted dependencies serialised the workers.
+        int off = 0;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolReuseAllowInternalDependencies, &off);
     }
 }
 
 void mcs_bvh_touch(const mcs_bvh* b, cudaStream_t st)
 {
     if (b && b->last_use) cudaEventRecord(b->last_use, st);
+}
+
+// Frees the handle's memory in the order of `st`, which must be a stream the handle's last use is ordered before
+// (the batch workers and the host entry points free on the stream they worked on: no detour through stream 0).
+void mcs_free_bvh_on(mcs_bvh* b, cudaStream_t st)
+{
+    if (!b) return;
+    int cur = 0;
+    cudaGetDevice(&cur);
+    if (cur != b->device) cudaSetDevice(b->device);
+    if (b->last_use) cudaStreamWaitEvent(st, b->last_use, 0);
+    void* ptrs[11] = { b->verts, b->faces, b->nodes, b->wide, b->tris, b->leaf_tri, b->face_slot, b->morton,
+                       b->wn_nodes, b->wn_order, b->wn_face_pos };
+    for (void* p : ptrs) if (p) cudaFreeAsync(p, st);
+    if (b->last_use) cudaEventDestroy(b->last_use);
+    if (cur != b->device) cudaSetDevice(cur);
+    delete b;
 }
 
 extern "C" void mcs_free_bvh(mcs_bvh* b)

@@ -512,21 +512,39 @@ done:
 // ---------------------------------------------------------------------------
 // Batch entry point (BASELINE config 4: "1024 seeded synthetic meshes ... interior and exterior DtN ... meshes/s end
 // to end"; ~450 k shapes, one shape after another per GPU).  A small mesh cannot keep the device busy: its
-// 0.5 M walks are over almost as soon as they start and most of the run is the tail of the longest walks, plus a
-// dozen small launches and the host read-backs of the build.  The batch call owns the schedule: `n_workers` host
-// threads, each with its own stream and workspace, take the meshes in turn (build, sidedness, both estimators into the
-// caller's dense outputs, free), so the device always has the bulk of some meshes next to the tails of others.  Every
-// mesh is computed exactly as by the single calls (fixed record slots, ordered accumulation): the results do not
-// depend on the number of workers or on the interleaving.
+// 0.5 M walks are over almost as soon as they start and 90 % of the run is the tail of its longest walks (a 400-jump
+// exterior walk is 10 000 dependent node visits).  Running several meshes' kernels side by side on worker streams does
+// not help much either (measured 1.4x for 4 streams: every warp of every kernel holds some long walk to the end, so the
+// block slots stay taken).  The batch call therefore owns the schedule (see the body): worker threads prepare the
+// meshes, ONE persistent launch walks them all, worker threads accumulate.  Every mesh is computed exactly as by the
+// single calls (fixed record slots, ordered accumulation): the results do not depend on the workers or the grouping.
 // ---------------------------------------------------------------------------
+#include <stdlib.h>
 #include <thread>
 #include <vector>
+
+namespace {
+
+struct BatchMeshState {                     // one item between the phases of the single-launch batch path
+    mcs_bvh* bvh = nullptr;
+    mcs_samples smp;
+    mcs_params p[2];
+    Layout L[2];
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    WalkLaunch wl[2];
+    unsigned long long* stats_dev[2] = { nullptr, nullptr };
+    int rc = MCS_OK;
+};
+
+}  // namespace
 
 extern "C" int mcs_estimate_dtn_batch(mcs_batch_item* items, int64_t n_items, const mcs_params* p_int, const mcs_params* p_ext,
                                       float orient_h_scale, float orient_beta, int32_t n_workers, void* stream)
 {
     if (!items || n_items < 1 || !p_int || !p_ext) return MCS_EINVAL;
     if (p_int->output_kind != 0 || p_ext->output_kind != 0) return MCS_EINVAL;      // dense [K][K] outputs
+    if (p_ext->exterior_query != 0) return MCS_EINVAL;                              // the batched launch runs the E3 query
     for (int64_t i = 0; i < n_items; ++i) {
         const mcs_batch_item& it = items[i];
         if (!it.verts || !it.faces || it.V < 1 || it.F < 1 || it.samples.n_s < 1 || !it.samples.tri || !it.samples.bary ||
@@ -540,76 +558,123 @@ extern "C" int mcs_estimate_dtn_batch(mcs_batch_item* items, int64_t n_items, co
     if (nw > 16) nw = 16;
     if ((int64_t)nw > n_items) nw = (int)n_items;
     cudaStream_t st = (cudaStream_t)stream;
-    cudaEvent_t ev_start = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_walk = nullptr;
     MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    MCS_CUDA_TRY(cudaEventCreateWithFlags(&ev_walk, cudaEventDisableTiming));
     MCS_CUDA_TRY(cudaEventRecord(ev_start, st));                 // the workers' streams start after what the caller has queued (uploads)
     std::vector<cudaStream_t> ws(nw, nullptr);
     std::vector<cudaEvent_t> ev_done(nw, nullptr);
-    std::vector<int> worker_rc(nw, MCS_OK);
     for (int w = 0; w < nw; ++w) {
         if (cudaStreamCreateWithFlags(&ws[w], cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&ev_done[w], cudaEventDisableTiming) != cudaSuccess) return MCS_ECUDA;
         cudaStreamWaitEvent(ws[w], ev_start, 0);
     }
-    auto work = [&](int w) {
-        cudaSetDevice(dev);
-        cudaStream_t s = ws[w];
-        void* d_ws = nullptr; size_t d_ws_bytes = 0;
-        for (int64_t i = w; i < n_items; i += nw) {
-            mcs_batch_item& it = items[i];
-            mcs_bvh* bvh = nullptr;
-            int rc = mcs_build_bvh(it.verts, it.V, it.faces, it.F, nullptr, s, &bvh);
-            if (rc == MCS_OK) {
-                mcs_samples smp = it.samples;
-                if (orient_h_scale > 0.0f) {
-                    if (orient_beta > 0.0f) rc = mcs_orient_samples_fast(bvh, &smp, orient_h_scale, orient_beta, it.normal_out, nullptr, s);
+    int rc_all = MCS_OK;
+    // Groups of at most GROUP meshes: within a group (1) the workers build the trees, decide the sides and prepare the
+    // walks of their meshes (tangent balls, Z-order), (2) ONE persistent launch runs the walks of both operators of all
+    // the group's meshes -- a small mesh alone leaves the device in the tail of its longest walks almost from the
+    // start; together the meshes are one job of the size the throughput kernel is made for -- and (3) the workers
+    // accumulate their meshes' records into the caller's matrices and free the trees.
+    const int64_t GROUP = 64;
+    void* batch_scratch = nullptr;
+    const size_t batch_scratch_bytes = walk_batch_scratch_bytes((int)(2 * (n_items < GROUP ? n_items : GROUP)));
+    if (cudaMallocAsync(&batch_scratch, batch_scratch_bytes, st) != cudaSuccess) return MCS_ENOMEM;
+    for (int64_t g0 = 0; g0 < n_items; g0 += GROUP) {
+        const int64_t gn = (n_items - g0) < GROUP ? (n_items - g0) : GROUP;
+        std::vector<BatchMeshState> state((size_t)gn);
+        auto phase1 = [&](int w) {
+            cudaSetDevice(dev);
+            cudaStream_t s = ws[w];
+            for (int64_t k = w; k < gn; k += nw) {
+                mcs_batch_item& it = items[g0 + k];
+                BatchMeshState& M = state[(size_t)k];
+                int rc = mcs_build_bvh(it.verts, it.V, it.faces, it.F, nullptr, s, &M.bvh);
+                M.smp = it.samples;
+                if (rc == MCS_OK && orient_h_scale > 0.0f) {
+                    if (orient_beta > 0.0f) rc = mcs_orient_samples_fast(M.bvh, &M.smp, orient_h_scale, orient_beta, it.normal_out, nullptr, s);
                     else {
-                        const size_t wb = mcs_winding_workspace_bytes(bvh, smp.n_s);
+                        const size_t wb = mcs_winding_workspace_bytes(M.bvh, M.smp.n_s);
                         void* wws = nullptr;
                         if (cudaMallocAsync(&wws, wb, s) != cudaSuccess) rc = MCS_ENOMEM;
-                        else { rc = mcs_orient_samples(bvh, &smp, orient_h_scale, it.normal_out, nullptr, wws, wb, s); cudaFreeAsync(wws, s); }
+                        else { rc = mcs_orient_samples(M.bvh, &M.smp, orient_h_scale, it.normal_out, nullptr, wws, wb, s); cudaFreeAsync(wws, s); }
                     }
-                    smp.normal = it.normal_out;
+                    M.smp.normal = it.normal_out;
                 }
                 if (rc == MCS_OK) {
-                    mcs_params pi = *p_int, pe = *p_ext;
-                    for (int d = 0; d < 3; ++d) pe.kelvin_origin[d] = it.kelvin_origin[d];
-                    mcs_matrix mi, me;
-                    memset(&mi, 0, sizeof mi); memset(&me, 0, sizeof me);
-                    mi.kind = 0; mi.K = it.basis.K; mi.dense = it.out_interior;
-                    me.kind = 0; me.K = it.basis.K; me.dense = it.out_exterior;
-                    const size_t need = mcs_workspace_bytes_both(bvh, &smp, &it.basis, &pi, &pe);
-                    if (need == 0) rc = MCS_EINVAL;
-                    if (rc == MCS_OK && need > d_ws_bytes) {
-                        if (d_ws) cudaFreeAsync(d_ws, s);
-                        d_ws = nullptr; d_ws_bytes = 0;
-                        if (cudaMallocAsync(&d_ws, need + need / 4, s) != cudaSuccess) rc = MCS_ENOMEM; else d_ws_bytes = need + need / 4;
-                    }
-                    if (rc == MCS_OK)
-                        rc = estimate_both(bvh, &smp, &it.basis, &pi, &pe, d_ws, d_ws_bytes, &mi, &me, nullptr, nullptr, s);
+                    M.p[0] = *p_int; M.p[1] = *p_ext;
+                    for (int d = 0; d < 3; ++d) M.p[1].kelvin_origin[d] = it.kelvin_origin[d];
+                    if (M.p[0].walks_per_sample < 1 || M.p[1].walks_per_sample < 1) rc = MCS_EINVAL;
                 }
+                if (rc == MCS_OK) {
+                    for (int x = 0; x < 2; ++x) M.L[x] = make_layout(M.bvh, &M.smp, &it.basis, &M.p[x], x, true, true);
+                    M.ws_bytes = M.L[0].total + M.L[1].total;
+                    if (cudaMallocAsync((void**)&M.ws, M.ws_bytes, s) != cudaSuccess) rc = MCS_ENOMEM;
+                }
+                for (int x = 1; x >= 0 && rc == MCS_OK; --x) {
+                    char* base = M.ws + (x ? M.L[0].total : 0);
+                    rc = walk_run(M.bvh, &M.smp, &M.p[x], x, base + M.L[x].walk_off, align_up(walk_workspace_bytes(&M.smp)),
+                                  (float4*)(base + M.L[x].records_off), nullptr, false, nullptr, false, &M.stats_dev[x], s, &M.wl[x]);
+                }
+                M.rc = rc;
             }
-            if (bvh) mcs_free_bvh(bvh);
-            it.rc = rc;
-            if (rc != MCS_OK && worker_rc[w] == MCS_OK) worker_rc[w] = rc;
+            cudaEventRecord(ev_done[w], s);
+        };
+        {
+            std::vector<std::thread> threads;
+            for (int w = 1; w < nw; ++w) threads.emplace_back(phase1, w);
+            phase1(0);
+            for (auto& t : threads) t.join();
         }
-        if (d_ws) cudaFreeAsync(d_ws, s);
-        cudaEventRecord(ev_done[w], s);
-    };
-    std::vector<std::thread> threads;
-    for (int w = 1; w < nw; ++w) threads.emplace_back(work, w);
-    work(0);
-    for (auto& t : threads) t.join();
-    int rc = MCS_OK;
-    for (int w = 0; w < nw; ++w) {
-        cudaStreamWaitEvent(st, ev_done[w], 0);                  // the caller's stream continues after every worker
-        if (worker_rc[w] != MCS_OK && rc == MCS_OK) rc = worker_rc[w];
+        // (2) one launch for the walks of every mesh that got this far
+        std::vector<WalkLaunch> launches; std::vector<int> ext, far;
+        for (int64_t k = 0; k < gn; ++k) {
+            const BatchMeshState& M = state[(size_t)k];
+            if (M.rc != MCS_OK) continue;
+            for (int x = 0; x < 2; ++x) { launches.push_back(M.wl[x]); ext.push_back(x); far.push_back(M.p[x].far_alpha > 0.0f ? 1 : 0); }
+        }
+        for (int w = 0; w < nw; ++w) cudaStreamWaitEvent(st, ev_done[w], 0);
+        int rc2 = MCS_OK;
+        if (!launches.empty())
+            rc2 = walk_launch_batch(launches.data(), ext.data(), far.data(), (int)launches.size(), batch_scratch, batch_scratch_bytes, st);
+        cudaEventRecord(ev_walk, st);
+        // (3) accumulation per mesh on the workers' streams
+        auto phase3 = [&](int w) {
+            cudaSetDevice(dev);
+            cudaStream_t s = ws[w];
+            cudaStreamWaitEvent(s, ev_walk, 0);
+            for (int64_t k = w; k < gn; k += nw) {
+                mcs_batch_item& it = items[g0 + k];
+                BatchMeshState& M = state[(size_t)k];
+                int rc = M.rc != MCS_OK ? M.rc : rc2;
+                for (int x = 0; x < 2 && rc == MCS_OK; ++x) {
+                    char* base = M.ws + (x ? M.L[0].total : 0);
+                    mcs_matrix m; memset(&m, 0, sizeof m);
+                    m.kind = 0; m.K = it.basis.K; m.dense = x ? it.out_exterior : it.out_interior;
+                    rc = acc_run(M.bvh, &M.smp, &it.basis, &M.p[x], (const float4*)(base + M.L[x].records_off), M.L[x].n_records,
+                                 base + M.L[x].acc_off, align_up(acc_ws_bytes(M.bvh, &M.smp, &it.basis, &M.p[x], M.L[x].n_records)),
+                                 &m, M.stats_dev[x], s);
+                }
+                if (M.bvh) { mcs_bvh_touch(M.bvh, s); mcs_free_bvh_on(M.bvh, s); M.bvh = nullptr; }
+                if (M.ws) { cudaFreeAsync(M.ws, s); M.ws = nullptr; }
+                it.rc = rc;
+            }
+            cudaEventRecord(ev_done[w], s);
+        };
+        {
+            std::vector<std::thread> threads;
+            for (int w = 1; w < nw; ++w) threads.emplace_back(phase3, w);
+            phase3(0);
+            for (auto& t : threads) t.join();
+        }
+        for (int w = 0; w < nw; ++w) cudaStreamWaitEvent(st, ev_done[w], 0);
+        for (int64_t k = 0; k < gn; ++k) if (items[g0 + k].rc != MCS_OK && rc_all == MCS_OK) rc_all = items[g0 + k].rc;
     }
+    cudaFreeAsync(batch_scratch, st);
     cudaError_t e = cudaStreamSynchronize(st);                   // streams and events are destroyed below: wait for them
-    for (int w = 0; w < nw; ++w) { cudaStreamDestroy(ws[w]); cudaEventDestroy(ev_done[w]); }
-    cudaEventDestroy(ev_start);
-    if (rc == MCS_OK && e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc = MCS_ECUDA; }
-    return rc;
+    for (int w = 0; w < nw; ++w) { cudaStreamSynchronize(ws[w]); cudaStreamDestroy(ws[w]); cudaEventDestroy(ev_done[w]); }
+    cudaEventDestroy(ev_start); cudaEventDestroy(ev_walk);
+    if (rc_all == MCS_OK && e != cudaSuccess) { mcs_set_last_cuda_error((int)e); rc_all = MCS_ECUDA; }
+    return rc_all;
 }
 
 extern "C" int mcs_tangent_balls(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,

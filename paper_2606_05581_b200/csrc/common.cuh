@@ -97,6 +97,7 @@ struct mcs_bvh {
 
 // Every entry point that enqueues work reading the tree calls this with its stream when it is done enqueuing.
 void mcs_bvh_touch(const mcs_bvh* b, cudaStream_t st);
+void mcs_free_bvh_on(mcs_bvh* b, cudaStream_t st);
 
 // ---------------------------------------------------------------------------
 // radix sort / scan (sort.cu)

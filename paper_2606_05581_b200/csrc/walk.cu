@@ -14,6 +14,8 @@
 #include "walk.cuh"
 
 #include <limits.h>
+#include <stdlib.h>
+#include <vector>
 
 namespace {
 
@@ -369,23 +371,25 @@ constexpr int CUR_NONE = INT_MIN;
 #endif
 
 struct LaneStack {
-    int*   s_ref;      // shared: [WSTACK][WT], this lane's column
+    int*   s_ref;      // shared: [WSTACK][block threads], this lane's column
     float* s_d;
     int    l_ref[MCS_STACK - WSTACK];            // local-memory spill
     float  l_d[MCS_STACK - WSTACK];
 };
 
+template <int TW>
 __device__ __forceinline__ void stack_push(LaneStack& st, int& sp, int ref, float d)
 {
-    if (sp < WSTACK) { st.s_ref[sp * WT] = ref; st.s_d[sp * WT] = d; }
+    if (sp < WSTACK) { st.s_ref[sp * TW] = ref; st.s_d[sp * TW] = d; }
     else if (sp < MCS_STACK) { st.l_ref[sp - WSTACK] = ref; st.l_d[sp - WSTACK] = d; }
     ++sp;                                        // sp > MCS_STACK cannot happen: depth <= 63 + log2(F)
 }
 
+template <int TW>
 __device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, float& d)
 {
     --sp;
-    if (sp < WSTACK) { ref = st.s_ref[sp * WT]; d = st.s_d[sp * WT]; }
+    if (sp < WSTACK) { ref = st.s_ref[sp * TW]; d = st.s_d[sp * TW]; }
     else { ref = st.l_ref[sp - WSTACK]; d = st.l_d[sp - WSTACK]; }
 }
 
@@ -428,7 +432,7 @@ struct CoopState {
     unsigned n_nodes, n_tris, q_nodes;       // increments (COUNT builds)
 };
 
-template <bool COUNT, bool FAR>
+template <bool COUNT, bool FAR, int TW>
 __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, const WideNode* __restrict__ wide,
                                                const PackedTri* __restrict__ tris, int L, float mesh_scale,
                                                int* __restrict__ co_nodes, int* __restrict__ co_leaves,
@@ -462,7 +466,7 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
         while (sp > 0) {
             int ref; float d;
             --sp;
-            if (sp < WSTACK) { ref = s_ref[sp * WT]; d = s_d[sp * WT]; }
+            if (sp < WSTACK) { ref = s_ref[sp * TW]; d = s_d[sp * TW]; }
             else { ref = l_ref[sp - WSTACK]; d = l_d[sp - WSTACK]; }
             if (d <= lim) { if (ref >= 0) co_nodes[ncount++] = ref; else co_leaves[lcount++] = ~ref; }
         }
@@ -578,368 +582,35 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 // The traversal runs on the SAME primal tree: a box is bounded below by box_ratio2, a face is tested by
 // inverted_ratio2_triangle; h.d2 holds the best squared ratio, the radius in Kelvin coordinates is ratio / |x - o|.
 // Lane path only (no cooperative take-over, no merged passes, no far-field cut): a cross-check variant.
-template <bool EXT, bool COUNT, bool COOP, bool MERGED, bool FAR, bool KEX = false>
-__global__ void __launch_bounds__(WT, MERGED ? 4 : (COOP ? WALK_COOP_BLOCKS : (KEX ? 6 : WALK_MIN_BLOCKS)))      // small jobs: registers instead of occupancy
-walk_kernel(WalkGeom g, WalkArgs a)
-{
-    __shared__ int   sh_ref[WSTACK * WT];
-    __shared__ float sh_d[WSTACK * WT];
-    // warp lists of the cooperative path: global scratch (L2-resident, used by monster queries only); shared
-    // memory here would take 10 KB per block away from the L1 that serves every node read
-    int* const co_nodes = a.coop_scratch + ((size_t)blockIdx.x * (WT / 32) + (threadIdx.x >> 5)) * (COOP_NCAP + COOP_LCAP);
-    int* const co_leaves = co_nodes + COOP_NCAP;
-    const unsigned FULL = 0xFFFFFFFFu;
-    const int lane = threadIdx.x & 31;
-    const unsigned lt = (1u << lane) - 1u;
-    const long long total = a.n_s * a.W + a.n_kill;
-    const long long n_main = a.n_s * a.W;
-    const uint2 key = make_uint2(a.key0, a.key1);
-    const float3 o = f3(a.ox, a.oy, a.oz);
-
-    LaneStack stk;
-    stk.s_ref = sh_ref + threadIdx.x;
-    stk.s_d = sh_d + threadIdx.x;
-
-    long long chunk_cur = 0, chunk_end = 0;      // warp-uniform
-    bool exhausted = false;                      // warp-uniform
-    // walk state
-    bool busy = false;                           // lane owns a walk
-    float3 x = f3(0.f, 0.f, 0.f);                // interior: position; exterior: Kelvin coordinates y
-    float wfac = 0.f;
-    unsigned sample = 0, walk = 0;
-    int k = 0, prev = -1;
-    long long slot = 0;
-    // query state
-    float3 xq = f3(0.f, 0.f, 0.f);
-    float rho = 0.f, far_radius = -1.0f;         // far_radius >= 0: jump radius known without a query (exterior far field)
-    ClosestHit h; h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.f;
-    float lim = 3.0e38f;
-    float lb2 = CUDART_INF_F, dnear2 = 0.0f;     // FAR: smallest box distance of the sub-trees taken as a whole; near threshold
-    int cur = CUR_NONE, sp = 0;
-    // statistics
-    unsigned n_nodes = 0, n_tris = 0, q_nodes = 0, n_far = 0;
-    int q_visits = 0;                            // nodes visited by the current query (hand-over to the warp at COOP_MIN)
-    unsigned n_steps = 0, n_queries = 0, n_trunc = 0;
-    int age_tri = 0, age_trans = 0;              // warp-uniform: passes since the kind last ran (or was last unwanted)
-
-    for (;;) {
-        // ---- next item of every lane that has none --------------------------------
-        if (busy && cur == CUR_NONE) {
-            while (sp > 0) {
-                int ref; float d;
-                stack_pop(stk, sp, ref, d);
-                if (d <= lim) { cur = ref; break; }
-            }
-        }
-        const int kind = busy ? (cur == CUR_NONE ? KIND_TRANS : (cur >= 0 ? KIND_NODE : KIND_TRI))
-                              : (exhausted ? KIND_IDLE : KIND_TRANS);
-        // Which kind runs this pass: NODE while at least VOTE_NODE lanes want it (one ballot), else TRI when
-        // at least VOTE_TRI lanes wait, else TRANS (the long pass: Philox, sincos, record, refill) when at least
-        // VOTE_TRANS lanes wait; otherwise the kind most lanes wait for.  Draining one kind lets the others fill.
-        // Aging keeps the wait bounded: a kind that has not run for VOTE_AGE passes runs next if any lane wants it
-        // (a few lanes inside thousand-node queries must not park the rest of the warp).
-        const unsigned m_node = __ballot_sync(FULL, MERGED ? (kind == KIND_NODE || kind == KIND_TRI) : kind == KIND_NODE);
-        int which = KIND_NODE;
-        ++age_tri; ++age_trans;
-        bool run_trav, run_trans;
-        if (MERGED) {
-            // every lane advances every pass: traversal items first, then the transitions
-            const unsigned m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
-            if ((m_node | m_trans) == 0) break;
-            run_trav = m_node != 0; run_trans = m_trans != 0;
-        } else if (__popc(m_node) < VOTE_NODE || age_tri >= VOTE_AGE || age_trans >= VOTE_AGE) {
-            const unsigned m_tri = __ballot_sync(FULL, kind == KIND_TRI), m_trans = __ballot_sync(FULL, kind == KIND_TRANS);
-            if ((m_node | m_tri | m_trans) == 0) break;
-            const int nn = __popc(m_node), nt = __popc(m_tri), nx = __popc(m_trans);
-            if (nx > 0 && age_trans >= VOTE_AGE) which = KIND_TRANS;
-            else if (nt > 0 && age_tri >= VOTE_AGE) which = KIND_TRI;
-            else if (nn >= VOTE_NODE) which = KIND_NODE;
-            else if (nt >= VOTE_TRI) which = KIND_TRI;
-            else if (nx >= VOTE_TRANS) which = KIND_TRANS;
-            else which = (nx > nn && nx > nt) ? KIND_TRANS : (nt > nn ? KIND_TRI : KIND_NODE);
-            if (nt == 0) age_tri = 0;
-            if (nx == 0) age_trans = 0;
-        }
-        if (which == KIND_TRI) age_tri = 0;
-        if (which == KIND_TRANS) age_trans = 0;
-        if (!MERGED) { run_trav = which == KIND_NODE; run_trans = which == KIND_TRANS; }
-
-        if (run_trav) {
-            const bool tri_lane = MERGED && kind == KIND_TRI;
-            if (kind == KIND_NODE || tri_lane) {
-                // 4-wide node: four box tests; the nearest surviving child is visited next, the others go on the stack
-                const char* wn = tri_lane ? reinterpret_cast<const char*>(g.tris + ~cur) : reinterpret_cast<const char*>(g.wide + cur);
-                const Vec8 q0 = ldg256(wn), q1 = ldg256(wn + 32);
-                Vec8 q2 = q0, q3 = q0;
-                if (!tri_lane) { q2 = ldg256(wn + 64); q3 = ldg256(wn + 96); }
-              if (tri_lane) {
-                const TriData T = unpack_tri(q0.lo, q0.hi, q1.lo, q1.hi);
-                float tv = 0.0f, tw = 0.0f;
-                const float td2 = closest_point_triangle(xq, T, CUDART_INF_F, tv, tw);
-                if (td2 < h.d2 || (td2 == h.d2 && T.orig < h.tri)) { h.d2 = td2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
-                if (COUNT) ++n_tris;
-                lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);
-                cur = CUR_NONE;
-              } else {
-                if (COUNT) { ++n_nodes; ++q_nodes; }
-                if (COOP) ++q_visits;
-                float d0, d1, d2, d3;
-                if (KEX) {
-                    d0 = box_ratio2(xq, o, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
-                    d1 = box_ratio2(xq, o, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
-                    d2 = box_ratio2(xq, o, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
-                    d3 = box_ratio2(xq, o, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
-                } else {
-                    d0 = box_dist2(xq, q0.lo.x, q0.lo.y, q0.lo.z, q0.lo.w, q0.hi.x, q0.hi.y);
-                    d1 = box_dist2(xq, q0.hi.z, q0.hi.w, q1.lo.x, q1.lo.y, q1.lo.z, q1.lo.w);
-                    d2 = box_dist2(xq, q1.hi.x, q1.hi.y, q1.hi.z, q1.hi.w, q2.lo.x, q2.lo.y);
-                    d3 = box_dist2(xq, q2.lo.z, q2.lo.w, q2.hi.x, q2.hi.y, q2.hi.z, q2.hi.w);
-                }
-                int c0 = __float_as_int(q3.lo.x), c1 = __float_as_int(q3.lo.y), c2 = __float_as_int(q3.lo.z), c3 = __float_as_int(q3.lo.w);
-                if (FAR) {
-                    // q3.hi = squared diagonals of the four child boxes (+inf for an empty slot, so it never qualifies)
-                    bool any = false;
-                    if (d0 >= dnear2 && d0 <= lim && q3.hi.x <= a.far_alpha2 * d0) { lb2 = fminf(lb2, d0); d0 = CUDART_INF_F; any = true; }
-                    if (d1 >= dnear2 && d1 <= lim && q3.hi.y <= a.far_alpha2 * d1) { lb2 = fminf(lb2, d1); d1 = CUDART_INF_F; any = true; }
-                    if (d2 >= dnear2 && d2 <= lim && q3.hi.z <= a.far_alpha2 * d2) { lb2 = fminf(lb2, d2); d2 = CUDART_INF_F; any = true; }
-                    if (d3 >= dnear2 && d3 <= lim && q3.hi.w <= a.far_alpha2 * d3) { lb2 = fminf(lb2, d3); d3 = CUDART_INF_F; any = true; }
-                    if (any) lim = fminf(lim, prune_limit(lb2, xq, a.mesh_scale));
-                }
-                // partial sorting network on (distance, child): (0,1)(2,3)(0,2) puts the nearest child first; the other
-                // three go on the stack as they are (the full network, two more comparators, visits 0.15 % fewer nodes
-                // and costs 1.5 % more time); empty slots have d = +inf
-#define MCS_CSWAP(da, ca, db, cb) { const bool s_ = db < da; const float td_ = s_ ? da : db; const int tc_ = s_ ? ca : cb; \
-                                    da = s_ ? db : da; ca = s_ ? cb : ca; db = td_; cb = tc_; }
-                MCS_CSWAP(d0, c0, d1, c1) MCS_CSWAP(d2, c2, d3, c3) MCS_CSWAP(d0, c0, d2, c2)
-#undef MCS_CSWAP
-                if (d3 <= lim) stack_push(stk, sp, c3, d3);
-                if (d2 <= lim) stack_push(stk, sp, c2, d2);
-                if (d1 <= lim) stack_push(stk, sp, c1, d1);
-                cur = d0 <= lim ? c0 : CUR_NONE;
-              }
-            }
-            // a lane whose query keeps going hands it to the warp (one query per pass)
-            const unsigned heavy = COOP ? __ballot_sync(FULL, kind == KIND_NODE && q_visits >= (MERGED ? COOP_MIN_MERGED : COOP_MIN)) : 0u;
-            if (COOP && heavy) {
-                const int L = __ffs(heavy) - 1;
-                CoopState cs;
-                cs.xq = xq; cs.h = h; cs.lim = lim; cs.sp = sp; cs.cur = cur; cs.n_nodes = 0; cs.n_tris = 0; cs.q_nodes = 0;
-                cs.lb2 = lb2; cs.dnear2 = dnear2; cs.alpha2 = a.far_alpha2;
-                coop_finish_query<COUNT, FAR>(g.nodes, g.wide, g.tris, L, a.mesh_scale, co_nodes, co_leaves,
-                                              stk.s_ref, stk.s_d, stk.l_ref, stk.l_d, &cs);
-                if (lane == L) { h = cs.h; lim = cs.lim; sp = cs.sp; cur = cs.cur; q_visits = 0; if (FAR) lb2 = cs.lb2; }
-                if (COUNT) { n_nodes += cs.n_nodes; n_tris += cs.n_tris; q_nodes += cs.q_nodes; }
-            }
-        }
-        if (!MERGED && which == KIND_TRI) {
-            if (kind == KIND_TRI) {
-                if (KEX) {
-                    const TriData T = load_tri(g.tris, ~cur);
-                    float tv = 0.0f, tw = 0.0f;
-                    const float r2 = inverted_ratio2_triangle(xq - o, T.a - o, T.b - o, T.c - o, T.n, T.nn, T.degenerate, tv, tw);
-                    if (r2 < h.d2 || (r2 == h.d2 && T.orig < h.tri)) { h.d2 = r2; h.tri = T.orig; h.k = ~cur; h.v = tv; h.w = tw; }
-                    lim = fminf(fmaf(h.d2, 4e-4f, h.d2) + 1e-14f, 3.0e38f);            // relative margin: lane path only, so the order is fixed
-                } else {
-                    test_triangle(g.tris, ~cur, xq, h, lim);
-                    lim = prune_limit(FAR ? fminf(h.d2, lb2) : h.d2, xq, a.mesh_scale);   // finite: an empty slot (box distance +inf) never passes
-                }
-                if (COUNT) ++n_tris;
-                cur = CUR_NONE;
-            }
-        }
-        if (run_trans) {
-            // ---- (1) finished queries: terminate or jump (R9) ----
-            bool start_query = false;
-            if (busy && kind == KIND_TRANS) {
-                float radius;
-                bool done = false;
-                if (far_radius >= 0.0f) {
-                    radius = far_radius;
-                } else {
-                    ++n_queries;
-                    if (COUNT) { atomicAdd(&a.stats[ST_HIST + (q_nodes > 0 ? min(31 - __clz(q_nodes), 15) : 0)], 1ull); q_nodes = 0; }
-                    prev = h.k;
-                    // FAR: the minimum over the cut is a box, not a face: jump with the lower bound, no shell test
-                    const bool far_hit = FAR && lb2 < h.d2;
-                    if (FAR && COUNT && far_hit) ++n_far;
-                    float D = sqrtf(far_hit ? lb2 : h.d2);
-                    if (KEX) {
-                        // D is the ratio |x - p| / |p - o| at its minimiser p: the exact distance to the inverted surface is
-                        // ratio / rho.  The primal distance to p is kept for the R10c test below.
-                        radius = D / rho;
-                        const float3 dp = hit_point(g.tris, h) - xq;
-                        D = sqrtf(dot3(dp, dp));
-                        h.d2 = D * D;
-                    } else {
-                        if (FAR) h.d2 = D * D;                    // the rules below read the distance from h.d2
-                        radius = EXT ? D / (rho * fminf(a.Rmax, rho + D)) : D;
-                    }
-                    if (!far_hit && radius < a.eps) {
-                        float wgt = wfac;
-                        if (EXT) {
-                            const float3 t = hit_point(g.tris, h) - o;
-                            wgt *= sqrtf(dot3(t, t));                    // 1/|t*| = |t - o|, Eq. 32
-                        }
-                        a.records[slot] = make_float4(__int_as_float(h.tri), h.v, h.w, wgt);
-                        if (a.steps) a.steps[slot] = k;
-                        done = true;
-                    }
-                }
-                // left the bounding box (R10b) / inside the solid that holds the inversion centre: the empty
-                // ball about the query point contains the centre, D > |x - o| = rho (R10c)
-                if (!done && (EXT ? (far_radius < 0.0f && sqrtf(h.d2) > rho) : radius > a.escape)) {
-                    a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                    if (a.steps) a.steps[slot] = -3;
-                    ++n_trunc;
-                    done = true;
-                }
-                if (!done) {
-                    if (k == a.max_steps) {                              // DESIGN.md R10
-                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                        if (a.steps) a.steps[slot] = -1;
-                        ++n_trunc;
-                        done = true;
-                    } else {
-                        ++k; ++n_steps;
-                        const uint4 rn = philox4x32_10(make_uint4(sample, walk, (unsigned)k, MCS_PURPOSE_STEP), key);
-                        const float ct = 1.0f - 2.0f * u01(rn.x);
-                        const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-                        float sphi, cphi;
-                        sincospif(2.0f * u01(rn.y), &sphi, &cphi);
-                        x = f3(fmaf(radius, st * cphi, x.x), fmaf(radius, st * sphi, x.y), fmaf(radius, ct, x.z));
-                        start_query = true;
-                    }
-                }
-                if (done) busy = false;
-            }
-            // ---- (2) refill idle lanes from the warp's chunk of the work queue ------------
-            unsigned idle = __ballot_sync(FULL, !busy);
-            while (idle != 0 && !exhausted) {
-                if (chunk_cur >= chunk_end) {
-                    long long base = 0;
-                    if (lane == 0) base = (long long)atomicAdd(a.work_counter, (unsigned long long)a.chunk);
-                    base = __shfl_sync(FULL, base, 0);
-                    if (base >= total) { exhausted = true; break; }
-                    chunk_cur = base;
-                    chunk_end = base + a.chunk < total ? base + a.chunk : total;
-                }
-                const int avail = (int)(chunk_end - chunk_cur);
-                const int n_idle = __popc(idle);
-                const int rank = __popc(idle & lt);
-                if (!busy && rank < avail) {
-                    const long long j = chunk_cur + rank;
-                    busy = true; k = 0; prev = -1; start_query = true;
-                    if (j < n_main) {
-                        const long long pos = j / a.W;
-                        walk = (unsigned)(j - pos * a.W);
-                        sample = a.order[pos];
-                        slot = (long long)sample * a.W + walk;
-                        const float4 b0 = __ldg(&a.balls[2 * (long long)sample]);
-                        const float4 b1 = __ldg(&a.balls[2 * (long long)sample + 1]);
-                        const float r = b0.w;
-                        if (!(r > 0.0f)) {                               // discarded sample
-                            a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                            if (a.steps) a.steps[slot] = -2;
-                            busy = false; start_query = false;
-                        } else if (a.naive) {                            // Alg. 1: start at the inset point, weight a_i / (W eps)
-                            x = f3(b0.x, b0.y, b0.z);
-                            wfac = (__ldg(&a.weight[sample]) / (float)a.W) * a.inv_inset;
-                            prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
-                        } else {
-                            // SampleBallSurface + BallJumpKernel (Eq. 23; R5-R7)
-                            const unsigned wq = a.antithetic ? (walk >> 1) : walk;
-                            const uint4 rn = philox4x32_10(make_uint4(sample, wq, 0u, MCS_PURPOSE_INIT), key);
-                            const float u1 = u01(rn.x), u2 = u01(rn.y);
-                            float q, factor;
-                            if (a.importance) {
-                                q = 1.0f / (a.inv_q0 - u1 * (a.inv_q0 - 1.0f));
-                                factor = (1.0f / (4.0f * r)) * (a.inv_q0 - 1.0f);
-                            } else {
-                                q = sqrtf(u1);
-                                factor = (q < a.q0) ? 0.0f : 1.0f / (8.0f * r * q * q * q);
-                            }
-                            const float ct = 1.0f - 2.0f * q * q;
-                            const float st = 2.0f * q * sqrtf(fmaxf(0.0f, 1.0f - q * q));
-                            float sphi, cphi;
-                            sincospif(2.0f * u2 + ((a.antithetic && (walk & 1u)) ? 1.0f : 0.0f), &sphi, &cphi);
-                            const float3 pole = f3(b1.x, b1.y, b1.z);
-                            float3 e1, e2;
-                            frame_from_normal(pole, e1, e2);
-                            x = f3(b0.x + r * (ct * pole.x + st * (cphi * e1.x + sphi * e2.x)),
-                                   b0.y + r * (ct * pole.y + st * (cphi * e1.y + sphi * e2.y)),
-                                   b0.z + r * (ct * pole.z + st * (cphi * e1.z + sphi * e2.z)));
-                            wfac = (__ldg(&a.weight[sample]) / (float)a.W) * factor;
-                            if (EXT) wfac *= b1.w * b1.w * b1.w;          // |s*|^3, Eq. 32
-                            prev = a.sample_slot ? __ldg(&a.sample_slot[sample]) : -1;
-                        }
-                    } else {                                             // killing walk from kappa(inf) = 0
-                        sample = MCS_KILLING_SAMPLE;
-                        walk = (unsigned)(j - n_main);
-                        slot = j;
-                        x = f3(0.f, 0.f, 0.f);
-                        wfac = 4.0f * CUDART_PI_F / (float)a.n_kill;
-                    }
-                }
-                chunk_cur += n_idle < avail ? n_idle : avail;
-                idle = __ballot_sync(FULL, !busy);
-            }
-            // ---- (3) set up the next closest-point query -------------------------------
-            if (start_query) {
-                xq = x; far_radius = -1.0f;
-                bool need_query = true;
-                if (EXT) {
-                    const float yn = sqrtf(dot3(x, x));
-                    if (!(yn < 3.0e38f)) {
-                        // Safety net behind R10c: the Kelvin coordinate left fp32.  Every later radius would be
-                        // inf or NaN (a NaN query point is inside every box), so the walk could only run to
-                        // max_steps and be truncated there.  Same outcome now.
-                        a.records[slot] = make_float4(__int_as_float(-1), 0.f, 0.f, 0.f);
-                        if (a.steps) a.steps[slot] = -1;
-                        ++n_trunc;
-                        busy = false; need_query = false;
-                        far_radius = 0.0f;
-                    } else if (yn * a.Rmax <= 0.5f) {                           // far field: no query needed (E3)
-                        far_radius = 1.0f / a.Rmax - yn;
-                        need_query = false;
-                    } else {
-                        const float inv = 1.0f / (yn * yn);
-                        xq = f3(fmaf(inv, x.x, o.x), fmaf(inv, x.y, o.y), fmaf(inv, x.z, o.z));
-                        rho = 1.0f / yn;
-                    }
-                }
-                h.d2 = CUDART_INF_F; h.tri = INT_MAX; h.k = -1; h.v = h.w = 0.0f;
-                lim = 3.0e38f;                               // finite: the +inf of an empty node slot never passes
-                sp = 0; cur = CUR_NONE; q_visits = 0;
-                if (FAR) {
-                    lb2 = CUDART_INF_F;
-                    if (EXT) {
-                        // smallest primal distance whose Kelvin radius D / (rho (rho + D)) <= R* reaches far_near = k eps
-                        const float tr = a.far_near * rho;
-                        const float dn = tr < 0.5f ? tr * rho / (1.0f - tr) : 3.0e18f;
-                        dnear2 = dn * dn;
-                    } else {
-                        dnear2 = a.far_near * a.far_near;
-                    }
-                }
-                if (need_query) {
-                    if (prev >= 0) { stack_push(stk, sp, 0, 0.0f); cur = ~prev; }   // last closest face first: a tight bound
-                    else cur = 0;                                                   // root
-                }
-            }
-        }
-    }
-
-    // ---- statistics ----------------------------------------------------------
-    unsigned vals[6] = { n_steps, n_queries, n_trunc, n_nodes, n_tris, n_far };
-    for (int q = 0; q < 6; ++q) {
-        unsigned long long v = vals[q];
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-        if (lane == 0 && v) {
-            const int idx = q == 0 ? ST_STEPS : q == 1 ? ST_QUERIES : q == 2 ? ST_TRUNCATED : q == 3 ? ST_NODES : q == 4 ? ST_TRIS : ST_FAR;
-            atomicAdd(&a.stats[idx], v);
-        }
-    }
-}
+// The kernel itself lives in walk_body.inc, compiled twice: once as walk_kernel (one mesh, one operator per launch;
+// operator and far-field mode are template parameters) and once as walk_batch_kernel (many (mesh, operator) segments in
+// ONE launch, per-lane context: mcs_estimate_dtn_batch).
+#define WK_NAME walk_kernel
+#define WK_BATCH 0
+#define A_ a
+#define G_ g
+#define EXT_ EXT
+#define FAR_ FAR
+#include "walk_body.inc"
+#undef WK_NAME
+#undef WK_BATCH
+#undef A_
+#undef G_
+#undef EXT_
+#undef FAR_
+#define WK_NAME walk_batch_kernel
+#define WK_BATCH 1
+#define A_ (cx->a)
+#define G_ (cx->g)
+#define EXT_ lext
+#define FAR_ lfar
+#include "walk_body.inc"
+#undef WK_NAME
+#undef WK_BATCH
+#undef A_
+#undef G_
+#undef EXT_
+#undef FAR_
 
 __global__ void face_slot_lookup_kernel(const int32_t* __restrict__ face_slot, const int32_t* __restrict__ tri,
                                         int64_t n_s, int32_t* __restrict__ sample_slot)
@@ -1127,33 +798,77 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     const walk_fn fn = kex ? kex_table[count ? 1 : 0]
                      : merged ? table[8 + (exterior ? 2 : 0) + (count ? 1 : 0)][far]
                               : table[(exterior ? 4 : 0) + (count ? 2 : 0) + (coop ? 1 : 0)][far];
-    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
+    const int tw = (merged && !kex) ? 32 : WT;        // threads per block of the chosen variant
+    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, tw, 0));
     if (per_sm < 1) per_sm = 1;
     const long long total = a.n_s * a.W + a.n_kill;
     long long grid = (long long)n_sm * per_sm;
-    const long long warps = grid * (WT / 32);
+    const long long warps = grid * (tw / 32);
     long long chunk = total / (warps * 8);
     chunk = chunk < 32 ? 32 : (chunk > 256 ? 256 : chunk);
     chunk = (chunk / 32) * 32;
     a.chunk = (int)chunk;
-    const long long need_blocks = ceil_div64(ceil_div64(total, chunk), WT / 32);
+    const long long need_blocks = ceil_div64(ceil_div64(total, chunk), tw / 32);
     if (grid > need_blocks) grid = need_blocks;
-    if (grid > MAX_WALK_BLOCKS) grid = MAX_WALK_BLOCKS;
+    if (grid * (tw / 32) > MAX_WALK_BLOCKS * (WT / 32)) grid = MAX_WALK_BLOCKS * (WT / 32) / (tw / 32);   // the cooperative scratch is sized per warp
     if (grid < 1) grid = 1;
     if (defer) {                                      // the caller launches it (two operators on two streams)
-        defer->fn = fn; defer->grid = (unsigned)grid; defer->g = g; defer->a = a;
+        defer->fn = fn; defer->grid = (unsigned)grid; defer->block = (unsigned)tw; defer->g = g; defer->a = a;
         return MCS_OK;
     }
     mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
-    mcs_note_launch(), fn<<<(unsigned)grid, WT, 0, st>>>(g, a);
+    mcs_note_launch(), fn<<<(unsigned)grid, tw, 0, st>>>(g, a);
     mcs_prof_mark(MCS_MARK_WALK_END, st);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }
 
+size_t walk_batch_scratch_bytes(int n_launches)
+{
+    return align_up((size_t)n_launches * sizeof(WalkCtx)) + 256
+         + align_up((size_t)MAX_WALK_BLOCKS * (WT / 32) * (COOP_NCAP + COOP_LCAP) * 4);
+}
+
+int walk_launch_batch(const WalkLaunch* launches, const int* exterior, const int* far, int n_launches,
+                      void* scratch, size_t scratch_bytes, cudaStream_t st)
+{
+    if (!launches || n_launches < 1 || !scratch || scratch_bytes < walk_batch_scratch_bytes(n_launches)) return MCS_EINVAL;
+    const int chunk = 64;
+    std::vector<WalkCtx> h((size_t)n_launches);
+    long long begin = 0;
+    for (int i = 0; i < n_launches; ++i) {
+        h[i].g = launches[i].g; h[i].a = launches[i].a; h[i].begin = begin; h[i].ext = exterior[i]; h[i].far = far[i];
+        const long long n = h[i].a.n_s * h[i].a.W + h[i].a.n_kill;
+        begin += ceil_div64(n, chunk) * chunk;
+    }
+    char* p = (char*)scratch;
+    WalkCtx* d_ctx = (WalkCtx*)p;                              p += align_up((size_t)n_launches * sizeof(WalkCtx));
+    unsigned long long* counter = (unsigned long long*)p;      p += 256;
+    int* coop_scratch = (int*)p;
+    MCS_CUDA_TRY(cudaMemcpyAsync(d_ctx, h.data(), (size_t)n_launches * sizeof(WalkCtx), cudaMemcpyHostToDevice, st));
+    MCS_CUDA_TRY(cudaMemsetAsync(counter, 0, 8, st));
+    WalkBatch bt;
+    bt.total = begin; bt.n_ctx = n_launches; bt.chunk = chunk; bt.work_counter = counter; bt.coop_scratch = coop_scratch;
+    int dev = 0, n_sm = 0, per_sm = 0;
+    MCS_CUDA_TRY(cudaGetDevice(&dev));
+    MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    auto fn = walk_batch_kernel<false, true, false, false>;
+    MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
+    if (per_sm < 1) per_sm = 1;
+    long long grid = (long long)n_sm * per_sm;
+    const long long need_blocks = ceil_div64(ceil_div64(begin, chunk), WT / 32);
+    if (grid > need_blocks) grid = need_blocks;
+    if (grid > MAX_WALK_BLOCKS) grid = MAX_WALK_BLOCKS;
+    if (grid < 1) grid = 1;
+    mcs_note_launch(), fn<<<(unsigned)grid, WT, 0, st>>>(d_ctx, bt);
+    MCS_CUDA_TRY(cudaGetLastError());
+    MCS_CUDA_TRY(cudaStreamSynchronize(st));                   // `h` is pageable and leaves scope
+    return MCS_OK;
+}
+
 int walk_launch(const WalkLaunch* w, cudaStream_t st)
 {
-    mcs_note_launch(), w->fn<<<w->grid, WT, 0, st>>>(w->g, w->a);
+    mcs_note_launch(), w->fn<<<w->grid, w->block, 0, st>>>(w->g, w->a);
     MCS_CUDA_TRY(cudaGetLastError());
     return MCS_OK;
 }

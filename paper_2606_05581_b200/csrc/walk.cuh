@@ -53,11 +53,30 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
 // enqueued on walk_run's stream; walk_launch may enqueue the kernel on another stream that waits for it.
 struct WalkLaunch {
     void (*fn)(WalkGeom, WalkArgs);
-    unsigned grid;
+    unsigned grid, block;
     WalkGeom g;
     WalkArgs a;
 };
 int walk_launch(const WalkLaunch* w, cudaStream_t st);
+
+// Batched launch (mcs_estimate_dtn_batch): the prepared launches of many (mesh, operator) pairs run as ONE persistent
+// kernel over the concatenation of their walks.  ctx / counter / scratch: device memory of the caller
+// (walk_batch_scratch_bytes); blocks the host only for the upload of the contexts (pageable source).
+struct WalkCtx {
+    WalkGeom g;
+    WalkArgs a;
+    long long begin;               // first global walk index of the segment (a multiple of the chunk)
+    int ext, far;                  // exterior operator; far-field cut on
+};
+struct WalkBatch {
+    long long total;               // padded walk count of all segments
+    int n_ctx, chunk;
+    unsigned long long* work_counter;
+    int* coop_scratch;
+};
+size_t walk_batch_scratch_bytes(int n_launches);
+int walk_launch_batch(const WalkLaunch* launches, const int* exterior, const int* far, int n_launches,
+                      void* scratch, size_t scratch_bytes, cudaStream_t st);
 
 size_t accumulate_workspace_bytes(const mcs_bvh* b, const mcs_basis* basis, int64_t n_records);
 size_t accumulate_coo_workspace_bytes(const mcs_bvh* b, int64_t n_records, int64_t coo_capacity);
