@@ -34,6 +34,7 @@ extern "C" {
 #define MCS_EDEGENERATE (-2)   /* zero total area, non-finite vertex, Kelvin origin on a vertex      */
 #define MCS_ENOMEM      (-3)   /* workspace too small or device allocation failed                     */
 #define MCS_ECUDA       (-4)   /* CUDA runtime error (code in mcs_stats.cuda_error when available)    */
+#define MCS_WNOTCONVERGED 1    /* warning (results written): an iteration stopped at its cap, see mcs_steklov_eigs */
 
 typedef struct mcs_bvh mcs_bvh;
 
@@ -224,7 +225,10 @@ size_t mcs_workspace_bytes(const mcs_bvh* bvh, const mcs_samples* samples, const
  *   largest tangent ball at s_i.  S is symmetric PSD by construction.
  * samples/basis/params/out are host structs holding device pointers.  The
  * library never allocates here: all scratch lives in `workspace`.
- * Asynchronous on `stream` unless host_stats != NULL.
+ * Work is enqueued on `stream`, but the call is NOT fully asynchronous: it blocks the host for two small read-backs
+ * during the preparation (sample-index check, Kelvin bounds of the exterior) and once per accumulation chunk (entry
+ * count), so it returns when the walk kernel has finished and the last accumulation chunk is enqueued; with
+ * host_stats != NULL it returns when everything is done.  It cannot be captured in a CUDA graph.
  * Errors: MCS_EINVAL, MCS_ENOMEM (workspace_bytes too small), MCS_ECUDA.
  */
 int mcs_estimate_dtn_interior(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,
@@ -461,7 +465,10 @@ int mcs_project_galerkin_coo(const int32_t* row, const int32_t* col, const float
  * evals [batch][n_eig] ascending; evecs [batch][n_eig][K] (may be NULL), M-orthonormal: psi_i^T M psi_j = delta_ij.
  * One-sided Jacobi in fp32 on M^-1/2 S M^-1/2 (all eigenpairs are computed; the n_eig smallest are returned).
  * sweeps_out (host, may be NULL): Jacobi sweeps used.  Blocks the host once per sweep (convergence flag).
- * K <= 16384.  Errors: MCS_EINVAL, MCS_ENOMEM (workspace), MCS_ECUDA. */
+ * The solver is made for the symmetric POSITIVE SEMI-DEFINITE matrices of Alg. 2 / Eq. 32: one-sided Jacobi diagonalises
+ * A^2, so an indefinite input (Alg. 1, estimator = 1) with eigenvalues +l and -l of equal magnitude can leave mixed
+ * vectors.  Returns MCS_WNOTCONVERGED (> 0, results written) when the sweep cap (30) was reached with rotations still
+ * being applied.  K <= 16384.  Errors: MCS_EINVAL, MCS_ENOMEM (workspace), MCS_ECUDA. */
 size_t mcs_steklov_eigs_workspace_bytes(int64_t K, int64_t batch);
 int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig,
                      float* evals, float* evecs, void* workspace, size_t workspace_bytes,

@@ -17,6 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("MCDTN_LIB") or os.path.join(HERE, "libmcdtn.so")     # MCDTN_LIB: another build of the same library
 
 MCS_OK, MCS_EINVAL, MCS_EDEGENERATE, MCS_ENOMEM, MCS_ECUDA = 0, -1, -2, -3, -4
+MCS_WNOTCONVERGED = 1
 
 
 class McsError(RuntimeError):
@@ -310,6 +311,12 @@ def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspa
     K = basis.K if basis is not None else bvh.V
     if out is None:
         out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
+    elif not (isinstance(out, torch.Tensor) and out.is_cuda and out.device == bvh.device and out.dtype == torch.float32
+              and out.is_contiguous() and tuple(out.shape) == (K, K)):
+        raise ValueError(f"out must be a contiguous CUDA float32 tensor of shape ({K}, {K}) on {bvh.device}")
+    if workspace is not None and not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.device == bvh.device
+                                      and workspace.dtype == torch.uint8 and workspace.is_contiguous()):
+        raise ValueError(f"workspace must be a contiguous CUDA uint8 tensor on {bvh.device}")
     need = workspace_bytes(bvh, samples, params, exterior, basis)
     if workspace is None or (workspace.numel() < need and not _exact_workspace):
         workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
@@ -787,9 +794,13 @@ def steklov_eigs(S, mass, n_eig, want_vectors=True):
     evecs = torch.empty((B, n_eig, K), dtype=torch.float32, device=S.device) if want_vectors else None
     sweeps = C.c_int32(0)
     with torch.cuda.device(S.device):
-        _check(lib().mcs_steklov_eigs(_ptr(S), _ptr(mass), C.c_int64(K), C.c_int64(B), C.c_int32(n_eig), _ptr(evals),
-                                      _ptr(evecs), _ptr(ws), C.c_size_t(need), C.byref(sweeps), _stream(S.device)),
-               "mcs_steklov_eigs")
+        rc = lib().mcs_steklov_eigs(_ptr(S), _ptr(mass), C.c_int64(K), C.c_int64(B), C.c_int32(n_eig), _ptr(evals),
+                                    _ptr(evecs), _ptr(ws), C.c_size_t(need), C.byref(sweeps), _stream(S.device))
+    if rc == MCS_WNOTCONVERGED:
+        import warnings
+        warnings.warn("mcs_steklov_eigs: sweep cap reached before convergence (input not positive semi-definite?)")
+    else:
+        _check(rc, "mcs_steklov_eigs")
     if single:
         return evals[0], (evecs[0] if evecs is not None else None), sweeps.value
     return evals, evecs, sweeps.value

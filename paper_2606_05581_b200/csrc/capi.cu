@@ -214,6 +214,10 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
                           (float4*)(base[x] + L[x].records_off), nullptr, false, nullptr, hh[x] != nullptr, &stats_dev[x], st, &wl[x]);
         if (rc != MCS_OK) return fail(rc, hh[x]);
     }
+    // Measured and not kept: both operators' walks as two segments of ONE launch of the batched kernel (no delay kernel, no
+    // priorities).  Bit-identical results, but slower: configs[1] 47.6 -> 57.4 ms per call (the per-lane context costs the
+    // lean 64-register variant 184 bytes of spills), config 3 walk span 891 -> 1191 ms (interior and exterior lanes, exact
+    // and far-field queries share warps and diverge).  The two specialised kernels on two streams stay.
     MCS_CUDA_TRY(cudaEventRecord(ev_prep, st));
     MCS_CUDA_TRY(cudaStreamWaitEvent(st1, ev_prep, 0));
     MCS_CUDA_TRY(cudaStreamWaitEvent(st2, ev_prep, 0));
@@ -776,6 +780,7 @@ extern "C" const char* mcs_error_string(int code)
 {
     switch (code) {
         case MCS_OK: return "ok";
+        case MCS_WNOTCONVERGED: return "warning: iteration stopped at its cap before converging (results written)";
         case MCS_EINVAL: return "invalid argument";
         case MCS_EDEGENERATE: return "degenerate input (zero area, non-finite vertex, or Kelvin origin on a vertex)";
         case MCS_ENOMEM: return "workspace too small or device allocation failed";

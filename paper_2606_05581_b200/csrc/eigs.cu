@@ -506,6 +506,32 @@ eig_vectors_kernel(const float* __restrict__ Q, const float* __restrict__ mass, 
 
 }  // namespace
 
+// Sorts the K (key, index) pairs of one matrix per block: bitonic network on 64-bit (key << 32 | index) words in shared
+// memory, so equal keys keep index order (what the stable radix sort gave).
+__global__ void __launch_bounds__(256)
+eig_sort_kernel(uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, int K, int P)
+{
+    extern __shared__ unsigned long long s_kv[];
+    uint32_t* k = keys + (size_t)blockIdx.x * K;
+    uint32_t* v = vals + (size_t)blockIdx.x * K;
+    for (int i = threadIdx.x; i < P; i += blockDim.x)
+        s_kv[i] = i < K ? ((unsigned long long)k[i] << 32) | (unsigned long long)v[i] : ~0ull;
+    __syncthreads();
+    for (int size = 2; size <= P; size <<= 1)
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int i = threadIdx.x; i < P; i += blockDim.x) {
+                const int j = i ^ stride;
+                if (j > i) {
+                    const unsigned long long a = s_kv[i], b = s_kv[j];
+                    const bool up = (i & size) == 0;
+                    if ((a > b) == up) { s_kv[i] = b; s_kv[j] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = threadIdx.x; i < K; i += blockDim.x) { k[i] = (uint32_t)(s_kv[i] >> 32); v[i] = (uint32_t)s_kv[i]; }
+}
+
 extern "C" size_t mcs_steklov_eigs_workspace_bytes(int64_t K, int64_t batch)
 {
     if (K < 1 || batch < 1) return 0;
@@ -538,6 +564,7 @@ extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, in
     a.G = G; a.Q = Q; a.K = K; a.Kp = (int)(K + (K & 1)); a.not_converged = flag; a.scale_bits = scale_bits;
     a.tol = fmaxf(1e-6f, 2e-7f * sqrtf((float)K));           // fp32 dot products of length K cannot resolve less
     int sweep = 0;
+    unsigned last_flag = 0;
     const int max_sweeps = 30;
     if (K > 1)
         for (; sweep < max_sweeps; ++sweep) {
@@ -561,10 +588,17 @@ extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, in
             unsigned h = 0;
             MCS_CUDA_TRY(cudaMemcpyAsync(&h, flag, 4, cudaMemcpyDeviceToHost, st));
             MCS_CUDA_TRY(cudaStreamSynchronize(st));
+            last_flag = h;
             if (!h) { ++sweep; break; }
         }
     if (sweeps_out) *sweeps_out = sweep;
+    const bool converged = K <= 1 || sweep < max_sweeps || last_flag == 0;
     mcs_note_launch(), eig_values_kernel<<<dim3((unsigned)K, (unsigned)batch), ET, 0, st>>>(G, Q, K, lam, keys, vals);
+    if (K <= 4096) {
+        // one block per matrix: (eigenvalue, index) pairs sorted in shared memory -- the same order as the stable sort
+        int P = 1; while (P < K) P <<= 1;
+        mcs_note_launch(), eig_sort_kernel<<<(unsigned)batch, 256, (size_t)P * 8, st>>>(keys, vals, (int)K, P);
+    } else
     for (int64_t b = 0; b < batch; ++b) {
         int rc = sort_pairs_u32(keys + b * K, vals + b * K, K, 32, sort_ws, sort_workspace_bytes(K, 4), st);
         if (rc != MCS_OK) return rc;
@@ -576,5 +610,5 @@ extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, in
         mcs_note_launch(), eig_vectors_kernel<<<dim3((unsigned)n_eig, (unsigned)batch), ET, 0, st>>>(Q, mass, lam, vals, K, n_eig, evals, G);
     }
     MCS_CUDA_TRY(cudaGetLastError());
-    return MCS_OK;
+    return converged ? MCS_OK : MCS_WNOTCONVERGED;
 }

@@ -813,7 +813,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     if (grid * (tw / 32) > MAX_WALK_BLOCKS * (WT / 32)) grid = MAX_WALK_BLOCKS * (WT / 32) / (tw / 32);   // the cooperative scratch is sized per warp
     if (grid < 1) grid = 1;
     if (defer) {                                      // the caller launches it (two operators on two streams)
-        defer->fn = fn; defer->grid = (unsigned)grid; defer->block = (unsigned)tw; defer->g = g; defer->a = a;
+        defer->fn = fn; defer->grid = (unsigned)grid; defer->block = (unsigned)tw; defer->g = g; defer->a = a; defer->coop = coop || merged;
         return MCS_OK;
     }
     mcs_prof_mark(MCS_MARK_WALK_BEGIN, st);
@@ -852,7 +852,10 @@ int walk_launch_batch(const WalkLaunch* launches, const int* exterior, const int
     int dev = 0, n_sm = 0, per_sm = 0;
     MCS_CUDA_TRY(cudaGetDevice(&dev));
     MCS_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    auto fn = walk_batch_kernel<false, true, false, false>;
+    // the warp-cooperative path when any segment would use it on its own (large trees or few walks), else the lean variant
+    bool coop = false;
+    for (int i = 0; i < n_launches; ++i) coop = coop || launches[i].coop;
+    auto fn = coop ? walk_batch_kernel<false, true, false, false> : walk_batch_kernel<false, false, false, false>;
     MCS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, WT, 0));
     if (per_sm < 1) per_sm = 1;
     long long grid = (long long)n_sm * per_sm;

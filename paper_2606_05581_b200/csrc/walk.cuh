@@ -54,6 +54,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
 struct WalkLaunch {
     void (*fn)(WalkGeom, WalkArgs);
     unsigned grid, block;
+    bool coop;                     // the variant with the warp-cooperative path was chosen
     WalkGeom g;
     WalkArgs a;
 };

@@ -533,3 +533,27 @@ def test_host_entry_point_equals_the_device_calls_bit_for_bit(api, ops):
         assert torch.equal(res["exterior"], api.estimate_dtn_exterior(bvh, S, P).cpu())
         assert res["stats"].n_walks == S.n_s * 48 + 7777
     assert res["d2h_bytes"] == (int(interior) + int(exterior)) * bvh.V * bvh.V * 4
+
+
+def test_handle_freed_while_work_is_queued_on_a_side_stream(api):
+    """mcs_free_bvh must order the release of the tree's memory after the last call that used the handle, also when that
+    call ran on a NON-BLOCKING stream (PyTorch's side streams), which the legacy default stream does not wait for: the
+    handle records an event on the stream of every call and the free waits for it.  Estimate on a side stream, drop the
+    handle at once, immediately build other trees (which reuse the pool's memory), and compare with an undisturbed run."""
+    v, f = icosphere(3)
+    smp = vertex_cell_samples(v, f, 4, seed=1)
+    vd, fd = torch.as_tensor(v).cuda(), torch.as_tensor(f).cuda()
+    S = api.Samples.from_arrays(smp["tri"], smp["bary"], smp["weight"])
+    P = api.Params(seed=3, walks_per_sample=256, eps=1e-4)
+    ref = api.estimate_dtn_interior(api.build_bvh(vd, fd), S, P).clone()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for _ in range(8):
+        with torch.cuda.stream(side):
+            bvh = api.build_bvh(vd, fd)
+            out = api.estimate_dtn_interior(bvh, S, P)
+            del bvh                                                   # freed while the accumulation may still be queued
+            junk = [api.build_bvh(vd * 1.5, fd) for _ in range(3)]    # grabs memory from the pool right away
+            del junk
+        side.synchronize()
+        assert torch.equal(out, ref)
