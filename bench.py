@@ -300,6 +300,42 @@ def walk_roofline(stats, t_kernel_s, level_gbs, level, fp32_tflops, note, tri_by
 
 
 # ------------------------------------------------------------------------------
+# the oracle-side ideal of the traversal ("a kernel could raise its fraction by touching more nodes")
+# ------------------------------------------------------------------------------
+def ideal_traversal_counts(bvh, points, dist, chunk=8):
+    """For query points with their EXACT distances (from the oracle's brute force): the number of 4-wide nodes and of
+    leaf references of THIS tree whose box is closer than the true distance -- what any exact traversal must visit,
+    however it orders its work.  The tree comes from mcs_bvh_dump (binary nodes; a wide node of the walk kernel is a
+    binary node at even depth, its box the union of its two child boxes); numpy only, no kernel involved."""
+    nodes, leaf_tri, _ = bvh.dump()
+    w = nodes.cpu().numpy()
+    del nodes
+    fw = w.view(np.float32)
+    c0, c1 = w[:, 12].copy(), w[:, 13].copy()
+    n = len(w)
+    depth = np.full(n, -1, np.int32)
+    depth[0] = 0
+    frontier = np.array([0], np.int64)
+    while len(frontier):
+        ch = np.concatenate([c0[frontier], c1[frontier]])
+        d = np.concatenate([depth[frontier], depth[frontier]]) + 1
+        keep = ch >= 0
+        depth[ch[keep]] = d[keep]
+        frontier = ch[keep].astype(np.int64)
+    even = np.flatnonzero((depth & 1) == 0)
+    lo = np.minimum(fw[even, 0:3], fw[even, 6:9]); hi = np.maximum(fw[even, 3:6], fw[even, 9:12])       # box of a wide node
+    leaf_lo = np.concatenate([fw[c0 < 0, 0:3], fw[c1 < 0, 6:9]]); leaf_hi = np.concatenate([fw[c0 < 0, 3:6], fw[c1 < 0, 9:12]])
+    n_nodes, n_leaves = [], []
+    for i in range(0, len(points), chunk):
+        for p, D in zip(points[i:i + chunk].astype(np.float32), dist[i:i + chunk]):
+            d2 = (np.maximum(np.maximum(lo - p, p - hi), 0.0) ** 2).sum(1)
+            n_nodes.append(int((d2 < D * D).sum()) + (0 if d2[0] < D * D else 1))                      # the root is always visited
+            l2 = (np.maximum(np.maximum(leaf_lo - p, p - leaf_hi), 0.0) ** 2).sum(1)
+            n_leaves.append(int((l2 <= D * D * (1 + 1e-6)).sum()))
+    return float(np.mean(n_nodes)), float(np.mean(n_leaves)), len(n_nodes)
+
+
+# ------------------------------------------------------------------------------
 # sub-record: configs[1] (icosphere L4, dense output, killing on) -- round 1's headline, kept for continuity
 # ------------------------------------------------------------------------------
 def bench_cfg1(api, torch, dev, args, seed, steps, warmup, flush, fp32_tflops, l2_gbs):
@@ -591,6 +627,27 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         s, dt, cores, desc = oracle_sample_cfg3(wl, args, args.cpu_samples, args.cpu_walks)
         cpu = {"value": s / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
+        # ideal node / leaf counts of the same tree on the oracle's own query points (a sample of the walks' queries)
+        try:
+            from oracle import Oracle, OracleParams, mesh_geom
+            orc = Oracle(mesh_geom(wl["v"], wl["f"]))
+            ids = np.arange(0, n_s, max(1, n_s // args.ideal_samples))[:args.ideal_samples]
+            bvh_i = api.build_bvh(vd, fd)
+            ids_d = torch.as_tensor(ids, device=dev)
+            nrm_i, _ = api.orient_samples(bvh_i, api.Samples(S0.tri[ids_d].contiguous(), S0.bary[ids_d].contiguous(), S0.weight[ids_d].contiguous()))
+            normal = np.zeros((n_s, 3), np.float32); normal[ids] = nrm_i.cpu().numpy()
+            ideal = {}
+            for ext in (False, True):
+                op = OracleParams(seed=args.seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, origin=wl["origin"])
+                pts, dd = orc.walk_query_points(op, ext, wl["tri"], wl["bary"], wl["weight"], ids, 2, max_pos=16, normal=normal)
+                nn, nl, nq = ideal_traversal_counts(bvh_i, pts, dd)
+                ideal["exterior" if ext else "interior"] = {"wide_nodes_per_query": nn, "leaf_boxes_per_query": nl, "queries": nq}
+            del bvh_i
+            roofline["ideal_exact_traversal"] = dict(ideal, note="wide nodes / leaf references of the same tree whose box is closer than the exact "
+                                                     "distance (oracle brute force) at the query points of the oracle's own walks: the least any exact "
+                                                     "traversal visits; compare with nodes_per_query / tris_per_query of the exact-query runs")
+        except Exception as exc:                     # a measurement aid: never fail the bench line
+            roofline["ideal_exact_traversal"] = {"error": repr(exc)}
 
     sub = {}
     if world == 1 and not args.no_sub and args.far_alpha > 0:
@@ -679,6 +736,7 @@ def main():
     ap.add_argument("--cpu-walks", type=int, default=8, help="walks per sample point of the cpu_baseline leg")
     ap.add_argument("--ref-samples", type=int, default=8, help="sample points per step of --impl reference")
     ap.add_argument("--ref-walks", type=int, default=4, help="walks per sample point per step of --impl reference")
+    ap.add_argument("--ideal-samples", type=int, default=24, help="sample points whose oracle walks give the query points of the ideal traversal count")
     ap.add_argument("--cfg4-meshes", type=int, default=32, help="meshes of the configs[4] sample sub-record")
     ap.add_argument("--cfg4-workers", type=int, default=4, help="host workers of mcs_estimate_dtn_batch in that sub-record")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -931,6 +931,65 @@ int64_t orc_run_walks_subset(const orc_geom *g, const orc_params *P, int exterio
 }
 
 /*
+ * Measurement helper (bench.py, SURVEY.md 8(d) "oracle-side ideal"): the PRIMAL query points of the closest-point
+ * queries that the walks w = 0..n_w-1 of the samples `ids` make (at most max_pos per walk; for the exterior the points
+ * x = kappa(y) at which the flat-triangle query is taken, far-field jumps without a query left out), with the exact
+ * distance found there.  The same loops as walk_on_spheres / walk_on_spheres_kelvin, recording instead of returning.
+ * pos [n_ids * n_w * max_pos][3], dist [same], in blocks of max_pos per walk; count [n_ids * n_w] = points in each
+ * block; returns the total.
+ */
+int64_t orc_walk_query_points(const orc_geom *g, const orc_params *P, int exterior,
+                              const int32_t *tri, const float *bary, const float *weight, const float *normal,
+                              const int64_t *ids, int64_t n_ids, int n_w, int max_pos, double *pos, double *dist,
+                              int32_t *count /* [n_ids * n_w]: points written in the block of walk (k, w) */)
+{
+    int64_t n_total = 0;
+    #pragma omp parallel for schedule(dynamic, 1) reduction(+:n_total)
+    for (int64_t k = 0; k < n_ids; ++k) {
+        const int64_t i = ids[k];
+        orc_sample S; orc_ball B;
+        fill_sample(g, tri, bary, weight, normal, NULL, i, &S);
+        if (exterior) orc_tangent_ball_exterior(g, P, &S, &B); else orc_tangent_ball_interior(g, P, &S, &B);
+        for (int w = 0; w < n_w; ++w) {
+            const int64_t blk = (k * n_w + w) * (int64_t)max_pos;
+            int n_here = 0;
+            count[k * n_w + w] = 0;
+            if (!(B.r > 0.0)) continue;
+            double z[3];
+            sample_ball_surface(P, &B, (uint32_t)i, (uint32_t)w, z);
+            double x[3] = { z[0], z[1], z[2] };
+            for (int step = 0; step <= P->max_steps && n_here < max_pos; ++step) {
+                orc_hit h;
+                double radius;
+                if (exterior) {
+                    double yn = norm3(x);
+                    if (yn * P->Rmax_norm <= 0.5) radius = 1.0 / P->Rmax_norm - yn;
+                    else {
+                        double q[3] = { P->origin[0] + x[0] / (yn * yn), P->origin[1] + x[1] / (yn * yn), P->origin[2] + x[2] / (yn * yn) };
+                        double rho = 1.0 / yn;
+                        orc_closest_point(g, q, &h);
+                        memcpy(pos + 3 * (blk + n_here), q, sizeof q); dist[blk + n_here] = h.dist; ++n_here;
+                        radius = h.dist / (rho * fmin(P->Rmax_norm, rho + h.dist));
+                        if (radius < P->eps || h.dist > rho) break;
+                    }
+                } else {
+                    orc_closest_point(g, x, &h);
+                    memcpy(pos + 3 * (blk + n_here), x, sizeof x); dist[blk + n_here] = h.dist; ++n_here;
+                    radius = h.dist;
+                    if (radius < P->eps || (P->escape_radius > 0.0 && radius > P->escape_radius)) break;
+                }
+                double wdir[3];
+                step_direction(P->seed, (uint32_t)i, (uint32_t)w, (uint32_t)(step + 1), wdir);
+                for (int j = 0; j < 3; ++j) x[j] += radius * wdir[j];
+            }
+            count[k * n_w + w] = n_here;
+            n_total += n_here;
+        }
+    }
+    return n_total;
+}
+
+/*
  * Accumulate S = sum_w weight_w d d^T in the hat basis (PAPER.md:177-190,
  * 277-285): d = b(s) - b(t) has the barycentric coordinates of s on the
  * vertices of tri_s and minus those of t on the vertices of tri_t; a killing

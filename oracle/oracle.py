@@ -29,6 +29,7 @@ def _load():
         _lib.orc_total_area.restype = C.c_double
         _lib.orc_run_walks.restype = C.c_int64
         _lib.orc_run_walks_subset.restype = C.c_int64
+        _lib.orc_walk_query_points.restype = C.c_int64
         _lib.orc_num_threads.restype = C.c_int
         for f in ("orc_sizeof_record", "orc_sizeof_params", "orc_sizeof_geom"):
             getattr(_lib, f).restype = C.c_size_t
@@ -285,6 +286,28 @@ class Oracle:
                                           C.c_int64(len(ids)), C.c_int(int(n_w)), C.c_int64(nk), ptr(rec))
         assert n == len(rec)
         return rec
+
+    def walk_query_points(self, params: OracleParams, exterior: bool, tri, bary, weight, ids, n_w, max_pos=64, normal=None):
+        """(points [n,3], exact distances [n]): the primal query points of the closest-point queries made by walks
+        0..n_w-1 of the samples `ids` (measurement helper of bench.py: the population on which the ideal traversal
+        counts of a tree are taken)."""
+        tri = np.ascontiguousarray(tri, np.int32)
+        bary = np.ascontiguousarray(bary, np.float32)
+        weight = np.ascontiguousarray(weight, np.float32)
+        ids = np.ascontiguousarray(ids, np.int64)
+        if normal is not None:
+            normal = np.ascontiguousarray(normal, np.float32)
+        cp = self._params(params, exterior)
+        cap = len(ids) * n_w * max_pos
+        pos = np.zeros((cap, 3))
+        dist = np.zeros(cap)
+        count = np.zeros(len(ids) * n_w, np.int32)
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        self.lib.orc_walk_query_points(C.byref(self.geom.c), C.byref(cp), C.c_int(int(exterior)), ptr(tri), ptr(bary), ptr(weight),
+                                       ptr(normal), ptr(ids), C.c_int64(len(ids)), C.c_int(int(n_w)), C.c_int(int(max_pos)),
+                                       ptr(pos), ptr(dist), ptr(count))
+        keep = (np.arange(max_pos)[None, :] < count[:, None]).ravel()
+        return pos[keep], dist[keep]
 
     def accumulate_hat(self, rec, tri, bary, want_var=False, naive=False):
         K = self.geom.c.V
