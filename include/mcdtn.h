@@ -34,6 +34,7 @@ extern "C" {
 #define MCS_EDEGENERATE (-2)   /* zero total area, non-finite vertex, Kelvin origin on a vertex      */
 #define MCS_ENOMEM      (-3)   /* workspace too small or device allocation failed                     */
 #define MCS_ECUDA       (-4)   /* CUDA runtime error (code in mcs_stats.cuda_error when available)    */
+#define MCS_ETOOLARGE   (-5)   /* size beyond a fixed maximum of the entry point (mcs_sort_pairs_u64_static)     */
 #define MCS_WNOTCONVERGED 1    /* warning (results written): an iteration stopped at its cap, see mcs_steklov_eigs */
 
 typedef struct mcs_bvh mcs_bvh;
@@ -392,6 +393,19 @@ int mcs_philox4x32_10(const uint32_t* counters, int64_t n, const uint32_t* key /
 size_t mcs_sort_workspace_bytes(int64_t n);
 int mcs_sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int32_t key_bits,
                        void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same sort for callers that may not allocate and have no workspace to hand in (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the workspace is a file-scope device array
+ * inside the library (sort.cu), 12.25 MiB that every GPU which loads the library holds until the process exits.
+ * keys [n] / vals [n]: device pointers, sorted in place (stable, low `key_bits` bits of the key), as above.
+ * Limit: n <= mcs_sort_static_max_n() = 2^20 pairs; beyond it the call returns MCS_ETOOLARGE and does nothing.
+ * The call allocates nothing and frees nothing (no cudaMalloc / cudaFree / allocating library routine) and is
+ * asynchronous on `stream`.  All calls on one device share the one array and it keeps the last call's contents
+ * (nothing in it needs to start at zero): calls that OVERLAP on the GPU -- different streams with no ordering
+ * between them, or two host threads -- race on it; order them on one stream or with events.
+ * Errors: MCS_EINVAL (null pointer, n < 0, key_bits outside [0, 64]), MCS_ETOOLARGE, MCS_ECUDA. */
+int64_t mcs_sort_static_max_n(void);
+int mcs_sort_pairs_u64_static(uint64_t* keys, uint32_t* vals, int64_t n, int32_t key_bits, void* stream);
 
 /* Measurement hooks (bench.py).  mcs_launch_count: kernels this library has launched in
  * this process.  mcs_profile_enable(1): estimate_* calls record CUDA events on their stream

@@ -590,6 +590,23 @@ def sort_pairs_u64(keys, vals, key_bits=64):
     return keys, vals
 
 
+def sort_static_max_n() -> int:
+    f = lib().mcs_sort_static_max_n
+    f.restype = C.c_int64
+    return int(f())
+
+
+def sort_pairs_u64_static(keys, vals, key_bits=64):
+    """mcs_sort_pairs_u64_static: the same in-place sort with the workspace in a static device array of the library
+    (no allocation in the call; n <= sort_static_max_n(); calls that overlap on the GPU race on the shared array)."""
+    assert keys.is_cuda and vals.is_cuda and keys.dtype == torch.int64 and vals.dtype == torch.int32
+    n = keys.numel()
+    with torch.cuda.device(keys.device):
+        _check(lib().mcs_sort_pairs_u64_static(_ptr(keys), _ptr(vals), C.c_int64(n), C.c_int32(key_bits),
+                                               _stream(keys.device)), "mcs_sort_pairs_u64_static")
+    return keys, vals
+
+
 class PhaseTimes(C.Structure):
     _fields_ = [("prep_ms", C.c_float), ("walk_ms", C.c_float), ("accumulate_ms", C.c_float),
                 ("total_ms", C.c_float), ("walk_interior_ms", C.c_float), ("walk_exterior_ms", C.c_float)]

@@ -785,6 +785,7 @@ extern "C" const char* mcs_error_string(int code)
         case MCS_EDEGENERATE: return "degenerate input (zero area, non-finite vertex, or Kelvin origin on a vertex)";
         case MCS_ENOMEM: return "workspace too small or device allocation failed";
         case MCS_ECUDA: return "CUDA runtime error";
+        case MCS_ETOOLARGE: return "size beyond the fixed maximum of this entry point";
         default: return "unknown error";
     }
 }

@@ -275,3 +275,50 @@ int sort_pairs_u32(uint32_t* keys, uint32_t* vals, int64_t n, int key_bits, void
 {
     return radix_sort_impl<uint32_t>(keys, vals, n, key_bits, ws, ws_bytes, st);
 }
+
+// ---------------------------------------------------------------------------
+// mcs_sort_pairs_u64_static -- the same sort for callers that may not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc) and have no workspace to pass: the workspace is a file-scope device array, so
+// every GPU that loads this library holds MCS_SORT_STATIC_BYTES (12.25 MiB) until the process exits.  Limit:
+// MCS_SORT_STATIC_MAX_N = 2^20 pairs.  The entry point calls no cudaMalloc / cudaFree / allocating routine; the
+// kernels are those of mcs_sort_pairs_u64 (radix_sort_impl above), so the result is the same stable order.
+// Every call on a device shares the one array: two calls that overlap on the GPU (different streams, no ordering
+// between them) race on it.  Nothing in it has to start at zero -- the histogram kernel writes every count of a
+// pass before the scan reads it, and the alternate key/value buffers are written before they are read -- so what the
+// previous call left there is harmless (tests/test_zz_no_alloc.py runs two calls of different sizes in a row).
+// ---------------------------------------------------------------------------
+#define MCS_SORT_STATIC_MAX_N (1 << 20)
+#define MCS_SORT_STATIC_BYTES ((size_t)MCS_SORT_STATIC_MAX_N * 12 + (256u << 10))
+static __device__ __align__(256) unsigned char g_sort_static_scratch[MCS_SORT_STATIC_BYTES];
+
+namespace {
+constexpr int SORT_STATIC_MAX_DEVICES = 64;
+void* g_sort_static_ptr[SORT_STATIC_MAX_DEVICES];      // device address of the array on each device, once resolved
+std::mutex g_sort_static_mutex;
+}  // namespace
+
+extern "C" int64_t mcs_sort_static_max_n(void) { return MCS_SORT_STATIC_MAX_N; }
+
+extern "C" int mcs_sort_pairs_u64_static(uint64_t* keys, uint32_t* vals, int64_t n, int32_t key_bits, void* stream)
+{
+    if (n < 0 || (n > 0 && (!keys || !vals))) return MCS_EINVAL;
+    if (n > MCS_SORT_STATIC_MAX_N) return MCS_ETOOLARGE;                // more pairs than the static scratch holds
+    if (sort_workspace_bytes(n, 8) > MCS_SORT_STATIC_BYTES) return MCS_ETOOLARGE;
+    int dev = 0;
+    MCS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= SORT_STATIC_MAX_DEVICES) return MCS_EINVAL;
+    void* ptr = nullptr;
+    {
+        // In host code `g_sort_static_scratch` is a host-side stand-in, not a device address: resolve it once per
+        // device, with that device current (it is: cudaGetDevice above).
+        std::lock_guard<std::mutex> lock(g_sort_static_mutex);
+        if (!g_sort_static_ptr[dev]) {
+            void* p = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress(&p, g_sort_static_scratch);
+            if (e != cudaSuccess || !p) { (void)cudaGetLastError(); return MCS_ECUDA; }
+            g_sort_static_ptr[dev] = p;
+        }
+        ptr = g_sort_static_ptr[dev];
+    }
+    return radix_sort_impl<uint64_t>(keys, vals, n, key_bits, ptr, MCS_SORT_STATIC_BYTES, (cudaStream_t)stream);
+}
