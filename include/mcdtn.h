@@ -179,7 +179,13 @@ typedef struct {
                                     query, the EXACT distance from y to the Kelvin-inverted faces = (1/|x|) min
                                     over the mesh of |x - p| / |p - o| (E4): larger balls, fewer jumps, a dearer
                                     query; same estimator.  Not combinable with far_alpha                              */
-    int32_t  pad3_;
+    int32_t  nonblocking;        /* mcs_estimate_dtn_interior / _exterior only.  0 (default): the call blocks the host for small
+                                    read-backs (below) and returns device-side input errors.  1: the call ONLY ENQUEUES work on
+                                    `stream` -- no read-back, no allocation, no copy from host memory -- so it returns at once and
+                                    may be captured in a CUDA graph.  Needs output_kind 0, basis kind 0 and host_stats == NULL
+                                    (MCS_EINVAL otherwise).  Same kernels, same bits.  Input errors only the device can see (a
+                                    sample's face index out of range, a vertex at the Kelvin origin) cannot be returned then:
+                                    such a call skips its walks and fills `out` with NaN                                 */
 } mcs_params;
 
 typedef struct {
@@ -226,10 +232,12 @@ size_t mcs_workspace_bytes(const mcs_bvh* bvh, const mcs_samples* samples, const
  *   largest tangent ball at s_i.  S is symmetric PSD by construction.
  * samples/basis/params/out are host structs holding device pointers.  The
  * library never allocates here: all scratch lives in `workspace`.
- * Work is enqueued on `stream`, but the call is NOT fully asynchronous: it blocks the host for two small read-backs
- * during the preparation (sample-index check, Kelvin bounds of the exterior) and once per accumulation chunk (entry
- * count), so it returns when the walk kernel has finished and the last accumulation chunk is enqueued; with
- * host_stats != NULL it returns when everything is done.  It cannot be captured in a CUDA graph.
+ * Work is enqueued on `stream`.  With params.nonblocking = 1 (dense output, hat basis, host_stats == NULL) that is all
+ * the call does: it returns at once and may be captured in a CUDA graph; workspace, out, the samples' arrays and the
+ * bvh handle must stay alive until the work has run (every time the graph runs).  Otherwise the call blocks the host:
+ * once after the preparation (one 16-byte read-back of the device-side input checks, so that MCS_EINVAL /
+ * MCS_EDEGENERATE come back before the walks start); COO output and the point basis once more per accumulation chunk
+ * (entry count); with host_stats != NULL it returns when everything is done.
  * Errors: MCS_EINVAL, MCS_ENOMEM (workspace_bytes too small), MCS_ECUDA.
  */
 int mcs_estimate_dtn_interior(const mcs_bvh* bvh, const mcs_samples* samples, const mcs_basis* basis,

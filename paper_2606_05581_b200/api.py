@@ -54,7 +54,7 @@ class _Params(C.Structure):
                 ("antithetic", C.c_int32), ("include_killing", C.c_int32), ("n_kill_walks", C.c_int64),
                 ("kelvin_origin", C.c_float * 3), ("output_kind", C.c_int32), ("coo_capacity", C.c_int64),
                 ("estimator", C.c_int32), ("inset", C.c_float), ("far_alpha", C.c_float), ("far_near_factor", C.c_float),
-                ("exterior_query", C.c_int32), ("pad3_", C.c_int32)]
+                ("exterior_query", C.c_int32), ("nonblocking", C.c_int32)]
 
 
 class _Matrix(C.Structure):
@@ -306,9 +306,17 @@ def workspace_bytes(bvh: Bvh, samples: Samples, params: Params, exterior: bool, 
     return int(lib().mcs_workspace_bytes(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), C.c_int(int(exterior))))
 
 
-def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace, _exact_workspace=False, basis=None):
+def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspace, _exact_workspace=False, basis=None,
+              nonblocking=False):
     cs, cb, cp = samples.c(), _basis(bvh, basis), params.c()
     K = basis.K if basis is not None else bvh.V
+    if nonblocking:
+        # mcs_params.nonblocking: the library only enqueues work (no read-back, no allocation), so the call may sit in
+        # a CUDA graph.  The caller owns `out` and `workspace` for as long as the work may run.
+        if want_stats or basis is not None or out is None or workspace is None:
+            raise ValueError("nonblocking=True needs out= and workspace= from the caller, the hat basis and want_stats=False")
+        if workspace.numel() < workspace_bytes(bvh, samples, params, exterior, basis):
+            raise ValueError("workspace too small")
     if out is None:
         out = torch.empty((K, K), dtype=torch.float32, device=bvh.device)
     elif not (isinstance(out, torch.Tensor) and out.is_cuda and out.device == bvh.device and out.dtype == torch.float32
@@ -322,6 +330,7 @@ def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspa
         workspace = torch.empty(need, dtype=torch.uint8, device=bvh.device)
     m = _Matrix(kind=0, K=K, dense=out.data_ptr())
     st = Stats() if want_stats else None
+    cp.nonblocking = 1 if nonblocking else 0
     with torch.cuda.device(bvh.device):
         rc = fn(bvh.handle, C.byref(cs), C.byref(cb), C.byref(cp), _ptr(workspace), C.c_size_t(workspace.numel()),
                 C.byref(m), C.byref(st) if st is not None else None, _stream(bvh.device))
@@ -330,18 +339,19 @@ def _estimate(fn, name, bvh, samples, params, exterior, want_stats, out, workspa
 
 
 def estimate_dtn_interior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
-                          _exact_workspace=False, basis=None):
+                          _exact_workspace=False, basis=None, nonblocking=False):
     """Interior DtN matrix, Alg. 2: dense [K,K] fp32 on the device (K = V, or the number of
-    points of a PointBasis)."""
+    points of a PointBasis).  nonblocking=True (hat basis, caller's out and workspace): only enqueues work on the
+    current stream -- capturable in a CUDA graph; input errors only the device can see then turn the output into NaN."""
     return _estimate(lib().mcs_estimate_dtn_interior, "mcs_estimate_dtn_interior", bvh, samples, params, False,
-                     want_stats, out, workspace, _exact_workspace, basis)
+                     want_stats, out, workspace, _exact_workspace, basis, nonblocking)
 
 
 def estimate_dtn_exterior(bvh: Bvh, samples: Samples, params: Params, want_stats=False, out=None, workspace=None,
-                          _exact_workspace=False, basis=None):
-    """Exterior DtN matrix, Eq. 32."""
+                          _exact_workspace=False, basis=None, nonblocking=False):
+    """Exterior DtN matrix, Eq. 32.  nonblocking: see estimate_dtn_interior."""
     return _estimate(lib().mcs_estimate_dtn_exterior, "mcs_estimate_dtn_exterior", bvh, samples, params, True,
-                     want_stats, out, workspace, _exact_workspace, basis)
+                     want_stats, out, workspace, _exact_workspace, basis, nonblocking)
 
 
 def workspace_bytes_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params, basis=None) -> int:

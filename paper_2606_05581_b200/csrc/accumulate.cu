@@ -439,10 +439,14 @@ expand_entries_kernel(AccArgs a, const PairRec* __restrict__ pairs, const uint32
 __global__ void __launch_bounds__(RT)
 reduce_runs_dense_kernel(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, long long n,
                          float* __restrict__ S, uint32_t* __restrict__ carry_key, float* __restrict__ carry_sum,
-                         unsigned long long* __restrict__ n_unique)
+                         unsigned long long* __restrict__ n_unique, const uint32_t* __restrict__ n_dev)
 {
     __shared__ float s_tail[RT / 32][1];
     __shared__ int s_has_head[RT / 32];
+    if (n_dev) {                                        // length known on the device only: the grid covers the capacity
+        n = (long long)*n_dev;
+        if ((long long)blockIdx.x * RT >= n) { if (threadIdx.x == 0) carry_key[blockIdx.x] = 0xFFFFFFFFu; return; }
+    }
     const long long i = (long long)blockIdx.x * RT + threadIdx.x;
     const bool valid = i < n;
     const uint32_t key = valid ? keys[i] : 0xFFFFFFFFu;
@@ -459,6 +463,8 @@ reduce_runs_dense_kernel(const uint32_t* __restrict__ keys, const uint32_t* __re
     const unsigned m = __ballot_sync(0xFFFFFFFFu, head);
     if (n_unique && (threadIdx.x & 31) == 0 && m) atomicAdd(n_unique, (unsigned long long)__popc(m));
 }
+
+__global__ void add_count_kernel(unsigned long long* __restrict__ total, const uint32_t* __restrict__ n) { *total += *n; }
 
 __global__ void __launch_bounds__(AT)
 carry_fixup_kernel(const uint32_t* __restrict__ carry_key, const float* __restrict__ carry_sum, long long n_tiles,
@@ -703,7 +709,7 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         int rc = kill_prereduce(records, n_main, n_kill, b->F, mface, keys, vals, L.E, carry_key, carry_sum, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
     }
-    unsigned long long entries_total = 0;
+    if (stats_dev) MCS_CUDA_TRY(cudaMemsetAsync(stats_dev + ST_ENTRIES, 0, 8, st));
     // phase 0: the walks of the samples, chunk by chunk; phase 1: one pair record per face from the killing walks
     for (int phase = 0; phase < 2; ++phase)
     for (int64_t j0 = 0, total = phase == 0 ? n_main : (n_kill > 0 ? b->F : 0); j0 < total; j0 += L.C) {
@@ -723,24 +729,22 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
         mcs_note_launch(), count_entries_kernel<<<nblk, AT, 0, st>>>(a, pp, pc, slots, counts);
         int rc = exclusive_scan_u32(counts, counts, slots, counts + slots, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
-        uint32_t n_entries = 0;
-        MCS_CUDA_TRY(cudaMemcpyAsync(&n_entries, counts + slots, 4, cudaMemcpyDeviceToHost, st));
-        MCS_CUDA_TRY(cudaStreamSynchronize(st));
-        if (n_entries == 0) continue;
-        entries_total += n_entries;
+        // The number of entries of the chunk stays on the device (counts[slots]): the sort and the run reduction take
+        // it from there and their grids cover the chunk's capacity (tiles beyond the length exit at once), so the loop
+        // never blocks the host and a call can be captured in a CUDA graph.
+        const uint32_t* n_entries_dev = counts + slots;
+        const long long cap = slots * MAX_ENTRIES_PER_PAIR;
+        if (stats_dev) mcs_note_launch(), add_count_kernel<<<1, 1, 0, st>>>(stats_dev + ST_ENTRIES, n_entries_dev);
         mcs_note_launch(), expand_entries_kernel<uint32_t><<<nblk, AT, 0, st>>>(a, pp, pc, slots, counts, keys, vals);
-        rc = sort_pairs_u32(keys, vals, n_entries, bits, sort_ws, sort_bytes, st);
+        rc = sort_pairs_u32_devn(keys, vals, cap, n_entries_dev, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
-        const long long n_tiles = ceil_div64(n_entries, RT);
+        const long long n_tiles = ceil_div64(cap, RT);
         mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
-            keys, vals, n_entries, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
+            keys, vals, 0, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr, n_entries_dev);
         mcs_note_launch(), carry_fixup_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(carry_key, carry_sum, n_tiles, out->dense);
     }
     mcs_note_launch(), mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);
-    if (stats_dev)
-        MCS_CUDA_TRY(cudaMemcpyAsync(stats_dev + ST_ENTRIES, &entries_total, 8, cudaMemcpyHostToDevice, st));
     MCS_CUDA_TRY(cudaGetLastError());
-    if (stats_dev) MCS_CUDA_TRY(cudaStreamSynchronize(st));     // entries_total lives on this stack frame
     return MCS_OK;
 }
 
@@ -1409,7 +1413,7 @@ int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basi
         if (rc != MCS_OK) return rc;
         const long long n_tiles = ceil_div64(n_entries, RT);
         mcs_note_launch(), reduce_runs_dense_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
-            keys, vals, n_entries, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr);
+            keys, vals, n_entries, out->dense, carry_key, carry_sum, stats_dev ? stats_dev + ST_UNIQUE : nullptr, nullptr);
         mcs_note_launch(), carry_fixup_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(carry_key, carry_sum, n_tiles, out->dense);
     }
     mcs_note_launch(), mirror_kernel<<<(unsigned)ceil_div64(K * K, AT), AT, 0, st>>>(out->dense, K);

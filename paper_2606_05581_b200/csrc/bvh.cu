@@ -464,7 +464,12 @@ static void keep_pool_memory()
 
 void mcs_bvh_touch(const mcs_bvh* b, cudaStream_t st)
 {
-    if (b && b->last_use) cudaEventRecord(b->last_use, st);
+    if (!b || !b->last_use) return;
+    // Under stream capture the record would become a node of the caller's graph and the event could no longer order
+    // mcs_free_bvh: skip it (the caller keeps the handle alive for as long as the graph may run, include/mcdtn.h).
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); return; }
+    if (cs == cudaStreamCaptureStatusNone) cudaEventRecord(b->last_use, st);
 }
 
 // Frees the handle's memory in the order of `st`, which must be a stream the handle's last use is ordered before

@@ -91,6 +91,15 @@ int fail(int rc, mcs_stats* hs)
     return rc;
 }
 
+// A poisoned call (WalkDyn.err, asynchronous path only: nothing is read back, so no error code can be returned) does not
+// leave a plausible matrix behind: the output is filled with NaN.
+__global__ void poison_output_kernel(const WalkDyn* __restrict__ dyn, float* __restrict__ out, long long n)
+{
+    if (!dyn->err) return;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        out[i] = __int_as_float(0x7FC00000);
+}
+
 int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, const mcs_params* p, int exterior,
              void* ws, size_t ws_bytes, const mcs_matrix* out, mcs_stats* hs, void* stream)
 {
@@ -107,11 +116,20 @@ int estimate(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis, con
     float4* records = (float4*)(base + L.records_off);
     unsigned long long* stats_dev = nullptr;
     mcs_prof_mark(MCS_MARK_BEGIN, st);
+    // params.nonblocking (dense output in the hat basis, no host_stats): the call only enqueues work -- nothing is read back, nothing is
+    // allocated, no host memory is copied -- so it returns at once and may be captured in a CUDA graph.
+    // Every other combination blocks (statistics and COO sizes are read back) and reports input errors early.
+    if (p->nonblocking != 0 && (p->nonblocking != 1 || hs || p->output_kind != 0 || basis->kind != 0)) return MCS_EINVAL;
+    const bool async_path = p->nonblocking == 1;
     int rc = walk_run(b, s, p, exterior, base + L.walk_off, align_up(walk_workspace_bytes(s)), records, nullptr,
-                      false, nullptr, hs != nullptr, &stats_dev, st);
+                      false, nullptr, hs != nullptr, &stats_dev, st, nullptr, !async_path);
     if (rc != MCS_OK) return fail(rc, hs);
     rc = acc_run(b, s, basis, p, records, L.n_records, base + L.acc_off,
-                 align_up(acc_ws_bytes(b, s, basis, p, L.n_records)), out, stats_dev, st);
+                 align_up(acc_ws_bytes(b, s, basis, p, L.n_records)), out, async_path ? nullptr : stats_dev, st);
+    if (rc == MCS_OK && async_path) {
+        mcs_note_launch(), poison_output_kernel<<<64, 256, 0, st>>>(walk_dyn_of(stats_dev), out->dense, (long long)out->K * out->K);
+        if (cudaGetLastError() != cudaSuccess) rc = MCS_ECUDA;
+    }
     mcs_bvh_touch(b, st);
     if (rc != MCS_OK) return fail(rc, hs);
     mcs_prof_mark(MCS_MARK_END, st);

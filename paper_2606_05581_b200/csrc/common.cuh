@@ -109,6 +109,10 @@ int sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int key_bits,
                    void* ws, size_t ws_bytes, cudaStream_t st);
 int sort_pairs_u32(uint32_t* keys, uint32_t* vals, int64_t n, int key_bits,
                    void* ws, size_t ws_bytes, cudaStream_t st);
+// The same with the number of pairs known on the device only: *n_dev <= n_cap pairs are sorted; n_cap sizes the grids and the
+// workspace (sort_workspace_bytes(n_cap, 4)).  Never blocks the host.
+int sort_pairs_u32_devn(uint32_t* keys, uint32_t* vals, int64_t n_cap, const uint32_t* n_dev, int key_bits,
+                        void* ws, size_t ws_bytes, cudaStream_t st);
 size_t scan_workspace_bytes(int64_t n);
 // Exclusive prefix sum of uint32 counts into uint64-safe? No: totals fit in
 // int64 on the host side; device array is uint32 (n_entries per chunk < 2^32).

@@ -34,9 +34,17 @@ __device__ __forceinline__ unsigned lanemask_lt()
 
 template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS)
-radix_hist_kernel(const K* __restrict__ keys, int64_t n, int shift, uint32_t* __restrict__ counts, int nblocks)
+radix_hist_kernel(const K* __restrict__ keys, int64_t n, int shift, uint32_t* __restrict__ counts, int nblocks,
+                  const uint32_t* __restrict__ n_dev)
 {
     __shared__ uint32_t hist[256];
+    if (n_dev) {                                        // length known on the device only: the grid covers the capacity
+        n = (int64_t)*n_dev;
+        if ((int64_t)blockIdx.x * SORT_TILE >= n) {
+            if (threadIdx.x < 256) counts[(size_t)threadIdx.x * nblocks + blockIdx.x] = 0;
+            return;
+        }
+    }
     if (threadIdx.x < 256) hist[threadIdx.x] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -60,9 +68,14 @@ template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS)
 radix_scatter_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin,
                      K* __restrict__ kout, uint32_t* __restrict__ vout,
-                     int64_t n, int shift, const uint32_t* __restrict__ offsets, int nblocks)
+                     int64_t n, int shift, const uint32_t* __restrict__ offsets, int nblocks,
+                     const uint32_t* __restrict__ n_dev)
 {
     extern __shared__ __align__(16) unsigned char sort_smem[];
+    if (n_dev) {
+        n = (int64_t)*n_dev;
+        if ((int64_t)blockIdx.x * SORT_TILE >= n) return;
+    }
     K* skey = reinterpret_cast<K*>(sort_smem);                                   // [SORT_TILE]
     uint32_t* sval = reinterpret_cast<uint32_t*>(skey + SORT_TILE);              // [SORT_TILE]
     uint32_t (*cnt)[256] = reinterpret_cast<uint32_t (*)[256]>(sval + SORT_TILE); // [SORT_WARPS][256]
@@ -182,8 +195,23 @@ scan_tile_kernel(const uint32_t* in, uint32_t* out, int64_t n,   // in may alias
     if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_THREADS - 1) *total_out = run;
 }
 
+// the sorted pairs ended up in the alternate buffers: copy them home (length known on the device only)
 template <typename K>
-int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st)
+__global__ void copy_pairs_devn_kernel(const K* __restrict__ kin, const uint32_t* __restrict__ vin, K* __restrict__ kout,
+                                       uint32_t* __restrict__ vout, const uint32_t* __restrict__ n_dev)
+{
+    const int64_t n = (int64_t)*n_dev;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        kout[i] = kin[i];
+        vout[i] = vin[i];
+    }
+}
+
+// n_dev == nullptr: n pairs.  n_dev != nullptr: *n_dev <= n pairs (n is the capacity: it sizes the grids and the
+// workspace; nothing is read back, so the call never blocks the host).
+template <typename K>
+int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st,
+                    const uint32_t* n_dev = nullptr)
 {
     if (n < 0 || key_bits < 0 || key_bits > (int)sizeof(K) * 8) return MCS_EINVAL;
     if (n <= 1 || key_bits == 0) return MCS_OK;
@@ -207,14 +235,17 @@ int radix_sort_impl(K* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, 
     }
     for (int pass = 0; pass < passes; ++pass) {
         int shift = pass * 8;
-        mcs_note_launch(), radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks);
+        mcs_note_launch(), radix_hist_kernel<K><<<nblocks, SORT_THREADS, 0, st>>>(kin, n, shift, counts, nblocks, n_dev);
         int rc = exclusive_scan_u32(counts, counts, (int64_t)256 * nblocks, nullptr, scan_ws, scan_ws_bytes, st);
         if (rc != MCS_OK) return rc;
-        mcs_note_launch(), radix_scatter_kernel<K><<<nblocks, SORT_THREADS, scatter_smem_bytes<K>(), st>>>(kin, vin, kout, vout, n, shift, counts, nblocks);
+        mcs_note_launch(), radix_scatter_kernel<K><<<nblocks, SORT_THREADS, scatter_smem_bytes<K>(), st>>>(kin, vin, kout, vout, n, shift, counts, nblocks, n_dev);
         K* tk = kin; kin = kout; kout = tk;
         uint32_t* tv = vin; vin = vout; vout = tv;
     }
-    if (kin != keys) {
+    if (kin != keys && n_dev) {
+        const unsigned nb = (unsigned)(nblocks < 1184 ? nblocks : 1184);
+        mcs_note_launch(), copy_pairs_devn_kernel<K><<<nb, 512, 0, st>>>(kin, vin, keys, vals, n_dev);
+    } else if (kin != keys) {
         MCS_CUDA_TRY(cudaMemcpyAsync(keys, kin, (size_t)n * sizeof(K), cudaMemcpyDeviceToDevice, st));
         MCS_CUDA_TRY(cudaMemcpyAsync(vals, vin, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
     }
@@ -274,6 +305,13 @@ int sort_pairs_u64(uint64_t* keys, uint32_t* vals, int64_t n, int key_bits, void
 int sort_pairs_u32(uint32_t* keys, uint32_t* vals, int64_t n, int key_bits, void* ws, size_t ws_bytes, cudaStream_t st)
 {
     return radix_sort_impl<uint32_t>(keys, vals, n, key_bits, ws, ws_bytes, st);
+}
+
+int sort_pairs_u32_devn(uint32_t* keys, uint32_t* vals, int64_t n_cap, const uint32_t* n_dev, int key_bits,
+                        void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (!n_dev) return MCS_EINVAL;
+    return radix_sort_impl<uint32_t>(keys, vals, n_cap, key_bits, ws, ws_bytes, st, n_dev);
 }
 
 // ---------------------------------------------------------------------------

@@ -64,6 +64,37 @@ kelvin_bounds_kernel(const float* __restrict__ verts, int64_t V, float3 o, int* 
     }
 }
 
+__global__ void kelvin_bounds_init_kernel(int* __restrict__ out)
+{
+    const int d = threadIdx.x;
+    if (d < 8) out[d] = d < 3 ? 0x7FFFFFFF : (d < 7 ? (int)0x80000000 : 0);
+}
+
+__device__ __forceinline__ float ordered_to_float(int h)
+{
+    return __int_as_float(h >= 0 ? h : h ^ 0x7FFFFFFF);
+}
+
+// r_max (rmax_scale x half the shortest side of the domain's bounding box; exterior: of the box of the
+// Kelvin-inverted vertices) and R_max, written where the later kernels of the call read them.  bounds = the int[8] of
+// kelvin_bounds_kernel (exterior) or unused (interior: `side` comes from the handle's AABB).
+__global__ void walk_dyn_kernel(const int* __restrict__ bounds, int exterior, float side, float rmax_scale, float rmax_override,
+                                WalkDyn* __restrict__ dyn)
+{
+    float Rmax = 0.0f;
+    int err = 0;
+    if (exterior) {
+        float f[7];
+        for (int d = 0; d < 7; ++d) f[d] = ordered_to_float(bounds[d]);
+        side = fminf(f[3] - f[0], fminf(f[4] - f[1], f[5] - f[2]));
+        Rmax = f[6];
+        if (bounds[7] || !(Rmax > 0.0f)) err = WALK_ERR_DEGENERATE;
+    }
+    dyn->rmax = rmax_override > 0.0f ? rmax_override : rmax_scale * (0.5f * side);
+    dyn->Rmax = Rmax;
+    dyn->err = err;
+}
+
 // ---------------------------------------------------------------------------
 // Z-order keys of the sample points ("sort sample points s via
 // Z-order curves, which greatly reduces warp divergence").
@@ -102,7 +133,7 @@ sample_keys_kernel(const float* __restrict__ verts, const int32_t* __restrict__ 
     const int64_t i = (int64_t)blockIdx.x * PT + threadIdx.x;
     if (i >= n_s) return;
     vals[i] = (uint32_t)i;
-    if (tri[i] < 0 || tri[i] >= F) { *err = 1; keys[i] = 0; return; }
+    if (tri[i] < 0 || tri[i] >= F) { atomicOr(err, WALK_ERR_SAMPLE_FACE); keys[i] = 0; return; }
     float3 s, n;
     sample_point(verts, faces, tri, bary, i, s, n);
     const float ex = hi.x - lo.x, ey = hi.y - lo.y, ez = hi.z - lo.z;
@@ -165,13 +196,19 @@ template <bool EXT>
 __global__ void __launch_bounds__(TB_WARPS * 32)
 tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
                     const float* __restrict__ normal, const uint32_t* __restrict__ order, int64_t n_s,
-                    float rmax, float eps, int iters, float3 o, float mesh_scale,
+                    const WalkDyn* __restrict__ dyn, float eps, int iters, float3 o, float mesh_scale,
                     float4* __restrict__ balls, unsigned long long* __restrict__ stats)
 {
     __shared__ int s_nodes[TB_WARPS][TB_NCAP];
     __shared__ int s_leaves[TB_WARPS][TB_LCAP];
     const unsigned FULL = 0xFFFFFFFFu;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    if (dyn->err) {                                   // poisoned call: every sample is discarded (radius 0), no geometry is read
+        for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < 2 * n_s; i += (int64_t)gridDim.x * blockDim.x)
+            balls[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    const float rmax = dyn->rmax;
     const unsigned lt = (1u << lane) - 1u;
     int* nstack = s_nodes[wib];
     int* lstack = s_leaves[wib];
@@ -305,10 +342,12 @@ tangent_ball_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __
 // x = s - inset * n_s.  Written in the layout of the tangent balls: (x, 1), (n, 1).
 __global__ void __launch_bounds__(PT)
 naive_start_kernel(WalkGeom g, const int32_t* __restrict__ tri, const float* __restrict__ bary,
-                   const float* __restrict__ normal, int64_t n_s, float inset, float4* __restrict__ balls)
+                   const float* __restrict__ normal, int64_t n_s, float inset, const WalkDyn* __restrict__ dyn,
+                   float4* __restrict__ balls)
 {
     const int64_t i = (int64_t)blockIdx.x * PT + threadIdx.x;
     if (i >= n_s) return;
+    if (dyn->err) { balls[2 * i] = balls[2 * i + 1] = make_float4(0.f, 0.f, 0.f, 0.f); return; }      // poisoned call
     float3 s, n;
     sample_point(g.verts, g.faces, tri, bary, i, s, n);
     if (normal) n = f3(normal[3 * i], normal[3 * i + 1], normal[3 * i + 2]);
@@ -612,11 +651,11 @@ __device__ __forceinline__ void coop_finish_query(const BvhNode* nodes_unused, c
 #undef EXT_
 #undef FAR_
 
-__global__ void face_slot_lookup_kernel(const int32_t* __restrict__ face_slot, const int32_t* __restrict__ tri,
+__global__ void face_slot_lookup_kernel(const int32_t* __restrict__ face_slot, const int32_t* __restrict__ tri, int64_t F,
                                         int64_t n_s, int32_t* __restrict__ sample_slot)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_s) sample_slot[i] = face_slot[tri[i]];
+    if (i < n_s) sample_slot[i] = (tri[i] >= 0 && tri[i] < F) ? face_slot[tri[i]] : -1;      // out of range: the call is poisoned anyway
 }
 
 __global__ void balls_export_kernel(const float4* __restrict__ balls, int64_t n_s, float* __restrict__ out)
@@ -642,12 +681,25 @@ int check_params(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, in
     if (exterior && p->include_killing && (p->n_kill_walks < 1 || p->n_kill_walks >= ((int64_t)1 << 32))) return MCS_EINVAL;
     if (s->n_s * (int64_t)p->walks_per_sample >= ((int64_t)1 << 40)) return MCS_EINVAL;
     if (!(p->far_alpha >= 0.0f) || p->far_alpha > 4.0f || !(p->far_near_factor >= 0.0f)) return MCS_EINVAL;
+    if (p->nonblocking != 0 && p->nonblocking != 1) return MCS_EINVAL;
     if (p->exterior_query != 0 && p->exterior_query != 1) return MCS_EINVAL;
     if (p->exterior_query == 1 && (!exterior || p->far_alpha > 0.0f)) return MCS_EINVAL;      // E4 is an exterior query; the far-field cut belongs to E3
     return MCS_OK;
 }
 
 }  // namespace
+
+const WalkDyn* walk_dyn_of(const unsigned long long* stats_dev)
+{
+    return reinterpret_cast<const WalkDyn*>(reinterpret_cast<const char*>(stats_dev) + ST_COUNT * 8 + 32);   // behind the 8 scratch ints
+}
+
+int walk_error_code(int err_bits)
+{
+    if (err_bits & WALK_ERR_DEGENERATE) return MCS_EDEGENERATE;
+    if (err_bits & WALK_ERR_SAMPLE_FACE) return MCS_EINVAL;
+    return MCS_OK;
+}
 
 int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior)
 {
@@ -671,7 +723,7 @@ size_t walk_workspace_bytes(const mcs_samples* s)
 // Runs A2-A6.  Layout of `ws`: see walk_workspace_bytes.
 int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
              void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
-             bool count, unsigned long long** stats_dev_out, cudaStream_t st, WalkLaunch* defer)
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st, WalkLaunch* defer, bool check_now)
 {
     int rc = check_params(b, s, p, exterior);
     if (rc != MCS_OK) return rc;
@@ -699,41 +751,24 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     const unsigned nblk_s = (unsigned)ceil_div64(n_s, PT);
     const float mesh_scale = fmaxf(fabsf(lo.x), fabsf(hi.x)) + fmaxf(fabsf(lo.y), fabsf(hi.y)) + fmaxf(fabsf(lo.z), fabsf(hi.z));
 
-    // r_max and, for the exterior, R_max
-    float side = fminf(hi.x - lo.x, fminf(hi.y - lo.y, hi.z - lo.z));
-    float Rmax = 0.0f;
+    // r_max and, for the exterior, R_max: computed on the device and read there (WalkDyn), together with
+    // the input errors only the device can see
+    WalkDyn* dyn = const_cast<WalkDyn*>(walk_dyn_of(stats));
+    const float side = fminf(hi.x - lo.x, fminf(hi.y - lo.y, hi.z - lo.z));
     if (exterior) {
-        int h[8];
-        for (int d = 0; d < 3; ++d) { h[d] = 0x7FFFFFFF; h[3 + d] = (int)0x80000000; }
-        h[6] = (int)0x80000000; h[7] = 0;
-        MCS_CUDA_TRY(cudaMemcpyAsync(ibuf, h, sizeof h, cudaMemcpyHostToDevice, st));
+        mcs_note_launch(), kelvin_bounds_init_kernel<<<1, 32, 0, st>>>(ibuf);
         mcs_note_launch(), kelvin_bounds_kernel<<<(unsigned)ceil_div64(b->V, PT), PT, 0, st>>>(b->verts, b->V, o, ibuf);
-        MCS_CUDA_TRY(cudaMemcpyAsync(h, ibuf, sizeof h, cudaMemcpyDeviceToHost, st));
-        MCS_CUDA_TRY(cudaStreamSynchronize(st));
-        if (h[7]) return MCS_EDEGENERATE;
-        float f[7];
-        for (int d = 0; d < 7; ++d) { int v = h[d] >= 0 ? h[d] : h[d] ^ 0x7FFFFFFF; memcpy(&f[d], &v, 4); }
-        side = fminf(f[3] - f[0], fminf(f[4] - f[1], f[5] - f[2]));
-        Rmax = f[6];
-        if (!(Rmax > 0.0f)) return MCS_EDEGENERATE;
     }
-    const float rmax = p->rmax_override > 0.0f ? p->rmax_override : p->rmax_scale * (0.5f * side);
+    mcs_note_launch(), walk_dyn_kernel<<<1, 1, 0, st>>>(ibuf, exterior, side, p->rmax_scale, p->rmax_override, dyn);
 
     // Z-order of the samples
-    int* err = ibuf + 7;
-    mcs_note_launch(), sample_keys_kernel<<<nblk_s, PT, 0, st>>>(b->verts, b->faces, b->F, s->tri, s->bary, n_s, lo, hi, keys, order, err);
+    mcs_note_launch(), sample_keys_kernel<<<nblk_s, PT, 0, st>>>(b->verts, b->faces, b->F, s->tri, s->bary, n_s, lo, hi, keys, order, &dyn->err);
     rc = sort_pairs_u32(keys, order, n_s, 30, sort_ws, sort_bytes, st);
     if (rc != MCS_OK) return rc;
-    {
-        int h_err = 0;
-        MCS_CUDA_TRY(cudaMemcpyAsync(&h_err, err, 4, cudaMemcpyDeviceToHost, st));
-        MCS_CUDA_TRY(cudaStreamSynchronize(st));
-        if (h_err) return MCS_EINVAL;                 // sample face index out of range
-    }
-    mcs_note_launch(), face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, n_s, sample_slot);
+    mcs_note_launch(), face_slot_lookup_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(b->face_slot, s->tri, b->F, n_s, sample_slot);
 
     if (p->estimator == 1) {
-        mcs_note_launch(), naive_start_kernel<<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, n_s, p->inset, balls);
+        mcs_note_launch(), naive_start_kernel<<<nblk_s, PT, 0, st>>>(g, s->tri, s->bary, s->normal, n_s, p->inset, dyn, balls);
     } else {
         int dev_tb = 0, n_sm_tb = 0;
         MCS_CUDA_TRY(cudaGetDevice(&dev_tb));
@@ -743,10 +778,17 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
         if (nblk_tb > cap_tb) nblk_tb = cap_tb;
         if (exterior)
             mcs_note_launch(), tangent_ball_kernel<true><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
-                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
+                g, s->tri, s->bary, s->normal, order, n_s, dyn, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
         else
             mcs_note_launch(), tangent_ball_kernel<false><<<(unsigned)nblk_tb, TB_WARPS * 32, 0, st>>>(
-                g, s->tri, s->bary, s->normal, order, n_s, rmax, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
+                g, s->tri, s->bary, s->normal, order, n_s, dyn, p->eps, p->bisection_iters, o, mesh_scale, balls, stats);
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    if (check_now) {                                 // one read-back: input errors before the expensive part runs
+        WalkDyn hd;
+        MCS_CUDA_TRY(cudaMemcpyAsync(&hd, dyn, sizeof hd, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (hd.err) return walk_error_code(hd.err);
     }
     if (balls_out) mcs_note_launch(), balls_export_kernel<<<(unsigned)ceil_div64(n_s, 256), 256, 0, st>>>(balls, n_s, balls_out);
     MCS_CUDA_TRY(cudaGetLastError());
@@ -761,7 +803,7 @@ int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int ex
     a.inv_q0 = 1.0f / a.q0;
     a.importance = p->importance_sample; a.antithetic = p->antithetic;
     a.naive = p->estimator == 1; a.inv_inset = p->estimator == 1 ? 1.0f / p->inset : 0.0f;
-    a.ox = o.x; a.oy = o.y; a.oz = o.z; a.Rmax = Rmax;
+    a.ox = o.x; a.oy = o.y; a.oz = o.z; a.dyn = dyn;
     a.mesh_scale = mesh_scale;
     a.far_alpha2 = p->far_alpha * p->far_alpha;
     a.far_near = (p->far_near_factor > 0.0f ? fmaxf(p->far_near_factor, 2.0f) : 16.0f) * p->eps;   // never below 2 eps

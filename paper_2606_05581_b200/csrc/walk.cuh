@@ -20,6 +20,17 @@ struct WalkGeom {
     const int32_t*   faces;
 };
 
+// Values of one call that are computed ON THE DEVICE (so that no call has to read them back before it can go on):
+// r_max of the tangent balls (exterior: from the AABB of the Kelvin-inverted vertices), R_max = max |v - o|
+// (E3), and the input errors only the device can see.  Lives behind the counters of the walk workspace.
+struct WalkDyn {
+    float rmax, Rmax;
+    int   err;                     // WALK_ERR_* bits; non-zero poisons the call: every record is written as discarded
+    int   pad_;
+};
+enum { WALK_ERR_SAMPLE_FACE = 1,   // a sample's face index is outside [0, F)            -> MCS_EINVAL
+       WALK_ERR_DEGENERATE = 2 };  // a vertex at the Kelvin origin, or R_max not > 0     -> MCS_EDEGENERATE
+
 struct WalkArgs {
     const float4*   balls;         // [n_s][2]: (c.xyz, r), (pole.xyz, |s*|)
     const uint32_t* order;         // Z-order permutation of the samples
@@ -31,7 +42,8 @@ struct WalkArgs {
     int   naive;                   // Alg. 1: balls hold the start point, no ball sampling
     float inv_inset;
     float eps, q0, inv_q0;
-    float ox, oy, oz, Rmax;
+    float ox, oy, oz;
+    const WalkDyn* dyn;            // R_max (exterior) and the poison flag, device-resident
     float mesh_scale;              // |coordinates|_1 bound of the mesh (prune_limit)
     float escape;                  // interior: AABB diagonal (R10b); exterior: +inf
     float far_alpha2, far_near;    // far-field lower-bound queries: alpha^2 (0: exact queries only), near threshold k eps
@@ -47,7 +59,14 @@ int64_t walk_num_records(const mcs_samples* s, const mcs_params* p, int exterior
 size_t  walk_workspace_bytes(const mcs_samples* s);
 int walk_run(const mcs_bvh* b, const mcs_samples* s, const mcs_params* p, int exterior,
              void* ws, size_t ws_bytes, float4* records, int32_t* steps, bool balls_only, float* balls_out,
-             bool count, unsigned long long** stats_dev_out, cudaStream_t st, struct WalkLaunch* defer = nullptr);
+             bool count, unsigned long long** stats_dev_out, cudaStream_t st, struct WalkLaunch* defer = nullptr,
+             bool check_now = true);
+// check_now = true: walk_run blocks once, after the preparation, and returns the device-side input errors (MCS_EINVAL for a
+// sample face out of range, MCS_EDEGENERATE for a vertex at the Kelvin origin) before the walk kernel is launched.
+// check_now = false: nothing is read back; a call with such an error is poisoned (all records discarded) and the caller
+// reads the flags later with walk_error_code / from the copy of the counters (walk_dyn_of).
+const WalkDyn* walk_dyn_of(const unsigned long long* stats_dev);
+int walk_error_code(int err_bits);
 
 // A prepared launch of the walk kernel (walk_run with `defer`): everything before the kernel has been
 // enqueued on walk_run's stream; walk_launch may enqueue the kernel on another stream that waits for it.
