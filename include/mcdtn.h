@@ -179,7 +179,7 @@ typedef struct {
                                     query, the EXACT distance from y to the Kelvin-inverted faces = (1/|x|) min
                                     over the mesh of |x - p| / |p - o| (E4): larger balls, fewer jumps, a dearer
                                     query; same estimator.  Not combinable with far_alpha                              */
-    int32_t  nonblocking;        /* mcs_estimate_dtn_interior / _exterior only.  0 (default): the call blocks the host for small
+    int32_t  nonblocking;        /* mcs_estimate_dtn_interior / _exterior / _both (there: in both blocks); ignored elsewhere.  0 (default): the call blocks the host for small
                                     read-backs (below) and returns device-side input errors.  1: the call ONLY ENQUEUES work on
                                     `stream` -- no read-back, no allocation, no copy from host memory -- so it returns at once and
                                     may be captured in a CUDA graph.  Needs output_kind 0, basis kind 0 and host_stats == NULL

@@ -363,11 +363,18 @@ def workspace_bytes_both(bvh: Bvh, samples: Samples, params_interior: Params, pa
 
 
 def estimate_dtn_both(bvh: Bvh, samples: Samples, params_interior: Params, params_exterior: Params, want_stats=False,
-                      out_interior=None, out_exterior=None, workspace=None, basis=None):
+                      out_interior=None, out_exterior=None, workspace=None, basis=None, nonblocking=False):
     """Interior and exterior DtN matrices of one mesh in one call (mcs_estimate_dtn_both): the same results as the
-    two single calls, bit for bit, with the two walk kernels overlapped on two streams."""
+    two single calls, bit for bit, with the two walk kernels overlapped on two streams.  nonblocking: see
+    estimate_dtn_interior (caller's outputs and workspace, hat basis, no statistics)."""
     cs, cb = samples.c(), _basis(bvh, basis)
     ci, ce = params_interior.c(), params_exterior.c()
+    if nonblocking:
+        if want_stats or basis is not None or out_interior is None or out_exterior is None or workspace is None:
+            raise ValueError("nonblocking=True needs out_interior=, out_exterior= and workspace= from the caller, the hat basis and want_stats=False")
+        if workspace.numel() < workspace_bytes_both(bvh, samples, params_interior, params_exterior, basis):
+            raise ValueError("workspace too small")
+        ci.nonblocking = ce.nonblocking = 1
     K = basis.K if basis is not None else bvh.V
     if out_interior is None:
         out_interior = torch.empty((K, K), dtype=torch.float32, device=bvh.device)

@@ -214,6 +214,11 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     if (s->n_s < 1) return MCS_EINVAL;
     if (out_int->kind == out_ext->kind && (out_int->kind == 0 ? out_int->dense == out_ext->dense : out_int->coo_val == out_ext->coo_val))
         return MCS_EINVAL;                            // the two operators run concurrently: separate outputs
+    // params.nonblocking (set in BOTH parameter blocks; dense output, hat basis, no host_stats): enqueue only, as in the
+    // single calls.  The side streams fork from `stream` by an event and join it again, so the whole call can be captured.
+    const bool nb = p_int->nonblocking != 0 || p_ext->nonblocking != 0;
+    if (nb && (p_int->nonblocking != 1 || p_ext->nonblocking != 1 || hs_int || hs_ext || host_int || host_ext ||
+               p_int->output_kind != 0 || p_ext->output_kind != 0 || basis->kind != 0)) return MCS_EINVAL;
     if (!g_both.ensure()) return MCS_ECUDA;
     cudaStream_t st = (cudaStream_t)stream, st1 = g_both.ss[0], st2 = g_both.ss[1];
 
@@ -229,7 +234,7 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     mcs_prof_mark(MCS_MARK_BEGIN, st);
     for (int x = 1; x >= 0; --x) {                    // exterior first: its host read-back happens before anything long runs
         int rc = walk_run(b, s, pp[x], x, base[x] + L[x].walk_off, align_up(walk_workspace_bytes(s)),
-                          (float4*)(base[x] + L[x].records_off), nullptr, false, nullptr, hh[x] != nullptr, &stats_dev[x], st, &wl[x]);
+                          (float4*)(base[x] + L[x].records_off), nullptr, false, nullptr, hh[x] != nullptr, &stats_dev[x], st, &wl[x], !nb);
         if (rc != MCS_OK) return fail(rc, hh[x]);
     }
     // Measured and not kept: both operators' walks as two segments of ONE launch of the batched kernel (no delay kernel, no
@@ -251,7 +256,11 @@ int estimate_both(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basis
     cudaStream_t ss[2] = { st1, st2 };
     for (int x = 0; x < 2 && rc == MCS_OK; ++x)
         rc = acc_run(b, s, basis, pp[x], (const float4*)(base[x] + L[x].records_off), L[x].n_records, base[x] + L[x].acc_off,
-                     align_up(acc_ws_bytes(b, s, basis, pp[x], L[x].n_records)), oo[x], stats_dev[x], ss[x]);
+                     align_up(acc_ws_bytes(b, s, basis, pp[x], L[x].n_records)), oo[x], nb ? nullptr : stats_dev[x], ss[x]);
+    for (int x = 0; x < 2 && rc == MCS_OK && nb; ++x) {
+        mcs_note_launch(), poison_output_kernel<<<64, 256, 0, ss[x]>>>(walk_dyn_of(stats_dev[x]), oo[x]->dense, (long long)oo[x]->K * oo[x]->K);
+        if (cudaGetLastError() != cudaSuccess) rc = MCS_ECUDA;
+    }
     float* host_out[2] = { host_int, host_ext };
     for (int x = 0; x < 2 && rc == MCS_OK; ++x)
         if (host_out[x] && oo[x]->kind == 0) {        // the interior's download runs beside the exterior's accumulation

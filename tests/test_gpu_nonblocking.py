@@ -77,6 +77,31 @@ def test_nonblocking_call_in_a_cuda_graph(api):
             assert torch.equal(out, ref)
 
 
+def test_nonblocking_both_operators_in_one_call_eager_and_in_a_graph(api):
+    v, f, smp, bvh, S = _case(api)
+    (_, Pi), (_, Pe) = _ops(api, S, 128)
+    ref_i, ref_e = api.estimate_dtn_interior(bvh, S, Pi), api.estimate_dtn_exterior(bvh, S, Pe)
+    ws = torch.empty(api.workspace_bytes_both(bvh, S, Pi, Pe), dtype=torch.uint8, device="cuda")
+    oi, oe = torch.zeros_like(ref_i), torch.zeros_like(ref_e)
+    api.estimate_dtn_both(bvh, S, Pi, Pe, out_interior=oi, out_exterior=oe, workspace=ws, nonblocking=True)
+    torch.cuda.synchronize()
+    assert torch.equal(oi, ref_i) and torch.equal(oe, ref_e)
+    oi.zero_(); oe.zero_()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):                              # the library's two side streams fork from and join the captured stream
+        api.estimate_dtn_both(bvh, S, Pi, Pe, out_interior=oi, out_exterior=oe, workspace=ws, nonblocking=True)
+    torch.cuda.synchronize()
+    assert float(oi.abs().sum()) == 0.0
+    for _ in range(2):
+        oi.fill_(-1.0); oe.fill_(-1.0)
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(oi, ref_i) and torch.equal(oe, ref_e)
+    # and the ordinary call still works on the same thread's streams afterwards
+    bi, be = api.estimate_dtn_both(bvh, S, Pi, Pe)
+    assert torch.equal(bi, ref_i) and torch.equal(be, ref_e)
+
+
 def test_nonblocking_input_errors_poison_the_output(api):
     v, f, smp, bvh, S = _case(api, level=1, ppv=2)
     K = len(v)
