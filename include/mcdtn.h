@@ -485,8 +485,15 @@ int mcs_project_galerkin_coo(const int32_t* row, const int32_t* col, const float
  *     S psi = lambda M psi,  M = diag(mass)  (lumped boundary mass),
  * for a batch of `batch` dense symmetric matrices S [batch][K][K] (symmetrised inside) with mass [batch][K] > 0.
  * evals [batch][n_eig] ascending; evecs [batch][n_eig][K] (may be NULL), M-orthonormal: psi_i^T M psi_j = delta_ij.
- * One-sided Jacobi in fp32 on M^-1/2 S M^-1/2 (all eigenpairs are computed; the n_eig smallest are returned).
- * sweeps_out (host, may be NULL): Jacobi sweeps used.  Blocks the host once per sweep (convergence flag).
+ * Two solvers, both fp32 on A = M^-1/2 S M^-1/2.  (1) One-sided Jacobi: all eigenpairs are computed, the n_eig smallest
+ * returned; the only choice for K < 1024.  (2) Chebyshev-filtered subspace iteration for FEW eigenpairs of a LARGE matrix
+ * (K >= 1024, n_eig <= 256, block of n_eig + max(16, n_eig / 4) columns rounded up to 64, at most K / 2): products A X only,
+ * 2 K^2 m flops each, so the lowest 64 modes at K = 2562 take 28 ms instead of 0.52 s and K = 16384 (the paper's 2^14
+ * points) is within reach; residuals |A x - theta x| <= 2e-5 x (Gershgorin bound of A) on exit.
+ * mcs_steklov_eigs chooses: (2) where it applies, and (1) after all if (2) did not converge within its 40 iterations (a
+ * spectrum crowded at its low end).  mcs_steklov_eigs_method: method 0 = that choice, 1 = Jacobi, 2 = subspace iteration
+ * (MCS_EINVAL where it does not apply; MCS_WNOTCONVERGED instead of the fall-back).
+ * sweeps_out (host, may be NULL): Jacobi sweeps or subspace iterations used.  Blocks the host once per sweep / iteration.
  * The solver is made for the symmetric POSITIVE SEMI-DEFINITE matrices of Alg. 2 / Eq. 32: one-sided Jacobi diagonalises
  * A^2, so an indefinite input (Alg. 1, estimator = 1) with eigenvalues +l and -l of equal magnitude can leave mixed
  * vectors.  Returns MCS_WNOTCONVERGED (> 0, results written) when the sweep cap (30) was reached with rotations still
@@ -495,6 +502,9 @@ size_t mcs_steklov_eigs_workspace_bytes(int64_t K, int64_t batch);
 int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig,
                      float* evals, float* evecs, void* workspace, size_t workspace_bytes,
                      int32_t* sweeps_out /* host */, void* stream);
+int mcs_steklov_eigs_method(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig, int32_t method,
+                            float* evals, float* evecs, void* workspace, size_t workspace_bytes,
+                            int32_t* sweeps_out /* host */, void* stream);
 
 /* Roofline denominators measured on this device (bench.py): FP32
  * CUDA-core throughput of independent FMA chains (TFLOP/s, 2 flop per FMA) and the read

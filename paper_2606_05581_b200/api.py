@@ -811,9 +811,11 @@ def estimate_dtn_coo_both(bvh: Bvh, samples: Samples, params_interior: Params, p
     raise McsError(MCS_ENOMEM, "estimate_dtn_coo_both", "capacity retries exhausted")
 
 
-def steklov_eigs(S, mass, n_eig, want_vectors=True):
+def steklov_eigs(S, mass, n_eig, want_vectors=True, method="auto"):
     """Smallest n_eig eigenpairs of S psi = lambda diag(mass) psi (mcs_steklov_eigs).  S: [K,K] or [B,K,K] CUDA fp32;
-    mass: [K] or [B,K].  Returns (evals [B,n_eig] or [n_eig], evecs [B,n_eig,K] or [n_eig,K] or None, sweeps)."""
+    mass: [K] or [B,K].  Returns (evals [B,n_eig] or [n_eig], evecs [B,n_eig,K] or [n_eig,K] or None, sweeps).
+    method: "auto" (subspace iteration for few eigenpairs of a large matrix, else Jacobi), "jacobi", "subspace"."""
+    method_code = {"auto": 0, "jacobi": 1, "subspace": 2}[method]
     S = _dev(S, torch.float32, "S")
     mass = _dev(mass, torch.float32, "mass")
     single = S.ndim == 2
@@ -828,11 +830,12 @@ def steklov_eigs(S, mass, n_eig, want_vectors=True):
     evecs = torch.empty((B, n_eig, K), dtype=torch.float32, device=S.device) if want_vectors else None
     sweeps = C.c_int32(0)
     with torch.cuda.device(S.device):
-        rc = lib().mcs_steklov_eigs(_ptr(S), _ptr(mass), C.c_int64(K), C.c_int64(B), C.c_int32(n_eig), _ptr(evals),
-                                    _ptr(evecs), _ptr(ws), C.c_size_t(need), C.byref(sweeps), _stream(S.device))
+        rc = lib().mcs_steklov_eigs_method(_ptr(S), _ptr(mass), C.c_int64(K), C.c_int64(B), C.c_int32(n_eig), C.c_int32(method_code),
+                                           _ptr(evals), _ptr(evecs), _ptr(ws), C.c_size_t(need), C.byref(sweeps), _stream(S.device))
     if rc == MCS_WNOTCONVERGED:
         import warnings
-        warnings.warn("mcs_steklov_eigs: sweep cap reached before convergence (input not positive semi-definite?)")
+        warnings.warn("mcs_steklov_eigs: iteration cap reached before convergence (input not positive semi-definite, or "
+                      "method='subspace' on a spectrum crowded at its low end?)")
     else:
         _check(rc, "mcs_steklov_eigs")
     if single:

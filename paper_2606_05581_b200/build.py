@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmcdtn.so")
 SOURCES = ["sort.cu", "bvh.cu", "query.cu", "walk.cu", "accumulate.cu", "capi.cu", "peaks.cu", "eigs.cu", "winding.cu", "project.cu"]
-HEADERS = ["common.cuh", "traverse.cuh", "walk.cuh", "walk_body.inc", os.path.join("..", "..", "include", "mcdtn.h")]
+HEADERS = ["common.cuh", "traverse.cuh", "walk.cuh", "walk_body.inc", "sgemm.cuh", os.path.join("..", "..", "include", "mcdtn.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--use_fast_math=false" if False else "-Xcompiler", "-fvisibility=default"]
 

@@ -10,7 +10,9 @@
 // fp32 throughout; Jacobi's rotations are orthogonal to rounding, so eigenvalues are good to ~1e-6 |A|.
 #include "common.cuh"
 
+#include <math.h>
 #include <string.h>
+#include <vector>
 
 namespace {
 
@@ -532,18 +534,307 @@ eig_sort_kernel(uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, int K,
     for (int i = threadIdx.x; i < K; i += blockDim.x) { k[i] = (uint32_t)(s_kv[i] >> 32); v[i] = (uint32_t)s_kv[i]; }
 }
 
+namespace {
+
+// ---------------------------------------------------------------------------
+// Large K, few eigenpairs: Chebyshev-filtered subspace iteration.
+// One-sided Jacobi computes ALL K eigenpairs (O(K^3) per sweep: 0.52 s at K = 2562, out of reach at the 2^14 points of
+// the paper's point-based discretisation); the applications want the lowest 64-128 modes (PAPER.md:357,
+// 401).  For n_eig << K a block X [K][m] (m = n_eig + guard columns) is iterated instead:
+//   filter      Y = p(A) X, p = the degree-d Chebyshev polynomial that is small on [a, b] (the unwanted part of the
+//               spectrum: a = the largest Ritz value of the block, b >= lambda_max by Gershgorin) and grows fast below
+//               a; three-term recurrence, one product A Y per degree, scaled so that nothing overflows;
+//   orthonormalise  G = Y^T Y = V D V^T (m x m, by the Jacobi solver above), Y <- Y V D^-1/2;
+//   Rayleigh-Ritz   H = Y^T A Y = W Theta W^T (m x m, same solver), X <- Y W: Ritz pairs (Theta, X);
+//   stop when the residuals |A x_i - theta_i x_i| of the n_eig lowest pairs are below tol * b.
+// fp32 throughout.  The Gram matrix squares the condition number of Y, and the filter spreads the columns' scales by
+// p(0) / p(a), so the degree is kept low enough (p(0) / p(a) <= ~1e3) for fp32 and the loop runs a few more times.
+// All products are the plain SIMT tiles of sgemm.cuh with split-K (the block is tall and thin: K/64 row tiles alone
+// do not fill 148 SMs); a dense contraction on tensor cores would need TF32 inputs, which the filter tolerates but
+// the Rayleigh-Ritz step does not -- left as fp32 CUDA cores (2 K^2 m flops per product: 1.7 GFLOP at K = 2562).
+// ---------------------------------------------------------------------------
+#include "sgemm.cuh"
+
+// row sums of |A|: Gershgorin bound of the largest eigenvalue (max over rows; non-negative floats order like their bits)
+__global__ void __launch_bounds__(ET)
+sub_gershgorin_kernel(const float* __restrict__ A, long long K, unsigned* __restrict__ bound_bits)
+{
+    __shared__ float s_red[ET / 32];
+    const float* row = A + (long long)blockIdx.x * K;
+    float v = 0.0f;
+    for (long long j = threadIdx.x; j < K; j += ET) v += fabsf(row[j]);
+    v = block_sum(v, s_red);
+    if (threadIdx.x == 0) atomicMax(bound_bits, __float_as_uint(v));
+}
+
+// deterministic start block: a hash of (row, column) mapped to (-1, 1)
+__global__ void sub_init_kernel(float* __restrict__ X, long long n, unsigned seed)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned h = (unsigned)i * 0x9E3779B1u + seed;
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    X[i] = (float)(h >> 8) * (2.0f / 16777216.0f) - 1.0f;
+}
+
+// out = alpha * (P[0] + P[1] + ... in order) + beta * D1 + gamma * D2   (D1, D2 may be NULL; out may alias D2)
+__global__ void sub_combine_kernel(const float* __restrict__ P, int n_z, long long n, float alpha,
+                                   const float* __restrict__ D1, float beta, const float* D2, float gamma, float* out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float s = 0.0f;
+    for (int z = 0; z < n_z; ++z) s += P[(long long)z * n + i];
+    float r = alpha * s;
+    if (D1) r = fmaf(beta, D1[i], r);
+    if (D2) r = fmaf(gamma, D2[i], r);
+    out[i] = r;
+}
+
+// B[j][i] = VT[i][j] * s_i: the eigenvectors of a small problem come as rows (VT[i] = i-th vector); the products above
+// want them as columns, scaled by d_i^-1/2 after the Gram step (scale = NULL: no scaling).  d_i below rel * d_max: the
+// column is dropped (rank-deficient block), its scale is 0.
+__global__ void sub_transpose_scale_kernel(const float* __restrict__ VT, const float* __restrict__ d, int m, int use_scale,
+                                           float* __restrict__ B)
+{
+    const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
+    if (i >= m || j >= m) return;
+    float s = 1.0f;
+    if (use_scale) {
+        const float dmax = d[m - 1];                   // ascending
+        s = d[i] > 1e-10f * dmax ? rsqrtf(d[i]) : 0.0f;
+    }
+    B[(long long)j * m + i] = VT[(long long)i * m + j] * s;
+}
+
+// residual norms: r2[i] = | AX[:, i] - theta_i X[:, i] |^2, one block per column, fixed order
+__global__ void __launch_bounds__(ET)
+sub_residual_kernel(const float* __restrict__ AX, const float* __restrict__ X, const float* __restrict__ theta, long long K, int m,
+                    float* __restrict__ r2)
+{
+    __shared__ float s_red[ET / 32];
+    const int i = blockIdx.x;
+    const float th = theta[i];
+    float v = 0.0f;
+    for (long long k = threadIdx.x; k < K; k += ET) { const float r = fmaf(-th, X[k * m + i], AX[k * m + i]); v = fmaf(r, r, v); }
+    v = block_sum(v, s_red);
+    if (threadIdx.x == 0) r2[i] = v;
+}
+
+// output: eigenvalue e and psi_e = M^-1/2 x_e with the sign rule of eig_vectors_kernel, rows [n_eig][K]
+__global__ void __launch_bounds__(ET)
+sub_output_kernel(const float* __restrict__ X, const float* __restrict__ theta, const float* __restrict__ mass, long long K, int m,
+                  float* __restrict__ evals, float* __restrict__ evecs)
+{
+    __shared__ float s_red[ET / 32];
+    __shared__ float s_sign;
+    const int e = blockIdx.x;
+    float v = 0.0f, n2 = 0.0f;
+    for (long long j = threadIdx.x; j < K; j += ET) { const float q = X[j * m + e]; v += q * q * q; n2 = fmaf(q, q, n2); }
+    v = block_sum(v, s_red); n2 = block_sum(n2, s_red);
+    if (threadIdx.x == 0) { s_sign = (v < 0.0f ? -1.0f : 1.0f) / sqrtf(n2); evals[e] = theta[e]; }
+    __syncthreads();
+    if (!evecs) return;
+    const float sg = s_sign;
+    for (long long j = threadIdx.x; j < K; j += ET) evecs[(long long)e * K + j] = sg * X[j * m + e] * rsqrtf(mass[j]);
+}
+
+__global__ void __launch_bounds__(ET)
+sub_matrix_kernel(const float* __restrict__ S, const float* __restrict__ mass, long long K, float* __restrict__ A)
+{
+    const long long i = (long long)blockIdx.x * ET + threadIdx.x;
+    if (i >= K * K) return;
+    const long long r = i / K, c = i - r * K;
+    A[i] = 0.5f * (S[r * K + c] + S[c * K + r]) * rsqrtf(mass[r]) * rsqrtf(mass[c]);     // as eig_init_kernel
+}
+
+__global__ void sub_fill_kernel(float* __restrict__ x, int n, float v)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) x[i] = v;
+}
+
+constexpr int SUB_MIN_K = 1024;        // below: one-sided Jacobi (all eigenpairs) is as fast
+constexpr int SUB_M_MAX = 320;         // widest block: n_eig <= 256
+constexpr int SUB_MAX_ITERS = 40;
+
+int sub_block_width(int n_eig)
+{
+    const int guard = n_eig / 4 > 16 ? n_eig / 4 : 16;
+    return ((n_eig + guard + 63) / 64) * 64;
+}
+
+int sub_split(long long tiles, long long Kd, int cap)
+{
+    long long nz = (296 + tiles - 1) / tiles;                 // about two blocks per SM
+    const long long by_depth = Kd / 128 > 1 ? Kd / 128 : 1;    // at least 128 of depth per slice
+    if (nz > by_depth) nz = by_depth;
+    if (nz > cap) nz = cap;
+    return nz < 1 ? 1 : (int)nz;
+}
+
+// capacity of the split-K partials: n_z <= 296 / tiles + 1 slices of tiles * 4096 entries each (tall products), or 64 slices
+// of an m x m product
+size_t sub_partial_floats(long long K)
+{
+    const size_t tall = (size_t)297 * 4096 + (size_t)(K + 64) * SUB_M_MAX;
+    const size_t small = (size_t)64 * SUB_M_MAX * SUB_M_MAX;
+    return tall > small ? tall : small;
+}
+
+size_t sub_extra_bytes(long long K)
+{
+    if (K < SUB_MIN_K) return 0;
+    const size_t m = SUB_M_MAX;
+    return align_up(sub_partial_floats(K) * 4) + 5 * align_up((size_t)K * m * 4) + 3 * align_up(m * m * 4) + 6 * align_up(m * 4) + 256
+         + align_up(mcs_steklov_eigs_workspace_bytes(SUB_M_MAX, 1));
+}
+
+struct SubBuffers {
+    float *A, *P, *X, *Y, *Z, *T, *U, *Gm, *VT, *Bm, *d, *theta, *r2, *ones;
+    unsigned* bound;
+    void* small_ws; size_t small_bytes;
+};
+
+// C [M][N] = op(A) B through split-K partials in `P`, then C = the ordered sum of the partials
+template <bool TA>
+int sub_gemm(const float* A, const float* B, float* C, int M, int N, int Kd, int n_z, float* P, cudaStream_t st)
+{
+    const int k_per_z = (int)(ceil_div64(ceil_div64(Kd, n_z), GK) * GK);
+    const dim3 g((unsigned)ceil_div64(N, GT), (unsigned)ceil_div64(M, GT), (unsigned)n_z);
+    mcs_note_launch(), sgemm_kernel<TA><<<g, 256, 0, st>>>(A, B, n_z == 1 ? C : P, M, N, Kd, k_per_z);
+    if (n_z > 1) {
+        const long long n = (long long)M * N;
+        mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(P, n_z, n, 1.0f, nullptr, 0.0f, nullptr, 0.0f, C);
+    }
+    MCS_CUDA_TRY(cudaGetLastError());
+    return MCS_OK;
+}
+
+// Y <- Y V D^-1/2 with Y^T Y = V D V^T (result in `out`); `Y` is left as it was
+int sub_orthonormalise(const float* Y, float* out, long long K, int m, const SubBuffers& w, cudaStream_t st)
+{
+    const int nz_small = sub_split((long long)(m / 64) * (m / 64), K, 64);
+    int rc = sub_gemm<true>(Y, Y, w.Gm, m, m, (int)K, nz_small, w.P, st);
+    if (rc != MCS_OK) return rc;
+    rc = mcs_steklov_eigs_method(w.Gm, w.ones, m, 1, m, 1, w.d, w.VT, w.small_ws, w.small_bytes, nullptr, st);
+    if (rc < 0) return rc;
+    const dim3 gt((unsigned)ceil_div64(m, 16), (unsigned)ceil_div64(m, 16));
+    mcs_note_launch(), sub_transpose_scale_kernel<<<gt, dim3(16, 16), 0, st>>>(w.VT, w.d, m, 1, w.Bm);
+    return sub_gemm<false>(Y, w.Bm, out, (int)K, m, m, 1, w.P, st);
+}
+
+// Smallest n_eig eigenpairs of ONE matrix.  evals [n_eig], evecs [n_eig][K] or NULL.  Returns MCS_OK, MCS_WNOTCONVERGED or an error.
+int sub_eigs_one(const float* S, const float* mass, long long K, int n_eig, float* evals, float* evecs,
+                 const SubBuffers& w, int* iters_out, cudaStream_t st)
+{
+    const int m = sub_block_width(n_eig);
+    const long long n = K * (long long)m;
+    mcs_note_launch(), sub_matrix_kernel<<<(unsigned)ceil_div64(K * K, ET), ET, 0, st>>>(S, mass, K, w.A);
+    MCS_CUDA_TRY(cudaMemsetAsync(w.bound, 0, 4, st));
+    mcs_note_launch(), sub_gershgorin_kernel<<<(unsigned)K, ET, 0, st>>>(w.A, K, w.bound);
+    mcs_note_launch(), sub_fill_kernel<<<(unsigned)ceil_div64(m, 256), 256, 0, st>>>(w.ones, m, 1.0f);
+    mcs_note_launch(), sub_init_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(w.Y, n, 0x1234567u);
+    float b = 0.0f;
+    MCS_CUDA_TRY(cudaMemcpyAsync(&b, w.bound, 4, cudaMemcpyDeviceToHost, st));
+    MCS_CUDA_TRY(cudaStreamSynchronize(st));
+    if (!(b > 0.0f) || !(b < 3.0e38f)) {               // the zero matrix (every vector is an eigenvector) or a non-finite entry
+        if (!(b == 0.0f)) return MCS_EINVAL;
+        b = 1.0f;
+    }
+    b *= 1.01f;
+    const int nz_tall = sub_split((long long)(m / 64) * ceil_div64(K, 64), K, 8);
+    const int nz_small = sub_split((long long)(m / 64) * (m / 64), K, 64);
+    if ((size_t)nz_tall * K * m > sub_partial_floats(K) || (size_t)nz_small * m * m > sub_partial_floats(K)) return MCS_ENOMEM;
+    const dim3 gt((unsigned)ceil_div64(m, 16), (unsigned)ceil_div64(m, 16));
+    std::vector<float> theta((size_t)m), r2((size_t)m);
+    const float tol = 2.0e-5f;
+    float a = 0.0f, a_low = 0.0f;
+    bool converged = false;
+    int it = 0;
+    for (; it <= SUB_MAX_ITERS; ++it) {
+        if (it > 0) {
+            // ---- filter: Y = p(A) X, scaled three-term recurrence (X, Y, T rotate) ----
+            const float e = 0.5f * (b - a), c = 0.5f * (b + a);
+            const float x0 = (c - a_low) / e;                                        // > 1: where the wanted end of the spectrum sits
+            int deg = (int)(7.6 / acosh((double)x0));                                // p(a_low) / p(a) <= ~1e3 (fp32 Gram step)
+            deg = deg < 4 ? 4 : (deg > 40 ? 40 : deg);
+            float sigma = e / (a_low - c);
+            const float sigma1 = sigma;
+            float *px = w.X, *py = w.Y, *pt = w.T;
+            // py = (sigma1 / e) (A px - c px)
+            {
+                const int k_per_z = (int)(ceil_div64(ceil_div64(K, nz_tall), GK) * GK);
+                const dim3 g((unsigned)(m / 64), (unsigned)ceil_div64(K, GT), (unsigned)nz_tall);
+                mcs_note_launch(), sgemm_kernel<false><<<g, 256, 0, st>>>(w.A, px, w.P, (int)K, m, (int)K, k_per_z);
+                mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(w.P, nz_tall, n, sigma1 / e, px, -c * sigma1 / e, nullptr, 0.0f, py);
+                for (int i = 2; i <= deg; ++i) {
+                    const float sigma2 = 1.0f / (2.0f / sigma1 - sigma);
+                    // pt = 2 (sigma2 / e) (A py - c py) - sigma sigma2 px
+                    mcs_note_launch(), sgemm_kernel<false><<<g, 256, 0, st>>>(w.A, py, w.P, (int)K, m, (int)K, k_per_z);
+                    mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(
+                        w.P, nz_tall, n, 2.0f * sigma2 / e, py, -2.0f * c * sigma2 / e, px, -sigma * sigma2, pt);
+                    float* t = px; px = py; py = pt; pt = t;
+                    sigma = sigma2;
+                }
+            }
+            MCS_CUDA_TRY(cudaGetLastError());
+            if (py != w.Y) MCS_CUDA_TRY(cudaMemcpyAsync(w.Y, py, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+        }
+        // ---- orthonormalise Y, twice (the Gram matrix squares the condition number; the second pass starts near I) ----
+        int rc = sub_orthonormalise(w.Y, w.U, K, m, w, st);
+        if (rc == MCS_OK) rc = sub_orthonormalise(w.U, w.Y, K, m, w, st);
+        if (rc != MCS_OK) return rc;
+        // ---- Rayleigh-Ritz: Z = A Y, H = Y^T Z = W Theta W^T, X = Y W, AX = Z W ----
+        rc = sub_gemm<false>(w.A, w.Y, w.Z, (int)K, m, (int)K, nz_tall, w.P, st);
+        if (rc == MCS_OK) rc = sub_gemm<true>(w.Y, w.Z, w.Gm, m, m, (int)K, nz_small, w.P, st);
+        if (rc != MCS_OK) return rc;
+        rc = mcs_steklov_eigs_method(w.Gm, w.ones, m, 1, m, 1, w.theta, w.VT, w.small_ws, w.small_bytes, nullptr, st);
+        if (rc < 0) return rc;
+        mcs_note_launch(), sub_transpose_scale_kernel<<<gt, dim3(16, 16), 0, st>>>(w.VT, w.theta, m, 0, w.Bm);
+        rc = sub_gemm<false>(w.Y, w.Bm, w.X, (int)K, m, m, 1, w.P, st);
+        if (rc == MCS_OK) rc = sub_gemm<false>(w.Z, w.Bm, w.U, (int)K, m, m, 1, w.P, st);
+        if (rc != MCS_OK) return rc;
+        mcs_note_launch(), sub_residual_kernel<<<(unsigned)m, ET, 0, st>>>(w.U, w.X, w.theta, K, m, w.r2);
+        MCS_CUDA_TRY(cudaMemcpyAsync(theta.data(), w.theta, (size_t)m * 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaMemcpyAsync(r2.data(), w.r2, (size_t)m * 4, cudaMemcpyDeviceToHost, st));
+        MCS_CUDA_TRY(cudaStreamSynchronize(st));
+        float worst = 0.0f;
+        for (int i = 0; i < n_eig; ++i) worst = fmaxf(worst, sqrtf(fmaxf(r2[(size_t)i], 0.0f)));
+        if (!(worst == worst)) return MCS_EINVAL;                                        // NaN: non-finite input
+        if (it > 0 && worst <= tol * b) { converged = true; ++it; break; }
+        a = theta[(size_t)m - 1];
+        a_low = theta[0] < 0.0f ? theta[0] : 0.0f;
+        if (!(a > a_low + 1e-6f * b)) a = a_low + 1e-6f * b;                             // a flat block: keep the interval proper
+        if (a > 0.999f * b) a = 0.999f * b;
+    }
+    if (iters_out) *iters_out = it;
+    mcs_note_launch(), sub_output_kernel<<<(unsigned)n_eig, ET, 0, st>>>(w.X, w.theta, mass, K, m, evals, evecs);
+    MCS_CUDA_TRY(cudaGetLastError());
+    return converged ? MCS_OK : MCS_WNOTCONVERGED;
+}
+
+}  // namespace
+
 extern "C" size_t mcs_steklov_eigs_workspace_bytes(int64_t K, int64_t batch)
 {
     if (K < 1 || batch < 1) return 0;
     const size_t n = (size_t)batch * K;
     return 2 * align_up((size_t)batch * K * K * 4) + align_up(n * 4) * 3 + align_up(sort_workspace_bytes(K, 4)) +
-           align_up((size_t)batch * 4) + 1024;
+           align_up((size_t)batch * 4) + 1024 + sub_extra_bytes(K);
 }
 
 extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig,
                                 float* evals, float* evecs, void* ws, size_t ws_bytes, int32_t* sweeps_out, void* stream)
 {
+    return mcs_steklov_eigs_method(S, mass, K, batch, n_eig, 0, evals, evecs, ws, ws_bytes, sweeps_out, stream);
+}
+
+extern "C" int mcs_steklov_eigs_method(const float* S, const float* mass, int64_t K, int64_t batch, int32_t n_eig, int32_t method,
+                                       float* evals, float* evecs, void* ws, size_t ws_bytes, int32_t* sweeps_out, void* stream)
+{
     if (!S || !mass || !evals || K < 1 || batch < 1 || n_eig < 1 || n_eig > K || K > 16384) return MCS_EINVAL;
+    if (method < 0 || method > 2) return MCS_EINVAL;
     if (!ws || ws_bytes < mcs_steklov_eigs_workspace_bytes(K, batch)) return MCS_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
     char* p = (char*)ws;
@@ -554,7 +845,39 @@ extern "C" int mcs_steklov_eigs(const float* S, const float* mass, int64_t K, in
     uint32_t* vals = (uint32_t*)p;  p += align_up((size_t)batch * K * 4);
     void* sort_ws = p;              p += align_up(sort_workspace_bytes(K, 4));
     unsigned* scale_bits = (unsigned*)p; p += align_up((size_t)batch * 4);
-    unsigned* flag = (unsigned*)p;
+    unsigned* flag = (unsigned*)p;  p += 1024;
+
+    // Few eigenpairs of a large matrix: subspace iteration, one matrix after the other (see above)
+    const bool sub_ok = K >= SUB_MIN_K && n_eig <= 256 && 2 * (int64_t)sub_block_width(n_eig) <= K;
+    if (method == 2 && !sub_ok) return MCS_EINVAL;
+    if (sub_ok && method != 1) {
+        const size_t mm = SUB_M_MAX;
+        SubBuffers w;
+        w.A = G;
+        w.P = (float*)p;  p += align_up(sub_partial_floats(K) * 4);
+        float** tall[5] = { &w.X, &w.Y, &w.Z, &w.T, &w.U };
+        for (float** t : tall) { *t = (float*)p; p += align_up((size_t)K * mm * 4); }
+        w.Gm = (float*)p; p += align_up(mm * mm * 4);
+        w.VT = (float*)p; p += align_up(mm * mm * 4);
+        w.Bm = (float*)p; p += align_up(mm * mm * 4);
+        float** vec[4] = { &w.d, &w.theta, &w.r2, &w.ones };
+        for (float** t : vec) { *t = (float*)p; p += align_up(mm * 4); }
+        w.bound = (unsigned*)p; p += align_up(mm * 4) * 2 + 256;
+        w.small_ws = p; w.small_bytes = mcs_steklov_eigs_workspace_bytes(SUB_M_MAX, 1);
+        int worst_rc = MCS_OK, iters = 0;
+        for (int64_t bi = 0; bi < batch; ++bi) {
+            int it_b = 0;
+            const int rc = sub_eigs_one(S + bi * K * K, mass + bi * K, K, n_eig, evals + bi * n_eig, evecs ? evecs + bi * n_eig * K : nullptr,
+                                        w, &it_b, st);
+            if (rc < 0) return rc;
+            if (rc > worst_rc) worst_rc = rc;
+            if (it_b > iters) iters = it_b;
+        }
+        if (sweeps_out) *sweeps_out = iters;
+        // automatic choice: a spectrum the filter cannot separate within its iteration cap (eigenvalues crowded at the low
+        // end) falls through to the Jacobi solver below, which does not care
+        if (worst_rc == MCS_OK || method == 2) return worst_rc;
+    }
 
     const dim3 g_init((unsigned)ceil_div64(K * K, ET), (unsigned)batch);
     mcs_note_launch(), eig_init_kernel<<<g_init, ET, 0, st>>>(S, mass, K, G, Q);

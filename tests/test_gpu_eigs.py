@@ -53,10 +53,10 @@ def test_random_spd_pencils(api, K, n_eig):
     A = rng.normal(size=(K, K + 3))
     S = (A @ A.T / K).astype(np.float32)
     m = rng.uniform(0.3, 2.0, K).astype(np.float32)
-    lam, psi, sweeps = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig)
+    lam, psi, sweeps = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig, method="jacobi")
     assert 1 <= sweeps < 30 or K == 1
     _check(S, m, lam.cpu().numpy().astype(np.float64), psi.cpu().numpy().astype(np.float64), n_eig)
-    lam2, none, _ = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig, want_vectors=False)
+    lam2, none, _ = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig, want_vectors=False, method="jacobi")
     assert none is None and torch.equal(lam, lam2)                                     # values do not depend on the vector output
 
 
@@ -67,7 +67,7 @@ def test_large_matrix_takes_the_row_pair_path(api):
     Q, _ = np.linalg.qr(rng.normal(size=(K, K)))
     S = ((Q * (2.0 * np.sqrt(np.arange(K)))) @ Q.T).astype(np.float32)
     m = np.ones(K, np.float32)
-    lam, psi, sweeps = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig)
+    lam, psi, sweeps = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig, method="jacobi")
     assert sweeps < 30
     _check(S, m, lam.cpu().numpy().astype(np.float64), psi.cpu().numpy().astype(np.float64), n_eig)
 
@@ -119,6 +119,72 @@ def test_spectrum_of_an_estimated_dtn_matrix(api):
     _check(S.cpu().numpy(), mass.astype(np.float32), lam.cpu().numpy().astype(np.float64), psi.cpu().numpy().astype(np.float64), 9)
     lam = lam.cpu().numpy()
     assert abs(lam[0]) < 0.05 and np.all(np.abs(lam[1:4] - 1) < 0.25) and np.all(np.abs(lam[4:9] - 2) < 0.5)
+
+
+def _check_subspace(S, m, lam, psi, n_eig, tol_rel=1e-4):
+    """Subspace iteration stops on residuals (2e-5 of the Gershgorin bound), so its bars are set from the matrix scale:
+    eigenvalues to tol_rel * scale (second order in the residual), vectors as subspaces of near eigenvalues."""
+    S = np.asarray(S, np.float64); m = np.asarray(m, np.float64)
+    wa, Va = steklov_eigpairs(S, m, len(S))
+    scale = np.abs(wa).max()
+    assert np.abs(lam - wa[:n_eig]).max() < tol_rel * scale
+    assert np.all(np.diff(lam) >= 0)
+    assert np.abs((psi * m) @ psi.T - np.eye(n_eig)).max() < 5e-5                      # M-orthonormal
+    Ssym = 0.5 * (S + S.T)
+    res = Ssym @ psi.T - (m[:, None] * psi.T) * lam[None, :]
+    assert np.abs(np.linalg.norm(res / np.sqrt(m)[:, None], axis=0)).max() < 1e-3 * scale
+    for e in range(n_eig):
+        near = np.abs(wa - lam[e]) < 2e-2 * scale
+        c = (Va[near] * m) @ psi[e]
+        assert abs(np.linalg.norm(c) - 1) < 2e-3
+
+
+@pytest.mark.parametrize("K,n_eig,kind", [(1024, 16, "sqrt"), (1500, 64, "sqrt"), (2562, 40, "sphere"), (1300, 100, "sqrt")])
+def test_subspace_iteration_for_few_eigenpairs_of_a_large_matrix(api, K, n_eig, kind):
+    """DtN-like spectra: lambda_n ~ sqrt(n) (a surface: eigenvalue l has multiplicity ~ 2l + 1), or exactly the sphere's
+    l with multiplicity 2l + 1 -- whole multiplets inside and across the end of the block."""
+    rng = np.random.default_rng(K + n_eig)
+    Q, _ = np.linalg.qr(rng.normal(size=(K, K)))
+    if kind == "sqrt":
+        w = np.sqrt(np.arange(K))
+    else:
+        w = np.floor(np.sqrt(np.arange(K))).astype(np.float64)                          # 0, 1 x3, 2 x5, 3 x7, ...
+    S = ((Q * w) @ Q.T).astype(np.float32)
+    m = rng.uniform(0.5, 2.0, K).astype(np.float32)
+    Sg, mg = torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda()
+    lam, psi, iters = api.steklov_eigs(Sg, mg, n_eig, method="subspace")
+    assert 1 <= iters <= 40
+    _check_subspace(S, m, lam.cpu().numpy().astype(np.float64), psi.cpu().numpy().astype(np.float64), n_eig)
+    # deterministic, the automatic choice takes the same path, and the values do not depend on the vector output
+    lam2, psi2, _ = api.steklov_eigs(Sg, mg, n_eig)
+    assert torch.equal(lam, lam2) and torch.equal(psi, psi2)
+    lam3, none, _ = api.steklov_eigs(Sg, mg, n_eig, want_vectors=False, method="subspace")
+    assert none is None and torch.equal(lam, lam3)
+    # against the Jacobi solver of the same library
+    lam_j, _, _ = api.steklov_eigs(Sg, mg, n_eig, method="jacobi", want_vectors=False)
+    assert (lam - lam_j).abs().max().item() < 1e-4 * float(np.abs(w).max())
+
+
+def test_subspace_iteration_batch_and_fallback(api):
+    rng = np.random.default_rng(3)
+    K, n_eig, B = 1100, 20, 2
+    S = np.empty((B, K, K), np.float32); m = rng.uniform(0.5, 2.0, (B, K)).astype(np.float32)
+    for b in range(B):
+        Q, _ = np.linalg.qr(rng.normal(size=(K, K)))
+        S[b] = ((Q * np.sqrt((b + 1.0) * np.arange(K))) @ Q.T).astype(np.float32)
+    lam, psi, _ = api.steklov_eigs(torch.from_numpy(S).cuda(), torch.from_numpy(m).cuda(), n_eig, method="subspace")
+    for b in range(B):
+        _check_subspace(S[b], m[b], lam[b].cpu().numpy().astype(np.float64), psi[b].cpu().numpy().astype(np.float64), n_eig)
+    # where subspace iteration does not apply it is refused; the automatic choice takes Jacobi there
+    with pytest.raises(api.McsError):
+        api.steklov_eigs(torch.eye(512, device="cuda"), torch.ones(512, device="cuda"), 8, method="subspace")
+    with pytest.raises(api.McsError):
+        api.steklov_eigs(torch.from_numpy(S[0]).cuda(), torch.from_numpy(m[0]).cuda(), 600, method="subspace")
+    # a spectrum crowded at its low end (Wishart): whatever the filter achieves, the automatic choice returns converged pairs
+    A = rng.normal(size=(K, K + 3))
+    W = (A @ A.T / K).astype(np.float32)
+    lam_a, psi_a, _ = api.steklov_eigs(torch.from_numpy(W).cuda(), torch.from_numpy(m[0]).cuda(), 8)
+    _check(W, m[0], lam_a.cpu().numpy().astype(np.float64), psi_a.cpu().numpy().astype(np.float64), 8)
 
 
 def test_argument_errors(api):
