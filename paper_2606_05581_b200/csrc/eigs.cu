@@ -544,11 +544,13 @@ namespace {
 //   filter      Y = p(A) X, p = the degree-d Chebyshev polynomial that is small on [a, b] (the unwanted part of the
 //               spectrum: a = the largest Ritz value of the block, b >= lambda_max by Gershgorin) and grows fast below
 //               a; three-term recurrence, one product A Y per degree, scaled so that nothing overflows;
-//   orthonormalise  G = Y^T Y = V D V^T (m x m, by the Jacobi solver above), Y <- Y V D^-1/2;
+//   orthonormalise  shifted Cholesky QR, three passes: G = Y^T Y (+ shift) = R^T R in one block, Y <- Y R^-1;
 //   Rayleigh-Ritz   H = Y^T A Y = W Theta W^T (m x m, same solver), X <- Y W: Ritz pairs (Theta, X);
 //   stop when the residuals |A x_i - theta_i x_i| of the n_eig lowest pairs are below tol * b.
 // fp32 throughout.  The Gram matrix squares the condition number of Y, and the filter spreads the columns' scales by
 // p(0) / p(a), so the degree is kept low enough (p(0) / p(a) <= ~1e3) for fp32 and the loop runs a few more times.
+// (A first version orthonormalised through the eigen-decomposition of the Gram matrix, twice per iteration: three
+// 1 ms Jacobi solves of an m x m matrix per iteration were 55 % of the run; Cholesky QR leaves one.)
 // All products are the plain SIMT tiles of sgemm.cuh with split-K (the block is tall and thin: K/64 row tiles alone
 // do not fill 148 SMs); a dense contraction on tensor cores would need TF32 inputs, which the filter tolerates but
 // the Rayleigh-Ritz step does not -- left as fp32 CUDA cores (2 K^2 m flops per product: 1.7 GFLOP at K = 2562).
@@ -639,6 +641,77 @@ sub_output_kernel(const float* __restrict__ X, const float* __restrict__ theta, 
     for (long long j = threadIdx.x; j < K; j += ET) evecs[(long long)e * K + j] = sg * X[j * m + e] * rsqrtf(mass[j]);
 }
 
+// Cholesky G = L L^T of an m x m Gram matrix and Linv = L^-1 (written to global memory, full rows, zeros above the
+// diagonal), one block.  SMEM: L and Linv live in shared memory as packed lower triangles (m <= 192: 2 x 74 KB);
+// otherwise everything stays in global memory (slow, m up to 320 only).  shift_rel > 0 adds shift_rel * trace(G) to the
+// diagonal first (shifted Cholesky QR: the first pass on a block whose Gram matrix is numerically singular in fp32);
+// pivots are clamped at 1e-12 of the largest diagonal entry.
+template <bool SMEM>
+__global__ void __launch_bounds__(1024)
+sub_chol_inv_kernel(float* __restrict__ G, int m, float shift_rel, float* __restrict__ Linv)
+{
+    extern __shared__ float s_tri[];
+    __shared__ float s_red[32];
+    __shared__ float s_piv, s_floor;
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int tri = m * (m + 1) / 2;
+    float* L = SMEM ? s_tri : G;                     // element (i, k), k <= i
+    float* X = SMEM ? s_tri + tri : Linv;            // Linv while it is built
+#define LIDX(i, k) (SMEM ? ((i) * ((i) + 1) / 2 + (k)) : ((i) * m + (k)))
+    if (SMEM) {
+        for (int e = tid; e < m * m; e += T) { const int i = e / m, k = e - i * m; if (k <= i) L[LIDX(i, k)] = G[e]; }
+        __syncthreads();
+    }
+    {
+        float tr = 0.0f, mx = 0.0f;
+        for (int i = tid; i < m; i += T) { const float d = L[LIDX(i, i)]; tr += d; mx = fmaxf(mx, d); }
+        for (int o = 16; o > 0; o >>= 1) { tr += __shfl_xor_sync(0xFFFFFFFFu, tr, o); mx = fmaxf(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o)); }
+        if ((tid & 31) == 0) s_red[tid >> 5] = tr;
+        __syncthreads();
+        float trace = 0.0f;
+        for (int w = 0; w < (T + 31) / 32; ++w) trace += s_red[w];
+        __syncthreads();
+        if ((tid & 31) == 0) s_red[tid >> 5] = mx;
+        __syncthreads();
+        float dmax = 0.0f;
+        for (int w = 0; w < (T + 31) / 32; ++w) dmax = fmaxf(dmax, s_red[w]);
+        if (tid == 0) s_floor = 1e-12f * dmax;
+        const float sh = shift_rel * trace;
+        if (sh > 0.0f) for (int i = tid; i < m; i += T) L[LIDX(i, i)] += sh;
+    }
+    for (int j = 0; j < m; ++j) {
+        __syncthreads();
+        if (tid == 0) { const float piv = sqrtf(fmaxf(L[LIDX(j, j)], s_floor)); L[LIDX(j, j)] = piv; s_piv = piv; }
+        __syncthreads();
+        const float inv = 1.0f / s_piv;
+        for (int i = j + 1 + tid; i < m; i += T) L[LIDX(i, j)] *= inv;
+        __syncthreads();
+        // trailing update of the lower triangle: a warp takes rows, its lanes the columns of a row
+        const int warp = tid >> 5, lane = tid & 31, n_warps = T >> 5;
+        for (int i = j + 1 + warp; i < m; i += n_warps) {
+            const float lij = L[LIDX(i, j)];
+            for (int k = j + 1 + lane; k <= i; k += 32) L[LIDX(i, k)] = fmaf(-lij, L[LIDX(k, j)], L[LIDX(i, k)]);
+        }
+    }
+    __syncthreads();
+    // Linv: thread c solves L x = e_c for column c
+    for (int c = tid; c < m; c += T) {
+        X[LIDX(c, c)] = 1.0f / L[LIDX(c, c)];
+        for (int i = c + 1; i < m; ++i) {
+            float acc = 0.0f;
+            for (int k = c; k < i; ++k) acc = fmaf(L[LIDX(i, k)], X[LIDX(k, c)], acc);
+            X[LIDX(i, c)] = -acc / L[LIDX(i, i)];
+        }
+    }
+    __syncthreads();
+    if (SMEM) {
+        for (int e = tid; e < m * m; e += T) { const int i = e / m, k = e - i * m; Linv[e] = k <= i ? X[LIDX(i, k)] : 0.0f; }
+    } else {
+        for (int e = tid; e < m * m; e += T) { const int i = e / m, k = e - i * m; if (k > i) Linv[e] = 0.0f; }
+    }
+#undef LIDX
+}
+
 __global__ void __launch_bounds__(ET)
 sub_matrix_kernel(const float* __restrict__ S, const float* __restrict__ mass, long long K, float* __restrict__ A)
 {
@@ -677,7 +750,7 @@ int sub_split(long long tiles, long long Kd, int cap)
 // of an m x m product
 size_t sub_partial_floats(long long K)
 {
-    const size_t tall = (size_t)297 * 4096 + (size_t)(K + 64) * SUB_M_MAX;
+    const size_t tall = (size_t)297 * TT * TT + (size_t)(K + TT) * (SUB_M_MAX + TT);
     const size_t small = (size_t)64 * SUB_M_MAX * SUB_M_MAX;
     return tall > small ? tall : small;
 }
@@ -711,16 +784,26 @@ int sub_gemm(const float* A, const float* B, float* C, int M, int N, int Kd, int
     return MCS_OK;
 }
 
-// Y <- Y V D^-1/2 with Y^T Y = V D V^T (result in `out`); `Y` is left as it was
-int sub_orthonormalise(const float* Y, float* out, long long K, int m, const SubBuffers& w, cudaStream_t st)
+// One pass of Cholesky QR: out = Y R^-1 with Y^T Y (+ shift) = R^T R.  Three passes, the first one shifted, orthonormalise a
+// block whose Gram matrix has a condition number up to ~1/eps^2... in exact terms: pass 1 brings cond(Y) down to ~1e3,
+// pass 2 leaves an orthogonality error of ~cond^2 eps, pass 3 of ~eps (shifted Cholesky QR3).  `Y` is left as it was.
+int sub_cholqr_pass(const float* Y, float* out, long long K, int m, float shift_rel, const SubBuffers& w, cudaStream_t st)
 {
     const int nz_small = sub_split((long long)(m / 64) * (m / 64), K, 64);
     int rc = sub_gemm<true>(Y, Y, w.Gm, m, m, (int)K, nz_small, w.P, st);
     if (rc != MCS_OK) return rc;
-    rc = mcs_steklov_eigs_method(w.Gm, w.ones, m, 1, m, 1, w.d, w.VT, w.small_ws, w.small_bytes, nullptr, st);
-    if (rc < 0) return rc;
+    if (m <= 192) {
+        static bool attr_set = false;
+        if (!attr_set) {
+            MCS_CUDA_TRY(cudaFuncSetAttribute(sub_chol_inv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 192 * 193 * 4));
+            attr_set = true;
+        }
+        mcs_note_launch(), sub_chol_inv_kernel<true><<<1, 1024, (size_t)m * (m + 1) * 4, st>>>(w.Gm, m, shift_rel, w.VT);
+    } else {
+        mcs_note_launch(), sub_chol_inv_kernel<false><<<1, 1024, 0, st>>>(w.Gm, m, shift_rel, w.VT);
+    }
     const dim3 gt((unsigned)ceil_div64(m, 16), (unsigned)ceil_div64(m, 16));
-    mcs_note_launch(), sub_transpose_scale_kernel<<<gt, dim3(16, 16), 0, st>>>(w.VT, w.d, m, 1, w.Bm);
+    mcs_note_launch(), sub_transpose_scale_kernel<<<gt, dim3(16, 16), 0, st>>>(w.VT, w.d, m, 0, w.Bm);      // R^-1 = (L^-1)^T
     return sub_gemm<false>(Y, w.Bm, out, (int)K, m, m, 1, w.P, st);
 }
 
@@ -743,7 +826,7 @@ int sub_eigs_one(const float* S, const float* mass, long long K, int n_eig, floa
         b = 1.0f;
     }
     b *= 1.01f;
-    const int nz_tall = sub_split((long long)(m / 64) * ceil_div64(K, 64), K, 8);
+    const int nz_tall = sub_split(ceil_div64(m, TT) * ceil_div64(K, TT), K, 8);
     const int nz_small = sub_split((long long)(m / 64) * (m / 64), K, 64);
     if ((size_t)nz_tall * K * m > sub_partial_floats(K) || (size_t)nz_small * m * m > sub_partial_floats(K)) return MCS_ENOMEM;
     const dim3 gt((unsigned)ceil_div64(m, 16), (unsigned)ceil_div64(m, 16));
@@ -764,14 +847,14 @@ int sub_eigs_one(const float* S, const float* mass, long long K, int n_eig, floa
             float *px = w.X, *py = w.Y, *pt = w.T;
             // py = (sigma1 / e) (A px - c px)
             {
-                const int k_per_z = (int)(ceil_div64(ceil_div64(K, nz_tall), GK) * GK);
-                const dim3 g((unsigned)(m / 64), (unsigned)ceil_div64(K, GT), (unsigned)nz_tall);
-                mcs_note_launch(), sgemm_kernel<false><<<g, 256, 0, st>>>(w.A, px, w.P, (int)K, m, (int)K, k_per_z);
+                const int k_per_z = (int)(ceil_div64(ceil_div64(K, nz_tall), TK) * TK);
+                const dim3 g((unsigned)ceil_div64(m, TT), (unsigned)ceil_div64(K, TT), (unsigned)nz_tall);
+                mcs_note_launch(), sgemm_tall_kernel<<<g, 256, 0, st>>>(w.A, px, w.P, (int)K, m, (int)K, k_per_z);
                 mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(w.P, nz_tall, n, sigma1 / e, px, -c * sigma1 / e, nullptr, 0.0f, py);
                 for (int i = 2; i <= deg; ++i) {
                     const float sigma2 = 1.0f / (2.0f / sigma1 - sigma);
                     // pt = 2 (sigma2 / e) (A py - c py) - sigma sigma2 px
-                    mcs_note_launch(), sgemm_kernel<false><<<g, 256, 0, st>>>(w.A, py, w.P, (int)K, m, (int)K, k_per_z);
+                    mcs_note_launch(), sgemm_tall_kernel<<<g, 256, 0, st>>>(w.A, py, w.P, (int)K, m, (int)K, k_per_z);
                     mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(
                         w.P, nz_tall, n, 2.0f * sigma2 / e, py, -2.0f * c * sigma2 / e, px, -sigma * sigma2, pt);
                     float* t = px; px = py; py = pt; pt = t;
@@ -781,12 +864,19 @@ int sub_eigs_one(const float* S, const float* mass, long long K, int n_eig, floa
             MCS_CUDA_TRY(cudaGetLastError());
             if (py != w.Y) MCS_CUDA_TRY(cudaMemcpyAsync(w.Y, py, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
         }
-        // ---- orthonormalise Y, twice (the Gram matrix squares the condition number; the second pass starts near I) ----
-        int rc = sub_orthonormalise(w.Y, w.U, K, m, w, st);
-        if (rc == MCS_OK) rc = sub_orthonormalise(w.U, w.Y, K, m, w, st);
+        // ---- orthonormalise Y: shifted Cholesky QR, three passes (Y -> U -> Z -> Y) ----
+        int rc = sub_cholqr_pass(w.Y, w.U, K, m, 3.0e-6f, w, st);
+        if (rc == MCS_OK) rc = sub_cholqr_pass(w.U, w.Z, K, m, 0.0f, w, st);
+        if (rc == MCS_OK) rc = sub_cholqr_pass(w.Z, w.Y, K, m, 0.0f, w, st);
         if (rc != MCS_OK) return rc;
         // ---- Rayleigh-Ritz: Z = A Y, H = Y^T Z = W Theta W^T, X = Y W, AX = Z W ----
-        rc = sub_gemm<false>(w.A, w.Y, w.Z, (int)K, m, (int)K, nz_tall, w.P, st);
+        {
+            const int k_per_z = (int)(ceil_div64(ceil_div64(K, nz_tall), TK) * TK);
+            const dim3 g((unsigned)ceil_div64(m, TT), (unsigned)ceil_div64(K, TT), (unsigned)nz_tall);
+            mcs_note_launch(), sgemm_tall_kernel<<<g, 256, 0, st>>>(w.A, w.Y, w.P, (int)K, m, (int)K, k_per_z);
+            mcs_note_launch(), sub_combine_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, st>>>(w.P, nz_tall, n, 1.0f, nullptr, 0.0f, nullptr, 0.0f, w.Z);
+            rc = cudaGetLastError() == cudaSuccess ? MCS_OK : MCS_ECUDA;
+        }
         if (rc == MCS_OK) rc = sub_gemm<true>(w.Y, w.Z, w.Gm, m, m, (int)K, nz_small, w.P, st);
         if (rc != MCS_OK) return rc;
         rc = mcs_steklov_eigs_method(w.Gm, w.ones, m, 1, m, 1, w.theta, w.VT, w.small_ws, w.small_bytes, nullptr, st);
