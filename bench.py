@@ -618,9 +618,14 @@ def run_ours(args):
     roofline["peak_source"] = (f"HBM {hbm_gbs:.0f} GB/s {hbm_src}: packed tree + triangles are {tree_bytes / 1e6:.0f} MB > L2; "
                                f"FP32 {fp32_tflops:.1f} TFLOP/s and L2 {l2_gbs:.0f} GB/s measured live")
     roofline["l2_frac"] = roofline["algorithmic_bytes_per_step"] / (l2_gbs * 1e9) / t_kernel
-    roofline["traffic"] = read_traffic("r02_cfg3_walk_traffic.csv")          # no such capture: ncu returned the interior launch only
-    roofline["traffic_note"] = ("null: ncu --set full gave counters for the interior launch only (profiles/r02_cfg3_walk_kernel.md: 18.9 GB of DRAM "
-                                "traffic at W = 1024 against 150 GB of algorithmic bytes -- the tree is served by L2, hit rate 87 %)")
+    # DRAM bytes of the two walk launches of one step from the committed ncu pass (profiles/r02_cfg3_walk_dram.md), which was
+    # taken at the default workload: any other size has no capture
+    default_wl = (args.faces == 2_000_000 and args.samples == 20_000 and args.walks == 4096 and args.components == 30
+                  and args.mesh_seed == 3 and abs(args.far_alpha - 0.5) < 1e-9 and abs(args.eps - 1e-3) < 1e-12)
+    roofline["traffic"] = read_traffic("r02_cfg3_walk_traffic.csv") if default_wl else None
+    roofline["traffic_note"] = ("dram__bytes_read.sum + dram__bytes_write.sum of the interior and the exterior launch of one step (ncu, "
+                                "profiles/r02_cfg3_walk_dram.md): 2 % of the algorithmic bytes -- the tree is served by L2 (2740 GB of L2 traffic)"
+                                if default_wl else "null: the committed capture is of the default workload")
     roofline["kernel_share_of_step"] = t_kernel * 1e3 / ms_per_step
     cut = (st_i.n_truncated + st_e.n_truncated) / float(st_i.n_walks + st_e.n_walks)
 
