@@ -443,14 +443,23 @@ enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
 // and the best hit is a warp arg-min under the tie rule (smaller d2, then smaller face index).  The
 // result is the same minimum the lane would have found; the order of the traversal does not matter.
 // ---------------------------------------------------------------------------
+// Thresholds measured on BASELINE config 3 at W = 1024 (walk kernels only): interior, exact queries (28 nodes per query on
+// average): 24 -> 99.7 ms, 32 -> 96.8, 40 -> 98.4; exterior with the far-field cut (24 nodes per query on average): 24 ->
+// 158.9 ms, 32 -> 140.5, 40 -> 134.3, 48 -> 133.7, 56 -> 133.2, 64 -> 134.2, 80 -> 135.8, 96 -> 138.5.  At 24 the take-over
+// fired for every query above the exterior's MEAN length -- a warp-wide pass for what one lane finishes in a few visits; it
+// belongs to the tail.  (Results do not depend on the threshold: the cooperative path finds the same minimum.)
 #ifndef COOP_MIN_NODES
-#define COOP_MIN_NODES 24
+#define COOP_MIN_NODES 32
+#endif
+#ifndef COOP_MIN_EXT_NODES
+#define COOP_MIN_EXT_NODES 56
 #endif
 #ifndef COOP_MIN_MERGED_NODES
 #define COOP_MIN_MERGED_NODES 8
 #endif
 constexpr int COOP_MIN_MERGED = COOP_MIN_MERGED_NODES;     // the same in the merged-pass variant (small jobs: idle lanes are free)
 constexpr int COOP_MIN = COOP_MIN_NODES;                      // nodes visited by a lane's query before the warp takes it over
+constexpr int COOP_MIN_EXT = COOP_MIN_EXT_NODES;              // the same for the exterior operator
 // Capacities.  Nodes: a 32-node pass runs only while ncount <= COOP_SOFT, so it leaves at most COOP_SOFT - 32 + 128
 // = 480 entries; above COOP_SOFT the warp goes depth-first (one node per pass: net +3 per level of the wide tree,
 // whose depth is at most (63 + log2 F) / 2 < 48), so ncount < 480 + 3 * 48 = 624 < COOP_NCAP.  Leaves: the lane's
