@@ -80,7 +80,7 @@ def cfg3_config(wl, args, extra=None):
                      f"{n_s} FPS samples of {args.candidates} candidates x {args.walks} walks per operator, interior + exterior "
                      f"(killing off: the paper's default, PAPER.md:383), sidedness pre-pass, hat basis, sparse COO output, "
                      f"eps={args.eps:g}, cap={args.cap:g} deg, Philox seed {args.seed}, "
-                     + (f"exterior far-field queries by lower bound (far_alpha={args.far_alpha:g}, near={args.far_near:g} eps), interior exact" if args.far_alpha > 0 else "exact closest-point queries"),
+                     + (f"far-field queries by lower bound (far_alpha: exterior {args.far_alpha:g}, interior {args.far_alpha_interior:g}; near={args.far_near:g} eps)" if args.far_alpha > 0 or args.far_alpha_interior > 0 else "exact closest-point queries"),
          "operators": ["interior", "exterior"], "walks_per_operator": n_s * args.walks,
          "includes_bvh_build": True, "includes_sidedness_prepass": True, "output": "coo (upper triangle)",
          "l2_policy": "inputs larger than L2 (tree 256 MB + records 2.6 GB per step) and a 256 MiB buffer written between timed steps",
@@ -439,7 +439,7 @@ def bench_cfg4_sample(api, torch, dev, args, seed, n_meshes, flush):
     Si = torch.empty((n_meshes, K, K), dtype=torch.float32, device=dev)
     Se = torch.empty_like(Si)
     mass = torch.empty((n_meshes, K), dtype=torch.float32, device=dev)
-    Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3)
+    Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, far_alpha=args.far_alpha_interior, far_near_factor=args.far_near)
     Pe = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, far_alpha=args.far_alpha, far_near_factor=args.far_near)
 
     def one_pass():
@@ -480,7 +480,7 @@ def bench_cfg4_sample(api, torch, dev, args, seed, n_meshes, flush):
     faces = [len(m["f"]) for m in meshes]
     return {"workload": f"configs[4] sample: {n_meshes} stress-style meshes (seeds 0..{n_meshes - 1}, {min(faces)}-{max(faces)} faces), per mesh: "
                         f"upload from pinned host memory, LBVH build, sidedness pre-pass, 512 FPS samples = nodes of the k-NN point basis "
-                        f"(k=8, face normals at the nodes), {W} walks per sample, interior + exterior (killing off; exterior far-field bound as "
+                        f"(k=8, face normals at the nodes), {W} walks per sample, interior + exterior (killing off; far-field bounds as "
                         f"in the headline) through ONE mcs_estimate_dtn_batch call ({args.cfg4_workers} workers prepare and accumulate, one launch walks "
                         f"all meshes), then top-{n_eig} Steklov eigenpairs of all {2 * n_meshes} matrices in one batched call",
             "metric": "meshes_per_s", "value": n_meshes / (ms * 1e-3), "unit": "meshes/s", "ms_per_mesh": ms / n_meshes,
@@ -515,9 +515,12 @@ def run_ours(args):
     tri_h, bary_h, w_h = (torch.as_tensor(wl[k]).pin_memory() for k in ("tri", "bary", "weight"))
     vd, fd = v_h.to(dev), f_h.to(dev)
     S0 = api.Samples(tri_h.to(dev), bary_h.to(dev), w_h.to(dev))
-    # far-field queries by lower bound for the EXTERIOR only: its walkers spend their time far from the surface (31-41 %
-    # of its queries are answered by a bound); the interior's do not (6 %), and there the exact query is as fast
-    P_int = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap)
+    # far-field queries by a lower bound of the distance in both operators (F1; any ball inside the domain is a
+    # valid walk-on-spheres jump): the walks take more, cheaper jumps and land with the same distribution.
+    # The exact-query step (far_alpha = 0) is measured next to it as a sub-record.
+    P_int0 = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap)
+    P_int = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap,
+                       far_alpha=args.far_alpha_interior, far_near_factor=args.far_near)
     P_ext = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, kelvin_origin=wl["origin"],
                        far_alpha=args.far_alpha, far_near_factor=args.far_near)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -621,7 +624,8 @@ def run_ours(args):
     # DRAM bytes of the two walk launches of one step from the committed ncu pass (profiles/r02_cfg3_walk_dram.md), which was
     # taken at the default workload: any other size has no capture
     default_wl = (args.faces == 2_000_000 and args.samples == 20_000 and args.walks == 4096 and args.components == 30
-                  and args.mesh_seed == 3 and abs(args.far_alpha - 0.5) < 1e-9 and abs(args.eps - 1e-3) < 1e-12)
+                  and args.mesh_seed == 3 and abs(args.far_alpha - 2.0) < 1e-9 and abs(args.far_alpha_interior - 1.0) < 1e-9
+                  and abs(args.far_near - 2.0) < 1e-9 and abs(args.eps - 1e-3) < 1e-12)
     roofline["traffic"] = read_traffic("r02_cfg3_walk_traffic.csv") if default_wl else None
     roofline["traffic_note"] = ("dram__bytes_read.sum + dram__bytes_write.sum of the interior and the exterior launch of one step (ncu, "
                                 "profiles/r02_cfg3_walk_dram.md): 2 % of the algorithmic bytes -- the tree is served by L2 (2740 GB of L2 traffic)"
@@ -656,7 +660,7 @@ def run_ours(args):
             roofline["ideal_exact_traversal"] = {"error": repr(exc)}
 
     sub = {}
-    if world == 1 and not args.no_sub and args.far_alpha > 0:
+    if world == 1 and not args.no_sub and (args.far_alpha > 0 or args.far_alpha_interior > 0):
         # the same step with EXACT closest-point queries in both operators (far_alpha = 0), for comparison
         P_ext0 = api.Params(seed=seed, walks_per_sample=W, eps=args.eps, cap_half_angle_deg=args.cap, kelvin_origin=wl["origin"])
         sc0 = {}
@@ -664,7 +668,7 @@ def run_ours(args):
         def step0():
             bvh = api.build_bvh(vd, fd)
             nrm, _ = api.orient_samples_fast(bvh, S0, beta=args.orient_beta) if args.orient_beta > 0 else api.orient_samples(bvh, S0)
-            api.estimate_dtn_coo_both(bvh, api.Samples(S0.tri, S0.bary, S0.weight, nrm), P_int, P_ext0, capacity=int(cap * 1.05), scratch=sc0)
+            api.estimate_dtn_coo_both(bvh, api.Samples(S0.tri, S0.bary, S0.weight, nrm), P_int0, P_ext0, capacity=int(cap * 1.05), scratch=sc0)
         for _ in range(2):
             step0(); flush.fill_(1)
         n0 = max(1, min(args.steps, 3))
@@ -678,13 +682,16 @@ def run_ours(args):
         bvh0 = api.build_bvh(vd, fd)
         nrm0, _ = api.orient_samples_fast(bvh0, S0, beta=args.orient_beta) if args.orient_beta > 0 else api.orient_samples(bvh0, S0)
         _, st_e0 = api.run_walks(bvh0, api.Samples(S0.tri, S0.bary, S0.weight, nrm0), P_ext0, True, want_stats=True)[1:]
+        _, st_i0 = api.run_walks(bvh0, api.Samples(S0.tri, S0.bary, S0.weight, nrm0), P_int0, False, want_stats=True)[1:]
         del bvh0, nrm0
         sc0.clear()
         torch.cuda.empty_cache()
-        steps0 = st_i.n_steps + st_e0.n_steps
+        steps0 = st_i0.n_steps + st_e0.n_steps
         sub["configs[3] exact queries"] = {"workload": "the headline step with far_alpha = 0 in both operators (every closest-point query exact)",
                                            "metric": METRIC, "value": steps0 / (ms0 * 1e-3), "unit": UNIT, "ms_per_step": ms0, "steps": n0,
                                            "walk_steps_per_step": steps0, "dtn_matrices_per_s": 2.0 / (ms0 * 1e-3),
+                                           "interior_nodes_per_query": (st_i0.n_nodes_visited - st_i0.n_prep_nodes) / max(st_i0.n_queries - st_i0.n_prep_queries, 1),
+                                           "interior_tris_per_query": (st_i0.n_tris_tested - st_i0.n_prep_tris) / max(st_i0.n_queries - st_i0.n_prep_queries, 1),
                                            "exterior_nodes_per_query": (st_e0.n_nodes_visited - st_e0.n_prep_nodes) / max(st_e0.n_queries - st_e0.n_prep_queries, 1),
                                            "exterior_tris_per_query": (st_e0.n_tris_tested - st_e0.n_prep_tris) / max(st_e0.n_queries - st_e0.n_prep_queries, 1)}
     if world == 1 and not args.no_sub:
@@ -699,6 +706,9 @@ def run_ours(args):
             "walk_steps_per_step": steps_per_step, "queries_per_step": queries_per_step,
             "nnz": {"interior": nnz[0], "exterior": nnz[1]},
             "far_query_fraction": (st_i.n_far_queries + st_e.n_far_queries) / float(max(queries_per_step, 1)),
+            "far_field_note": ("value counts the jumps the walks really take; with far-field bounds they take more, shorter ones than the exact "
+                               "run for the same matrices in distribution (tests/test_gpu_farfield.py), so ms_per_step / dtn_matrices_per_s "
+                               "compare configurations, and value_exact_equivalent = (jumps of the exact-query run of sub_records) / (this step's time)"),
             "cut_fraction": cut, "cut_walks": {"interior": st_i.n_truncated, "exterior": st_e.n_truncated,
                                                "rule": "R10 max_steps / R10b left the bounding box / R10c inside the solid (DESIGN.md section 2)"},
             "discarded_samples": {"interior": st_i.n_discarded, "exterior": st_e.n_discarded},
@@ -714,6 +724,8 @@ def run_ours(args):
                     "ms_per_step": e2e_t * 1e3, "ms_per_call": e2e_each, "steps": e2e_steps,
                     "call": "mcs_estimate_dtn_host_coo (pinned host buffers: mesh + samples up, COO entries of both operators down)"},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "sub_records": sub}
+    ex = sub.get("configs[3] exact queries")
+    line["value_exact_equivalent"] = (world * ex["walk_steps_per_step"] / (ms_per_step * 1e-3)) if ex else None
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -736,8 +748,9 @@ def main():
     ap.add_argument("--cap", type=float, default=2.5)
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--orient-beta", type=float, default=2.5, help="sidedness pre-pass: opening parameter of mcs_orient_samples_fast (0: exhaustive mcs_orient_samples)")
-    ap.add_argument("--far-alpha", type=float, default=0.5, help="mcs_params.far_alpha: > 0 answers far-field queries with a lower bound of the distance")
-    ap.add_argument("--far-near", type=float, default=4.0, help="mcs_params.far_near_factor (multiples of eps)")
+    ap.add_argument("--far-alpha", type=float, default=2.0, help="mcs_params.far_alpha of the exterior: > 0 answers far-field queries with a lower bound of the distance")
+    ap.add_argument("--far-alpha-interior", type=float, default=1.0, help="mcs_params.far_alpha of the interior (0: exact queries)")
+    ap.add_argument("--far-near", type=float, default=2.0, help="mcs_params.far_near_factor (multiples of eps)")
     ap.add_argument("--cpu-samples", type=int, default=16, help="sample points of the cpu_baseline leg")
     ap.add_argument("--cpu-walks", type=int, default=8, help="walks per sample point of the cpu_baseline leg")
     ap.add_argument("--ref-samples", type=int, default=8, help="sample points per step of --impl reference")
