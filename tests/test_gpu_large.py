@@ -206,3 +206,70 @@ def test_config3_sparse_matrix_entries_against_the_oracle_on_a_sample_subset(api
         out_norm = np.sqrt((coo2.val.cpu().numpy()[~inside].astype(np.float64) ** 2).sum())
         assert out_norm <= 0.2 * np.linalg.norm(So), (out_norm, np.linalg.norm(So))
         assert np.linalg.norm(S2 - So) <= np.linalg.norm(se) + 0.05 * np.linalg.norm(So)
+
+
+def test_config3_in_the_bench_configuration_far_field_bounds_against_exact_queries(api):
+    """BASELINE config 3 as bench.py times it: the 2 M-face stress mesh, 20 000 FPS samples, hierarchical sidedness,
+    both operators in one sparse call, far-field lower bounds (interior far_alpha 1, exterior 2, near 2 eps), at the full
+    4096 walks per sample.  Properties that hold at any size -- sorted upper-triangular entries without duplicates, the
+    interior matrix annihilating constants, bit-identical reruns -- and the far-field estimator against the exact-query
+    one on quadratic forms of smooth functions: 4 independent seeds each at 512 walks (same mean within the spread of the
+    difference), and the two full-size runs within that spread scaled by sqrt(512 / 4096)."""
+    import argparse
+    import dataclasses
+    from bench import make_cfg3
+    args = argparse.Namespace(faces=2_000_000, components=30, samples=20_000, candidates=1_000_000, mesh_seed=3, no_cache=False)
+    wl = make_cfg3(args)
+    v = wl["v"]
+    bvh = api.build_bvh(torch.as_tensor(v).cuda(), torch.as_tensor(wl["f"]).cuda())
+    S0 = api.Samples.from_arrays(wl["tri"], wl["bary"], wl["weight"])
+    nrm, _ = api.orient_samples_fast(bvh, S0, beta=2.5)
+    S = api.Samples(S0.tri, S0.bary, S0.weight, nrm)
+    far = (dict(far_alpha=1.0, far_near_factor=2.0), dict(far_alpha=2.0, far_near_factor=2.0))
+    exact = (dict(), dict())
+    xs = torch.as_tensor(np.stack([v[:, 0], v[:, 1], v[:, 2], v[:, 0] * v[:, 1], np.sin(3.0 * v[:, 2]), np.ones(len(v))], 1)).cuda().double()
+
+    def run(kinds, W, seed, scratch):
+        Pi = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, **kinds[0])
+        Pe = api.Params(seed=seed, walks_per_sample=W, eps=1e-3, kelvin_origin=wl["origin"], **kinds[1])
+        return api.estimate_dtn_coo_both(bvh, S, Pi, Pe, scratch=scratch)
+
+    def forms(coo):
+        r, c, val = coo.row.long(), coo.col.long(), coo.val.double()
+        w = torch.where(r == c, 1.0, 2.0).double() * val
+        return (w[:, None] * xs[r] * xs[c]).sum(0).cpu().numpy()
+
+    # ---- full size, the bench's own call
+    sc = {}
+    ci, ce = run(far, 4096, 0, sc)
+    keep = [(m.row.clone(), m.col.clone(), m.val.clone()) for m in (ci, ce)]
+    for m in (ci, ce):
+        r, c = m.row.long(), m.col.long()
+        assert m.nnz > 10_000_000 and bool((r <= c).all()) and int(c.max()) < len(v)
+        key = r * len(v) + c
+        assert bool((key[1:] > key[:-1]).all())                               # sorted by (row, col), one entry per position
+        assert bool(torch.isfinite(m.val).all())
+    q_far = [forms(ci), forms(ce)]
+    # interior: S 1 = 0 (PAPER.md:385), row by row against the row's absolute sum
+    r, c, val = ci.row.long(), ci.col.long(), ci.val.double()
+    off = r != c
+    rs = torch.zeros(len(v), dtype=torch.float64, device="cuda").index_add_(0, r, val).index_add_(0, c[off], val[off])
+    ra = torch.zeros(len(v), dtype=torch.float64, device="cuda").index_add_(0, r, val.abs()).index_add_(0, c[off], val[off].abs())
+    assert float((rs.abs() / ra.clamp_min(1e-30)).max()) < 1e-4
+    assert abs(q_far[0][5]) < 1e-4 * float(ci.val.abs().sum())                # the constant's quadratic form
+    ci2, ce2 = run(far, 4096, 0, sc)                                          # bit-identical rerun (same buffers: compare with the copies)
+    for m, k in zip((ci2, ce2), keep):
+        assert torch.equal(m.row, k[0]) and torch.equal(m.col, k[1]) and torch.equal(m.val, k[2])
+    cxi, cxe = run(exact, 4096, 0, sc)
+    q_exact = [forms(cxi), forms(cxe)]
+    # ---- independent seeds at 512 walks: the two estimators have the same mean
+    R = 4
+    qf = np.array([[forms(m) for m in run(far, 512, 100 + s, sc)] for s in range(R)])        # [R][2][6]
+    qx = np.array([[forms(m) for m in run(exact, 512, 200 + s, sc)] for s in range(R)])
+    sd = np.sqrt(qf.std(0, ddof=1) ** 2 + qx.std(0, ddof=1) ** 2)                               # spread of one difference
+    scale = np.abs(qx.mean(0)) + 1e-12
+    for op in range(2):
+        for k in range(5):                                                                      # the five non-constant functions
+            assert abs(qf[:, op, k].mean() - qx[:, op, k].mean()) <= 5.0 * sd[op, k] / np.sqrt(R) + 1e-3 * scale[op, k], (op, k)
+            # full size, same seed in both runs: inside the spread of two independent full-size runs
+            assert abs(q_far[op][k] - q_exact[op][k]) <= 5.0 * sd[op, k] * np.sqrt(512.0 / 4096.0) + 1e-3 * scale[op, k], (op, k)
