@@ -394,7 +394,13 @@ constexpr int WALK_MIN_BLOCKS = 8;                  // 64 registers per thread; 
 #ifndef WALK_COOP_BLOCKS
 #define WALK_COOP_BLOCKS 5
 #endif
-constexpr int WSTACK = 16;                       // shared-memory stack entries per lane
+// Shared-memory stack entries per lane (the rest of a deep stack lives in local memory).  BASELINE config 3 (tree depth 41),
+// walks of both operators at W = 1024: 12 -> 186.7 ms, 16 -> 179.6, 20 -> 175.8, 24 -> 174.4, 28 -> 173.4, 32 -> 175.8;
+// configs[1] (depth 14) is flat up to 24 and loses 3-5 % at 28-32 (8 blocks per SM: the stacks take the L1's room).
+#ifndef MCS_WSTACK
+#define MCS_WSTACK 24
+#endif
+constexpr int WSTACK = MCS_WSTACK;
 constexpr int CUR_NONE = INT_MIN;
 #ifndef VOTE_NODE
 #define VOTE_NODE 8
@@ -433,6 +439,7 @@ __device__ __forceinline__ void stack_pop(LaneStack& st, int& sp, int& ref, floa
 }
 
 enum { KIND_IDLE = 0, KIND_NODE = 1, KIND_TRI = 2, KIND_TRANS = 3 };
+
 
 // ---------------------------------------------------------------------------
 // Warp-cooperative completion of ONE heavy query.  A query that has already visited COOP_MIN nodes
