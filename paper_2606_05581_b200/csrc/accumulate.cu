@@ -33,7 +33,10 @@ constexpr int CH = 256;                               // record slots per level-
 constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << 22;
 // Sparse output: the running list of unique entries is re-sorted with every chunk's new entries, so fewer, larger chunks
 // pay (B200: 180 GB; a 16 Mi-walk chunk takes about 17 GB of workspace per operator at BASELINE config 3's sizes).
-constexpr int64_t MAX_CHUNK_WALKS_COO = (int64_t)1 << 24;
+#ifndef MCS_COO_CHUNK_LOG2
+#define MCS_COO_CHUNK_LOG2 24
+#endif
+constexpr int64_t MAX_CHUNK_WALKS_COO = (int64_t)1 << MCS_COO_CHUNK_LOG2;
 constexpr int MAX_ENTRIES_PER_PAIR = 21;              // upper triangle of a 6 x 6 block
 constexpr int RT = 1024;                              // entries per tile of the run reduction
 
