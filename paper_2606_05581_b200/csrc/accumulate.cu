@@ -759,6 +759,66 @@ int accumulate_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* basi
 // ---------------------------------------------------------------------------
 namespace {
 
+// ---------------------------------------------------------------------------
+// Stable merge of two sorted (key, value) lists, A before B on equal keys: out = the sequence a stable sort of the
+// concatenation A | B would give.  The running list of unique entries (A) is already sorted, so only a chunk's new
+// entries (B) go through the radix sort and one merge pass replaces five radix passes over the running list.
+// Merge path: a block finds where its tile of MG_TILE outputs starts and ends in A and B (two binary searches in global
+// memory), stages both pieces in shared memory, every thread finds its own start (binary search in shared memory) and
+// merges MG_V outputs; the tile leaves through shared memory, coalesced.
+// ---------------------------------------------------------------------------
+constexpr int MG_T = 256, MG_V = 7, MG_TILE = MG_T * MG_V;
+
+template <typename Ptr>
+__device__ __forceinline__ long long merge_path_split(Ptr A, long long na, Ptr B, long long nb, long long diag)
+{
+    long long lo = diag > nb ? diag - nb : 0, hi = diag < na ? diag : na;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (A[mid] <= B[diag - 1 - mid]) lo = mid + 1; else hi = mid;      // A[mid] precedes B[diag-1-mid] (ties: A first)
+    }
+    return lo;                                                           // elements of A among the first `diag` outputs
+}
+
+__global__ void __launch_bounds__(MG_T)
+merge_sorted_kernel(const unsigned long long* __restrict__ ka, const uint32_t* __restrict__ va, long long na,
+                    const unsigned long long* __restrict__ kb, const uint32_t* __restrict__ vb, long long nb,
+                    unsigned long long* __restrict__ ko, uint32_t* __restrict__ vo)
+{
+    __shared__ unsigned long long s_k[MG_TILE], s_ok[MG_TILE];
+    __shared__ uint32_t s_v[MG_TILE], s_ov[MG_TILE];
+    __shared__ long long s_split[2];
+    const long long n = na + nb;
+    const long long d0 = (long long)blockIdx.x * MG_TILE;
+    const long long d1 = d0 + MG_TILE < n ? d0 + MG_TILE : n;
+    if (threadIdx.x < 2) s_split[threadIdx.x] = merge_path_split(ka, na, kb, nb, threadIdx.x == 0 ? d0 : d1);
+    __syncthreads();
+    const long long a0 = s_split[0], a1 = s_split[1], b0 = d0 - a0, b1 = d1 - a1;
+    const int ca = (int)(a1 - a0), cb = (int)(b1 - b0);
+    for (int i = threadIdx.x; i < ca; i += MG_T) { s_k[i] = ka[a0 + i]; s_v[i] = va[a0 + i]; }
+    for (int i = threadIdx.x; i < cb; i += MG_T) { s_k[ca + i] = kb[b0 + i]; s_v[ca + i] = vb[b0 + i]; }
+    __syncthreads();
+    const unsigned long long* A = s_k;
+    const unsigned long long* B = s_k + ca;
+    const int total = ca + cb;
+    int diag = threadIdx.x * MG_V;
+    if (diag > total) diag = total;
+    int ia = (int)merge_path_split(A, (long long)ca, B, (long long)cb, (long long)diag);
+    int ib = diag - ia;
+#pragma unroll
+    for (int i = 0; i < MG_V; ++i) {
+        const int o = diag + i;
+        if (o < total) {
+            const bool take_a = ib >= cb || (ia < ca && A[ia] <= B[ib]);
+            const int src = take_a ? ia : ca + ib;
+            s_ok[o] = s_k[src]; s_ov[o] = s_v[src];
+            ia += take_a ? 1 : 0; ib += take_a ? 0 : 1;
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < total; i += MG_T) { ko[d0 + i] = s_ok[i]; vo[d0 + i] = s_ov[i]; }
+}
+
 struct CooLayout {
     size_t pairs, pairs2, pair_counts, pair_counts2, counts, keys[2], vals[2], tile_heads, carry_key, carry_sum, mface, scan, sort, total;
     int64_t C, E, cap, n_blocks, n_tiles;
@@ -878,10 +938,18 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
         mcs_note_launch(), expand_entries_kernel<unsigned long long><<<nblk, AT, 0, st>>>(
             a, pp, pc, slots, counts, keys[cur] + n_u, vals[cur] + n_u);
         const long long n_tot = n_u + n_entries;
-        rc = sort_pairs_u64((uint64_t*)keys[cur], vals[cur], n_tot, bits, sort_ws, sort_bytes, st);
+        // the chunk's new entries are sorted on their own; the running list (sorted, unique) joins by one stable merge
+        // pass, running entry first on equal keys: the same sequence a stable sort of the whole would give
+        rc = sort_pairs_u64((uint64_t*)(keys[cur] + n_u), vals[cur] + n_u, n_entries, bits, sort_ws, sort_bytes, st);
         if (rc != MCS_OK) return rc;
+        int src = cur;                                // buffer that holds the sorted sequence
+        if (n_u > 0) {
+            mcs_note_launch(), merge_sorted_kernel<<<(unsigned)ceil_div64(n_tot, MG_TILE), MG_T, 0, st>>>(
+                keys[cur], vals[cur], n_u, keys[cur] + n_u, vals[cur] + n_u, (long long)n_entries, keys[1 - cur], vals[1 - cur]);
+            src = 1 - cur;
+        }
         const long long n_tiles = ceil_div64(n_tot, RT);
-        mcs_note_launch(), count_heads_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(keys[cur], n_tot, tile_heads);
+        mcs_note_launch(), count_heads_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(keys[src], n_tot, tile_heads);
         rc = exclusive_scan_u32(tile_heads, tile_heads, n_tiles, tile_heads + n_tiles, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
         uint32_t n_heads = 0;
@@ -894,10 +962,10 @@ int accumulate_coo_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basis* 
             return MCS_ENOMEM;
         }
         mcs_note_launch(), reduce_runs_compact_kernel<<<(unsigned)n_tiles, RT, 0, st>>>(
-            keys[cur], vals[cur], n_tot, tile_heads, keys[1 - cur], (float*)vals[1 - cur], carry_key, carry_sum);
+            keys[src], vals[src], n_tot, tile_heads, keys[1 - src], (float*)vals[1 - src], carry_key, carry_sum);
         mcs_note_launch(), carry_fixup_compact_kernel<<<(unsigned)ceil_div64(n_tiles, AT), AT, 0, st>>>(
-            carry_key, carry_sum, n_tiles, tile_heads, (float*)vals[1 - cur]);
-        cur = 1 - cur;
+            carry_key, carry_sum, n_tiles, tile_heads, (float*)vals[1 - src]);
+        cur = 1 - src;
         n_u = n_heads;
     }
     if (n_u > 0)
