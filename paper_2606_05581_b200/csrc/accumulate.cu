@@ -30,7 +30,10 @@ namespace {
 
 constexpr int AT = 256;
 constexpr int CH = 256;                               // record slots per level-1 block
-constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << 22;
+#ifndef MCS_DENSE_CHUNK_LOG2
+#define MCS_DENSE_CHUNK_LOG2 22
+#endif
+constexpr int64_t MAX_CHUNK_WALKS = (int64_t)1 << MCS_DENSE_CHUNK_LOG2;
 // Sparse output: the running list of unique entries is re-sorted with every chunk's new entries, so fewer, larger chunks
 // pay (B200: 180 GB; a 16 Mi-walk chunk takes about 17 GB of workspace per operator at BASELINE config 3's sizes).
 #ifndef MCS_COO_CHUNK_LOG2
