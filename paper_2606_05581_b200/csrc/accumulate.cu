@@ -1023,13 +1023,17 @@ struct PointBasisDev {
 
 constexpr int KNN_GRID_MIN = 1024;
 
-// Insert candidate (d2, idx) into the sorted list of the KNN_MAX best: order by d2, then by smaller index [Rk2].
-__device__ __forceinline__ void knn_insert(float (&bd)[KNN_MAX], int (&bi)[KNN_MAX], float d2, int idx)
+// Insert candidate (d2, idx) into the sorted list of the KL best: order by d2, then by smaller index [Rk2].
+// KL = 8 for k <= 8, else KNN_MAX: the list only has to hold the k nearest, and its length is what an insertion costs -- in
+// a warp some lane inserts at almost every candidate, so all 32 pay for it (ncu, config-4 sample, k = 8 with a 16-entry
+// list: 41 000 warp instructions per record warp = 80 per candidate, 200 registers, one block per SM).
+template <int KL>
+__device__ __forceinline__ void knn_insert(float (&bd)[KL], int (&bi)[KL], float d2, int idx)
 {
-    if (d2 < bd[KNN_MAX - 1] || (d2 == bd[KNN_MAX - 1] && idx < bi[KNN_MAX - 1])) {
-        bd[KNN_MAX - 1] = d2; bi[KNN_MAX - 1] = idx;
+    if (d2 < bd[KL - 1] || (d2 == bd[KL - 1] && idx < bi[KL - 1])) {
+        bd[KL - 1] = d2; bi[KL - 1] = idx;
 #pragma unroll
-        for (int m = KNN_MAX - 1; m > 0; --m)
+        for (int m = KL - 1; m > 0; --m)
             if (bd[m] < bd[m - 1] || (bd[m] == bd[m - 1] && bi[m] < bi[m - 1])) {
                 const float td = bd[m]; bd[m] = bd[m - 1]; bd[m - 1] = td;
                 const int ti = bi[m]; bi[m] = bi[m - 1]; bi[m - 1] = ti;
@@ -1039,7 +1043,8 @@ __device__ __forceinline__ void knn_insert(float (&bd)[KNN_MAX], int (&bi)[KNN_M
 
 // Grid search: rings of cells about the query's cell.  After ring r every point within r*h - off of q has been
 // seen (off = distance from q to its clamped cell), so the search stops when the k-th best is closer than that.
-__device__ __forceinline__ void knn_gather_grid(const PointBasisDev& pb, float3 q, float (&bd)[KNN_MAX], int (&bi)[KNN_MAX])
+template <int KL>
+__device__ __forceinline__ void knn_gather_grid(const PointBasisDev& pb, float3 q, float (&bd)[KL], int (&bi)[KL])
 {
     const PointGrid& G = pb.grid;
     const float fx = (q.x - G.lox) * G.inv_h, fy = (q.y - G.loy) * G.inv_h, fz = (q.z - G.loz) * G.inv_h;
@@ -1067,7 +1072,7 @@ __device__ __forceinline__ void knn_gather_grid(const PointBasisDev& pb, float3 
                         const int i = (int)G.sorted_idx[s0 + j];
                         const float dxp = q.x - pb.points[3 * (long long)i], dyp = q.y - pb.points[3 * (long long)i + 1],
                                     dzp = q.z - pb.points[3 * (long long)i + 2];
-                        knn_insert(bd, bi, fmaf(dxp, dxp, fmaf(dyp, dyp, dzp * dzp)), i);
+                        knn_insert<KL>(bd, bi, fmaf(dxp, dxp, fmaf(dyp, dyp, dzp * dzp)), i);
                     }
                 }
             }
@@ -1079,15 +1084,16 @@ __device__ __forceinline__ void knn_gather_grid(const PointBasisDev& pb, float3 
 
 // k-NN of one query per thread: exhaustive (points staged through shared memory; every thread of the block must
 // call this) or through the grid; the k best are kept sorted in registers (static indices only).
+template <int KL>
 __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool active, float3 q, float3 nq,
                                                    float4* s_pts, int* idx_out, float* w_out)
 {
-    float bd[KNN_MAX]; int bi[KNN_MAX];
+    float bd[KL]; int bi[KL];
 #pragma unroll
-    for (int j = 0; j < KNN_MAX; ++j) { bd[j] = CUDART_INF_F; bi[j] = -1; }
+    for (int j = 0; j < KL; ++j) { bd[j] = CUDART_INF_F; bi[j] = -1; }
     const int k = pb.k;
     if (pb.use_grid) {
-        if (active) knn_gather_grid(pb, q, bd, bi);
+        if (active) knn_gather_grid<KL>(pb, q, bd, bi);
     } else {
         for (long long base = 0; base < pb.K; base += KNN_TILE) {
             const int n = (int)((pb.K - base) < KNN_TILE ? (pb.K - base) : KNN_TILE);
@@ -1099,16 +1105,16 @@ __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool
                 for (int j = 0; j < n; ++j) {
                     const float4 p = s_pts[j];
                     const float dx = q.x - p.x, dy = q.y - p.y, dz = q.z - p.z;
-                    knn_insert(bd, bi, fmaf(dx, dx, fmaf(dy, dy, dz * dz)), (int)(base + j));
+                    knn_insert<KL>(bd, bi, fmaf(dx, dx, fmaf(dy, dy, dz * dz)), (int)(base + j));
                 }
             }
         }
     }
     if (!active) return;
-    // only the first k count: the list holds the KNN_MAX nearest in order
-    float lg[KNN_MAX], lmax = -CUDART_INF_F;
+    // only the first k count: the list holds the KL >= k nearest in order
+    float lg[KL], lmax = -CUDART_INF_F;
 #pragma unroll
-    for (int j = 0; j < KNN_MAX; ++j) {
+    for (int j = 0; j < KL; ++j) {
         const bool use = j < k && bi[j] >= 0;
         float c = 0.0f;
         if (use) {
@@ -1120,10 +1126,10 @@ __device__ __forceinline__ void knn_weights_device(const PointBasisDev& pb, bool
     }
     float sum = 0.0f;
 #pragma unroll
-    for (int j = 0; j < KNN_MAX; ++j) { lg[j] = (j < k && bi[j] >= 0) ? expf(lg[j] - lmax) : 0.0f; sum += lg[j]; }
+    for (int j = 0; j < KL; ++j) { lg[j] = (j < k && bi[j] >= 0) ? expf(lg[j] - lmax) : 0.0f; sum += lg[j]; }
     const float inv = 1.0f / sum;
 #pragma unroll
-    for (int j = 0; j < KNN_MAX; ++j)
+    for (int j = 0; j < KL; ++j)
         if (j < k) { idx_out[j] = bi[j]; w_out[j] = lg[j] * inv; }
 }
 
@@ -1166,6 +1172,7 @@ points_ranges_kernel(const uint32_t* __restrict__ keys, long long K, uint32_t* _
     }
 }
 
+template <int KL>
 __global__ void __launch_bounds__(AT)
 knn_queries_kernel(PointBasisDev pb, const float* __restrict__ q, const float* __restrict__ nq, long long Q,
                    int32_t* __restrict__ idx, float* __restrict__ w)
@@ -1175,8 +1182,8 @@ knn_queries_kernel(PointBasisDev pb, const float* __restrict__ q, const float* _
     const bool active = i < Q;
     float3 qq = make_float3(0.f, 0.f, 0.f), nn = make_float3(0.f, 0.f, 1.f);
     if (active) { qq = make_float3(q[3 * i], q[3 * i + 1], q[3 * i + 2]); nn = make_float3(nq[3 * i], nq[3 * i + 1], nq[3 * i + 2]); }
-    int io[KNN_MAX]; float wo[KNN_MAX];
-    knn_weights_device(pb, active, qq, nn, s_pts, io, wo);
+    int io[KL]; float wo[KL];
+    knn_weights_device<KL>(pb, active, qq, nn, s_pts, io, wo);
     if (active)
         for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
 }
@@ -1196,6 +1203,7 @@ __device__ __forceinline__ void face_point_normal(const float* __restrict__ vert
 }
 
 // b(s) of every sample
+template <int KL>
 __global__ void __launch_bounds__(AT)
 knn_samples_kernel(PointBasisDev pb, const float* __restrict__ verts, const int32_t* __restrict__ faces,
                    const int32_t* __restrict__ s_tri, const float* __restrict__ s_bary, const float* __restrict__ s_normal,
@@ -1209,13 +1217,14 @@ knn_samples_kernel(PointBasisDev pb, const float* __restrict__ verts, const int3
         face_point_normal(verts, faces, s_tri[i], s_bary[3 * i], s_bary[3 * i + 1], s_bary[3 * i + 2], p, n);
         if (s_normal) n = make_float3(s_normal[3 * i], s_normal[3 * i + 1], s_normal[3 * i + 2]);
     }
-    int io[KNN_MAX]; float wo[KNN_MAX];
-    knn_weights_device(pb, active, p, n, s_pts, io, wo);
+    int io[KL]; float wo[KL];
+    knn_weights_device<KL>(pb, active, p, n, s_pts, io, wo);
     if (active)
         for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
 }
 
 // b(t) of the records [j0, j0 + n): idx = -1 everywhere for a record without contribution
+template <int KL>
 __global__ void __launch_bounds__(AT)
 knn_records_kernel(PointBasisDev pb, const float* __restrict__ verts, const int32_t* __restrict__ faces,
                    const float4* __restrict__ records, long long j0, long long n,
@@ -1231,8 +1240,8 @@ knn_records_kernel(PointBasisDev pb, const float* __restrict__ verts, const int3
         if (tri_t >= 0 && rec.w != 0.0f) face_point_normal(verts, faces, tri_t, 1.0f - rec.y - rec.z, rec.y, rec.z, p, nrm);
         else { active = false; for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = -1; w[i * pb.k + j] = 0.0f; } }
     }
-    int io[KNN_MAX]; float wo[KNN_MAX];
-    knn_weights_device(pb, active, p, nrm, s_pts, io, wo);
+    int io[KL]; float wo[KL];
+    knn_weights_device<KL>(pb, active, p, nrm, s_pts, io, wo);
     if (active)
         for (int j = 0; j < pb.k; ++j) { idx[i * pb.k + j] = io[j]; w[i * pb.k + j] = wo[j]; }
 }
@@ -1424,7 +1433,8 @@ int knn_weights_run(const mcs_basis* basis, const float* q, const float* nq, int
         if (rc != MCS_OK) { cudaFree(scratch); return rc; }
         pb.use_grid = 1;
     }
-    mcs_note_launch(), knn_queries_kernel<<<(unsigned)ceil_div64(Q, AT), AT, 0, st>>>(pb, q, nq, Q, idx, w);
+    if (pb.k <= 8) mcs_note_launch(), knn_queries_kernel<8><<<(unsigned)ceil_div64(Q, AT), AT, 0, st>>>(pb, q, nq, Q, idx, w);
+    else mcs_note_launch(), knn_queries_kernel<KNN_MAX><<<(unsigned)ceil_div64(Q, AT), AT, 0, st>>>(pb, q, nq, Q, idx, w);
     cudaError_t e = cudaGetLastError();
     if (scratch) { cudaStreamSynchronize(st); cudaFree(scratch); }
     if (e != cudaSuccess) { mcs_set_last_cuda_error((int)e); return MCS_ECUDA; }
@@ -1466,13 +1476,16 @@ int accumulate_points_run(const mcs_bvh* b, const mcs_samples* s, const mcs_basi
     const int bits = key_bits_for(K);
 
     MCS_CUDA_TRY(cudaMemsetAsync(out->dense, 0, (size_t)K * K * sizeof(float), st));
-    mcs_note_launch(), knn_samples_kernel<<<(unsigned)ceil_div64(s->n_s, AT), AT, 0, st>>>(
+    if (k <= 8) mcs_note_launch(), knn_samples_kernel<8><<<(unsigned)ceil_div64(s->n_s, AT), AT, 0, st>>>(
+        pb, b->verts, b->faces, s->tri, s->bary, s->normal, s->n_s, is, wsm);
+    else mcs_note_launch(), knn_samples_kernel<KNN_MAX><<<(unsigned)ceil_div64(s->n_s, AT), AT, 0, st>>>(
         pb, b->verts, b->faces, s->tri, s->bary, s->normal, s->n_s, is, wsm);
     unsigned long long entries_total = 0;
     for (int64_t j0 = 0; j0 < n_records; j0 += L.C) {
         const long long n = (n_records - j0) < L.C ? (n_records - j0) : L.C;
         const unsigned nblk = (unsigned)ceil_div64(n, AT);
-        mcs_note_launch(), knn_records_kernel<<<nblk, AT, 0, st>>>(pb, b->verts, b->faces, records, j0, n, it, wt);
+        if (k <= 8) mcs_note_launch(), knn_records_kernel<8><<<nblk, AT, 0, st>>>(pb, b->verts, b->faces, records, j0, n, it, wt);
+        else mcs_note_launch(), knn_records_kernel<KNN_MAX><<<nblk, AT, 0, st>>>(pb, b->verts, b->faces, records, j0, n, it, wt);
         mcs_note_launch(), count_entries_points_kernel<<<nblk, AT, 0, st>>>(k, j0, n, n_main, W, is, wsm, it, wt, counts);
         rc = exclusive_scan_u32(counts, counts, n, counts + n, scan_ws, scan_bytes, st);
         if (rc != MCS_OK) return rc;
