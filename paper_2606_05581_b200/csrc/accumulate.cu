@@ -1224,8 +1224,11 @@ knn_samples_kernel(PointBasisDev pb, const float* __restrict__ verts, const int3
 }
 
 // b(t) of the records [j0, j0 + n): idx = -1 everywhere for a record without contribution
+// Blocks per SM: the kernel compiles to ~195 registers unbounded (one block of 256 threads per SM, 12 % of the warp slots); held
+// to 85 registers (three blocks) with the 8-entry list the config-4 sample goes 78.7 -> 83.8 meshes/s (two blocks: 83.1; four
+// blocks spill: 73.9).
 template <int KL>
-__global__ void __launch_bounds__(AT)
+__global__ void __launch_bounds__(AT, KL <= 8 ? 3 : 2)
 knn_records_kernel(PointBasisDev pb, const float* __restrict__ verts, const int32_t* __restrict__ faces,
                    const float4* __restrict__ records, long long j0, long long n,
                    int32_t* __restrict__ idx, float* __restrict__ w)
