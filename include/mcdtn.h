@@ -172,7 +172,8 @@ typedef struct {
                                     radius between D / (1 + far_alpha) and D.  WoS only needs a ball inside the domain
                                     (PAPER.md:155), so the estimator is unchanged in expectation; single walks differ from
                                     the exact run.  The shell test and the exit point always come from an exact query.
-                                    Deterministic (independent of the schedule).  Typical: 0.5                          */
+                                    Deterministic (independent of the schedule).  Measured best on a 2 M-face in-the-
+                                    wild mesh: 1 (interior), 2 (exterior) with far_near_factor 2; at most 4             */
     float    far_near_factor;    /* far_alpha > 0: boxes closer than this many eps are always descended (0: 16; >= 2)  */
     int32_t  exterior_query;     /* exterior only.  0 (default): flat-triangle query at x = kappa(y) on the primal tree with
                                     the conservative radius D / (rho min(R_max, rho + D)) (E3).  1: the paper's own
