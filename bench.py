@@ -732,6 +732,24 @@ def run_ours(args):
     return 0
 
 
+def run_only(args):
+    """One sub-record alone on cuda:0 (so that an ncu launch list shows that workload and nothing else)."""
+    import torch
+    from paper_2606_05581_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    api.lib()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    if args.only == "cfg4":
+        rec = bench_cfg4_sample(api, torch, dev, args, args.seed, args.cfg4_meshes, flush)
+    else:
+        rec = bench_cfg1(api, torch, dev, args, args.seed, min(args.steps, 5), 3, flush, api.measure_fp32_tflops(dev), api.measure_l2_gbs(dev))
+    print(json.dumps({"only": args.only, **rec}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -761,7 +779,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sub", action="store_true", help="skip the configs[1] / configs[4] sub-records")
     ap.add_argument("--no-cache", action="store_true", help="regenerate the workload instead of reading the temp-dir cache")
+    ap.add_argument("--only", choices=["cfg1", "cfg4"], default=None,
+                    help="run ONE sub-record alone and print its JSON (profiling aid: profiles/r02_cfg4_launches.md); not the bench line")
     args = ap.parse_args()
+    if args.only:
+        return run_only(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
